@@ -1,0 +1,402 @@
+"""Pins of the fp64 CPU oracle against what the paper and the mathematics fix (no GPU).
+
+Each test names the passage of arXiv 2212.09807 (P:L### = /root/reference/PAPER.md line) or the
+SURVEY.md 8(c.4) row it checks.  None of them retypes the oracle's own formula: they use printed
+values (tests/golden/), invariants, closed forms of special cases, brute force and a per-electron
+Monte Carlo written independently in numpy.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2212_09807_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _rows(name):
+    out = []
+    for line in open(os.path.join(GOLD, name)):
+        line = line.split("#")[0].strip()
+        if line:
+            out.append(line.split())
+    return out
+
+
+def _one_segment(xs, ys, zs, xe, ye, ze, dE, ts=0.0, te=0.0):
+    f = lambda v: np.atleast_1d(np.asarray(v, dtype=np.float32))
+    return dict(xs=f(xs), ys=f(ys), zs=f(zs), ts=f(ts), xe=f(xe), ye=f(ye), ze=f(ze), te=f(te), dE=f(dE))
+
+
+def _small_setup(nx=12, ny=12, drift=12.0, n_ticks=None, **over):
+    p = W.default_params(**over)
+    tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, drift, nx, ny, 0)]
+    p["n_readout_ticks"] = n_ticks if n_ticks is not None else W._n_ticks(p, drift, 0.0)
+    return p, tpcs, W.pad_response_lut(p)
+
+
+def _chain(p, tpcs, seg):
+    dedx, ne = oracle.quench(p, seg)
+    dr = oracle.drift(p, tpcs, seg, ne)
+    pm = oracle.pixmap(p, tpcs, seg, dr)
+    return dedx, ne, dr, pm
+
+
+# ------------------------------------------------------------------ O1 recombination
+
+def test_recombination_golden_values():
+    """SURVEY 8(c.4) O1 table; the paper prints 'around 0.7' for a MIP with both models."""
+    for row in _rows("recombination.txt"):
+        q, box212, box207, birks = map(float, row)
+        seg = _one_segment(0, 0, 5, 0.1, 0, 5, q * 0.1)
+        # float32 rounding of 0.1 and dE: use the actual length and energy the oracle sees
+        L = float(seg["xe"][0]) - float(seg["xs"][0])
+        Q0 = float(seg["dE"][0]) / 23.6e-6
+        for model, beta, want in ((1, 0.212, box212), (1, 0.207, box207), (0, 0.212, birks)):
+            p = W.default_params(recomb_model=model, box_beta=beta)
+            dedx, ne = oracle.quench(p, seg)
+            assert dedx[0] == pytest.approx(float(seg["dE"][0]) / L, rel=1e-12)
+            assert ne[0] / Q0 == pytest.approx(want, abs=2e-6)
+    # 1 mm MIP segment: Q_0 = 8898.31 e-, 6266.62 (Box .212) / 6201.38 (Birks)
+    seg = _one_segment(0, 0, 5, 0.1, 0, 5, 0.21)
+    assert oracle.quench(W.default_params(recomb_model=1), seg)[1][0] == pytest.approx(6266.62, rel=2e-6)
+    assert oracle.quench(W.default_params(recomb_model=0), seg)[1][0] == pytest.approx(6201.38, rel=2e-6)
+    for model in (0, 1):                                    # "around 0.7"
+        ne = oracle.quench(W.default_params(recomb_model=model, box_beta=0.207), seg)[1][0]
+        assert abs(ne / (0.21 / 23.6e-6) - 0.7) < 0.01
+
+
+def test_recombination_invariants():
+    """Birks: 1/R is linear in dE/dx with slope k_b/(A_b eps) and R(0+) = A_b (eq. 3.1).
+    Box: R*xi = ln(alpha + xi) so exp(R*xi) - xi = alpha for every dE/dx (eq. 3.2); clamp below ~0.228 (D6)."""
+    q = np.array([0.5, 1.0, 2.0, 4.0, 8.0, 16.0, 40.0])
+    seg = _one_segment(np.zeros(7), np.zeros(7), np.full(7, 5.0), np.full(7, 0.25), np.zeros(7), np.full(7, 5.0),
+                       q * 0.25)
+    Q0 = seg["dE"].astype(np.float64) / 23.6e-6
+    qd = seg["dE"].astype(np.float64) / 0.25
+    eps = 0.5 * 1.38
+    R = oracle.quench(W.default_params(recomb_model=0), seg)[1] / Q0
+    slope = np.diff(1.0 / R) / np.diff(qd)
+    assert np.allclose(slope, 0.0486 / (0.800 * eps), rtol=1e-9)
+    assert np.allclose(1.0 / R - slope[0] * qd, 1.0 / 0.800, rtol=1e-9)
+    R = oracle.quench(W.default_params(recomb_model=1, box_beta=0.212), seg)[1] / Q0
+    xi = 0.212 * qd / eps
+    assert np.allclose(np.exp(R * xi) - xi, 0.93, rtol=1e-9)
+    assert np.all(np.diff(R[qd >= 2.0]) < 0)                  # falls with dE/dx above a MIP; 'inadequate' below
+    low = _one_segment(0, 0, 5, 1.0, 0, 5, 0.2)             # dE/dx = 0.2 < 0.228 -> negative log -> clamp
+    assert oracle.quench(W.default_params(recomb_model=1), low)[1][0] == 0.0
+    zero = _one_segment(1, 1, 5, 1, 1, 5, 0.2)              # zero length
+    assert oracle.quench(W.default_params(), zero)[1][0] == 0.0
+
+
+# ------------------------------------------------------------------ O2 transport
+
+def test_transport_golden_values():
+    """exp(-t/tau) and sigma = sqrt(2 D t) (eqs. 3.3-3.5)."""
+    p, tpcs, _ = _small_setup(drift=60.0)
+    for row in _rows("transport.txt"):
+        d, att, sT_mm, sL_mm, st_ticks = map(float, row)
+        seg = _one_segment(2.0, 2.0, d, 2.0, 2.1, d, 0.21)
+        ne = np.array([1000.0])
+        dr = oracle.drift(p, tpcs, seg, ne)
+        assert dr["tpc"][0] == 0
+        assert dr["q_a"][0] / 1000.0 == pytest.approx(att, abs=1e-6)
+        assert dr["sigma_T"][0] * 10 == pytest.approx(sT_mm, abs=1e-5)
+        assert dr["sigma_t"][0] * p["v_drift_cm_us"] * 10 == pytest.approx(sL_mm, abs=1e-5)
+        assert dr["sigma_t"][0] / p["tick_us"] == pytest.approx(st_ticks, abs=1e-4)
+        assert dr["T_s"][0] == pytest.approx(d / 0.16, rel=1e-7)
+    # sigma^2 is linear in drift time, ratio D_T/D_L = 2.2 (eq. 3.5)
+    assert (dr["sigma_T"][0] / (dr["sigma_t"][0] * 0.16)) ** 2 == pytest.approx(8.8 / 4.0, rel=1e-12)
+
+
+def test_drift_two_sided_module_and_inactive():
+    """Two TPCs back to back: the sign of eq. (3.3) flips; midpoint outside every TPC -> inactive (D8)."""
+    p = W.default_params()
+    tpcs = [W.make_tpc(0, 0, -30.0, +1, 30.0, 10, 10, 0), W.make_tpc(0, 0, +30.0, -1, 30.0, 10, 10, 100)]
+    seg = _one_segment([1, 1, 1, 50], [1, 1, 1, 1], [-20.0, 20.0, -31.0, 0.0], [1.1, 1.1, 1.1, 50.1], [1, 1, 1, 1],
+                       [-20.0, 20.0, -31.0, 0.0], [0.2] * 4, ts=[3.0] * 4, te=[3.0] * 4)
+    dr = oracle.drift(p, tpcs, seg, np.full(4, 100.0))
+    assert dr["tpc"].tolist() == [0, 1, -1, -1]
+    assert dr["T_s"][0] == pytest.approx(3.0 + 10.0 / 0.16)
+    assert dr["T_s"][1] == pytest.approx(3.0 + 10.0 / 0.16)
+    assert dr["q_a"][2] == 0.0 and dr["q_a"][3] == 0.0
+    assert dr["q_a"][0] == pytest.approx(100.0 * math.exp(-(10.0 / 0.16) / 2200.0), rel=1e-12)
+
+
+# ------------------------------------------------------------------ O3 pixel mapping
+
+def test_pixmap_hand_cases():
+    """segment inside one pixel, sigma = 0, W = 5 -> exactly 5x5; clipping at the plane edge."""
+    p, tpcs, _ = _small_setup(nx=12, ny=12)
+    pitch = p["pixel_pitch_cm"]
+    seg = _one_segment((5 + 0.33) * pitch, (6 + 0.44) * pitch, 0.0, (5 + 0.68) * pitch, (6 + 0.55) * pitch, 0.0, 0.1)
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    assert (pm["ix0"][0], pm["ix1"][0], pm["iy0"][0], pm["iy1"][0]) == (3, 7, 4, 8)
+    assert pm["npix"][0] == 25 and pm["a_lo"][0] == 53 and pm["a_hi"][0] == 56
+    assert pm["jt0"][0] == 0 and pm["jt1"][0] == 0
+    seg = _one_segment(0.2 * pitch, 0.5 * pitch, 0.0, 0.4 * pitch, 0.5 * pitch, 0.0, 0.1)   # corner pixel
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    assert (pm["ix0"][0], pm["ix1"][0], pm["iy0"][0], pm["iy1"][0]) == (0, 2, 0, 2) and pm["npix"][0] == 9
+    # sample count N = max(1, ceil(L / 10 um))
+    seg = _one_segment(1.0, 1.0, 1.0, 1.0 + 0.0255, 1.0, 1.0, 0.1)
+    assert _chain(p, tpcs, seg)[3]["n_samples"][0] == 26
+    seg = _one_segment(1.0, 1.0, 1.0, 1.0 + 1e-5, 1.0, 1.0, 0.1)
+    assert _chain(p, tpcs, seg)[3]["n_samples"][0] == 1
+
+
+def test_pixmap_complete_and_minimal():
+    """Every pixel that receives more than 1e-5 of a segment's charge lies in its rectangle (completeness,
+    the 5-sigma tail bound of SURVEY 8(c.1) O3), and for an axis-aligned segment the charged range is the
+    exact set of pixels within reach (minimality)."""
+    p, tpcs, lut = _small_setup(nx=14, ny=14, drift=12.0)
+    rng = np.random.Generator(np.random.PCG64(5))
+    pitch = p["pixel_pitch_cm"]
+    for trial in range(3):
+        c = np.array([rng.uniform(5, 9) * pitch, rng.uniform(5, 9) * pitch, rng.uniform(0.5, 11.0)])
+        d = W._iso_dir(rng)
+        seg = _one_segment(*(c - 0.05 * d), *(c + 0.05 * d), 0.21)
+        _, _, dr, pm = _chain(p, tpcs, seg)
+        ix, iy = np.meshgrid(np.arange(14), np.arange(14))
+        waves, qp = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, ix.ravel(), iy.ravel())
+        amp = np.abs(waves).sum(axis=1).reshape(14, 14)
+        inside = np.zeros((14, 14), bool)
+        inside[pm["iy0"][0]:pm["iy1"][0] + 1, pm["ix0"][0]:pm["ix1"][0] + 1] = True
+        assert amp[~inside].max() < 1e-5 * dr["q_a"][0]
+        assert amp[inside].min() > 0.0
+    # axis-aligned along x, sigma_T known: charged pixels = those within 5 sigma of [u_s, u_e]
+    seg = _one_segment(6.25 * pitch, 7.5 * pitch, 8.0, 6.75 * pitch, 7.5 * pitch, 8.0, 0.21)
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    r = 5.0 * dr["sigma_T"][0]
+    lo = math.floor((float(seg["xs"][0]) - r) / pitch)
+    hi = math.floor((float(seg["xe"][0]) + r) / pitch)
+    assert pm["ix0"][0] == lo - 2 and pm["ix1"][0] == hi + 2
+
+
+# ------------------------------------------------------------------ O4 induced current
+
+def test_point_charge_reproduces_lut():
+    """zero diffusion, L -> 0 (N = 1), above a bin centre: the waveform on every pixel of
+    the window is Q_a times the LUT series of the bin it is seen through, shifted to the arrival tick."""
+    p, tpcs, lut = _small_setup(nx=9, ny=9, drift=5.0, n_ticks=260)
+    pitch, nb = p["pixel_pitch_cm"], p["bins_per_pixel"]
+    binw = pitch / nb
+    ca, cb = 3, 7                                          # in-pixel bin of the charge, pixel (4, 4)
+    x = 4 * pitch + (ca + 0.5) * binw
+    y = 4 * pitch + (cb + 0.5) * binw
+    seg = _one_segment(x, y, 0.0, x + 2e-6, y, 0.0, 0.21, ts=1.23, te=1.23)   # at the anode: sigma = 0
+    _, ne, dr, pm = _chain(p, tpcs, seg)
+    assert dr["sigma_T"][0] == 0.0 and pm["n_samples"][0] == 1
+    j = int(math.floor(1.23 / 0.1))
+    K = p["lut_ticks"]
+    for (ix, iy) in [(4, 4), (3, 4), (4, 6), (2, 2), (6, 5)]:
+        waves, qp = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, [ix], [iy])
+        cx = ca + nb * (4 - ix + 2)
+        cy = cb + nb * (4 - iy + 2)
+        want = np.zeros(p["n_readout_ticks"])
+        want[j:j + K] = dr["q_a"][0] * lut[cy, cx].astype(np.float64)
+        assert np.allclose(waves[0], want, rtol=1e-13, atol=1e-12)
+    waves, qp = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, [4, 3], [4, 4])
+    assert qp[0] == pytest.approx(dr["q_a"][0], rel=1e-6)   # LUT normalised to one electron
+    assert abs(qp[1]) < 1e-5 * dr["q_a"][0]                  # neighbours: bipolar, integrates to zero
+
+
+def test_charge_conservation_and_linearity():
+    """sum over pixels and ticks of I equals sum of Q_a for tracks >= 2 pixels from the
+    edge (harness LUT columns sum to 1/0); the result is linear in the segments and invariant under
+    translation by whole pixels and whole ticks."""
+    p, tpcs, lut = _small_setup(nx=14, ny=14, drift=12.0, n_ticks=1100)
+    rng = np.random.Generator(np.random.PCG64(11))
+    pitch = p["pixel_pitch_cm"]
+    c = np.array([6.3 * pitch, 7.1 * pitch, 6.0])
+    d = np.array([0.6, 0.3, 0.74])
+    d /= np.linalg.norm(d)
+    seg = W.line_segments(c - 0.15 * d, c + 0.15 * d, 0.1, 2.0, lambda s, L, n: np.array([2.1, 6.0, 3.0]))
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    ix, iy = oracle.active_pixels(tpcs, pm, dr, 0)
+    waves, qp = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, ix, iy)
+    assert qp.sum() == pytest.approx(dr["q_a"].sum(), rel=2e-6)
+    # linearity: sum of single-segment results
+    acc = np.zeros_like(waves)
+    for s in range(3):
+        one = {k: v[s:s + 1] for k, v in seg.items()}
+        _, _, dr1, pm1 = _chain(p, tpcs, one)
+        acc += oracle.pixel_currents(p, tpcs, lut, dr1, pm1, 0, ix, iy)[0]
+    assert np.allclose(acc, waves, rtol=1e-12, atol=1e-9)
+    # translation by (+2, -1) pixels and +7 ticks
+    seg2 = {k: v.copy() for k, v in seg.items()}
+    # shift in float64 then round: the shifted float32 coordinates differ from the exact shift by < 1e-6 cm
+    for k in ("xs", "xe"):
+        seg2[k] = (seg[k].astype(np.float64) + 2 * pitch).astype(np.float32)
+    for k in ("ys", "ye"):
+        seg2[k] = (seg[k].astype(np.float64) - 1 * pitch).astype(np.float32)
+    for k in ("ts", "te"):
+        seg2[k] = (seg[k].astype(np.float64) + 0.7).astype(np.float32)
+    _, _, dr2, pm2 = _chain(p, tpcs, seg2)
+    waves2, _ = oracle.pixel_currents(p, tpcs, lut, dr2, pm2, 0, ix + 2, iy - 1)
+    scale = np.abs(waves).max()
+    assert np.abs(waves2[:, 7:] - waves[:, :-7]).max() < 2e-4 * scale   # float32 rounding of the shifted inputs
+
+
+def test_long_track_closed_form():
+    """a long straight track parallel to the plane, centred on a pixel row, deposits
+    Q_p = lambda * pitch * erf(pitch / (2 sqrt(2) sigma_T)) on each pixel of that row."""
+    p, tpcs, lut = _small_setup(nx=16, ny=9, drift=12.0, n_ticks=1000)
+    pitch = p["pixel_pitch_cm"]
+    y = 4.5 * pitch
+    seg = W.line_segments([1.0 * pitch, y, 10.0], [15.0 * pitch, y, 10.0], 0.1, 0.0, lambda s, L, n: np.full(n, 2.1))
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    lam = dr["q_a"].sum() / (14.0 * pitch)
+    sT = dr["sigma_T"][0]
+    waves, qp = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, [7, 8, 7], [4, 4, 5])
+    want_row = lam * pitch * math.erf(pitch / (2.0 * math.sqrt(2.0) * sT))
+    assert qp[0] == pytest.approx(want_row, rel=2e-5)
+    assert qp[1] == pytest.approx(want_row, rel=2e-5)
+    want_next = lam * pitch * 0.5 * (math.erf(1.5 * pitch / (math.sqrt(2.0) * sT)) - math.erf(0.5 * pitch / (math.sqrt(2.0) * sT)))
+    assert qp[2] == pytest.approx(want_next, rel=2e-4, abs=0.05)
+    # whole chain: MIP at 10 cm -> 6.091e4 e-/cm
+    assert lam == pytest.approx(2.1 / 23.6e-6 * 0.704248 * 0.971991, rel=1e-4)
+
+
+def test_direct_sum_equals_lattice_form():
+    """The literal six-fold sum of SURVEY 8(c.1) equals the two-step (rho on the lattice, then eq. 3.7) form."""
+    p, tpcs, lut = _small_setup(nx=7, ny=7, drift=3.0, n_ticks=150, lut_ticks=40, window_pixels=3,
+                                sample_step_cm=0.01)
+    pitch = p["pixel_pitch_cm"]
+    seg = _one_segment([3.2 * pitch, 3.6 * pitch], [3.4 * pitch, 2.9 * pitch], [1.0, 0.0],
+                       [3.35 * pitch, 3.7 * pitch], [3.5 * pitch, 2.95 * pitch], [1.05, 0.0], [0.1, 0.05])
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    for (ix, iy) in [(3, 3), (2, 3), (4, 2)]:
+        a = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, [ix], [iy])[0][0]
+        b = oracle.direct_current(p, lut, dr, pm, 0, ix, iy)
+        assert np.abs(a).max() > 0
+        assert np.allclose(a, b, rtol=1e-11, atol=1e-12 * np.abs(a).max())
+
+
+def test_per_electron_monte_carlo():
+    """SURVEY 8(c.4) O4(iv) / BASELINE north_star: brute-force per-electron Monte Carlo of eqs. (3.8)-(3.9):
+    every electron is placed at one of the N points, displaced by N(0, sigma_T) in x and y and N(0, sigma_L)
+    along the drift, looked up in the nearest LUT bin at its arrival tick.  The mean agrees with the oracle's
+    expectation form within 5 standard errors per (pixel, tick)."""
+    p, tpcs, lut = _small_setup(nx=9, ny=9, drift=12.0, n_ticks=620)
+    pitch, nb, K, dt = p["pixel_pitch_cm"], p["bins_per_pixel"], p["lut_ticks"], p["tick_us"]
+    binw = pitch / nb
+    c = np.array([4.4 * pitch, 4.7 * pitch, 4.0])
+    d = np.array([0.5, -0.4, 0.77])
+    d /= np.linalg.norm(d)
+    seg = W.line_segments(c - 0.1 * d, c + 0.1 * d, 0.1, 0.5, lambda s, L, n: np.array([2.1, 4.0]))
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    pix = [(4, 4), (5, 4), (4, 5), (3, 3)]
+    waves, qp = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, [a for a, _ in pix], [b for _, b in pix])
+    rng = np.random.Generator(np.random.PCG64(99))
+    nbatch, per = 16, 60000
+    nt = p["n_readout_ticks"]
+    est = np.zeros((nbatch, len(pix), nt))
+    lut64 = lut.astype(np.float64)
+    for bi in range(nbatch):
+        for s in range(2):
+            N = int(pm["n_samples"][s])
+            mu = rng.integers(0, N, size=per)
+            f = (mu + 0.5) / N
+            x = dr["u_s"][s] + (dr["u_e"][s] - dr["u_s"][s]) * f + rng.normal(0, dr["sigma_T"][s], per)
+            y = dr["v_s"][s] + (dr["v_e"][s] - dr["v_s"][s]) * f + rng.normal(0, dr["sigma_T"][s], per)
+            T = dr["T_s"][s] + (dr["T_e"][s] - dr["T_s"][s]) * f + rng.normal(0, dr["sigma_t"][s], per)
+            a = np.floor(x / binw).astype(int)
+            b = np.floor(y / binw).astype(int)
+            j = np.floor((T - p["t_origin_us"]) / dt).astype(int)
+            w = dr["q_a"][s] / per
+            for k, (ix, iy) in enumerate(pix):
+                cx, cy = a - nb * (ix - 2), b - nb * (iy - 2)
+                ok = (cx >= 0) & (cx < 5 * nb) & (cy >= 0) & (cy < 5 * nb) & (j >= 0) & (j <= nt - K)
+                cell = (cy[ok] * 5 * nb + cx[ok]) * (nt - K + 1) + j[ok]
+                G = np.bincount(cell, minlength=(5 * nb) ** 2 * (nt - K + 1)).reshape((5 * nb) ** 2, nt - K + 1)
+                rows = np.nonzero(G.any(axis=1))[0]
+                for r in rows:
+                    cols = np.nonzero(G[r])[0]
+                    for jj in cols:
+                        est[bi, k, jj:jj + K] += w * G[r, jj] * lut64.reshape(-1, K)[r]
+    mean = est.mean(axis=0)
+    se = est.std(axis=0, ddof=1) / math.sqrt(nbatch)
+    big = np.abs(waves) > 1e-3 * np.abs(waves).max()
+    zscore = np.abs(mean - waves)[big] / np.maximum(se[big], 1e-9)
+    assert big.sum() > 200
+    assert np.quantile(zscore, 0.99) < 4.0 and zscore.max() < 6.0
+    # integrated charge per pixel agrees to MC precision as well
+    q_mc = est.sum(axis=2)
+    q_se = q_mc.std(axis=0, ddof=1) / math.sqrt(nbatch)
+    # (tails holding < 1e-6 of the charge are invisible to 1e6 electrons)
+    assert np.all(np.abs(q_mc.mean(axis=0) - qp) < 5 * q_se + 1e-6 * dr["q_a"].sum())
+
+
+# ------------------------------------------------------------------ O6 electronics + Philox
+
+def test_philox_known_answers():
+    """Philox4x32-10 known-answer vectors (tests/golden/philox4x32_10.txt)."""
+    for row in _rows("philox4x32_10.txt"):
+        h = [int(x, 16) for x in row]
+        assert oracle.philox4x32_10(h[:4], h[4:6]) == h[6:]
+
+
+def test_noise_normal_moments():
+    """Box-Muller normals keyed by (seed, pixel, tick): mean 0, variance 1, fourth moment 3, uncorrelated."""
+    z = np.array([oracle.noise_normals(1234, pix, t) for pix in range(40) for t in range(500)])
+    n = z.shape[0]
+    for k in range(3):
+        assert abs(z[:, k].mean()) < 4 / math.sqrt(n)
+        assert abs(z[:, k].var() - 1) < 4 * math.sqrt(2 / n)
+        assert abs((z[:, k] ** 4).mean() - 3) < 4 * math.sqrt(96 / n)
+    assert abs(np.corrcoef(z.T)[0, 1]) < 4 / math.sqrt(n) and abs(np.corrcoef(z.T)[0, 2]) < 4 / math.sqrt(n)
+    assert oracle.noise_normals(1234, 7, 9) != oracle.noise_normals(1235, 7, 9)
+
+
+def test_electronics_hand_cases():
+    """constant current c e-/tick without noise crosses 7000 e- at tick ceil(7000/c) - 1, is
+    sampled 16 ticks (1.6 us) later with adc = floor((580 + 4 q/1000 - 288) / 3.953125); a pixel that
+    never reaches the threshold gives no hit; 28 mV <=> 7000 e- at 4 mV/ke- (P:L708)."""
+    p = W.default_params(n_readout_ticks=400)
+    lsb = (1300.0 - 288.0) / 256
+    assert lsb == 3.953125
+    for c in (250.0, 999.0, 3500.0, 7000.0):
+        wave = np.full((1, 400), c)
+        hp, ht, ha, cnt = oracle.electronics(p, 0, [17], wave)
+        n_c = math.ceil(7000.0 / c) - 1
+        assert ht[0] == n_c + 16
+        q_s = c * (n_c + 17)
+        assert ha[0] == min(255, math.floor((580 + 4 * q_s / 1000 - 288) / lsb))
+        # after the reset the same pattern repeats with period (n_c + 17) ticks
+        assert np.all(np.diff(ht) == n_c + 17)
+        assert cnt[0] == len(ht) == (400 // (n_c + 17))
+    sub = np.zeros((1, 400))
+    sub[0, 10:60] = 139.0                                    # 6950 e- in total: below threshold
+    assert oracle.electronics(p, 0, [3], sub)[3][0] == 0
+    edge = np.zeros((1, 400))
+    edge[0, 100] = 7000.0                                    # exactly the threshold: q >= threshold fires (D13)
+    hp, ht, ha, cnt = oracle.electronics(p, 0, [3], edge)
+    assert ht.tolist() == [116] and ha[0] == math.floor((580 + 28.0 - 288) / lsb)
+    late = np.zeros((1, 400))
+    late[0, 390] = 9000.0                                    # sample tick 406 is past the window: nothing (O6 step 4)
+    assert oracle.electronics(p, 0, [3], late)[3][0] == 0
+    # whole chain estimate of SURVEY 8(c.4): 2.70e4 e- collected in one hit -> ADC about 101
+    one = np.zeros((1, 400))
+    one[0, 50:60] = 2700.0
+    assert abs(int(oracle.electronics(p, 0, [3], one)[2][0]) - 101) <= 1
+
+
+def test_electronics_noise_is_keyed_and_reproducible():
+    """Noise terms: reset / discriminator / uncorrelated; draws depend only on (seed, pixel, tick)."""
+    p = W.default_params(n_readout_ticks=300, noise_reset_e=900.0, noise_uncorr_e=500.0, noise_disc_e=650.0)
+    wave = np.zeros((2, 300))
+    wave[:, 20:80] = 400.0
+    a = oracle.electronics(p, 42, [5, 6], wave)
+    b = oracle.electronics(p, 42, [5, 6], wave)
+    c = oracle.electronics(p, 43, [5, 6], wave)
+    assert all(np.array_equal(x, y) for x, y in zip(a, b))
+    assert not all(np.array_equal(x, y) for x, y in zip(a, c))
+    # uncorrelated noise alone shifts the ADC by (500 e- * z_u) * 4 mV/ke- / LSB counts at the sample tick
+    p2 = W.default_params(n_readout_ticks=300, noise_uncorr_e=500.0)
+    hp, ht, ha, _ = oracle.electronics(p2, 42, [5], wave[:1])
+    z = oracle.noise_normals(42, 5, int(ht[0]))
+    q = 400.0 * (ht[0] - 20 + 1)
+    assert ha[0] == math.floor((580 + 4 * (q + 500.0 * z[1]) / 1000 - 288) / 3.953125)
