@@ -1,0 +1,240 @@
+/*
+ * lartpc.h -- C-ABI boundary of the B200-native charge-readout hot path of the pixelated
+ * LArTPC simulation of arXiv 2212.09807 (P:L### = line of /root/reference/PAPER.md).
+ *
+ * Path:  segments S_i = (r_s, r_e, E)_i  (eq. 2.1)
+ *   S1 lartpc_quench               recombination, eqs. (3.1)/(3.2)
+ *   S2 lartpc_drift                drift time, lifetime, diffusion, eqs. (3.3)-(3.5)
+ *   S3 lartpc_pixels_from_segments pixel / tick pre-sizing
+ *   S4 lartpc_induced_current      eq. (3.9) against the response LUT
+ *   S5 lartpc_sum_pixel_signals    per-pixel sum over tracks
+ *   S6 lartpc_electronics          LArPix CSA / discriminator / 8-bit ADC / noise
+ *   S7 lartpc_run_spill            S1..S6 streamed in TPC batches
+ *
+ * Conventions
+ *   - Plain C, no C++/torch types.  Every pointer inside a lartpc_*_t bundle is a DEVICE pointer
+ *     allocated and owned by the caller unless the field comment says "host".  The library owns
+ *     only what lartpc_sim_create copies (response LUT, TPC table) plus internal planning scratch
+ *     sized by the geometry and grown on demand (tile lists); see lartpc_sim_t.
+ *   - Units: cm, us, MeV, electrons, mV; ticks are integers of params.tick_us.
+ *   - All stage calls enqueue work on `stream` (a cudaStream_t passed as void*; NULL = default
+ *     stream).  S1, S2, S4, S6 return without synchronising.  S3 and S5 (plan mode) synchronise the
+ *     stream once because they report data-dependent sizes to the host, as the paper's pre-sizing
+ *     step does.  lartpc_run_spill synchronises internally per TPC batch.
+ *   - Return value: 0 = LARTPC_OK, negative = error (lartpc_strerror).  Nothing is thrown or
+ *     aborted across the ABI.  Capacity overflows found on the device (hit list full, more than
+ *     max_hits_per_pixel hits on a pixel) are counted in the output bundle / stats and never write
+ *     out of bounds.
+ *   - There is no CPU fallback and no dispatch: lartpc_sim_create fails unless the current device
+ *     has compute capability 10.x.
+ *   - A lartpc_sim_t holds the plan made by S3 for ONE batch of segments; S4/S5/S6 must follow on
+ *     the same sim, in order, before the next S3.  A sim is not re-entrant across streams.
+ */
+#ifndef LARTPC_H
+#define LARTPC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LARTPC_OK                 0
+#define LARTPC_ERR_BAD_ARGUMENT  (-1)
+#define LARTPC_ERR_CAPACITY      (-2)   /* a caller buffer is too small; the needed size is reported */
+#define LARTPC_ERR_CUDA          (-3)
+#define LARTPC_ERR_LUT_SHAPE     (-4)
+#define LARTPC_ERR_DEVICE        (-5)   /* not a compute-capability 10.x device */
+#define LARTPC_ERR_UNSUPPORTED   (-6)
+#define LARTPC_ERR_ORDER         (-7)   /* stage called without the plan of the preceding stage */
+
+typedef struct lartpc_sim lartpc_sim_t;   /* opaque: LUT copy, TPC table, planning scratch */
+
+/* All physics constants as doubles so that both sides of a parity test start from identical values.
+ * Defaults in brackets. */
+typedef struct {
+    double e_field_kv_cm, lar_density_g_cm3, w_ion_mev;        /* [0.5, 1.38, 23.6e-6] */
+    int    recomb_model;                                       /* 0 = Birks eq. (3.1), 1 = modified Box eq. (3.2) */
+    double birks_ab, birks_kb, box_alpha, box_beta;            /* [0.800, 0.0486, 0.93, 0.212 | 0.207] */
+    double v_drift_cm_us, lifetime_us;                         /* [0.16, 2200] */
+    double d_long_cm2_us, d_tran_cm2_us;                       /* [4.0e-6, 8.8e-6] = 4.0, 8.8 cm^2/s */
+    double tick_us, t_origin_us;                               /* [0.1, 0]; arrival tick j = floor((T - t_origin)/tick) */
+    double pixel_pitch_cm;                                     /* [0.4434] */
+    int    bins_per_pixel, window_pixels, lut_ticks;           /* nb [10], W [5 | 9, odd], K [200..2000, multiple of 4] */
+    int    n_readout_ticks;                                    /* readout ticks n = j + k, n in [0, n_readout_ticks) */
+    double sample_step_cm, n_sigma_map;                        /* [1e-3 = 10 um, 5.0] */
+    double gain_mv_per_ke, v_cm_mv, v_ref_mv, v_pedestal_mv;   /* [4, 288, 1300, 580] */
+    int    adc_bits;                                           /* [8] */
+    double threshold_e;                                        /* [7000] = 28 mV */
+    int    hold_ticks, min_spacing_ticks, periodic_reset_ticks;/* [16, 11, 0 = off] */
+    double noise_reset_e, noise_disc_e, noise_uncorr_e;        /* [0|900, 0|650, 0|500] */
+    int    max_hits_per_pixel;                                 /* capacity of the per-pixel hit scratch [32] */
+} lartpc_params_t;
+
+/* One TPC drift volume and its pixel plane.  Plane-local u = x - x0, v = y - y0; drift along z:
+ * d(z) = clamp(drift_sign * (z - z_anode), 0, drift_len) (eq. 3.3 with a sign for two-sided modules,
+ * P:L830).  Pixel (ix, iy) has global id first_pixel_id + iy * nx + ix. */
+typedef struct {
+    double x0, y0, z_anode;
+    int    drift_sign;          /* +1 or -1 */
+    double drift_len;
+    int    nx, ny;
+    int    first_pixel_id;
+} lartpc_tpc_t;
+
+/* Input: structure-of-arrays segments, each array float32[n] (eq. 2.1). */
+typedef struct {
+    const float *xs, *ys, *zs, *ts;     /* start point (cm) and time (us) */
+    const float *xe, *ye, *ze, *te;     /* end point and time */
+    const float *dE;                    /* deposited energy (MeV) */
+} lartpc_segments_t;
+
+/* S2 output, each array [n].  Endpoints stay in float64 so that the diffusion weights of S4 do not
+ * lose the sub-micron position of a segment on a 3 m plane ("fp32 cancellation"). */
+typedef struct {
+    int32_t *tpc;                       /* TPC index, -1 = midpoint in no TPC (inactive, D8) */
+    float   *q_anode;                   /* Q_a = n_e exp(-t_mid/tau), electrons (eq. 3.4) */
+    float   *sigma_T;                   /* transverse sigma, cm (eq. 3.5 with D_T) */
+    float   *sigma_t;                   /* longitudinal sigma as a time, us (sigma_L / v_drift) */
+    double  *u_s, *v_s, *u_e, *v_e;     /* plane-local endpoints, cm */
+    double  *T_s, *T_e;                 /* anode arrival times of the two ends, us */
+} lartpc_drifted_t;
+
+/* S3 output, each array int32[n] except offsets int64[n+1].  All integers are bit-exact functions of
+ * the float32 inputs (float64 IEEE arithmetic in a fixed order). */
+typedef struct {
+    int32_t *a_lo, *a_hi, *b_lo, *b_hi; /* charged-bin box (bin = pitch / bins_per_pixel), inclusive */
+    int32_t *ix0, *ix1, *iy0, *iy1;     /* pixel rectangle, inclusive; empty when ix0 > ix1 */
+    int32_t *jt0, *jt1;                 /* arrival-tick range, inclusive (not clipped to the window) */
+    int32_t *npix;                      /* pixels in the rectangle */
+    int32_t *n_samples;                 /* N = max(1, ceil(L / sample_step)) */
+    int64_t *offsets;                   /* exclusive scan of npix, [n+1] */
+} lartpc_pixmap_t;
+
+/* S3 host-side report (the paper's "longest signal / largest number of pixels") plus the sizes
+ * the caller needs to allocate the S4/S5/S6 outputs. */
+typedef struct {
+    int32_t max_npix;                   /* largest rectangle */
+    int32_t max_ticks;                  /* longest signal: max(jt1 - jt0 + 1) + lut_ticks - 1 */
+    int64_t total_npix;                 /* offsets[n] */
+    int64_t n_active_segments;          /* segments with a non-empty rectangle */
+    int64_t n_tiles;                    /* charge tiles (charged pixel x arrival-tick chunk) S4 will process */
+    int64_t n_pairs;                    /* (segment, charged pixel) incidences */
+    int64_t n_active_pixels;            /* pixels that can receive current */
+    int64_t total_samples;              /* sum of the per-pixel waveform lengths S5 will write */
+    int32_t tile_targets;               /* W*W: partial waveforms per tile */
+    int32_t tile_ticks;                 /* readout ticks per partial waveform (padded) */
+} lartpc_pixmap_info_t;
+
+/* S4 output: per-tile partial waveforms, float32 [n_tiles][tile_targets][tile_ticks] (electrons per
+ * tick).  Tile (charged pixel P, chunk c) holds the current its charge induces on the W x W pixels
+ * around P during readout ticks [c * chunk_ticks, c * chunk_ticks + tile_ticks).  The tile -> pixel
+ * map is part of the sim's plan.  `tile_range` int32[n_tiles][2] = first / last 8-tick block written. */
+typedef struct {
+    int64_t  tile_capacity;             /* host value: tiles the two buffers can hold */
+    float   *partial;
+    int32_t *tile_range;
+} lartpc_signals_t;
+
+/* S5 output: one waveform per active pixel, sorted by pixel id. */
+typedef struct {
+    int64_t  pixel_capacity;            /* host values: capacities of the arrays below */
+    int64_t  sample_capacity;
+    int32_t *pixel_id;                  /* [n_active] sorted unique global pixel ids */
+    int32_t *first_tick;                /* [n_active] readout tick of samples[offset] */
+    int32_t *length;                    /* [n_active] */
+    int64_t *offset;                    /* [n_active + 1] */
+    float   *samples;                   /* [total_samples] electrons per tick */
+    int64_t  n_active;                  /* host value, set by lartpc_sum_pixel_signals */
+    int64_t  total_samples;             /* host value, set by lartpc_sum_pixel_signals */
+} lartpc_waveforms_t;
+
+/* S6 output: compact hit list sorted by (pixel id, tick). */
+typedef struct {
+    int64_t  hit_capacity;              /* host value */
+    int32_t *hit_pixel;                 /* [hit_capacity] global pixel id */
+    int32_t *hit_tick;                  /* [hit_capacity] digitisation tick (D14) */
+    int32_t *hit_adc;                   /* [hit_capacity] ADC count 0 .. 2^adc_bits - 1 */
+    int32_t *hits_per_pixel;            /* [n_active] all hits, also those beyond max_hits_per_pixel */
+    float   *q_pixel;                   /* [n_active] Q_p = sum_n I_p[n], electrons */
+    int64_t *counters;                  /* device int64[4]: n_hits written, n_hits total, pixels over
+                                           max_hits_per_pixel, hits dropped for hit_capacity */
+} lartpc_hits_t;
+
+typedef struct {
+    int64_t n_segments, n_active_segments, n_tiles, n_pairs, n_active_pixels, total_samples;
+    int64_t n_hits, n_hits_total, n_pixels_overflow, n_hits_dropped;
+    int32_t n_batches;
+    int32_t reserved;
+    double  flops_current;              /* FMA * 2 issued by the S4 response + splat loops (counted on the host
+                                           from the plan; 0 when not computed) */
+} lartpc_stats_t;
+
+/* ---- lifetime -------------------------------------------------------------------------------- */
+
+/* Copies params, the TPC table and the response LUT (HOST pointer, float32 [W*nb][W*nb][K], tick
+ * fastest, R[cy][cx][k] = electrons induced during LUT tick k on the centre pixel of the W x W window by
+ * one electron above bin (cx, cy) that arrives during LUT tick K-1, D4, D5).  lut_elems must
+ * equal (W*nb)^2 * K. */
+int  lartpc_sim_create(const lartpc_params_t *params, const lartpc_tpc_t *tpcs, int n_tpcs,
+                       const float *response_lut_host, size_t lut_elems, lartpc_sim_t **out);
+void lartpc_sim_destroy(lartpc_sim_t *sim);
+
+/* Optional mask of disabled channels: HOST array of global pixel ids; S6 emits no hit for them. */
+int  lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *pixel_ids_host, int64_t n);
+
+/* Arrival ticks per charge tile (chunk_ticks) chosen for this LUT shape. */
+int  lartpc_chunk_ticks(const lartpc_sim_t *sim);
+
+/* Recommended workspace for lartpc_run_spill on up to max_segments segments. */
+size_t lartpc_workspace_bytes(const lartpc_sim_t *sim, int64_t max_segments);
+
+/* ---- stages ---------------------------------------------------------------------------------- */
+
+/* S1 (eqs. 3.1/3.2): dEdx[n] MeV/cm, n_e[n] electrons after recombination. */
+int  lartpc_quench(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n,
+                   float *dEdx, float *n_e, void *stream);
+
+/* S2 (eqs. 3.3-3.5). */
+int  lartpc_drift(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, const float *n_e,
+                  lartpc_drifted_t *out, void *stream);
+
+/* S3: pixel rectangles, tick ranges, sample counts; builds the sim's tile plan; fills *info (host)
+ * after one stream synchronisation. */
+int  lartpc_pixels_from_segments(lartpc_sim_t *sim, const lartpc_segments_t *seg,
+                                 const lartpc_drifted_t *drifted, int64_t n,
+                                 lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, void *stream);
+
+/* S4: needs out->tile_capacity >= info.n_tiles. */
+int  lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t *drifted, const lartpc_pixmap_t *pixmap,
+                            int64_t n, lartpc_signals_t *out, void *stream);
+
+/* S5: needs pixel_capacity >= info.n_active_pixels and sample_capacity >= info.total_samples. */
+int  lartpc_sum_pixel_signals(lartpc_sim_t *sim, const lartpc_signals_t *signals,
+                              lartpc_waveforms_t *out, void *stream);
+
+/* S6: Philox4x32-10 noise keyed by (seed, pixel id, tick). */
+int  lartpc_electronics(lartpc_sim_t *sim, const lartpc_waveforms_t *waveforms, uint64_t seed,
+                        lartpc_hits_t *out, void *stream);
+
+/* S7: the whole path on device-resident segments; hits of all batches are appended to *out in
+ * (pixel id, tick) order per batch (batches are TPC ranges, so the list is globally sorted).
+ * out->hits_per_pixel and out->q_pixel may be NULL. */
+int  lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, uint64_t seed,
+                      lartpc_hits_t *out, lartpc_stats_t *stats, void *workspace, size_t ws_bytes,
+                      void *stream);
+
+/* ---- measurement aids ------------------------------------------------------------------------ */
+
+/* Runs an FFMA-chain microbenchmark on `stream` and returns the measured FP32 rate in TFLOP/s
+ * (2 flop per FMA) through *tflops; variant 0 = scalar FFMA, 1 = packed FFMA2.  Used as the
+ * roofline denominator of S4. */
+int  lartpc_measure_fp32_peak(int variant, double *tflops, void *stream);
+
+const char *lartpc_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LARTPC_H */

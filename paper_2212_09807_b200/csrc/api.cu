@@ -1,0 +1,421 @@
+// C-ABI entry points of liblartpc (include/lartpc.h): sim lifetime, stage wrappers, the spill driver
+// and the FP32 peak microbenchmark used as the roofline denominator of S4.
+#include <stdio.h>
+#include <string.h>
+#include <algorithm>
+#include <new>
+#include "common.cuh"
+
+size_t lartpc_current_smem(const DevParams &p);
+int lartpc_current_tasks_per_group();
+
+static thread_local char g_last_cuda_error[256] = "";
+
+void lartpc_note_cuda_error(cudaError_t e, const char *file, int line)
+{
+    snprintf(g_last_cuda_error, sizeof(g_last_cuda_error), "%s (%s:%d)", cudaGetErrorString(e), file, line);
+    cudaGetLastError();
+}
+
+extern "C" const char *lartpc_strerror(int code)
+{
+    switch (code) {
+        case LARTPC_OK: return "ok";
+        case LARTPC_ERR_BAD_ARGUMENT: return "bad argument";
+        case LARTPC_ERR_CAPACITY: return "caller buffer too small";
+        case LARTPC_ERR_CUDA: return g_last_cuda_error[0] ? g_last_cuda_error : "CUDA error";
+        case LARTPC_ERR_LUT_SHAPE: return "response LUT shape does not match (W*nb)^2 * K";
+        case LARTPC_ERR_DEVICE: return "device is not compute capability 10.x (sm_100a only, no fallback)";
+        case LARTPC_ERR_UNSUPPORTED: return "unsupported parameter combination";
+        case LARTPC_ERR_ORDER: return "stage called out of order (no plan from lartpc_pixels_from_segments)";
+        default: return "unknown error";
+    }
+}
+
+static void sim_free(lartpc_sim *s)
+{
+    if (!s) return;
+    cudaFree(s->d_tpcs); cudaFree(s->d_lut);
+    cudaFree(s->pix_count); cudaFree(s->pix_start); cudaFree(s->pix_tile0); cudaFree(s->pix_cursor);
+    cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
+    cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->scan_tmp);
+    cudaFree(s->d_counters); cudaFree(s->disabled_mask); cudaFree(s->elec_slots); cudaFree(s->elec_offs);
+    if (s->h_counters) cudaFreeHost(s->h_counters);
+    delete s;
+}
+
+extern "C" void lartpc_sim_destroy(lartpc_sim_t *sim) { sim_free(sim); }
+
+extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t *tpcs, int n_tpcs,
+                                 const float *lut_host, size_t lut_elems, lartpc_sim_t **out)
+{
+    if (!prm || !tpcs || n_tpcs <= 0 || !lut_host || !out) return LARTPC_ERR_BAD_ARGUMENT;
+    *out = nullptr;
+    int dev = 0;
+    cudaDeviceProp prop;
+    LARTPC_CUDA_TRY(cudaGetDevice(&dev));
+    LARTPC_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) return LARTPC_ERR_DEVICE;
+    const int nb = prm->bins_per_pixel, W = prm->window_pixels, K = prm->lut_ticks;
+    if (nb < 1 || W < 1 || (W & 1) == 0 || K < 1 || prm->n_readout_ticks < K || prm->tick_us <= 0 ||
+        prm->pixel_pitch_cm <= 0 || prm->sample_step_cm <= 0 || prm->adc_bits < 1 || prm->adc_bits > 12 ||
+        prm->max_hits_per_pixel < 1 || prm->hold_ticks < 0 || prm->v_drift_cm_us <= 0)
+        return LARTPC_ERR_BAD_ARGUMENT;
+    if (lut_elems != (size_t)W * nb * W * nb * K) return LARTPC_ERR_LUT_SHAPE;
+    if (prm->n_readout_ticks >= (1 << 19)) return LARTPC_ERR_UNSUPPORTED;
+
+    lartpc_sim *s = new (std::nothrow) lartpc_sim();
+    if (!s) return LARTPC_ERR_BAD_ARGUMENT;
+    s->params = *prm;
+    s->tpcs.assign(tpcs, tpcs + n_tpcs);
+    s->sm_count = prop.multiProcessorCount;
+    DevParams &p = s->dp;
+    memset(&p, 0, sizeof(p));
+    p.eps = prm->e_field_kv_cm * prm->lar_density_g_cm3;  p.w_ion = prm->w_ion_mev;
+    p.birks_ab = prm->birks_ab; p.birks_kb = prm->birks_kb; p.box_alpha = prm->box_alpha; p.box_beta = prm->box_beta;
+    p.v_drift = prm->v_drift_cm_us; p.lifetime = prm->lifetime_us; p.d_long = prm->d_long_cm2_us;
+    p.d_tran = prm->d_tran_cm2_us; p.dt = prm->tick_us; p.t_origin = prm->t_origin_us; p.pitch = prm->pixel_pitch_cm;
+    p.bin = prm->pixel_pitch_cm / (double)nb;  p.sample_step = prm->sample_step_cm;  p.n_sigma_map = prm->n_sigma_map;
+    p.recomb_model = prm->recomb_model;
+    p.nb = nb; p.W = W; p.H = (W - 1) / 2; p.K = K; p.WW = W * W; p.NB2 = nb * nb;
+    p.n_ticks = prm->n_readout_ticks;  p.j_max = p.n_ticks - K;
+    p.RS = K + 22;
+    while ((p.RS & 3) != 0 || ((p.RS >> 2) & 1) == 0) ++p.RS;             // RS = 4 * odd: conflict-free LDS.128 rows
+    // arrival ticks per tile: as many as fit in shared memory, at most 120, multiple of 8
+    p.Jc = 120;
+    const size_t smem_limit = (size_t)prop.sharedMemPerBlockOptin;
+    for (;;) {
+        p.nblk_max = ((p.Jc + K - 2) >> 3) + 1;  p.tile_ticks = 8 * p.nblk_max;
+        if (lartpc_current_smem(p) <= smem_limit || p.Jc <= 8) break;
+        p.Jc -= 8;
+    }
+    if (lartpc_current_smem(p) > smem_limit) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    p.n_chunks = (p.j_max + p.Jc) / p.Jc;
+    if (p.n_chunks > 64) {                                                  // chunk masks are 64-bit
+        sim_free(s);
+        return LARTPC_ERR_UNSUPPORTED;
+    }
+    const int per_group = lartpc_current_tasks_per_group();
+    p.n_groups = (p.WW * p.nblk_max + per_group - 1) / per_group;
+    p.n_tpcs = n_tpcs;
+    p.gain_mv_per_ke = prm->gain_mv_per_ke; p.v_cm = prm->v_cm_mv; p.v_ref = prm->v_ref_mv; p.v_ped = prm->v_pedestal_mv;
+    p.adc_full = ldexp(1.0, prm->adc_bits);  p.threshold = prm->threshold_e;
+    p.noise_reset = prm->noise_reset_e; p.noise_disc = prm->noise_disc_e; p.noise_uncorr = prm->noise_uncorr_e;
+    p.hold = prm->hold_ticks; p.min_spacing = prm->min_spacing_ticks; p.periodic = prm->periodic_reset_ticks;
+    p.max_hits = prm->max_hits_per_pixel;
+
+    std::vector<DevTpc> dt(n_tpcs);
+    int64_t cp = 0, pix = 0;
+    for (int k = 0; k < n_tpcs; ++k) {
+        const lartpc_tpc_t &t = tpcs[k];
+        if (t.nx < 1 || t.ny < 1 || (t.drift_sign != 1 && t.drift_sign != -1) || t.drift_len < 0 ||
+            t.first_pixel_id != pix) {                                      // pixel ids must be dense, in table order
+            sim_free(s);
+            return LARTPC_ERR_BAD_ARGUMENT;
+        }
+        DevTpc &d = dt[k];
+        d.x0 = t.x0; d.y0 = t.y0; d.z_anode = t.z_anode; d.drift_len = t.drift_len;
+        d.x1 = t.x0 + (double)t.nx * prm->pixel_pitch_cm;  d.y1 = t.y0 + (double)t.ny * prm->pixel_pitch_cm;
+        d.sign = t.drift_sign; d.nx = t.nx; d.ny = t.ny; d.first_pixel_id = t.first_pixel_id;
+        d.gw = t.nx + 2 * p.H; d.gh = t.ny + 2 * p.H; d.cp_base = (int)cp; d.pad = 0;
+        cp += (int64_t)d.gw * d.gh;
+        pix += (int64_t)t.nx * t.ny;
+    }
+    if (cp >= INT32_MAX || pix >= INT32_MAX) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    s->n_cp = cp; s->n_pix = pix;
+
+    // LUT re-laid out as [bin c = cb*nb+ca][target d = dyi*W+dxi][RS] with LUT tick k at word 7+k and zero
+    // padding around it, so that S4 stages all W*W rows of one bin with a single contiguous copy and reads
+    // 16-tap windows with aligned 128-bit loads.  Row (c, d) is R[cy = nb*dyi + cb][cx = nb*dxi + ca][.].
+    std::vector<float> re((size_t)p.NB2 * p.WW * p.RS, 0.f);
+    const int NB = W * nb;
+    for (int cb = 0; cb < nb; ++cb)
+        for (int ca = 0; ca < nb; ++ca)
+            for (int dyi = 0; dyi < W; ++dyi)
+                for (int dxi = 0; dxi < W; ++dxi) {
+                    const float *src = lut_host + ((size_t)(nb * dyi + cb) * NB + (nb * dxi + ca)) * K;
+                    float *dst = re.data() + ((size_t)(cb * nb + ca) * p.WW + (dyi * W + dxi)) * p.RS + 7;
+                    memcpy(dst, src, sizeof(float) * K);
+                }
+#define SIM_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { \
+        lartpc_note_cuda_error(_e, __FILE__, __LINE__); sim_free(s); return LARTPC_ERR_CUDA; } } while (0)
+    SIM_TRY(cudaMalloc(&s->d_lut, sizeof(float) * re.size()));
+    SIM_TRY(cudaMemcpy(s->d_lut, re.data(), sizeof(float) * re.size(), cudaMemcpyHostToDevice));
+    SIM_TRY(cudaMalloc(&s->d_tpcs, sizeof(DevTpc) * n_tpcs));
+    SIM_TRY(cudaMemcpy(s->d_tpcs, dt.data(), sizeof(DevTpc) * n_tpcs, cudaMemcpyHostToDevice));
+    SIM_TRY(cudaMalloc(&s->pix_count, sizeof(int32_t) * cp));
+    SIM_TRY(cudaMalloc(&s->pix_start, sizeof(int32_t) * cp));
+    SIM_TRY(cudaMalloc(&s->pix_tile0, sizeof(int32_t) * cp));
+    SIM_TRY(cudaMalloc(&s->pix_cursor, sizeof(int32_t) * cp));
+    SIM_TRY(cudaMalloc(&s->pix_mask, sizeof(unsigned long long) * cp));
+    SIM_TRY(cudaMalloc(&s->act_first, sizeof(int32_t) * pix));
+    SIM_TRY(cudaMalloc(&s->act_last, sizeof(int32_t) * pix));
+    SIM_TRY(cudaMalloc(&s->act_slot, sizeof(int32_t) * pix));
+    SIM_TRY(cudaMalloc(&s->d_counters, sizeof(long long) * CNT_COUNT));
+    SIM_TRY(cudaMallocHost(&s->h_counters, sizeof(long long) * CNT_COUNT));
+    s->pair_cap = 1 << 16;  s->tile_cap = 1 << 14;
+    SIM_TRY(cudaMalloc(&s->pair_seg, sizeof(int32_t) * s->pair_cap));
+    SIM_TRY(cudaMalloc(&s->tile_cp, sizeof(int32_t) * s->tile_cap));
+    SIM_TRY(cudaMalloc(&s->tile_desc, sizeof(TileDesc) * s->tile_cap));
+#undef SIM_TRY
+    *out = s;
+    return LARTPC_OK;
+}
+
+extern "C" int lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *ids, int64_t n)
+{
+    if (!sim || (n > 0 && !ids)) return LARTPC_ERR_BAD_ARGUMENT;
+    const size_t words = (size_t)(sim->n_pix + 31) / 32;
+    std::vector<uint32_t> m(words, 0u);
+    for (int64_t i = 0; i < n; ++i) {
+        if (ids[i] < 0 || ids[i] >= sim->n_pix) return LARTPC_ERR_BAD_ARGUMENT;
+        m[ids[i] >> 5] |= 1u << (ids[i] & 31);
+    }
+    if (!sim->disabled_mask) LARTPC_CUDA_TRY(cudaMalloc(&sim->disabled_mask, sizeof(uint32_t) * words));
+    LARTPC_CUDA_TRY(cudaMemcpy(sim->disabled_mask, m.data(), sizeof(uint32_t) * words, cudaMemcpyHostToDevice));
+    return LARTPC_OK;
+}
+
+extern "C" int lartpc_chunk_ticks(const lartpc_sim_t *sim) { return sim ? sim->dp.Jc : 0; }
+
+// ---- stage wrappers -------------------------------------------------------------------------------
+extern "C" int lartpc_quench(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, float *dEdx, float *n_e,
+                             void *stream)
+{
+    if (!sim || !seg || n < 0 || (n > 0 && (!dEdx || !n_e))) return LARTPC_ERR_BAD_ARGUMENT;
+    return launch_quench(sim, seg, n, dEdx, n_e, (cudaStream_t)stream);
+}
+
+extern "C" int lartpc_drift(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, const float *n_e,
+                            lartpc_drifted_t *out, void *stream)
+{
+    if (!sim || !seg || n < 0 || !out || (n > 0 && !n_e)) return LARTPC_ERR_BAD_ARGUMENT;
+    return launch_drift(sim, seg, n, n_e, out, (cudaStream_t)stream);
+}
+
+extern "C" int lartpc_pixels_from_segments(lartpc_sim_t *sim, const lartpc_segments_t *seg,
+                                           const lartpc_drifted_t *dr, int64_t n, lartpc_pixmap_t *out,
+                                           lartpc_pixmap_info_t *info, void *stream)
+{
+    if (!sim || !seg || !dr || !out || n < 0) return LARTPC_ERR_BAD_ARGUMENT;
+    return launch_plan(sim, seg, dr, n, 0, sim->dp.n_tpcs, out, info, (cudaStream_t)stream);
+}
+
+extern "C" int lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm,
+                                      int64_t n, lartpc_signals_t *out, void *stream)
+{
+    if (!sim || !dr || !pm || !out) return LARTPC_ERR_BAD_ARGUMENT;
+    if (!sim->have_plan || n != sim->plan_n) return LARTPC_ERR_ORDER;
+    if (out->tile_capacity < sim->n_tiles) return LARTPC_ERR_CAPACITY;
+    int rc = launch_current(sim, dr, pm, n, out, (cudaStream_t)stream);
+    if (rc == 0) sim->have_signals = true;
+    return rc;
+}
+
+extern "C" int lartpc_sum_pixel_signals(lartpc_sim_t *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out,
+                                        void *stream)
+{
+    if (!sim || !sig || !out) return LARTPC_ERR_BAD_ARGUMENT;
+    if (!sim->have_plan || !sim->have_signals) return LARTPC_ERR_ORDER;
+    if (out->pixel_capacity < sim->n_active || out->sample_capacity < sim->total_samples) return LARTPC_ERR_CAPACITY;
+    return launch_sum(sim, sig, out, (cudaStream_t)stream);
+}
+
+static int ensure_i32(int32_t **p, int64_t *cap, int64_t need)
+{
+    if (need <= *cap) return LARTPC_OK;
+    if (*p) cudaFree(*p);
+    *p = nullptr;
+    LARTPC_CUDA_TRY(cudaMalloc(p, sizeof(int32_t) * (need + need / 4 + 256)));
+    *cap = need + need / 4 + 256;
+    return LARTPC_OK;
+}
+
+extern "C" int lartpc_electronics(lartpc_sim_t *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
+                                  void *stream)
+{
+    if (!sim || !wf || !out || !out->counters || !out->hits_per_pixel || !out->q_pixel) return LARTPC_ERR_BAD_ARGUMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    LARTPC_CUDA_TRY(cudaMemsetAsync(out->counters, 0, sizeof(int64_t) * 4, st));
+    // the per-pixel hit slots live in sim-owned scratch, grown on demand (no allocation after warm-up)
+    int rc;
+    if ((rc = ensure_i32(&sim->elec_slots, &sim->elec_slots_cap, wf->n_active * sim->dp.max_hits)) != 0) return rc;
+    if ((rc = ensure_i32(&sim->elec_offs, &sim->elec_offs_cap, wf->n_active + 1)) != 0) return rc;
+    return launch_electronics(sim, wf, seed, out, sim->elec_slots, sim->elec_offs, 0, st);
+}
+
+// ---- S7 spill driver ------------------------------------------------------------------------------
+namespace {
+struct Arena {
+    char *base; size_t size, used;
+    template <typename T> T *take(int64_t n)
+    {
+        size_t bytes = ((size_t)(n > 0 ? n : 1) * sizeof(T) + 255) & ~(size_t)255;
+        if (used + bytes > size) return nullptr;
+        T *p = (T *)(base + used);
+        used += bytes;
+        return p;
+    }
+};
+}  // namespace
+
+extern "C" size_t lartpc_workspace_bytes(const lartpc_sim_t *sim, int64_t max_segments)
+{
+    if (!sim) return 0;
+    // per segment: n_e, dEdx (8) + drifted (64) + pixmap (12*4 + 8) = 128 B; plus tile partials / waveforms of
+    // the largest TPC batch, which depend on the data: 3 GiB covers the BASELINE configs with room to spare.
+    return (size_t)max_segments * 160 + ((size_t)3 << 30);
+}
+
+extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, uint64_t seed,
+                                lartpc_hits_t *out, lartpc_stats_t *stats, void *workspace, size_t ws_bytes,
+                                void *stream)
+{
+    if (!sim || !seg || !out || !out->counters || !workspace || n < 0) return LARTPC_ERR_BAD_ARGUMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const DevParams &p = sim->dp;
+    Arena ar{(char *)workspace, ws_bytes, 0};
+    lartpc_stats_t stt;
+    memset(&stt, 0, sizeof(stt));
+    stt.n_segments = n;
+    LARTPC_CUDA_TRY(cudaMemsetAsync(out->counters, 0, sizeof(int64_t) * 4, st));
+
+    float *dEdx = ar.take<float>(n), *n_e = ar.take<float>(n);
+    lartpc_drifted_t dr;
+    dr.tpc = ar.take<int32_t>(n); dr.q_anode = ar.take<float>(n); dr.sigma_T = ar.take<float>(n);
+    dr.sigma_t = ar.take<float>(n);
+    dr.u_s = ar.take<double>(n); dr.v_s = ar.take<double>(n); dr.u_e = ar.take<double>(n); dr.v_e = ar.take<double>(n);
+    dr.T_s = ar.take<double>(n); dr.T_e = ar.take<double>(n);
+    lartpc_pixmap_t pm;
+    pm.a_lo = ar.take<int32_t>(n); pm.a_hi = ar.take<int32_t>(n); pm.b_lo = ar.take<int32_t>(n);
+    pm.b_hi = ar.take<int32_t>(n); pm.ix0 = ar.take<int32_t>(n); pm.ix1 = ar.take<int32_t>(n);
+    pm.iy0 = ar.take<int32_t>(n); pm.iy1 = ar.take<int32_t>(n); pm.jt0 = ar.take<int32_t>(n);
+    pm.jt1 = ar.take<int32_t>(n); pm.npix = ar.take<int32_t>(n); pm.n_samples = ar.take<int32_t>(n);
+    pm.offsets = ar.take<int64_t>(n + 1);
+    if (!pm.offsets || !dEdx) return LARTPC_ERR_CAPACITY;
+    const size_t mark = ar.used;
+
+    int rc;
+    if ((rc = launch_quench(sim, seg, n, dEdx, n_e, st)) != 0) return rc;
+    if ((rc = launch_drift(sim, seg, n, n_e, &dr, st)) != 0) return rc;
+
+    // batches of consecutive TPCs; a batch whose tiles / waveforms do not fit the workspace is halved
+    int tpc_lo = 0;
+    int batch = p.n_tpcs;
+    while (tpc_lo < p.n_tpcs) {
+        int tpc_hi = std::min(p.n_tpcs, tpc_lo + batch);
+        lartpc_pixmap_info_t info;
+        if ((rc = launch_plan(sim, seg, &dr, n, tpc_lo, tpc_hi, &pm, &info, st)) != 0) return rc;
+        ar.used = mark;
+        lartpc_signals_t sig;
+        sig.tile_capacity = info.n_tiles;
+        sig.partial = ar.take<float>(info.n_tiles * p.WW * p.tile_ticks);
+        sig.tile_range = ar.take<int32_t>(info.n_tiles * 2);
+        lartpc_waveforms_t wf;
+        wf.pixel_capacity = info.n_active_pixels;  wf.sample_capacity = info.total_samples;
+        wf.pixel_id = ar.take<int32_t>(info.n_active_pixels);
+        wf.first_tick = ar.take<int32_t>(info.n_active_pixels);
+        wf.length = ar.take<int32_t>(info.n_active_pixels);
+        wf.offset = ar.take<int64_t>(info.n_active_pixels + 1);
+        wf.samples = ar.take<float>(info.total_samples);
+        int32_t *slots = ar.take<int32_t>(info.n_active_pixels * p.max_hits);
+        int32_t *offs = ar.take<int32_t>(info.n_active_pixels + 2);
+        lartpc_hits_t h = *out;
+        h.hits_per_pixel = ar.take<int32_t>(info.n_active_pixels);
+        h.q_pixel = ar.take<float>(info.n_active_pixels);
+        if (!sig.partial || !sig.tile_range || !wf.samples || !slots || !offs || !h.q_pixel) {
+            if (tpc_hi - tpc_lo <= 1) return LARTPC_ERR_CAPACITY;       // one TPC does not fit the workspace
+            batch = std::max(1, (tpc_hi - tpc_lo) / 2);
+            continue;
+        }
+        if (tpc_lo == 0) { stt.n_active_segments = info.n_active_segments; }
+        stt.n_tiles += info.n_tiles;  stt.n_pairs += info.n_pairs;
+        stt.n_active_pixels += info.n_active_pixels;  stt.total_samples += info.total_samples;
+        stt.n_batches += 1;
+        if ((rc = launch_current(sim, &dr, &pm, n, &sig, st)) != 0) return rc;
+        sim->have_signals = true;
+        if ((rc = launch_sum(sim, &sig, &wf, st)) != 0) return rc;
+        if ((rc = launch_electronics(sim, &wf, seed, &h, slots, offs, 0, st)) != 0) return rc;
+        tpc_lo = tpc_hi;
+    }
+    long long hc[4];
+    LARTPC_CUDA_TRY(cudaMemcpyAsync(hc, out->counters, sizeof(hc), cudaMemcpyDeviceToHost, st));
+    LARTPC_CUDA_TRY(cudaStreamSynchronize(st));
+    stt.n_hits = hc[0]; stt.n_hits_total = hc[1]; stt.n_pixels_overflow = hc[2]; stt.n_hits_dropped = hc[3];
+    if (stats) *stats = stt;
+    return LARTPC_OK;
+}
+
+// ---- FP32 peak microbenchmark (roofline denominator of S4) -----------------------------
+template <int VARIANT>
+__global__ void __launch_bounds__(256) fp32_peak_kernel(float *sink, int iters, float seed)
+{
+    if (VARIANT == 0) {
+        float a[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) a[i] = seed + (float)(threadIdx.x + i);
+        const float b = 0.999f, c = 1e-3f;
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int i = 0; i < 16; ++i) a[i] = fmaf(a[i], b, c);
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) s += a[i];
+        if (s == 123.456f) sink[0] = s;
+    } else {
+        float2 a[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) a[i] = make_float2(seed + (float)(threadIdx.x + i), seed - (float)i);
+        const float2 b = make_float2(0.999f, 0.998f), c = make_float2(1e-3f, 2e-3f);
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    unsigned long long av, bv, cv;
+                    av = *(unsigned long long *)&a[i]; bv = *(const unsigned long long *)&b; cv = *(const unsigned long long *)&c;
+                    asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(av) : "l"(av), "l"(bv), "l"(cv));
+                    a[i] = *(float2 *)&av;
+                }
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) s += a[i].x + a[i].y;
+        if (s == 123.456f) sink[0] = s;
+    }
+}
+
+extern "C" int lartpc_measure_fp32_peak(int variant, double *tflops, void *stream)
+{
+    if (!tflops || variant < 0 || variant > 1) return LARTPC_ERR_BAD_ARGUMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    LARTPC_CUDA_TRY(cudaGetDevice(&dev));
+    LARTPC_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float *sink = nullptr;
+    LARTPC_CUDA_TRY(cudaMalloc(&sink, 16));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 4096, blocks = sms * 8, threads = 256;
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, st);
+        if (variant == 0) fp32_peak_kernel<0><<<blocks, threads, 0, st>>>(sink, iters, 1.0f);
+        else fp32_peak_kernel<1><<<blocks, threads, 0, st>>>(sink, iters, 1.0f);
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double fma = (double)blocks * threads * iters * 128.0;       // 8 rounds x 16 FMA per thread per iteration
+        double tf = 2.0 * fma / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    *tflops = best;
+    return LARTPC_OK;
+}

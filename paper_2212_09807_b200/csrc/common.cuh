@@ -1,0 +1,120 @@
+// Internal definitions shared by the sm_100a kernels of liblartpc (not part of the C-ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <vector>
+#include "../../include/lartpc.h"
+
+#define LARTPC_CUDA_TRY(expr)                                   \
+    do {                                                        \
+        cudaError_t _e = (expr);                                \
+        if (_e != cudaSuccess) { lartpc_note_cuda_error(_e, __FILE__, __LINE__); return LARTPC_ERR_CUDA; } \
+    } while (0)
+
+void lartpc_note_cuda_error(cudaError_t e, const char *file, int line);
+
+// ---- constants copied to every kernel by value ------------------------------------------------
+struct DevParams {
+    // recombination / transport (float64: the index path must be IEEE-exact)
+    double eps, w_ion, birks_ab, birks_kb, box_alpha, box_beta;
+    double v_drift, lifetime, d_long, d_tran, dt, t_origin, pitch, bin, sample_step, n_sigma_map;
+    int recomb_model;
+    int nb, W, H, K, WW, NB2;        // bins per pixel, window pixels, half window, LUT ticks, W*W, nb*nb
+    int n_ticks, j_max;              // readout ticks, last arrival tick inside the window (n_ticks - K)
+    int Jc, n_chunks;                // arrival ticks per charge tile, chunks covering [0, j_max]
+    int nblk_max, tile_ticks;        // 8-tick output blocks per tile, 8 * nblk_max
+    int RS;                          // padded LUT row stride in floats: [7 zeros][K][zeros], RS = 4 * odd
+    int n_groups;                    // thread-task groups per tile (1 for W = 5, K = 200)
+    int n_tpcs;
+    // electronics
+    double gain_mv_per_ke, v_cm, v_ref, v_ped, adc_full, threshold;
+    double noise_reset, noise_disc, noise_uncorr;
+    int hold, min_spacing, periodic, max_hits;
+};
+
+struct DevTpc {
+    double x0, y0, x1, y1, z_anode, drift_len;
+    int sign, nx, ny, first_pixel_id;
+    int gw, gh;                      // charged-pixel grid (nx + 2H) x (ny + 2H): charge just outside the
+    int cp_base;                     // plane still acts on in-plane pixels
+    int pad;
+};
+
+struct SegPtrs { const float *xs, *ys, *zs, *ts, *xe, *ye, *ze, *te, *dE; };
+
+// charge tile = (charged pixel, arrival-tick chunk)
+struct TileDesc { int tpc, px, py, chunk; };
+
+// device counters written by the planning kernels (mirrored to pinned host memory)
+enum {
+    CNT_MAX_NPIX = 0, CNT_MAX_TICKS, CNT_ACTIVE_SEGS, CNT_PAIRS, CNT_TILES, CNT_ACTIVE_PIX,
+    CNT_TOTAL_SAMPLES, CNT_TOTAL_NPIX, CNT_OVERFLOW, CNT_COUNT = 16
+};
+
+struct lartpc_sim {
+    lartpc_params_t params;
+    std::vector<lartpc_tpc_t> tpcs;
+    DevParams dp;
+    DevTpc *d_tpcs = nullptr;
+    float *d_lut = nullptr;              // [NB2][WW][RS], zero padded rows
+    int64_t n_cp = 0;                    // charged-pixel grid cells over all TPCs
+    int64_t n_pix = 0;                   // pixels over all TPCs (global pixel ids are 0 .. n_pix-1)
+    int32_t pix_id_base = 0;
+    // dense planning arrays
+    int32_t *pix_count = nullptr, *pix_start = nullptr, *pix_tile0 = nullptr, *pix_cursor = nullptr;
+    unsigned long long *pix_mask = nullptr;
+    int32_t *act_first = nullptr, *act_last = nullptr, *act_slot = nullptr;
+    // growable planning arrays
+    int32_t *pair_seg = nullptr;  int64_t pair_cap = 0;
+    int32_t *tile_cp = nullptr;   TileDesc *tile_desc = nullptr;  int64_t tile_cap = 0;
+    // scan scratch + counters
+    long long *scan_tmp = nullptr;  int64_t scan_tmp_elems = 0;
+    long long *d_counters = nullptr;  long long *h_counters = nullptr;
+    uint32_t *disabled_mask = nullptr;
+    int32_t *elec_slots = nullptr, *elec_offs = nullptr;  int64_t elec_slots_cap = 0, elec_offs_cap = 0;
+    // plan state
+    bool have_plan = false, have_signals = false;
+    int64_t plan_n = 0, n_tiles = 0, n_pairs = 0, n_active = 0, total_samples = 0;
+    const lartpc_drifted_t *plan_drifted = nullptr;
+    lartpc_drifted_t drifted_copy;
+    lartpc_pixmap_t pixmap_copy;
+    int sm_count = 148;
+};
+
+// ---- IEEE-exact float64 helpers (never contracted into FMA) -----------------------------------
+__device__ __forceinline__ double xmul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double xadd(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double xsub(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ double xdiv(double a, double b) { return __ddiv_rn(a, b); }
+__device__ __forceinline__ double xsqrt(double a) { return __dsqrt_rn(a); }
+__device__ __forceinline__ long long floor_div_ll(long long a, long long b)
+{
+    long long q = a / b;
+    if ((a % b != 0) && ((a < 0) != (b < 0))) --q;
+    return q;
+}
+
+// drift distance of a point, eq. (3.3): clamp(sign * (z - z_anode), 0, drift_len)
+__device__ __forceinline__ double drift_dist(const DevTpc &t, double z)
+{
+    double d = xmul((double)t.sign, xsub(z, t.z_anode));
+    if (d < 0.0) d = 0.0;
+    if (d > t.drift_len) d = t.drift_len;
+    return d;
+}
+
+// ---- launch helpers -----------------------------------------------------------------------------
+static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// stage launchers (host, C++ linkage)
+int launch_quench(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, float *dEdx, float *n_e, cudaStream_t st);
+int launch_drift(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, const float *n_e, lartpc_drifted_t *out,
+                 cudaStream_t st);
+int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drifted_t *dr, int64_t n,
+                int tpc_lo, int tpc_hi, lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, cudaStream_t st);
+int launch_current(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
+                   lartpc_signals_t *out, cudaStream_t st);
+int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out, cudaStream_t st);
+int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
+                       int32_t *slot_scratch, int32_t *scan_scratch, int64_t hit_base, cudaStream_t st);
+int sim_ensure_scan_tmp(lartpc_sim *sim, int64_t elems);

@@ -1,0 +1,237 @@
+// S5 per-pixel sum and S6 LArPix-style electronics: parallel over pixels.
+#include "common.cuh"
+#include "scan.cuh"
+
+// -------------------------------------------------------------------------------------------------
+// S5: active-pixel table (sorted by pixel id) and the gather-sum of the tile partial waveforms.
+// Every sample is written once by one thread, adding the <= W*W x 3 contributing tiles in a fixed
+// order (target index ascending, chunk ascending), so the sum is reproducible bit for bit.
+// -------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+active_table_kernel(int64_t n_pix, const int32_t *__restrict__ act_first, const int32_t *__restrict__ act_last,
+                    const int32_t *__restrict__ act_slot, int32_t *pixel_id, int32_t *first_tick, int32_t *length)
+{
+    int64_t gp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gp >= n_pix) return;
+    int last = act_last[gp];
+    if (last < 0) return;
+    int slot = act_slot[gp];
+    pixel_id[slot] = (int32_t)gp;
+    first_tick[slot] = act_first[gp];
+    length[slot] = last - act_first[gp] + 1;
+}
+
+struct LenF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
+
+__global__ void __launch_bounds__(256)
+sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__restrict__ pixel_id,
+                 const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,
+                 const int64_t *__restrict__ offset, const unsigned long long *__restrict__ pix_mask,
+                 const int32_t *__restrict__ pix_tile0, const float *__restrict__ partial,
+                 const int32_t *__restrict__ tile_range, float *samples)
+{
+    __shared__ unsigned long long s_mask[128];
+    __shared__ int s_tile0[128];
+    const int slot = blockIdx.x;
+    const int gp = pixel_id[slot];
+    int tpc = 0;
+    while (tpc + 1 < p.n_tpcs && tpcs[tpc + 1].first_pixel_id <= gp) ++tpc;
+    const DevTpc &t = tpcs[tpc];
+    const int rel = gp - t.first_pixel_id, iy = rel / t.nx, ix = rel - iy * t.nx;
+    for (int d = threadIdx.x; d < p.WW; d += blockDim.x) {
+        const int dyi = d / p.W, dxi = d - dyi * p.W;
+        const int cp = t.cp_base + (iy + dyi) * t.gw + (ix + dxi);   // charged pixel px = ix - H + dxi
+        s_mask[d] = pix_mask[cp];
+        s_tile0[d] = pix_tile0[cp];
+    }
+    __syncthreads();
+    const int first = first_tick[slot], len = length[slot];
+    const int64_t off = offset[slot];
+    const int span = p.Jc + p.K - 2;                                  // a tile reaches readout ticks [c Jc, c Jc + span]
+    for (int i = threadIdx.x; i < len; i += blockDim.x) {
+        const int n = first + i;
+        const int c_hi = min(n / p.Jc, p.n_chunks - 1);
+        const int c_lo = n > span ? (n - span + p.Jc - 1) / p.Jc : 0;
+        float sum = 0.f;
+        for (int d = 0; d < p.WW; ++d) {
+            const unsigned long long m = s_mask[d];
+            if (!m) continue;
+            for (int c = c_lo; c <= c_hi; ++c) {
+                if (!((m >> c) & 1ull)) continue;
+                const int tix = s_tile0[d] + __popcll(m & ((1ull << c) - 1ull));
+                const int nrel = n - c * p.Jc, blk = nrel >> 3;
+                if (blk >= tile_range[2 * tix] && blk <= tile_range[2 * tix + 1])
+                    sum += partial[((size_t)tix * p.WW + d) * p.tile_ticks + nrel];
+            }
+        }
+        samples[off + i] = sum;
+    }
+}
+
+int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out, cudaStream_t st)
+{
+    const DevParams &p = sim->dp;
+    out->n_active = sim->n_active;
+    out->total_samples = sim->total_samples;
+    if (sim->n_active == 0) {
+        LARTPC_CUDA_TRY(cudaMemsetAsync(out->offset, 0, sizeof(int64_t), st));
+        return LARTPC_OK;
+    }
+    if (p.WW > 128) return LARTPC_ERR_UNSUPPORTED;
+    active_table_kernel<<<div_up(sim->n_pix, 256), 256, 0, st>>>(sim->n_pix, sim->act_first, sim->act_last,
+                                                                sim->act_slot, out->pixel_id, out->first_tick,
+                                                                out->length);
+    int rc = sim_ensure_scan_tmp(sim, sim->n_active);
+    if (rc) return rc;
+    LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_active, LenF{out->length}, out->offset, true, (long long *)nullptr,
+                                          sim->scan_tmp, st));
+    sum_pixel_kernel<<<(unsigned)sim->n_active, 256, 0, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
+                                                             out->length, out->offset, sim->pix_mask, sim->pix_tile0,
+                                                             sig->partial, sig->tile_range, out->samples);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}
+
+// -------------------------------------------------------------------------------------------------
+// S6: one thread per active pixel, serial over ticks, state in registers.
+// Noise: Philox4x32-10, counter (pixel id, tick, 0, 0), key (seed lo, seed hi); Box-Muller in float64 so
+// that the ADC decision is taken in the same precision as the oracle's.
+// -------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t lo0 = 0xD2511F53u * c0, hi0 = __umulhi(0xD2511F53u, c0);
+        const uint32_t lo1 = 0xCD9E8D57u * c2, hi1 = __umulhi(0xCD9E8D57u, c2);
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+__device__ __forceinline__ void noise_normals(unsigned long long seed, uint32_t pixel, uint32_t tick, double (&z)[3])
+{
+    uint32_t x[4];
+    philox4x32_10(pixel, tick, 0u, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), x);
+    const double s = 1.0 / 4294967296.0, two_pi = 6.283185307179586476925286766559;
+    const double u0 = ((double)x[0] + 0.5) * s, u1 = ((double)x[1] + 0.5) * s;
+    const double u2 = ((double)x[2] + 0.5) * s, u3 = ((double)x[3] + 0.5) * s;
+    const double r01 = sqrt(-2.0 * log(u0)), r23 = sqrt(-2.0 * log(u2));
+    z[0] = r01 * cos(two_pi * u1);
+    z[1] = r01 * sin(two_pi * u1);
+    z[2] = r23 * cos(two_pi * u3);
+}
+
+constexpr int ADC_SHIFT = 12;   // hit slot = tick << 12 | adc
+
+__global__ void __launch_bounds__(128)
+electronics_kernel(DevParams p, unsigned long long seed, int64_t n_active, const int32_t *__restrict__ pixel_id,
+                   const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,
+                   const int64_t *__restrict__ offset, const float *__restrict__ samples,
+                   const uint32_t *__restrict__ disabled, int32_t *slots, int32_t *hits_per_pixel, float *q_pixel)
+{
+    const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= n_active) return;
+    const int pid = pixel_id[slot];
+    const int first = first_tick[slot], len = length[slot];
+    const float *w = samples + offset[slot];
+    const bool every_tick = p.noise_disc != 0.0 || p.periodic > 0;     // the state can change outside the support
+    const bool any_noise = p.noise_disc != 0.0 || p.noise_uncorr != 0.0 || p.noise_reset != 0.0;
+    const bool off_channel = disabled && ((disabled[pid >> 5] >> (pid & 31)) & 1u);
+    int n_begin = every_tick ? 0 : first;
+    int n_end = every_tick ? p.n_ticks : first + len;                    // exclusive; extended while a hold is pending
+    double q = 0.0, qsum = 0.0;
+    bool armed = true;
+    int n_c = 0, nhits = 0;
+    long long rearm_at = 0;
+    int32_t *my = slots + slot * p.max_hits;
+    for (int n = n_begin; n < p.n_ticks; ++n) {
+        if (n >= n_end && armed && q < p.threshold) break;            // nothing can happen any more
+        double z[3] = {0.0, 0.0, 0.0};
+        bool have_z = false;
+        if (p.noise_disc != 0.0) { noise_normals(seed, (uint32_t)pid, (uint32_t)n, z); have_z = true; }
+        if (armed && p.periodic > 0 && n > 0 && (n % p.periodic) == 0) q = 0.0;
+        const int i = n - first;
+        const double cur = (i >= 0 && i < len) ? (double)w[i] : 0.0;
+        q += cur;  qsum += cur;
+        if (armed && n >= rearm_at && q >= p.threshold + p.noise_disc * z[0]) { armed = false; n_c = n; }
+        if (!armed && n == n_c + p.hold) {
+            if (!have_z && any_noise) noise_normals(seed, (uint32_t)pid, (uint32_t)n, z);
+            const double q_s = q + p.noise_uncorr * z[1];
+            const double V = p.v_ped + p.gain_mv_per_ke * q_s / 1000.0;
+            double a = floor((V - p.v_cm) / (p.v_ref - p.v_cm) * p.adc_full);
+            a = fmin(fmax(a, 0.0), p.adc_full - 1.0);
+            if (!off_channel) {
+                if (nhits < p.max_hits) my[nhits] = (n << ADC_SHIFT) | (int)a;
+                ++nhits;
+            }
+            q = p.noise_reset * z[2];
+            armed = true;
+            rearm_at = max((long long)n + 1, (long long)n + p.min_spacing - p.hold);
+        }
+    }
+    hits_per_pixel[slot] = nhits;
+    q_pixel[slot] = (float)qsum;
+}
+
+struct HitCountF {
+    const int32_t *v; int cap;
+    __device__ long long operator()(int64_t i) const { return v[i] < cap ? v[i] : cap; }
+};
+
+__global__ void __launch_bounds__(256)
+compact_hits_kernel(int64_t n_active, int max_hits, const int32_t *__restrict__ pixel_id,
+                    const int32_t *__restrict__ slots, const int32_t *__restrict__ hits_per_pixel,
+                    const int32_t *__restrict__ hit_off, long long *counters, int64_t hit_capacity,
+                    int32_t *hit_pixel, int32_t *hit_tick, int32_t *hit_adc)
+{
+    const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= n_active) return;
+    const int cnt = hits_per_pixel[slot];
+    const int m = cnt < max_hits ? cnt : max_hits;
+    const int64_t base = counters[0] + hit_off[slot];
+    int dropped = 0;
+    for (int k = 0; k < m; ++k) {
+        const int64_t h = base + k;
+        if (h < hit_capacity) {
+            const int v = slots[slot * max_hits + k];
+            hit_pixel[h] = pixel_id[slot];
+            hit_tick[h] = v >> ADC_SHIFT;
+            hit_adc[h] = v & ((1 << ADC_SHIFT) - 1);
+        } else ++dropped;
+    }
+    if (cnt > max_hits) atomicAdd((unsigned long long *)&counters[2], 1ull);
+    if (cnt) atomicAdd((unsigned long long *)&counters[1], (unsigned long long)cnt);
+    if (dropped) atomicAdd((unsigned long long *)&counters[3], (unsigned long long)dropped);
+}
+
+__global__ void advance_hit_base_kernel(long long *counters, const long long *batch_total, int64_t hit_capacity)
+{
+    long long v = counters[0] + *batch_total;
+    counters[0] = v < hit_capacity ? v : hit_capacity;
+}
+
+// slot_scratch: int32[n_active * max_hits]; scan_scratch: int32[n_active] + one long long (aligned) after it
+int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
+                       int32_t *slot_scratch, int32_t *scan_scratch, int64_t, cudaStream_t st)
+{
+    const DevParams &p = sim->dp;
+    const int64_t na = wf->n_active;
+    if (na == 0) return LARTPC_OK;
+    electronics_kernel<<<div_up(na, 128), 128, 0, st>>>(p, seed, na, wf->pixel_id, wf->first_tick, wf->length,
+                                                       wf->offset, wf->samples, sim->disabled_mask, slot_scratch,
+                                                       out->hits_per_pixel, out->q_pixel);
+    int rc = sim_ensure_scan_tmp(sim, na);
+    if (rc) return rc;
+    long long *batch_total = sim->d_counters + CNT_COUNT - 1;
+    LARTPC_CUDA_TRY(lscan::exclusive_scan(na, HitCountF{out->hits_per_pixel, p.max_hits}, scan_scratch, false,
+                                          batch_total, sim->scan_tmp, st));
+    compact_hits_kernel<<<div_up(na, 256), 256, 0, st>>>(na, p.max_hits, wf->pixel_id, slot_scratch,
+                                                        out->hits_per_pixel, scan_scratch, (long long *)out->counters,
+                                                        out->hit_capacity, out->hit_pixel, out->hit_tick, out->hit_adc);
+    advance_hit_base_kernel<<<1, 1, 0, st>>>((long long *)out->counters, batch_total, out->hit_capacity);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}

@@ -1,0 +1,458 @@
+// S1 quench, S2 drift, S3 pixel mapping + tile plan: one thread per segment,
+// structure-of-arrays float32 inputs read with coalesced 128-bit loads where alignment allows.
+// These stages are HBM-bound; arithmetic per segment is a few dozen operations.
+#include "common.cuh"
+#include "scan.cuh"
+
+// -------------------------------------------------------------------------------------------------
+// S1  recombination, eqs. (3.1)/(3.2) P:L575-583.  float32 arithmetic.
+// -------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void quench_one(const DevParams &p, float dx, float dy, float dz, float dE,
+                                           float &dEdx, float &n_e)
+{
+    float L = sqrtf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+    if (!(L > 0.0f) || !(dE > 0.0f)) { dEdx = 0.0f; n_e = 0.0f; return; }
+    float q = dE / L;
+    float R;
+    if (p.recomb_model == 0) {
+        R = (float)p.birks_ab / (1.0f + (float)(p.birks_kb / p.eps) * q);           // eq. (3.1)
+    } else {
+        float xi = (float)(p.box_beta / p.eps) * q;
+        R = fmaxf(logf((float)p.box_alpha + xi) / xi, 0.0f);                          // eq. (3.2), D6
+    }
+    dEdx = q;
+    n_e = R * (dE * (float)(1.0 / p.w_ion));
+}
+
+template <int VEC>
+__global__ void __launch_bounds__(256) quench_kernel(DevParams p, SegPtrs s, int64_t n, float *dEdx, float *n_e)
+{
+    int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * VEC;
+    if (i >= n) return;
+    if (VEC == 4 && i + 3 < n) {
+        float4 xs = *(const float4 *)(s.xs + i), ys = *(const float4 *)(s.ys + i), zs = *(const float4 *)(s.zs + i);
+        float4 xe = *(const float4 *)(s.xe + i), ye = *(const float4 *)(s.ye + i), ze = *(const float4 *)(s.ze + i);
+        float4 de = *(const float4 *)(s.dE + i);
+        float4 o1, o2;
+        quench_one(p, xe.x - xs.x, ye.x - ys.x, ze.x - zs.x, de.x, o1.x, o2.x);
+        quench_one(p, xe.y - xs.y, ye.y - ys.y, ze.y - zs.y, de.y, o1.y, o2.y);
+        quench_one(p, xe.z - xs.z, ye.z - ys.z, ze.z - zs.z, de.z, o1.z, o2.z);
+        quench_one(p, xe.w - xs.w, ye.w - ys.w, ze.w - zs.w, de.w, o1.w, o2.w);
+        *(float4 *)(dEdx + i) = o1;
+        *(float4 *)(n_e + i) = o2;
+    } else {
+        for (int k = 0; k < VEC && i + k < n; ++k) {
+            int64_t j = i + k;
+            quench_one(p, s.xe[j] - s.xs[j], s.ye[j] - s.ys[j], s.ze[j] - s.zs[j], s.dE[j], dEdx[j], n_e[j]);
+        }
+    }
+}
+
+static bool aligned16(const void *p) { return ((uintptr_t)p & 15u) == 0; }
+
+int launch_quench(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, float *dEdx, float *n_e, cudaStream_t st)
+{
+    if (n == 0) return LARTPC_OK;
+    SegPtrs s{seg->xs, seg->ys, seg->zs, seg->ts, seg->xe, seg->ye, seg->ze, seg->te, seg->dE};
+    bool vec = aligned16(s.xs) && aligned16(s.ys) && aligned16(s.zs) && aligned16(s.xe) && aligned16(s.ye) &&
+               aligned16(s.ze) && aligned16(s.dE) && aligned16(dEdx) && aligned16(n_e);
+    if (vec)
+        quench_kernel<4><<<div_up(div_up(n, 4), 256), 256, 0, st>>>(sim->dp, s, n, dEdx, n_e);
+    else
+        quench_kernel<1><<<div_up(n, 256), 256, 0, st>>>(sim->dp, s, n, dEdx, n_e);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}
+
+// -------------------------------------------------------------------------------------------------
+// S2  transport, eqs. (3.3)-(3.5) P:L599-616.  The index path (TPC, distances, times, sigma) is float64
+// with individually rounded operations in the order DESIGN.md fixes, because S3 turns them into integers.
+// -------------------------------------------------------------------------------------------------
+struct DriftCore {
+    int tpc;
+    double t_mid, sigma_T, sigma_t, u_s, v_s, u_e, v_e, T_s, T_e;
+};
+
+__device__ __forceinline__ int find_tpc(const DevParams &p, const DevTpc *__restrict__ tpcs, double xm, double ym,
+                                        double zm)
+{
+    for (int k = 0; k < p.n_tpcs; ++k) {
+        const DevTpc &t = tpcs[k];
+        double dm = xmul((double)t.sign, xsub(zm, t.z_anode));
+        if (xm >= t.x0 && xm < t.x1 && ym >= t.y0 && ym < t.y1 && dm >= 0.0 && dm <= t.drift_len) return k;
+    }
+    return -1;
+}
+
+__device__ __forceinline__ void drift_core(const DevParams &p, const DevTpc *__restrict__ tpcs, int tpc,
+                                           float xs, float ys, float zs, float ts, float xe, float ye, float ze,
+                                           float te, DriftCore &o)
+{
+    const DevTpc &t = tpcs[tpc];
+    double zm = xmul(0.5, xadd((double)zs, (double)ze));
+    o.tpc = tpc;
+    o.t_mid = xdiv(drift_dist(t, zm), p.v_drift);
+    o.sigma_T = xsqrt(xmul(xmul(2.0, p.d_tran), o.t_mid));
+    double sigma_L = xsqrt(xmul(xmul(2.0, p.d_long), o.t_mid));
+    o.sigma_t = xdiv(sigma_L, p.v_drift);
+    o.u_s = xsub((double)xs, t.x0);  o.v_s = xsub((double)ys, t.y0);
+    o.u_e = xsub((double)xe, t.x0);  o.v_e = xsub((double)ye, t.y0);
+    o.T_s = xadd((double)ts, xdiv(drift_dist(t, (double)zs), p.v_drift));
+    o.T_e = xadd((double)te, xdiv(drift_dist(t, (double)ze), p.v_drift));
+}
+
+__global__ void __launch_bounds__(256) drift_kernel(DevParams p, const DevTpc *__restrict__ tpcs, SegPtrs s,
+                                                    int64_t n, const float *__restrict__ n_e, lartpc_drifted_t o)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float xs = s.xs[i], ys = s.ys[i], zs = s.zs[i], ts = s.ts[i];
+    float xe = s.xe[i], ye = s.ye[i], ze = s.ze[i], te = s.te[i];
+    double xm = xmul(0.5, xadd((double)xs, (double)xe));
+    double ym = xmul(0.5, xadd((double)ys, (double)ye));
+    double zm = xmul(0.5, xadd((double)zs, (double)ze));
+    int tpc = find_tpc(p, tpcs, xm, ym, zm);
+    o.tpc[i] = tpc;
+    if (tpc < 0) {
+        o.q_anode[i] = 0.0f; o.sigma_T[i] = 0.0f; o.sigma_t[i] = 0.0f;
+        o.u_s[i] = o.v_s[i] = o.u_e[i] = o.v_e[i] = o.T_s[i] = o.T_e[i] = 0.0;
+        return;
+    }
+    DriftCore c;
+    drift_core(p, tpcs, tpc, xs, ys, zs, ts, xe, ye, ze, te, c);
+    o.q_anode[i] = (float)((double)n_e[i] * exp(-c.t_mid / p.lifetime));              // eq. (3.4)
+    o.sigma_T[i] = (float)c.sigma_T;                                                   // eq. (3.5)
+    o.sigma_t[i] = (float)c.sigma_t;
+    o.u_s[i] = c.u_s; o.v_s[i] = c.v_s; o.u_e[i] = c.u_e; o.v_e[i] = c.v_e;
+    o.T_s[i] = c.T_s; o.T_e[i] = c.T_e;
+}
+
+int launch_drift(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, const float *n_e, lartpc_drifted_t *out,
+                 cudaStream_t st)
+{
+    if (n == 0) return LARTPC_OK;
+    SegPtrs s{seg->xs, seg->ys, seg->zs, seg->ts, seg->xe, seg->ye, seg->ze, seg->te, seg->dE};
+    drift_kernel<<<div_up(n, 256), 256, 0, st>>>(sim->dp, sim->d_tpcs, s, n, n_e, *out);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}
+
+// -------------------------------------------------------------------------------------------------
+// S3  pixel mapping (reading D10) and the tile plan S4 runs on.
+// -------------------------------------------------------------------------------------------------
+struct SegBox {
+    int a_lo, a_hi, b_lo, b_hi, ix0, ix1, iy0, iy1, jt0, jt1, npix, n_samples;
+    int cpx0, cpx1, cpy0, cpy1, c0, c1;          // charged pixels (clamped to the +-H margin), chunk range
+    bool deposits;
+};
+
+__device__ __forceinline__ void chunk_and_cp_range(const DevParams &p, const DevTpc &t, SegBox &b)
+{
+    long long x0 = floor_div_ll(b.a_lo, p.nb), x1 = floor_div_ll(b.a_hi, p.nb);
+    long long y0 = floor_div_ll(b.b_lo, p.nb), y1 = floor_div_ll(b.b_hi, p.nb);
+    b.cpx0 = (int)max(x0, (long long)-p.H);  b.cpx1 = (int)min(x1, (long long)(t.nx - 1 + p.H));
+    b.cpy0 = (int)max(y0, (long long)-p.H);  b.cpy1 = (int)min(y1, (long long)(t.ny - 1 + p.H));
+    int j0 = max(b.jt0, 0), j1 = min(b.jt1, p.j_max);      // charge outside the readout window is dropped (D23)
+    b.c0 = j0 / p.Jc;  b.c1 = j1 / p.Jc;
+    b.deposits = b.npix > 0 && j0 <= j1 && b.cpx0 <= b.cpx1 && b.cpy0 <= b.cpy1;
+}
+
+__device__ __forceinline__ void seg_box(const DevParams &p, const DevTpc *__restrict__ tpcs, int tpc, float q_anode,
+                                        float xs, float ys, float zs, float ts, float xe, float ye, float ze, float te,
+                                        SegBox &b)
+{
+    double dx = xsub((double)xe, (double)xs), dy = xsub((double)ye, (double)ys), dz = xsub((double)ze, (double)zs);
+    double L = xsqrt(xadd(xadd(xmul(dx, dx), xmul(dy, dy)), xmul(dz, dz)));
+    long long N = (long long)ceil(xdiv(L, p.sample_step));
+    b.n_samples = (int)(N < 1 ? 1 : N);
+    b.deposits = false;
+    if (tpc < 0 || !(q_anode > 0.0f)) {
+        b.a_lo = b.b_lo = 0; b.a_hi = b.b_hi = -1; b.ix0 = b.iy0 = 0; b.ix1 = b.iy1 = -1; b.jt0 = 0; b.jt1 = -1;
+        b.npix = 0;
+        return;
+    }
+    DriftCore c;
+    drift_core(p, tpcs, tpc, xs, ys, zs, ts, xe, ye, ze, te, c);
+    const DevTpc &t = tpcs[tpc];
+    double r = xmul(p.n_sigma_map, c.sigma_T);
+    double umin = fmin(c.u_s, c.u_e), umax = fmax(c.u_s, c.u_e), vmin = fmin(c.v_s, c.v_e), vmax = fmax(c.v_s, c.v_e);
+    long long al = (long long)floor(xdiv(xsub(umin, r), p.bin)), ah = (long long)floor(xdiv(xadd(umax, r), p.bin));
+    long long bl = (long long)floor(xdiv(xsub(vmin, r), p.bin)), bh = (long long)floor(xdiv(xadd(vmax, r), p.bin));
+    b.a_lo = (int)al; b.a_hi = (int)ah; b.b_lo = (int)bl; b.b_hi = (int)bh;
+    long long x0 = floor_div_ll(al, p.nb) - p.H, x1 = floor_div_ll(ah, p.nb) + p.H;
+    long long y0 = floor_div_ll(bl, p.nb) - p.H, y1 = floor_div_ll(bh, p.nb) + p.H;
+    if (x0 < 0) x0 = 0;
+    if (y0 < 0) y0 = 0;
+    if (x1 > t.nx - 1) x1 = t.nx - 1;
+    if (y1 > t.ny - 1) y1 = t.ny - 1;
+    b.ix0 = (int)x0; b.ix1 = (int)x1; b.iy0 = (int)y0; b.iy1 = (int)y1;
+    b.npix = (x0 <= x1 && y0 <= y1) ? (int)((x1 - x0 + 1) * (y1 - y0 + 1)) : 0;
+    double rt = xmul(p.n_sigma_map, c.sigma_t);
+    double tmin = fmin(c.T_s, c.T_e), tmax = fmax(c.T_s, c.T_e);
+    b.jt0 = (int)floor(xdiv(xsub(xsub(tmin, rt), p.t_origin), p.dt));
+    b.jt1 = (int)floor(xdiv(xsub(xadd(tmax, rt), p.t_origin), p.dt));
+    chunk_and_cp_range(p, t, b);
+}
+
+__device__ __forceinline__ long long warp_max_ll(long long v)
+{
+    for (int d = 16; d; d >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, d));
+    return v;
+}
+__device__ __forceinline__ long long warp_sum_ll(long long v)
+{
+    for (int d = 16; d; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
+__global__ void __launch_bounds__(256)
+pixmap_kernel(DevParams p, const DevTpc *__restrict__ tpcs, SegPtrs s, int64_t n, const int32_t *__restrict__ seg_tpc,
+              const float *__restrict__ q_anode, int tpc_lo, int tpc_hi, lartpc_pixmap_t o,
+              int32_t *pix_count, unsigned long long *pix_mask, long long *counters)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    long long m_npix = 0, m_ticks = 0, n_act = 0, n_pairs = 0;
+    if (i < n) {
+        int tpc = seg_tpc[i];
+        SegBox b;
+        seg_box(p, tpcs, tpc, q_anode[i], s.xs[i], s.ys[i], s.zs[i], s.ts[i], s.xe[i], s.ye[i], s.ze[i], s.te[i], b);
+        o.a_lo[i] = b.a_lo; o.a_hi[i] = b.a_hi; o.b_lo[i] = b.b_lo; o.b_hi[i] = b.b_hi;
+        o.ix0[i] = b.ix0; o.ix1[i] = b.ix1; o.iy0[i] = b.iy0; o.iy1[i] = b.iy1;
+        o.jt0[i] = b.jt0; o.jt1[i] = b.jt1; o.npix[i] = b.npix; o.n_samples[i] = b.n_samples;
+        if (b.npix > 0) {
+            m_npix = b.npix;
+            m_ticks = (long long)(b.jt1 - b.jt0 + 1) + p.K - 1;
+            n_act = 1;
+        }
+        if (b.deposits && tpc >= tpc_lo && tpc < tpc_hi) {
+            const DevTpc &t = tpcs[tpc];
+            unsigned long long mask = (b.c1 >= 63 ? ~0ull : ((1ull << (b.c1 + 1)) - 1ull)) & ~((1ull << b.c0) - 1ull);
+            for (int cy = b.cpy0; cy <= b.cpy1; ++cy)
+                for (int cx = b.cpx0; cx <= b.cpx1; ++cx) {
+                    int cp = t.cp_base + (cy + p.H) * t.gw + (cx + p.H);
+                    atomicAdd(&pix_count[cp], 1);
+                    atomicOr(&pix_mask[cp], mask);
+                    ++n_pairs;
+                }
+        }
+    }
+    m_npix = warp_max_ll(m_npix); m_ticks = warp_max_ll(m_ticks);
+    n_act = warp_sum_ll(n_act); n_pairs = warp_sum_ll(n_pairs);
+    if ((threadIdx.x & 31) == 0) {
+        if (m_npix) atomicMax(&counters[CNT_MAX_NPIX], m_npix);
+        if (m_ticks) atomicMax(&counters[CNT_MAX_TICKS], m_ticks);
+        if (n_act) atomicAdd((unsigned long long *)&counters[CNT_ACTIVE_SEGS], (unsigned long long)n_act);
+        if (n_pairs) atomicAdd((unsigned long long *)&counters[CNT_PAIRS], (unsigned long long)n_pairs);
+    }
+}
+
+// second pass over the segments: write the (segment, charged pixel) incidence lists
+__global__ void __launch_bounds__(256)
+pair_fill_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n, const int32_t *__restrict__ seg_tpc,
+                 lartpc_pixmap_t o, int tpc_lo, int tpc_hi, const int32_t *__restrict__ pix_start, int32_t *pix_cursor,
+                 int32_t *pair_seg, int64_t pair_cap, long long *counters)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int tpc = seg_tpc[i];
+    if (tpc < tpc_lo || tpc >= tpc_hi) return;
+    SegBox b;
+    b.a_lo = o.a_lo[i]; b.a_hi = o.a_hi[i]; b.b_lo = o.b_lo[i]; b.b_hi = o.b_hi[i];
+    b.jt0 = o.jt0[i]; b.jt1 = o.jt1[i]; b.npix = o.npix[i];
+    if (b.npix <= 0) return;
+    const DevTpc &t = tpcs[tpc];
+    chunk_and_cp_range(p, t, b);
+    if (!b.deposits) return;
+    for (int cy = b.cpy0; cy <= b.cpy1; ++cy)
+        for (int cx = b.cpx0; cx <= b.cpx1; ++cx) {
+            int cp = t.cp_base + (cy + p.H) * t.gw + (cx + p.H);
+            int64_t slot = (int64_t)pix_start[cp] + atomicAdd(&pix_cursor[cp], 1);
+            if (slot < pair_cap) pair_seg[slot] = (int32_t)i;
+            else atomicAdd((unsigned long long *)&counters[CNT_OVERFLOW], 1ull);
+        }
+}
+
+// the atomics above fill each list in arbitrary order; sort it by segment id so that the float32
+// accumulation order of S4 (and hence every output bit) is reproducible from run to run
+__global__ void __launch_bounds__(128)
+pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int32_t *__restrict__ pix_count,
+                 int32_t *pair_seg, int64_t pair_cap)
+{
+    int64_t cp = (int64_t)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5);
+    if (cp >= n_cp) return;
+    int cnt = pix_count[cp];
+    if (cnt < 2) return;
+    int lane = threadIdx.x & 31;
+    int64_t base = pix_start[cp];
+    if (base + cnt > pair_cap) return;
+    int32_t *v = pair_seg + base;
+    // odd-even transposition sort by one warp (lists hold tens of entries; long ones take cnt passes)
+    for (int pass = 0; pass < cnt; ++pass) {
+        for (int k = (pass & 1) + 2 * lane; k + 1 < cnt; k += 64) {
+            int32_t a = v[k], b = v[k + 1];
+            if (a > b) { v[k] = b; v[k + 1] = a; }
+        }
+        __syncwarp();
+    }
+}
+
+// one thread per charged-pixel grid cell: emit its tiles and mark the pixels they can reach
+__global__ void __launch_bounds__(256)
+tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n_cp, const int32_t *__restrict__ pix_tile0,
+                 const unsigned long long *__restrict__ pix_mask, int32_t *tile_cp, TileDesc *tile_desc,
+                 int64_t tile_cap, int32_t *act_first, int32_t *act_last, long long *counters)
+{
+    int64_t cp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cp >= n_cp) return;
+    unsigned long long mask = pix_mask[cp];
+    if (!mask) return;
+    int tpc = 0;
+    while (tpc + 1 < p.n_tpcs && tpcs[tpc + 1].cp_base <= cp) ++tpc;
+    const DevTpc &t = tpcs[tpc];
+    int rel = (int)(cp - t.cp_base);
+    int px = rel % t.gw - p.H, py = rel / t.gw - p.H;
+    int64_t tix = pix_tile0[cp];
+    int c_lo = __ffsll((long long)mask) - 1, c_hi = 63 - __clzll((long long)mask);
+    for (unsigned long long m = mask; m; m &= m - 1) {
+        int c = __ffsll((long long)m) - 1;
+        if (tix < tile_cap) { tile_cp[tix] = (int32_t)cp; tile_desc[tix] = TileDesc{tpc, px, py, c}; }
+        else atomicAdd((unsigned long long *)&counters[CNT_OVERFLOW], 1ull);
+        ++tix;
+    }
+    int first = c_lo * p.Jc;
+    int last = min(c_hi * p.Jc + p.Jc + p.K - 2, p.n_ticks - 1);
+    for (int iy = max(py - p.H, 0); iy <= min(py + p.H, t.ny - 1); ++iy)
+        for (int ix = max(px - p.H, 0); ix <= min(px + p.H, t.nx - 1); ++ix) {
+            int gp = t.first_pixel_id + iy * t.nx + ix;
+            atomicMin(&act_first[gp], first);
+            atomicMax(&act_last[gp], last);
+        }
+}
+
+struct NpixF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
+struct PopcF { const unsigned long long *m; __device__ long long operator()(int64_t i) const { return __popcll(m[i]); } };
+struct ActiveF { const int32_t *last; __device__ long long operator()(int64_t i) const { return last[i] >= 0 ? 1 : 0; } };
+struct ActiveLenF {
+    const int32_t *first, *last;
+    __device__ long long operator()(int64_t i) const { return last[i] >= 0 ? (long long)(last[i] - first[i] + 1) : 0; }
+};
+
+__global__ void fill_i32_kernel(int32_t *p, int64_t n, int32_t v)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+
+int sim_ensure_scan_tmp(lartpc_sim *sim, int64_t elems)
+{
+    int64_t need = lscan::tmp_elems(elems);
+    if (need > sim->scan_tmp_elems) {
+        if (sim->scan_tmp) cudaFree(sim->scan_tmp);
+        sim->scan_tmp = nullptr;
+        LARTPC_CUDA_TRY(cudaMalloc(&sim->scan_tmp, sizeof(long long) * need));
+        sim->scan_tmp_elems = need;
+    }
+    return LARTPC_OK;
+}
+
+static int grow_i32(int32_t **p, int64_t *cap, int64_t need)
+{
+    if (need <= *cap) return LARTPC_OK;
+    if (*p) cudaFree(*p);
+    *p = nullptr;
+    int64_t c = need + need / 4 + 1024;
+    LARTPC_CUDA_TRY(cudaMalloc(p, sizeof(int32_t) * c));
+    *cap = c;
+    return LARTPC_OK;
+}
+
+// S3 launcher.  Segments whose TPC lies outside [tpc_lo, tpc_hi) get their rectangles but no tiles
+// (lartpc_run_spill plans one TPC batch at a time; the staged API passes the full range).
+int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drifted_t *dr, int64_t n,
+                int tpc_lo, int tpc_hi, lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, cudaStream_t st)
+{
+    const DevParams &p = sim->dp;
+    SegPtrs s{seg->xs, seg->ys, seg->zs, seg->ts, seg->xe, seg->ye, seg->ze, seg->te, seg->dE};
+    int rc;
+    if ((rc = sim_ensure_scan_tmp(sim, sim->n_cp > n ? sim->n_cp : (n > sim->n_pix ? n : sim->n_pix))) != 0) return rc;
+    sim->have_plan = false;
+    sim->have_signals = false;
+
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_counters, 0, sizeof(long long) * CNT_COUNT, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_count, 0, sizeof(int32_t) * sim->n_cp, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_cursor, 0, sizeof(int32_t) * sim->n_cp, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_mask, 0, sizeof(unsigned long long) * sim->n_cp, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->act_last, 0xff, sizeof(int32_t) * sim->n_pix, st));
+        fill_i32_kernel<<<div_up(sim->n_pix, 256), 256, 0, st>>>(sim->act_first, sim->n_pix, INT32_MAX);
+        if (n > 0) {
+            pixmap_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, s, n, dr->tpc, dr->q_anode, tpc_lo, tpc_hi,
+                                                         *out, sim->pix_count, sim->pix_mask, sim->d_counters);
+            LARTPC_CUDA_TRY(cudaGetLastError());
+        }
+        // offsets[n+1] = exclusive scan of npix
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(n, NpixF{out->npix}, out->offsets, true,
+                                              sim->d_counters + CNT_TOTAL_NPIX, sim->scan_tmp, st));
+        // per charged pixel: start of its segment list, index of its first tile
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_cp, NpixF{sim->pix_count}, sim->pix_start, false,
+                                              (long long *)nullptr, sim->scan_tmp, st));
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_cp, PopcF{sim->pix_mask}, sim->pix_tile0, false,
+                                              sim->d_counters + CNT_TILES, sim->scan_tmp, st));
+        if (n > 0) {
+            pair_fill_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, n, dr->tpc, *out, tpc_lo, tpc_hi,
+                                                            sim->pix_start, sim->pix_cursor, sim->pair_seg,
+                                                            sim->pair_cap, sim->d_counters);
+            pair_sort_kernel<<<div_up(sim->n_cp, 4), 128, 0, st>>>(sim->n_cp, sim->pix_start, sim->pix_count,
+                                                                  sim->pair_seg, sim->pair_cap);
+        }
+        tile_emit_kernel<<<div_up(sim->n_cp, 256), 256, 0, st>>>(p, sim->d_tpcs, sim->n_cp, sim->pix_tile0,
+                                                                sim->pix_mask, sim->tile_cp, sim->tile_desc,
+                                                                sim->tile_cap, sim->act_first, sim->act_last,
+                                                                sim->d_counters);
+        LARTPC_CUDA_TRY(cudaGetLastError());
+        // active pixels: slot = rank among active pixels (sorted by id), total waveform samples
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_pix, ActiveF{sim->act_last}, sim->act_slot, false,
+                                              sim->d_counters + CNT_ACTIVE_PIX, sim->scan_tmp, st));
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_pix, ActiveLenF{sim->act_first, sim->act_last},
+                                              (long long *)nullptr, false, sim->d_counters + CNT_TOTAL_SAMPLES,
+                                              sim->scan_tmp, st));
+        LARTPC_CUDA_TRY(cudaMemcpyAsync(sim->h_counters, sim->d_counters, sizeof(long long) * CNT_COUNT,
+                                        cudaMemcpyDeviceToHost, st));
+        LARTPC_CUDA_TRY(cudaStreamSynchronize(st));
+        const long long *h = sim->h_counters;
+        if (h[CNT_OVERFLOW] == 0) break;
+        if (attempt == 1) return LARTPC_ERR_CAPACITY;
+        // grow the plan buffers to the sizes just counted and plan again
+        if ((rc = grow_i32(&sim->pair_seg, &sim->pair_cap, h[CNT_PAIRS])) != 0) return rc;
+        if (h[CNT_TILES] > sim->tile_cap) {
+            int64_t cap = sim->tile_cap;
+            if ((rc = grow_i32(&sim->tile_cp, &cap, h[CNT_TILES])) != 0) return rc;
+            if (sim->tile_desc) cudaFree(sim->tile_desc);
+            sim->tile_desc = nullptr;
+            LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc, sizeof(TileDesc) * cap));
+            sim->tile_cap = cap;
+        }
+    }
+    const long long *h = sim->h_counters;
+    sim->plan_n = n;
+    sim->n_tiles = h[CNT_TILES];
+    sim->n_pairs = h[CNT_PAIRS];
+    sim->n_active = h[CNT_ACTIVE_PIX];
+    sim->total_samples = h[CNT_TOTAL_SAMPLES];
+    sim->drifted_copy = *dr;
+    sim->pixmap_copy = *out;
+    sim->have_plan = true;
+    if (info) {
+        info->max_npix = (int32_t)h[CNT_MAX_NPIX];
+        info->max_ticks = (int32_t)h[CNT_MAX_TICKS];
+        info->total_npix = h[CNT_TOTAL_NPIX];
+        info->n_active_segments = h[CNT_ACTIVE_SEGS];
+        info->n_tiles = h[CNT_TILES];
+        info->n_pairs = h[CNT_PAIRS];
+        info->n_active_pixels = h[CNT_ACTIVE_PIX];
+        info->total_samples = h[CNT_TOTAL_SAMPLES];
+        info->tile_targets = p.WW;
+        info->tile_ticks = p.tile_ticks;
+    }
+    return LARTPC_OK;
+}

@@ -1,0 +1,339 @@
+"""Thin Python binding of the C-ABI library ``liblartpc.so`` (include/lartpc.h).
+
+Argument marshalling only: every step of the path runs in the library's sm_100a kernels.
+PyTorch supplies device memory (``torch.empty(..., device="cuda")``) and the CUDA stream.
+There is no CPU fallback: importing works anywhere, but creating a :class:`Sim` raises if the
+library is missing or the device is not a compute-capability 10.x GPU.
+
+Function names follow the C entry points: ``quench`` -> ``lartpc_quench`` (eqs. 3.1/3.2 of
+arXiv 2212.09807), ``drift`` (eqs. 3.3-3.5), ``pixels_from_segments``,
+``induced_current`` (eq. 3.9), ``sum_pixel_signals``, ``electronics``,
+``run_spill``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblartpc.so")
+_lib = None
+
+SEG_FIELDS = ("xs", "ys", "zs", "ts", "xe", "ye", "ze", "te", "dE")
+
+
+class LartpcError(RuntimeError):
+    pass
+
+
+class Params(C.Structure):
+    _fields_ = [
+        ("e_field_kv_cm", C.c_double), ("lar_density_g_cm3", C.c_double), ("w_ion_mev", C.c_double),
+        ("recomb_model", C.c_int),
+        ("birks_ab", C.c_double), ("birks_kb", C.c_double), ("box_alpha", C.c_double), ("box_beta", C.c_double),
+        ("v_drift_cm_us", C.c_double), ("lifetime_us", C.c_double),
+        ("d_long_cm2_us", C.c_double), ("d_tran_cm2_us", C.c_double),
+        ("tick_us", C.c_double), ("t_origin_us", C.c_double),
+        ("pixel_pitch_cm", C.c_double),
+        ("bins_per_pixel", C.c_int), ("window_pixels", C.c_int), ("lut_ticks", C.c_int),
+        ("n_readout_ticks", C.c_int),
+        ("sample_step_cm", C.c_double), ("n_sigma_map", C.c_double),
+        ("gain_mv_per_ke", C.c_double), ("v_cm_mv", C.c_double), ("v_ref_mv", C.c_double),
+        ("v_pedestal_mv", C.c_double),
+        ("adc_bits", C.c_int),
+        ("threshold_e", C.c_double),
+        ("hold_ticks", C.c_int), ("min_spacing_ticks", C.c_int), ("periodic_reset_ticks", C.c_int),
+        ("noise_reset_e", C.c_double), ("noise_disc_e", C.c_double), ("noise_uncorr_e", C.c_double),
+        ("max_hits_per_pixel", C.c_int),
+    ]
+
+
+class Tpc(C.Structure):
+    _fields_ = [("x0", C.c_double), ("y0", C.c_double), ("z_anode", C.c_double), ("drift_sign", C.c_int),
+                ("drift_len", C.c_double), ("nx", C.c_int), ("ny", C.c_int), ("first_pixel_id", C.c_int)]
+
+
+_P = C.c_void_p
+
+
+class Segments(C.Structure):
+    _fields_ = [(k, _P) for k in SEG_FIELDS]
+
+
+class Drifted(C.Structure):
+    _fields_ = [(k, _P) for k in ("tpc", "q_anode", "sigma_T", "sigma_t", "u_s", "v_s", "u_e", "v_e", "T_s", "T_e")]
+
+
+_PIX_I32 = ("a_lo", "a_hi", "b_lo", "b_hi", "ix0", "ix1", "iy0", "iy1", "jt0", "jt1", "npix", "n_samples")
+
+
+class Pixmap(C.Structure):
+    _fields_ = [(k, _P) for k in _PIX_I32 + ("offsets",)]
+
+
+class PixmapInfo(C.Structure):
+    _fields_ = [("max_npix", C.c_int32), ("max_ticks", C.c_int32), ("total_npix", C.c_int64),
+                ("n_active_segments", C.c_int64), ("n_tiles", C.c_int64), ("n_pairs", C.c_int64),
+                ("n_active_pixels", C.c_int64), ("total_samples", C.c_int64),
+                ("tile_targets", C.c_int32), ("tile_ticks", C.c_int32)]
+
+
+class Signals(C.Structure):
+    _fields_ = [("tile_capacity", C.c_int64), ("partial", _P), ("tile_range", _P)]
+
+
+class Waveforms(C.Structure):
+    _fields_ = [("pixel_capacity", C.c_int64), ("sample_capacity", C.c_int64), ("pixel_id", _P),
+                ("first_tick", _P), ("length", _P), ("offset", _P), ("samples", _P),
+                ("n_active", C.c_int64), ("total_samples", C.c_int64)]
+
+
+class Hits(C.Structure):
+    _fields_ = [("hit_capacity", C.c_int64), ("hit_pixel", _P), ("hit_tick", _P), ("hit_adc", _P),
+                ("hits_per_pixel", _P), ("q_pixel", _P), ("counters", _P)]
+
+
+class Stats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("n_segments", "n_active_segments", "n_tiles", "n_pairs", "n_active_pixels",
+                                        "total_samples", "n_hits", "n_hits_total", "n_pixels_overflow",
+                                        "n_hits_dropped")] + \
+               [("n_batches", C.c_int32), ("reserved", C.c_int32), ("flops_current", C.c_double)]
+
+
+EXPORTS = ("lartpc_sim_create", "lartpc_sim_destroy", "lartpc_set_disabled_pixels", "lartpc_chunk_ticks",
+           "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
+           "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_run_spill",
+           "lartpc_measure_fp32_peak", "lartpc_strerror")
+
+
+def load_library():
+    """dlopen liblartpc.so; raises LartpcError when it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise LartpcError("liblartpc.so is not built: run `python -m paper_2212_09807_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        lib = C.CDLL(LIB_PATH)
+        lib.lartpc_strerror.restype = C.c_char_p
+        lib.lartpc_workspace_bytes.restype = C.c_size_t
+        lib.lartpc_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
+        lib.lartpc_sim_destroy.restype = None
+        lib.lartpc_sim_destroy.argtypes = [C.c_void_p]
+        for name in EXPORTS:
+            getattr(lib, name)
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise LartpcError("%s failed: %s (%d)" % (what, load_library().lartpc_strerror(rc).decode(), rc))
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise LartpcError("no CUDA device: the LArTPC path runs only on an sm_100a GPU (no CPU fallback)")
+    return torch
+
+
+def _stream_ptr(torch):
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def measure_fp32_peak(variant: int = 0) -> float:
+    """FP32 FMA rate in TFLOP/s from the library's FFMA-chain microbenchmark (0 scalar, 1 packed FFMA2)."""
+    torch = _torch()
+    out = C.c_double(0.0)
+    _check(load_library().lartpc_measure_fp32_peak(C.c_int(variant), C.byref(out), _stream_ptr(torch)),
+           "lartpc_measure_fp32_peak")
+    return float(out.value)
+
+
+class Sim:
+    """Owns a ``lartpc_sim_t`` (detector / physics parameters, TPC table, response LUT)."""
+
+    def __init__(self, params: Dict, tpcs: Sequence[dict], lut: np.ndarray, device: str = "cuda:0"):
+        torch = _torch()
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.lib = load_library()
+        self.params = dict(params)
+        self.tpcs = list(tpcs)
+        p = Params()
+        for name, _ in Params._fields_:
+            setattr(p, name, params[name])
+        arr = (Tpc * len(tpcs))()
+        for i, t in enumerate(tpcs):
+            arr[i] = Tpc(t["x0"], t["y0"], t["z_anode"], t["drift_sign"], t["drift_len"], t["nx"], t["ny"],
+                         t["first_pixel_id"])
+        lut = np.ascontiguousarray(lut, dtype=np.float32)
+        h = C.c_void_p()
+        _check(self.lib.lartpc_sim_create(C.byref(p), arr, C.c_int(len(tpcs)),
+                                          lut.ctypes.data_as(C.c_void_p), C.c_size_t(lut.size), C.byref(h)),
+               "lartpc_sim_create")
+        self.handle = h
+        self.chunk_ticks = int(self.lib.lartpc_chunk_ticks(self.handle))
+        self.info: Optional[PixmapInfo] = None
+        self._keep = {}
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.lartpc_sim_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers ------------------------------------------------------------------------------------
+    def _empty(self, n, dtype):
+        return self.torch.empty(int(max(n, 0)), dtype=dtype, device=self.device)
+
+    def upload_segments(self, seg: Dict[str, np.ndarray]):
+        """Host SoA arrays -> device tensors (one float32 tensor per field)."""
+        t = self.torch
+        return {k: t.from_numpy(np.ascontiguousarray(seg[k], dtype=np.float32)).to(self.device) for k in SEG_FIELDS}
+
+    def _seg_struct(self, seg):
+        s = Segments()
+        n = None
+        for k in SEG_FIELDS:
+            v = seg[k]
+            if v.dtype != self.torch.float32 or not v.is_cuda or not v.is_contiguous():
+                raise LartpcError("segment field %s must be a contiguous float32 CUDA tensor" % k)
+            n = v.numel() if n is None else n
+            if v.numel() != n:
+                raise LartpcError("segment fields differ in length")
+            setattr(s, k, v.data_ptr())
+        return s, int(n)
+
+    def set_disabled_pixels(self, ids: np.ndarray):
+        ids = np.ascontiguousarray(ids, dtype=np.int32)
+        _check(self.lib.lartpc_set_disabled_pixels(self.handle, ids.ctypes.data_as(C.c_void_p), C.c_int64(ids.size)),
+               "lartpc_set_disabled_pixels")
+
+    # -- stages -------------------------------------------------------------------------------------
+    def quench(self, seg):
+        """S1: returns (dEdx, n_e) float32 tensors."""
+        t = self.torch
+        s, n = self._seg_struct(seg)
+        dedx, ne = self._empty(n, t.float32), self._empty(n, t.float32)
+        _check(self.lib.lartpc_quench(self.handle, C.byref(s), C.c_int64(n), C.c_void_p(dedx.data_ptr()),
+                                      C.c_void_p(ne.data_ptr()), _stream_ptr(t)), "lartpc_quench")
+        return dedx, ne
+
+    def drift(self, seg, n_e):
+        """S2: returns a dict of tensors named like ``lartpc_drifted_t``."""
+        t = self.torch
+        s, n = self._seg_struct(seg)
+        out = dict(tpc=self._empty(n, t.int32), q_anode=self._empty(n, t.float32),
+                   sigma_T=self._empty(n, t.float32), sigma_t=self._empty(n, t.float32))
+        for k in ("u_s", "v_s", "u_e", "v_e", "T_s", "T_e"):
+            out[k] = self._empty(n, t.float64)
+        d = Drifted(**{k: v.data_ptr() for k, v in out.items()})
+        _check(self.lib.lartpc_drift(self.handle, C.byref(s), C.c_int64(n), C.c_void_p(n_e.data_ptr()), C.byref(d),
+                                     _stream_ptr(t)), "lartpc_drift")
+        out["_struct"] = d
+        return out
+
+    def pixels_from_segments(self, seg, drifted):
+        """S3: returns (pixmap dict, PixmapInfo).  Synchronises the stream once (sizes go to the host)."""
+        t = self.torch
+        s, n = self._seg_struct(seg)
+        out = {k: self._empty(n, t.int32) for k in _PIX_I32}
+        out["offsets"] = self._empty(n + 1, t.int64)
+        pm = Pixmap(**{k: v.data_ptr() for k, v in out.items()})
+        info = PixmapInfo()
+        _check(self.lib.lartpc_pixels_from_segments(self.handle, C.byref(s), C.byref(drifted["_struct"]),
+                                                    C.c_int64(n), C.byref(pm), C.byref(info), _stream_ptr(t)),
+               "lartpc_pixels_from_segments")
+        out["_struct"] = pm
+        out["_n"] = n
+        self.info = info
+        return out, info
+
+    def induced_current(self, drifted, pixmap):
+        """S4: returns the signals dict (tile partial waveforms)."""
+        t = self.torch
+        info = self.info
+        nt = int(info.n_tiles)
+        out = dict(partial=self._empty(nt * info.tile_targets * info.tile_ticks, t.float32),
+                   tile_range=self._empty(nt * 2, t.int32))
+        sig = Signals(nt, out["partial"].data_ptr(), out["tile_range"].data_ptr())
+        _check(self.lib.lartpc_induced_current(self.handle, C.byref(drifted["_struct"]), C.byref(pixmap["_struct"]),
+                                               C.c_int64(pixmap["_n"]), C.byref(sig), _stream_ptr(t)),
+               "lartpc_induced_current")
+        out["_struct"] = sig
+        return out
+
+    def sum_pixel_signals(self, signals):
+        """S5: returns the waveforms dict (pixel_id, first_tick, length, offset, samples)."""
+        t = self.torch
+        info = self.info
+        na, ns = int(info.n_active_pixels), int(info.total_samples)
+        out = dict(pixel_id=self._empty(na, t.int32), first_tick=self._empty(na, t.int32),
+                   length=self._empty(na, t.int32), offset=self._empty(na + 1, t.int64),
+                   samples=self._empty(ns, t.float32))
+        wf = Waveforms(na, ns, out["pixel_id"].data_ptr(), out["first_tick"].data_ptr(), out["length"].data_ptr(),
+                       out["offset"].data_ptr(), out["samples"].data_ptr(), 0, 0)
+        _check(self.lib.lartpc_sum_pixel_signals(self.handle, C.byref(signals["_struct"]), C.byref(wf),
+                                                 _stream_ptr(t)), "lartpc_sum_pixel_signals")
+        out["_struct"] = wf
+        return out
+
+    def _hits(self, capacity, n_active):
+        t = self.torch
+        out = dict(hit_pixel=self._empty(capacity, t.int32), hit_tick=self._empty(capacity, t.int32),
+                   hit_adc=self._empty(capacity, t.int32), counters=t.zeros(4, dtype=t.int64, device=self.device))
+        if n_active is not None:
+            out["hits_per_pixel"] = self._empty(n_active, t.int32)
+            out["q_pixel"] = self._empty(n_active, t.float32)
+        h = Hits(int(capacity), out["hit_pixel"].data_ptr(), out["hit_tick"].data_ptr(), out["hit_adc"].data_ptr(),
+                 out["hits_per_pixel"].data_ptr() if n_active is not None else None,
+                 out["q_pixel"].data_ptr() if n_active is not None else None, out["counters"].data_ptr())
+        return out, h
+
+    def electronics(self, waveforms, seed: int, hit_capacity: Optional[int] = None):
+        """S6: returns the hits dict; ``counters`` = [written, total, pixels over capacity, dropped]."""
+        t = self.torch
+        na = int(waveforms["_struct"].n_active)
+        cap = int(hit_capacity if hit_capacity is not None else na * self.params["max_hits_per_pixel"])
+        out, h = self._hits(cap, na)
+        _check(self.lib.lartpc_electronics(self.handle, C.byref(waveforms["_struct"]), C.c_uint64(seed), C.byref(h),
+                                           _stream_ptr(t)), "lartpc_electronics")
+        out["_struct"] = h
+        return out
+
+    def workspace_bytes(self, max_segments: int) -> int:
+        return int(self.lib.lartpc_workspace_bytes(self.handle, C.c_int64(max_segments)))
+
+    def run_spill(self, seg, seed: int, hit_capacity: int, workspace=None, hits=None):
+        """S7: whole path on device-resident segments.  Returns (hits dict, Stats).  Pass ``workspace``
+        (a uint8 CUDA tensor) and ``hits`` (from a previous call) to reuse buffers."""
+        t = self.torch
+        s, n = self._seg_struct(seg)
+        if workspace is None:
+            workspace = self._empty(self.workspace_bytes(n), t.uint8)
+        if hits is None:
+            out, h = self._hits(hit_capacity, None)
+            out["_struct"] = h
+        else:
+            out, h = hits, hits["_struct"]
+        st = Stats()
+        _check(self.lib.lartpc_run_spill(self.handle, C.byref(s), C.c_int64(n), C.c_uint64(seed), C.byref(h),
+                                         C.byref(st), C.c_void_p(workspace.data_ptr()),
+                                         C.c_size_t(workspace.numel()), _stream_ptr(t)), "lartpc_run_spill")
+        return out, st
+
+
+def hits_to_numpy(hits, n: Optional[int] = None):
+    """(pixel, tick, adc) int32 numpy arrays of the first ``n`` (default: counters[0]) hits."""
+    n = int(hits["counters"][0].item()) if n is None else n
+    return (hits["hit_pixel"][:n].cpu().numpy(), hits["hit_tick"][:n].cpu().numpy(), hits["hit_adc"][:n].cpu().numpy())

@@ -1,0 +1,198 @@
+"""Parity of the CUDA path (through the C-ABI) with the fp64 oracle, element by element, on seeded inputs.
+
+Tolerances are BASELINE.json north_star's: pixel mapping bit-exact; per-pixel integrated charge within
+relative 1e-4 (absolute 1 e-); >= 99.9 % of hits identical in (pixel, tick, adc), the rest off by <= 1 tick
+or 1 count.  Float32 stage outputs (S1, S2) are held to 2e-6 relative (a few float32 ulp).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2212_09807_b200 import workloads as W
+
+from gpu_helpers import compare_hits, dense_waves, run_staged
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lartpc():
+    from paper_2212_09807_b200 import lartpc as L
+    L.load_library()
+    return L
+
+
+def _oracle_stages(wl):
+    dedx, ne = oracle.quench(wl.params, wl.segments)
+    dr = oracle.drift(wl.params, wl.tpcs, wl.segments, ne)
+    pm = oracle.pixmap(wl.params, wl.tpcs, wl.segments, dr)
+    return dedx, ne, dr, pm
+
+
+def _check_segment_stages(res, wl):
+    dedx, ne, dr, pm = _oracle_stages(wl)
+    assert np.allclose(res["dEdx"], dedx, rtol=2e-6, atol=0)
+    assert np.allclose(res["n_e"], ne, rtol=2e-6, atol=1e-3)
+    g = res["drift"]
+    assert np.array_equal(g["tpc"], dr["tpc"])
+    assert np.allclose(g["q_anode"], dr["q_a"], rtol=2e-6, atol=1e-3)
+    assert np.allclose(g["sigma_T"], dr["sigma_T"], rtol=2e-7, atol=0)
+    assert np.allclose(g["sigma_t"], dr["sigma_t"], rtol=2e-7, atol=0)
+    for a, b in (("u_s", "u_s"), ("v_s", "v_s"), ("u_e", "u_e"), ("v_e", "v_e"), ("T_s", "T_s"), ("T_e", "T_e")):
+        assert np.array_equal(g[a], dr[b]), a                      # float64, same operations: bit-exact
+    gp = res["pixmap"]
+    for k in ("a_lo", "a_hi", "b_lo", "b_hi", "ix0", "ix1", "iy0", "iy1", "jt0", "jt1", "npix", "n_samples"):
+        assert np.array_equal(gp[k], pm[k]), k                     # pixel mapping: bit-exact
+    assert np.array_equal(gp["offsets"], pm["offsets"])
+    info = res["info"]
+    assert info.max_npix == pm["npix"].max()
+    assert info.total_npix == pm["offsets"][-1]
+    act = pm["npix"] > 0
+    assert info.n_active_segments == act.sum()
+    if act.any():
+        assert info.max_ticks == (pm["jt1"] - pm["jt0"] + 1)[act].max() + wl.params["lut_ticks"] - 1
+    return dr, pm
+
+
+def _check_currents(res, wl, dr, pm, max_pixels=None, seed=0):
+    """Waveforms and Q_p of (a sample of) the active pixels against O4/O5."""
+    nt = wl.params["n_readout_ticks"]
+    dense = dense_waves(res, nt)
+    gpu_ids = res["waveforms"]["pixel_id"][:res["n_active"]]
+    # active set = union of the O3 rectangles
+    ids = []
+    for ti, t in enumerate(wl.tpcs):
+        ix, iy = oracle.active_pixels(wl.tpcs, pm, dr, ti)
+        ids.append(t["first_pixel_id"] + iy.astype(np.int64) * t["nx"] + ix)
+    ids = np.concatenate(ids)
+    assert np.array_equal(np.sort(ids), gpu_ids)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    worst_q, worst_w = 0.0, 0.0
+    for ti, t in enumerate(wl.tpcs):
+        sel = np.nonzero((gpu_ids >= t["first_pixel_id"]) & (gpu_ids < t["first_pixel_id"] + t["nx"] * t["ny"]))[0]
+        if len(sel) == 0:
+            continue
+        if max_pixels is not None and len(sel) > max_pixels:
+            # the pixels carrying the most charge plus a random sample of the rest
+            q = np.abs(dense[sel]).sum(axis=1)
+            top = sel[np.argsort(q)[-max_pixels // 2:]]
+            rest = rng.choice(sel, size=max_pixels // 2, replace=False)
+            sel = np.unique(np.concatenate([top, rest]))
+        rel = gpu_ids[sel] - t["first_pixel_id"]
+        waves, qp = oracle.pixel_currents(wl.params, wl.tpcs, wl.lut, dr, pm, ti, rel % t["nx"], rel // t["nx"])
+        gq = dense[sel].sum(axis=1)
+        tol = np.maximum(1e-4 * np.abs(qp), 1.0)
+        assert np.all(np.abs(gq - qp) <= tol), (np.abs(gq - qp) / tol).max()
+        worst_q = max(worst_q, (np.abs(gq - qp) / tol).max())
+        # sample by sample: 1e-4 of the pixel's peak current plus 0.02 e- (float32 accumulation of ~1e4 terms)
+        peak = np.abs(waves).max(axis=1, keepdims=True)
+        err = np.abs(dense[sel] - waves)
+        assert np.all(err <= 1e-4 * peak + 0.02), (err / (1e-4 * peak + 0.02)).max()
+        worst_w = max(worst_w, (err / (1e-4 * peak + 0.02)).max())
+        # Q_p reported by S6 is the same sum
+        assert np.allclose(res["hits"]["q_pixel"][sel], gq, rtol=1e-5, atol=0.05)
+    return worst_q, worst_w
+
+
+def _check_hits(res, wl, dr, pm, seed):
+    """S6 on the oracle's own currents of every active pixel (full chain parity)."""
+    r = oracle.run_chain(wl, seed=seed)
+    h = res["hits"]
+    n = int(h["counters"][0])
+    gpu = (h["hit_pixel"][:n], h["hit_tick"][:n], h["hit_adc"][:n])
+    frac, near, ng, no = compare_hits(gpu, (r["hit_pixel"], r["hit_tick"], r["hit_adc"]))
+    assert no > 0
+    assert frac >= 0.999 and near, (frac, near, ng, no)
+    assert ng == no
+    # sorted by (pixel, tick)
+    key = gpu[0].astype(np.int64) * (1 << 20) + gpu[1]
+    assert np.all(np.diff(key) > 0)
+    return frac
+
+
+def test_config0_full_chain(lartpc):
+    """BASELINE configs[0]: 100 segments of one MIP track, every stage and every active pixel."""
+    wl = W.make_config(0)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_currents(res, wl, dr, pm)
+    _check_hits(res, wl, dr, pm, wl.seed)
+    sim.close()
+
+
+@pytest.mark.parametrize("seed", [7, 8, 9])
+def test_config0_other_tracks(lartpc, seed):
+    wl = W.make_config(0, seed=seed)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_currents(res, wl, dr, pm)
+    _check_hits(res, wl, dr, pm, wl.seed)
+    sim.close()
+
+
+def test_run_spill_matches_staged(lartpc):
+    """lartpc_run_spill gives the same hit list as the staged calls (same kernels, bit for bit)."""
+    wl = W.make_config(0)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    seg = sim.upload_segments(wl.segments)
+    hits, st = sim.run_spill(seg, wl.seed, hit_capacity=4096)
+    n = int(res["hits"]["counters"][0])
+    assert st.n_hits == n and st.n_hits_total == n and st.n_hits_dropped == 0
+    assert st.n_tiles == res["info"].n_tiles and st.n_active_pixels == res["n_active"]
+    got = lartpc.hits_to_numpy(hits)
+    for a, k in zip(got, ("hit_pixel", "hit_tick", "hit_adc")):
+        assert np.array_equal(a, res["hits"][k][:n])
+    sim.close()
+
+
+def test_config1_sampled_pixels(lartpc):
+    """BASELINE configs[1] (cosmics, 70x70 pixels, 30 cm drift, noise on): all segment stages, and the
+    currents of a sample of pixels (the busiest ones plus a random draw) against the oracle."""
+    wl = W.make_config(1)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_currents(res, wl, dr, pm, max_pixels=48)
+    sim.close()
+
+
+def test_zero_drift_and_edges(lartpc):
+    """Degenerate cases: segments at the anode (sigma = 0, indicator weights), at the plane edge (charge bins
+    outside the plane act on in-plane pixels), outside every TPC, zero length and zero energy."""
+    p = W.default_params(n_readout_ticks=900)
+    tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, 10.0, 16, 16, 0)]
+    pitch = p["pixel_pitch_cm"]
+    rng = np.random.Generator(np.random.PCG64(3))
+    parts = [
+        W.line_segments([3.3 * pitch, 4.2 * pitch, 0.0], [6.1 * pitch, 5.9 * pitch, 0.0], 0.1, 0.5, W._mip(2.1)),  # anode
+        W.line_segments([0.05 * pitch, 7.0 * pitch, 4.0], [2.0 * pitch, 7.7 * pitch, 4.3], 0.1, 0.0, W._mip(2.1)),  # left edge
+        W.line_segments([14.0 * pitch, 15.95 * pitch, 2.0], [15.9 * pitch, 15.6 * pitch, 2.5], 0.1, 0.0, W._mip(2.1)),  # corner
+        W.line_segments([30.0, 1.0, 1.0], [30.5, 1.0, 1.0], 0.1, 0.0, W._mip(2.1)),                                  # outside
+    ]
+    seg = W._concat(parts)
+    for k in seg:
+        seg[k] = np.concatenate([seg[k], seg[k][:2]])
+    seg["xe"][-1] = seg["xs"][-1]; seg["ye"][-1] = seg["ys"][-1]; seg["ze"][-1] = seg["zs"][-1]    # zero length
+    seg["dE"][-2] = 0.0                                                                               # zero energy
+    wl = W.Workload("edges", 5, p, tpcs, seg, W.pad_response_lut(p))
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_currents(res, wl, dr, pm)
+    _check_hits(res, wl, dr, pm, wl.seed)
+    sim.close()
+
+
+def test_empty_input(lartpc):
+    wl = W.make_config(0)
+    wl = wl.subset(np.zeros(0, dtype=np.int64))
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    assert res["n_active"] == 0 and int(res["hits"]["counters"][0]) == 0 and res["info"].n_tiles == 0
+    seg = sim.upload_segments(wl.segments)
+    hits, st = sim.run_spill(seg, 1, hit_capacity=16)
+    assert st.n_hits == 0
+    sim.close()
