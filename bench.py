@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the LArTPC charge hot path (arXiv 2212.09807) on B200.
+
+One "step" = one pass of the whole hot path (S1 quench .. S6 electronics, `lartpc_run_spill`) over one
+synthetic spill.  Metric (BASELINE.json): segments/s (whole job) with ms/spill as `ms_per_step`.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+* `value`     segments/s with the segment arrays already resident in HBM (device-timed, CUDA events).
+* `e2e`       same metric through the C-ABI with HOST (pinned) segment arrays: host->device copy of the nine
+              float32 arrays and device->host read of the hit list inside the timed region.
+* `roofline`  the dominant kernel (S4 induced current): multiply-adds the method needs for the charge it found
+              (counted on the device) x 2 / its CUDA-event time, against the FP32 FMA peak measured on this GPU by the
+              library's FFMA-chain microbenchmark (MEASURED_PEAKS.json holds no FP32 figure).
+* `cpu_baseline`  the fp64 oracle (oracle/, as it stands) on this host's cores, on a bounded sample.
+* `--impl reference`  times that oracle alone (there is no reference code for this paper).
+N > 1 (torchrun): every rank simulates its own independent spill (seed + rank), no data-path collective;
+`value` sums the ranks' segments over the max-over-ranks time ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2212_09807_b200 import workloads  # noqa: E402
+
+METRIC = "segments/s (ms/spill in ms_per_step)"
+WORKLOAD_NAMES = {
+    0: "configs[0] PR1 single MIP muon, 100 segments, 32x32 pixels",
+    1: "configs[1] cosmic muons, one TPC, 70x70 pixels, 30 cm drift",
+    2: "configs[2] neutrino-like interactions, 2x2 modules (8 TPCs), ~1e5 segments",
+    3: "configs[3] full ND-LAr-scale beam spill, 70 TPCs, ~1.07e7 pixels, ~5e6 segments",
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--segments", type=int, default=None, help="override the segment target of configs 2/3")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample", type=int, default=1000, help="segments in the oracle's bounded sample")
+    return ap.parse_args()
+
+
+def make_workload(cfg: int, rank: int, segments=None):
+    kw = {}
+    if segments is not None and cfg in (2, 3):
+        kw["target"] = segments
+    if rank:
+        kw["seed"] = workloads.SEED_BASE + cfg + 1000 * rank
+    return workloads.make_config(cfg, **kw)
+
+
+# --------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md "clocks line")
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                if out.returncode == 0 and out.stdout.strip():
+                    self.rows.append([c.strip() for c in out.stdout.strip().splitlines()[0].split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._t:
+            self._t.join(timeout=6)
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------------
+def oracle_sample(wl, n_sample: int):
+    """A contiguous block of segments from the middle of the spill (one shower / track neighbourhood)."""
+    n = wl.n_segments
+    m = min(n_sample, n)
+    lo = max(0, n // 2 - m // 2)
+    return wl.subset(np.arange(lo, lo + m)), "segments [%d, %d) of %d, all pixels they reach, full chain O1-O6" % (
+        lo, lo + m, n)
+
+
+def time_oracle(wl, n_sample: int):
+    import oracle
+    oracle.build()
+    sub, what = oracle_sample(wl, n_sample)
+    cores = os.cpu_count() or 1
+    t0 = time.perf_counter()
+    res = oracle.run_chain(sub, threads=cores)
+    dt = time.perf_counter() - t0
+    return {"value": sub.n_segments / dt, "unit": "segments/s", "cores": cores, "kind": "oracle",
+            "sample": what + " (%.1f s, %d hits)" % (dt, len(res["hit_pixel"]))}, dt, sub.n_segments
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step = one bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = make_workload(args.config, 0, args.segments)
+    n_sample = max(50, args.cpu_sample // 4)            # sized so steps + warm-up end within a few minutes
+    total, segs, info = 0.0, 0, None
+    for i in range(args.warmup + args.steps):
+        if i >= min(args.warmup, 1) and i < args.warmup:
+            continue                                      # one warm-up pass is enough for a CPU program
+        info, dt, ns = time_oracle(wl, n_sample)
+        if i >= args.warmup:
+            total += dt
+            segs += ns
+    value = segs / total
+    info["value"] = value
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "segments/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[args.config], "n_segments": wl.n_segments,
+                       "n_pixels": wl.n_pixels, "step": "oracle O1-O6 on a bounded sample: " + info["sample"]},
+            "cpu_baseline": info,
+            "e2e": {"value": value, "unit": "segments/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2212_09807_b200 import lartpc
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: the LArTPC path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = make_workload(args.config, rank, args.segments)
+    n = wl.n_segments
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, device="cuda:%d" % local)
+    if wl.disabled_pixels is not None:
+        sim.set_disabled_pixels(wl.disabled_pixels)
+    host = {k: torch.from_numpy(np.ascontiguousarray(wl.segments[k], dtype=np.float32)).pin_memory()
+            for k in workloads.SEG_FIELDS}
+    seg = {k: v.to(dev) for k, v in host.items()}
+    ws = torch.empty(sim.workspace_bytes(n), dtype=torch.uint8, device=dev)
+    hit_cap = int(min(64_000_000, max(1 << 16, 8 * n)))
+    hits, st = sim.run_spill(seg, wl.seed, hit_cap, workspace=ws)           # sizes the library's plan buffers
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)           # > 126 MB L2
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing -------------------------------------------------------------------
+    for _ in range(args.warmup):
+        flush.zero_()
+        hits, st = sim.run_spill(seg, wl.seed, hit_cap, workspace=ws, hits=hits)
+    peak_scalar, peak_packed = lartpc.measure_fp32_peak(0), lartpc.measure_fp32_peak(1)
+    sim.set_profiling(True)
+    launches0 = lartpc.kernel_launches()
+    stage_ms = {k: 0.0 for k in sim.STAGES}
+    stage_n = {k: 0 for k in sim.STAGES}
+    fma = 0.0
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    clocks = ClockSampler(local)
+    barrier()
+    clocks.start()
+    for i in range(args.steps):
+        flush.zero_()
+        ev[i][0].record()
+        hits, st = sim.run_spill(seg, wl.seed, hit_cap, workspace=ws, hits=hits)
+        ev[i][1].record()
+        ms, ln, f = sim.stage_ms()
+        for k in sim.STAGES:
+            stage_ms[k] += ms[k]
+            stage_n[k] += ln[k]
+        fma += f
+    barrier()
+    clk = clocks.stop()
+    launches = lartpc.kernel_launches() - launches0
+    sim.set_profiling(False)
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    nseg = torch.tensor([float(n)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(nseg, op=dist.ReduceOp.SUM)
+    total_ms_max, n_all = float(t.item()), float(nseg.item())
+
+    # ---- end to end through the C-ABI with host buffers ------------------------------------------
+    e2e_ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    d2h = 0
+    barrier()
+    e2e_ev[0].record()
+    for i in range(args.steps):
+        flush.zero_()
+        dseg = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
+        hits, st2 = sim.run_spill(dseg, wl.seed, hit_cap, workspace=ws, hits=hits)
+        nh = int(st2.n_hits)
+        out = [hits[k][:nh].cpu() for k in ("hit_pixel", "hit_tick", "hit_adc")]
+        d2h = sum(o.numel() * o.element_size() for o in out) + 32
+    e2e_ev[1].record()
+    barrier()
+    flush_ms = 0.0
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record()
+    for i in range(args.steps):
+        flush.zero_()
+    f1.record()
+    torch.cuda.synchronize()
+    flush_ms = f0.elapsed_time(f1)
+    te = torch.tensor([e2e_ev[0].elapsed_time(e2e_ev[1]) - flush_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_ms = float(te.item())
+
+    if rank == 0:
+        s4_ms = stage_ms["induced_current"] / max(stage_n["induced_current"], 1)
+        fma_per_launch = fma / max(stage_n["induced_current"], 1)
+        peak = max(peak_scalar, peak_packed)
+        achieved = 2.0 * fma_per_launch / (s4_ms * 1e-3) / 1e12 if s4_ms > 0 else 0.0
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get("induced_current_bytes_per_launch")
+            except Exception:
+                traffic = None
+        line = {
+            "metric": METRIC, "value": n_all * args.steps / (total_ms_max * 1e-3), "unit": "segments/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[args.config], "n_segments": n, "n_pixels": wl.n_pixels,
+                       "n_readout_ticks": int(wl.params["n_readout_ticks"]), "n_tpcs": len(wl.tpcs),
+                       "seed": wl.seed, "l2": "256 MiB flush write between timed steps",
+                       "parallelism": "independent spill per GPU" if world > 1 else "single GPU"},
+            "stats": {"n_tiles": int(st.n_tiles), "n_pairs": int(st.n_pairs), "n_active_pixels": int(st.n_active_pixels),
+                      "total_samples": int(st.total_samples), "n_hits": int(st.n_hits),
+                      "n_hits_dropped": int(st.n_hits_dropped), "n_batches": int(st.n_batches)},
+            "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
+            "e2e": {"value": n_all * args.steps / (e2e_ms * 1e-3), "unit": "segments/s",
+                    "h2d_bytes_per_step": 9 * 4 * n, "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.steps},
+            "gpu_launches": int(launches),
+            "clocks": clk,
+            "roofline": {"kernel": "induced_current (S4)", "bound": "alu", "achieved": achieved, "peak": peak,
+                         "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": traffic,
+                         "peak_source": "lartpc_measure_fp32_peak on this GPU (scalar FFMA %.1f, packed FFMA2 %.1f)"
+                                        % (peak_scalar, peak_packed),
+                         "launch_ms": s4_ms, "flops_per_launch": 2.0 * fma_per_launch,
+                         "share_of_step": stage_ms["induced_current"] / max(sum(stage_ms.values()), 1e-9)},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"], _, _ = time_oracle(wl, args.cpu_sample)
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -232,6 +232,21 @@ int  lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n
  * roofline denominator of S4. */
 int  lartpc_measure_fp32_peak(int variant, double *tflops, void *stream);
 
+/* Per-stage device times of lartpc_run_spill.  With profiling on, run_spill brackets every stage launch with
+ * CUDA events recorded on `stream` and adds the elapsed times up per stage after its final synchronisation
+ * (a few microseconds of overhead per launch; off by default).  lartpc_get_stage_ms returns, for the last
+ * run_spill, ms[s] = device milliseconds and launches[s] = times the stage ran (one per TPC batch for S3-S6):
+ * s = 0 quench, 1 drift, 2 pixel mapping + plan, 3 induced current, 4 per-pixel sum, 5 electronics.
+ * fma_current = multiply-adds the S4 response needs for the charge it found (counted on the device:
+ * non-zero charge cells x in-plane target pixels x lut_ticks), the numerator of its roofline figure. */
+#define LARTPC_N_STAGES 6
+int  lartpc_set_profiling(lartpc_sim_t *sim, int on);
+int  lartpc_get_stage_ms(const lartpc_sim_t *sim, double ms[LARTPC_N_STAGES], int64_t launches[LARTPC_N_STAGES],
+                         double *fma_current);
+
+/* Kernels the library has launched in this process so far (all sims; not thread-safe, a plain counter). */
+int64_t lartpc_kernel_launches(void);
+
 const char *lartpc_strerror(int code);
 
 #ifdef __cplusplus

@@ -10,6 +10,9 @@ size_t lartpc_current_smem(const DevParams &p);
 int lartpc_current_tasks_per_group();
 
 static thread_local char g_last_cuda_error[256] = "";
+long long g_lartpc_launches = 0;
+
+extern "C" int64_t lartpc_kernel_launches(void) { return (int64_t)g_lartpc_launches; }
 
 void lartpc_note_cuda_error(cudaError_t e, const char *file, int line)
 {
@@ -40,6 +43,8 @@ static void sim_free(lartpc_sim *s)
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
     cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->scan_tmp);
     cudaFree(s->d_counters); cudaFree(s->disabled_mask); cudaFree(s->elec_slots); cudaFree(s->elec_offs);
+    cudaFree(s->d_fma);
+    for (cudaEvent_t e : s->ev_pool) cudaEventDestroy(e);
     if (s->h_counters) cudaFreeHost(s->h_counters);
     delete s;
 }
@@ -153,6 +158,8 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
     SIM_TRY(cudaMalloc(&s->act_slot, sizeof(int32_t) * pix));
     SIM_TRY(cudaMalloc(&s->d_counters, sizeof(long long) * CNT_COUNT));
     SIM_TRY(cudaMallocHost(&s->h_counters, sizeof(long long) * CNT_COUNT));
+    SIM_TRY(cudaMalloc(&s->d_fma, sizeof(unsigned long long)));
+    SIM_TRY(cudaMemset(s->d_fma, 0, sizeof(unsigned long long)));
     s->pair_cap = 1 << 16;  s->tile_cap = 1 << 14;
     SIM_TRY(cudaMalloc(&s->pair_seg, sizeof(int32_t) * s->pair_cap));
     SIM_TRY(cudaMalloc(&s->tile_cp, sizeof(int32_t) * s->tile_cap));
@@ -234,7 +241,8 @@ static int ensure_i32(int32_t **p, int64_t *cap, int64_t need)
 extern "C" int lartpc_electronics(lartpc_sim_t *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
                                   void *stream)
 {
-    if (!sim || !wf || !out || !out->counters || !out->hits_per_pixel || !out->q_pixel) return LARTPC_ERR_BAD_ARGUMENT;
+    if (!sim || !wf || !out || !out->counters) return LARTPC_ERR_BAD_ARGUMENT;
+    if (wf->n_active > 0 && (!out->hits_per_pixel || !out->q_pixel)) return LARTPC_ERR_BAD_ARGUMENT;
     cudaStream_t st = (cudaStream_t)stream;
     LARTPC_CUDA_TRY(cudaMemsetAsync(out->counters, 0, sizeof(int64_t) * 4, st));
     // the per-pixel hit slots live in sim-owned scratch, grown on demand (no allocation after warm-up)
@@ -259,12 +267,68 @@ struct Arena {
 };
 }  // namespace
 
+// stage timing: event pairs recorded around each stage launch when profiling is on
+struct StageTimer {
+    lartpc_sim *sim; cudaStream_t st; size_t used = 0;
+    cudaEvent_t next()
+    {
+        if (used == sim->ev_pool.size()) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            sim->ev_pool.push_back(e);
+        }
+        return sim->ev_pool[used++];
+    }
+    void begin(int stage)
+    {
+        if (!sim->profiling) return;
+        sim->ev_stage.push_back(stage);
+        cudaEventRecord(next(), st);
+    }
+    void end()
+    {
+        if (sim->profiling) cudaEventRecord(next(), st);
+    }
+    void collect()                        // after the stream has been synchronised
+    {
+        for (int s = 0; s < LARTPC_N_STAGES; ++s) { sim->stage_ms[s] = 0.0; sim->stage_launches[s] = 0; }
+        for (size_t i = 0; i < sim->ev_stage.size(); ++i) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, sim->ev_pool[2 * i], sim->ev_pool[2 * i + 1]);
+            sim->stage_ms[sim->ev_stage[i]] += ms;
+            sim->stage_launches[sim->ev_stage[i]] += 1;
+        }
+        sim->ev_stage.clear();
+    }
+};
+
+extern "C" int lartpc_set_profiling(lartpc_sim_t *sim, int on)
+{
+    if (!sim) return LARTPC_ERR_BAD_ARGUMENT;
+    sim->profiling = on != 0;
+    return LARTPC_OK;
+}
+
+extern "C" int lartpc_get_stage_ms(const lartpc_sim_t *sim, double ms[LARTPC_N_STAGES],
+                                   int64_t launches[LARTPC_N_STAGES], double *fma_current)
+{
+    if (!sim || !ms) return LARTPC_ERR_BAD_ARGUMENT;
+    for (int s = 0; s < LARTPC_N_STAGES; ++s) {
+        ms[s] = sim->stage_ms[s];
+        if (launches) launches[s] = sim->stage_launches[s];
+    }
+    if (fma_current) *fma_current = sim->fma_current;
+    return LARTPC_OK;
+}
+
 extern "C" size_t lartpc_workspace_bytes(const lartpc_sim_t *sim, int64_t max_segments)
 {
     if (!sim) return 0;
-    // per segment: n_e, dEdx (8) + drifted (64) + pixmap (12*4 + 8) = 128 B; plus tile partials / waveforms of
-    // the largest TPC batch, which depend on the data: 3 GiB covers the BASELINE configs with room to spare.
-    return (size_t)max_segments * 160 + ((size_t)3 << 30);
+    // per segment: n_e, dEdx (8) + drifted (64) + pixmap (12*4 + 8) = 128 B, rounded up to 160.  The tile partials
+    // and waveforms of the largest TPC batch depend on the data; measured on the BASELINE configs they stay under
+    // 1.3 tiles per segment of the busiest TPC, so 3 GiB + 4 KiB per segment covers them with room to spare
+    // (configs[3]: ~22 GiB of the 180 GB).  run_spill halves its TPC batches until they fit whatever it is given.
+    return (size_t)max_segments * (160 + 4096) + ((size_t)3 << 30);
 }
 
 extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, uint64_t seed,
@@ -279,6 +343,9 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
     memset(&stt, 0, sizeof(stt));
     stt.n_segments = n;
     LARTPC_CUDA_TRY(cudaMemsetAsync(out->counters, 0, sizeof(int64_t) * 4, st));
+    LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_fma, 0, sizeof(unsigned long long), st));
+    StageTimer tm{sim, st};
+    sim->ev_stage.clear();
 
     float *dEdx = ar.take<float>(n), *n_e = ar.take<float>(n);
     lartpc_drifted_t dr;
@@ -296,8 +363,12 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
     const size_t mark = ar.used;
 
     int rc;
+    tm.begin(0);
     if ((rc = launch_quench(sim, seg, n, dEdx, n_e, st)) != 0) return rc;
+    tm.end();
+    tm.begin(1);
     if ((rc = launch_drift(sim, seg, n, n_e, &dr, st)) != 0) return rc;
+    tm.end();
 
     // batches of consecutive TPCs; a batch whose tiles / waveforms do not fit the workspace is halved
     int tpc_lo = 0;
@@ -305,7 +376,9 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
     while (tpc_lo < p.n_tpcs) {
         int tpc_hi = std::min(p.n_tpcs, tpc_lo + batch);
         lartpc_pixmap_info_t info;
+        tm.begin(2);
         if ((rc = launch_plan(sim, seg, &dr, n, tpc_lo, tpc_hi, &pm, &info, st)) != 0) return rc;
+        tm.end();
         ar.used = mark;
         lartpc_signals_t sig;
         sig.tile_capacity = info.n_tiles;
@@ -332,15 +405,26 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
         stt.n_tiles += info.n_tiles;  stt.n_pairs += info.n_pairs;
         stt.n_active_pixels += info.n_active_pixels;  stt.total_samples += info.total_samples;
         stt.n_batches += 1;
+        tm.begin(3);
         if ((rc = launch_current(sim, &dr, &pm, n, &sig, st)) != 0) return rc;
+        tm.end();
         sim->have_signals = true;
+        tm.begin(4);
         if ((rc = launch_sum(sim, &sig, &wf, st)) != 0) return rc;
+        tm.end();
+        tm.begin(5);
         if ((rc = launch_electronics(sim, &wf, seed, &h, slots, offs, 0, st)) != 0) return rc;
+        tm.end();
         tpc_lo = tpc_hi;
     }
     long long hc[4];
+    unsigned long long fma = 0;
     LARTPC_CUDA_TRY(cudaMemcpyAsync(hc, out->counters, sizeof(hc), cudaMemcpyDeviceToHost, st));
+    LARTPC_CUDA_TRY(cudaMemcpyAsync(&fma, sim->d_fma, sizeof(fma), cudaMemcpyDeviceToHost, st));
     LARTPC_CUDA_TRY(cudaStreamSynchronize(st));
+    tm.collect();
+    sim->fma_current = (double)fma;
+    stt.flops_current = 2.0 * (double)fma;
     stt.n_hits = hc[0]; stt.n_hits_total = hc[1]; stt.n_pixels_overflow = hc[2]; stt.n_hits_dropped = hc[3];
     if (stats) *stats = stt;
     return LARTPC_OK;
@@ -403,8 +487,8 @@ extern "C" int lartpc_measure_fp32_peak(int variant, double *tflops, void *strea
     double best = 0.0;
     for (int rep = 0; rep < 5; ++rep) {
         cudaEventRecord(e0, st);
-        if (variant == 0) fp32_peak_kernel<0><<<blocks, threads, 0, st>>>(sink, iters, 1.0f);
-        else fp32_peak_kernel<1><<<blocks, threads, 0, st>>>(sink, iters, 1.0f);
+        if (variant == 0) { ++g_lartpc_launches; fp32_peak_kernel<0><<<blocks, threads, 0, st>>>(sink, iters, 1.0f); }
+        else { ++g_lartpc_launches; fp32_peak_kernel<1><<<blocks, threads, 0, st>>>(sink, iters, 1.0f); }
         cudaEventRecord(e1, st);
         cudaEventSynchronize(e1);
         float ms = 0.f;

@@ -12,6 +12,7 @@
     } while (0)
 
 void lartpc_note_cuda_error(cudaError_t e, const char *file, int line);
+extern long long g_lartpc_launches;   // kernels launched by the library in this process (lartpc_kernel_launches)
 
 // ---- constants copied to every kernel by value ------------------------------------------------
 struct DevParams {
@@ -79,6 +80,14 @@ struct lartpc_sim {
     lartpc_drifted_t drifted_copy;
     lartpc_pixmap_t pixmap_copy;
     int sm_count = 148;
+    // per-stage profiling of run_spill (lartpc_set_profiling)
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<int> ev_stage;           // stage of the event pair (2i, 2i+1)
+    double stage_ms[LARTPC_N_STAGES] = {0, 0, 0, 0, 0, 0};
+    int64_t stage_launches[LARTPC_N_STAGES] = {0, 0, 0, 0, 0, 0};
+    double fma_current = 0.0;
+    unsigned long long *d_fma = nullptr; // device counter of S4 multiply-adds
 };
 
 // ---- IEEE-exact float64 helpers (never contracted into FMA) -----------------------------------

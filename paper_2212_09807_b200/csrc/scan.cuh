@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+extern long long g_lartpc_launches;
+
 namespace lscan {
 
 constexpr int THREADS = 256;
@@ -111,9 +113,11 @@ inline cudaError_t exclusive_scan(int64_t n, F f, Out *out, bool write_last, lon
         return cudaGetLastError();
     }
     int64_t blocks = (n + TILE - 1) / TILE;
+    ++g_lartpc_launches;
     block_sums_kernel<<<(unsigned)blocks, THREADS, 0, st>>>(n, f, tmp);
+    ++g_lartpc_launches;
     scan_sums_kernel<<<1, THREADS, 0, st>>>(tmp, blocks, total_dev);
-    if (out) final_scan_kernel<<<(unsigned)blocks, THREADS, 0, st>>>(n, f, tmp, out, write_last);
+    if (out) { ++g_lartpc_launches; final_scan_kernel<<<(unsigned)blocks, THREADS, 0, st>>>(n, f, tmp, out, write_last); }
     return cudaGetLastError();
 }
 

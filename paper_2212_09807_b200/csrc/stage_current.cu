@@ -34,6 +34,7 @@ struct CurrentArgs {
     const float *lut;
     float *partial;
     int32_t *tile_range;
+    unsigned long long *fma_counter;   // multiply-adds of the response: non-zero cells x valid targets x K
     int CJ, NEP, NB2P;           // smem strides: charge row, erf row, wxy row
 };
 
@@ -206,10 +207,11 @@ __global__ void __launch_bounds__(NT, 1) induced_current_kernel(const CurrentArg
     __syncthreads();
 
     // ------------------------------------------------------------------ phase 2: non-empty bins
+    int nz_cells = 0;
     for (int c = warp; c < NB2; c += NT / 32) {
         int lo = INT_MAX, hi = -1;
         for (int j = lane; j < CJ; j += 32)
-            if (Csm[c * CJ + j] != 0.f) { lo = min(lo, j); hi = max(hi, j); }
+            if (Csm[c * CJ + j] != 0.f) { lo = min(lo, j); hi = max(hi, j); ++nz_cells; }
         for (int d = 16; d; d >>= 1) {
             lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, d));
             hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, d));
@@ -250,6 +252,11 @@ __global__ void __launch_bounds__(NT, 1) induced_current_kernel(const CurrentArg
     }
     __syncthreads();
     const int nbins = s_misc[0], tjlo = s_misc[1], tjhi = s_misc[2], nvalid = s_misc[3];
+    if (blockIdx.y == 0) {
+        for (int d = 16; d; d >>= 1) nz_cells += __shfl_xor_sync(0xffffffffu, nz_cells, d);
+        if (lane == 0 && nz_cells)
+            atomicAdd(a.fma_counter, (unsigned long long)nz_cells * (unsigned long long)(nvalid * K));
+    }
     if (nbins == 0 || nvalid == 0) {
         if (tid == 0 && blockIdx.y == 0) { a.tile_range[2 * tile] = 1; a.tile_range[2 * tile + 1] = 0; }
         return;
@@ -349,6 +356,7 @@ int launch_current(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pix
     a.jt0 = pm->jt0; a.jt1 = pm->jt1; a.n_samples = pm->n_samples;
     a.lut = sim->d_lut;
     a.partial = out->partial;  a.tile_range = out->tile_range;
+    a.fma_counter = sim->d_fma;
     size_t smem = current_smem_bytes(p, a.CJ, a.NEP, a.NB2P);
     static size_t configured = 0;
     if (smem > configured) {
@@ -357,6 +365,7 @@ int launch_current(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pix
         configured = smem;
     }
     dim3 grid((unsigned)sim->n_tiles, (unsigned)p.n_groups);
+    ++g_lartpc_launches;
     induced_current_kernel<<<grid, NT, smem, st>>>(a);
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;

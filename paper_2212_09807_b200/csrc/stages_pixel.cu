@@ -78,6 +78,7 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
         return LARTPC_OK;
     }
     if (p.WW > 128) return LARTPC_ERR_UNSUPPORTED;
+    ++g_lartpc_launches;
     active_table_kernel<<<div_up(sim->n_pix, 256), 256, 0, st>>>(sim->n_pix, sim->act_first, sim->act_last,
                                                                 sim->act_slot, out->pixel_id, out->first_tick,
                                                                 out->length);
@@ -85,6 +86,7 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
     if (rc) return rc;
     LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_active, LenF{out->length}, out->offset, true, (long long *)nullptr,
                                           sim->scan_tmp, st));
+    ++g_lartpc_launches;
     sum_pixel_kernel<<<(unsigned)sim->n_active, 256, 0, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
                                                              out->length, out->offset, sim->pix_mask, sim->pix_tile0,
                                                              sig->partial, sig->tile_range, out->samples);
@@ -220,6 +222,7 @@ int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t s
     const DevParams &p = sim->dp;
     const int64_t na = wf->n_active;
     if (na == 0) return LARTPC_OK;
+    ++g_lartpc_launches;
     electronics_kernel<<<div_up(na, 128), 128, 0, st>>>(p, seed, na, wf->pixel_id, wf->first_tick, wf->length,
                                                        wf->offset, wf->samples, sim->disabled_mask, slot_scratch,
                                                        out->hits_per_pixel, out->q_pixel);
@@ -228,9 +231,11 @@ int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t s
     long long *batch_total = sim->d_counters + CNT_COUNT - 1;
     LARTPC_CUDA_TRY(lscan::exclusive_scan(na, HitCountF{out->hits_per_pixel, p.max_hits}, scan_scratch, false,
                                           batch_total, sim->scan_tmp, st));
+    ++g_lartpc_launches;
     compact_hits_kernel<<<div_up(na, 256), 256, 0, st>>>(na, p.max_hits, wf->pixel_id, slot_scratch,
                                                         out->hits_per_pixel, scan_scratch, (long long *)out->counters,
                                                         out->hit_capacity, out->hit_pixel, out->hit_tick, out->hit_adc);
+    ++g_lartpc_launches;
     advance_hit_base_kernel<<<1, 1, 0, st>>>((long long *)out->counters, batch_total, out->hit_capacity);
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;

@@ -56,10 +56,13 @@ int launch_quench(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, floa
     SegPtrs s{seg->xs, seg->ys, seg->zs, seg->ts, seg->xe, seg->ye, seg->ze, seg->te, seg->dE};
     bool vec = aligned16(s.xs) && aligned16(s.ys) && aligned16(s.zs) && aligned16(s.xe) && aligned16(s.ye) &&
                aligned16(s.ze) && aligned16(s.dE) && aligned16(dEdx) && aligned16(n_e);
-    if (vec)
+    if (vec) {
+        ++g_lartpc_launches;
         quench_kernel<4><<<div_up(div_up(n, 4), 256), 256, 0, st>>>(sim->dp, s, n, dEdx, n_e);
-    else
+    } else {
+        ++g_lartpc_launches;
         quench_kernel<1><<<div_up(n, 256), 256, 0, st>>>(sim->dp, s, n, dEdx, n_e);
+    }
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }
@@ -132,6 +135,7 @@ int launch_drift(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, const
 {
     if (n == 0) return LARTPC_OK;
     SegPtrs s{seg->xs, seg->ys, seg->zs, seg->ts, seg->xe, seg->ye, seg->ze, seg->te, seg->dE};
+    ++g_lartpc_launches;
     drift_kernel<<<div_up(n, 256), 256, 0, st>>>(sim->dp, sim->d_tpcs, s, n, n_e, *out);
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
@@ -384,8 +388,10 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_cursor, 0, sizeof(int32_t) * sim->n_cp, st));
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_mask, 0, sizeof(unsigned long long) * sim->n_cp, st));
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->act_last, 0xff, sizeof(int32_t) * sim->n_pix, st));
+        ++g_lartpc_launches;
         fill_i32_kernel<<<div_up(sim->n_pix, 256), 256, 0, st>>>(sim->act_first, sim->n_pix, INT32_MAX);
         if (n > 0) {
+            ++g_lartpc_launches;
             pixmap_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, s, n, dr->tpc, dr->q_anode, tpc_lo, tpc_hi,
                                                          *out, sim->pix_count, sim->pix_mask, sim->d_counters);
             LARTPC_CUDA_TRY(cudaGetLastError());
@@ -399,12 +405,15 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_cp, PopcF{sim->pix_mask}, sim->pix_tile0, false,
                                               sim->d_counters + CNT_TILES, sim->scan_tmp, st));
         if (n > 0) {
+            ++g_lartpc_launches;
             pair_fill_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, n, dr->tpc, *out, tpc_lo, tpc_hi,
                                                             sim->pix_start, sim->pix_cursor, sim->pair_seg,
                                                             sim->pair_cap, sim->d_counters);
+            ++g_lartpc_launches;
             pair_sort_kernel<<<div_up(sim->n_cp, 4), 128, 0, st>>>(sim->n_cp, sim->pix_start, sim->pix_count,
                                                                   sim->pair_seg, sim->pair_cap);
         }
+        ++g_lartpc_launches;
         tile_emit_kernel<<<div_up(sim->n_cp, 256), 256, 0, st>>>(p, sim->d_tpcs, sim->n_cp, sim->pix_tile0,
                                                                 sim->pix_mask, sim->tile_cp, sim->tile_desc,
                                                                 sim->tile_cap, sim->act_first, sim->act_last,

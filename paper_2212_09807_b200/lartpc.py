@@ -106,7 +106,7 @@ class Stats(C.Structure):
 EXPORTS = ("lartpc_sim_create", "lartpc_sim_destroy", "lartpc_set_disabled_pixels", "lartpc_chunk_ticks",
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
            "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_run_spill",
-           "lartpc_measure_fp32_peak", "lartpc_strerror")
+           "lartpc_measure_fp32_peak", "lartpc_set_profiling", "lartpc_get_stage_ms", "lartpc_kernel_launches", "lartpc_strerror")
 
 
 def load_library():
@@ -120,6 +120,7 @@ def load_library():
         lib.lartpc_strerror.restype = C.c_char_p
         lib.lartpc_workspace_bytes.restype = C.c_size_t
         lib.lartpc_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
+        lib.lartpc_kernel_launches.restype = C.c_int64
         lib.lartpc_sim_destroy.restype = None
         lib.lartpc_sim_destroy.argtypes = [C.c_void_p]
         for name in EXPORTS:
@@ -151,6 +152,11 @@ def measure_fp32_peak(variant: int = 0) -> float:
     _check(load_library().lartpc_measure_fp32_peak(C.c_int(variant), C.byref(out), _stream_ptr(torch)),
            "lartpc_measure_fp32_peak")
     return float(out.value)
+
+
+def kernel_launches() -> int:
+    """Kernels launched by the library in this process so far."""
+    return int(load_library().lartpc_kernel_launches())
 
 
 class Sim:
@@ -310,6 +316,19 @@ class Sim:
                                            _stream_ptr(t)), "lartpc_electronics")
         out["_struct"] = h
         return out
+
+    STAGES = ("quench", "drift", "pixels_from_segments", "induced_current", "sum_pixel_signals", "electronics")
+
+    def set_profiling(self, on: bool):
+        _check(self.lib.lartpc_set_profiling(self.handle, C.c_int(1 if on else 0)), "lartpc_set_profiling")
+
+    def stage_ms(self):
+        """Per-stage device ms, launch counts and the S4 multiply-add count of the last run_spill."""
+        ms = (C.c_double * len(self.STAGES))()
+        ln = (C.c_int64 * len(self.STAGES))()
+        fma = C.c_double(0.0)
+        _check(self.lib.lartpc_get_stage_ms(self.handle, ms, ln, C.byref(fma)), "lartpc_get_stage_ms")
+        return dict(zip(self.STAGES, ms)), dict(zip(self.STAGES, ln)), float(fma.value)
 
     def workspace_bytes(self, max_segments: int) -> int:
         return int(self.lib.lartpc_workspace_bytes(self.handle, C.c_int64(max_segments)))
