@@ -130,7 +130,7 @@ typedef struct {
 /* S4 output: per-tile partial waveforms, float32 [n_tiles][tile_targets][tile_ticks] (electrons per
  * tick).  Tile (charged pixel P, chunk c) holds the current its charge induces on the W x W pixels
  * around P during readout ticks [c * chunk_ticks, c * chunk_ticks + tile_ticks).  The tile -> pixel
- * map is part of the sim's plan.  `tile_range` int32[n_tiles][2] = first / last 8-tick block written. */
+ * map is part of the sim's plan.  `tile_range` int32[n_tiles][2] = first / last 16-tick block written. */
 typedef struct {
     int64_t  tile_capacity;             /* host value: tiles the two buffers can hold */
     float   *partial;

@@ -7,7 +7,7 @@
 #include "common.cuh"
 
 size_t lartpc_current_smem(const DevParams &p);
-int lartpc_current_tasks_per_group();
+int lartpc_current_threads();
 
 static thread_local char g_last_cuda_error[256] = "";
 long long g_lartpc_launches = 0;
@@ -84,24 +84,35 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
     p.recomb_model = prm->recomb_model;
     p.nb = nb; p.W = W; p.H = (W - 1) / 2; p.K = K; p.WW = W * W; p.NB2 = nb * nb;
     p.n_ticks = prm->n_readout_ticks;  p.j_max = p.n_ticks - K;
-    p.RS = K + 22;
-    while ((p.RS & 3) != 0 || ((p.RS >> 2) & 1) == 0) ++p.RS;             // RS = 4 * odd: conflict-free LDS.128 rows
-    // arrival ticks per tile: as many as fit in shared memory, at most 120, multiple of 8
-    p.Jc = 120;
+    // S4 geometry.  A response task is (pair of target pixels, 16 output ticks); a CTA group of NT threads covers PG
+    // pairs x nblk_max blocks.  Jc (arrival ticks per tile, multiple of 8, at most 120) is chosen to minimise the number
+    // of pair groups per arrival tick, because every group repeats the tile's splat.
+    p.RS = K + 38;
+    while ((p.RS & 1) != 0 || ((p.RS >> 1) & 1) == 0) ++p.RS;               // RS = 2 * odd: conflict-free LDS.128 rows
+    const int n_pairs = (p.WW + 1) / 2, nthreads = lartpc_current_threads();
     const size_t smem_limit = (size_t)prop.sharedMemPerBlockOptin;
-    for (;;) {
-        p.nblk_max = ((p.Jc + K - 2) >> 3) + 1;  p.tile_ticks = 8 * p.nblk_max;
-        if (lartpc_current_smem(p) <= smem_limit || p.Jc <= 8) break;
-        p.Jc -= 8;
+    double best = 0.0;
+    int best_jc = 0;
+    for (int jc = 120; jc >= 8; jc -= 8) {
+        const int nblk = (jc + K - 2) / 16 + 1;
+        if (nblk > nthreads) continue;
+        DevParams q = p;
+        q.Jc = jc;  q.PG = std::min(n_pairs, nthreads / nblk);  q.n_groups = (n_pairs + q.PG - 1) / q.PG;
+        q.PG = (n_pairs + q.n_groups - 1) / q.n_groups;                     // even out the groups
+        if (lartpc_current_smem(q) > smem_limit) continue;
+        const double score = (double)jc / q.n_groups;
+        if (score > best) { best = score; best_jc = jc; }
     }
-    if (lartpc_current_smem(p) > smem_limit) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    if (best_jc == 0) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    p.Jc = best_jc;
+    p.nblk_max = (p.Jc + K - 2) / 16 + 1;  p.tile_ticks = 16 * p.nblk_max;
+    p.PG = std::min(n_pairs, nthreads / p.nblk_max);  p.n_groups = (n_pairs + p.PG - 1) / p.PG;
+    p.PG = (n_pairs + p.n_groups - 1) / p.n_groups;  p.NP = p.n_groups * p.PG;
     p.n_chunks = (p.j_max + p.Jc) / p.Jc;
     if (p.n_chunks > 64) {                                                  // chunk masks are 64-bit
         sim_free(s);
         return LARTPC_ERR_UNSUPPORTED;
     }
-    const int per_group = lartpc_current_tasks_per_group();
-    p.n_groups = (p.WW * p.nblk_max + per_group - 1) / per_group;
     p.n_tpcs = n_tpcs;
     p.gain_mv_per_ke = prm->gain_mv_per_ke; p.v_cm = prm->v_cm_mv; p.v_ref = prm->v_ref_mv; p.v_ped = prm->v_pedestal_mv;
     p.adc_full = ldexp(1.0, prm->adc_bits);  p.threshold = prm->threshold_e;
@@ -129,18 +140,20 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
     if (cp >= INT32_MAX || pix >= INT32_MAX) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
     s->n_cp = cp; s->n_pix = pix;
 
-    // LUT re-laid out as [bin c = cb*nb+ca][target d = dyi*W+dxi][RS] with LUT tick k at word 7+k and zero
-    // padding around it, so that S4 stages all W*W rows of one bin with a single contiguous copy and reads
-    // 16-tap windows with aligned 128-bit loads.  Row (c, d) is R[cy = nb*dyi + cb][cx = nb*dxi + ca][.].
-    std::vector<float> re((size_t)p.NB2 * p.WW * p.RS, 0.f);
+    // LUT re-laid out as [bin c = cb*nb+ca][pair q][RS][2]: pair q interleaves the rows of targets d = 2q and 2q+1
+    // (d = dyi*W + dxi; row (c, d) is R[cy = nb*dyi + cb][cx = nb*dxi + ca][.]), LUT tick k at pair-word 16 + k with
+    // zero padding around it.  S4 stages the PG pair rows of one bin with a single bulk copy, reads 24-tap windows
+    // with aligned 128-bit loads and feeds both targets of a pair to one packed f32x2 multiply-add.
+    std::vector<float> re((size_t)p.NB2 * p.NP * p.RS * 2, 0.f);
     const int NB = W * nb;
     for (int cb = 0; cb < nb; ++cb)
         for (int ca = 0; ca < nb; ++ca)
             for (int dyi = 0; dyi < W; ++dyi)
                 for (int dxi = 0; dxi < W; ++dxi) {
+                    const int d = dyi * W + dxi;
                     const float *src = lut_host + ((size_t)(nb * dyi + cb) * NB + (nb * dxi + ca)) * K;
-                    float *dst = re.data() + ((size_t)(cb * nb + ca) * p.WW + (dyi * W + dxi)) * p.RS + 7;
-                    memcpy(dst, src, sizeof(float) * K);
+                    float *dst = re.data() + (((size_t)(cb * nb + ca) * p.NP + d / 2) * p.RS + 16) * 2 + (d & 1);
+                    for (int k = 0; k < K; ++k) dst[2 * k] = src[k];
                 }
 #define SIM_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { \
         lartpc_note_cuda_error(_e, __FILE__, __LINE__); sim_free(s); return LARTPC_ERR_CUDA; } } while (0)

@@ -23,9 +23,10 @@ struct DevParams {
     int nb, W, H, K, WW, NB2;        // bins per pixel, window pixels, half window, LUT ticks, W*W, nb*nb
     int n_ticks, j_max;              // readout ticks, last arrival tick inside the window (n_ticks - K)
     int Jc, n_chunks;                // arrival ticks per charge tile, chunks covering [0, j_max]
-    int nblk_max, tile_ticks;        // 8-tick output blocks per tile, 8 * nblk_max
-    int RS;                          // padded LUT row stride in floats: [7 zeros][K][zeros], RS = 4 * odd
-    int n_groups;                    // thread-task groups per tile (1 for W = 5, K = 200)
+    int nblk_max, tile_ticks;        // 16-tick output blocks per tile, 16 * nblk_max
+    int RS;                          // padded LUT row length in pair-words: [16 zeros][K][>= 22 zeros], RS = 2 * odd
+    int PG, NP;                      // target pairs per CTA group; pairs incl. padding = n_groups * PG
+    int n_groups;                    // pair groups per tile = gridDim.y of S4 (1 for W = 5, K = 200)
     int n_tpcs;
     // electronics
     double gain_mv_per_ke, v_cm, v_ref, v_ped, adc_full, threshold;

@@ -9,16 +9,19 @@
 //   phase 1  splat the tile's segments into C[nb*nb][Jc] in shared memory (register-tiled outer products
 //            of per-sample erf-difference weights, no atomics);
 //   phase 2  find the non-empty bins and their tick ranges;
-//   phase 3  response: every thread keeps TPT x 8 output ticks of one of the W*W target pixels in registers
-//            and slides a 16-tap LUT window from shared memory over the charge row (64 FMA per 4 LDS.128);
-//            the LUT rows of the current bin are staged from L2 into shared memory;
+//   phase 3  response: a thread keeps 16 output ticks of a PAIR of target pixels in registers (32 accumulators
+//            as 16 packed f32x2) and slides a 24-tap window of the pair-interleaved LUT rows over the charge row:
+//            128 FFMA2 (256 multiply-adds) per 4 LDS.128 of taps + 2 broadcast LDS.128 of charge.  The LUT rows of
+//            the next non-empty bin arrive by cp.async.bulk (TMA engine, mbarrier completion) into the other half
+//            of a double buffer while the current bin is being used;
 //   phase 4  the tile's partial waveforms go to global memory; S5 sums them per pixel in a fixed order.
 #include "common.cuh"
 
 namespace {
 
-constexpr int NT = 512;          // threads per CTA
-constexpr int TPT = 2;           // output tasks (target pixel x 8-tick block) per thread
+constexpr int NT = 256;          // threads per CTA (two CTAs per SM)
+constexpr int NO = 16;           // output ticks per response task
+constexpr int LUT_OFF = 16;      // LUT tick k sits at word LUT_OFF + k of its zero-padded row
 constexpr int SB = 32;           // samples per splat batch
 constexpr int SEGCAP = 32;       // segments staged per batch
 
@@ -43,26 +46,72 @@ struct SegLocal {               // one staged segment, tile-relative
     int N, alo, ahi, blo, bhi, jlo, jhi, seg, zero_sigma;
 };
 
-__device__ __forceinline__ void load8(float (&d)[8], const float *s)
+typedef unsigned long long u64;   // one packed f32x2 register pair: (target 2p, target 2p+1)
+
+__device__ __forceinline__ u64 pack2(float x)
+{
+    u64 r;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ void ffma2(u64 &d, u64 a, u64 b)      // d = a * b + d on both halves
+{
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ void load8w(u64 (&d)[8], const float *s)    // 8 pair-words = 64 bytes
+{
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        ulonglong2 v = *(const ulonglong2 *)(s + 4 * q);
+        d[2 * q] = v.x;  d[2 * q + 1] = v.y;
+    }
+}
+__device__ __forceinline__ void load8c(u64 (&c)[8], const float *s)    // 8 charges, each duplicated into a pair
 {
     float4 x = *(const float4 *)s, y = *(const float4 *)(s + 4);
-    d[0] = x.x; d[1] = x.y; d[2] = x.z; d[3] = x.w; d[4] = y.x; d[5] = y.y; d[6] = y.z; d[7] = y.w;
+    c[0] = pack2(x.x); c[1] = pack2(x.y); c[2] = pack2(x.z); c[3] = pack2(x.w);
+    c[4] = pack2(y.x); c[5] = pack2(y.y); c[6] = pack2(y.z); c[7] = pack2(y.w);
 }
-
-// acc[i] += sum_jj c[jj] * w[i - jj + 7],  w = lo[0..7] ++ hi[0..7]
-__device__ __forceinline__ void fma_block(float (&acc)[8], const float (&c)[8], const float (&lo)[8],
-                                          const float (&hi)[8])
+// acc[i] += sum_jj c[jj] * w[i - jj + 8],  w = lo[0..7] ++ mid[0..7] ++ hi[0..7]  (i < 16, jj < 8)
+__device__ __forceinline__ void fma_step(u64 (&acc)[NO], const u64 (&c)[8], const u64 (&lo)[8], const u64 (&mid)[8],
+                                         const u64 (&hi)[8])
 {
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int jj = 0; jj < 8; ++jj)
 #pragma unroll
-        for (int jj = 0; jj < 8; ++jj) {
-            const int m = i - jj + 7;
-            acc[i] = fmaf(c[jj], m < 8 ? lo[m] : hi[m - 8], acc[i]);
+        for (int i = 0; i < NO; ++i) {
+            const int m = i - jj + 8;
+            ffma2(acc[i], c[jj], m < 8 ? lo[m] : (m < 16 ? mid[m - 8] : hi[m - 16]));
         }
 }
 
-__global__ void __launch_bounds__(NT, 1) induced_current_kernel(const CurrentArgs a)
+// ---- mbarrier + bulk copy (TMA engine) -------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// one thread: expect `bytes` on the barrier and start the global -> shared bulk copy
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, void *bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+__global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const DevParams &p = a.p;
@@ -71,11 +120,13 @@ __global__ void __launch_bounds__(NT, 1) induced_current_kernel(const CurrentArg
 
     float *Csm = (float *)smem_raw;                                  // [NB2][CJ] charge per (bin, arrival tick)
     float *scratch = Csm + NB2 * CJ;                                 // splat scratch, later the LUT stage
-    size_t scratch_floats = max((size_t)WW * RS, (size_t)SB * (a.NEP + a.NB2P + CJ));
+    const int stage_floats = p.PG * RS * 2;                          // one LUT stage: PG pair rows of RS pair-words
+    size_t scratch_floats = max((size_t)2 * stage_floats, (size_t)SB * (a.NEP + a.NB2P + CJ));
     int *s_int = (int *)(scratch + scratch_floats);
-    int *bin_jlo = s_int, *bin_jhi = s_int + NB2, *bin_list = s_int + 2 * NB2, *valid_list = s_int + 3 * NB2;
-    int *s_misc = valid_list + WW;                                   // [0] n bins, [1] tile jlo, [2] tile jhi, [3] nvalid
-    SegLocal *segs = (SegLocal *)(s_misc + 8);
+    int *bin_jlo = s_int, *bin_jhi = s_int + NB2, *bin_list = s_int + 2 * NB2;
+    int *s_misc = bin_list + NB2;                                    // [0] n bins, [1] tile jlo, [2] tile jhi
+    u64 *mbar = (u64 *)(s_misc + 8);                                 // [2] "stage full" barriers
+    SegLocal *segs = (SegLocal *)(mbar + 2);
 
     const int tile = blockIdx.x;
     const TileDesc td = a.tile_desc[tile];
@@ -85,6 +136,11 @@ __global__ void __launch_bounds__(NT, 1) induced_current_kernel(const CurrentArg
     const int lstart = a.pix_start[cp], lcount = a.pix_count[cp];
 
     for (int i = tid; i < NB2 * CJ / 4; i += NT) ((float4 *)Csm)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (tid == 0) {
+        mbar_init(&mbar[0], 1);
+        mbar_init(&mbar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
 
     // ------------------------------------------------------------------ phase 1: splat
     float *erfv = scratch, *wxy = scratch + SB * a.NEP, *wt = wxy + SB * a.NB2P;
@@ -235,92 +291,102 @@ __global__ void __launch_bounds__(NT, 1) induced_current_kernel(const CurrentArg
             tlo = min(tlo, __shfl_xor_sync(0xffffffffu, tlo, d));
             thi = max(thi, __shfl_xor_sync(0xffffffffu, thi, d));
         }
-        int nvalid = 0;                       // targets inside the plane: ix = px + H - dxi, iy = py + H - dyi
-        for (int base = 0; base < WW; base += 32) {
-            const int d = base + lane;
-            bool f = false;
-            if (d < WW) {
-                const int dyi = d / p.W, dxi = d - dyi * p.W;
-                const int ix = td.px + p.H - dxi, iy = td.py + p.H - dyi;
-                f = ix >= 0 && ix < tp.nx && iy >= 0 && iy < tp.ny;
-            }
-            const unsigned bal = __ballot_sync(0xffffffffu, f);
-            if (f) valid_list[nvalid + __popc(bal & ((1u << lane) - 1u))] = d;
-            nvalid += __popc(bal);
-        }
-        if (lane == 0) { s_misc[0] = nbins; s_misc[1] = tlo; s_misc[2] = thi; s_misc[3] = nvalid; }
+        if (lane == 0) { s_misc[0] = nbins; s_misc[1] = tlo; s_misc[2] = thi; }
     }
     __syncthreads();
-    const int nbins = s_misc[0], tjlo = s_misc[1], tjhi = s_misc[2], nvalid = s_misc[3];
-    if (blockIdx.y == 0) {
-        for (int d = 16; d; d >>= 1) nz_cells += __shfl_xor_sync(0xffffffffu, nz_cells, d);
-        if (lane == 0 && nz_cells)
-            atomicAdd(a.fma_counter, (unsigned long long)nz_cells * (unsigned long long)(nvalid * K));
-    }
-    if (nbins == 0 || nvalid == 0) {
+    const int nbins = s_misc[0], tjlo = s_misc[1], tjhi = s_misc[2];
+    if (nbins == 0) {
         if (tid == 0 && blockIdx.y == 0) { a.tile_range[2 * tile] = 1; a.tile_range[2 * tile + 1] = 0; }
         return;
     }
+    if (blockIdx.y == 0) {
+        // multiply-adds the method needs here: non-zero cells x in-plane targets x K
+        for (int d = 16; d; d >>= 1) nz_cells += __shfl_xor_sync(0xffffffffu, nz_cells, d);
+        const int vx = min(td.px + p.H, tp.nx - 1) - max(td.px - p.H, 0) + 1;
+        const int vy = min(td.py + p.H, tp.ny - 1) - max(td.py - p.H, 0) + 1;
+        if (lane == 0 && nz_cells && vx > 0 && vy > 0)
+            atomicAdd(a.fma_counter, (unsigned long long)nz_cells * (unsigned long long)(vx * vy * K));
+    }
 
     // ------------------------------------------------------------------ phase 3: response
-    const int nB_lo = tjlo >> 3, nB_hi = (tjhi + K - 1) >> 3;
-    const int ntasks = nvalid * (nB_hi - nB_lo + 1);
-    int t_delta[TPT], t_nB[TPT];
-    bool t_ok[TPT];
-    float acc[TPT][8];
-#pragma unroll
-    for (int s = 0; s < TPT; ++s) {
-        const int task = (blockIdx.y * TPT + s) * NT + tid;
-        t_ok[s] = task < ntasks;
-        const int nBi = t_ok[s] ? task / nvalid : 0;
-        t_delta[s] = valid_list[t_ok[s] ? task - nBi * nvalid : 0];
-        t_nB[s] = nB_lo + nBi;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) acc[s][i] = 0.f;
+    // this CTA's pair group g = blockIdx.y: pairs [g PG, (g+1) PG); its LUT stage for bin c is one contiguous block
+    const int g = blockIdx.y;
+    const uint32_t stage_bytes = (uint32_t)stage_floats * 4u;
+    const float *lut_g = a.lut + (size_t)g * stage_floats;
+    const size_t lut_bin_stride = (size_t)p.NP * RS * 2;
+    float *Rsm0 = scratch, *Rsm1 = scratch + stage_floats;
+    if (tid == 0) {
+        // the splat used this memory through the generic proxy; order those accesses before the bulk copies
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        bulk_load(Rsm0, lut_g + bin_list[0] * lut_bin_stride, stage_bytes, &mbar[0]);
+        if (nbins > 1) bulk_load(Rsm1, lut_g + bin_list[1] * lut_bin_stride, stage_bytes, &mbar[1]);
     }
-    float *Rsm = scratch;                                            // [WW][RS]: word 7 + k holds LUT tick k
+    const int nB_lo = tjlo >> 4, nB_hi = (tjhi + K - 1) >> 4;          // 16-tick output blocks, tile-relative
+    const int blk = tid / p.PG, pl = tid - blk * p.PG;
+    const bool t_ok = blk <= nB_hi - nB_lo;
+    const int n0 = NO * (nB_lo + blk);
+    u64 acc[NO];
+#pragma unroll
+    for (int i = 0; i < NO; ++i) acc[i] = 0ull;
     for (int bi = 0; bi < nbins; ++bi) {
         const int c = bin_list[bi];
-        __syncthreads();                                             // previous bin's readers are done
-        const float4 *src = (const float4 *)(a.lut + (size_t)c * WW * RS);
-        for (int i = tid; i < WW * RS / 4; i += NT) ((float4 *)Rsm)[i] = __ldg(src + i);
-        __syncthreads();
-        const int jlo_c = bin_jlo[c], jhi_c = bin_jhi[c];
-        const float *Crow = Csm + c * CJ;
-#pragma unroll
-        for (int s = 0; s < TPT; ++s) {
-            if (!t_ok[s]) continue;
-            const int n8 = 8 * t_nB[s];
-            // j blocks whose 8x8 (n, j) square meets the band 0 <= n - j < K
-            int jb = max(jlo_c & ~7, ((n8 - (K + 6) + 7) >> 3) << 3);
-            const int jb_end = min(jhi_c & ~7, n8);
-            if (jb > jb_end) continue;
-            const float *rowp = Rsm + t_delta[s] * RS;
-            int base = n8 - jb;                                      // window words [base, base+16)
-            float A[8], B[8], cv[8];
-            load8(B, rowp + base + 8);
-            while (true) {
-                load8(A, rowp + base);  load8(cv, Crow + jb);
-                fma_block(acc[s], cv, A, B);
-                jb += 8;  base -= 8;
-                if (jb > jb_end) break;
-                load8(B, rowp + base);  load8(cv, Crow + jb);
-                fma_block(acc[s], cv, B, A);
-                jb += 8;  base -= 8;
-                if (jb > jb_end) break;
+        float *Rsm = (bi & 1) ? Rsm1 : Rsm0;
+        mbar_wait(&mbar[bi & 1], (uint32_t)((bi >> 1) & 1));
+        if (t_ok) {
+            const int jlo_c = bin_jlo[c], jhi_c = bin_jhi[c];
+            // groups of 8 charges whose taps k = n - j meet [0, K) for some of this task's outputs
+            int jb = max(jlo_c & ~7, (n0 - K + 1) & ~7);
+            const int jb_end = min(jhi_c & ~7, n0 + 8);
+            if (jb <= jb_end) {
+                const float *Crow = Csm + c * CJ;
+                // window of 24 pair-words starting at LUT tick n0 - jb - 8, i.e. word n0 - jb + 8 of the row
+                const float *w = Rsm + (pl * RS + (n0 - jb + LUT_OFF - 8)) * 2;
+                u64 G0[8], G1[8], G2[8], cv[8];
+                load8w(G1, w + 16);  load8w(G2, w + 32);
+                while (true) {
+                    load8w(G0, w);  load8c(cv, Crow + jb);
+                    fma_step(acc, cv, G0, G1, G2);
+                    jb += 8;  w -= 16;
+                    if (jb > jb_end) break;
+                    load8w(G2, w);  load8c(cv, Crow + jb);
+                    fma_step(acc, cv, G2, G0, G1);
+                    jb += 8;  w -= 16;
+                    if (jb > jb_end) break;
+                    load8w(G1, w);  load8c(cv, Crow + jb);
+                    fma_step(acc, cv, G1, G2, G0);
+                    jb += 8;  w -= 16;
+                    if (jb > jb_end) break;
+                }
             }
+        }
+        __syncthreads();                                             // every reader is done with this stage
+        if (tid == 0 && bi + 2 < nbins) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            bulk_load(Rsm, lut_g + bin_list[bi + 2] * lut_bin_stride, stage_bytes, &mbar[bi & 1]);
         }
     }
 
     // ------------------------------------------------------------------ phase 4: partial waveforms out
+    if (t_ok) {
+        const int d0 = 2 * (g * p.PG + pl);
+        float lo[NO], hi[NO];
 #pragma unroll
-    for (int s = 0; s < TPT; ++s) {
-        if (!t_ok[s]) continue;
-        float *dst = a.partial + ((size_t)tile * WW + t_delta[s]) * p.tile_ticks + 8 * t_nB[s];
-        *(float4 *)dst = make_float4(acc[s][0], acc[s][1], acc[s][2], acc[s][3]);
-        *(float4 *)(dst + 4) = make_float4(acc[s][4], acc[s][5], acc[s][6], acc[s][7]);
+        for (int i = 0; i < NO; ++i) {
+            lo[i] = __uint_as_float((unsigned)(acc[i] & 0xffffffffull));
+            hi[i] = __uint_as_float((unsigned)(acc[i] >> 32));
+        }
+        if (d0 < WW) {
+            float4 *dst = (float4 *)(a.partial + ((size_t)tile * WW + d0) * p.tile_ticks + n0);
+#pragma unroll
+            for (int q = 0; q < NO / 4; ++q) dst[q] = make_float4(lo[4 * q], lo[4 * q + 1], lo[4 * q + 2], lo[4 * q + 3]);
+        }
+        if (d0 + 1 < WW) {
+            float4 *dst = (float4 *)(a.partial + ((size_t)tile * WW + d0 + 1) * p.tile_ticks + n0);
+#pragma unroll
+            for (int q = 0; q < NO / 4; ++q) dst[q] = make_float4(hi[4 * q], hi[4 * q + 1], hi[4 * q + 2], hi[4 * q + 3]);
+        }
     }
-    if (tid == 0 && blockIdx.y == 0) { a.tile_range[2 * tile] = nB_lo; a.tile_range[2 * tile + 1] = nB_hi; }
+    if (tid == 0 && g == 0) { a.tile_range[2 * tile] = nB_lo; a.tile_range[2 * tile + 1] = nB_hi; }
 }
 
 size_t current_smem_bytes(const DevParams &p, int &CJ, int &NEP, int &NB2P)
@@ -328,10 +394,10 @@ size_t current_smem_bytes(const DevParams &p, int &CJ, int &NEP, int &NB2P)
     CJ = p.Jc;
     NEP = ((2 * (p.nb + 1) + p.Jc + 1) + 3) & ~3;
     NB2P = (p.NB2 + 3) & ~3;
-    size_t scratch = (size_t)p.WW * p.RS;
+    size_t scratch = (size_t)2 * p.PG * p.RS * 2;
     size_t splat = (size_t)SB * (NEP + NB2P + CJ);
     if (splat > scratch) scratch = splat;
-    size_t ints = 3 * (size_t)p.NB2 + p.WW + 8;
+    size_t ints = 3 * (size_t)p.NB2 + 8 + 4;                      // bin tables, misc, two 64-bit mbarriers
     size_t bytes = ((size_t)p.NB2 * CJ + scratch) * 4 + ints * 4;
     bytes = (bytes + 15) & ~(size_t)15;
     return bytes + sizeof(SegLocal) * SEGCAP;
@@ -377,4 +443,4 @@ size_t lartpc_current_smem(const DevParams &p)
     int a, b, c;
     return current_smem_bytes(p, a, b, c);
 }
-int lartpc_current_tasks_per_group() { return NT * TPT; }
+int lartpc_current_threads() { return NT; }

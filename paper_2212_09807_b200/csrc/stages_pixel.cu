@@ -59,7 +59,7 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
             for (int c = c_lo; c <= c_hi; ++c) {
                 if (!((m >> c) & 1ull)) continue;
                 const int tix = s_tile0[d] + __popcll(m & ((1ull << c) - 1ull));
-                const int nrel = n - c * p.Jc, blk = nrel >> 3;
+                const int nrel = n - c * p.Jc, blk = nrel >> 4;
                 if (blk >= tile_range[2 * tix] && blk <= tile_range[2 * tix + 1])
                     sum += partial[((size_t)tix * p.WW + d) * p.tile_ticks + nrel];
             }
