@@ -62,7 +62,7 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
     LARTPC_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
     if (prop.major != 10) return LARTPC_ERR_DEVICE;
     const int nb = prm->bins_per_pixel, W = prm->window_pixels, K = prm->lut_ticks;
-    if (nb < 1 || W < 1 || (W & 1) == 0 || K < 1 || prm->n_readout_ticks < K || prm->tick_us <= 0 ||
+    if (nb < 1 || nb > 15 || W < 1 || (W & 1) == 0 || K < 1 || prm->n_readout_ticks < K || prm->tick_us <= 0 ||
         prm->pixel_pitch_cm <= 0 || prm->sample_step_cm <= 0 || prm->adc_bits < 1 || prm->adc_bits > 12 ||
         prm->max_hits_per_pixel < 1 || prm->hold_ticks < 0 || prm->v_drift_cm_us <= 0)
         return LARTPC_ERR_BAD_ARGUMENT;

@@ -22,7 +22,8 @@ namespace {
 constexpr int NT = 256;          // threads per CTA (two CTAs per SM)
 constexpr int NO = 16;           // output ticks per response task
 constexpr int LUT_OFF = 16;      // LUT tick k sits at word LUT_OFF + k of its zero-padded row
-constexpr int SB = 32;           // samples per splat batch
+constexpr int SB = 64;           // samples per splat batch
+constexpr int XS = 16;           // row length of the per-sample x / y weight tables (bins_per_pixel <= 15)
 constexpr int SEGCAP = 32;       // segments staged per batch
 
 struct CurrentArgs {
@@ -121,7 +122,7 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
     float *Csm = (float *)smem_raw;                                  // [NB2][CJ] charge per (bin, arrival tick)
     float *scratch = Csm + NB2 * CJ;                                 // splat scratch, later the LUT stage
     const int stage_floats = p.PG * RS * 2;                          // one LUT stage: PG pair rows of RS pair-words
-    size_t scratch_floats = max((size_t)2 * stage_floats, (size_t)SB * (a.NEP + a.NB2P + CJ));
+    size_t scratch_floats = max((size_t)2 * stage_floats, (size_t)SB * (2 * XS + CJ));
     int *s_int = (int *)(scratch + scratch_floats);
     int *bin_jlo = s_int, *bin_jhi = s_int + NB2, *bin_list = s_int + 2 * NB2;
     int *s_misc = bin_list + NB2;                                    // [0] n bins, [1] tile jlo, [2] tile jhi
@@ -143,7 +144,7 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
     }
 
     // ------------------------------------------------------------------ phase 1: splat
-    float *erfv = scratch, *wxy = scratch + SB * a.NEP, *wt = wxy + SB * a.NB2P;
+    float *WX = scratch, *WY = scratch + SB * XS, *WT = scratch + 2 * SB * XS;     // [SB][XS], [SB][XS], [SB][CJ]
     for (int l0 = 0; l0 < lcount; l0 += SEGCAP) {
         __syncthreads();
         const int nseg = min(SEGCAP, lcount - l0);
@@ -193,66 +194,61 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
                 continue;
             }
             const int na = L.ahi - L.alo + 1, nbb = L.bhi - L.blo + 1, nj = L.jhi - L.jlo + 1;
-            const int ncell = na * nbb, ncell4 = (ncell + 3) >> 2, nj4 = (nj + 3) >> 2;
-            const int nex = na + 1, ney = nbb + 1, ne = nex + ney + nj + 1;
+            const int na4 = (na + 3) >> 2, nj4 = (nj + 3) >> 2, units = na4 * nbb * nj4;
+            const int truns = (nj + 30) / 31, runs = 1 + truns;       // warp runs per sample: (x | y) and the t pieces
             const float invN = 1.0f / (float)L.N;
-            for (int mu0 = 0; mu0 < L.N; mu0 += SB) {
-                const int nsb = min(SB, L.N - mu0);
-                // (A) erf at every bin / tick edge of the segment's box for each sample of the batch
-                for (int idx = tid; idx < nsb * ne; idx += NT) {
-                    const int ml = idx / ne, e = idx - ml * ne;
+            const int npass = (L.N + SB - 1) / SB, nsb_max = (L.N + npass - 1) / npass;
+            for (int mu0 = 0; mu0 < L.N; mu0 += nsb_max) {
+                const int nsb = min(nsb_max, L.N - mu0);
+                // (A) one-dimensional cell weights of every sample of the batch.  A warp evaluates erf once per bin /
+                // tick edge and takes the difference with its neighbour lane: w = (erf(e+1) - erf(e)) / 2.
+                for (int r = warp; r < nsb * runs; r += NT / 32) {
+                    const int ml = r / runs, k = r - ml * runs;
                     const float f = ((float)(mu0 + ml) + 0.5f) * invN;
-                    float arg;
-                    if (e < nex)            arg = ((float)(L.alo + e) - fmaf(L.ae - L.as, f, L.as)) * L.isT;
-                    else if (e < nex + ney) arg = ((float)(L.blo + e - nex) - fmaf(L.be - L.bs, f, L.bs)) * L.isT;
-                    else                    arg = ((float)(L.jlo + e - nex - ney) - fmaf(L.te - L.ts, f, L.ts)) * L.ist;
-                    erfv[ml * a.NEP + e] = erff(arg);
-                }
-                __syncthreads();
-                // (B) cell weights: wxy = q (Phi_y[b+1]-Phi_y[b]) (Phi_x[a+1]-Phi_x[a]), wt = Phi_t[j+1]-Phi_t[j]
-                for (int idx = tid; idx < nsb * (ncell4 * 4); idx += NT) {
-                    const int ml = idx / (ncell4 * 4), c = idx - ml * (ncell4 * 4);
-                    float w = 0.f;
-                    if (c < ncell) {
-                        const int b = c / na, aa = c - b * na;
-                        const float *E = erfv + ml * a.NEP;
-                        w = 0.25f * L.q * (E[nex + b + 1] - E[nex + b]) * (E[aa + 1] - E[aa]);
+                    if (k == 0) {
+                        const int half = lane >> 4, e = lane & 15;     // lanes 0-15: x edges, 16-31: y edges
+                        const float pos = half ? fmaf(L.be - L.bs, f, L.bs) : fmaf(L.ae - L.as, f, L.as);
+                        const float E = erff(((float)((half ? L.blo : L.alo) + e) - pos) * L.isT);
+                        const float En = __shfl_down_sync(0xffffffffu, E, 1);
+                        if (e < (half ? nbb : na)) (half ? WY : WX)[ml * XS + e] = 0.5f * (En - E);
+                    } else {
+                        const int e = 31 * (k - 1) + lane;            // 32 edges -> 31 weights per run
+                        const float pos = fmaf(L.te - L.ts, f, L.ts);
+                        const float E = erff(((float)(L.jlo + e) - pos) * L.ist);
+                        const float En = __shfl_down_sync(0xffffffffu, E, 1);
+                        if (lane < 31 && e < nj) WT[ml * CJ + e] = 0.5f * L.q * (En - E);
                     }
-                    wxy[ml * a.NB2P + c] = w;
-                }
-                for (int idx = tid; idx < nsb * (nj4 * 4); idx += NT) {
-                    const int ml = idx / (nj4 * 4), jj = idx - ml * (nj4 * 4);
-                    const float *E = erfv + ml * a.NEP + nex + ney;
-                    wt[ml * CJ + jj] = jj < nj ? 0.5f * (E[jj + 1] - E[jj]) : 0.f;
                 }
                 __syncthreads();
-                // (C) accumulate 4 cells x 4 ticks per thread over the batch
-                for (int unit = tid; unit < ncell4 * nj4; unit += NT) {
-                    const int cq = unit / nj4, jq = unit - cq * nj4;
-                    float acc[4][4];
+                // (B) a thread owns 4 cells (consecutive in a) x 4 ticks and adds the batch's outer products to them;
+                // entries past na / nj multiply stale shared memory and are never stored
+                for (int unit = tid; unit < units; unit += NT) {
+                    const int cu = unit / nj4, jq = unit - cu * nj4, b = cu / na4, aq = cu - b * na4;
+                    u64 acc[4][2];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i)
-#pragma unroll
-                        for (int k = 0; k < 4; ++k) acc[i][k] = 0.f;
-                    const float *pw = wxy + cq * 4, *pt = wt + jq * 4;
+                    for (int i = 0; i < 4; ++i) acc[i][0] = acc[i][1] = 0ull;
+                    const float *px = WX + aq * 4, *py = WY + b, *pt = WT + jq * 4;
+#pragma unroll 2
                     for (int ml = 0; ml < nsb; ++ml) {
-                        const float4 w4 = *(const float4 *)(pw + ml * a.NB2P);
-                        const float4 t4 = *(const float4 *)(pt + ml * CJ);
-                        const float wv[4] = {w4.x, w4.y, w4.z, w4.w}, tv[4] = {t4.x, t4.y, t4.z, t4.w};
+                        const float4 x4 = *(const float4 *)(px + ml * XS);
+                        const float y = py[ml * XS];
+                        const ulonglong2 t4 = *(const ulonglong2 *)(pt + ml * CJ);
+                        const float w[4] = {x4.x * y, x4.y * y, x4.z * y, x4.w * y};
 #pragma unroll
-                        for (int i = 0; i < 4; ++i)
-#pragma unroll
-                            for (int k = 0; k < 4; ++k) acc[i][k] = fmaf(wv[i], tv[k], acc[i][k]);
+                        for (int i = 0; i < 4; ++i) {
+                            ffma2(acc[i][0], pack2(w[i]), t4.x);
+                            ffma2(acc[i][1], pack2(w[i]), t4.y);
+                        }
                     }
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
-                        const int c = cq * 4 + i;
-                        if (c < ncell) {
-                            const int b = c / na, aa = c - b * na;
-                            float *row = Csm + ((L.blo + b) * nb + (L.alo + aa)) * CJ + L.jlo + jq * 4;
+                        if (aq * 4 + i < na) {
+                            float *row = Csm + ((L.blo + b) * nb + (L.alo + aq * 4 + i)) * CJ + L.jlo + jq * 4;
+                            const float v[4] = {__uint_as_float((unsigned)acc[i][0]), __uint_as_float((unsigned)(acc[i][0] >> 32)),
+                                                __uint_as_float((unsigned)acc[i][1]), __uint_as_float((unsigned)(acc[i][1] >> 32))};
 #pragma unroll
                             for (int k = 0; k < 4; ++k)
-                                if (jq * 4 + k < nj) row[k] += acc[i][k];
+                                if (jq * 4 + k < nj) row[k] += v[k];
                         }
                     }
                 }
@@ -395,7 +391,7 @@ size_t current_smem_bytes(const DevParams &p, int &CJ, int &NEP, int &NB2P)
     NEP = ((2 * (p.nb + 1) + p.Jc + 1) + 3) & ~3;
     NB2P = (p.NB2 + 3) & ~3;
     size_t scratch = (size_t)2 * p.PG * p.RS * 2;
-    size_t splat = (size_t)SB * (NEP + NB2P + CJ);
+    size_t splat = (size_t)SB * (2 * XS + CJ);
     if (splat > scratch) scratch = splat;
     size_t ints = 3 * (size_t)p.NB2 + 8 + 4;                      // bin tables, misc, two 64-bit mbarriers
     size_t bytes = ((size_t)p.NB2 * CJ + scratch) * 4 + ints * 4;
