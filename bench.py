@@ -259,8 +259,8 @@ def run_ours(args):
     e2e_ms = float(te.item())
 
     if rank == 0:
-        s4_ms = stage_ms["induced_current"] / max(stage_n["induced_current"], 1)
-        fma_per_launch = fma / max(stage_n["induced_current"], 1)
+        s4_ms = stage_ms["induced_current_response"] / max(stage_n["induced_current_response"], 1)
+        fma_per_launch = fma / max(stage_n["induced_current_response"], 1)
         peak = max(peak_scalar, peak_packed)
         achieved = 2.0 * fma_per_launch / (s4_ms * 1e-3) / 1e12 if s4_ms > 0 else 0.0
         traffic = None
@@ -286,12 +286,12 @@ def run_ours(args):
                     "h2d_bytes_per_step": 9 * 4 * n, "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches),
             "clocks": clk,
-            "roofline": {"kernel": "induced_current (S4)", "bound": "alu", "achieved": achieved, "peak": peak,
+            "roofline": {"kernel": "response_kernel (S4 induced current, response part)", "bound": "alu", "achieved": achieved, "peak": peak,
                          "unit": "TFLOP/s", "frac": achieved / peak if peak else None, "traffic": traffic,
                          "peak_source": "lartpc_measure_fp32_peak on this GPU (scalar FFMA %.1f, packed FFMA2 %.1f)"
                                         % (peak_scalar, peak_packed),
                          "launch_ms": s4_ms, "flops_per_launch": 2.0 * fma_per_launch,
-                         "share_of_step": stage_ms["induced_current"] / max(sum(stage_ms.values()), 1e-9)},
+                         "share_of_step": stage_ms["induced_current_response"] / max(sum(stage_ms.values()), 1e-9)},
         }
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"], _, _ = time_oracle(wl, args.cpu_sample)

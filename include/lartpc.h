@@ -119,22 +119,31 @@ typedef struct {
     int32_t max_ticks;                  /* longest signal: max(jt1 - jt0 + 1) + lut_ticks - 1 */
     int64_t total_npix;                 /* offsets[n] */
     int64_t n_active_segments;          /* segments with a non-empty rectangle */
-    int64_t n_tiles;                    /* charge tiles (charged pixel x arrival-tick chunk) S4 will process */
+    int64_t n_tiles;                    /* charge tiles (charged pixel x window of arrival ticks) S4 will process */
     int64_t n_pairs;                    /* (segment, charged pixel) incidences */
     int64_t n_active_pixels;            /* pixels that can receive current */
     int64_t total_samples;              /* sum of the per-pixel waveform lengths S5 will write */
     int32_t tile_targets;               /* W*W: partial waveforms per tile */
     int32_t tile_ticks;                 /* readout ticks per partial waveform (padded) */
+    int32_t tile_charge_floats;         /* 32-bit words of one tile's packed charge lattice (lartpc_signals_t.charge) */
+    int32_t reserved;
 } lartpc_pixmap_info_t;
 
-/* S4 output: per-tile partial waveforms, float32 [n_tiles][tile_targets][tile_ticks] (electrons per
- * tick).  Tile (charged pixel P, chunk c) holds the current its charge induces on the W x W pixels
- * around P during readout ticks [c * chunk_ticks, c * chunk_ticks + tile_ticks).  The tile -> pixel
- * map is part of the sim's plan.  `tile_range` int32[n_tiles][2] = first / last 16-tick block written. */
+/* S4 output.  A tile is (charged pixel P, window of lartpc_chunk_ticks() arrival ticks that starts at
+ * j_start = first arrival tick on P, rounded down to even, + a multiple of the window length).
+ *   charge      float32 [n_tiles][tile_charge_floats]: the charge lattice of eq. (3.8) in expectation, C[bin][j]
+ *               electrons per (x, y) LUT bin of P and arrival tick, packed per tile as a header (bins, charge
+ *               groups, first / last output block), one item per non-empty bin (bin, first tick, groups of 4
+ *               ticks, row offset) and the charge rows themselves;
+ *   partial     float32 [n_tiles][tile_targets][tile_ticks] (electrons per tick): the current that charge
+ *               induces on the W x W pixels around P during readout ticks [j_start, j_start + tile_ticks);
+ *   tile_range  int32 [n_tiles][2] = first / last 16-tick block of `partial` written (first > last: no charge).
+ * The tile -> pixel map is part of the sim's plan. */
 typedef struct {
-    int64_t  tile_capacity;             /* host value: tiles the two buffers can hold */
+    int64_t  tile_capacity;             /* host value: tiles the three buffers can hold */
     float   *partial;
     int32_t *tile_range;
+    float   *charge;
 } lartpc_signals_t;
 
 /* S5 output: one waveform per active pixel, sorted by pixel id. */
@@ -184,7 +193,7 @@ void lartpc_sim_destroy(lartpc_sim_t *sim);
 /* Optional mask of disabled channels: HOST array of global pixel ids; S6 emits no hit for them. */
 int  lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *pixel_ids_host, int64_t n);
 
-/* Arrival ticks per charge tile (chunk_ticks) chosen for this LUT shape. */
+/* Arrival ticks per charge tile (window length) chosen for this LUT shape. */
 int  lartpc_chunk_ticks(const lartpc_sim_t *sim);
 
 /* Recommended workspace for lartpc_run_spill on up to max_segments segments. */
@@ -206,7 +215,8 @@ int  lartpc_pixels_from_segments(lartpc_sim_t *sim, const lartpc_segments_t *seg
                                  const lartpc_drifted_t *drifted, int64_t n,
                                  lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, void *stream);
 
-/* S4: needs out->tile_capacity >= info.n_tiles. */
+/* S4: needs out->tile_capacity >= info.n_tiles.  Two kernels: the charge lattice of every tile (splat), then the
+ * response of the W x W pixels around it (persistent, LUT rows streamed through shared memory). */
 int  lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t *drifted, const lartpc_pixmap_t *pixmap,
                             int64_t n, lartpc_signals_t *out, void *stream);
 
@@ -236,10 +246,11 @@ int  lartpc_measure_fp32_peak(int variant, double *tflops, void *stream);
  * CUDA events recorded on `stream` and adds the elapsed times up per stage after its final synchronisation
  * (a few microseconds of overhead per launch; off by default).  lartpc_get_stage_ms returns, for the last
  * run_spill, ms[s] = device milliseconds and launches[s] = times the stage ran (one per TPC batch for S3-S6):
- * s = 0 quench, 1 drift, 2 pixel mapping + plan, 3 induced current, 4 per-pixel sum, 5 electronics.
+ * s = 0 quench, 1 drift, 2 pixel mapping + plan, 3 induced current: charge lattice, 4 induced current: response,
+ * 5 per-pixel sum, 6 electronics.
  * fma_current = multiply-adds the S4 response needs for the charge it found (counted on the device:
  * non-zero charge cells x in-plane target pixels x lut_ticks), the numerator of its roofline figure. */
-#define LARTPC_N_STAGES 6
+#define LARTPC_N_STAGES 7
 int  lartpc_set_profiling(lartpc_sim_t *sim, int on);
 int  lartpc_get_stage_ms(const lartpc_sim_t *sim, double ms[LARTPC_N_STAGES], int64_t launches[LARTPC_N_STAGES],
                          double *fma_current);

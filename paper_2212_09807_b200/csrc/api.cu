@@ -6,8 +6,8 @@
 #include <new>
 #include "common.cuh"
 
-size_t lartpc_current_smem(const DevParams &p);
-int lartpc_current_threads();
+size_t lartpc_splat_smem(const DevParams &p);
+size_t lartpc_response_smem(const DevParams &p);
 
 static thread_local char g_last_cuda_error[256] = "";
 long long g_lartpc_launches = 0;
@@ -43,13 +43,63 @@ static void sim_free(lartpc_sim *s)
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
     cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->scan_tmp);
     cudaFree(s->d_counters); cudaFree(s->disabled_mask); cudaFree(s->elec_slots); cudaFree(s->elec_offs);
-    cudaFree(s->d_fma);
+    cudaFree(s->d_fma); cudaFree(s->d_work); cudaFree(s->pix_jmin); cudaFree(s->d_end_row);
     for (cudaEvent_t e : s->ev_pool) cudaEventDestroy(e);
     if (s->h_counters) cudaFreeHost(s->h_counters);
     delete s;
 }
 
 extern "C" void lartpc_sim_destroy(lartpc_sim_t *sim) { sim_free(sim); }
+
+
+// Output blocks at both ends of a tile have fewer taps inside [0, K) than the interior ones, and consumer threads are
+// laid out slot-major (slot = tid / PG), so giving slot k block k would load the four SM sub-partitions (warp % 4)
+// unevenly and the busiest one would set the pace.  Pick, once per geometry, the block of every slot by a seeded
+// hill-climb that minimises the mean of max/mean sub-partition load over typical charge rows (1..16 groups).
+static void balance_blocks(const DevParams &p, unsigned char *blk_of_slot)
+{
+    const int nblk = p.nblk_max, PG = p.PG, K = p.K;
+    std::vector<int> perm(nblk);
+    for (int b = 0; b < nblk; ++b) perm[b] = b;
+    std::vector<double> share(4 * nblk, 0.0);
+    for (int t = 0; t < PG * nblk && t < RESP_CONSUMERS; ++t) share[((t / 32) % 4) * nblk + t / PG] += 1.0;
+    std::vector<std::vector<double>> prof;
+    const int jb0s[4] = {0, 2, 6, 10};
+    for (int ng = 1; ng <= 16; ++ng)
+        for (int jb0 : jb0s) {
+            std::vector<double> w(nblk);
+            for (int b = 0; b < nblk; ++b) {
+                const int n0 = RESP_NO * b;
+                const int lo = std::max(0, (n0 - jb0 - K - 2 + 3) >> 2), hi = std::min(ng - 1, (n0 - jb0 + RESP_NO - 1) >> 2);
+                w[b] = std::max(0, hi - lo + 1);
+            }
+            prof.push_back(w);
+        }
+    auto cost = [&](const std::vector<int> &pm) {
+        double tot = 0.0;
+        for (const auto &w : prof) {
+            double mx = 0.0, sum = 0.0;
+            for (int sp = 0; sp < 4; ++sp) {
+                double l = 0.0;
+                for (int k = 0; k < nblk; ++k) l += share[sp * nblk + k] * w[pm[k]];
+                mx = std::max(mx, l);  sum += l;
+            }
+            if (sum > 0.0) tot += mx / (sum / 4.0);
+        }
+        return tot;
+    };
+    double best = cost(perm);
+    uint64_t rng = 0x9E3779B97F4A7C15ull;
+    auto next = [&]() { rng = rng * 6364136223846793005ull + 1442695040888963407ull; return (uint32_t)(rng >> 33); };
+    for (int it = 0; it < 4000 && nblk > 1; ++it) {
+        const int i = next() % nblk, j = next() % nblk;
+        if (i == j) continue;
+        std::swap(perm[i], perm[j]);
+        const double c = cost(perm);
+        if (c < best) best = c; else std::swap(perm[i], perm[j]);
+    }
+    for (int k = 0; k < 256; ++k) blk_of_slot[k] = (unsigned char)(k < nblk ? perm[k] : 255);
+}
 
 extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t *tpcs, int n_tpcs,
                                  const float *lut_host, size_t lut_elems, lartpc_sim_t **out)
@@ -84,35 +134,37 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
     p.recomb_model = prm->recomb_model;
     p.nb = nb; p.W = W; p.H = (W - 1) / 2; p.K = K; p.WW = W * W; p.NB2 = nb * nb;
     p.n_ticks = prm->n_readout_ticks;  p.j_max = p.n_ticks - K;
-    // S4 geometry.  A response task is (pair of target pixels, 16 output ticks); a CTA group of NT threads covers PG
-    // pairs x nblk_max blocks.  Jc (arrival ticks per tile, multiple of 8, at most 120) is chosen to minimise the number
-    // of pair groups per arrival tick, because every group repeats the tile's splat.
-    p.RS = K + 38;
+    // S4 geometry.  A response task is (pair of target pixels, RESP_NO output ticks); the consumer threads of one CTA
+    // cover PG pairs x nblk_max blocks, and a tile needs n_groups passes to cover all pairs.  Jc (arrival ticks per
+    // tile, multiple of 4, at most 120) is chosen to maximise the arrival ticks covered per pass.
+    p.RS = LUT_OFF + K + 22;
     while ((p.RS & 1) != 0 || ((p.RS >> 1) & 1) == 0) ++p.RS;               // RS = 2 * odd: conflict-free LDS.128 rows
-    const int n_pairs = (p.WW + 1) / 2, nthreads = lartpc_current_threads();
+    const int n_pairs = (p.WW + 1) / 2, ncons = RESP_CONSUMERS;
     const size_t smem_limit = (size_t)prop.sharedMemPerBlockOptin;
     double best = 0.0;
-    int best_jc = 0;
-    for (int jc = 120; jc >= 8; jc -= 8) {
-        const int nblk = (jc + K - 2) / 16 + 1;
-        if (nblk > nthreads) continue;
+    int best_groups = 0;
+    for (int g = 1; g <= n_pairs; ++g) {
         DevParams q = p;
-        q.Jc = jc;  q.PG = std::min(n_pairs, nthreads / nblk);  q.n_groups = (n_pairs + q.PG - 1) / q.PG;
-        q.PG = (n_pairs + q.n_groups - 1) / q.n_groups;                     // even out the groups
-        if (lartpc_current_smem(q) > smem_limit) continue;
-        const double score = (double)jc / q.n_groups;
-        if (score > best) { best = score; best_jc = jc; }
+        q.n_groups = g;  q.PG = (n_pairs + g - 1) / g;
+        int jc = std::min(120, RESP_NO * (ncons / q.PG) - K + 1) & ~3;
+        if (jc < 8) continue;
+        q.Jc = jc;  q.CJ = jc + 4;
+        q.nblk_max = (jc + K - 2) / RESP_NO + 1;
+        if (q.nblk_max > 255) continue;
+        if (lartpc_splat_smem(q) > smem_limit || lartpc_response_smem(q) > smem_limit) continue;
+        const double score = (double)jc / g;
+        if (score > best) { best = score; best_groups = g; }
     }
-    if (best_jc == 0) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
-    p.Jc = best_jc;
-    p.nblk_max = (p.Jc + K - 2) / 16 + 1;  p.tile_ticks = 16 * p.nblk_max;
-    p.PG = std::min(n_pairs, nthreads / p.nblk_max);  p.n_groups = (n_pairs + p.PG - 1) / p.PG;
-    p.PG = (n_pairs + p.n_groups - 1) / p.n_groups;  p.NP = p.n_groups * p.PG;
-    p.n_chunks = (p.j_max + p.Jc) / p.Jc;
-    if (p.n_chunks > 64) {                                                  // chunk masks are 64-bit
+    if (best_groups == 0) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    p.n_groups = best_groups;  p.PG = (n_pairs + p.n_groups - 1) / p.n_groups;  p.NP = p.n_groups * p.PG;
+    p.Jc = std::min(120, RESP_NO * (ncons / p.PG) - K + 1) & ~3;  p.CJ = p.Jc + 4;
+    p.nblk_max = (p.Jc + K - 2) / RESP_NO + 1;  p.tile_ticks = RESP_NO * p.nblk_max;
+    p.slab_floats = (SLAB_HDR + 2 * p.NB2 + p.NB2 * (4 + p.CJ) + 3) & ~3;
+    if (p.j_max / p.Jc + 2 > MAX_WINDOWS) {                                 // window masks are 128 bits
         sim_free(s);
         return LARTPC_ERR_UNSUPPORTED;
     }
+    balance_blocks(p, s->blk_of_slot);
     p.n_tpcs = n_tpcs;
     p.gain_mv_per_ke = prm->gain_mv_per_ke; p.v_cm = prm->v_cm_mv; p.v_ref = prm->v_ref_mv; p.v_ped = prm->v_pedestal_mv;
     p.adc_full = ldexp(1.0, prm->adc_bits);  p.threshold = prm->threshold_e;
@@ -141,8 +193,8 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
     s->n_cp = cp; s->n_pix = pix;
 
     // LUT re-laid out as [bin c = cb*nb+ca][pair q][RS][2]: pair q interleaves the rows of targets d = 2q and 2q+1
-    // (d = dyi*W + dxi; row (c, d) is R[cy = nb*dyi + cb][cx = nb*dxi + ca][.]), LUT tick k at pair-word 16 + k with
-    // zero padding around it.  S4 stages the PG pair rows of one bin with a single bulk copy, reads 24-tap windows
+    // (d = dyi*W + dxi; row (c, d) is R[cy = nb*dyi + cb][cx = nb*dxi + ca][.]), LUT tick k at pair-word LUT_OFF + k
+    // with zero padding around it.  S4 stages the PG pair rows of one bin with a single bulk copy, reads 20-tap windows
     // with aligned 128-bit loads and feeds both targets of a pair to one packed f32x2 multiply-add.
     std::vector<float> re((size_t)p.NB2 * p.NP * p.RS * 2, 0.f);
     const int NB = W * nb;
@@ -152,9 +204,12 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
                 for (int dxi = 0; dxi < W; ++dxi) {
                     const int d = dyi * W + dxi;
                     const float *src = lut_host + ((size_t)(nb * dyi + cb) * NB + (nb * dxi + ca)) * K;
-                    float *dst = re.data() + (((size_t)(cb * nb + ca) * p.NP + d / 2) * p.RS + 16) * 2 + (d & 1);
+                    float *dst = re.data() + (((size_t)(cb * nb + ca) * p.NP + d / 2) * p.RS + LUT_OFF) * 2 + (d & 1);
                     for (int k = 0; k < K; ++k) dst[2 * k] = src[k];
                 }
+    for (int c = 0; c < p.NB2; ++c)
+        for (int g = 0; g < p.n_groups; ++g)
+            memcpy(&re[((size_t)c * p.NP + (size_t)g * p.PG) * p.RS * 2], &g, sizeof(int));
 #define SIM_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { \
         lartpc_note_cuda_error(_e, __FILE__, __LINE__); sim_free(s); return LARTPC_ERR_CUDA; } } while (0)
     SIM_TRY(cudaMalloc(&s->d_lut, sizeof(float) * re.size()));
@@ -165,7 +220,14 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
     SIM_TRY(cudaMalloc(&s->pix_start, sizeof(int32_t) * cp));
     SIM_TRY(cudaMalloc(&s->pix_tile0, sizeof(int32_t) * cp));
     SIM_TRY(cudaMalloc(&s->pix_cursor, sizeof(int32_t) * cp));
-    SIM_TRY(cudaMalloc(&s->pix_mask, sizeof(unsigned long long) * cp));
+    SIM_TRY(cudaMalloc(&s->pix_mask, sizeof(unsigned long long) * MASK_WORDS * cp));
+    SIM_TRY(cudaMalloc(&s->pix_jmin, sizeof(int32_t) * cp));
+    SIM_TRY(cudaMalloc(&s->d_work, sizeof(int)));
+    {
+        const int end_row[4] = {0, 0, 2, 0};                                // {first tick, groups, flags = END, tile}
+        SIM_TRY(cudaMalloc(&s->d_end_row, sizeof(end_row)));
+        SIM_TRY(cudaMemcpy(s->d_end_row, end_row, sizeof(end_row), cudaMemcpyHostToDevice));
+    }
     SIM_TRY(cudaMalloc(&s->act_first, sizeof(int32_t) * pix));
     SIM_TRY(cudaMalloc(&s->act_last, sizeof(int32_t) * pix));
     SIM_TRY(cudaMalloc(&s->act_slot, sizeof(int32_t) * pix));
@@ -227,7 +289,9 @@ extern "C" int lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t 
     if (!sim || !dr || !pm || !out) return LARTPC_ERR_BAD_ARGUMENT;
     if (!sim->have_plan || n != sim->plan_n) return LARTPC_ERR_ORDER;
     if (out->tile_capacity < sim->n_tiles) return LARTPC_ERR_CAPACITY;
-    int rc = launch_current(sim, dr, pm, n, out, (cudaStream_t)stream);
+    if (sim->n_tiles > 0 && (!out->partial || !out->tile_range || !out->charge)) return LARTPC_ERR_BAD_ARGUMENT;
+    int rc = launch_current_splat(sim, dr, pm, n, out, (cudaStream_t)stream);
+    if (rc == 0) rc = launch_current_response(sim, out, (cudaStream_t)stream);
     if (rc == 0) sim->have_signals = true;
     return rc;
 }
@@ -337,11 +401,12 @@ extern "C" int lartpc_get_stage_ms(const lartpc_sim_t *sim, double ms[LARTPC_N_S
 extern "C" size_t lartpc_workspace_bytes(const lartpc_sim_t *sim, int64_t max_segments)
 {
     if (!sim) return 0;
-    // per segment: n_e, dEdx (8) + drifted (64) + pixmap (12*4 + 8) = 128 B, rounded up to 160.  The tile partials
-    // and waveforms of the largest TPC batch depend on the data; measured on the BASELINE configs they stay under
-    // 1.3 tiles per segment of the busiest TPC, so 3 GiB + 4 KiB per segment covers them with room to spare
-    // (configs[3]: ~22 GiB of the 180 GB).  run_spill halves its TPC batches until they fit whatever it is given.
-    return (size_t)max_segments * (160 + 4096) + ((size_t)3 << 30);
+    // per segment: n_e, dEdx (8) + drifted (64) + pixmap (12*4 + 8) = 128 B, rounded up to 160.  The tile buffers
+    // (packed charge + partial waveforms, ~58 KB per tile for 5x5 x 200) and the waveforms of the largest TPC batch
+    // depend on the data; on the BASELINE configs there are up to ~1.5 tiles per segment of a batch, so 2 GiB +
+    // 16 KiB per segment lets run_spill take several TPCs per batch; it halves its batches until they fit whatever
+    // it is given (one TPC of configs[3] needs ~6 GiB).
+    return (size_t)max_segments * (160 + 16384) + ((size_t)2 << 30);
 }
 
 extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, uint64_t seed,
@@ -397,6 +462,7 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
         sig.tile_capacity = info.n_tiles;
         sig.partial = ar.take<float>(info.n_tiles * p.WW * p.tile_ticks);
         sig.tile_range = ar.take<int32_t>(info.n_tiles * 2);
+        sig.charge = ar.take<float>(info.n_tiles * p.slab_floats);
         lartpc_waveforms_t wf;
         wf.pixel_capacity = info.n_active_pixels;  wf.sample_capacity = info.total_samples;
         wf.pixel_id = ar.take<int32_t>(info.n_active_pixels);
@@ -409,7 +475,7 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
         lartpc_hits_t h = *out;
         h.hits_per_pixel = ar.take<int32_t>(info.n_active_pixels);
         h.q_pixel = ar.take<float>(info.n_active_pixels);
-        if (!sig.partial || !sig.tile_range || !wf.samples || !slots || !offs || !h.q_pixel) {
+        if (!sig.partial || !sig.tile_range || !sig.charge || !wf.samples || !slots || !offs || !h.q_pixel) {
             if (tpc_hi - tpc_lo <= 1) return LARTPC_ERR_CAPACITY;       // one TPC does not fit the workspace
             batch = std::max(1, (tpc_hi - tpc_lo) / 2);
             continue;
@@ -419,13 +485,16 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
         stt.n_active_pixels += info.n_active_pixels;  stt.total_samples += info.total_samples;
         stt.n_batches += 1;
         tm.begin(3);
-        if ((rc = launch_current(sim, &dr, &pm, n, &sig, st)) != 0) return rc;
+        if ((rc = launch_current_splat(sim, &dr, &pm, n, &sig, st)) != 0) return rc;
+        tm.end();
+        tm.begin(4);
+        if ((rc = launch_current_response(sim, &sig, st)) != 0) return rc;
         tm.end();
         sim->have_signals = true;
-        tm.begin(4);
+        tm.begin(5);
         if ((rc = launch_sum(sim, &sig, &wf, st)) != 0) return rc;
         tm.end();
-        tm.begin(5);
+        tm.begin(6);
         if ((rc = launch_electronics(sim, &wf, seed, &h, slots, offs, 0, st)) != 0) return rc;
         tm.end();
         tpc_lo = tpc_hi;

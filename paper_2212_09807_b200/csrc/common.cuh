@@ -22,11 +22,12 @@ struct DevParams {
     int recomb_model;
     int nb, W, H, K, WW, NB2;        // bins per pixel, window pixels, half window, LUT ticks, W*W, nb*nb
     int n_ticks, j_max;              // readout ticks, last arrival tick inside the window (n_ticks - K)
-    int Jc, n_chunks;                // arrival ticks per charge tile, chunks covering [0, j_max]
-    int nblk_max, tile_ticks;        // 16-tick output blocks per tile, 16 * nblk_max
-    int RS;                          // padded LUT row length in pair-words: [16 zeros][K][>= 22 zeros], RS = 2 * odd
-    int PG, NP;                      // target pairs per CTA group; pairs incl. padding = n_groups * PG
-    int n_groups;                    // pair groups per tile = gridDim.y of S4 (1 for W = 5, K = 200)
+    int Jc, CJ;                      // arrival ticks per charge tile; row stride of the tile's charge lattice (Jc + 4)
+    int nblk_max, tile_ticks;        // output blocks of RESP_NO ticks per tile, RESP_NO * nblk_max
+    int RS;                          // padded LUT row length in pair-words: [20 zeros][K][>= 22 zeros], RS = 2 * odd
+    int PG, NP;                      // target pairs per consumer group; pairs incl. padding = n_groups * PG
+    int n_groups;                    // pair groups per tile = response passes over a tile (1 for W = 5, K = 200)
+    int slab_floats;                 // packed charge lattice of one tile: header, bin items, charge rows
     int n_tpcs;
     // electronics
     double gain_mv_per_ke, v_cm, v_ref, v_ped, adc_full, threshold;
@@ -44,8 +45,15 @@ struct DevTpc {
 
 struct SegPtrs { const float *xs, *ys, *zs, *ts, *xe, *ye, *ze, *te, *dE; };
 
-// charge tile = (charged pixel, arrival-tick chunk)
-struct TileDesc { int tpc, px, py, chunk; };
+// charge tile = (charged pixel, window of Jc arrival ticks starting at j_start = first tick of the pixel + win * Jc)
+struct TileDesc { int tpc, px, py, j_start; };
+
+constexpr int MASK_WORDS = 2;        // window masks are 128 bits per charged pixel
+constexpr int MAX_WINDOWS = 64 * MASK_WORDS;
+constexpr int LUT_OFF = 20;          // LUT tick k sits at pair-word LUT_OFF + k of its zero-padded row
+constexpr int SLAB_HDR = 4;          // slab header ints: bins, charge groups, first / last output block
+constexpr int RESP_NO = 14;          // output ticks per response task (one thread: RESP_NO ticks x 2 target pixels)
+constexpr int RESP_CONSUMERS = 256;  // consumer threads of the response kernel (8 warps, two per SM sub-partition)
 
 // device counters written by the planning kernels (mirrored to pinned host memory)
 enum {
@@ -64,7 +72,8 @@ struct lartpc_sim {
     int32_t pix_id_base = 0;
     // dense planning arrays
     int32_t *pix_count = nullptr, *pix_start = nullptr, *pix_tile0 = nullptr, *pix_cursor = nullptr;
-    unsigned long long *pix_mask = nullptr;
+    int32_t *pix_jmin = nullptr;         // first arrival tick on the charged pixel (window origin, rounded down to even)
+    unsigned long long *pix_mask = nullptr;   // [n_cp][MASK_WORDS] windows that hold charge
     int32_t *act_first = nullptr, *act_last = nullptr, *act_slot = nullptr;
     // growable planning arrays
     int32_t *pair_seg = nullptr;  int64_t pair_cap = 0;
@@ -85,10 +94,13 @@ struct lartpc_sim {
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;
     std::vector<int> ev_stage;           // stage of the event pair (2i, 2i+1)
-    double stage_ms[LARTPC_N_STAGES] = {0, 0, 0, 0, 0, 0};
-    int64_t stage_launches[LARTPC_N_STAGES] = {0, 0, 0, 0, 0, 0};
+    double stage_ms[LARTPC_N_STAGES] = {};
+    int64_t stage_launches[LARTPC_N_STAGES] = {};
     double fma_current = 0.0;
     unsigned long long *d_fma = nullptr; // device counter of S4 multiply-adds
+    int *d_work = nullptr;               // work-queue cursor of the persistent response kernel
+    int *d_end_row = nullptr;            // 16-byte row header with the END flag (terminates the consumers)
+    unsigned char blk_of_slot[256];      // response kernel: output block of consumer-thread slot (balances the SM sub-partitions)
 };
 
 // ---- IEEE-exact float64 helpers (never contracted into FMA) -----------------------------------
@@ -122,8 +134,9 @@ int launch_drift(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, const
                  cudaStream_t st);
 int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drifted_t *dr, int64_t n,
                 int tpc_lo, int tpc_hi, lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, cudaStream_t st);
-int launch_current(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
-                   lartpc_signals_t *out, cudaStream_t st);
+int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
+                         lartpc_signals_t *out, cudaStream_t st);
+int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st);
 int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out, cudaStream_t st);
 int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
                        int32_t *slot_scratch, int32_t *scan_scratch, int64_t hit_base, cudaStream_t st);

@@ -5,47 +5,30 @@
 //     C[b][a][j]  = sum_seg sum_mu (Q_a/N) wx[a] wy[b] wt[j]          (charge per LUT cell, eq. 3.8)
 //     I_p[n]      = sum_{a,b,j} C[b][a][j] * R[b - nb(iy-H)][a - nb(ix-H)][n - j]      (eq. 3.7)
 // which needs ~50x fewer operations and shares the charge lattice between neighbouring segments.
-// One CTA owns one charge tile = (charged pixel P, chunk of Jc arrival ticks):
-//   phase 1  splat the tile's segments into C[nb*nb][Jc] in shared memory (register-tiled outer products
-//            of per-sample erf-difference weights, no atomics);
-//   phase 2  find the non-empty bins and their tick ranges;
-//   phase 3  response: a thread keeps 16 output ticks of a PAIR of target pixels in registers (32 accumulators
-//            as 16 packed f32x2) and slides a 24-tap window of the pair-interleaved LUT rows over the charge row:
-//            128 FFMA2 (256 multiply-adds) per 4 LDS.128 of taps + 2 broadcast LDS.128 of charge.  The LUT rows of
-//            the next non-empty bin arrive by cp.async.bulk (TMA engine, mbarrier completion) into the other half
-//            of a double buffer while the current bin is being used;
-//   phase 4  the tile's partial waveforms go to global memory; S5 sums them per pixel in a fixed order.
+// A tile is (charged pixel P, window of Jc arrival ticks).  Two kernels:
+//
+//   charge_lattice_kernel (one CTA per tile)
+//     splat the tile's segments into C[nb*nb][Jc] in shared memory (register-tiled outer products of
+//     per-sample erf-difference weights, no atomics, fixed order), then pack the non-empty bins: per bin the
+//     first charged tick rounded down to even, the number of 4-tick charge groups and the charge row.
+//
+//   response_kernel (persistent, two CTAs per SM, no CTA-wide barrier after start-up)
+//     warp 8 is the producer: it takes tiles from a work counter and, per non-empty bin, streams the bin's
+//     LUT rows (one contiguous block, pair-interleaved targets) and its charge row into a ring of shared-memory
+//     stages with cp.async.bulk (TMA engine), completion on an mbarrier per stage.
+//     Warps 0-7 are consumers (two per SM sub-partition): a thread owns RESP_NO = 14 output ticks of a PAIR of
+//     target pixels (28 accumulators as 14 packed f32x2 registers) for the whole tile and slides a 20-tap window of
+//     the pair-interleaved LUT row over the charge row, 4 charges per step: 56 FFMA2 (112 multiply-adds) per
+//     2 LDS.128 of taps + 1 broadcast LDS.128 of charge.  Warps run freely through the ring (full / empty
+//     mbarriers), so threads with edge output blocks never hold back the others, and the output blocks are dealt
+//     to the thread slots so that the four sub-partitions carry the same load (api.cu balance_blocks).  After the
+//     last bin of a tile the accumulators go to global memory as the tile's partial waveforms; S5 sums them per
+//     pixel in a fixed order.
+#include <string.h>
+#include <algorithm>
 #include "common.cuh"
 
 namespace {
-
-constexpr int NT = 256;          // threads per CTA (two CTAs per SM)
-constexpr int NO = 16;           // output ticks per response task
-constexpr int LUT_OFF = 16;      // LUT tick k sits at word LUT_OFF + k of its zero-padded row
-constexpr int SB = 64;           // samples per splat batch
-constexpr int XS = 16;           // row length of the per-sample x / y weight tables (bins_per_pixel <= 15)
-constexpr int SEGCAP = 32;       // segments staged per batch
-
-struct CurrentArgs {
-    DevParams p;
-    const DevTpc *tpcs;
-    const int32_t *tile_cp;
-    const TileDesc *tile_desc;
-    const int32_t *pix_start, *pix_count, *pair_seg;
-    const float *q_anode, *sigma_T, *sigma_t;
-    const double *u_s, *v_s, *u_e, *v_e, *T_s, *T_e;
-    const int32_t *a_lo, *a_hi, *b_lo, *b_hi, *jt0, *jt1, *n_samples;
-    const float *lut;
-    float *partial;
-    int32_t *tile_range;
-    unsigned long long *fma_counter;   // multiply-adds of the response: non-zero cells x valid targets x K
-    int CJ, NEP, NB2P;           // smem strides: charge row, erf row, wxy row
-};
-
-struct SegLocal {               // one staged segment, tile-relative
-    float as, ae, bs, be, ts, te, isT, ist, q;
-    int N, alo, ahi, blo, bhi, jlo, jhi, seg, zero_sigma;
-};
 
 typedef unsigned long long u64;   // one packed f32x2 register pair: (target 2p, target 2p+1)
 
@@ -58,32 +41,6 @@ __device__ __forceinline__ u64 pack2(float x)
 __device__ __forceinline__ void ffma2(u64 &d, u64 a, u64 b)      // d = a * b + d on both halves
 {
     asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
-}
-__device__ __forceinline__ void load8w(u64 (&d)[8], const float *s)    // 8 pair-words = 64 bytes
-{
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        ulonglong2 v = *(const ulonglong2 *)(s + 4 * q);
-        d[2 * q] = v.x;  d[2 * q + 1] = v.y;
-    }
-}
-__device__ __forceinline__ void load8c(u64 (&c)[8], const float *s)    // 8 charges, each duplicated into a pair
-{
-    float4 x = *(const float4 *)s, y = *(const float4 *)(s + 4);
-    c[0] = pack2(x.x); c[1] = pack2(x.y); c[2] = pack2(x.z); c[3] = pack2(x.w);
-    c[4] = pack2(y.x); c[5] = pack2(y.y); c[6] = pack2(y.z); c[7] = pack2(y.w);
-}
-// acc[i] += sum_jj c[jj] * w[i - jj + 8],  w = lo[0..7] ++ mid[0..7] ++ hi[0..7]  (i < 16, jj < 8)
-__device__ __forceinline__ void fma_step(u64 (&acc)[NO], const u64 (&c)[8], const u64 (&lo)[8], const u64 (&mid)[8],
-                                         const u64 (&hi)[8])
-{
-#pragma unroll
-    for (int jj = 0; jj < 8; ++jj)
-#pragma unroll
-        for (int i = 0; i < NO; ++i) {
-            const int m = i - jj + 8;
-            ffma2(acc[i], c[jj], m < 8 ? lo[m] : (m < 16 ? mid[m - 8] : hi[m - 16]));
-        }
 }
 
 // ---- mbarrier + bulk copy (TMA engine) -------------------------------------------------------------
@@ -104,44 +61,101 @@ __device__ __forceinline__ void mbar_wait(void *bar, uint32_t parity)
         "WAIT_DONE:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-// one thread: expect `bytes` on the barrier and start the global -> shared bulk copy
-__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, void *bar)
+__device__ __forceinline__ bool mbar_try_wait(void *bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+// the whole warp waits, one lane polls (32 lanes polling one mbarrier serialise in the shared-memory pipe)
+__device__ __forceinline__ void mbar_wait_warp(void *bar, uint32_t parity, int lane)
+{
+    while (true) {
+        bool ok = false;
+        if (lane == 0) ok = mbar_try_wait(bar, parity);
+        if (__any_sync(0xffffffffu, ok)) break;
+    }
+}
+__device__ __forceinline__ bool mbar_try_wait_u32(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_arrive(void *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// global -> shared bulk copy, completion counted in bytes on `bar`
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, void *bar)
+{
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-__global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArgs a)
+// =====================================================================================================
+// Kernel 1: charge lattice of every tile
+// =====================================================================================================
+constexpr int NT1 = 256;         // threads per CTA
+constexpr int SB = 64;           // samples per splat batch
+constexpr int XS = 16;           // row length of the per-sample x / y weight tables (bins_per_pixel <= 15)
+constexpr int SEGCAP = 32;       // segments staged per batch
+
+struct SplatArgs {
+    DevParams p;
+    const DevTpc *tpcs;
+    const int32_t *tile_cp;
+    const TileDesc *tile_desc;
+    const int32_t *pix_start, *pix_count, *pair_seg;
+    const float *q_anode, *sigma_T, *sigma_t;
+    const double *u_s, *v_s, *u_e, *v_e, *T_s, *T_e;
+    const int32_t *a_lo, *a_hi, *b_lo, *b_hi, *jt0, *jt1, *n_samples;
+    float *charge;                     // [n_tiles][slab_floats]
+    int32_t *tile_range;
+    unsigned long long *fma_counter;   // multiply-adds of the response: non-zero cells x valid targets x K
+};
+
+struct SegLocal {               // one staged segment, tile-relative
+    float as, ae, bs, be, ts, te, isT, ist, q;
+    int N, alo, ahi, blo, bhi, jlo, jhi, seg, zero_sigma;
+};
+
+__global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const DevParams &p = a.p;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int NB2 = p.NB2, CJ = a.CJ, nb = p.nb, K = p.K, WW = p.WW, RS = p.RS;
+    const int NB2 = p.NB2, CJ = p.CJ, nb = p.nb, K = p.K;
 
     float *Csm = (float *)smem_raw;                                  // [NB2][CJ] charge per (bin, arrival tick)
-    float *scratch = Csm + NB2 * CJ;                                 // splat scratch, later the LUT stage
-    const int stage_floats = p.PG * RS * 2;                          // one LUT stage: PG pair rows of RS pair-words
-    size_t scratch_floats = max((size_t)2 * stage_floats, (size_t)SB * (2 * XS + CJ));
-    int *s_int = (int *)(scratch + scratch_floats);
-    int *bin_jlo = s_int, *bin_jhi = s_int + NB2, *bin_list = s_int + 2 * NB2;
-    int *s_misc = bin_list + NB2;                                    // [0] n bins, [1] tile jlo, [2] tile jhi
-    u64 *mbar = (u64 *)(s_misc + 8);                                 // [2] "stage full" barriers
-    SegLocal *segs = (SegLocal *)(mbar + 2);
+    float *scratch = Csm + NB2 * CJ;                                 // splat scratch
+    int *s_int = (int *)(scratch + SB * (2 * XS + CJ));
+    int *bin_jlo = s_int, *bin_jhi = s_int + NB2, *bin_list = s_int + 2 * NB2, *bin_off = s_int + 3 * NB2;
+    int *s_misc = s_int + 4 * NB2;                                   // [0] n bins, [1] tile jlo, [2] tile jhi, [3] groups
+    SegLocal *segs = (SegLocal *)(s_misc + 8);
 
     const int tile = blockIdx.x;
     const TileDesc td = a.tile_desc[tile];
     const int cp = a.tile_cp[tile];
     const DevTpc &tp = a.tpcs[td.tpc];
-    const int A_t = td.px * nb, B_t = td.py * nb, J_t = td.chunk * p.Jc;
+    const int A_t = td.px * nb, B_t = td.py * nb, J_t = td.j_start;
     const int lstart = a.pix_start[cp], lcount = a.pix_count[cp];
 
-    for (int i = tid; i < NB2 * CJ / 4; i += NT) ((float4 *)Csm)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (tid == 0) {
-        mbar_init(&mbar[0], 1);
-        mbar_init(&mbar[1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
+    for (int i = tid; i < NB2 * CJ / 4; i += NT1) ((float4 *)Csm)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
     // ------------------------------------------------------------------ phase 1: splat
     float *WX = scratch, *WY = scratch + SB * XS, *WT = scratch + 2 * SB * XS;     // [SB][XS], [SB][XS], [SB][CJ]
@@ -178,7 +192,7 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
                 // float64 with the oracle's operation order (SURVEY section 7 "sigma -> 0 branch")
                 const int s = L.seg;
                 const double us = a.u_s[s], ue = a.u_e[s], vs = a.v_s[s], ve = a.v_e[s], Ts = a.T_s[s], Te = a.T_e[s];
-                for (int mu = tid; mu < L.N; mu += NT) {
+                for (int mu = tid; mu < L.N; mu += NT1) {
                     double f = xdiv(xadd((double)mu, 0.5), (double)L.N);
                     double u = xadd(us, xmul(xsub(ue, us), f));
                     double v = xadd(vs, xmul(xsub(ve, vs), f));
@@ -202,7 +216,7 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
                 const int nsb = min(nsb_max, L.N - mu0);
                 // (A) one-dimensional cell weights of every sample of the batch.  A warp evaluates erf once per bin /
                 // tick edge and takes the difference with its neighbour lane: w = (erf(e+1) - erf(e)) / 2.
-                for (int r = warp; r < nsb * runs; r += NT / 32) {
+                for (int r = warp; r < nsb * runs; r += NT1 / 32) {
                     const int ml = r / runs, k = r - ml * runs;
                     const float f = ((float)(mu0 + ml) + 0.5f) * invN;
                     if (k == 0) {
@@ -222,7 +236,7 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
                 __syncthreads();
                 // (B) a thread owns 4 cells (consecutive in a) x 4 ticks and adds the batch's outer products to them;
                 // entries past na / nj multiply stale shared memory and are never stored
-                for (int unit = tid; unit < units; unit += NT) {
+                for (int unit = tid; unit < units; unit += NT1) {
                     const int cu = unit / nj4, jq = unit - cu * nj4, b = cu / na4, aq = cu - b * na4;
                     u64 acc[4][2];
 #pragma unroll
@@ -258,11 +272,11 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
     }
     __syncthreads();
 
-    // ------------------------------------------------------------------ phase 2: non-empty bins
+    // ------------------------------------------------------------------ phase 2: non-empty bins and their tick ranges
     int nz_cells = 0;
-    for (int c = warp; c < NB2; c += NT / 32) {
+    for (int c = warp; c < NB2; c += NT1 / 32) {
         int lo = INT_MAX, hi = -1;
-        for (int j = lane; j < CJ; j += 32)
+        for (int j = lane; j < p.Jc; j += 32)
             if (Csm[c * CJ + j] != 0.f) { lo = min(lo, j); hi = max(hi, j); ++nz_cells; }
         for (int d = 16; d; d >>= 1) {
             lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, d));
@@ -272,30 +286,46 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
     }
     __syncthreads();
     if (warp == 0) {
-        int nbins = 0, tlo = INT_MAX, thi = -1;
+        // bin list in ascending bin order; row offsets = running sum of 4 * groups
+        int nbins = 0, tlo = INT_MAX, thi = -1, off = SLAB_HDR + 2 * NB2, groups = 0;
         for (int base = 0; base < NB2; base += 32) {
             const int c = base + lane;
             const bool f = c < NB2 && bin_jhi[c] >= 0;
             const unsigned bal = __ballot_sync(0xffffffffu, f);
+            const int ng = f ? ((bin_jhi[c] - (bin_jlo[c] & ~1)) >> 2) + 1 : 0;
+            int inc = f ? ng + 1 : 0;                                // inclusive warp scan of the row lengths in 16-byte units
+            for (int d = 1; d < 32; d <<= 1) {
+                const int o = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += o;
+            }
             if (f) {
-                bin_list[nbins + __popc(bal & ((1u << lane) - 1u))] = c;
+                const int k = nbins + __popc(bal & ((1u << lane) - 1u));
+                bin_list[k] = c;
+                bin_off[k] = off + 4 * (inc - ng - 1);
                 tlo = min(tlo, bin_jlo[c]);  thi = max(thi, bin_jhi[c]);
             }
+            const int tot = __shfl_sync(0xffffffffu, inc, 31);
+            off += 4 * tot;  groups += tot - __popc(bal);
             nbins += __popc(bal);
         }
         for (int d = 16; d; d >>= 1) {
             tlo = min(tlo, __shfl_xor_sync(0xffffffffu, tlo, d));
             thi = max(thi, __shfl_xor_sync(0xffffffffu, thi, d));
         }
-        if (lane == 0) { s_misc[0] = nbins; s_misc[1] = tlo; s_misc[2] = thi; }
+        if (lane == 0) { s_misc[0] = nbins; s_misc[1] = tlo; s_misc[2] = thi; s_misc[3] = groups; }
     }
     __syncthreads();
     const int nbins = s_misc[0], tjlo = s_misc[1], tjhi = s_misc[2];
+    float *slab = a.charge + (size_t)tile * p.slab_floats;
+    int *slab_i = (int *)slab;
     if (nbins == 0) {
-        if (tid == 0 && blockIdx.y == 0) { a.tile_range[2 * tile] = 1; a.tile_range[2 * tile + 1] = 0; }
+        if (tid == 0) {
+            slab_i[0] = 0; slab_i[1] = 0; slab_i[2] = 1; slab_i[3] = 0;
+            a.tile_range[2 * tile] = 1;  a.tile_range[2 * tile + 1] = 0;
+        }
         return;
     }
-    if (blockIdx.y == 0) {
+    {
         // multiply-adds the method needs here: non-zero cells x in-plane targets x K
         for (int d = 16; d; d >>= 1) nz_cells += __shfl_xor_sync(0xffffffffu, nz_cells, d);
         const int vx = min(td.px + p.H, tp.nx - 1) - max(td.px - p.H, 0) + 1;
@@ -304,110 +334,282 @@ __global__ void __launch_bounds__(NT, 2) induced_current_kernel(const CurrentArg
             atomicAdd(a.fma_counter, (unsigned long long)nz_cells * (unsigned long long)(vx * vy * K));
     }
 
-    // ------------------------------------------------------------------ phase 3: response
-    // this CTA's pair group g = blockIdx.y: pairs [g PG, (g+1) PG); its LUT stage for bin c is one contiguous block
-    const int g = blockIdx.y;
-    const uint32_t stage_bytes = (uint32_t)stage_floats * 4u;
-    const float *lut_g = a.lut + (size_t)g * stage_floats;
-    const size_t lut_bin_stride = (size_t)p.NP * RS * 2;
-    float *Rsm0 = scratch, *Rsm1 = scratch + stage_floats;
+    // ------------------------------------------------------------------ phase 3: packed tile out
+    const int nB_lo = tjlo / RESP_NO, nB_hi = (tjhi + K - 1) / RESP_NO; // output blocks, tile-relative
     if (tid == 0) {
-        // the splat used this memory through the generic proxy; order those accesses before the bulk copies
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        bulk_load(Rsm0, lut_g + bin_list[0] * lut_bin_stride, stage_bytes, &mbar[0]);
-        if (nbins > 1) bulk_load(Rsm1, lut_g + bin_list[1] * lut_bin_stride, stage_bytes, &mbar[1]);
+        slab_i[0] = nbins; slab_i[1] = s_misc[3]; slab_i[2] = nB_lo; slab_i[3] = nB_hi;
+        a.tile_range[2 * tile] = nB_lo;  a.tile_range[2 * tile + 1] = nB_hi;
     }
-    const int nB_lo = tjlo >> 4, nB_hi = (tjhi + K - 1) >> 4;          // 16-tick output blocks, tile-relative
-    const int blk = tid / p.PG, pl = tid - blk * p.PG;
-    const bool t_ok = blk <= nB_hi - nB_lo;
-    const int n0 = NO * (nB_lo + blk);
-    u64 acc[NO];
-#pragma unroll
-    for (int i = 0; i < NO; ++i) acc[i] = 0ull;
-    for (int bi = 0; bi < nbins; ++bi) {
-        const int c = bin_list[bi];
-        float *Rsm = (bi & 1) ? Rsm1 : Rsm0;
-        mbar_wait(&mbar[bi & 1], (uint32_t)((bi >> 1) & 1));
-        if (t_ok) {
-            const int jlo_c = bin_jlo[c], jhi_c = bin_jhi[c];
-            // groups of 8 charges whose taps k = n - j meet [0, K) for some of this task's outputs
-            int jb = max(jlo_c & ~7, (n0 - K + 1) & ~7);
-            const int jb_end = min(jhi_c & ~7, n0 + 8);
-            if (jb <= jb_end) {
-                const float *Crow = Csm + c * CJ;
-                // window of 24 pair-words starting at LUT tick n0 - jb - 8, i.e. word n0 - jb + 8 of the row
-                const float *w = Rsm + (pl * RS + (n0 - jb + LUT_OFF - 8)) * 2;
-                u64 G0[8], G1[8], G2[8], cv[8];
-                load8w(G1, w + 16);  load8w(G2, w + 32);
-                while (true) {
-                    load8w(G0, w);  load8c(cv, Crow + jb);
-                    fma_step(acc, cv, G0, G1, G2);
-                    jb += 8;  w -= 16;
-                    if (jb > jb_end) break;
-                    load8w(G2, w);  load8c(cv, Crow + jb);
-                    fma_step(acc, cv, G2, G0, G1);
-                    jb += 8;  w -= 16;
-                    if (jb > jb_end) break;
-                    load8w(G1, w);  load8c(cv, Crow + jb);
-                    fma_step(acc, cv, G1, G2, G0);
-                    jb += 8;  w -= 16;
-                    if (jb > jb_end) break;
-                }
-            }
-        }
-        __syncthreads();                                             // every reader is done with this stage
-        if (tid == 0 && bi + 2 < nbins) {
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            bulk_load(Rsm, lut_g + bin_list[bi + 2] * lut_bin_stride, stage_bytes, &mbar[bi & 1]);
+    for (int k = tid; k < nbins; k += NT1) {
+        const int c = bin_list[k], jb0 = bin_jlo[c] & ~1, ng = ((bin_jhi[c] - jb0) >> 2) + 1;
+        slab_i[SLAB_HDR + 2 * k] = c | (ng << 8) | (jb0 << 16);
+        slab_i[SLAB_HDR + 2 * k + 1] = bin_off[k];
+    }
+    // a row = 16-byte header {first charged tick, groups, flags, tile} + 4 * groups charges; the response kernel copies
+    // it into a pipeline stage as it is
+    const int row_flags = (nB_lo << 8) | (nB_hi << 16);
+    for (int k = warp; k < nbins; k += NT1 / 32) {
+        const int c = bin_list[k], jb0 = bin_jlo[c] & ~1, ng = ((bin_jhi[c] - jb0) >> 2) + 1;
+        const float4 *src = (const float4 *)(Csm + c * CJ + jb0);     // CJ and jb0 even, rows padded by 4 zeros:
+        float4 *dst = (float4 *)(slab + bin_off[k]);                  // 8-byte aligned source, 16-byte aligned target
+        if (lane == 0) *(int4 *)dst = make_int4(jb0, ng, row_flags | (k == nbins - 1 ? 1 : 0), tile);
+        for (int g = lane; g < ng; g += 32) {
+            const float2 x = ((const float2 *)src)[2 * g], y = ((const float2 *)src)[2 * g + 1];
+            dst[1 + g] = make_float4(x.x, x.y, y.x, y.y);
         }
     }
-
-    // ------------------------------------------------------------------ phase 4: partial waveforms out
-    if (t_ok) {
-        const int d0 = 2 * (g * p.PG + pl);
-        float lo[NO], hi[NO];
-#pragma unroll
-        for (int i = 0; i < NO; ++i) {
-            lo[i] = __uint_as_float((unsigned)(acc[i] & 0xffffffffull));
-            hi[i] = __uint_as_float((unsigned)(acc[i] >> 32));
-        }
-        if (d0 < WW) {
-            float4 *dst = (float4 *)(a.partial + ((size_t)tile * WW + d0) * p.tile_ticks + n0);
-#pragma unroll
-            for (int q = 0; q < NO / 4; ++q) dst[q] = make_float4(lo[4 * q], lo[4 * q + 1], lo[4 * q + 2], lo[4 * q + 3]);
-        }
-        if (d0 + 1 < WW) {
-            float4 *dst = (float4 *)(a.partial + ((size_t)tile * WW + d0 + 1) * p.tile_ticks + n0);
-#pragma unroll
-            for (int q = 0; q < NO / 4; ++q) dst[q] = make_float4(hi[4 * q], hi[4 * q + 1], hi[4 * q + 2], hi[4 * q + 3]);
-        }
-    }
-    if (tid == 0 && g == 0) { a.tile_range[2 * tile] = nB_lo; a.tile_range[2 * tile + 1] = nB_hi; }
 }
 
-size_t current_smem_bytes(const DevParams &p, int &CJ, int &NEP, int &NB2P)
+size_t splat_smem_bytes(const DevParams &p)
 {
-    CJ = p.Jc;
-    NEP = ((2 * (p.nb + 1) + p.Jc + 1) + 3) & ~3;
-    NB2P = (p.NB2 + 3) & ~3;
-    size_t scratch = (size_t)2 * p.PG * p.RS * 2;
-    size_t splat = (size_t)SB * (2 * XS + CJ);
-    if (splat > scratch) scratch = splat;
-    size_t ints = 3 * (size_t)p.NB2 + 8 + 4;                      // bin tables, misc, two 64-bit mbarriers
-    size_t bytes = ((size_t)p.NB2 * CJ + scratch) * 4 + ints * 4;
+    size_t floats = (size_t)p.NB2 * p.CJ + (size_t)SB * (2 * XS + p.CJ);
+    size_t ints = 4 * (size_t)p.NB2 + 8;
+    size_t bytes = (floats + ints) * 4;
     bytes = (bytes + 15) & ~(size_t)15;
     return bytes + sizeof(SegLocal) * SEGCAP;
 }
 
+// =====================================================================================================
+// Kernel 2: response of the W x W pixels around every tile (persistent, warp-specialised)
+// =====================================================================================================
+constexpr int NCW = RESP_CONSUMERS / 32;   // consumer warps
+constexpr int NT2 = RESP_CONSUMERS + 32;   // threads per CTA: 8 consumer warps + 1 producer warp, two CTAs per SM
+constexpr int NO = RESP_NO;                // output ticks per response task
+constexpr int FLAG_LAST = 1, FLAG_END = 2;
+
+struct ResponseArgs {
+    DevParams p;
+    const float *lut;            // [NB2][NP][RS][2]
+    const float *charge;         // [n_tiles][slab_floats]
+    float *partial;              // [n_tiles][WW][tile_ticks]
+    int *work;                   // work-queue cursor
+    int n_work;                  // n_tiles * n_groups
+    int n_stages;
+    int stage_floats;            // LUT block + charge row + header, in floats (multiple of 4)
+    int lut_floats;              // PG * RS * 2
+    const int *end_row;          // 16 bytes: a row header with FLAG_END
+    unsigned char blk_of_slot[256];
+};
+
+__device__ __forceinline__ void load4w(u64 (&d)[4], const float *s)     // 4 pair-words = 32 bytes
+{
+    const ulonglong2 v0 = *(const ulonglong2 *)s, v1 = *(const ulonglong2 *)(s + 4);
+    d[0] = v0.x; d[1] = v0.y; d[2] = v1.x; d[3] = v1.y;
+}
+__device__ __forceinline__ void load4c(u64 (&c)[4], const float *s)     // 4 charges, each duplicated into a pair
+{
+    const float4 x = *(const float4 *)s;
+    c[0] = pack2(x.x); c[1] = pack2(x.y); c[2] = pack2(x.z); c[3] = pack2(x.w);
+}
+// acc[i] += sum_jj c[jj] * w[i - jj + 4],  w = q0[0..3] ++ q1 ++ q2 ++ q3 ++ q4  (i < 16, jj < 4)
+__device__ __forceinline__ void fma_step(u64 (&acc)[NO], const u64 (&c)[4], const u64 (&q0)[4], const u64 (&q1)[4],
+                                         const u64 (&q2)[4], const u64 (&q3)[4], const u64 (&q4)[4])
+{
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj)
+#pragma unroll
+        for (int i = 0; i < NO; ++i) {
+            const int m = i - jj + 4;
+            ffma2(acc[i], c[jj], m < 4 ? q0[m] : (m < 8 ? q1[m - 4] : (m < 12 ? q2[m - 8] : (m < 16 ? q3[m - 12] : q4[m - 16]))));
+        }
+}
+
+#ifdef LARTPC_DEBUG_CLOCKS
+__device__ unsigned long long g_dbg[8];
+#define DBG_T(x) long long x = clock64()
+#define DBG_ADD(i, v) dbg_acc[i] += (unsigned long long)(v)
+#define DBG_DECL unsigned long long dbg_acc[4] = {0, 0, 0, 0}
+#define DBG_FLUSH do { if (lane == 0) for (int i_ = 0; i_ < 4; ++i_) atomicAdd(&g_dbg[i_], dbg_acc[i_]); } while (0)
+#else
+#define DBG_T(x)
+#define DBG_ADD(i, v)
+#define DBG_DECL
+#define DBG_FLUSH
+#endif
+
+__global__ void __launch_bounds__(NT2, 2) response_kernel(const ResponseArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const DevParams &p = a.p;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int S = a.n_stages;
+    float *stages = (float *)smem_raw;                                // [S][stage_floats]: LUT rows, charge row, header
+    u64 *full = (u64 *)(stages + (size_t)S * a.stage_floats);        // [S] "stage filled" (1 arrival + bytes)
+    u64 *empty = full + S;                                            // [S] "stage released" (NCW arrivals)
+
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == NCW) {
+        // ------------------------------------------------------------------ producer: one thread, few instructions per
+        // bin (it shares its sub-partition's issue port with four consumer warps)
+        if (lane != 0) return;
+        int s = 0;
+        uint32_t ph = 0;
+        const uint32_t lut_bytes = (uint32_t)a.lut_floats * 4u, stage_bytes = (uint32_t)a.stage_floats * 4u;
+        const uint32_t stage0 = smem_u32(stages), full0 = smem_u32(full), empty0 = smem_u32(empty);
+        const size_t lut_bin_stride = (size_t)p.NP * p.RS * 2;
+        int q = atomicAdd(a.work, 1), q_next = atomicAdd(a.work, 1);
+        while (q < a.n_work) {
+            const int tile = q / p.n_groups, g = q - tile * p.n_groups;
+            const float *slab = a.charge + (size_t)tile * p.slab_floats;
+            const int nbins = *(const int *)slab;
+            const int2 *items = (const int2 *)(slab + SLAB_HDR);
+            const float *lut_g = a.lut + (size_t)g * a.lut_floats;
+            int4 nxt = *(const int4 *)items;                         // two items per 16-byte load, one pair ahead
+            for (int k = 0; k < nbins; k += 2) {
+                const int4 cur = nxt;
+                if (k + 2 < nbins) nxt = *(const int4 *)(items + k + 2);
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    if (k + e >= nbins) break;
+                    const int w0 = e ? cur.z : cur.x, off = e ? cur.w : cur.y;
+                    const int c = w0 & 0xff, ng = (w0 >> 8) & 0xff;
+                    const uint32_t st = stage0 + (uint32_t)s * stage_bytes, fb = full0 + 8u * s;
+                    const uint32_t row_bytes = 16u + (uint32_t)ng * 16u;
+                    while (!mbar_try_wait_u32(empty0 + 8u * s, ph ^ 1u)) {}
+                    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fb), "r"(lut_bytes + row_bytes) : "memory");
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                 ::"r"(st), "l"(lut_g + (size_t)c * lut_bin_stride), "r"(lut_bytes), "r"(fb) : "memory");
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                 ::"r"(st + lut_bytes), "l"(slab + off), "r"(row_bytes), "r"(fb) : "memory");
+                    if (++s == S) { s = 0; ph ^= 1u; }
+                }
+            }
+            q = q_next;
+            q_next = atomicAdd(a.work, 1);
+        }
+        {                                                            // terminator: a header-only row with the END flag
+            const uint32_t st = stage0 + (uint32_t)s * stage_bytes, fb = full0 + 8u * s;
+            while (!mbar_try_wait_u32(empty0 + 8u * s, ph ^ 1u)) {}
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fb), "r"(16u) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(st + lut_bytes), "l"(a.end_row), "r"(16u), "r"(fb) : "memory");
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------------- consumers
+    const int slot = tid / p.PG, pl = tid - slot * p.PG;
+    const bool valid = slot < p.nblk_max;
+    const int blk = valid ? a.blk_of_slot[slot] : 0;
+    const int n0 = NO * blk;
+    const int K = p.K, WW = p.WW;
+    // float offset of pair-word (LUT_OFF + n0 - 4) of this thread's pair row inside a stage; m-range constants
+    const int tap0 = (pl * p.RS + (LUT_OFF + n0 - 4)) * 2;
+    const int lo_num = n0 - K - 2 + 3, hi_num = n0 + NO - 1;
+    const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
+    u64 acc[NO];
+#pragma unroll
+    for (int i = 0; i < NO; ++i) acc[i] = 0ull;
+    int s = 0;
+    uint32_t ph = 0;
+    DBG_DECL;
+    while (true) {
+        const float *st = stages + (size_t)s * a.stage_floats;
+        DBG_T(t0);
+        while (!mbar_try_wait_u32(full0 + 8u * s, ph)) {}
+        DBG_T(t1);
+        DBG_ADD(0, t1 - t0);
+        DBG_ADD(3, 1);
+        const float *row = st + a.lut_floats;
+        const int4 h = *(const int4 *)row;                            // first charged tick, groups, flags, tile
+        if (h.z & FLAG_END) { DBG_FLUSH; break; }
+        if (valid) {
+            const int jb0 = h.x, ng = h.y;
+            // group m holds charges j = jb0 + 4m .. + 3; its taps k = n - j meet [0, K) for this task's outputs when
+            int m = max(0, (lo_num - jb0) >> 2);
+            const int m_hi = min(ng - 1, (hi_num - jb0) >> 2);
+            if (m <= m_hi) {
+                // window of 20 pair-words starting at LUT tick n0 - jb - 4, i.e. word LUT_OFF + n0 - jb - 4 of the row
+                const float *w = st + (tap0 - 2 * jb0 - 8 * m);
+                const float *cq = row + 4 + 4 * m;
+                u64 Q0[4], Q1[4], Q2[4], Q3[4], Q4[4], cv[4];
+                load4w(Q1, w + 8);  load4w(Q2, w + 16);  load4w(Q3, w + 24);  load4w(Q4, w + 32);
+                while (true) {
+                    load4w(Q0, w);  load4c(cv, cq);
+                    fma_step(acc, cv, Q0, Q1, Q2, Q3, Q4);
+                    w -= 8;  cq += 4;
+                    if (++m > m_hi) break;
+                    load4w(Q4, w);  load4c(cv, cq);
+                    fma_step(acc, cv, Q4, Q0, Q1, Q2, Q3);
+                    w -= 8;  cq += 4;
+                    if (++m > m_hi) break;
+                    load4w(Q3, w);  load4c(cv, cq);
+                    fma_step(acc, cv, Q3, Q4, Q0, Q1, Q2);
+                    w -= 8;  cq += 4;
+                    if (++m > m_hi) break;
+                    load4w(Q2, w);  load4c(cv, cq);
+                    fma_step(acc, cv, Q2, Q3, Q4, Q0, Q1);
+                    w -= 8;  cq += 4;
+                    if (++m > m_hi) break;
+                    load4w(Q1, w);  load4c(cv, cq);
+                    fma_step(acc, cv, Q1, Q2, Q3, Q4, Q0);
+                    w -= 8;  cq += 4;
+                    if (++m > m_hi) break;
+                }
+            }
+        }
+        int g = 0;
+        if (h.z & FLAG_LAST) g = *(const int *)st;                    // pair group of this pass: word 0 of the LUT block
+        __syncwarp();
+        DBG_T(t2);
+        DBG_ADD(1, t2 - t1);
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty0 + 8u * s) : "memory");
+        if (h.z & FLAG_LAST) {
+            // partial waveforms of the tile out; accumulators back to zero for the next tile
+            const int nB_lo = (h.z >> 8) & 0xff, nB_hi = (h.z >> 16) & 0xff;
+            const int d0 = 2 * (g * p.PG + pl);
+            if (valid && blk >= nB_lo && blk <= nB_hi) {
+                float lo[NO], hi[NO];
+#pragma unroll
+                for (int i = 0; i < NO; ++i) {
+                    lo[i] = __uint_as_float((unsigned)(acc[i] & 0xffffffffull));
+                    hi[i] = __uint_as_float((unsigned)(acc[i] >> 32));
+                }
+                if (d0 < WW) {
+                    float2 *dst = (float2 *)(a.partial + ((size_t)h.w * WW + d0) * p.tile_ticks + n0);
+#pragma unroll
+                    for (int q = 0; q < NO / 2; ++q) dst[q] = make_float2(lo[2 * q], lo[2 * q + 1]);
+                }
+                if (d0 + 1 < WW) {
+                    float2 *dst = (float2 *)(a.partial + ((size_t)h.w * WW + d0 + 1) * p.tile_ticks + n0);
+#pragma unroll
+                    for (int q = 0; q < NO / 2; ++q) dst[q] = make_float2(hi[2 * q], hi[2 * q + 1]);
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < NO; ++i) acc[i] = 0ull;
+        }
+        if (++s == S) { s = 0; ph ^= 1u; }
+        DBG_T(t3);
+        DBG_ADD(2, t3 - t2);
+    }
+}
+
+int response_stage_floats(const DevParams &p)
+{
+    return p.PG * p.RS * 2 + 4 + ((p.CJ + 3) & ~3);                  // LUT rows, row header, charge row
+}
+int response_stages(const DevParams &p, size_t smem_limit_per_cta)
+{
+    const size_t stage = (size_t)response_stage_floats(p) * 4;
+    int s = (int)((smem_limit_per_cta - 256) / stage);
+    return s > 4 ? 4 : s;
+}
+
 }  // namespace
 
-int launch_current(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
-                   lartpc_signals_t *out, cudaStream_t st)
+int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
+                         lartpc_signals_t *out, cudaStream_t st)
 {
     (void)n;
     const DevParams &p = sim->dp;
     if (sim->n_tiles == 0) return LARTPC_OK;
-    CurrentArgs a;
+    SplatArgs a;
     a.p = p;
     a.tpcs = sim->d_tpcs;
     a.tile_cp = sim->tile_cp;  a.tile_desc = sim->tile_desc;
@@ -416,27 +618,69 @@ int launch_current(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pix
     a.u_s = dr->u_s; a.v_s = dr->v_s; a.u_e = dr->u_e; a.v_e = dr->v_e; a.T_s = dr->T_s; a.T_e = dr->T_e;
     a.a_lo = pm->a_lo; a.a_hi = pm->a_hi; a.b_lo = pm->b_lo; a.b_hi = pm->b_hi;
     a.jt0 = pm->jt0; a.jt1 = pm->jt1; a.n_samples = pm->n_samples;
-    a.lut = sim->d_lut;
-    a.partial = out->partial;  a.tile_range = out->tile_range;
+    a.charge = out->charge;  a.tile_range = out->tile_range;
     a.fma_counter = sim->d_fma;
-    size_t smem = current_smem_bytes(p, a.CJ, a.NEP, a.NB2P);
+    size_t smem = splat_smem_bytes(p);
     static size_t configured = 0;
     if (smem > configured) {
-        LARTPC_CUDA_TRY(cudaFuncSetAttribute(induced_current_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)smem));
         configured = smem;
     }
-    dim3 grid((unsigned)sim->n_tiles, (unsigned)p.n_groups);
     ++g_lartpc_launches;
-    induced_current_kernel<<<grid, NT, smem, st>>>(a);
+    charge_lattice_kernel<<<(unsigned)sim->n_tiles, NT1, smem, st>>>(a);
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }
 
-// shared-memory need of the S4 kernel for a parameter set (used by lartpc_sim_create to pick Jc)
-size_t lartpc_current_smem(const DevParams &p)
+// two CTAs per SM: each may use half of the SM's shared memory minus the 1 KB the system reserves per CTA
+static size_t response_smem_budget() { return (size_t)(228 * 1024) / 2 - 1024; }
+
+int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st)
 {
-    int a, b, c;
-    return current_smem_bytes(p, a, b, c);
+    const DevParams &p = sim->dp;
+    if (sim->n_tiles == 0) return LARTPC_OK;
+    ResponseArgs a;
+    a.p = p;
+    a.lut = sim->d_lut;
+    a.charge = out->charge;
+    a.partial = out->partial;
+    a.work = sim->d_work;
+    const int64_t n_work = sim->n_tiles * p.n_groups;
+    if (n_work >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
+    a.n_work = (int)n_work;
+    a.stage_floats = response_stage_floats(p);
+    a.lut_floats = p.PG * p.RS * 2;
+    a.n_stages = response_stages(p, response_smem_budget());
+    memcpy(a.blk_of_slot, sim->blk_of_slot, sizeof(a.blk_of_slot));
+    a.end_row = sim->d_end_row;
+    if (a.n_stages < 2) return LARTPC_ERR_UNSUPPORTED;
+    size_t smem = (size_t)a.n_stages * a.stage_floats * 4 + 2 * (size_t)a.n_stages * sizeof(u64);
+    static size_t configured = 0;
+    if (smem > configured) {
+        LARTPC_CUDA_TRY(cudaFuncSetAttribute(response_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
+    int grid = (int)std::min<int64_t>(n_work, 2 * (int64_t)sim->sm_count);
+    ++g_lartpc_launches;
+    response_kernel<<<grid, NT2, smem, st>>>(a);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
 }
-int lartpc_current_threads() { return NT; }
+
+#ifdef LARTPC_DEBUG_CLOCKS
+extern "C" int lartpc_debug_clocks(unsigned long long out[8], int reset)
+{
+    cudaMemcpyFromSymbol(out, g_dbg, sizeof(unsigned long long) * 8);
+    if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_dbg, z, sizeof(z)); }
+    return 0;
+}
+#endif
+
+// shared-memory needs for a parameter set (used by lartpc_sim_create to pick the tile geometry)
+size_t lartpc_splat_smem(const DevParams &p) { return splat_smem_bytes(p); }
+size_t lartpc_response_smem(const DevParams &p)
+{
+    return 2 * (size_t)response_stage_floats(p) * 4 + 64;           // at least two stages must fit
+}

@@ -27,11 +27,11 @@ __global__ void __launch_bounds__(256)
 sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__restrict__ pixel_id,
                  const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,
                  const int64_t *__restrict__ offset, const unsigned long long *__restrict__ pix_mask,
-                 const int32_t *__restrict__ pix_tile0, const float *__restrict__ partial,
-                 const int32_t *__restrict__ tile_range, float *samples)
+                 const int32_t *__restrict__ pix_tile0, const int32_t *__restrict__ pix_jmin,
+                 const float *__restrict__ partial, const int32_t *__restrict__ tile_range, float *samples)
 {
-    __shared__ unsigned long long s_mask[128];
-    __shared__ int s_tile0[128];
+    __shared__ unsigned long long s_mask[128][MASK_WORDS];
+    __shared__ int s_tile0[128], s_js[128];
     const int slot = blockIdx.x;
     const int gp = pixel_id[slot];
     int tpc = 0;
@@ -41,25 +41,30 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
     for (int d = threadIdx.x; d < p.WW; d += blockDim.x) {
         const int dyi = d / p.W, dxi = d - dyi * p.W;
         const int cp = t.cp_base + (iy + dyi) * t.gw + (ix + dxi);   // charged pixel px = ix - H + dxi
-        s_mask[d] = pix_mask[cp];
+#pragma unroll
+        for (int wd = 0; wd < MASK_WORDS; ++wd) s_mask[d][wd] = pix_mask[(size_t)cp * MASK_WORDS + wd];
         s_tile0[d] = pix_tile0[cp];
+        s_js[d] = pix_jmin[cp] & ~1;                                 // window origin of that charged pixel
     }
     __syncthreads();
     const int first = first_tick[slot], len = length[slot];
     const int64_t off = offset[slot];
-    const int span = p.Jc + p.K - 2;                                  // a tile reaches readout ticks [c Jc, c Jc + span]
+    const int span = p.Jc + p.K - 2;                                  // a tile reaches readout ticks [j_start, j_start + span]
     for (int i = threadIdx.x; i < len; i += blockDim.x) {
         const int n = first + i;
-        const int c_hi = min(n / p.Jc, p.n_chunks - 1);
-        const int c_lo = n > span ? (n - span + p.Jc - 1) / p.Jc : 0;
         float sum = 0.f;
         for (int d = 0; d < p.WW; ++d) {
-            const unsigned long long m = s_mask[d];
-            if (!m) continue;
-            for (int c = c_lo; c <= c_hi; ++c) {
-                if (!((m >> c) & 1ull)) continue;
-                const int tix = s_tile0[d] + __popcll(m & ((1ull << c) - 1ull));
-                const int nrel = n - c * p.Jc, blk = nrel >> 4;
+            const int r = n - s_js[d];
+            if (r < 0 || !(s_mask[d][0] | s_mask[d][MASK_WORDS - 1])) continue;
+            const int w_hi = min(r / p.Jc, MAX_WINDOWS - 1);
+            const int w_lo = r > span ? (r - span + p.Jc - 1) / p.Jc : 0;
+            for (int w = w_lo; w <= w_hi; ++w) {
+                const unsigned long long m = s_mask[d][w >> 6];
+                if (!((m >> (w & 63)) & 1ull)) continue;
+                int below = __popcll(m & ((1ull << (w & 63)) - 1ull));
+                if (w >= 64) below += __popcll(s_mask[d][0]);
+                const int tix = s_tile0[d] + below;
+                const int nrel = r - w * p.Jc, blk = nrel / RESP_NO;
                 if (blk >= tile_range[2 * tix] && blk <= tile_range[2 * tix + 1])
                     sum += partial[((size_t)tix * p.WW + d) * p.tile_ticks + nrel];
             }
@@ -89,7 +94,8 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
     ++g_lartpc_launches;
     sum_pixel_kernel<<<(unsigned)sim->n_active, 256, 0, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
                                                              out->length, out->offset, sim->pix_mask, sim->pix_tile0,
-                                                             sig->partial, sig->tile_range, out->samples);
+                                                             sim->pix_jmin, sig->partial, sig->tile_range,
+                                                             out->samples);
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }

@@ -146,7 +146,7 @@ int launch_drift(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, const
 // -------------------------------------------------------------------------------------------------
 struct SegBox {
     int a_lo, a_hi, b_lo, b_hi, ix0, ix1, iy0, iy1, jt0, jt1, npix, n_samples;
-    int cpx0, cpx1, cpy0, cpy1, c0, c1;          // charged pixels (clamped to the +-H margin), chunk range
+    int cpx0, cpx1, cpy0, cpy1, j0, j1;          // charged pixels (clamped to the +-H margin), arrival ticks in the window
     bool deposits;
 };
 
@@ -156,9 +156,8 @@ __device__ __forceinline__ void chunk_and_cp_range(const DevParams &p, const Dev
     long long y0 = floor_div_ll(b.b_lo, p.nb), y1 = floor_div_ll(b.b_hi, p.nb);
     b.cpx0 = (int)max(x0, (long long)-p.H);  b.cpx1 = (int)min(x1, (long long)(t.nx - 1 + p.H));
     b.cpy0 = (int)max(y0, (long long)-p.H);  b.cpy1 = (int)min(y1, (long long)(t.ny - 1 + p.H));
-    int j0 = max(b.jt0, 0), j1 = min(b.jt1, p.j_max);      // charge outside the readout window is dropped (D23)
-    b.c0 = j0 / p.Jc;  b.c1 = j1 / p.Jc;
-    b.deposits = b.npix > 0 && j0 <= j1 && b.cpx0 <= b.cpx1 && b.cpy0 <= b.cpy1;
+    b.j0 = max(b.jt0, 0);  b.j1 = min(b.jt1, p.j_max);     // charge outside the readout window is dropped (D23)
+    b.deposits = b.npix > 0 && b.j0 <= b.j1 && b.cpx0 <= b.cpx1 && b.cpy0 <= b.cpy1;
 }
 
 __device__ __forceinline__ void seg_box(const DevParams &p, const DevTpc *__restrict__ tpcs, int tpc, float q_anode,
@@ -212,7 +211,7 @@ __device__ __forceinline__ long long warp_sum_ll(long long v)
 __global__ void __launch_bounds__(256)
 pixmap_kernel(DevParams p, const DevTpc *__restrict__ tpcs, SegPtrs s, int64_t n, const int32_t *__restrict__ seg_tpc,
               const float *__restrict__ q_anode, int tpc_lo, int tpc_hi, lartpc_pixmap_t o,
-              int32_t *pix_count, unsigned long long *pix_mask, long long *counters)
+              int32_t *pix_count, int32_t *pix_jmin, long long *counters)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     long long m_npix = 0, m_ticks = 0, n_act = 0, n_pairs = 0;
@@ -230,12 +229,11 @@ pixmap_kernel(DevParams p, const DevTpc *__restrict__ tpcs, SegPtrs s, int64_t n
         }
         if (b.deposits && tpc >= tpc_lo && tpc < tpc_hi) {
             const DevTpc &t = tpcs[tpc];
-            unsigned long long mask = (b.c1 >= 63 ? ~0ull : ((1ull << (b.c1 + 1)) - 1ull)) & ~((1ull << b.c0) - 1ull);
             for (int cy = b.cpy0; cy <= b.cpy1; ++cy)
                 for (int cx = b.cpx0; cx <= b.cpx1; ++cx) {
                     int cp = t.cp_base + (cy + p.H) * t.gw + (cx + p.H);
                     atomicAdd(&pix_count[cp], 1);
-                    atomicOr(&pix_mask[cp], mask);
+                    atomicMin(&pix_jmin[cp], b.j0);
                     ++n_pairs;
                 }
         }
@@ -254,6 +252,7 @@ pixmap_kernel(DevParams p, const DevTpc *__restrict__ tpcs, SegPtrs s, int64_t n
 __global__ void __launch_bounds__(256)
 pair_fill_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n, const int32_t *__restrict__ seg_tpc,
                  lartpc_pixmap_t o, int tpc_lo, int tpc_hi, const int32_t *__restrict__ pix_start, int32_t *pix_cursor,
+                 const int32_t *__restrict__ pix_jmin, unsigned long long *pix_mask,
                  int32_t *pair_seg, int64_t pair_cap, long long *counters)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -273,6 +272,14 @@ pair_fill_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n, const 
             int64_t slot = (int64_t)pix_start[cp] + atomicAdd(&pix_cursor[cp], 1);
             if (slot < pair_cap) pair_seg[slot] = (int32_t)i;
             else atomicAdd((unsigned long long *)&counters[CNT_OVERFLOW], 1ull);
+            // windows of Jc arrival ticks counted from the pixel's first tick (rounded down to even)
+            const int js = pix_jmin[cp] & ~1;
+            const int w0 = min((b.j0 - js) / p.Jc, MAX_WINDOWS - 1), w1 = min((b.j1 - js) / p.Jc, MAX_WINDOWS - 1);
+            for (int wd = w0 >> 6; wd <= (w1 >> 6); ++wd) {
+                const int lo = max(w0 - 64 * wd, 0), hi = min(w1 - 64 * wd, 63);
+                const unsigned long long m = (hi >= 63 ? ~0ull : ((1ull << (hi + 1)) - 1ull)) & ~((1ull << lo) - 1ull);
+                atomicOr(&pix_mask[(size_t)cp * MASK_WORDS + wd], m);
+            }
         }
 }
 
@@ -300,31 +307,41 @@ pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int3
     }
 }
 
-// one thread per charged-pixel grid cell: emit its tiles and mark the pixels they can reach
+// one thread per charged-pixel grid cell: emit its tiles (one per window that holds charge) and mark the pixels
+// they can reach
 __global__ void __launch_bounds__(256)
 tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n_cp, const int32_t *__restrict__ pix_tile0,
-                 const unsigned long long *__restrict__ pix_mask, int32_t *tile_cp, TileDesc *tile_desc,
-                 int64_t tile_cap, int32_t *act_first, int32_t *act_last, long long *counters)
+                 const unsigned long long *__restrict__ pix_mask, const int32_t *__restrict__ pix_jmin,
+                 int32_t *tile_cp, TileDesc *tile_desc, int64_t tile_cap, int32_t *act_first, int32_t *act_last,
+                 long long *counters)
 {
     int64_t cp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (cp >= n_cp) return;
-    unsigned long long mask = pix_mask[cp];
-    if (!mask) return;
+    unsigned long long mask[MASK_WORDS];
+    bool any = false;
+#pragma unroll
+    for (int wd = 0; wd < MASK_WORDS; ++wd) { mask[wd] = pix_mask[(size_t)cp * MASK_WORDS + wd]; any |= mask[wd] != 0; }
+    if (!any) return;
     int tpc = 0;
     while (tpc + 1 < p.n_tpcs && tpcs[tpc + 1].cp_base <= cp) ++tpc;
     const DevTpc &t = tpcs[tpc];
     int rel = (int)(cp - t.cp_base);
     int px = rel % t.gw - p.H, py = rel / t.gw - p.H;
     int64_t tix = pix_tile0[cp];
-    int c_lo = __ffsll((long long)mask) - 1, c_hi = 63 - __clzll((long long)mask);
-    for (unsigned long long m = mask; m; m &= m - 1) {
-        int c = __ffsll((long long)m) - 1;
-        if (tix < tile_cap) { tile_cp[tix] = (int32_t)cp; tile_desc[tix] = TileDesc{tpc, px, py, c}; }
-        else atomicAdd((unsigned long long *)&counters[CNT_OVERFLOW], 1ull);
-        ++tix;
-    }
-    int first = c_lo * p.Jc;
-    int last = min(c_hi * p.Jc + p.Jc + p.K - 2, p.n_ticks - 1);
+    const int js = pix_jmin[cp] & ~1;
+    int w_lo = -1, w_hi = -1;
+#pragma unroll
+    for (int wd = 0; wd < MASK_WORDS; ++wd)
+        for (unsigned long long m = mask[wd]; m; m &= m - 1) {
+            int w = 64 * wd + __ffsll((long long)m) - 1;
+            if (w_lo < 0) w_lo = w;
+            w_hi = w;
+            if (tix < tile_cap) { tile_cp[tix] = (int32_t)cp; tile_desc[tix] = TileDesc{tpc, px, py, js + w * p.Jc}; }
+            else atomicAdd((unsigned long long *)&counters[CNT_OVERFLOW], 1ull);
+            ++tix;
+        }
+    int first = js + w_lo * p.Jc;
+    int last = min(js + w_hi * p.Jc + p.Jc + p.K - 2, p.n_ticks - 1);
     for (int iy = max(py - p.H, 0); iy <= min(py + p.H, t.ny - 1); ++iy)
         for (int ix = max(px - p.H, 0); ix <= min(px + p.H, t.nx - 1); ++ix) {
             int gp = t.first_pixel_id + iy * t.nx + ix;
@@ -334,7 +351,16 @@ tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n_cp, con
 }
 
 struct NpixF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
-struct PopcF { const unsigned long long *m; __device__ long long operator()(int64_t i) const { return __popcll(m[i]); } };
+struct PopcF {
+    const unsigned long long *m;
+    __device__ long long operator()(int64_t i) const
+    {
+        int c = 0;
+#pragma unroll
+        for (int wd = 0; wd < MASK_WORDS; ++wd) c += __popcll(m[(size_t)i * MASK_WORDS + wd]);
+        return c;
+    }
+};
 struct ActiveF { const int32_t *last; __device__ long long operator()(int64_t i) const { return last[i] >= 0 ? 1 : 0; } };
 struct ActiveLenF {
     const int32_t *first, *last;
@@ -386,38 +412,42 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_counters, 0, sizeof(long long) * CNT_COUNT, st));
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_count, 0, sizeof(int32_t) * sim->n_cp, st));
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_cursor, 0, sizeof(int32_t) * sim->n_cp, st));
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_mask, 0, sizeof(unsigned long long) * sim->n_cp, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_mask, 0, sizeof(unsigned long long) * MASK_WORDS * sim->n_cp, st));
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->act_last, 0xff, sizeof(int32_t) * sim->n_pix, st));
         ++g_lartpc_launches;
         fill_i32_kernel<<<div_up(sim->n_pix, 256), 256, 0, st>>>(sim->act_first, sim->n_pix, INT32_MAX);
+        ++g_lartpc_launches;
+        fill_i32_kernel<<<div_up(sim->n_cp, 256), 256, 0, st>>>(sim->pix_jmin, sim->n_cp, INT32_MAX);
         if (n > 0) {
             ++g_lartpc_launches;
             pixmap_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, s, n, dr->tpc, dr->q_anode, tpc_lo, tpc_hi,
-                                                         *out, sim->pix_count, sim->pix_mask, sim->d_counters);
+                                                         *out, sim->pix_count, sim->pix_jmin, sim->d_counters);
             LARTPC_CUDA_TRY(cudaGetLastError());
         }
         // offsets[n+1] = exclusive scan of npix
         LARTPC_CUDA_TRY(lscan::exclusive_scan(n, NpixF{out->npix}, out->offsets, true,
                                               sim->d_counters + CNT_TOTAL_NPIX, sim->scan_tmp, st));
-        // per charged pixel: start of its segment list, index of its first tile
+        // per charged pixel: start of its segment list
         LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_cp, NpixF{sim->pix_count}, sim->pix_start, false,
                                               (long long *)nullptr, sim->scan_tmp, st));
-        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_cp, PopcF{sim->pix_mask}, sim->pix_tile0, false,
-                                              sim->d_counters + CNT_TILES, sim->scan_tmp, st));
         if (n > 0) {
             ++g_lartpc_launches;
             pair_fill_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, n, dr->tpc, *out, tpc_lo, tpc_hi,
-                                                            sim->pix_start, sim->pix_cursor, sim->pair_seg,
-                                                            sim->pair_cap, sim->d_counters);
+                                                            sim->pix_start, sim->pix_cursor, sim->pix_jmin,
+                                                            sim->pix_mask, sim->pair_seg, sim->pair_cap,
+                                                            sim->d_counters);
             ++g_lartpc_launches;
             pair_sort_kernel<<<div_up(sim->n_cp, 4), 128, 0, st>>>(sim->n_cp, sim->pix_start, sim->pix_count,
                                                                   sim->pair_seg, sim->pair_cap);
         }
+        // index of the first tile of every charged pixel (one tile per window that holds charge)
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_cp, PopcF{sim->pix_mask}, sim->pix_tile0, false,
+                                              sim->d_counters + CNT_TILES, sim->scan_tmp, st));
         ++g_lartpc_launches;
         tile_emit_kernel<<<div_up(sim->n_cp, 256), 256, 0, st>>>(p, sim->d_tpcs, sim->n_cp, sim->pix_tile0,
-                                                                sim->pix_mask, sim->tile_cp, sim->tile_desc,
-                                                                sim->tile_cap, sim->act_first, sim->act_last,
-                                                                sim->d_counters);
+                                                                sim->pix_mask, sim->pix_jmin, sim->tile_cp,
+                                                                sim->tile_desc, sim->tile_cap, sim->act_first,
+                                                                sim->act_last, sim->d_counters);
         LARTPC_CUDA_TRY(cudaGetLastError());
         // active pixels: slot = rank among active pixels (sorted by id), total waveform samples
         LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_pix, ActiveF{sim->act_last}, sim->act_slot, false,
@@ -462,6 +492,8 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         info->total_samples = h[CNT_TOTAL_SAMPLES];
         info->tile_targets = p.WW;
         info->tile_ticks = p.tile_ticks;
+        info->tile_charge_floats = p.slab_floats;
+        info->reserved = 0;
     }
     return LARTPC_OK;
 }

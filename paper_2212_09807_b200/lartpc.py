@@ -78,11 +78,12 @@ class PixmapInfo(C.Structure):
     _fields_ = [("max_npix", C.c_int32), ("max_ticks", C.c_int32), ("total_npix", C.c_int64),
                 ("n_active_segments", C.c_int64), ("n_tiles", C.c_int64), ("n_pairs", C.c_int64),
                 ("n_active_pixels", C.c_int64), ("total_samples", C.c_int64),
-                ("tile_targets", C.c_int32), ("tile_ticks", C.c_int32)]
+                ("tile_targets", C.c_int32), ("tile_ticks", C.c_int32),
+                ("tile_charge_floats", C.c_int32), ("reserved", C.c_int32)]
 
 
 class Signals(C.Structure):
-    _fields_ = [("tile_capacity", C.c_int64), ("partial", _P), ("tile_range", _P)]
+    _fields_ = [("tile_capacity", C.c_int64), ("partial", _P), ("tile_range", _P), ("charge", _P)]
 
 
 class Waveforms(C.Structure):
@@ -271,8 +272,9 @@ class Sim:
         info = self.info
         nt = int(info.n_tiles)
         out = dict(partial=self._empty(nt * info.tile_targets * info.tile_ticks, t.float32),
-                   tile_range=self._empty(nt * 2, t.int32))
-        sig = Signals(nt, out["partial"].data_ptr(), out["tile_range"].data_ptr())
+                   tile_range=self._empty(nt * 2, t.int32),
+                   charge=self._empty(nt * info.tile_charge_floats, t.float32))
+        sig = Signals(nt, out["partial"].data_ptr(), out["tile_range"].data_ptr(), out["charge"].data_ptr())
         _check(self.lib.lartpc_induced_current(self.handle, C.byref(drifted["_struct"]), C.byref(pixmap["_struct"]),
                                                C.c_int64(pixmap["_n"]), C.byref(sig), _stream_ptr(t)),
                "lartpc_induced_current")
@@ -317,7 +319,8 @@ class Sim:
         out["_struct"] = h
         return out
 
-    STAGES = ("quench", "drift", "pixels_from_segments", "induced_current", "sum_pixel_signals", "electronics")
+    STAGES = ("quench", "drift", "pixels_from_segments", "induced_current_charge", "induced_current_response",
+              "sum_pixel_signals", "electronics")
 
     def set_profiling(self, on: bool):
         _check(self.lib.lartpc_set_profiling(self.handle, C.c_int(1 if on else 0)), "lartpc_set_profiling")
