@@ -52,6 +52,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--segments", type=int, default=None, help="override the segment target of configs 2/3")
+    ap.add_argument("--response", default="auto", choices=["auto", "tensor", "ffma"],
+                    help="S4 response path: tcgen05 tensor cores or the FP32-pipe FFMA2 kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=1000, help="segments in the oracle's bounded sample")
     return ap.parse_args()
@@ -178,7 +180,7 @@ def run_ours(args):
 
     wl = make_workload(args.config, rank, args.segments)
     n = wl.n_segments
-    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, device="cuda:%d" % local)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, device="cuda:%d" % local, response=args.response)
     if wl.disabled_pixels is not None:
         sim.set_disabled_pixels(wl.disabled_pixels)
     host = {k: torch.from_numpy(np.ascontiguousarray(wl.segments[k], dtype=np.float32)).pin_memory()

@@ -131,16 +131,21 @@ typedef struct {
 
 /* S4 output.  A tile is (charged pixel P, window of lartpc_chunk_ticks() arrival ticks that starts at
  * j_start = first arrival tick on P, rounded down to even, + a multiple of the window length).
- *   charge      float32 [n_tiles][tile_charge_floats]: the charge lattice of eq. (3.8) in expectation, C[bin][j]
- *               electrons per (x, y) LUT bin of P and arrival tick, packed per tile as a header (bins, charge
- *               groups, first / last output block), one item per non-empty bin (bin, first tick, groups of 4
- *               ticks, row offset) and the charge rows themselves;
+ *   charge      the charge lattice of eq. (3.8) in expectation, C[bin][j] electrons per (x, y) LUT bin of P and
+ *               arrival tick, tile_charge_floats 32-bit words per tile.
+ *               Tensor-core response (lartpc_response_mode() == LARTPC_RESPONSE_TENSOR): the fp16 operand image
+ *               the MMA reads, [tile / 128][bin][hi | lo][tile % 128][64 ticks] with the 16-byte chunks of a row
+ *               permuted by (tile % 8) (128-byte swizzle), C = (hi + lo) * 2^e with e in tile_range; the buffer
+ *               must hold a whole number of 128-tile blocks: tile_capacity >= n_tiles rounded up to 128.
+ *               FFMA response: packed per tile as a header (bins, charge groups, first / last output block), one
+ *               item per non-empty bin (bin, first tick, groups of 4 ticks, row offset) and the charge rows;
  *   partial     float32 [n_tiles][tile_targets][tile_ticks] (electrons per tick): the current that charge
  *               induces on the W x W pixels around P during readout ticks [j_start, j_start + tile_ticks);
- *   tile_range  int32 [n_tiles][2] = first / last 16-tick block of `partial` written (first > last: no charge).
+ *   tile_range  int32 [n_tiles][4] = first / last 14-tick block of `partial` that can be non-zero (first > last:
+ *               no charge), the scale exponent e, 0.
  * The tile -> pixel map is part of the sim's plan. */
 typedef struct {
-    int64_t  tile_capacity;             /* host value: tiles the three buffers can hold */
+    int64_t  tile_capacity;             /* host value: tiles the charge buffer can hold (partial / tile_range: n_tiles) */
     float   *partial;
     int32_t *tile_range;
     float   *charge;
@@ -190,6 +195,21 @@ int  lartpc_sim_create(const lartpc_params_t *params, const lartpc_tpc_t *tpcs, 
                        const float *response_lut_host, size_t lut_elems, lartpc_sim_t **out);
 void lartpc_sim_destroy(lartpc_sim_t *sim);
 
+/* As lartpc_sim_create, choosing how S4 applies the response (eq. 3.7):
+ *   LARTPC_RESPONSE_TENSOR  dense contraction of the charge lattice with the LUT on the tcgen05 tensor cores, fp16
+ *                           operands split hi + lo (three products, fp32 accumulation); needs lut_ticks <= 241;
+ *   LARTPC_RESPONSE_FFMA    sliding-window convolution on the FP32 pipe (packed FFMA2), any lut_ticks;
+ *   LARTPC_RESPONSE_AUTO    TENSOR where it applies, else FFMA (what lartpc_sim_create does).
+ * Both give the same currents within the S4 tolerance; LARTPC_ERR_UNSUPPORTED when TENSOR
+ * is asked for a LUT it cannot take. */
+#define LARTPC_RESPONSE_AUTO   0
+#define LARTPC_RESPONSE_TENSOR 1
+#define LARTPC_RESPONSE_FFMA   2
+int  lartpc_sim_create_ex(const lartpc_params_t *params, const lartpc_tpc_t *tpcs, int n_tpcs,
+                          const float *response_lut_host, size_t lut_elems, int response_mode, lartpc_sim_t **out);
+/* LARTPC_RESPONSE_TENSOR or LARTPC_RESPONSE_FFMA: the path this sim runs. */
+int  lartpc_response_mode(const lartpc_sim_t *sim);
+
 /* Optional mask of disabled channels: HOST array of global pixel ids; S6 emits no hit for them. */
 int  lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *pixel_ids_host, int64_t n);
 
@@ -215,8 +235,9 @@ int  lartpc_pixels_from_segments(lartpc_sim_t *sim, const lartpc_segments_t *seg
                                  const lartpc_drifted_t *drifted, int64_t n,
                                  lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, void *stream);
 
-/* S4: needs out->tile_capacity >= info.n_tiles.  Two kernels: the charge lattice of every tile (splat), then the
- * response of the W x W pixels around it (persistent, LUT rows streamed through shared memory). */
+/* S4: needs out->tile_capacity >= info.n_tiles (rounded up to 128 for the tensor-core response).  Two kernels: the
+ * charge lattice of every tile (splat), then the response of the W x W pixels around it (persistent; tensor cores, or
+ * LUT rows streamed through shared memory for the FFMA form). */
 int  lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t *drifted, const lartpc_pixmap_t *pixmap,
                             int64_t n, lartpc_signals_t *out, void *stream);
 

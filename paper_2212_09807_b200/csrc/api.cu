@@ -38,7 +38,7 @@ extern "C" const char *lartpc_strerror(int code)
 static void sim_free(lartpc_sim *s)
 {
     if (!s) return;
-    cudaFree(s->d_tpcs); cudaFree(s->d_lut);
+    cudaFree(s->d_tpcs); cudaFree(s->d_lut); cudaFree(s->d_lut_tc);
     cudaFree(s->pix_count); cudaFree(s->pix_start); cudaFree(s->pix_tile0); cudaFree(s->pix_cursor);
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
     cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->scan_tmp);
@@ -104,7 +104,16 @@ static void balance_blocks(const DevParams &p, unsigned char *blk_of_slot)
 extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t *tpcs, int n_tpcs,
                                  const float *lut_host, size_t lut_elems, lartpc_sim_t **out)
 {
+    return lartpc_sim_create_ex(prm, tpcs, n_tpcs, lut_host, lut_elems, LARTPC_RESPONSE_AUTO, out);
+}
+
+extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc_t *tpcs, int n_tpcs,
+                                    const float *lut_host, size_t lut_elems, int response_mode, lartpc_sim_t **out)
+{
     if (!prm || !tpcs || n_tpcs <= 0 || !lut_host || !out) return LARTPC_ERR_BAD_ARGUMENT;
+    if (response_mode != LARTPC_RESPONSE_AUTO && response_mode != LARTPC_RESPONSE_TENSOR &&
+        response_mode != LARTPC_RESPONSE_FFMA)
+        return LARTPC_ERR_BAD_ARGUMENT;
     *out = nullptr;
     int dev = 0;
     cudaDeviceProp prop;
@@ -155,16 +164,32 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
         const double score = (double)jc / g;
         if (score > best) { best = score; best_groups = g; }
     }
-    if (best_groups == 0) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
-    p.n_groups = best_groups;  p.PG = (n_pairs + p.n_groups - 1) / p.n_groups;  p.NP = p.n_groups * p.PG;
-    p.Jc = std::min(120, RESP_NO * (ncons / p.PG) - K + 1) & ~3;  p.CJ = p.Jc + 4;
-    p.nblk_max = (p.Jc + K - 2) / RESP_NO + 1;  p.tile_ticks = RESP_NO * p.nblk_max;
-    p.slab_floats = (SLAB_HDR + 2 * p.NB2 + p.NB2 * (4 + p.CJ) + 3) & ~3;
+    // Tensor-core response (response_tc.cuh): tiles of 64 arrival ticks, the accumulator of one target pixel
+    // (48 + NBW columns, NBW = roundup16(K + 15)) must fit the 512 TMEM columns with NBW <= 256 (one MMA's N).
+    const int nbw = (K + 15 + 15) & ~15;
+    const bool tc_ok = nbw <= 256 && p.WW <= 128;
+    if (response_mode == LARTPC_RESPONSE_TENSOR && !tc_ok) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    p.tc_mode = (response_mode != LARTPC_RESPONSE_FFMA && tc_ok) ? 1 : 0;
+    if (best_groups == 0 && !p.tc_mode) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    if (p.tc_mode) {
+        p.NBW = nbw;
+        p.n_groups = 1;  p.PG = n_pairs;  p.NP = n_pairs;                 // (unused by the tensor-core response)
+        p.Jc = 64;  p.CJ = p.Jc + 4;
+        p.tile_ticks = (p.Jc + K - 1 + 7) & ~7;                           // 264 for K = 200
+        p.nblk_max = (p.tile_ticks + RESP_NO - 1) / RESP_NO;
+        p.slab_floats = p.NB2 * p.Jc;                                     // NB2 rows of (64 hi + 64 lo) fp16
+        if (lartpc_splat_smem(p) > smem_limit) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    } else {
+        p.n_groups = best_groups;  p.PG = (n_pairs + p.n_groups - 1) / p.n_groups;  p.NP = p.n_groups * p.PG;
+        p.Jc = std::min(120, RESP_NO * (ncons / p.PG) - K + 1) & ~3;  p.CJ = p.Jc + 4;
+        p.nblk_max = (p.Jc + K - 2) / RESP_NO + 1;  p.tile_ticks = RESP_NO * p.nblk_max;
+        p.slab_floats = (SLAB_HDR + 2 * p.NB2 + p.NB2 * (4 + p.CJ) + 3) & ~3;
+    }
     if (p.j_max / p.Jc + 2 > MAX_WINDOWS) {                                 // window masks are 128 bits
         sim_free(s);
         return LARTPC_ERR_UNSUPPORTED;
     }
-    balance_blocks(p, s->blk_of_slot);
+    if (!p.tc_mode) balance_blocks(p, s->blk_of_slot);
     p.n_tpcs = n_tpcs;
     p.gain_mv_per_ke = prm->gain_mv_per_ke; p.v_cm = prm->v_cm_mv; p.v_ref = prm->v_ref_mv; p.v_ped = prm->v_pedestal_mv;
     p.adc_full = ldexp(1.0, prm->adc_bits);  p.threshold = prm->threshold_e;
@@ -196,9 +221,9 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
     // (d = dyi*W + dxi; row (c, d) is R[cy = nb*dyi + cb][cx = nb*dxi + ca][.]), LUT tick k at pair-word LUT_OFF + k
     // with zero padding around it.  S4 stages the PG pair rows of one bin with a single bulk copy, reads 20-tap windows
     // with aligned 128-bit loads and feeds both targets of a pair to one packed f32x2 multiply-add.
-    std::vector<float> re((size_t)p.NB2 * p.NP * p.RS * 2, 0.f);
+    std::vector<float> re(p.tc_mode ? 0 : (size_t)p.NB2 * p.NP * p.RS * 2, 0.f);
     const int NB = W * nb;
-    for (int cb = 0; cb < nb; ++cb)
+    for (int cb = 0; cb < nb && !p.tc_mode; ++cb)
         for (int ca = 0; ca < nb; ++ca)
             for (int dyi = 0; dyi < W; ++dyi)
                 for (int dxi = 0; dxi < W; ++dxi) {
@@ -207,13 +232,17 @@ extern "C" int lartpc_sim_create(const lartpc_params_t *prm, const lartpc_tpc_t 
                     float *dst = re.data() + (((size_t)(cb * nb + ca) * p.NP + d / 2) * p.RS + LUT_OFF) * 2 + (d & 1);
                     for (int k = 0; k < K; ++k) dst[2 * k] = src[k];
                 }
-    for (int c = 0; c < p.NB2; ++c)
+    for (int c = 0; c < p.NB2 && !p.tc_mode; ++c)
         for (int g = 0; g < p.n_groups; ++g)
             memcpy(&re[((size_t)c * p.NP + (size_t)g * p.PG) * p.RS * 2], &g, sizeof(int));
 #define SIM_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { \
         lartpc_note_cuda_error(_e, __FILE__, __LINE__); sim_free(s); return LARTPC_ERR_CUDA; } } while (0)
-    SIM_TRY(cudaMalloc(&s->d_lut, sizeof(float) * re.size()));
-    SIM_TRY(cudaMemcpy(s->d_lut, re.data(), sizeof(float) * re.size(), cudaMemcpyHostToDevice));
+    if (p.tc_mode) {
+        if (lartpc_build_lut_tc(p, lut_host, &s->d_lut_tc) == 0) { sim_free(s); return LARTPC_ERR_CUDA; }
+    } else {
+        SIM_TRY(cudaMalloc(&s->d_lut, sizeof(float) * re.size()));
+        SIM_TRY(cudaMemcpy(s->d_lut, re.data(), sizeof(float) * re.size(), cudaMemcpyHostToDevice));
+    }
     SIM_TRY(cudaMalloc(&s->d_tpcs, sizeof(DevTpc) * n_tpcs));
     SIM_TRY(cudaMemcpy(s->d_tpcs, dt.data(), sizeof(DevTpc) * n_tpcs, cudaMemcpyHostToDevice));
     SIM_TRY(cudaMalloc(&s->pix_count, sizeof(int32_t) * cp));
@@ -259,6 +288,10 @@ extern "C" int lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *ids,
 }
 
 extern "C" int lartpc_chunk_ticks(const lartpc_sim_t *sim) { return sim ? sim->dp.Jc : 0; }
+extern "C" int lartpc_response_mode(const lartpc_sim_t *sim)
+{
+    return sim ? (sim->dp.tc_mode ? LARTPC_RESPONSE_TENSOR : LARTPC_RESPONSE_FFMA) : LARTPC_ERR_BAD_ARGUMENT;
+}
 
 // ---- stage wrappers -------------------------------------------------------------------------------
 extern "C" int lartpc_quench(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, float *dEdx, float *n_e,
@@ -288,10 +321,11 @@ extern "C" int lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t 
 {
     if (!sim || !dr || !pm || !out) return LARTPC_ERR_BAD_ARGUMENT;
     if (!sim->have_plan || n != sim->plan_n) return LARTPC_ERR_ORDER;
-    if (out->tile_capacity < sim->n_tiles) return LARTPC_ERR_CAPACITY;
+    if (out->tile_capacity < tiles_alloc(sim->dp, sim->n_tiles)) return LARTPC_ERR_CAPACITY;
     if (sim->n_tiles > 0 && (!out->partial || !out->tile_range || !out->charge)) return LARTPC_ERR_BAD_ARGUMENT;
     int rc = launch_current_splat(sim, dr, pm, n, out, (cudaStream_t)stream);
-    if (rc == 0) rc = launch_current_response(sim, out, (cudaStream_t)stream);
+    if (rc == 0) rc = sim->dp.tc_mode ? launch_current_response_tc(sim, out, (cudaStream_t)stream)
+                                       : launch_current_response(sim, out, (cudaStream_t)stream);
     if (rc == 0) sim->have_signals = true;
     return rc;
 }
@@ -459,10 +493,10 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
         tm.end();
         ar.used = mark;
         lartpc_signals_t sig;
-        sig.tile_capacity = info.n_tiles;
+        sig.tile_capacity = tiles_alloc(p, info.n_tiles);
         sig.partial = ar.take<float>(info.n_tiles * p.WW * p.tile_ticks);
-        sig.tile_range = ar.take<int32_t>(info.n_tiles * 2);
-        sig.charge = ar.take<float>(info.n_tiles * p.slab_floats);
+        sig.tile_range = ar.take<int32_t>(info.n_tiles * TILE_META);
+        sig.charge = ar.take<float>(sig.tile_capacity * p.slab_floats);
         lartpc_waveforms_t wf;
         wf.pixel_capacity = info.n_active_pixels;  wf.sample_capacity = info.total_samples;
         wf.pixel_id = ar.take<int32_t>(info.n_active_pixels);
@@ -488,7 +522,8 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
         if ((rc = launch_current_splat(sim, &dr, &pm, n, &sig, st)) != 0) return rc;
         tm.end();
         tm.begin(4);
-        if ((rc = launch_current_response(sim, &sig, st)) != 0) return rc;
+        if ((rc = p.tc_mode ? launch_current_response_tc(sim, &sig, st) : launch_current_response(sim, &sig, st)) != 0)
+            return rc;
         tm.end();
         sim->have_signals = true;
         tm.begin(5);

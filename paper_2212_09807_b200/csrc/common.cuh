@@ -28,6 +28,9 @@ struct DevParams {
     int PG, NP;                      // target pairs per consumer group; pairs incl. padding = n_groups * PG
     int n_groups;                    // pair groups per tile = response passes over a tile (1 for W = 5, K = 200)
     int slab_floats;                 // packed charge lattice of one tile: header, bin items, charge rows
+                                     // (tensor-core mode: NB2 * 64 = the tile's rows of the fp16 hi / lo operand image)
+    int tc_mode;                     // 1: S4 response on the tensor cores (response_tc.cuh), 0: packed-FFMA2 response
+    int NBW;                         // tensor-core mode: output columns per 16-tick arrival block, roundup16(K + 15)
     int n_tpcs;
     // electronics
     double gain_mv_per_ke, v_cm, v_ref, v_ped, adc_full, threshold;
@@ -54,6 +57,8 @@ constexpr int LUT_OFF = 20;          // LUT tick k sits at pair-word LUT_OFF + k
 constexpr int SLAB_HDR = 4;          // slab header ints: bins, charge groups, first / last output block
 constexpr int RESP_NO = 14;          // output ticks per response task (one thread: RESP_NO ticks x 2 target pixels)
 constexpr int RESP_CONSUMERS = 256;  // consumer threads of the response kernel (8 warps, two per SM sub-partition)
+constexpr int TILE_META = 4;         // ints per tile in lartpc_signals_t.tile_range: first / last output block, scale exponent, 0
+constexpr int TC_TILE_BLOCK = 128;   // tiles per tensor-core tile block (MMA M)
 
 // device counters written by the planning kernels (mirrored to pinned host memory)
 enum {
@@ -67,6 +72,7 @@ struct lartpc_sim {
     DevParams dp;
     DevTpc *d_tpcs = nullptr;
     float *d_lut = nullptr;              // [NB2][WW][RS], zero padded rows
+    void *d_lut_tc = nullptr;            // tensor-core mode: fp16 hi / lo operand images of the LUT, [WW][NB2][2][NBW * 16]
     int64_t n_cp = 0;                    // charged-pixel grid cells over all TPCs
     int64_t n_pix = 0;                   // pixels over all TPCs (global pixel ids are 0 .. n_pix-1)
     int32_t pix_id_base = 0;
@@ -137,6 +143,12 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
 int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
                          lartpc_signals_t *out, cudaStream_t st);
 int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st);
+int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st);
+size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_out);   // returns bytes, 0 on failure
+static inline int64_t tiles_alloc(const DevParams &p, int64_t n_tiles)
+{
+    return p.tc_mode ? (n_tiles + TC_TILE_BLOCK - 1) / TC_TILE_BLOCK * TC_TILE_BLOCK : n_tiles;
+}
 int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out, cudaStream_t st);
 int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
                        int32_t *slot_scratch, int32_t *scan_scratch, int64_t hit_base, cudaStream_t st);

@@ -27,6 +27,7 @@
 #include <string.h>
 #include <algorithm>
 #include "common.cuh"
+#include "response_tc.cuh"
 
 namespace {
 
@@ -319,13 +320,15 @@ __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs 
     float *slab = a.charge + (size_t)tile * p.slab_floats;
     int *slab_i = (int *)slab;
     if (nbins == 0) {
+        // no charge: S5 skips the tile (first block > last block); the tensor-core response still multiplies whatever
+        // the tile's operand rows hold, and nobody reads the result
         if (tid == 0) {
-            slab_i[0] = 0; slab_i[1] = 0; slab_i[2] = 1; slab_i[3] = 0;
-            a.tile_range[2 * tile] = 1;  a.tile_range[2 * tile + 1] = 0;
+            if (!p.tc_mode) { slab_i[0] = 0; slab_i[1] = 0; slab_i[2] = 1; slab_i[3] = 0; }
+            *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(1, 0, 0, 0);
         }
-        return;
+        if (!p.tc_mode) return;
     }
-    {
+    if (nbins) {
         // multiply-adds the method needs here: non-zero cells x in-plane targets x K
         for (int d = 16; d; d >>= 1) nz_cells += __shfl_xor_sync(0xffffffffu, nz_cells, d);
         const int vx = min(td.px + p.H, tp.nx - 1) - max(td.px - p.H, 0) + 1;
@@ -334,11 +337,43 @@ __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs 
             atomicAdd(a.fma_counter, (unsigned long long)nz_cells * (unsigned long long)(vx * vy * K));
     }
 
-    // ------------------------------------------------------------------ phase 3: packed tile out
+    // ------------------------------------------------------------------ phase 3: tile out
     const int nB_lo = tjlo / RESP_NO, nB_hi = (tjhi + K - 1) / RESP_NO; // output blocks, tile-relative
+    if (p.tc_mode) {
+        // Tensor-core operand image (response_tc.cuh): C * 2^-e split into fp16 hi + lo, row (tile % 128) of the
+        // 128-byte-swizzled K-major [128 x 64] block of every bin; e keeps the largest cell below 2^15.
+        float mx = 0.f;
+        for (int i = tid; i < NB2 * CJ; i += NT1) mx = fmaxf(mx, fabsf(Csm[i]));
+        for (int d = 16; d; d >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+        __syncthreads();                                                  // scratch is free: the splat is over
+        if (lane == 0) scratch[warp] = mx;
+        __syncthreads();
+        mx = scratch[0];
+#pragma unroll
+        for (int w = 1; w < NT1 / 32; ++w) mx = fmaxf(mx, scratch[w]);
+        int e = 0;
+        if (mx >= 32768.f) e = min(((__float_as_int(mx) >> 23) & 0xff) - 127 - 14, 100);   // mx * 2^-e in [2^14, 2^15)
+        if (!(mx < 3.0e38f)) e = 0;                                       // inf / nan charge: leave it visible
+        const float sc = __int_as_float((127 - e) << 23);
+        if (tid == 0 && nbins) *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(nB_lo, nB_hi, e, 0);
+        const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;
+        __half *Ab = (__half *)a.charge + (size_t)tb * NB2 * (2 * rtc::TB * rtc::JC);
+        const int k = 2 * lane, off = rtc::a_image_offset(r, k);
+        for (int c = warp; c < NB2; c += NT1 / 32) {
+            const float2 x = *(const float2 *)(Csm + c * CJ + k);
+            const float x0 = x.x * sc, x1 = x.y * sc;
+            const __half2 hi = __floats2half2_rn(x0, x1);
+            const float2 hf = __half22float2(hi);
+            const __half2 lo = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
+            __half *dst = Ab + (size_t)c * (2 * rtc::TB * rtc::JC) + off;
+            *(__half2 *)dst = hi;
+            *(__half2 *)(dst + rtc::TB * rtc::JC) = lo;
+        }
+        return;
+    }
     if (tid == 0) {
         slab_i[0] = nbins; slab_i[1] = s_misc[3]; slab_i[2] = nB_lo; slab_i[3] = nB_hi;
-        a.tile_range[2 * tile] = nB_lo;  a.tile_range[2 * tile + 1] = nB_hi;
+        *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(nB_lo, nB_hi, 0, 0);
     }
     for (int k = tid; k < nbins; k += NT1) {
         const int c = bin_list[k], jb0 = bin_jlo[c] & ~1, ng = ((bin_jhi[c] - jb0) >> 2) + 1;
@@ -683,4 +718,63 @@ size_t lartpc_splat_smem(const DevParams &p) { return splat_smem_bytes(p); }
 size_t lartpc_response_smem(const DevParams &p)
 {
     return 2 * (size_t)response_stage_floats(p) * 4 + 64;           // at least two stages must fit
+}
+
+// =====================================================================================================
+// Tensor-core response: launcher and the LUT operand images
+// =====================================================================================================
+int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st)
+{
+    const DevParams &p = sim->dp;
+    if (sim->n_tiles == 0) return LARTPC_OK;
+    if (p.Jc != rtc::JC || !sim->d_lut_tc) return LARTPC_ERR_UNSUPPORTED;
+    rtc::Args a;
+    a.A = (const __half *)out->charge;
+    a.B = (const __half *)sim->d_lut_tc;
+    a.partial = out->partial;
+    a.tile_meta = out->tile_range;
+    if (sim->n_tiles >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
+    a.n_tiles = (int)sim->n_tiles;
+    a.n_tb = (int)((sim->n_tiles + rtc::TB - 1) / rtc::TB);
+    a.NC = p.NB2;  a.WW = p.WW;  a.NBW = p.NBW;  a.tile_ticks = p.tile_ticks;
+    a.n_items = (long long)a.n_tb * p.WW;
+    const int smem = rtc::smem_bytes(p.NBW);
+    static int configured = 0;
+    if (smem > configured) {
+        LARTPC_CUDA_TRY(cudaFuncSetAttribute(rtc::response_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        configured = smem;
+    }
+    const int grid = (int)std::min<long long>(a.n_items, sim->sm_count);
+    ++g_lartpc_launches;
+    rtc::response_tc_kernel<<<grid, rtc::THREADS, smem, st>>>(a);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}
+
+// Bs[d][c][hi | lo][NBW x 16] with Bs[n'][jj] = R[c][d][n' - jj] * 2^10 (0 outside the LUT), each half in the canonical
+// un-swizzled K-major layout of rtc::b_image_offset.  Built once per sim on the host.
+size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_out)
+{
+    const int nb = p.nb, W = p.W, K = p.K, NBW = p.NBW, NB = W * nb;
+    const size_t half_elems = (size_t)NBW * 16, n = (size_t)p.WW * p.NB2 * 2 * half_elems;
+    std::vector<__half> img(n);
+    for (int d = 0; d < p.WW; ++d) {
+        const int dyi = d / W, dxi = d - dyi * W;
+        for (int cb = 0; cb < nb; ++cb)
+            for (int ca = 0; ca < nb; ++ca) {
+                const float *src = lut_host + ((size_t)(nb * dyi + cb) * NB + (nb * dxi + ca)) * K;
+                __half *hi = img.data() + ((size_t)d * p.NB2 + (cb * nb + ca)) * 2 * half_elems, *lo = hi + half_elems;
+                for (int nn = 0; nn < NBW; ++nn)
+                    for (int jj = 0; jj < 16; ++jj) {
+                        const int k = nn - jj;
+                        const float x = (k >= 0 && k < K) ? ldexpf(src[k], rtc::B_SCALE_LOG2) : 0.f;
+                        const __half h = __float2half_rn(x);
+                        hi[rtc::b_image_offset(nn, jj)] = h;
+                        lo[rtc::b_image_offset(nn, jj)] = __float2half_rn(x - __half2float(h));
+                    }
+            }
+    }
+    if (cudaMalloc(d_out, n * sizeof(__half)) != cudaSuccess) return 0;
+    if (cudaMemcpy(*d_out, img.data(), n * sizeof(__half), cudaMemcpyHostToDevice) != cudaSuccess) return 0;
+    return n * sizeof(__half);
 }

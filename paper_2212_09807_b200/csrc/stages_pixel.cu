@@ -65,7 +65,7 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
                 if (w >= 64) below += __popcll(s_mask[d][0]);
                 const int tix = s_tile0[d] + below;
                 const int nrel = r - w * p.Jc, blk = nrel / RESP_NO;
-                if (blk >= tile_range[2 * tix] && blk <= tile_range[2 * tix + 1])
+                if (blk >= tile_range[TILE_META * tix] && blk <= tile_range[TILE_META * tix + 1])
                     sum += partial[((size_t)tix * p.WW + d) * p.tile_ticks + nrel];
             }
         }

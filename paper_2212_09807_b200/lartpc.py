@@ -104,7 +104,7 @@ class Stats(C.Structure):
                [("n_batches", C.c_int32), ("reserved", C.c_int32), ("flops_current", C.c_double)]
 
 
-EXPORTS = ("lartpc_sim_create", "lartpc_sim_destroy", "lartpc_set_disabled_pixels", "lartpc_chunk_ticks",
+EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", "lartpc_sim_destroy", "lartpc_set_disabled_pixels", "lartpc_chunk_ticks",
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
            "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_run_spill",
            "lartpc_measure_fp32_peak", "lartpc_set_profiling", "lartpc_get_stage_ms", "lartpc_kernel_launches", "lartpc_strerror")
@@ -163,7 +163,11 @@ def kernel_launches() -> int:
 class Sim:
     """Owns a ``lartpc_sim_t`` (detector / physics parameters, TPC table, response LUT)."""
 
-    def __init__(self, params: Dict, tpcs: Sequence[dict], lut: np.ndarray, device: str = "cuda:0"):
+    RESPONSE_MODES = {"auto": 0, "tensor": 1, "ffma": 2}
+
+    def __init__(self, params: Dict, tpcs: Sequence[dict], lut: np.ndarray, device: str = "cuda:0",
+                 response: str = "auto"):
+        """``response``: how S4 applies the LUT -- "tensor" (tcgen05), "ffma" (FP32 pipe) or "auto"."""
         torch = _torch()
         self.torch = torch
         self.device = torch.device(device)
@@ -180,10 +184,12 @@ class Sim:
                          t["first_pixel_id"])
         lut = np.ascontiguousarray(lut, dtype=np.float32)
         h = C.c_void_p()
-        _check(self.lib.lartpc_sim_create(C.byref(p), arr, C.c_int(len(tpcs)),
-                                          lut.ctypes.data_as(C.c_void_p), C.c_size_t(lut.size), C.byref(h)),
-               "lartpc_sim_create")
+        _check(self.lib.lartpc_sim_create_ex(C.byref(p), arr, C.c_int(len(tpcs)),
+                                             lut.ctypes.data_as(C.c_void_p), C.c_size_t(lut.size),
+                                             C.c_int(self.RESPONSE_MODES[response]), C.byref(h)),
+               "lartpc_sim_create_ex")
         self.handle = h
+        self.response_mode = {1: "tensor", 2: "ffma"}[int(self.lib.lartpc_response_mode(self.handle))]
         self.chunk_ticks = int(self.lib.lartpc_chunk_ticks(self.handle))
         self.info: Optional[PixmapInfo] = None
         self._keep = {}
@@ -271,10 +277,11 @@ class Sim:
         t = self.torch
         info = self.info
         nt = int(info.n_tiles)
+        nt_cap = (nt + 127) // 128 * 128                 # the tensor-core operand image comes in 128-tile blocks
         out = dict(partial=self._empty(nt * info.tile_targets * info.tile_ticks, t.float32),
-                   tile_range=self._empty(nt * 2, t.int32),
-                   charge=self._empty(nt * info.tile_charge_floats, t.float32))
-        sig = Signals(nt, out["partial"].data_ptr(), out["tile_range"].data_ptr(), out["charge"].data_ptr())
+                   tile_range=self._empty(nt * 4, t.int32),
+                   charge=self._empty(nt_cap * info.tile_charge_floats, t.float32))
+        sig = Signals(nt_cap, out["partial"].data_ptr(), out["tile_range"].data_ptr(), out["charge"].data_ptr())
         _check(self.lib.lartpc_induced_current(self.handle, C.byref(drifted["_struct"]), C.byref(pixmap["_struct"]),
                                                C.c_int64(pixmap["_n"]), C.byref(sig), _stream_ptr(t)),
                "lartpc_induced_current")

@@ -91,6 +91,7 @@ def _check_currents(res, wl, dr, pm, max_pixels=None, seed=0):
         worst_w = max(worst_w, (err / (1e-4 * peak + 0.02)).max())
         # Q_p reported by S6 is the same sum
         assert np.allclose(res["hits"]["q_pixel"][sel], gq, rtol=1e-5, atol=0.05)
+    print("currents vs oracle: worst |dQ| / tol = %.3f, worst sample error / tol = %.3f" % (worst_q, worst_w))
     return worst_q, worst_w
 
 
@@ -110,10 +111,15 @@ def _check_hits(res, wl, dr, pm, seed):
     return frac
 
 
-def test_config0_full_chain(lartpc):
+MODES = ["tensor", "ffma"]          # both S4 response paths are held to the same bar
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_config0_full_chain(lartpc, mode):
     """BASELINE configs[0]: 100 segments of one MIP track, every stage and every active pixel."""
     wl = W.make_config(0)
-    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, response=mode)
+    assert sim.response_mode == mode
     res = run_staged(sim, wl)
     dr, pm = _check_segment_stages(res, wl)
     _check_currents(res, wl, dr, pm)
@@ -148,18 +154,20 @@ def test_run_spill_matches_staged(lartpc):
     sim.close()
 
 
-def test_config1_sampled_pixels(lartpc):
+@pytest.mark.parametrize("mode", MODES)
+def test_config1_sampled_pixels(lartpc, mode):
     """BASELINE configs[1] (cosmics, 70x70 pixels, 30 cm drift, noise on): all segment stages, and the
     currents of a sample of pixels (the busiest ones plus a random draw) against the oracle."""
     wl = W.make_config(1)
-    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, response=mode)
     res = run_staged(sim, wl)
     dr, pm = _check_segment_stages(res, wl)
     _check_currents(res, wl, dr, pm, max_pixels=48)
     sim.close()
 
 
-def test_zero_drift_and_edges(lartpc):
+@pytest.mark.parametrize("mode", MODES)
+def test_zero_drift_and_edges(lartpc, mode):
     """Degenerate cases: segments at the anode (sigma = 0, indicator weights), at the plane edge (charge bins
     outside the plane act on in-plane pixels), outside every TPC, zero length and zero energy."""
     p = W.default_params(n_readout_ticks=900)
@@ -178,7 +186,7 @@ def test_zero_drift_and_edges(lartpc):
     seg["xe"][-1] = seg["xs"][-1]; seg["ye"][-1] = seg["ys"][-1]; seg["ze"][-1] = seg["zs"][-1]    # zero length
     seg["dE"][-2] = 0.0                                                                               # zero energy
     wl = W.Workload("edges", 5, p, tpcs, seg, W.pad_response_lut(p))
-    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, response=mode)
     res = run_staged(sim, wl)
     dr, pm = _check_segment_stages(res, wl)
     _check_currents(res, wl, dr, pm)
