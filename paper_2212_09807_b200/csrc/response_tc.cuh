@@ -22,8 +22,10 @@
 //                      stage, tcgen05.commit frees the stage; after the last bin a commit signals the epilogue
 //   warps 2-5          epilogue: tcgen05.ld the 128 x 264 fp32 accumulator (thread = tile row), undo the scales, write
 //                      the partial waveform rows, re-zero the TMEM columns that only later blocks b touch
-// Items are dealt round-robin (all cost the same), consecutive items share the tile block, so the 25 CTAs that stream
-// one A block do it at the same time and A is read from HBM once.
+// Items are taken from an atomic cursor by the producer (which hands the item to the MMA warp in a stage header and
+// from there to the epilogue), consecutive items share the tile block, so the 25 CTAs that stream one A block do it at
+// the same time and A is read from HBM once.  (A static round-robin deal lets the CTAs drift apart over a long
+// launch: measured, the L2 reuse of A is lost and the kernel becomes HBM-bound.)
 #pragma once
 #include <cuda_fp16.h>
 #include <stdint.h>
@@ -45,6 +47,8 @@ struct Args {
     const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), 0
     int n_tiles, n_tb, NC, WW, NBW, tile_ticks;
     long long n_items;             // n_tb * WW
+    int *work;                     // item cursor, zero at launch: items are taken in order as CTAs become free, so the
+                                   // CTAs that stream one tile block stay together however long the launch runs
 };
 
 // byte image of one precision half of an A stage: row r (tile in block), element k (arrival tick), SWIZZLE_128B K-major
@@ -139,7 +143,8 @@ __device__ __forceinline__ void tmem_zero16(uint32_t taddr)
 }
 
 constexpr int stage_bytes(int NBW) { return 2 * A_HALF_BYTES + 2 * NBW * 32; }
-constexpr int smem_bytes(int NBW) { return STAGES * stage_bytes(NBW) + 1024 /* alignment slack */ + 256 /* barriers */; }
+constexpr int smem_bytes(int NBW) { return STAGES * stage_bytes(NBW) + 1024 /* alignment slack */ + 256 /* barriers, headers */; }
+constexpr int HDR_LAST = 1, HDR_END = 2;
 
 __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
 {
@@ -152,13 +157,16 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
     const uint32_t base = (s32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bars = base + STAGES * stage_sz;                    // full[S], empty[S], tmem_full, tmem_empty, tmem ptr
     const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull = bars + 16 * STAGES, tempty = tfull + 8;
-    const uint32_t tptr_addr = tempty + 8;
+    const uint32_t titem = tempty + 8, tptr_addr = titem + 8;
     volatile uint32_t *tptr = (volatile uint32_t *)(smem_raw + (tptr_addr - s32(smem_raw)));
+    volatile int4 *hdr = (volatile int4 *)(smem_raw + (tptr_addr + 8 - s32(smem_raw)));   // [STAGES] {tb, d, c, flags}
+    volatile int4 *epi_item = hdr + STAGES;                                              // {tb, d, 0, flags}
 
     if (tid == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
         mbar_init(tfull, 1);
         mbar_init(tempty, 4);                                          // one arrival per epilogue warp
+        mbar_init(titem, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {                                                   // the MMA warp owns the TMEM allocation
@@ -176,19 +184,26 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
         if (lane == 0) {
             int s = 0;
             uint32_t ph = 0;
-            for (long long q = blockIdx.x; q < a.n_items; q += gridDim.x) {
+            long long q = atomicAdd(a.work, 1);
+            while (q < a.n_items) {
+                const long long q_next = atomicAdd(a.work, 1);         // in flight while this item streams
                 const int tb = (int)(q / a.WW), d = (int)(q - (long long)tb * a.WW);
                 const unsigned char *Ab = (const unsigned char *)a.A + (size_t)tb * NC * (2 * A_HALF_BYTES);
                 const unsigned char *Bb = (const unsigned char *)a.B + (size_t)d * NC * (2 * b_half);
                 for (int c = 0; c < NC; ++c) {
                     mbar_wait(empty0 + 8 * s, ph ^ 1u);
                     const uint32_t st = base + s * stage_sz, fb = full0 + 8 * s;
-                    mbar_expect_tx(fb, stage_sz);
+                    hdr[s].x = tb;  hdr[s].y = d;  hdr[s].z = c;  hdr[s].w = (c == NC - 1) ? HDR_LAST : 0;
+                    mbar_expect_tx(fb, stage_sz);                      // release: the header is visible to the waiter
                     bulk_g2s(st, Ab + (size_t)c * (2 * A_HALF_BYTES), 2 * A_HALF_BYTES, fb);
                     bulk_g2s(st + 2 * A_HALF_BYTES, Bb + (size_t)c * (2 * b_half), 2 * b_half, fb);
                     if (++s == STAGES) { s = 0; ph ^= 1u; }
                 }
+                q = q_next;
             }
+            mbar_wait(empty0 + 8 * s, ph ^ 1u);                        // terminator: a header-only stage
+            hdr[s].w = HDR_END;
+            mbar_arrive(full0 + 8 * s);
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
@@ -197,29 +212,36 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
             const uint32_t idesc = (1u << 4) | ((uint32_t)(NBW >> 3) << 17) | ((uint32_t)(TB >> 4) << 24);
             int s = 0;
             uint32_t ph = 0, tph = 0;
-            for (long long q = blockIdx.x; q < a.n_items; q += gridDim.x) {
-                mbar_wait(tempty, tph);                                // accumulator drained and re-zeroed
-                tc_fence_after();
-                for (int c = 0; c < NC; ++c) {
-                    mbar_wait(full0 + 8 * s, ph);
-                    tc_fence_after();
-                    const uint32_t st = base + s * stage_sz;
-                    const uint64_t bd_hi = smem_desc(st + 2 * A_HALF_BYTES, 128, 256, 0);
-                    const uint64_t bd_lo = smem_desc(st + 2 * A_HALF_BYTES + b_half, 128, 256, 0);
-#pragma unroll
-                    for (int b = 0; b < NBLK; ++b) {
-                        const uint64_t ad_hi = smem_desc(st + 32 * b, 16, 1024, 2);
-                        const uint64_t ad_lo = smem_desc(st + A_HALF_BYTES + 32 * b, 16, 1024, 2);
-                        const uint32_t dcol = tmem + 16 * b;
-                        tc_mma_f16(dcol, ad_hi, bd_hi, idesc, (c | b) ? 1u : 0u);
-                        tc_mma_f16(dcol, ad_hi, bd_lo, idesc, 1u);
-                        tc_mma_f16(dcol, ad_lo, bd_hi, idesc, 1u);
-                    }
-                    tc_commit(empty0 + 8 * s);                         // stage free once these MMAs have read it
-                    if (++s == STAGES) { s = 0; ph ^= 1u; }
+            while (true) {
+                mbar_wait(full0 + 8 * s, ph);
+                const int tb = hdr[s].x, d = hdr[s].y, c = hdr[s].z, flags = hdr[s].w;
+                if (flags & HDR_END) {
+                    mbar_wait(tempty, tph);                            // the epilogue has read the previous item slot
+                    epi_item->w = HDR_END;
+                    mbar_arrive(titem);
+                    break;
                 }
-                tc_commit(tfull);                                      // accumulator complete
-                tph ^= 1u;
+                if (c == 0) {
+                    mbar_wait(tempty, tph);                            // accumulator drained and re-zeroed
+                    epi_item->x = tb;  epi_item->y = d;  epi_item->w = 0;
+                    mbar_arrive(titem);                                // release: hands the item to the epilogue
+                }
+                tc_fence_after();
+                const uint32_t st = base + s * stage_sz;
+                const uint64_t bd_hi = smem_desc(st + 2 * A_HALF_BYTES, 128, 256, 0);
+                const uint64_t bd_lo = smem_desc(st + 2 * A_HALF_BYTES + b_half, 128, 256, 0);
+#pragma unroll
+                for (int b = 0; b < NBLK; ++b) {
+                    const uint64_t ad_hi = smem_desc(st + 32 * b, 16, 1024, 2);
+                    const uint64_t ad_lo = smem_desc(st + A_HALF_BYTES + 32 * b, 16, 1024, 2);
+                    const uint32_t dcol = tmem + 16 * b;
+                    tc_mma_f16(dcol, ad_hi, bd_hi, idesc, (c | b) ? 1u : 0u);
+                    tc_mma_f16(dcol, ad_hi, bd_lo, idesc, 1u);
+                    tc_mma_f16(dcol, ad_lo, bd_hi, idesc, 1u);
+                }
+                tc_commit(empty0 + 8 * s);                             // stage free once these MMAs have read it
+                if (flags & HDR_LAST) { tc_commit(tfull); tph ^= 1u; } // accumulator complete
+                if (++s == STAGES) { s = 0; ph ^= 1u; }
             }
         }
     } else {
@@ -234,8 +256,10 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
         if (lane == 0) mbar_arrive(tempty);
         uint32_t tph = 0;
         const int n_full = a.tile_ticks / 32, n_rem = a.tile_ticks - 32 * n_full;   // tile_ticks = 264: 8 x 32 + 8
-        for (long long q = blockIdx.x; q < a.n_items; q += gridDim.x) {
-            const int tb = (int)(q / a.WW), d = (int)(q - (long long)tb * a.WW);
+        while (true) {
+            mbar_wait(titem, tph);                                     // acquire: the MMA warp has published the item
+            if (epi_item->w & HDR_END) break;
+            const int tb = epi_item->x, d = epi_item->y;
             const int tile = tb * TB + 32 * quad + lane;
             const bool live = tile < a.n_tiles;
             float scale = 0.f;
@@ -250,8 +274,8 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 if (live) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i)
-                        ((float4 *)(dst + 32 * ch))[i] = make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
-                                                                     __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale);
+                        __stcs((float4 *)(dst + 32 * ch) + i, make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
+                                                                     __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale));
                 }
             }
             if (n_rem) {
@@ -261,8 +285,8 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 if (live) {
 #pragma unroll
                     for (int i = 0; i < 2; ++i)
-                        ((float4 *)(dst + 32 * n_full))[i] = make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
-                                                                         __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale);
+                        __stcs((float4 *)(dst + 32 * n_full) + i, make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
+                                                                         __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale));
                 }
             }
             for (int c0 = NBW; c0 < n_acc_cols; c0 += 16) tmem_zero16(tlane + c0);

@@ -738,6 +738,9 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     a.n_tb = (int)((sim->n_tiles + rtc::TB - 1) / rtc::TB);
     a.NC = p.NB2;  a.WW = p.WW;  a.NBW = p.NBW;  a.tile_ticks = p.tile_ticks;
     a.n_items = (long long)a.n_tb * p.WW;
+    if (a.n_items >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
+    a.work = sim->d_work;
+    LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
     const int smem = rtc::smem_bytes(p.NBW);
     static int configured = 0;
     if (smem > configured) {
