@@ -1,6 +1,7 @@
 // C-ABI entry points of liblartpc (include/lartpc.h): sim lifetime, stage wrappers, the spill driver
 // and the FP32 peak microbenchmark used as the roofline denominator of S4.
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include <algorithm>
 #include <new>
@@ -133,6 +134,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     s->params = *prm;
     s->tpcs.assign(tpcs, tpcs + n_tpcs);
     s->sm_count = prop.multiProcessorCount;
+    { const char *e = getenv("LARTPC_SPLAT"); s->splat_tc = !(e && strcmp(e, "ffma") == 0); }   // measurement aid
     DevParams &p = s->dp;
     memset(&p, 0, sizeof(p));
     p.eps = prm->e_field_kv_cm * prm->lar_density_g_cm3;  p.w_ion = prm->w_ion_mev;

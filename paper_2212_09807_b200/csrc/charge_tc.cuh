@@ -1,0 +1,280 @@
+// S4 charge lattice on the tensor cores (included by stage_current.cu inside its anonymous namespace, after SplatArgs
+// and SegLocal).  Eq. (3.8) in expectation, reading D1:
+//     C[b][a][j] = sum_seg sum_mu (Q_a / N) wx_mu[a] wy_mu[b] wt_mu[j]
+// is, per tile, the matrix product  D[m = b nb + a][j] = sum_s WXY[m][s] WT[j][s]  over the samples s of every segment
+// that crosses the tile: M = 128 cell rows (nb^2 = 100 used), N = 64 arrival ticks, K = samples.  One CTA per tile,
+// 128 threads, 64 samples per batch: warps 0-1 build the WXY operand of their sample (11 + 11 erf, 100 products), warps
+// 2-3 the WT operand (up to 65 erf), both split hi + lo in fp16 and stored MN-major (a thread writes 16-byte runs of
+// cells / ticks of its own sample column: conflict-free STS.128) in the canonical un-swizzled UMMA layout; thread 0
+// then issues 3 x ceil(samples / 16) tcgen05.mma (hi hi + hi lo + lo hi) into a 64-column TMEM accumulator.  When the
+// last segment is in, every thread reads its cell row from TMEM, the tile's scale exponent is agreed on, and the row
+// goes out as the fp16 hi / lo operand image the tensor-core response reads (rtc::a_image_offset).
+// sigma = 0 segments take the float64 indicator path of the oracle (one-hot weights), as in charge_lattice_kernel.
+
+constexpr int CT_THREADS = 128;
+constexpr int CT_KB = 64;                              // samples per batch
+constexpr int CT_A_HALF = 128 * CT_KB * 2;             // bytes of one precision half of the WXY operand (16 KB)
+constexpr int CT_B_HALF = 64 * CT_KB * 2;              // ... of the WT operand (8 KB)
+constexpr int CT_SMEM = 2 * CT_A_HALF + 2 * CT_B_HALF + 1024 + sizeof(SegLocal) * SEGCAP;
+
+// MN-major canonical layout: element (mn, k) of an operand with G groups of 8 along MN:
+//   (mn % 8) * 2 + (k % 8) * 16 + (mn / 8) * 128 [SBO] + (k / 8) * 128 * G [LBO]   bytes
+__device__ __forceinline__ uint32_t ct_col_offset(int k, int G) { return (uint32_t)((k & 7) * 16 + (k >> 3) * 128 * G); }
+
+__device__ __forceinline__ void split_store8(unsigned char *hi, unsigned char *lo, const float (&x)[8])
+{
+    __half2 h[4], l[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        h[i] = __floats2half2_rn(x[2 * i], x[2 * i + 1]);
+        const float2 f = __half22float2(h[i]);
+        l[i] = __floats2half2_rn(x[2 * i] - f.x, x[2 * i + 1] - f.y);
+    }
+    *(uint4 *)hi = *(const uint4 *)h;
+    *(uint4 *)lo = *(const uint4 *)l;
+}
+
+template <int NB>
+__global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const SplatArgs a)
+{
+    extern __shared__ unsigned char smem_dyn[];
+    const DevParams &p = a.p;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NB2 = NB * NB;
+    constexpr int MG = 16, NG = 8;                                   // groups of 8 along M (128 cells) and N (64 ticks)
+    const uint32_t sbase = (rtc::s32(smem_dyn) + 127u) & ~127u;
+    unsigned char *base = smem_dyn + (sbase - rtc::s32(smem_dyn));
+    unsigned char *Ahi = base, *Alo = base + CT_A_HALF, *Bhi = base + 2 * CT_A_HALF, *Blo = Bhi + CT_B_HALF;
+    unsigned char *ctl = Blo + CT_B_HALF;                            // mbarrier, TMEM pointer, reduction scratch
+    const uint32_t bar = sbase + 2 * CT_A_HALF + 2 * CT_B_HALF, tptr_addr = bar + 8;
+    volatile uint32_t *tptr = (volatile uint32_t *)(ctl + 8);
+    float *red = (float *)(ctl + 16);                                // [4] max, then ints
+    int *redi = (int *)(ctl + 32);                                   // [4][3] lo, hi, nz
+    SegLocal *segs = (SegLocal *)(ctl + 128);
+
+    const int tile = blockIdx.x;
+    const TileDesc td = a.tile_desc[tile];
+    const int cp = a.tile_cp[tile];
+    const DevTpc &tp = a.tpcs[td.tpc];
+    const int A_t = td.px * NB, B_t = td.py * NB, J_t = td.j_start;
+    const int lstart = a.pix_start[cp], lcount = a.pix_count[cp];
+
+    if (tid == 0) {
+        rtc::mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tptr_addr), "r"(64u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    // cell rows NB2 .. 127 of the WXY operand are never written: zero the whole operand once
+    for (int i = tid; i < 2 * CT_A_HALF / 16; i += CT_THREADS) ((uint4 *)Ahi)[i] = make_uint4(0u, 0u, 0u, 0u);
+    rtc::tc_fence_before();
+    __syncthreads();
+    rtc::tc_fence_after();
+    const uint32_t tmem = *tptr;
+    // instruction descriptor: D fp32, A / B fp16, both MN-major, N = 64, M = 128
+    const uint32_t idesc = (1u << 4) | (1u << 15) | (1u << 16) | ((uint32_t)(64 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+
+    const int s_in = tid & (CT_KB - 1);                              // sample column of this thread
+    const bool role_a = tid < CT_KB;                                 // warps 0-1: WXY, warps 2-3: WT
+    uint32_t mma_phase = 0;
+    bool any_mma = false;
+
+    for (int l0 = 0; l0 < lcount; l0 += SEGCAP) {
+        __syncthreads();
+        const int nseg = min(SEGCAP, lcount - l0);
+        if (tid < nseg) {
+            const int s = a.pair_seg[lstart + l0 + tid];
+            SegLocal L;
+            L.seg = s;
+            L.N = a.n_samples[s];
+            L.alo = max(a.a_lo[s] - A_t, 0);  L.ahi = min(a.a_hi[s] - A_t, NB - 1);
+            L.blo = max(a.b_lo[s] - B_t, 0);  L.bhi = min(a.b_hi[s] - B_t, NB - 1);
+            L.jlo = max(max(a.jt0[s], 0) - J_t, 0);
+            L.jhi = min(min(a.jt1[s], p.j_max) - J_t, p.Jc - 1);
+            const double inv_bin = 1.0 / p.bin, inv_dt = 1.0 / p.dt;
+            L.as = (float)(a.u_s[s] * inv_bin - (double)A_t);  L.ae = (float)(a.u_e[s] * inv_bin - (double)A_t);
+            L.bs = (float)(a.v_s[s] * inv_bin - (double)B_t);  L.be = (float)(a.v_e[s] * inv_bin - (double)B_t);
+            L.ts = (float)((a.T_s[s] - p.t_origin) * inv_dt - (double)J_t);
+            L.te = (float)((a.T_e[s] - p.t_origin) * inv_dt - (double)J_t);
+            const float sT = a.sigma_T[s], st = a.sigma_t[s];
+            L.zero_sigma = !(sT > 0.0f) || !(st > 0.0f);
+            L.isT = L.zero_sigma ? 0.f : (float)(p.bin * 0.70710678118654752440 / (double)sT);
+            L.ist = L.zero_sigma ? 0.f : (float)(p.dt * 0.70710678118654752440 / (double)st);
+            L.q = a.q_anode[s] / (float)L.N;                          // eq. (3.8): Q_a / N per sample point
+            segs[tid] = L;
+        }
+        __syncthreads();
+        for (int li = 0; li < nseg; ++li) {
+            const SegLocal L = segs[li];
+            if (L.jlo > L.jhi || L.alo > L.ahi || L.blo > L.bhi) continue;          // CTA-uniform
+            const float invN = 1.0f / (float)L.N;
+            for (int mu0 = 0; mu0 < L.N; mu0 += CT_KB) {
+                const int nsb = min(CT_KB, L.N - mu0), nk16 = (nsb + 15) >> 4;
+                if (s_in < 16 * nk16) {
+                    const bool real = s_in < nsb;
+                    const int mu = mu0 + s_in;
+                    const float f = ((float)mu + 0.5f) * invN;
+                    // sigma = 0: the bin / tick is an integer decision taken in float64 in the oracle's order
+                    int ia = -1, ib = -1, jj = -1;
+                    if (L.zero_sigma && real) {
+                        const int s = L.seg;
+                        const double fd = xdiv(xadd((double)mu, 0.5), (double)L.N);
+                        if (role_a) {
+                            const double us = a.u_s[s], ue = a.u_e[s], vs = a.v_s[s], ve = a.v_e[s];
+                            const long long xa = (long long)floor(xdiv(xadd(us, xmul(xsub(ue, us), fd)), p.bin)) - A_t;
+                            const long long xb = (long long)floor(xdiv(xadd(vs, xmul(xsub(ve, vs), fd)), p.bin)) - B_t;
+                            if (xa >= 0 && xa < NB && xb >= 0 && xb < NB) { ia = (int)xa; ib = (int)xb; }
+                        } else {
+                            const double Ts = a.T_s[s], Te = a.T_e[s];
+                            long long j = (long long)floor(xdiv(xsub(xadd(Ts, xmul(xsub(Te, Ts), fd)), p.t_origin), p.dt));
+                            if (j >= 0 && j <= p.j_max && j - J_t >= 0 && j - J_t < p.Jc) jj = (int)(j - J_t);
+                        }
+                    }
+                    if (role_a) {
+                        float wx[NB], wy[NB];
+                        if (!real) {
+#pragma unroll
+                            for (int i = 0; i < NB; ++i) wx[i] = wy[i] = 0.f;
+                        } else if (L.zero_sigma) {
+#pragma unroll
+                            for (int i = 0; i < NB; ++i) { wx[i] = (i == ia) ? 1.f : 0.f; wy[i] = (i == ib) ? 1.f : 0.f; }
+                        } else {
+                            const float px = fmaf(L.ae - L.as, f, L.as), py = fmaf(L.be - L.bs, f, L.bs);
+                            float ex = erff((0.f - px) * L.isT), ey = erff((0.f - py) * L.isT);
+#pragma unroll
+                            for (int i = 0; i < NB; ++i) {
+                                const float ex1 = erff(((float)(i + 1) - px) * L.isT), ey1 = erff(((float)(i + 1) - py) * L.isT);
+                                wx[i] = (i >= L.alo && i <= L.ahi) ? 0.5f * (ex1 - ex) : 0.f;
+                                wy[i] = (i >= L.blo && i <= L.bhi) ? 0.5f * (ey1 - ey) : 0.f;
+                                ex = ex1;  ey = ey1;
+                            }
+                        }
+                        const uint32_t col = ct_col_offset(s_in, MG);
+#pragma unroll
+                        for (int g = 0; g < (NB2 + 7) / 8; ++g) {
+                            float x[8];
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) {
+                                const int m = 8 * g + i;
+                                x[i] = m < NB2 ? wx[m % NB] * wy[m / NB] : 0.f;
+                            }
+                            split_store8(Ahi + col + 128 * g, Alo + col + 128 * g, x);
+                        }
+                    } else {
+                        const uint32_t col = ct_col_offset(s_in, NG);
+                        const float pt = fmaf(L.te - L.ts, f, L.ts);
+                        for (int g = 0; g < NG; ++g) {
+                            float x[8];
+                            const int j0 = 8 * g;
+                            if (!real || j0 + 7 < L.jlo || j0 > L.jhi) {
+#pragma unroll
+                                for (int i = 0; i < 8; ++i) x[i] = 0.f;
+                            } else if (L.zero_sigma) {
+#pragma unroll
+                                for (int i = 0; i < 8; ++i) x[i] = (j0 + i == jj) ? L.q : 0.f;
+                            } else {
+                                float e0 = erff(((float)j0 - pt) * L.ist);
+#pragma unroll
+                                for (int i = 0; i < 8; ++i) {
+                                    const float e1 = erff(((float)(j0 + i + 1) - pt) * L.ist);
+                                    x[i] = (j0 + i >= L.jlo && j0 + i <= L.jhi) ? 0.5f * L.q * (e1 - e0) : 0.f;
+                                    e0 = e1;
+                                }
+                            }
+                            split_store8(Bhi + col + 128 * g, Blo + col + 128 * g, x);
+                        }
+                    }
+                }
+                // operands written by the generic proxy, read by the tensor core (async proxy)
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncthreads();
+                if (tid == 0) {
+                    rtc::tc_fence_after();
+                    for (int k16 = 0; k16 < nk16; ++k16) {
+                        const uint32_t ao = 2 * k16 * 128 * MG, bo = 2 * k16 * 128 * NG;
+                        const uint64_t ah = rtc::smem_desc(sbase + ao, 128 * MG, 128, 0);
+                        const uint64_t al = rtc::smem_desc(sbase + CT_A_HALF + ao, 128 * MG, 128, 0);
+                        const uint64_t bh = rtc::smem_desc(sbase + 2 * CT_A_HALF + bo, 128 * NG, 128, 0);
+                        const uint64_t bl = rtc::smem_desc(sbase + 2 * CT_A_HALF + CT_B_HALF + bo, 128 * NG, 128, 0);
+                        rtc::tc_mma_f16(tmem, ah, bh, idesc, (any_mma || k16) ? 1u : 0u);
+                        rtc::tc_mma_f16(tmem, ah, bl, idesc, 1u);
+                        rtc::tc_mma_f16(tmem, al, bh, idesc, 1u);
+                    }
+                    rtc::tc_commit(bar);
+                }
+                any_mma = true;
+                rtc::mbar_wait(bar, mma_phase);                        // the MMAs have read the operands (and landed)
+                mma_phase ^= 1u;
+            }
+        }
+    }
+    // ------------------------------------------------------------------ accumulator -> operand image of the response
+    if (!any_mma) {                                                   // CTA-uniform: no segment reaches this window
+        if (tid == 0) *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(1, 0, 0, 0);
+    } else {
+        rtc::tc_fence_after();
+        uint32_t v[2][32];
+        const uint32_t tlane = tmem + ((uint32_t)(32 * warp) << 16);  // thread = cell row m = tid
+        rtc::tmem_ld32(tlane, v[0]);
+        rtc::tmem_ld32(tlane + 32, v[1]);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        float mx = 0.f;
+        int lo = INT_MAX, hi = -1, nz = 0;
+#pragma unroll
+        for (int j = 0; j < 64; ++j) {
+            const float x = __uint_as_float(v[j >> 5][j & 31]);
+            mx = fmaxf(mx, fabsf(x));
+            if (x != 0.f) { lo = min(lo, j); hi = j; ++nz; }
+        }
+        for (int d = 16; d; d >>= 1) {
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+            lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, d));
+            hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, d));
+            nz += __shfl_xor_sync(0xffffffffu, nz, d);
+        }
+        if (lane == 0) { red[warp] = mx; redi[3 * warp] = lo; redi[3 * warp + 1] = hi; redi[3 * warp + 2] = nz; }
+        __syncthreads();
+#pragma unroll
+        for (int w = 0; w < CT_THREADS / 32; ++w) {
+            mx = w ? fmaxf(mx, red[w]) : red[0];
+            lo = w ? min(lo, redi[3 * w]) : redi[0];
+            hi = w ? max(hi, redi[3 * w + 1]) : redi[1];
+            nz = w ? nz + redi[3 * w + 2] : redi[2];
+        }
+        int e = 0;
+        if (mx >= 32768.f) e = min(((__float_as_int(mx) >> 23) & 0xff) - 127 - 14, 100);   // mx * 2^-e in [2^14, 2^15)
+        if (!(mx < 3.0e38f)) e = 0;                                   // inf / nan charge: leave it visible
+        const float sc = __int_as_float((127 - e) << 23);
+        if (tid == 0) {
+            if (nz == 0) *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(1, 0, 0, 0);
+            else {
+                *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(lo / RESP_NO, (hi + p.K - 1) / RESP_NO, e, 0);
+                // multiply-adds the method needs here: non-zero cells x in-plane targets x K
+                const int vx = min(td.px + p.H, tp.nx - 1) - max(td.px - p.H, 0) + 1;
+                const int vy = min(td.py + p.H, tp.ny - 1) - max(td.py - p.H, 0) + 1;
+                if (vx > 0 && vy > 0) atomicAdd(a.fma_counter, (unsigned long long)nz * (unsigned long long)(vx * vy * p.K));
+            }
+        }
+        if (tid < NB2) {
+            const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;
+            unsigned char *row = (unsigned char *)a.charge +
+                                 (((size_t)tb * NB2 + tid) * 2 * rtc::TB + r) * (rtc::JC * 2);   // hi row of (bin, tile)
+#pragma unroll
+            for (int ch = 0; ch < 8; ++ch) {
+                float x[8];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) x[i] = __uint_as_float(v[(8 * ch + i) >> 5][(8 * ch + i) & 31]) * sc;
+                const int o = ((ch ^ (r & 7)) << 4);                  // 16-byte chunk permutation of the 128-byte swizzle
+                split_store8(row + o, row + rtc::TB * rtc::JC * 2 + o, x);
+            }
+        }
+    }
+    rtc::tc_fence_before();
+    __syncthreads();
+    if (warp == 0) {
+        rtc::tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(64u) : "memory");
+    }
+}

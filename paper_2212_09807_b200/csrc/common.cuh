@@ -96,6 +96,7 @@ struct lartpc_sim {
     lartpc_drifted_t drifted_copy;
     lartpc_pixmap_t pixmap_copy;
     int sm_count = 148;
+    bool splat_tc = true;                // tensor-core mode: charge lattice on the tensor cores too (env LARTPC_SPLAT=ffma turns it off)
     // per-stage profiling of run_spill (lartpc_set_profiling)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;

@@ -395,6 +395,8 @@ __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs 
     }
 }
 
+#include "charge_tc.cuh"
+
 size_t splat_smem_bytes(const DevParams &p)
 {
     size_t floats = (size_t)p.NB2 * p.CJ + (size_t)SB * (2 * XS + p.CJ);
@@ -655,6 +657,20 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     a.jt0 = pm->jt0; a.jt1 = pm->jt1; a.n_samples = pm->n_samples;
     a.charge = out->charge;  a.tile_range = out->tile_range;
     a.fma_counter = sim->d_fma;
+    if (p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5)) {
+        // tensor-core splat (charge_tc.cuh); other bin counts use the FFMA2 splat below, which writes the same image
+        static bool configured_tc = false;
+        if (!configured_tc) {
+            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
+            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
+            configured_tc = true;
+        }
+        ++g_lartpc_launches;
+        if (p.nb == 10) charge_lattice_tc_kernel<10><<<(unsigned)sim->n_tiles, CT_THREADS, CT_SMEM, st>>>(a);
+        else charge_lattice_tc_kernel<5><<<(unsigned)sim->n_tiles, CT_THREADS, CT_SMEM, st>>>(a);
+        LARTPC_CUDA_TRY(cudaGetLastError());
+        return LARTPC_OK;
+    }
     size_t smem = splat_smem_bytes(p);
     static size_t configured = 0;
     if (smem > configured) {
