@@ -23,22 +23,29 @@ active_table_kernel(int64_t n_pix, const int32_t *__restrict__ act_first, const 
 
 struct LenF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
 
-__global__ void __launch_bounds__(256)
+constexpr int SUM_THREADS = 128;
+
+// CTA = active pixel.  Its waveform is accumulated in shared memory, tile by tile: for every target index d of the
+// W x W window (ascending) and every charge window of that charged pixel (ascending) the partial row of the tile is
+// streamed once, coalesced, over the ticks it can be non-zero on.  A thread always owns the same ticks (i = tid mod
+// 128), so there is no race, no barrier between tiles, and the order of the float32 additions is fixed.
+__global__ void __launch_bounds__(SUM_THREADS)
 sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__restrict__ pixel_id,
                  const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,
                  const int64_t *__restrict__ offset, const unsigned long long *__restrict__ pix_mask,
                  const int32_t *__restrict__ pix_tile0, const int32_t *__restrict__ pix_jmin,
                  const float *__restrict__ partial, const int32_t *__restrict__ tile_range, float *samples)
 {
+    extern __shared__ float acc[];                                    // [length of this pixel's waveform]
     __shared__ unsigned long long s_mask[128][MASK_WORDS];
     __shared__ int s_tile0[128], s_js[128];
-    const int slot = blockIdx.x;
+    const int slot = blockIdx.x, tid = threadIdx.x;
     const int gp = pixel_id[slot];
     int tpc = 0;
     while (tpc + 1 < p.n_tpcs && tpcs[tpc + 1].first_pixel_id <= gp) ++tpc;
     const DevTpc &t = tpcs[tpc];
     const int rel = gp - t.first_pixel_id, iy = rel / t.nx, ix = rel - iy * t.nx;
-    for (int d = threadIdx.x; d < p.WW; d += blockDim.x) {
+    for (int d = tid; d < p.WW; d += SUM_THREADS) {
         const int dyi = d / p.W, dxi = d - dyi * p.W;
         const int cp = t.cp_base + (iy + dyi) * t.gw + (ix + dxi);   // charged pixel px = ix - H + dxi
 #pragma unroll
@@ -46,31 +53,32 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
         s_tile0[d] = pix_tile0[cp];
         s_js[d] = pix_jmin[cp] & ~1;                                 // window origin of that charged pixel
     }
-    __syncthreads();
     const int first = first_tick[slot], len = length[slot];
-    const int64_t off = offset[slot];
-    const int span = p.Jc + p.K - 2;                                  // a tile reaches readout ticks [j_start, j_start + span]
-    for (int i = threadIdx.x; i < len; i += blockDim.x) {
-        const int n = first + i;
-        float sum = 0.f;
-        for (int d = 0; d < p.WW; ++d) {
-            const int r = n - s_js[d];
-            if (r < 0 || !(s_mask[d][0] | s_mask[d][MASK_WORDS - 1])) continue;
-            const int w_hi = min(r / p.Jc, MAX_WINDOWS - 1);
-            const int w_lo = r > span ? (r - span + p.Jc - 1) / p.Jc : 0;
-            for (int w = w_lo; w <= w_hi; ++w) {
-                const unsigned long long m = s_mask[d][w >> 6];
-                if (!((m >> (w & 63)) & 1ull)) continue;
-                int below = __popcll(m & ((1ull << (w & 63)) - 1ull));
-                if (w >= 64) below += __popcll(s_mask[d][0]);
-                const int tix = s_tile0[d] + below;
-                const int nrel = r - w * p.Jc, blk = nrel / RESP_NO;
-                if (blk >= tile_range[TILE_META * tix] && blk <= tile_range[TILE_META * tix + 1])
-                    sum += partial[((size_t)tix * p.WW + d) * p.tile_ticks + nrel];
+    for (int i = tid; i < len; i += SUM_THREADS) acc[i] = 0.f;
+    __syncthreads();
+    const int last = first + len - 1;
+    for (int d = 0; d < p.WW; ++d) {
+        int tix = s_tile0[d];
+        const int js = s_js[d];
+#pragma unroll
+        for (int wd = 0; wd < MASK_WORDS; ++wd)
+            for (unsigned long long m = s_mask[d][wd]; m; m &= m - 1, ++tix) {
+                const int w = 64 * wd + __ffsll((long long)m) - 1;
+                const int2 rg = *(const int2 *)(tile_range + TILE_META * tix);      // first / last output block
+                if (rg.x > rg.y) continue;
+                const int j_start = js + w * p.Jc;
+                const int n_a = max(first, j_start + rg.x * RESP_NO);
+                const int n_b = min(last, j_start + min(rg.y * RESP_NO + RESP_NO - 1, p.tile_ticks - 1));
+                const float *row = partial + ((size_t)tix * p.WW + d) * p.tile_ticks - j_start;
+                // first tick >= n_a owned by this thread
+                int i = n_a - first;
+                i += (tid - i) & (SUM_THREADS - 1);
+                for (; first + i <= n_b; i += SUM_THREADS) acc[i] += __ldcs(row + first + i);
             }
-        }
-        samples[off + i] = sum;
     }
+    __syncthreads();
+    const int64_t off = offset[slot];
+    for (int i = tid; i < len; i += SUM_THREADS) samples[off + i] = acc[i];
 }
 
 int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out, cudaStream_t st)
@@ -92,7 +100,13 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
     LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_active, LenF{out->length}, out->offset, true, (long long *)nullptr,
                                           sim->scan_tmp, st));
     ++g_lartpc_launches;
-    sum_pixel_kernel<<<(unsigned)sim->n_active, 256, 0, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
+    const size_t smem = sizeof(float) * (size_t)p.n_ticks;             // a waveform is at most the readout window
+    static size_t configured = 0;
+    if (smem > 40 * 1024 && smem > configured) {
+        LARTPC_CUDA_TRY(cudaFuncSetAttribute(sum_pixel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = smem;
+    }
+    sum_pixel_kernel<<<(unsigned)sim->n_active, SUM_THREADS, smem, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
                                                              out->length, out->offset, sim->pix_mask, sim->pix_tile0,
                                                              sim->pix_jmin, sig->partial, sig->tile_range,
                                                              out->samples);
