@@ -34,6 +34,26 @@ __device__ __forceinline__ void split_store8(unsigned char *hi, unsigned char *l
     *(uint4 *)lo = *(const uint4 *)l;
 }
 
+// erf(x) = sign(x) (1 - 2^(-t P(t))), t = min(|x|, 4.2): one branch-free formula, P a degree-7 fit of -log2(erfc(t)) / t
+// weighted by t erfc(t) (fit in _work, checked against scipy: |error| <= 1.1e-7 ABSOLUTE over the whole line, float32
+// evaluation included).  The weights are differences of erf at neighbouring edges, so absolute accuracy is what counts;
+// erff() spends twice the instructions on relative accuracy near 0 that the difference throws away.
+__device__ __forceinline__ float erf_fast(float x)
+{
+    const float t = fminf(fabsf(x), 4.2f);
+    float pp = 4.535783592e-05f;
+    pp = fmaf(pp, t, -4.455014132e-04f);
+    pp = fmaf(pp, t, 1.489421586e-03f);
+    pp = fmaf(pp, t, 7.746618357e-04f);
+    pp = fmaf(pp, t, -2.825370803e-02f);
+    pp = fmaf(pp, t, 1.484816223e-01f);
+    pp = fmaf(pp, t, 9.184163809e-01f);
+    pp = fmaf(pp, t, 1.627908587e+00f);
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(-pp * t));
+    return copysignf(1.0f - e, x);
+}
+
 template <int NB>
 __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const SplatArgs a)
 {
@@ -50,7 +70,8 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
     volatile uint32_t *tptr = (volatile uint32_t *)(ctl + 8);
     float *red = (float *)(ctl + 16);                                // [4] max, then ints
     int *redi = (int *)(ctl + 32);                                   // [4][3] lo, hi, nz
-    SegLocal *segs = (SegLocal *)(ctl + 128);
+    int *pre = (int *)(ctl + 96);                                    // [SEGCAP + 1] running sample counts
+    SegLocal *segs = (SegLocal *)(ctl + 256);
 
     const int tile = blockIdx.x;
     const TileDesc td = a.tile_desc[tile];
@@ -84,6 +105,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
     for (int l0 = 0; l0 < lcount; l0 += SEGCAP) {
         __syncthreads();
         const int nseg = min(SEGCAP, lcount - l0);
+        int n_eff = 0;
         if (tid < nseg) {
             const int s = a.pair_seg[lstart + l0 + tid];
             SegLocal L;
@@ -104,110 +126,125 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             L.ist = L.zero_sigma ? 0.f : (float)(p.dt * 0.70710678118654752440 / (double)st);
             L.q = a.q_anode[s] / (float)L.N;                          // eq. (3.8): Q_a / N per sample point
             segs[tid] = L;
+            if (!(L.jlo > L.jhi || L.alo > L.ahi || L.blo > L.bhi)) n_eff = L.N;   // box misses this tile: no samples
+        }
+        // The K dimension of the contraction is "sample", whichever segment it belongs to: the samples of the staged
+        // segments are laid end to end (pre[] = running sum of their counts, in list order) and cut into batches of 64.
+        if (warp == 0) {
+            int inc = n_eff;
+            for (int d = 1; d < 32; d <<= 1) {
+                const int o = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += o;
+            }
+            pre[lane + 1] = inc;
+            if (lane == 0) pre[0] = 0;
         }
         __syncthreads();
-        for (int li = 0; li < nseg; ++li) {
-            const SegLocal L = segs[li];
-            if (L.jlo > L.jhi || L.alo > L.ahi || L.blo > L.bhi) continue;          // CTA-uniform
-            const float invN = 1.0f / (float)L.N;
-            for (int mu0 = 0; mu0 < L.N; mu0 += CT_KB) {
-                const int nsb = min(CT_KB, L.N - mu0), nk16 = (nsb + 15) >> 4;
-                if (s_in < 16 * nk16) {
-                    const bool real = s_in < nsb;
-                    const int mu = mu0 + s_in;
-                    const float f = ((float)mu + 0.5f) * invN;
-                    // sigma = 0: the bin / tick is an integer decision taken in float64 in the oracle's order
-                    int ia = -1, ib = -1, jj = -1;
-                    if (L.zero_sigma && real) {
-                        const int s = L.seg;
-                        const double fd = xdiv(xadd((double)mu, 0.5), (double)L.N);
-                        if (role_a) {
-                            const double us = a.u_s[s], ue = a.u_e[s], vs = a.v_s[s], ve = a.v_e[s];
-                            const long long xa = (long long)floor(xdiv(xadd(us, xmul(xsub(ue, us), fd)), p.bin)) - A_t;
-                            const long long xb = (long long)floor(xdiv(xadd(vs, xmul(xsub(ve, vs), fd)), p.bin)) - B_t;
-                            if (xa >= 0 && xa < NB && xb >= 0 && xb < NB) { ia = (int)xa; ib = (int)xb; }
-                        } else {
-                            const double Ts = a.T_s[s], Te = a.T_e[s];
-                            long long j = (long long)floor(xdiv(xsub(xadd(Ts, xmul(xsub(Te, Ts), fd)), p.t_origin), p.dt));
-                            if (j >= 0 && j <= p.j_max && j - J_t >= 0 && j - J_t < p.Jc) jj = (int)(j - J_t);
+        const int total = pre[nseg];
+        for (int s0 = 0; s0 < total; s0 += CT_KB) {
+            const int nsb = min(CT_KB, total - s0), nk16 = (nsb + 15) >> 4;
+            if (s_in < 16 * nk16) {
+                const bool real = s_in < nsb;
+                const int slot = s0 + min(s_in, nsb - 1);
+                int li = 0;                                           // last li with pre[li] <= slot (SEGCAP = 32)
+#pragma unroll
+                for (int step = 16; step; step >>= 1)
+                    if (li + step < nseg && pre[li + step] <= slot) li += step;
+                const SegLocal L = segs[li];
+                const int mu = slot - pre[li];
+                const float f = ((float)mu + 0.5f) * (1.0f / (float)L.N);
+                // sigma = 0: the bin / tick is an integer decision taken in float64 in the oracle's order
+                int ia = -1, ib = -1, jj = -1;
+                if (L.zero_sigma && real) {
+                    const int s = L.seg;
+                    const double fd = xdiv(xadd((double)mu, 0.5), (double)L.N);
+                    if (role_a) {
+                        const double us = a.u_s[s], ue = a.u_e[s], vs = a.v_s[s], ve = a.v_e[s];
+                        const long long xa = (long long)floor(xdiv(xadd(us, xmul(xsub(ue, us), fd)), p.bin)) - A_t;
+                        const long long xb = (long long)floor(xdiv(xadd(vs, xmul(xsub(ve, vs), fd)), p.bin)) - B_t;
+                        if (xa >= 0 && xa < NB && xb >= 0 && xb < NB) { ia = (int)xa; ib = (int)xb; }
+                    } else {
+                        const double Ts = a.T_s[s], Te = a.T_e[s];
+                        long long j = (long long)floor(xdiv(xsub(xadd(Ts, xmul(xsub(Te, Ts), fd)), p.t_origin), p.dt));
+                        if (j >= 0 && j <= p.j_max && j - J_t >= 0 && j - J_t < p.Jc) jj = (int)(j - J_t);
+                    }
+                }
+                if (role_a) {
+                    float wx[NB], wy[NB];
+                    if (!real) {
+#pragma unroll
+                        for (int i = 0; i < NB; ++i) wx[i] = wy[i] = 0.f;
+                    } else if (L.zero_sigma) {
+#pragma unroll
+                        for (int i = 0; i < NB; ++i) { wx[i] = (i == ia) ? 1.f : 0.f; wy[i] = (i == ib) ? 1.f : 0.f; }
+                    } else {
+                        const float px = fmaf(L.ae - L.as, f, L.as), py = fmaf(L.be - L.bs, f, L.bs);
+                        float ex = erf_fast((0.f - px) * L.isT), ey = erf_fast((0.f - py) * L.isT);
+#pragma unroll
+                        for (int i = 0; i < NB; ++i) {
+                            const float ex1 = erf_fast(((float)(i + 1) - px) * L.isT), ey1 = erf_fast(((float)(i + 1) - py) * L.isT);
+                            wx[i] = (i >= L.alo && i <= L.ahi) ? 0.5f * (ex1 - ex) : 0.f;
+                            wy[i] = (i >= L.blo && i <= L.bhi) ? 0.5f * (ey1 - ey) : 0.f;
+                            ex = ex1;  ey = ey1;
                         }
                     }
-                    if (role_a) {
-                        float wx[NB], wy[NB];
-                        if (!real) {
+                    const uint32_t col = ct_col_offset(s_in, MG);
 #pragma unroll
-                            for (int i = 0; i < NB; ++i) wx[i] = wy[i] = 0.f;
+                    for (int g = 0; g < (NB2 + 7) / 8; ++g) {
+                        float x[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            const int m = 8 * g + i;
+                            x[i] = m < NB2 ? wx[m % NB] * wy[m / NB] : 0.f;
+                        }
+                        split_store8(Ahi + col + 128 * g, Alo + col + 128 * g, x);
+                    }
+                } else {
+                    const uint32_t col = ct_col_offset(s_in, NG);
+                    const float pt = fmaf(L.te - L.ts, f, L.ts);
+                    const float hq = 0.5f * L.q;
+                    for (int g = 0; g < NG; ++g) {
+                        float x[8];
+                        const int j0 = 8 * g;
+                        if (!real || j0 + 7 < L.jlo || j0 > L.jhi) {
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) x[i] = 0.f;
                         } else if (L.zero_sigma) {
 #pragma unroll
-                            for (int i = 0; i < NB; ++i) { wx[i] = (i == ia) ? 1.f : 0.f; wy[i] = (i == ib) ? 1.f : 0.f; }
+                            for (int i = 0; i < 8; ++i) x[i] = (j0 + i == jj) ? L.q : 0.f;
                         } else {
-                            const float px = fmaf(L.ae - L.as, f, L.as), py = fmaf(L.be - L.bs, f, L.bs);
-                            float ex = erff((0.f - px) * L.isT), ey = erff((0.f - py) * L.isT);
-#pragma unroll
-                            for (int i = 0; i < NB; ++i) {
-                                const float ex1 = erff(((float)(i + 1) - px) * L.isT), ey1 = erff(((float)(i + 1) - py) * L.isT);
-                                wx[i] = (i >= L.alo && i <= L.ahi) ? 0.5f * (ex1 - ex) : 0.f;
-                                wy[i] = (i >= L.blo && i <= L.bhi) ? 0.5f * (ey1 - ey) : 0.f;
-                                ex = ex1;  ey = ey1;
-                            }
-                        }
-                        const uint32_t col = ct_col_offset(s_in, MG);
-#pragma unroll
-                        for (int g = 0; g < (NB2 + 7) / 8; ++g) {
-                            float x[8];
+                            float e0 = erf_fast(((float)j0 - pt) * L.ist);
 #pragma unroll
                             for (int i = 0; i < 8; ++i) {
-                                const int m = 8 * g + i;
-                                x[i] = m < NB2 ? wx[m % NB] * wy[m / NB] : 0.f;
+                                const float e1 = erf_fast(((float)(j0 + i + 1) - pt) * L.ist);
+                                x[i] = (j0 + i >= L.jlo && j0 + i <= L.jhi) ? hq * (e1 - e0) : 0.f;
+                                e0 = e1;
                             }
-                            split_store8(Ahi + col + 128 * g, Alo + col + 128 * g, x);
                         }
-                    } else {
-                        const uint32_t col = ct_col_offset(s_in, NG);
-                        const float pt = fmaf(L.te - L.ts, f, L.ts);
-                        for (int g = 0; g < NG; ++g) {
-                            float x[8];
-                            const int j0 = 8 * g;
-                            if (!real || j0 + 7 < L.jlo || j0 > L.jhi) {
-#pragma unroll
-                                for (int i = 0; i < 8; ++i) x[i] = 0.f;
-                            } else if (L.zero_sigma) {
-#pragma unroll
-                                for (int i = 0; i < 8; ++i) x[i] = (j0 + i == jj) ? L.q : 0.f;
-                            } else {
-                                float e0 = erff(((float)j0 - pt) * L.ist);
-#pragma unroll
-                                for (int i = 0; i < 8; ++i) {
-                                    const float e1 = erff(((float)(j0 + i + 1) - pt) * L.ist);
-                                    x[i] = (j0 + i >= L.jlo && j0 + i <= L.jhi) ? 0.5f * L.q * (e1 - e0) : 0.f;
-                                    e0 = e1;
-                                }
-                            }
-                            split_store8(Bhi + col + 128 * g, Blo + col + 128 * g, x);
-                        }
+                        split_store8(Bhi + col + 128 * g, Blo + col + 128 * g, x);
                     }
                 }
-                // operands written by the generic proxy, read by the tensor core (async proxy)
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                __syncthreads();
-                if (tid == 0) {
-                    rtc::tc_fence_after();
-                    for (int k16 = 0; k16 < nk16; ++k16) {
-                        const uint32_t ao = 2 * k16 * 128 * MG, bo = 2 * k16 * 128 * NG;
-                        const uint64_t ah = rtc::smem_desc(sbase + ao, 128 * MG, 128, 0);
-                        const uint64_t al = rtc::smem_desc(sbase + CT_A_HALF + ao, 128 * MG, 128, 0);
-                        const uint64_t bh = rtc::smem_desc(sbase + 2 * CT_A_HALF + bo, 128 * NG, 128, 0);
-                        const uint64_t bl = rtc::smem_desc(sbase + 2 * CT_A_HALF + CT_B_HALF + bo, 128 * NG, 128, 0);
-                        rtc::tc_mma_f16(tmem, ah, bh, idesc, (any_mma || k16) ? 1u : 0u);
-                        rtc::tc_mma_f16(tmem, ah, bl, idesc, 1u);
-                        rtc::tc_mma_f16(tmem, al, bh, idesc, 1u);
-                    }
-                    rtc::tc_commit(bar);
-                }
-                any_mma = true;
-                rtc::mbar_wait(bar, mma_phase);                        // the MMAs have read the operands (and landed)
-                mma_phase ^= 1u;
             }
+            // operands written by the generic proxy, read by the tensor core (async proxy)
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncthreads();
+            if (tid == 0) {
+                rtc::tc_fence_after();
+                for (int k16 = 0; k16 < nk16; ++k16) {
+                    const uint32_t ao = 2 * k16 * 128 * MG, bo = 2 * k16 * 128 * NG;
+                    const uint64_t ah = rtc::smem_desc(sbase + ao, 128 * MG, 128, 0);
+                    const uint64_t al = rtc::smem_desc(sbase + CT_A_HALF + ao, 128 * MG, 128, 0);
+                    const uint64_t bh = rtc::smem_desc(sbase + 2 * CT_A_HALF + bo, 128 * NG, 128, 0);
+                    const uint64_t bl = rtc::smem_desc(sbase + 2 * CT_A_HALF + CT_B_HALF + bo, 128 * NG, 128, 0);
+                    rtc::tc_mma_f16(tmem, ah, bh, idesc, (any_mma || k16) ? 1u : 0u);
+                    rtc::tc_mma_f16(tmem, ah, bl, idesc, 1u);
+                    rtc::tc_mma_f16(tmem, al, bh, idesc, 1u);
+                }
+                rtc::tc_commit(bar);
+            }
+            any_mma = true;
+            rtc::mbar_wait(bar, mma_phase);                        // the MMAs have read the operands (and landed)
+            mma_phase ^= 1u;
         }
     }
     // ------------------------------------------------------------------ accumulator -> operand image of the response
