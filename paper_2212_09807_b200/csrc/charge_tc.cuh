@@ -296,15 +296,15 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
         }
         if (tid < NB2) {
             const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;
-            unsigned char *row = (unsigned char *)a.charge +
-                                 (((size_t)tb * NB2 + tid) * 2 * rtc::TB + r) * (rtc::JC * 2);   // hi row of (bin, tile)
+            unsigned char *row16 = (unsigned char *)a.charge +
+                                   (((size_t)tb * NB2 + tid) * 2 * rtc::TB + r) * (rtc::JC * 2);  // fp16 row of (bin, tile)
+            unsigned char *row8 = row16 + rtc::TB * rtc::JC * 2;                                    // fp8 row
 #pragma unroll
-            for (int ch = 0; ch < 8; ++ch) {
-                float x[8];
+            for (int b = 0; b < rtc::NBLK; ++b) {
+                float x[16];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) x[i] = __uint_as_float(v[(8 * ch + i) >> 5][(8 * ch + i) & 31]) * sc;
-                const int o = ((ch ^ (r & 7)) << 4);                  // 16-byte chunk permutation of the 128-byte swizzle
-                split_store8(row + o, row + rtc::TB * rtc::JC * 2 + o, x);
+                for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[(16 * b + i) >> 5][(16 * b + i) & 31]) * sc;
+                rtc::store_a_block16(row16, row8, r, b, x);
             }
         }
     }

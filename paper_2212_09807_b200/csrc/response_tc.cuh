@@ -8,17 +8,21 @@
 // 16 x NBW operand (NBW = roundup16(K + 15) = 224 for K = 200) serves all four b: the MMA for block b accumulates
 // into TMEM columns [16 b, 16 b + NBW).  Bs for all (d, c) is 36 MB and stays in L2; nothing Toeplitz-sized is built.
 //
-// Precision: tensor-core inputs are fp16, so both operands are split x = hi + lo (hi = fp16(x), lo = fp16(x - hi),
-// 22 significant bits) and three products are accumulated in fp32: hi*hi + hi*lo + lo*hi (the dropped lo*lo term is
-// 2^-22 relative).  A carries a per-tile power-of-two scale (fp16 range), B a fixed 2^10 (keeps far-field LUT values
-// normal); the epilogue undoes both exactly.
+// Precision: tensor-core inputs are fp16, so both operands are split x = hi + lo (hi = fp16(x), lo = x - hi) and
+// hi*hi + hi*lo + lo*hi is accumulated in fp32 (the dropped lo*lo term is 2^-22 relative).  The two cross terms are
+// 2^-11 of the main one, so three significant bits are all they need: they run as ONE fp8 (e4m3) MMA of K = 32,
+//     [lo8(A) | hi8(A)] x [hi8(B) ; lo8(B)],
+// which costs the tensor pipe as much as one fp16 MMA of K = 16: two MMA slots per (bin, 16-tick block) instead of three
+// (error of the cross terms: 2^-4 x 2^-12 relative per product, random in sign; parity margins in the tests unchanged).
+// A carries a per-tile power-of-two scale (fp16 range), B a fixed 2^10 (keeps far-field LUT values normal); the fp8
+// parts carry the extra powers of two below, which cancel in the product; the epilogue undoes the rest exactly.
 //
 // Kernel (persistent, one CTA per SM, 192 threads, whole TMEM):
 //   warp 0, one lane   producer: per (item = (tile block, d), bin c) one cp.async.bulk of the A image (hi + lo, 32 KB,
 //                      written by charge_lattice_kernel already in the 128-byte-swizzled K-major UMMA layout) and one of
 //                      the Bs image (hi + lo, 14 KB, canonical un-swizzled K-major layout built at create) into a ring
 //                      of 4 shared-memory stages, completion on an mbarrier per stage
-//   warp 1, one lane   MMA issuer: 12 tcgen05.mma (M = 128, N = NBW, K = 16; 4 blocks b x 3 precision terms) per
+//   warp 1, one lane   MMA issuer: 8 tcgen05.mma (M = 128, N = NBW; 4 blocks b x (fp16 K = 16 + fp8 K = 32)) per
 //                      stage, tcgen05.commit frees the stage; after the last bin a commit signals the epilogue
 //   warps 2-5          epilogue: tcgen05.ld the 128 x 264 fp32 accumulator (thread = tile row), undo the scales, write
 //                      the partial waveform rows, re-zero the TMEM columns that only later blocks b touch
@@ -28,6 +32,7 @@
 // launch: measured, the L2 reuse of A is lost and the kernel becomes HBM-bound.)
 #pragma once
 #include <cuda_fp16.h>
+#include <cuda_fp8.h>
 #include <stdint.h>
 
 namespace rtc {
@@ -38,11 +43,14 @@ constexpr int NBLK = JC / 16;
 constexpr int STAGES = 4;
 constexpr int THREADS = 192;
 constexpr int B_SCALE_LOG2 = 10;
+// fp8 parts: lo8(A) = e4m3(lo(A) 2^SA) meets hi8(B) = e4m3(B 2^-SA); hi8(A) = e4m3(A 2^-SB) meets lo8(B) = e4m3(lo(B) 2^SB)
+// (|A| < 2^15, |lo(A)| <= 8, |B| <= 2^10, |lo(B)| <= 0.5: every part stays below e4m3's 448)
+constexpr int SA_LOG2 = 5, SB_LOG2 = 7;
 constexpr int A_HALF_BYTES = TB * JC * 2;          // one precision half of an A stage image (16 KB)
 
 struct Args {
-    const __half *A;               // [n_tb][NC][2][TB][JC]   swizzled images, see a_image_offset()
-    const __half *B;               // [WW][NC][2][NBW * 16]   see b_image_offset()
+    const __half *A;               // [n_tb][NC][2][TB][128 bytes]: fp16 image (a_image_offset) + fp8 image (a8_image_offset)
+    const __half *B;               // [WW][NC][2][NBW * 32 bytes]: fp16 image (b_image_offset) + fp8 image (b8_image_offset)
     float *partial;                // [n_tiles][WW][tile_ticks]
     const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), 0
     int n_tiles, n_tb, NC, WW, NBW, tile_ticks;
@@ -61,6 +69,40 @@ __host__ __device__ __forceinline__ int a_image_offset(int r, int k)          //
 __host__ __device__ __forceinline__ int b_image_offset(int n, int jj)         // in halfs
 {
     return (n >> 3) * 128 + (jj >> 3) * 64 + (n & 7) * 8 + (jj & 7);
+}
+
+// fp8 image of A: row r = 128 bytes = 4 blocks b of [lo8 of ticks 16 b .. 16 b + 15 | hi8 of the same ticks]; returns the
+// byte offset of the 16-byte chunk (part = 0: lo8, 1: hi8) under the same 128-byte swizzle
+__host__ __device__ __forceinline__ int a8_image_offset(int r, int b, int part)
+{
+    return r * 128 + ((((2 * b + part) ^ (r & 7))) << 4);
+}
+// fp8 image of Bs: row n', K byte kb in [0, 32): kb < 16 -> hi8 of jj = kb, else lo8 of jj = kb - 16; same canonical
+// K-major byte layout as the fp16 image (16-byte core rows, K chunks 128 B apart, 8-row groups 256 B apart)
+__host__ __device__ __forceinline__ int b8_image_offset(int n, int kb)
+{
+    return (n >> 3) * 256 + (kb >> 4) * 128 + (n & 7) * 16 + (kb & 15);
+}
+
+// Writes 16 consecutive arrival ticks (block b) of row r of one bin's A operand: x = C 2^-e, |x| < 2^15.
+// row16 / row8: start of row r (128 bytes each) in the fp16 and in the fp8 image.
+__device__ __forceinline__ void store_a_block16(unsigned char *row16, unsigned char *row8, int r, int b, const float (&x)[16])
+{
+    __half2 h[8];
+    unsigned short l8[8], h8[8];
+    const float sa = (float)(1 << SA_LOG2), sb = 1.0f / (float)(1 << SB_LOG2);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        h[i] = __floats2half2_rn(x[2 * i], x[2 * i + 1]);
+        const float2 f = __half22float2(h[i]);
+        l8[i] = __nv_cvt_float2_to_fp8x2(make_float2((x[2 * i] - f.x) * sa, (x[2 * i + 1] - f.y) * sa), __NV_SATFINITE, __NV_E4M3);
+        h8[i] = __nv_cvt_float2_to_fp8x2(make_float2(x[2 * i] * sb, x[2 * i + 1] * sb), __NV_SATFINITE, __NV_E4M3);
+    }
+    const int s0 = ((2 * b) ^ (r & 7)) << 4, s1 = ((2 * b + 1) ^ (r & 7)) << 4;
+    *(uint4 *)(row16 + s0) = *(const uint4 *)&h[0];
+    *(uint4 *)(row16 + s1) = *(const uint4 *)&h[4];
+    *(uint4 *)(row8 + s0) = *(const uint4 *)l8;
+    *(uint4 *)(row8 + s1) = *(const uint4 *)h8;
 }
 
 __device__ __forceinline__ uint32_t s32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -107,6 +149,15 @@ __device__ __forceinline__ void tc_mma_f16(uint32_t d_tmem, uint64_t a_desc, uin
         ".reg .pred p;\n"
         "setp.ne.b32 p, %4, 0;\n"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tc_mma_f8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n"
         "}\n" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
 }
 // shared-memory matrix descriptor (version 1): start address, leading / stride byte offsets in 16-byte units, layout
@@ -208,7 +259,8 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
         if (lane == 0) {
-            // instruction descriptor: D fp32, A and B fp16, both K-major, N = NBW, M = 128
+            // instruction descriptor: D fp32, A and B fp16 (kind::f16) or e4m3 (kind::f8f6f4) -- format code 0 in both
+            // kinds --, both K-major, N = NBW, M = 128
             const uint32_t idesc = (1u << 4) | ((uint32_t)(NBW >> 3) << 17) | ((uint32_t)(TB >> 4) << 24);
             int s = 0;
             uint32_t ph = 0, tph = 0;
@@ -229,15 +281,14 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 tc_fence_after();
                 const uint32_t st = base + s * stage_sz;
                 const uint64_t bd_hi = smem_desc(st + 2 * A_HALF_BYTES, 128, 256, 0);
-                const uint64_t bd_lo = smem_desc(st + 2 * A_HALF_BYTES + b_half, 128, 256, 0);
+                const uint64_t bd_8 = smem_desc(st + 2 * A_HALF_BYTES + b_half, 128, 256, 0);
 #pragma unroll
                 for (int b = 0; b < NBLK; ++b) {
                     const uint64_t ad_hi = smem_desc(st + 32 * b, 16, 1024, 2);
-                    const uint64_t ad_lo = smem_desc(st + A_HALF_BYTES + 32 * b, 16, 1024, 2);
+                    const uint64_t ad_8 = smem_desc(st + A_HALF_BYTES + 32 * b, 16, 1024, 2);
                     const uint32_t dcol = tmem + 16 * b;
                     tc_mma_f16(dcol, ad_hi, bd_hi, idesc, (c | b) ? 1u : 0u);
-                    tc_mma_f16(dcol, ad_hi, bd_lo, idesc, 1u);
-                    tc_mma_f16(dcol, ad_lo, bd_hi, idesc, 1u);
+                    tc_mma_f8(dcol, ad_8, bd_8, idesc, 1u);
                 }
                 tc_commit(empty0 + 8 * s);                             // stage free once these MMAs have read it
                 if (flags & HDR_LAST) { tc_commit(tfull); tph ^= 1u; } // accumulator complete

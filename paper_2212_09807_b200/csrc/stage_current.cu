@@ -357,17 +357,14 @@ __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs 
         const float sc = __int_as_float((127 - e) << 23);
         if (tid == 0 && nbins) *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(nB_lo, nB_hi, e, 0);
         const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;
-        __half *Ab = (__half *)a.charge + (size_t)tb * NB2 * (2 * rtc::TB * rtc::JC);
-        const int k = 2 * lane, off = rtc::a_image_offset(r, k);
-        for (int c = warp; c < NB2; c += NT1 / 32) {
-            const float2 x = *(const float2 *)(Csm + c * CJ + k);
-            const float x0 = x.x * sc, x1 = x.y * sc;
-            const __half2 hi = __floats2half2_rn(x0, x1);
-            const float2 hf = __half22float2(hi);
-            const __half2 lo = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
-            __half *dst = Ab + (size_t)c * (2 * rtc::TB * rtc::JC) + off;
-            *(__half2 *)dst = hi;
-            *(__half2 *)(dst + rtc::TB * rtc::JC) = lo;
+        unsigned char *Ab = (unsigned char *)a.charge + (size_t)tb * NB2 * (2 * rtc::A_HALF_BYTES);
+        for (int item = tid; item < NB2 * rtc::NBLK; item += NT1) {
+            const int c = item / rtc::NBLK, b = item - c * rtc::NBLK;
+            float x[16];
+#pragma unroll
+            for (int i = 0; i < 16; ++i) x[i] = Csm[c * CJ + 16 * b + i] * sc;
+            unsigned char *row16 = Ab + (size_t)c * (2 * rtc::A_HALF_BYTES) + r * 128;
+            rtc::store_a_block16(row16, row16 + rtc::A_HALF_BYTES, r, b, x);
         }
         return;
     }
@@ -770,8 +767,9 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     return LARTPC_OK;
 }
 
-// Bs[d][c][hi | lo][NBW x 16] with Bs[n'][jj] = R[c][d][n' - jj] * 2^10 (0 outside the LUT), each half in the canonical
-// un-swizzled K-major layout of rtc::b_image_offset.  Built once per sim on the host.
+// Bs[d][c][fp16 | fp8][NBW x 32 bytes] with Bs[n'][jj] = R[c][d][n' - jj] * 2^10 (0 outside the LUT): the fp16 image
+// (rtc::b_image_offset) and the fp8 image of the cross terms (rtc::b8_image_offset), both in the canonical un-swizzled
+// K-major layout.  Built once per sim on the host.
 size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_out)
 {
     const int nb = p.nb, W = p.W, K = p.K, NBW = p.NBW, NB = W * nb;
@@ -782,14 +780,18 @@ size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_o
         for (int cb = 0; cb < nb; ++cb)
             for (int ca = 0; ca < nb; ++ca) {
                 const float *src = lut_host + ((size_t)(nb * dyi + cb) * NB + (nb * dxi + ca)) * K;
-                __half *hi = img.data() + ((size_t)d * p.NB2 + (cb * nb + ca)) * 2 * half_elems, *lo = hi + half_elems;
+                __half *hi = img.data() + ((size_t)d * p.NB2 + (cb * nb + ca)) * 2 * half_elems;
+                unsigned char *f8 = (unsigned char *)(hi + half_elems);                  // NBW x 32 bytes
                 for (int nn = 0; nn < NBW; ++nn)
                     for (int jj = 0; jj < 16; ++jj) {
                         const int k = nn - jj;
                         const float x = (k >= 0 && k < K) ? ldexpf(src[k], rtc::B_SCALE_LOG2) : 0.f;
                         const __half h = __float2half_rn(x);
                         hi[rtc::b_image_offset(nn, jj)] = h;
-                        lo[rtc::b_image_offset(nn, jj)] = __float2half_rn(x - __half2float(h));
+                        f8[rtc::b8_image_offset(nn, jj)] =
+                            __nv_cvt_float_to_fp8(ldexpf(x, -rtc::SA_LOG2), __NV_SATFINITE, __NV_E4M3);
+                        f8[rtc::b8_image_offset(nn, 16 + jj)] =
+                            __nv_cvt_float_to_fp8(ldexpf(x - __half2float(h), rtc::SB_LOG2), __NV_SATFINITE, __NV_E4M3);
                     }
             }
     }
