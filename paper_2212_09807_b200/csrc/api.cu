@@ -143,6 +143,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     p.d_tran = prm->d_tran_cm2_us; p.dt = prm->tick_us; p.t_origin = prm->t_origin_us; p.pitch = prm->pixel_pitch_cm;
     p.bin = prm->pixel_pitch_cm / (double)nb;  p.sample_step = prm->sample_step_cm;  p.n_sigma_map = prm->n_sigma_map;
     p.recomb_model = prm->recomb_model;
+    { const char *e = getenv("LARTPC_NODE_RULES"); p.node_rules = !(e && strcmp(e, "0") == 0); }  // measurement aid
     p.nb = nb; p.W = W; p.H = (W - 1) / 2; p.K = K; p.WW = W * W; p.NB2 = nb * nb;
     p.n_ticks = prm->n_readout_ticks;  p.j_max = p.n_ticks - K;
     // S4 geometry.  A response task is (pair of target pixels, RESP_NO output ticks); the consumer threads of one CTA

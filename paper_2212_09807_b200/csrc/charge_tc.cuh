@@ -125,8 +125,22 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             L.isT = L.zero_sigma ? 0.f : (float)(p.bin * 0.70710678118654752440 / (double)sT);
             L.ist = L.zero_sigma ? 0.f : (float)(p.dt * 0.70710678118654752440 / (double)st);
             L.q = a.q_anode[s] / (float)L.N;                          // eq. (3.8): Q_a / N per sample point
+            // Node rule instead of the N midpoints (quadrature_tables.cuh): rho = the segment's extent over the diffusion
+            // sigma, per axis, decides how many nodes reproduce the midpoint sum to ~1e-6 of the largest cell (DESIGN.md
+            // section 6 has the measured errors); short or sharp segments keep their own N points.
+            L.qa = a.q_anode[s];
+            L.inv_n2 = 1.0f / ((float)L.N * (float)L.N);
+            L.inv_n4 = L.inv_n2 * L.inv_n2;
+            L.rule = -1;
+            int nq = L.N;
+            if (!L.zero_sigma && p.node_rules) {
+                const float rho = 1.41421356f * fmaxf(fmaxf(fabsf(L.ae - L.as), fabsf(L.be - L.bs)) * L.isT,
+                                                      fabsf(L.te - L.ts) * L.ist);
+                const int k = rho <= 3.5f ? 0 : rho <= 5.5f ? 1 : rho <= 8.f ? 2 : rho <= 12.f ? 3 : rho <= 16.f ? 4 : -1;
+                if (k >= 0 && L.N >= 3 * c_quad_n[k]) { L.rule = c_quad_off[k]; nq = c_quad_n[k]; }
+            }
             segs[tid] = L;
-            if (!(L.jlo > L.jhi || L.alo > L.ahi || L.blo > L.bhi)) n_eff = L.N;   // box misses this tile: no samples
+            if (!(L.jlo > L.jhi || L.alo > L.ahi || L.blo > L.bhi)) n_eff = nq;   // box misses this tile: no samples
         }
         // The K dimension of the contraction is "sample", whichever segment it belongs to: the samples of the staged
         // segments are laid end to end (pre[] = running sum of their counts, in list order) and cut into batches of 64.
@@ -152,7 +166,12 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                     if (li + step < nseg && pre[li + step] <= slot) li += step;
                 const SegLocal L = segs[li];
                 const int mu = slot - pre[li];
-                const float f = ((float)mu + 0.5f) * (1.0f / (float)L.N);
+                float f = ((float)mu + 0.5f) * (1.0f / (float)L.N), qw = L.q;   // position along the segment, charge
+                if (L.rule >= 0) {
+                    const float4 r = __ldg(&g_quad[L.rule + mu]);
+                    f = r.x;
+                    qw = L.qa * (r.y - r.z * L.inv_n2 + r.w * L.inv_n4);
+                }
                 // sigma = 0: the bin / tick is an integer decision taken in float64 in the oracle's order
                 int ia = -1, ib = -1, jj = -1;
                 if (L.zero_sigma && real) {
@@ -202,7 +221,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                 } else {
                     const uint32_t col = ct_col_offset(s_in, NG);
                     const float pt = fmaf(L.te - L.ts, f, L.ts);
-                    const float hq = 0.5f * L.q;
+                    const float hq = 0.5f * qw;
                     for (int g = 0; g < NG; ++g) {
                         float x[8];
                         const int j0 = 8 * g;
@@ -211,7 +230,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                             for (int i = 0; i < 8; ++i) x[i] = 0.f;
                         } else if (L.zero_sigma) {
 #pragma unroll
-                            for (int i = 0; i < 8; ++i) x[i] = (j0 + i == jj) ? L.q : 0.f;
+                            for (int i = 0; i < 8; ++i) x[i] = (j0 + i == jj) ? qw : 0.f;
                         } else {
                             float e0 = erf_fast(((float)j0 - pt) * L.ist);
 #pragma unroll

@@ -29,6 +29,7 @@ struct DevParams {
     int n_groups;                    // pair groups per tile = response passes over a tile (1 for W = 5, K = 200)
     int slab_floats;                 // packed charge lattice of one tile: header, bin items, charge rows
                                      // (tensor-core mode: NB2 * 64 = the tile's rows of the fp16 hi / lo operand image)
+    int node_rules;                  // 1: the tensor-core splat may replace a segment's N midpoints by a node rule (charge_tc.cuh)
     int tc_mode;                     // 1: S4 response on the tensor cores (response_tc.cuh), 0: packed-FFMA2 response
     int NBW;                         // tensor-core mode: output columns per 16-tick arrival block, roundup16(K + 15)
     int n_tpcs;

@@ -133,6 +133,8 @@ struct SplatArgs {
 struct SegLocal {               // one staged segment, tile-relative
     float as, ae, bs, be, ts, te, isT, ist, q;
     int N, alo, ahi, blo, bhi, jlo, jhi, seg, zero_sigma;
+    float qa, inv_n2, inv_n4;   // tensor-core splat: Q_a and 1/N^2, 1/N^4 of the node-rule weights (charge_tc.cuh)
+    int rule;                   // first row of the segment's node rule in g_quad, -1: its own N midpoints
 };
 
 __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs a)
@@ -392,6 +394,7 @@ __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs 
     }
 }
 
+#include "quadrature_tables.cuh"
 #include "charge_tc.cuh"
 
 size_t splat_smem_bytes(const DevParams &p)

@@ -204,3 +204,28 @@ def test_empty_input(lartpc):
     hits, st = sim.run_spill(seg, 1, hit_capacity=16)
     assert st.n_hits == 0
     sim.close()
+
+
+def test_short_drift_all_node_rules(lartpc):
+    """The tensor-core splat replaces a segment's N midpoints by an n-node rule chosen from its extent over the
+    diffusion sigma (n = 8 .. 32, or its own midpoints when the segment is sharp or short).  Tracks along x, along the
+    drift direction and oblique, at 0.2 .. 8 cm of drift, with 1 mm, 0.5 mm and 0.25 mm segments, walk through every
+    rule and the fall-back; every pixel is compared with the oracle (which always sums the N midpoints)."""
+    p = W.default_params(n_readout_ticks=1400)
+    tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, 12.0, 24, 24, 0)]
+    pitch = p["pixel_pitch_cm"]
+    parts = []
+    for k, (z, step) in enumerate([(0.2, 0.1), (0.5, 0.1), (1.0, 0.1), (2.0, 0.1), (4.0, 0.1), (8.0, 0.1),
+                                   (0.5, 0.05), (2.0, 0.05), (8.0, 0.025)]):
+        y = (2.2 + 2.1 * k) * pitch
+        parts.append(W.line_segments([3.1 * pitch, y, z], [6.3 * pitch, y + 0.013, z], step, 0.0, W._mip(2.1)))        # along x
+        parts.append(W.line_segments([9.4 * pitch, y, z], [9.4 * pitch + 0.01, y + 0.02, z + 0.6], step, 0.0, W._mip(2.1)))  # along the drift
+        parts.append(W.line_segments([13.2 * pitch, y, z], [15.9 * pitch, y + 0.5 * pitch, z + 0.35], step, 0.0, W._mip(6.0)))  # oblique
+    seg = W._concat(parts)
+    wl = W.Workload("short-drift", 6, p, tpcs, seg, W.pad_response_lut(p))
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_currents(res, wl, dr, pm)
+    _check_hits(res, wl, dr, pm, wl.seed)
+    sim.close()
