@@ -42,7 +42,7 @@ static void sim_free(lartpc_sim *s)
     cudaFree(s->d_tpcs); cudaFree(s->d_lut); cudaFree(s->d_lut_tc);
     cudaFree(s->pix_count); cudaFree(s->pix_start); cudaFree(s->pix_tile0); cudaFree(s->pix_cursor);
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
-    cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->scan_tmp);
+    cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->tile_list); cudaFree(s->seg_rec); cudaFree(s->scan_tmp);
     cudaFree(s->d_counters); cudaFree(s->disabled_mask); cudaFree(s->elec_slots); cudaFree(s->elec_offs);
     cudaFree(s->d_fma); cudaFree(s->d_work); cudaFree(s->pix_jmin); cudaFree(s->d_end_row);
     for (cudaEvent_t e : s->ev_pool) cudaEventDestroy(e);
@@ -271,6 +271,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     SIM_TRY(cudaMalloc(&s->pair_seg, sizeof(int32_t) * s->pair_cap));
     SIM_TRY(cudaMalloc(&s->tile_cp, sizeof(int32_t) * s->tile_cap));
     SIM_TRY(cudaMalloc(&s->tile_desc, sizeof(TileDesc) * s->tile_cap));
+    SIM_TRY(cudaMalloc(&s->tile_list, sizeof(int2) * s->tile_cap));
 #undef SIM_TRY
     *out = s;
     return LARTPC_OK;

@@ -85,6 +85,8 @@ struct lartpc_sim {
     // growable planning arrays
     int32_t *pair_seg = nullptr;  int64_t pair_cap = 0;
     int32_t *tile_cp = nullptr;   TileDesc *tile_desc = nullptr;  int64_t tile_cap = 0;
+    int2 *tile_list = nullptr;           // [tile_cap] {start, count} of the tile's segment list in pair_seg
+    void *seg_rec = nullptr;  int64_t seg_rec_cap = 0;   // per-segment records of the tensor-core splat (charge_tc.cuh)
     // scan scratch + counters
     long long *scan_tmp = nullptr;  int64_t scan_tmp_elems = 0;
     long long *d_counters = nullptr;  long long *h_counters = nullptr;

@@ -128,6 +128,11 @@ struct SplatArgs {
     float *charge;                     // [n_tiles][slab_floats]
     int32_t *tile_range;
     unsigned long long *fma_counter;   // multiply-adds of the response: non-zero cells x valid targets x K
+    // tensor-core splat (charge_tc.cuh): persistent CTAs
+    const void *rec;                   // SegRec[n]
+    const int2 *tile_list;             // [n_tiles] {start, count} of the tile's segment list in pair_seg
+    int *work;                         // tile cursor, zero at launch
+    int n_tiles;
 };
 
 struct SegLocal {               // one staged segment, tile-relative
@@ -657,6 +662,7 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     a.jt0 = pm->jt0; a.jt1 = pm->jt1; a.n_samples = pm->n_samples;
     a.charge = out->charge;  a.tile_range = out->tile_range;
     a.fma_counter = sim->d_fma;
+    a.rec = nullptr;  a.tile_list = nullptr;  a.work = nullptr;  a.n_tiles = 0;
     if (p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5)) {
         // tensor-core splat (charge_tc.cuh); other bin counts use the FFMA2 splat below, which writes the same image
         static bool configured_tc = false;
@@ -665,9 +671,25 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
             LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
             configured_tc = true;
         }
+        if (n >= (1ll << 30) || sim->n_tiles >= INT32_MAX - 8 * (int64_t)sim->sm_count) return LARTPC_ERR_UNSUPPORTED;
+        if (n > sim->seg_rec_cap) {
+            if (sim->seg_rec) cudaFree(sim->seg_rec);
+            sim->seg_rec = nullptr;  sim->seg_rec_cap = 0;
+            LARTPC_CUDA_TRY(cudaMalloc(&sim->seg_rec, sizeof(SegRec) * (size_t)(n + n / 8 + 1024)));
+            sim->seg_rec_cap = n + n / 8 + 1024;
+        }
+        if (n > 0) {
+            ++g_lartpc_launches;
+            seg_record_kernel<<<div_up(n, 256), 256, 0, st>>>(p, n, dr->q_anode, dr->sigma_T, dr->sigma_t, dr->u_s, dr->v_s,
+                                                             dr->u_e, dr->v_e, dr->T_s, dr->T_e, pm->a_lo, pm->a_hi, pm->b_lo,
+                                                             pm->b_hi, pm->jt0, pm->jt1, pm->n_samples, (SegRec *)sim->seg_rec);
+        }
+        a.rec = sim->seg_rec;  a.tile_list = sim->tile_list;  a.work = sim->d_work;  a.n_tiles = (int)sim->n_tiles;
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
+        const unsigned grid = (unsigned)std::min<int64_t>(sim->n_tiles, 4 * (int64_t)sim->sm_count);
         ++g_lartpc_launches;
-        if (p.nb == 10) charge_lattice_tc_kernel<10><<<(unsigned)sim->n_tiles, CT_THREADS, CT_SMEM, st>>>(a);
-        else charge_lattice_tc_kernel<5><<<(unsigned)sim->n_tiles, CT_THREADS, CT_SMEM, st>>>(a);
+        if (p.nb == 10) charge_lattice_tc_kernel<10><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+        else charge_lattice_tc_kernel<5><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
         LARTPC_CUDA_TRY(cudaGetLastError());
         return LARTPC_OK;
     }

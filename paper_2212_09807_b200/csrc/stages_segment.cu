@@ -312,7 +312,8 @@ pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int3
 __global__ void __launch_bounds__(256)
 tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n_cp, const int32_t *__restrict__ pix_tile0,
                  const unsigned long long *__restrict__ pix_mask, const int32_t *__restrict__ pix_jmin,
-                 int32_t *tile_cp, TileDesc *tile_desc, int64_t tile_cap, int32_t *act_first, int32_t *act_last,
+                 const int32_t *__restrict__ pix_start, const int32_t *__restrict__ pix_count,
+                 int32_t *tile_cp, TileDesc *tile_desc, int2 *tile_list, int64_t tile_cap, int32_t *act_first, int32_t *act_last,
                  long long *counters)
 {
     int64_t cp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -336,7 +337,11 @@ tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n_cp, con
             int w = 64 * wd + __ffsll((long long)m) - 1;
             if (w_lo < 0) w_lo = w;
             w_hi = w;
-            if (tix < tile_cap) { tile_cp[tix] = (int32_t)cp; tile_desc[tix] = TileDesc{tpc, px, py, js + w * p.Jc}; }
+            if (tix < tile_cap) {
+                tile_cp[tix] = (int32_t)cp;
+                tile_desc[tix] = TileDesc{tpc, px, py, js + w * p.Jc};
+                tile_list[tix] = make_int2(pix_start[cp], pix_count[cp]);
+            }
             else atomicAdd((unsigned long long *)&counters[CNT_OVERFLOW], 1ull);
             ++tix;
         }
@@ -445,8 +450,9 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
                                               sim->d_counters + CNT_TILES, sim->scan_tmp, st));
         ++g_lartpc_launches;
         tile_emit_kernel<<<div_up(sim->n_cp, 256), 256, 0, st>>>(p, sim->d_tpcs, sim->n_cp, sim->pix_tile0,
-                                                                sim->pix_mask, sim->pix_jmin, sim->tile_cp,
-                                                                sim->tile_desc, sim->tile_cap, sim->act_first,
+                                                                sim->pix_mask, sim->pix_jmin, sim->pix_start,
+                                                                sim->pix_count, sim->tile_cp, sim->tile_desc,
+                                                                sim->tile_list, sim->tile_cap, sim->act_first,
                                                                 sim->act_last, sim->d_counters);
         LARTPC_CUDA_TRY(cudaGetLastError());
         // active pixels: slot = rank among active pixels (sorted by id), total waveform samples
@@ -469,6 +475,9 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
             if (sim->tile_desc) cudaFree(sim->tile_desc);
             sim->tile_desc = nullptr;
             LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc, sizeof(TileDesc) * cap));
+            if (sim->tile_list) cudaFree(sim->tile_list);
+            sim->tile_list = nullptr;
+            LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list, sizeof(int2) * cap));
             sim->tile_cap = cap;
         }
     }
