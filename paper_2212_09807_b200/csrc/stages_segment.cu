@@ -284,7 +284,7 @@ pair_fill_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n, const 
 }
 
 // the atomics above fill each list in arbitrary order; sort it by segment id so that the float32
-// accumulation order of S4 (and hence every output bit) is reproducible from run to run
+// accumulation order of S4 (and hence every output bit) is reproducible from run to run: one warp per list
 __global__ void __launch_bounds__(128)
 pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int32_t *__restrict__ pix_count,
                  int32_t *pair_seg, int64_t pair_cap)
@@ -297,14 +297,42 @@ pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int3
     int64_t base = pix_start[cp];
     if (base + cnt > pair_cap) return;
     int32_t *v = pair_seg + base;
-    // odd-even transposition sort by one warp (lists hold tens of entries; long ones take cnt passes)
-    for (int pass = 0; pass < cnt; ++pass) {
-        for (int k = (pass & 1) + 2 * lane; k + 1 < cnt; k += 64) {
-            int32_t a = v[k], b = v[k + 1];
-            if (a > b) { v[k] = b; v[k + 1] = a; }
-        }
-        __syncwarp();
+    if (cnt <= 32) {
+        // one element per lane (INT32_MAX past the end), bitonic network over the warp by shuffles
+        int32_t x = lane < cnt ? v[lane] : INT32_MAX;
+#pragma unroll
+        for (int k = 2; k <= 32; k <<= 1)
+#pragma unroll
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                const int32_t y = __shfl_xor_sync(0xffffffffu, x, j);
+                const bool up = ((lane & k) == 0) == ((lane & j) == 0);   // this lane keeps the smaller of the pair
+                x = up ? min(x, y) : max(x, y);
+            }
+        if (lane < cnt) v[lane] = x;
+        return;
     }
+    // longer lists: the same-direction bitonic network on the list in place (first step of every merge pairs i with
+    // its mirror image inside the block, so elements past the end behave as +infinity and are simply skipped)
+    int P = 64;
+    while (P < cnt) P <<= 1;
+    for (int k = 2; k <= P; k <<= 1)
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = lane; t < P / 2; t += 32) {
+                int i, l;
+                if (j == (k >> 1)) {                                   // mirror step
+                    const int blk = t / j, off = t - blk * j;
+                    i = blk * k + off;  l = blk * k + k - 1 - off;
+                } else {
+                    const int blk = t / j, off = t - blk * j;
+                    i = blk * 2 * j + off;  l = i + j;
+                }
+                if (l < cnt) {
+                    const int32_t a = v[i], b = v[l];
+                    if (a > b) { v[i] = b; v[l] = a; }
+                }
+            }
+            __syncwarp();
+        }
 }
 
 // one thread per charged-pixel grid cell: emit its tiles (one per window that holds charge) and mark the pixels
