@@ -25,7 +25,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile with nvcc for sm_100a (cross-compiles without a GPU)."""
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        extra = os.environ.get("LARTPC_NVCC_EXTRA", "").split()       # e.g. -DLARTPC_DEBUG_CLOCKS (measurement builds)
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
               [os.path.join(CSRC, f) for f in SOURCES] + ["-o", LIB]
         subprocess.check_call(cmd)
     return LIB

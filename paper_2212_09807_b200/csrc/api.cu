@@ -153,12 +153,14 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     while ((p.RS & 1) != 0 || ((p.RS >> 1) & 1) == 0) ++p.RS;               // RS = 2 * odd: conflict-free LDS.128 rows
     const int n_pairs = (p.WW + 1) / 2, ncons = RESP_CONSUMERS;
     const size_t smem_limit = (size_t)prop.sharedMemPerBlockOptin;
+    int jc_cap = 120;
+    { const char *e = getenv("LARTPC_JC_CAP"); if (e && atoi(e) >= 8) jc_cap = std::min(120, atoi(e) & ~3); }   // debugging aid
     double best = 0.0;
     int best_groups = 0;
     for (int g = 1; g <= n_pairs; ++g) {
         DevParams q = p;
         q.n_groups = g;  q.PG = (n_pairs + g - 1) / g;
-        int jc = std::min(120, RESP_NO * (ncons / q.PG) - K + 1) & ~3;
+        int jc = std::min(jc_cap, RESP_NO * (ncons / q.PG) - K + 1) & ~3;
         if (jc < 8) continue;
         q.Jc = jc;  q.CJ = jc + 4;
         q.nblk_max = (jc + K - 2) / RESP_NO + 1;
@@ -184,7 +186,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
         if (lartpc_splat_smem(p) > smem_limit) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
     } else {
         p.n_groups = best_groups;  p.PG = (n_pairs + p.n_groups - 1) / p.n_groups;  p.NP = p.n_groups * p.PG;
-        p.Jc = std::min(120, RESP_NO * (ncons / p.PG) - K + 1) & ~3;  p.CJ = p.Jc + 4;
+        p.Jc = std::min(jc_cap, RESP_NO * (ncons / p.PG) - K + 1) & ~3;  p.CJ = p.Jc + 4;
         p.nblk_max = (p.Jc + K - 2) / RESP_NO + 1;  p.tile_ticks = RESP_NO * p.nblk_max;
         p.slab_floats = (SLAB_HDR + 2 * p.NB2 + p.NB2 * (4 + p.CJ) + 3) & ~3;
     }
@@ -235,9 +237,6 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
                     float *dst = re.data() + (((size_t)(cb * nb + ca) * p.NP + d / 2) * p.RS + LUT_OFF) * 2 + (d & 1);
                     for (int k = 0; k < K; ++k) dst[2 * k] = src[k];
                 }
-    for (int c = 0; c < p.NB2 && !p.tc_mode; ++c)
-        for (int g = 0; g < p.n_groups; ++g)
-            memcpy(&re[((size_t)c * p.NP + (size_t)g * p.PG) * p.RS * 2], &g, sizeof(int));
 #define SIM_TRY(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) { \
         lartpc_note_cuda_error(_e, __FILE__, __LINE__); sim_free(s); return LARTPC_ERR_CUDA; } } while (0)
     if (p.tc_mode) {

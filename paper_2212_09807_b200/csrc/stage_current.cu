@@ -477,7 +477,7 @@ __global__ void __launch_bounds__(NT2, 2) response_kernel(const ResponseArgs a)
     const int S = a.n_stages;
     float *stages = (float *)smem_raw;                                // [S][stage_floats]: LUT rows, charge row, header
     u64 *full = (u64 *)(stages + (size_t)S * a.stage_floats);        // [S] "stage filled" (1 arrival + bytes)
-    u64 *empty = full + S;                                            // [S] "stage released" (NCW arrivals)
+    u64 *empty = full + S;                                            // [S] "stage released" (NCW arrivals); then int[S]: pair group
 
     if (tid == 0) {
         for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
@@ -513,6 +513,7 @@ __global__ void __launch_bounds__(NT2, 2) response_kernel(const ResponseArgs a)
                     const uint32_t st = stage0 + (uint32_t)s * stage_bytes, fb = full0 + 8u * s;
                     const uint32_t row_bytes = 16u + (uint32_t)ng * 16u;
                     while (!mbar_try_wait_u32(empty0 + 8u * s, ph ^ 1u)) {}
+                    ((volatile int *)(empty + S))[s] = g;                      // pair group of the stage (released by the arrive below)
                     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fb), "r"(lut_bytes + row_bytes) : "memory");
                     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                                  ::"r"(st), "l"(lut_g + (size_t)c * lut_bin_stride), "r"(lut_bytes), "r"(fb) : "memory");
@@ -559,7 +560,8 @@ __global__ void __launch_bounds__(NT2, 2) response_kernel(const ResponseArgs a)
         DBG_ADD(3, 1);
         const float *row = st + a.lut_floats;
         const int4 h = *(const int4 *)row;                            // first charged tick, groups, flags, tile
-        if (h.z & FLAG_END) { DBG_FLUSH; break; }
+        const int g = ((volatile int *)(empty + S))[s];              // pair group of this pass, published by the producer
+        if ((h.z & FLAG_END) | (g < 0)) { DBG_FLUSH; break; }
         if (valid) {
             const int jb0 = h.x, ng = h.y;
             // group m holds charges j = jb0 + 4m .. + 3; its taps k = n - j meet [0, K) for this task's outputs when
@@ -595,8 +597,6 @@ __global__ void __launch_bounds__(NT2, 2) response_kernel(const ResponseArgs a)
                 }
             }
         }
-        int g = 0;
-        if (h.z & FLAG_LAST) g = *(const int *)st;                    // pair group of this pass: word 0 of the LUT block
         __syncwarp();
         DBG_T(t2);
         DBG_ADD(1, t2 - t1);
@@ -728,7 +728,7 @@ int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t
     memcpy(a.blk_of_slot, sim->blk_of_slot, sizeof(a.blk_of_slot));
     a.end_row = sim->d_end_row;
     if (a.n_stages < 2) return LARTPC_ERR_UNSUPPORTED;
-    size_t smem = (size_t)a.n_stages * a.stage_floats * 4 + 2 * (size_t)a.n_stages * sizeof(u64);
+    size_t smem = (size_t)a.n_stages * a.stage_floats * 4 + 2 * (size_t)a.n_stages * sizeof(u64) + 64;   // + pair group per stage
     static size_t configured = 0;
     if (smem > configured) {
         LARTPC_CUDA_TRY(cudaFuncSetAttribute(response_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -736,6 +736,8 @@ int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t
     }
     LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
     int grid = (int)std::min<int64_t>(n_work, 2 * (int64_t)sim->sm_count);
+    { const char *e = getenv("LARTPC_RESP_GRID"); if (e && atoi(e) > 0) grid = std::min(grid, atoi(e)); }      // debugging aid
+    { const char *e = getenv("LARTPC_RESP_STAGES"); if (e && atoi(e) >= 2) a.n_stages = std::min(a.n_stages, atoi(e)); }
     ++g_lartpc_launches;
     response_kernel<<<grid, NT2, smem, st>>>(a);
     LARTPC_CUDA_TRY(cudaGetLastError());

@@ -229,3 +229,21 @@ def test_short_drift_all_node_rules(lartpc):
     _check_currents(res, wl, dr, pm)
     _check_hits(res, wl, dr, pm, wl.seed)
     sim.close()
+
+
+@pytest.mark.parametrize("window,lut_ticks,mode", [(9, 200, "tensor"), (9, 200, "ffma"), (5, 500, "ffma"), (5, 120, "tensor")])
+def test_config4_axes_small(lartpc, window, lut_ticks, mode):
+    """BASELINE configs[4] sweep axes at a size the oracle finishes in seconds: 9x9 response window and LUT lengths
+    other than 200 ticks (K > 241 has no tensor-core path: NBW would exceed one MMA's N, the FFMA2 kernel takes it)."""
+    p = W.default_params(window_pixels=window, lut_ticks=lut_ticks, n_readout_ticks=700 + lut_ticks)
+    tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, 20.0, 20, 20, 0)]
+    pitch = p["pixel_pitch_cm"]
+    parts = [W.line_segments([2.3 * pitch, 3.1 * pitch, 6.0], [9.7 * pitch, 12.4 * pitch, 7.5], 0.1, 0.0, W._mip(2.1)),
+             W.line_segments([15.2 * pitch, 1.1 * pitch, 1.0], [18.9 * pitch, 3.0 * pitch, 1.2], 0.05, 0.3, W._mip(8.0))]
+    wl = W.Workload("c4-small", 4, p, tpcs, W._concat(parts), W.pad_response_lut(p))
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, response=mode)
+    assert sim.response_mode == mode
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_currents(res, wl, dr, pm, max_pixels=40)
+    sim.close()
