@@ -5,6 +5,7 @@ One "step" = one pass of the whole hot path (S1 quench .. S6 electronics, `lartp
 synthetic spill.  Metric (BASELINE.json): segments/s (whole job) with ms/spill as `ms_per_step`.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+  python bench.py --config 4            BASELINE configs[4]: the induced-current sweep (S4 + S5 only), one JSON line
 
 * `value`     segments/s with the segment arrays already resident in HBM (device-timed, CUDA events).
 * `e2e`       same metric through the C-ABI with HOST (pinned) segment arrays: host->device copy of the nine
@@ -49,7 +50,9 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3, 4],
+                    help="0-3: one spill of that BASELINE config; 4: the induced-current sweep (S4 + S5 only, one axis at a time)")
+    ap.add_argument("--sweep-max-segments", type=int, default=10_000_000, help="largest segment count of the config-4 sweep")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--segments", type=int, default=None, help="override the segment target of configs 2/3")
     ap.add_argument("--response", default="auto", choices=["auto", "tensor", "ffma"],
@@ -283,14 +286,16 @@ def run_ours(args):
             K, nb2, ww = int(wl.params["lut_ticks"]), int(wl.params["bins_per_pixel"]) ** 2, int(wl.params["window_pixels"]) ** 2
             nbw = (K + 15 + 15) // 16 * 16
             tiles_per_launch = int(st.n_tiles) * args.steps / n_resp
-            executed = 2.0 * (tiles_per_launch / 128.0) * ww * nb2 * 12 * 128.0 * nbw * 16     # 4 blocks x 3 hi/lo products
+            # 4 blocks x (one fp16 MMA of K = 16 + one fp8 MMA of K = 32, which occupies the pipe like an fp16 K = 16):
+            # 8 fp16-equivalent MMA slots per (tile block, target, bin)
+            executed = 2.0 * (tiles_per_launch / 128.0) * ww * nb2 * 8 * 128.0 * nbw * 16
             roof = {"kernel": "rtc::response_tc_kernel (S4 induced current, response on tcgen05)", "bound": "tensor",
                     "achieved": useful, "peak": peak, "unit": "TFLOP/s", "frac": useful / peak,
                     "achieved_note": "algorithmic: non-zero charge cells x in-plane targets x lut_ticks x 2 (counted on "
                                      "the device), what the method needs whatever the decomposition",
                     "executed_tflops": executed / (s4_ms * 1e-3) / 1e12 if s4_ms > 0 else 0.0,
                     "executed_frac": executed / (s4_ms * 1e-3) / 1e12 / peak if s4_ms > 0 else None,
-                    "executed_note": "dense MMA flops issued: tiles x bins x 64 ticks x targets x NBW columns x 3 products",
+                    "executed_note": "dense MMA work issued in fp16-equivalent flops: tile blocks x targets x bins x 8 MMA slots (4 x (fp16 K=16 + fp8 K=32)) x 128 x NBW x 16 x 2",
                     "fp32_alu_peak": max(peak_scalar, peak_packed), "peak_source": peak_src}
         else:
             peak = max(peak_scalar, peak_packed)
@@ -333,10 +338,108 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------------------------------
+# BASELINE configs[4]: induced-current kernel sweep (S4 charge lattice + S4 response + S5 sum), one axis at a time
+# about the base point (1e5 segments of 1 mm at 30 cm drift, 5x5 window, K = 200), track-like placement on one plane
+# --------------------------------------------------------------------------------------------------
+SWEEP_BASE = dict(n_segments=100_000, seg_len_cm=0.1, drift_cm=30.0, window_pixels=5, lut_ticks=200)
+
+
+def sweep_points(max_segments):
+    pts = [("base", {})]
+    pts += [("count", dict(n_segments=n)) for n in (1_000, 10_000, 1_000_000, 10_000_000) if n <= max_segments]
+    pts += [("length", dict(seg_len_cm=l)) for l in (0.05, 0.2, 0.5, 1.0)]
+    pts += [("drift", dict(drift_cm=d)) for d in (0.0, 1.0, 10.0, 50.0)]
+    pts += [("window", dict(window_pixels=9))]
+    pts += [("lut_ticks", dict(lut_ticks=k)) for k in (500, 1000, 2000)]
+    return pts
+
+
+def run_sweep(args):
+    import torch
+    from paper_2212_09807_b200 import lartpc
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: the LArTPC path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    hbm_peak = 6541.1
+    try:
+        hbm_peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        pass
+    fp32_peak = max(lartpc.measure_fp32_peak(0), lartpc.measure_fp32_peak(1))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    rows, launches0 = [], lartpc.kernel_launches()
+    clocks = ClockSampler(0)
+    clocks.start()
+    for axis, over in sweep_points(args.sweep_max_segments):
+        kw = dict(SWEEP_BASE, **over)
+        wl = workloads.make_config(4, **kw)
+        n = wl.n_segments
+        sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, device="cuda:0", response=args.response)
+        seg = sim.upload_segments(wl.segments)
+        _, ne = sim.quench(seg)                                      # staged S1-S3 once: the tile geometry of this sim
+        dr = sim.drift(seg, ne)
+        _, pinfo = sim.pixels_from_segments(seg, dr)
+        tile_bytes = 4.0 * pinfo.tile_charge_floats + 4.0 * pinfo.tile_targets * pinfo.tile_ticks
+        del dr, ne
+        free, _ = torch.cuda.mem_get_info()
+        # longer segments and wider windows need more tile memory per segment than the library's 1 mm estimate
+        ws = torch.empty(int(min(max(sim.workspace_bytes(n), 64 << 30), 0.8 * free)), dtype=torch.uint8, device=dev)
+        hit_cap = int(min(64_000_000, max(1 << 16, 8 * n)))
+        hits, st = sim.run_spill(seg, wl.seed, hit_cap, workspace=ws)
+        for _ in range(max(args.warmup - 1, 0)):
+            flush.zero_()
+            hits, st = sim.run_spill(seg, wl.seed, hit_cap, workspace=ws, hits=hits)
+        sim.set_profiling(True)
+        acc = {k: 0.0 for k in sim.STAGES}
+        fma = 0.0
+        for _ in range(args.steps):
+            flush.zero_()
+            hits, st = sim.run_spill(seg, wl.seed, hit_cap, workspace=ws, hits=hits)
+            ms, _, f = sim.stage_ms()
+            for k in sim.STAGES:
+                acc[k] += ms[k] / args.steps
+            fma += f / args.steps
+        t_ch, t_rs, t_sum = acc["induced_current_charge"], acc["induced_current_response"], acc["sum_pixel_signals"]
+        t = t_ch + t_rs + t_sum
+        # algorithmic HBM bytes of S4 + S5: 48 B / segment in, every stored waveform sample written once (4 B); the
+        # tile intermediates (charge image + partial rows, written once and read once) are the decomposition's own
+        inter = 2.0 * int(st.n_tiles) * tile_bytes
+        alg = 48.0 * n + 4.0 * int(st.total_samples)
+        rows.append(dict(axis=axis, **kw, n_segments_actual=n, response_mode=sim.response_mode,
+                         n_tiles=int(st.n_tiles), n_active_pixels=int(st.n_active_pixels),
+                         ms_charge=t_ch, ms_response=t_rs, ms_sum=t_sum, ms_s4_s5=t,
+                         segments_per_s=n / (t * 1e-3) if t > 0 else None,
+                         useful_tflops=2.0 * fma / ((t_ch + t_rs) * 1e-3) / 1e12 if t_ch + t_rs > 0 else None,
+                         frac_fp32_peak=2.0 * fma / ((t_ch + t_rs) * 1e-3) / 1e12 / fp32_peak if t_ch + t_rs > 0 else None,
+                         hbm_gbs_algorithmic=alg / (t * 1e-3) / 1e9 if t > 0 else None,
+                         hbm_gbs_with_tile_intermediates=(alg + inter) / (t * 1e-3) / 1e9 if t > 0 else None,
+                         frac_hbm_peak_with_intermediates=(alg + inter) / (t * 1e-3) / 1e9 / hbm_peak if t > 0 else None))
+        sys.stderr.write("sweep %-9s %s: %d segments, %d tiles, S4+S5 %.2f ms (%s)\n"
+                         % (axis, over, n, int(st.n_tiles), t, sim.response_mode))
+        sim.close()
+        del ws, seg, hits
+        torch.cuda.empty_cache()
+    clk = clocks.stop()
+    base = rows[0]
+    line = {"metric": "segments/s through S4 + S5 (induced current + per-pixel sum), configs[4] base point",
+            "value": base["segments_per_s"], "unit": "segments/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": base["ms_s4_s5"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "configs[4] induced-current sweep, one 226x677 plane, track-like placement",
+                       "base": SWEEP_BASE, "l2": "256 MiB flush write between timed steps"},
+            "fp32_alu_peak_tflops": fp32_peak, "hbm_peak_gbs": hbm_peak, "clocks": clk,
+            "gpu_launches": int(lartpc.kernel_launches() - launches0), "sweep": rows}
+    print(json.dumps(line))
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.config == 4:
+        run_sweep(args)
     else:
         run_ours(args)
 

@@ -416,7 +416,7 @@ def config4(seed=None, n_segments=100_000, seg_len_cm=0.1, drift_cm=30.0, window
     rng = np.random.Generator(np.random.PCG64(seed))
     p = default_params(recomb_model=0, window_pixels=window_pixels, lut_ticks=lut_ticks)
     nx, ny = 226, 677
-    max_drift = 50.0
+    max_drift = 51.0                                  # the 50 cm sweep point sits inside the volume, not on the cathode
     tpcs = [make_tpc(0.0, 0.0, 0.0, +1, max_drift, nx, ny, 0)]
     W, H = nx * PITCH_CM, ny * PITCH_CM
     parts, n = [], 0
