@@ -42,7 +42,8 @@ static void sim_free(lartpc_sim *s)
     cudaFree(s->d_tpcs); cudaFree(s->d_lut); cudaFree(s->d_lut_tc);
     cudaFree(s->pix_count); cudaFree(s->pix_start); cudaFree(s->pix_tile0); cudaFree(s->pix_cursor);
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
-    cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->tile_list); cudaFree(s->seg_rec); cudaFree(s->scan_tmp);
+    cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->tile_list); cudaFree(s->seg_rec);
+    cudaFree(s->tile_perm); cudaFree(s->tile_desc_p); cudaFree(s->tile_list_p); cudaFree(s->tb_mask); cudaFree(s->cls_hist); cudaFree(s->scan_tmp);
     cudaFree(s->d_counters); cudaFree(s->disabled_mask); cudaFree(s->elec_slots); cudaFree(s->elec_offs);
     cudaFree(s->d_fma); cudaFree(s->d_work); cudaFree(s->pix_jmin); cudaFree(s->d_end_row);
     for (cudaEvent_t e : s->ev_pool) cudaEventDestroy(e);
@@ -135,6 +136,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     s->tpcs.assign(tpcs, tpcs + n_tpcs);
     s->sm_count = prop.multiProcessorCount;
     { const char *e = getenv("LARTPC_SPLAT"); s->splat_tc = !(e && strcmp(e, "ffma") == 0); }   // measurement aid
+    { const char *e = getenv("LARTPC_TILE_SORT"); s->tile_sort = !(e && strcmp(e, "0") == 0); } // measurement aid
     DevParams &p = s->dp;
     memset(&p, 0, sizeof(p));
     p.eps = prm->e_field_kv_cm * prm->lar_density_g_cm3;  p.w_ion = prm->w_ion_mev;
@@ -266,11 +268,9 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     SIM_TRY(cudaMallocHost(&s->h_counters, sizeof(long long) * CNT_COUNT));
     SIM_TRY(cudaMalloc(&s->d_fma, sizeof(unsigned long long)));
     SIM_TRY(cudaMemset(s->d_fma, 0, sizeof(unsigned long long)));
-    s->pair_cap = 1 << 16;  s->tile_cap = 1 << 14;
+    s->pair_cap = 1 << 16;
     SIM_TRY(cudaMalloc(&s->pair_seg, sizeof(int32_t) * s->pair_cap));
-    SIM_TRY(cudaMalloc(&s->tile_cp, sizeof(int32_t) * s->tile_cap));
-    SIM_TRY(cudaMalloc(&s->tile_desc, sizeof(TileDesc) * s->tile_cap));
-    SIM_TRY(cudaMalloc(&s->tile_list, sizeof(int2) * s->tile_cap));
+    if (sim_grow_tiles(s, 1 << 14) != 0) { sim_free(s); return LARTPC_ERR_CUDA; }
 #undef SIM_TRY
     *out = s;
     return LARTPC_OK;

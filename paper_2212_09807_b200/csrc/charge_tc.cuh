@@ -426,16 +426,17 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                 }
             }
             if (tid < NB2) {
+                // rows of the response's operand image; only the 16-tick blocks some tile of the block charges exist
                 const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;
-                unsigned char *row16 = (unsigned char *)a.charge +
-                                       (((size_t)tb * NB2 + tid) * 2 * rtc::TB + r) * (rtc::JC * 2);  // fp16 row of (bin, tile)
-                unsigned char *row8 = row16 + rtc::TB * rtc::JC * 2;                                    // fp8 row
-    #pragma unroll
+                const int bm = a.tb_mask[tb];
+                unsigned char *cb = (unsigned char *)a.charge + ((size_t)tb * NB2 + tid) * (rtc::NBLK * rtc::A_BLOCK_BYTES);
+#pragma unroll
                 for (int b = 0; b < rtc::NBLK; ++b) {
+                    if (!(bm >> b & 1)) continue;
                     float x[16];
-    #pragma unroll
+#pragma unroll
                     for (int i = 0; i < 16; ++i) x[i] = __uint_as_float(v[(16 * b + i) >> 5][(16 * b + i) & 31]) * sc;
-                    rtc::store_a_block16(row16, row8, r, b, x);
+                    rtc::store_a_block16(cb + b * rtc::A_BLOCK_BYTES, r, x);
                 }
             }
         }

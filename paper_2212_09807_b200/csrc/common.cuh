@@ -86,6 +86,11 @@ struct lartpc_sim {
     int32_t *pair_seg = nullptr;  int64_t pair_cap = 0;
     int32_t *tile_cp = nullptr;   TileDesc *tile_desc = nullptr;  int64_t tile_cap = 0;
     int2 *tile_list = nullptr;           // [tile_cap] {start, count} of the tile's segment list in pair_seg
+    // tensor-core mode: tiles sorted by the 16-tick blocks they charge (launch_plan): slot of a tile, descriptors and
+    // lists in slot order, per 128-slot block the OR of its tiles' block masks
+    int32_t *tile_perm = nullptr;  TileDesc *tile_desc_p = nullptr;  int2 *tile_list_p = nullptr;
+    int32_t *tb_mask = nullptr;  int32_t *cls_hist = nullptr;   // [tile_cap / 128 + 2], [32]: class counts then cursors
+    bool tile_sort = true;               // env LARTPC_TILE_SORT=0: identity order, every block kept (measurement aid)
     void *seg_rec = nullptr;  int64_t seg_rec_cap = 0;   // per-segment records of the tensor-core splat (charge_tc.cuh)
     // scan scratch + counters
     long long *scan_tmp = nullptr;  int64_t scan_tmp_elems = 0;
@@ -142,6 +147,7 @@ static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); 
 int launch_quench(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, float *dEdx, float *n_e, cudaStream_t st);
 int launch_drift(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, const float *n_e, lartpc_drifted_t *out,
                  cudaStream_t st);
+int sim_grow_tiles(lartpc_sim *sim, int64_t cap);
 int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drifted_t *dr, int64_t n,
                 int tpc_lo, int tpc_hi, lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, cudaStream_t st);
 int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,

@@ -46,24 +46,26 @@ constexpr int B_SCALE_LOG2 = 10;
 // fp8 parts: lo8(A) = e4m3(lo(A) 2^SA) meets hi8(B) = e4m3(B 2^-SA); hi8(A) = e4m3(A 2^-SB) meets lo8(B) = e4m3(lo(B) 2^SB)
 // (|A| < 2^15, |lo(A)| <= 8, |B| <= 2^10, |lo(B)| <= 0.5: every part stays below e4m3's 448)
 constexpr int SA_LOG2 = 5, SB_LOG2 = 7;
-constexpr int A_HALF_BYTES = TB * JC * 2;          // one precision half of an A stage image (16 KB)
+constexpr int A_HALF_BYTES = TB * JC * 2;          // half of a stage's A area (the area holds NBLK blocks of 8 KB)
 
 struct Args {
     const __half *A;               // [n_tb][NC][2][TB][128 bytes]: fp16 image (a_image_offset) + fp8 image (a8_image_offset)
     const __half *B;               // [WW][NC][2][NBW * 32 bytes]: fp16 image (b_image_offset) + fp8 image (b8_image_offset)
     float *partial;                // [n_tiles][WW][tile_ticks]
     const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), 0
+    const int32_t *tb_mask;        // [n_tb] 16-tick blocks that hold charge in any tile of the block (bit b)
     int n_tiles, n_tb, NC, WW, NBW, tile_ticks;
     long long n_items;             // n_tb * WW
     int *work;                     // item cursor, zero at launch: items are taken in order as CTAs become free, so the
                                    // CTAs that stream one tile block stay together however long the launch runs
 };
 
-// byte image of one precision half of an A stage: row r (tile in block), element k (arrival tick), SWIZZLE_128B K-major
-__host__ __device__ __forceinline__ int a_image_offset(int r, int k)          // in halfs
-{
-    return r * JC + ((((k >> 3) ^ (r & 7)) << 3) | (k & 7));
-}
+// A image: [tile block][bin c][16-tick block b][fp16 part | fp8 part][128 rows x 32 bytes], each part a canonical
+// un-swizzled K-major operand of one MMA (row r = tile in block; 16-byte K chunks 128 B apart, 8-row groups 256 B apart),
+// so that a stage copies only the 16-tick blocks that hold charge.  Byte offset of K chunk kc (0 / 1) of row r in a part:
+__host__ __device__ __forceinline__ int a_part_offset(int r, int kc) { return (r >> 3) * 256 + kc * 128 + (r & 7) * 16; }
+constexpr int A_PART_BYTES = 128 * 32;                 // one part of one block: 4 KB
+constexpr int A_BLOCK_BYTES = 2 * A_PART_BYTES;        // fp16 part + fp8 part
 // canonical un-swizzled K-major image of Bs: row n' (output column), element jj: 8 x 16-byte core matrices,
 // K chunks 128 B apart (LBO), 8-row groups 256 B apart (SBO)
 __host__ __device__ __forceinline__ int b_image_offset(int n, int jj)         // in halfs
@@ -71,12 +73,6 @@ __host__ __device__ __forceinline__ int b_image_offset(int n, int jj)         //
     return (n >> 3) * 128 + (jj >> 3) * 64 + (n & 7) * 8 + (jj & 7);
 }
 
-// fp8 image of A: row r = 128 bytes = 4 blocks b of [lo8 of ticks 16 b .. 16 b + 15 | hi8 of the same ticks]; returns the
-// byte offset of the 16-byte chunk (part = 0: lo8, 1: hi8) under the same 128-byte swizzle
-__host__ __device__ __forceinline__ int a8_image_offset(int r, int b, int part)
-{
-    return r * 128 + ((((2 * b + part) ^ (r & 7))) << 4);
-}
 // fp8 image of Bs: row n', K byte kb in [0, 32): kb < 16 -> hi8 of jj = kb, else lo8 of jj = kb - 16; same canonical
 // K-major byte layout as the fp16 image (16-byte core rows, K chunks 128 B apart, 8-row groups 256 B apart)
 __host__ __device__ __forceinline__ int b8_image_offset(int n, int kb)
@@ -84,9 +80,9 @@ __host__ __device__ __forceinline__ int b8_image_offset(int n, int kb)
     return (n >> 3) * 256 + (kb >> 4) * 128 + (n & 7) * 16 + (kb & 15);
 }
 
-// Writes 16 consecutive arrival ticks (block b) of row r of one bin's A operand: x = C 2^-e, |x| < 2^15.
-// row16 / row8: start of row r (128 bytes each) in the fp16 and in the fp8 image.
-__device__ __forceinline__ void store_a_block16(unsigned char *row16, unsigned char *row8, int r, int b, const float (&x)[16])
+// Writes 16 consecutive arrival ticks (one block b) of row r of one bin's A operand: x = C 2^-e, |x| < 2^15.
+// blk: start of that (bin, block) in the image (A_BLOCK_BYTES).  fp16 part: ticks 0-7 | 8-15; fp8 part: lo8 | hi8.
+__device__ __forceinline__ void store_a_block16(unsigned char *blk, int r, const float (&x)[16])
 {
     __half2 h[8];
     unsigned short l8[8], h8[8];
@@ -98,11 +94,11 @@ __device__ __forceinline__ void store_a_block16(unsigned char *row16, unsigned c
         l8[i] = __nv_cvt_float2_to_fp8x2(make_float2((x[2 * i] - f.x) * sa, (x[2 * i + 1] - f.y) * sa), __NV_SATFINITE, __NV_E4M3);
         h8[i] = __nv_cvt_float2_to_fp8x2(make_float2(x[2 * i] * sb, x[2 * i + 1] * sb), __NV_SATFINITE, __NV_E4M3);
     }
-    const int s0 = ((2 * b) ^ (r & 7)) << 4, s1 = ((2 * b + 1) ^ (r & 7)) << 4;
-    *(uint4 *)(row16 + s0) = *(const uint4 *)&h[0];
-    *(uint4 *)(row16 + s1) = *(const uint4 *)&h[4];
-    *(uint4 *)(row8 + s0) = *(const uint4 *)l8;
-    *(uint4 *)(row8 + s1) = *(const uint4 *)h8;
+    const int o0 = a_part_offset(r, 0), o1 = a_part_offset(r, 1);
+    *(uint4 *)(blk + o0) = *(const uint4 *)&h[0];
+    *(uint4 *)(blk + o1) = *(const uint4 *)&h[4];
+    *(uint4 *)(blk + A_PART_BYTES + o0) = *(const uint4 *)l8;
+    *(uint4 *)(blk + A_PART_BYTES + o1) = *(const uint4 *)h8;
 }
 
 __device__ __forceinline__ uint32_t s32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -241,12 +237,17 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 const int tb = (int)(q / a.WW), d = (int)(q - (long long)tb * a.WW);
                 const unsigned char *Ab = (const unsigned char *)a.A + (size_t)tb * NC * (2 * A_HALF_BYTES);
                 const unsigned char *Bb = (const unsigned char *)a.B + (size_t)d * NC * (2 * b_half);
-                for (int c = 0; c < NC; ++c) {
+                const int bm = a.tb_mask[tb] & ((1 << NBLK) - 1);
+                const uint32_t a_bytes = (uint32_t)__popc(bm) * A_BLOCK_BYTES;
+                for (int c = 0; c < NC && bm; ++c) {
                     mbar_wait(empty0 + 8 * s, ph ^ 1u);
                     const uint32_t st = base + s * stage_sz, fb = full0 + 8 * s;
-                    hdr[s].x = tb;  hdr[s].y = d;  hdr[s].z = c;  hdr[s].w = (c == NC - 1) ? HDR_LAST : 0;
-                    mbar_expect_tx(fb, stage_sz);                      // release: the header is visible to the waiter
-                    bulk_g2s(st, Ab + (size_t)c * (2 * A_HALF_BYTES), 2 * A_HALF_BYTES, fb);
+                    hdr[s].x = tb;  hdr[s].y = d;  hdr[s].z = c | (bm << 16);  hdr[s].w = (c == NC - 1) ? HDR_LAST : 0;
+                    mbar_expect_tx(fb, a_bytes + 2 * b_half);          // release: the header is visible to the waiter
+                    const unsigned char *Ac = Ab + (size_t)c * (NBLK * A_BLOCK_BYTES);
+#pragma unroll
+                    for (int b = 0; b < NBLK; ++b)
+                        if (bm >> b & 1) bulk_g2s(st + b * A_BLOCK_BYTES, Ac + b * A_BLOCK_BYTES, A_BLOCK_BYTES, fb);
                     bulk_g2s(st + 2 * A_HALF_BYTES, Bb + (size_t)c * (2 * b_half), 2 * b_half, fb);
                     if (++s == STAGES) { s = 0; ph ^= 1u; }
                 }
@@ -266,7 +267,8 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
             uint32_t ph = 0, tph = 0;
             while (true) {
                 mbar_wait(full0 + 8 * s, ph);
-                const int tb = hdr[s].x, d = hdr[s].y, c = hdr[s].z, flags = hdr[s].w;
+                const int tb = hdr[s].x, d = hdr[s].y, cz = hdr[s].z, flags = hdr[s].w;
+                const int c = cz & 0xffff, bm = cz >> 16;
                 if (flags & HDR_END) {
                     mbar_wait(tempty, tph);                            // the epilogue has read the previous item slot
                     epi_item->w = HDR_END;
@@ -274,7 +276,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                     break;
                 }
                 if (c == 0) {
-                    mbar_wait(tempty, tph);                            // accumulator drained and re-zeroed
+                    mbar_wait(tempty, tph);                            // accumulator drained and zeroed
                     epi_item->x = tb;  epi_item->y = d;  epi_item->w = 0;
                     mbar_arrive(titem);                                // release: hands the item to the epilogue
                 }
@@ -284,10 +286,11 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 const uint64_t bd_8 = smem_desc(st + 2 * A_HALF_BYTES + b_half, 128, 256, 0);
 #pragma unroll
                 for (int b = 0; b < NBLK; ++b) {
-                    const uint64_t ad_hi = smem_desc(st + 32 * b, 16, 1024, 2);
-                    const uint64_t ad_8 = smem_desc(st + A_HALF_BYTES + 32 * b, 16, 1024, 2);
+                    if (!(bm >> b & 1)) continue;                      // no tile of the block has charge in these 16 ticks
+                    const uint64_t ad_hi = smem_desc(st + b * A_BLOCK_BYTES, 128, 256, 0);
+                    const uint64_t ad_8 = smem_desc(st + b * A_BLOCK_BYTES + A_PART_BYTES, 128, 256, 0);
                     const uint32_t dcol = tmem + 16 * b;
-                    tc_mma_f16(dcol, ad_hi, bd_hi, idesc, (c | b) ? 1u : 0u);
+                    tc_mma_f16(dcol, ad_hi, bd_hi, idesc, 1u);         // the epilogue leaves the whole accumulator zero
                     tc_mma_f8(dcol, ad_8, bd_8, idesc, 1u);
                 }
                 tc_commit(empty0 + 8 * s);                             // stage free once these MMAs have read it
@@ -299,8 +302,8 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
         // ------------------------------------------------------------------ epilogue (warps 2-5)
         const int quad = warp & 3;                                     // TMEM lanes [32 quad, 32 quad + 32)
         const uint32_t tlane = tmem + ((uint32_t)(32 * quad) << 16);
-        // columns [NBW, n_acc_cols) are only ever accumulated into: zero them before the first item
-        for (int c0 = NBW; c0 < n_acc_cols; c0 += 16) tmem_zero16(tlane + c0);
+        // every MMA accumulates: the accumulator is zero before the first item and zeroed again after each read-out
+        for (int c0 = 0; c0 < n_acc_cols; c0 += 16) tmem_zero16(tlane + c0);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         tc_fence_before();
         __syncwarp();
@@ -340,7 +343,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                                                                          __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale));
                 }
             }
-            for (int c0 = NBW; c0 < n_acc_cols; c0 += 16) tmem_zero16(tlane + c0);
+            for (int c0 = 0; c0 < n_acc_cols; c0 += 16) tmem_zero16(tlane + c0);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();

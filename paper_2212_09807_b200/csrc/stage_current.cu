@@ -133,6 +133,7 @@ struct SplatArgs {
     const int2 *tile_list;             // [n_tiles] {start, count} of the tile's segment list in pair_seg
     int *work;                         // tile cursor, zero at launch
     int n_tiles;
+    const int32_t *tb_mask;            // [tile blocks] 16-tick blocks that hold charge (bit b)
 };
 
 struct SegLocal {               // one staged segment, tile-relative
@@ -364,14 +365,13 @@ __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs 
         const float sc = __int_as_float((127 - e) << 23);
         if (tid == 0 && nbins) *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(nB_lo, nB_hi, e, 0);
         const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;
-        unsigned char *Ab = (unsigned char *)a.charge + (size_t)tb * NB2 * (2 * rtc::A_HALF_BYTES);
+        unsigned char *Ab = (unsigned char *)a.charge + (size_t)tb * NB2 * (rtc::NBLK * rtc::A_BLOCK_BYTES);
         for (int item = tid; item < NB2 * rtc::NBLK; item += NT1) {
             const int c = item / rtc::NBLK, b = item - c * rtc::NBLK;
             float x[16];
 #pragma unroll
             for (int i = 0; i < 16; ++i) x[i] = Csm[c * CJ + 16 * b + i] * sc;
-            unsigned char *row16 = Ab + (size_t)c * (2 * rtc::A_HALF_BYTES) + r * 128;
-            rtc::store_a_block16(row16, row16 + rtc::A_HALF_BYTES, r, b, x);
+            rtc::store_a_block16(Ab + ((size_t)c * rtc::NBLK + b) * rtc::A_BLOCK_BYTES, r, x);
         }
         return;
     }
@@ -654,7 +654,7 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     SplatArgs a;
     a.p = p;
     a.tpcs = sim->d_tpcs;
-    a.tile_cp = sim->tile_cp;  a.tile_desc = sim->tile_desc;
+    a.tile_cp = sim->tile_cp;  a.tile_desc = sim->tile_desc;   // the tensor-core splat walks the sorted copies (below)
     a.pix_start = sim->pix_start;  a.pix_count = sim->pix_count;  a.pair_seg = sim->pair_seg;
     a.q_anode = dr->q_anode;  a.sigma_T = dr->sigma_T;  a.sigma_t = dr->sigma_t;
     a.u_s = dr->u_s; a.v_s = dr->v_s; a.u_e = dr->u_e; a.v_e = dr->v_e; a.T_s = dr->T_s; a.T_e = dr->T_e;
@@ -662,7 +662,7 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     a.jt0 = pm->jt0; a.jt1 = pm->jt1; a.n_samples = pm->n_samples;
     a.charge = out->charge;  a.tile_range = out->tile_range;
     a.fma_counter = sim->d_fma;
-    a.rec = nullptr;  a.tile_list = nullptr;  a.work = nullptr;  a.n_tiles = 0;
+    a.rec = nullptr;  a.tile_list = nullptr;  a.work = nullptr;  a.n_tiles = 0;  a.tb_mask = sim->tb_mask;
     if (p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5)) {
         // tensor-core splat (charge_tc.cuh); other bin counts use the FFMA2 splat below, which writes the same image
         static bool configured_tc = false;
@@ -684,7 +684,8 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
                                                              dr->u_e, dr->v_e, dr->T_s, dr->T_e, pm->a_lo, pm->a_hi, pm->b_lo,
                                                              pm->b_hi, pm->jt0, pm->jt1, pm->n_samples, (SegRec *)sim->seg_rec);
         }
-        a.rec = sim->seg_rec;  a.tile_list = sim->tile_list;  a.work = sim->d_work;  a.n_tiles = (int)sim->n_tiles;
+        a.rec = sim->seg_rec;  a.work = sim->d_work;  a.n_tiles = (int)sim->n_tiles;
+        a.tile_desc = sim->tile_desc_p;  a.tile_list = sim->tile_list_p;        // physical (sorted) tile order
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
         const unsigned grid = (unsigned)std::min<int64_t>(sim->n_tiles, 4 * (int64_t)sim->sm_count);
         ++g_lartpc_launches;
@@ -773,6 +774,7 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     a.B = (const __half *)sim->d_lut_tc;
     a.partial = out->partial;
     a.tile_meta = out->tile_range;
+    a.tb_mask = sim->tb_mask;
     if (sim->n_tiles >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.n_tiles = (int)sim->n_tiles;
     a.n_tb = (int)((sim->n_tiles + rtc::TB - 1) / rtc::TB);

@@ -34,7 +34,8 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
                  const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,
                  const int64_t *__restrict__ offset, const unsigned long long *__restrict__ pix_mask,
                  const int32_t *__restrict__ pix_tile0, const int32_t *__restrict__ pix_jmin,
-                 const float *__restrict__ partial, const int32_t *__restrict__ tile_range, float *samples)
+                 const float *__restrict__ partial, const int32_t *__restrict__ tile_range,
+                 const int32_t *__restrict__ tile_perm /* slot of a tile, or null: identity */, float *samples)
 {
     extern __shared__ float acc[];                                    // [length of this pixel's waveform]
     __shared__ unsigned long long s_mask[128][MASK_WORDS];
@@ -64,12 +65,13 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
         for (int wd = 0; wd < MASK_WORDS; ++wd)
             for (unsigned long long m = s_mask[d][wd]; m; m &= m - 1, ++tix) {
                 const int w = 64 * wd + __ffsll((long long)m) - 1;
-                const int2 rg = *(const int2 *)(tile_range + TILE_META * tix);      // first / last output block
+                const int slot = tile_perm ? tile_perm[tix] : tix;
+                const int2 rg = *(const int2 *)(tile_range + TILE_META * slot);     // first / last output block
                 if (rg.x > rg.y) continue;
                 const int j_start = js + w * p.Jc;
                 const int n_a = max(first, j_start + rg.x * RESP_NO);
                 const int n_b = min(last, j_start + min(rg.y * RESP_NO + RESP_NO - 1, p.tile_ticks - 1));
-                const float *row = partial + ((size_t)tix * p.WW + d) * p.tile_ticks - j_start;
+                const float *row = partial + ((size_t)slot * p.WW + d) * p.tile_ticks - j_start;
                 // first tick >= n_a owned by this thread
                 int i = n_a - first;
                 i += (tid - i) & (SUM_THREADS - 1);
@@ -109,7 +111,7 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
     sum_pixel_kernel<<<(unsigned)sim->n_active, SUM_THREADS, smem, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
                                                              out->length, out->offset, sim->pix_mask, sim->pix_tile0,
                                                              sim->pix_jmin, sig->partial, sig->tile_range,
-                                                             out->samples);
+                                                             p.tc_mode ? sim->tile_perm : nullptr, out->samples);
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }

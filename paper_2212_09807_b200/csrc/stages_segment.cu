@@ -418,6 +418,80 @@ int sim_ensure_scan_tmp(lartpc_sim *sim, int64_t elems)
     return LARTPC_OK;
 }
 
+
+// (re)allocates every per-tile planning array for `cap` tiles
+int sim_grow_tiles(lartpc_sim *sim, int64_t cap)
+{
+    cudaFree(sim->tile_cp); cudaFree(sim->tile_desc); cudaFree(sim->tile_list); cudaFree(sim->tile_perm);
+    cudaFree(sim->tile_desc_p); cudaFree(sim->tile_list_p); cudaFree(sim->tb_mask);
+    sim->tile_cp = nullptr; sim->tile_desc = nullptr; sim->tile_list = nullptr; sim->tile_perm = nullptr;
+    sim->tile_desc_p = nullptr; sim->tile_list_p = nullptr; sim->tb_mask = nullptr; sim->tile_cap = 0;
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_cp, sizeof(int32_t) * cap));
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc, sizeof(TileDesc) * cap));
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list, sizeof(int2) * cap));
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_perm, sizeof(int32_t) * cap));
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc_p, sizeof(TileDesc) * cap));
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list_p, sizeof(int2) * cap));
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->tb_mask, sizeof(int32_t) * (cap / TC_TILE_BLOCK + 2)));
+    if (!sim->cls_hist) LARTPC_CUDA_TRY(cudaMalloc(&sim->cls_hist, sizeof(int32_t) * 32));
+    sim->tile_cap = cap;
+    return LARTPC_OK;
+}
+
+// ---- tensor-core mode: tiles sorted by the 16-tick arrival blocks they charge ------------------------------------
+// The response multiplies 128 tiles at a time and can skip a 16-tick block only when none of the 128 charges it, so
+// tiles with the same block mask are given neighbouring slots (counting sort over the 16 masks; the order inside a class
+// is whatever the atomics give: a tile's slot only decides where its rows live, never a sum).
+__global__ void __launch_bounds__(256)
+tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td, const int2 *__restrict__ tl,
+                  const int32_t *__restrict__ pair_seg, const int32_t *__restrict__ jt0, const int32_t *__restrict__ jt1,
+                  int32_t *cls, int32_t *hist, int sort)
+{
+    __shared__ int s_hist[16];
+    if (threadIdx.x < 16) s_hist[threadIdx.x] = 0;
+    __syncthreads();
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n_tiles) {
+        int mask = 0;
+        if (!sort) mask = 15;
+        else {
+            const TileDesc d = td[t];
+            const int2 l = tl[t];
+            for (int k = 0; k < l.y; ++k) {
+                const int s = pair_seg[l.x + k];
+                const int jlo = max(max(jt0[s], 0) - d.j_start, 0), jhi = min(min(jt1[s], p.j_max) - d.j_start, p.Jc - 1);
+                if (jlo <= jhi) mask |= ((2 << (jhi >> 4)) - 1) & ~((1 << (jlo >> 4)) - 1);
+            }
+        }
+        cls[t] = mask;
+        atomicAdd(&s_hist[mask], 1);
+    }
+    __syncthreads();
+    if (threadIdx.x < 16 && s_hist[threadIdx.x]) atomicAdd(&hist[threadIdx.x], s_hist[threadIdx.x]);
+}
+
+__global__ void class_offsets_kernel(int32_t *hist)                 // [0..15] counts -> [16..31] first slot of the class
+{
+    if (threadIdx.x == 0) {
+        int run = 0;
+        for (int k = 0; k < 16; ++k) { hist[16 + k] = run; run += hist[k]; }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+tile_scatter_kernel(int64_t n_tiles, int32_t *perm /* in: class, out: slot */, int32_t *hist, const TileDesc *__restrict__ td,
+                    const int2 *__restrict__ tl, TileDesc *td_p, int2 *tl_p, int32_t *tb_mask, int sort)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_tiles) return;
+    const int mask = perm[t];
+    const int slot = sort ? atomicAdd(&hist[16 + mask], 1) : (int)t;
+    perm[t] = slot;
+    td_p[slot] = td[t];
+    tl_p[slot] = tl[t];
+    if (mask) atomicOr(&tb_mask[slot / TC_TILE_BLOCK], mask);
+}
+
 static int grow_i32(int32_t **p, int64_t *cap, int64_t need)
 {
     if (need <= *cap) return LARTPC_OK;
@@ -497,21 +571,25 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         if (attempt == 1) return LARTPC_ERR_CAPACITY;
         // grow the plan buffers to the sizes just counted and plan again
         if ((rc = grow_i32(&sim->pair_seg, &sim->pair_cap, h[CNT_PAIRS])) != 0) return rc;
-        if (h[CNT_TILES] > sim->tile_cap) {
-            int64_t cap = sim->tile_cap;
-            if ((rc = grow_i32(&sim->tile_cp, &cap, h[CNT_TILES])) != 0) return rc;
-            if (sim->tile_desc) cudaFree(sim->tile_desc);
-            sim->tile_desc = nullptr;
-            LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc, sizeof(TileDesc) * cap));
-            if (sim->tile_list) cudaFree(sim->tile_list);
-            sim->tile_list = nullptr;
-            LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list, sizeof(int2) * cap));
-            sim->tile_cap = cap;
-        }
+        if (h[CNT_TILES] > sim->tile_cap && (rc = sim_grow_tiles(sim, h[CNT_TILES] + h[CNT_TILES] / 4 + 1024)) != 0) return rc;
     }
     const long long *h = sim->h_counters;
     sim->plan_n = n;
     sim->n_tiles = h[CNT_TILES];
+    if (p.tc_mode && sim->n_tiles > 0) {
+        const int sort = sim->tile_sort && sim->splat_tc ? 1 : 0;
+        const int64_t nt = sim->n_tiles;
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->cls_hist, 0, sizeof(int32_t) * 32, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->tb_mask, 0, sizeof(int32_t) * (nt / TC_TILE_BLOCK + 1), st));
+        g_lartpc_launches += 3;
+        tile_class_kernel<<<div_up(nt, 256), 256, 0, st>>>(p, nt, sim->tile_desc, sim->tile_list, sim->pair_seg, out->jt0,
+                                                          out->jt1, sim->tile_perm, sim->cls_hist, sort);
+        class_offsets_kernel<<<1, 32, 0, st>>>(sim->cls_hist);
+        tile_scatter_kernel<<<div_up(nt, 256), 256, 0, st>>>(nt, sim->tile_perm, sim->cls_hist, sim->tile_desc,
+                                                            sim->tile_list, sim->tile_desc_p, sim->tile_list_p,
+                                                            sim->tb_mask, sort);
+        LARTPC_CUDA_TRY(cudaGetLastError());
+    }
     sim->n_pairs = h[CNT_PAIRS];
     sim->n_active = h[CNT_ACTIVE_PIX];
     sim->total_samples = h[CNT_TOTAL_SAMPLES];
