@@ -79,7 +79,7 @@ struct lartpc_sim {
     int32_t pix_id_base = 0;
     // dense planning arrays
     int32_t *pix_count = nullptr, *pix_start = nullptr, *pix_tile0 = nullptr, *pix_cursor = nullptr;
-    int32_t *pix_jmin = nullptr;         // first arrival tick on the charged pixel (window origin, rounded down to even)
+    int32_t *pix_jmin = nullptr;         // first arrival tick on the charged pixel (window origin = this rounded down to a multiple of 4)
     unsigned long long *pix_mask = nullptr;   // [n_cp][MASK_WORDS] windows that hold charge
     int32_t *act_first = nullptr, *act_last = nullptr, *act_slot = nullptr;
     // growable planning arrays

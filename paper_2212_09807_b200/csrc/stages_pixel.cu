@@ -24,11 +24,14 @@ active_table_kernel(int64_t n_pix, const int32_t *__restrict__ act_first, const 
 struct LenF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
 
 constexpr int SUM_THREADS = 128;
+constexpr int SUM_LCAP = 192;      // partial rows listed per round (a pixel usually has W*W x 1.3 of them)
 
-// CTA = active pixel.  Its waveform is accumulated in shared memory, tile by tile: for every target index d of the
-// W x W window (ascending) and every charge window of that charged pixel (ascending) the partial row of the tile is
-// streamed once, coalesced, over the ticks it can be non-zero on.  A thread always owns the same ticks (i = tid mod
-// 128), so there is no race, no barrier between tiles, and the order of the float32 additions is fixed.
+// CTA = active pixel.  Threads d < W*W first list, in parallel, the partial rows that reach the pixel: for target index d
+// of the W x W window and every charge window of that charged pixel, the row of the tile (through the slot map) and the
+// ticks it can be non-zero on.  Then a thread owns the ticks i = tid mod 128 of the waveform and adds the listed rows in
+// list order (d ascending, window ascending): the loads of one tick are independent of each other, the row reads of a
+// warp are coalesced, and the order of the float32 additions -- hence every output bit -- is fixed.
+template <int VEC>                 // ticks per thread and load: 4 when tile_ticks is a multiple of 4 (rows 16-byte aligned), else 2
 __global__ void __launch_bounds__(SUM_THREADS)
 sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__restrict__ pixel_id,
                  const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,
@@ -37,50 +40,85 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
                  const float *__restrict__ partial, const int32_t *__restrict__ tile_range,
                  const int32_t *__restrict__ tile_perm /* slot of a tile, or null: identity */, float *samples)
 {
-    extern __shared__ float acc[];                                    // [length of this pixel's waveform]
     __shared__ unsigned long long s_mask[128][MASK_WORDS];
-    __shared__ int s_tile0[128], s_js[128];
+    __shared__ int s_tile0[128], s_js[128], s_base[129];
+    __shared__ const float *e_row[SUM_LCAP];
+    __shared__ int e_na[SUM_LCAP], e_nb[SUM_LCAP];
     const int slot = blockIdx.x, tid = threadIdx.x;
     const int gp = pixel_id[slot];
     int tpc = 0;
     while (tpc + 1 < p.n_tpcs && tpcs[tpc + 1].first_pixel_id <= gp) ++tpc;
     const DevTpc &t = tpcs[tpc];
     const int rel = gp - t.first_pixel_id, iy = rel / t.nx, ix = rel - iy * t.nx;
-    for (int d = tid; d < p.WW; d += SUM_THREADS) {
-        const int dyi = d / p.W, dxi = d - dyi * p.W;
+    const int first = first_tick[slot], len = length[slot], last = first + len - 1;
+    if (tid < p.WW) {
+        const int d = tid, dyi = d / p.W, dxi = d - dyi * p.W;
         const int cp = t.cp_base + (iy + dyi) * t.gw + (ix + dxi);   // charged pixel px = ix - H + dxi
+        int cnt = 0;
 #pragma unroll
-        for (int wd = 0; wd < MASK_WORDS; ++wd) s_mask[d][wd] = pix_mask[(size_t)cp * MASK_WORDS + wd];
+        for (int wd = 0; wd < MASK_WORDS; ++wd) {
+            s_mask[d][wd] = pix_mask[(size_t)cp * MASK_WORDS + wd];
+            cnt += __popcll(s_mask[d][wd]);
+        }
         s_tile0[d] = pix_tile0[cp];
-        s_js[d] = pix_jmin[cp] & ~1;                                 // window origin of that charged pixel
-    }
-    const int first = first_tick[slot], len = length[slot];
-    for (int i = tid; i < len; i += SUM_THREADS) acc[i] = 0.f;
-    __syncthreads();
-    const int last = first + len - 1;
-    for (int d = 0; d < p.WW; ++d) {
-        int tix = s_tile0[d];
-        const int js = s_js[d];
-#pragma unroll
-        for (int wd = 0; wd < MASK_WORDS; ++wd)
-            for (unsigned long long m = s_mask[d][wd]; m; m &= m - 1, ++tix) {
-                const int w = 64 * wd + __ffsll((long long)m) - 1;
-                const int slot = tile_perm ? tile_perm[tix] : tix;
-                const int2 rg = *(const int2 *)(tile_range + TILE_META * slot);     // first / last output block
-                if (rg.x > rg.y) continue;
-                const int j_start = js + w * p.Jc;
-                const int n_a = max(first, j_start + rg.x * RESP_NO);
-                const int n_b = min(last, j_start + min(rg.y * RESP_NO + RESP_NO - 1, p.tile_ticks - 1));
-                const float *row = partial + ((size_t)slot * p.WW + d) * p.tile_ticks - j_start;
-                // first tick >= n_a owned by this thread
-                int i = n_a - first;
-                i += (tid - i) & (SUM_THREADS - 1);
-                for (; first + i <= n_b; i += SUM_THREADS) acc[i] += __ldcs(row + first + i);
-            }
+        s_js[d] = pix_jmin[cp] & ~3;                                 // window origin of that charged pixel
+        s_base[d + 1] = cnt;
     }
     __syncthreads();
+    if (tid == 0) {
+        s_base[0] = 0;
+        for (int d = 0; d < p.WW; ++d) s_base[d + 1] += s_base[d];
+    }
+    __syncthreads();
+    const int total = s_base[p.WW];
     const int64_t off = offset[slot];
-    for (int i = tid; i < len; i += SUM_THREADS) samples[off + i] = acc[i];
+    for (int r0 = 0; r0 < total; r0 += SUM_LCAP) {
+        if (tid < p.WW) {
+            const int d = tid, js = s_js[d];
+            int tix = s_tile0[d], gi = s_base[d] - r0;
+#pragma unroll
+            for (int wd = 0; wd < MASK_WORDS; ++wd)
+                for (unsigned long long m = s_mask[d][wd]; m; m &= m - 1, ++tix, ++gi) {
+                    if (gi < 0 || gi >= SUM_LCAP) continue;
+                    const int w = 64 * wd + __ffsll((long long)m) - 1;
+                    const int ts = tile_perm ? tile_perm[tix] : tix;
+                    const int2 rg = *(const int2 *)(tile_range + TILE_META * ts);       // first / last output block
+                    const int j_start = js + w * p.Jc;
+                    e_row[gi] = partial + ((size_t)ts * p.WW + d) * p.tile_ticks - j_start;
+                    e_na[gi] = rg.x > rg.y ? INT_MAX : max(first, j_start + rg.x * RESP_NO);
+                    e_nb[gi] = rg.x > rg.y ? -1 : min(last, j_start + min(rg.y * RESP_NO + RESP_NO - 1, p.tile_ticks - 1));
+                }
+        }
+        __syncthreads();
+        const int ne = min(SUM_LCAP, total - r0);
+        // a thread owns VEC consecutive ticks starting at a multiple of VEC: window origins are multiples of 4, so that is
+        // one aligned load of a row
+        const int n_al0 = first & ~(VEC - 1);
+        for (int iv = tid; VEC * iv < last - n_al0 + 1; iv += SUM_THREADS) {
+            const int n = n_al0 + VEC * iv;
+            float a[VEC];
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) a[k] = (r0 && n + k >= first && n + k <= last) ? samples[off + (n + k - first)] : 0.f;
+#pragma unroll 8
+            for (int e = 0; e < ne; ++e) {
+                const int na = e_na[e], nb = e_nb[e];
+                if (n + VEC - 1 >= na && n <= nb) {
+                    float v[VEC];
+                    if (VEC == 4) { const float4 q = __ldcs((const float4 *)(e_row[e] + n)); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
+                    else { const float2 q = __ldcs((const float2 *)(e_row[e] + n)); v[0] = q.x; v[1] = q.y; }
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k)
+                        if (n + k >= na && n + k <= nb) a[k] += v[k];
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < VEC; ++k)
+                if (n + k >= first && n + k <= last) samples[off + (n + k - first)] = a[k];
+        }
+        __syncthreads();
+    }
+    if (total == 0)
+        for (int i = tid; i < len; i += SUM_THREADS) samples[off + i] = 0.f;
 }
 
 int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out, cudaStream_t st)
@@ -102,13 +140,13 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
     LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_active, LenF{out->length}, out->offset, true, (long long *)nullptr,
                                           sim->scan_tmp, st));
     ++g_lartpc_launches;
-    const size_t smem = sizeof(float) * (size_t)p.n_ticks;             // a waveform is at most the readout window
-    static size_t configured = 0;
-    if (smem > 40 * 1024 && smem > configured) {
-        LARTPC_CUDA_TRY(cudaFuncSetAttribute(sum_pixel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
-    sum_pixel_kernel<<<(unsigned)sim->n_active, SUM_THREADS, smem, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
+    if (p.tile_ticks % 4 == 0)
+        sum_pixel_kernel<4><<<(unsigned)sim->n_active, SUM_THREADS, 0, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
+                                                             out->length, out->offset, sim->pix_mask, sim->pix_tile0,
+                                                             sim->pix_jmin, sig->partial, sig->tile_range,
+                                                             p.tc_mode ? sim->tile_perm : nullptr, out->samples);
+    else
+        sum_pixel_kernel<2><<<(unsigned)sim->n_active, SUM_THREADS, 0, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
                                                              out->length, out->offset, sim->pix_mask, sim->pix_tile0,
                                                              sim->pix_jmin, sig->partial, sig->tile_range,
                                                              p.tc_mode ? sim->tile_perm : nullptr, out->samples);

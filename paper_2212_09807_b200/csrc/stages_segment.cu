@@ -272,8 +272,9 @@ pair_fill_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n, const 
             int64_t slot = (int64_t)pix_start[cp] + atomicAdd(&pix_cursor[cp], 1);
             if (slot < pair_cap) pair_seg[slot] = (int32_t)i;
             else atomicAdd((unsigned long long *)&counters[CNT_OVERFLOW], 1ull);
-            // windows of Jc arrival ticks counted from the pixel's first tick (rounded down to even)
-            const int js = pix_jmin[cp] & ~1;
+            // windows of Jc arrival ticks counted from the pixel's first tick (rounded down to a multiple of 4: S5 reads
+            // the partial rows with aligned 16-byte loads)
+            const int js = pix_jmin[cp] & ~3;
             const int w0 = min((b.j0 - js) / p.Jc, MAX_WINDOWS - 1), w1 = min((b.j1 - js) / p.Jc, MAX_WINDOWS - 1);
             for (int wd = w0 >> 6; wd <= (w1 >> 6); ++wd) {
                 const int lo = max(w0 - 64 * wd, 0), hi = min(w1 - 64 * wd, 63);
@@ -357,7 +358,7 @@ tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n_cp, con
     int rel = (int)(cp - t.cp_base);
     int px = rel % t.gw - p.H, py = rel / t.gw - p.H;
     int64_t tix = pix_tile0[cp];
-    const int js = pix_jmin[cp] & ~1;
+    const int js = pix_jmin[cp] & ~3;
     int w_lo = -1, w_hi = -1;
 #pragma unroll
     for (int wd = 0; wd < MASK_WORDS; ++wd)
