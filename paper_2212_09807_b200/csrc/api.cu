@@ -487,7 +487,9 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
 
     // batches of consecutive TPCs; a batch whose tiles / waveforms do not fit the workspace is halved
     int tpc_lo = 0;
-    int batch = p.n_tpcs;
+    // batch size that fitted this workspace last time (a sizing hint like the plan buffers' capacities: a wrong hint only
+    // costs a halving or leaves memory unused, never changes a result)
+    int batch = (sim->batch_hint > 0 && sim->batch_hint_ws == ws_bytes) ? std::min(sim->batch_hint, p.n_tpcs) : p.n_tpcs;
     while (tpc_lo < p.n_tpcs) {
         int tpc_hi = std::min(p.n_tpcs, tpc_lo + batch);
         lartpc_pixmap_info_t info;
@@ -517,7 +519,7 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
             batch = std::max(1, (tpc_hi - tpc_lo) / 2);
             continue;
         }
-        if (tpc_lo == 0) { stt.n_active_segments = info.n_active_segments; }
+        if (tpc_lo == 0) { stt.n_active_segments = info.n_active_segments;  sim->batch_hint = batch;  sim->batch_hint_ws = ws_bytes; }
         stt.n_tiles += info.n_tiles;  stt.n_pairs += info.n_pairs;
         stt.n_active_pixels += info.n_active_pixels;  stt.total_samples += info.total_samples;
         stt.n_batches += 1;
