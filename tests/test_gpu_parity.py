@@ -247,3 +247,120 @@ def test_config4_axes_small(lartpc, window, lut_ticks, mode):
     dr, pm = _check_segment_stages(res, wl)
     _check_currents(res, wl, dr, pm, max_pixels=40)
     sim.close()
+
+
+def _sampled_hits_check(lartpc_mod, wl, res, dr, pm, per_tpc, seed, only_tpcs=None):
+    """Currents and hits of a sample of pixels per TPC (the busiest ones plus a random draw) against O4-O6."""
+    nt = wl.params["n_readout_ticks"]
+    gpu_ids = res["waveforms"]["pixel_id"][:res["n_active"]]
+    disabled = set() if wl.disabled_pixels is None else set(int(x) for x in wl.disabled_pixels)
+    dense_q = res["hits"]["q_pixel"][:res["n_active"]]
+    rng = np.random.Generator(np.random.PCG64(seed))
+    h = res["hits"]
+    n = int(h["counters"][0])
+    ghits = {}
+    for p_, t_, a_ in zip(h["hit_pixel"][:n].tolist(), h["hit_tick"][:n].tolist(), h["hit_adc"][:n].tolist()):
+        ghits.setdefault(p_, []).append((t_, a_))
+    assert not any(p_ in disabled for p_ in ghits), "a disabled pixel produced a hit"
+    n_o = n_same = 0
+    worst_q = 0.0
+    wf = res["waveforms"]
+    for ti, t in enumerate(wl.tpcs):
+        if only_tpcs is not None and ti not in only_tpcs:
+            continue
+        sel = np.nonzero((gpu_ids >= t["first_pixel_id"]) & (gpu_ids < t["first_pixel_id"] + t["nx"] * t["ny"]))[0]
+        sel = np.array([i for i in sel if int(gpu_ids[i]) not in disabled], dtype=np.int64)
+        if len(sel) == 0:
+            continue
+        if len(sel) > per_tpc:
+            top = sel[np.argsort(np.abs(dense_q[sel]))[-per_tpc // 2:]]
+            rest = rng.choice(sel, size=per_tpc // 2, replace=False)
+            sel = np.unique(np.concatenate([top, rest]))
+        rel = gpu_ids[sel] - t["first_pixel_id"]
+        waves, qp = oracle.pixel_currents(wl.params, wl.tpcs, wl.lut, dr, pm, ti, rel % t["nx"], rel // t["nx"])
+        gq = np.zeros(len(sel))
+        for k, i in enumerate(sel):
+            o, f, l = int(wf["offset"][i]), int(wf["first_tick"][i]), int(wf["length"][i])
+            g = np.zeros(nt)
+            g[f:f + l] = wf["samples"][o:o + l]
+            gq[k] = g.sum()
+            peak = np.abs(waves[k]).max()
+            assert np.all(np.abs(g - waves[k]) <= 1e-4 * peak + 0.02)
+        tol = np.maximum(1e-4 * np.abs(qp), 1.0)
+        assert np.all(np.abs(gq - qp) <= tol), (np.abs(gq - qp) / tol).max()
+        worst_q = max(worst_q, float((np.abs(gq - qp) / tol).max()))
+        hp, ht, ha, _ = oracle.electronics(wl.params, seed, gpu_ids[sel].astype(np.int32), waves)
+        for p_, t_, a_ in zip(hp.tolist(), ht.tolist(), ha.tolist()):
+            n_o += 1
+            got = ghits.get(p_, [])
+            if (t_, a_) in got:
+                n_same += 1
+            else:
+                assert any(abs(t2 - t_) <= 1 and abs(a2 - a_) <= 1 for t2, a2 in got), (p_, t_, a_, got)
+        ohits = {}
+        for p_, t_ in zip(hp.tolist(), ht.tolist()):
+            ohits[p_] = ohits.get(p_, 0) + 1
+        for i in sel:
+            assert len(ghits.get(int(gpu_ids[i]), [])) == ohits.get(int(gpu_ids[i]), 0)
+    assert n_o > 0 and n_same >= 0.999 * n_o, (n_same, n_o)
+    print("sampled pixels: worst |dQ| / tol = %.3f, %d / %d oracle hits identical" % (worst_q, n_same, n_o))
+
+
+def test_config2_sampled_full_chain(lartpc):
+    """BASELINE configs[2] at full size (1e5 segments, 8 TPCs, Birks, noise on, 7.8 % of the pixels disabled): every
+    segment-stage output, the currents and hits of a sample of pixels per TPC against the oracle, and the hit list of
+    lartpc_run_spill (TPC batches) against the staged calls."""
+    wl = W.make_config(2)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    sim.set_disabled_pixels(wl.disabled_pixels)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _sampled_hits_check(lartpc, wl, res, dr, pm, per_tpc=12, seed=wl.seed)
+    seg = sim.upload_segments(wl.segments)
+    hits, st = sim.run_spill(seg, wl.seed, hit_capacity=1 << 20)
+    n = int(res["hits"]["counters"][0])
+    assert st.n_hits == n and st.n_hits_dropped == 0
+    for a, k in zip(lartpc.hits_to_numpy(hits), ("hit_pixel", "hit_tick", "hit_adc")):
+        assert np.array_equal(a, res["hits"][k][:n])
+    sim.close()
+
+
+def test_config3_full_spill(lartpc):
+    """BASELINE configs[3] at full size, in the configuration bench.py times (lartpc_run_spill over 70 TPCs in batches).
+    The oracle cannot do 5e6 segments, so: (a) the two busiest TPCs are simulated alone through the staged calls, at
+    their full density, and a sample of their pixels is held to the oracle (currents and hits); (b) the full spill's hits
+    on those two TPCs must be the staged ones bit for bit (batching, tile sorting and the slot map change no result);
+    (c) properties of the whole list: sorted by (pixel, tick), nothing dropped, ADC within 8 bits, ticks inside the window."""
+    wl = W.make_config(3)
+    _, ne = oracle.quench(wl.params, wl.segments)
+    tpc_of = oracle.drift(wl.params, wl.tpcs, wl.segments, ne)["tpc"]
+    counts = np.bincount(tpc_of[tpc_of >= 0], minlength=len(wl.tpcs))
+    busy = [int(x) for x in np.argsort(counts)[-2:]]
+    sub = wl.subset(np.nonzero(np.isin(tpc_of, busy))[0])
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, sub)
+    dr, pm = _check_segment_stages(res, sub)
+    _sampled_hits_check(lartpc, sub, res, dr, pm, per_tpc=10, seed=wl.seed, only_tpcs=busy)
+    n_sub = int(res["hits"]["counters"][0])
+    sub_hits = [res["hits"][k][:n_sub].copy() for k in ("hit_pixel", "hit_tick", "hit_adc")]
+    del res
+    import torch
+    torch.cuda.empty_cache()
+    seg = sim.upload_segments(wl.segments)
+    hits, st = sim.run_spill(seg, wl.seed, hit_capacity=int(8 * wl.n_segments))
+    assert st.n_hits > 0 and st.n_hits_dropped == 0 and st.n_batches >= 1
+    # pixels with more than max_hits_per_pixel hits are counted, never silent (D18): a handful in the shower cores
+    assert st.n_pixels_overflow <= 1e-4 * st.n_active_pixels and st.n_hits_total - st.n_hits >= st.n_pixels_overflow
+    hp, ht, ha = lartpc.hits_to_numpy(hits)
+    key = hp.astype(np.int64) * (1 << 20) + ht
+    assert np.all(np.diff(key) > 0)
+    assert ha.min() >= 0 and ha.max() <= 255 and ht.min() >= 0 and ht.max() < wl.params["n_readout_ticks"]
+    in_busy = np.zeros(len(hp), dtype=bool)
+    for ti in busy:
+        t = wl.tpcs[ti]
+        in_busy |= (hp >= t["first_pixel_id"]) & (hp < t["first_pixel_id"] + t["nx"] * t["ny"])
+    assert in_busy.sum() == n_sub
+    assert np.array_equal(hp[in_busy], sub_hits[0]) and np.array_equal(ht[in_busy], sub_hits[1]) and np.array_equal(ha[in_busy], sub_hits[2])
+    print("config 3: %d segments, %d tiles, %d hits; TPCs %s alone: %d hits, identical inside the full spill"
+          % (wl.n_segments, st.n_tiles, st.n_hits, busy, n_sub))
+    sim.close()
