@@ -238,6 +238,82 @@ electronics_kernel(DevParams p, unsigned long long seed, int64_t n_active, const
     q_pixel[slot] = (float)qsum;
 }
 
+// Warp per active pixel, for parameter sets whose state can only change on the pixel's own support (no discriminator
+// noise, no periodic reset: every BASELINE config).  Same state machine as electronics_kernel, but the charge
+// integral runs 32 ticks at a time: lane l holds tick n + l, an inclusive warp scan in float64 gives q after every tick of
+// the chunk, the first threshold crossing is a ballot, and the sample / reset 16 ticks later restarts the chunk behind it.
+// The loads are coalesced and the serial depth is (support / 32 + 2 per hit) steps instead of one step per tick.
+__global__ void __launch_bounds__(128)
+electronics_warp_kernel(DevParams p, unsigned long long seed, int64_t n_active, const int32_t *__restrict__ pixel_id,
+                        const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,
+                        const int64_t *__restrict__ offset, const float *__restrict__ samples,
+                        const uint32_t *__restrict__ disabled, int32_t *slots, int32_t *hits_per_pixel, float *q_pixel)
+{
+    const int64_t slot = (int64_t)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5);
+    if (slot >= n_active) return;
+    const int lane = threadIdx.x & 31;
+    const int pid = pixel_id[slot];
+    const int first = first_tick[slot], len = length[slot];
+    const float *w = samples + offset[slot];
+    const bool any_noise = p.noise_uncorr != 0.0 || p.noise_reset != 0.0;
+    const bool off_channel = disabled && ((disabled[pid >> 5] >> (pid & 31)) & 1u);
+    // Q_p = sum of the waveform
+    double qsum = 0.0;
+    for (int i = lane; i < len; i += 32) qsum += (double)w[i];
+    for (int d = 16; d; d >>= 1) qsum += __shfl_xor_sync(0xffffffffu, qsum, d);
+    const int n_end = first + len;                                    // exclusive end of the support
+    double q = 0.0;
+    bool armed = true;
+    int n_c = 0, nhits = 0;
+    long long rearm_at = 0;
+    int32_t *my = slots + slot * p.max_hits;
+    int n = first;
+    while (n < p.n_ticks) {
+        if (n >= n_end && armed && q < p.threshold) break;            // nothing can happen any more
+        const int i = n + lane - first;
+        const double cur = (i >= 0 && i < len && n + lane < p.n_ticks) ? (double)w[i] : 0.0;
+        double pref = cur;                                            // q after tick n + lane, minus q before the chunk
+        for (int d = 1; d < 32; d <<= 1) {
+            const double o = __shfl_up_sync(0xffffffffu, pref, d);
+            if (lane >= d) pref += o;
+        }
+        pref += q;
+        if (armed) {
+            const unsigned hit = __ballot_sync(0xffffffffu, (long long)n + lane >= rearm_at && pref >= p.threshold &&
+                                                               n + lane < p.n_ticks);
+            if (hit) { armed = false; n_c = n + __ffs(hit) - 1; }
+        }
+        if (!armed) {
+            const int ns = n_c + p.hold;                              // digitisation tick (D14)
+            if (ns >= p.n_ticks) break;                               // the sample falls past the window: no hit
+            if (ns <= n + 31) {
+                const double q_at = __shfl_sync(0xffffffffu, pref, ns - n);
+                double z[3] = {0.0, 0.0, 0.0};
+                if (any_noise) noise_normals(seed, (uint32_t)pid, (uint32_t)ns, z);
+                const double q_s = q_at + p.noise_uncorr * z[1];
+                const double V = p.v_ped + p.gain_mv_per_ke * q_s / 1000.0;
+                double a = floor((V - p.v_cm) / (p.v_ref - p.v_cm) * p.adc_full);
+                a = fmin(fmax(a, 0.0), p.adc_full - 1.0);
+                if (!off_channel) {
+                    if (nhits < p.max_hits && lane == 0) my[nhits] = (ns << ADC_SHIFT) | (int)a;
+                    ++nhits;
+                }
+                q = p.noise_reset * z[2];
+                armed = true;
+                rearm_at = max((long long)ns + 1, (long long)ns + p.min_spacing - p.hold);
+                n = ns + 1;                                           // the ticks behind the sample start from the new q
+                continue;
+            }
+        }
+        q = __shfl_sync(0xffffffffu, pref, 31);
+        n += 32;
+    }
+    if (lane == 0) {
+        hits_per_pixel[slot] = nhits;
+        q_pixel[slot] = (float)qsum;
+    }
+}
+
 struct HitCountF {
     const int32_t *v; int cap;
     __device__ long long operator()(int64_t i) const { return v[i] < cap ? v[i] : cap; }
@@ -283,9 +359,14 @@ int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t s
     const int64_t na = wf->n_active;
     if (na == 0) return LARTPC_OK;
     ++g_lartpc_launches;
-    electronics_kernel<<<div_up(na, 128), 128, 0, st>>>(p, seed, na, wf->pixel_id, wf->first_tick, wf->length,
-                                                       wf->offset, wf->samples, sim->disabled_mask, slot_scratch,
-                                                       out->hits_per_pixel, out->q_pixel);
+    if (p.noise_disc != 0.0 || p.periodic > 0 || p.hold < 0)
+        electronics_kernel<<<div_up(na, 128), 128, 0, st>>>(p, seed, na, wf->pixel_id, wf->first_tick, wf->length,
+                                                           wf->offset, wf->samples, sim->disabled_mask, slot_scratch,
+                                                           out->hits_per_pixel, out->q_pixel);
+    else
+        electronics_warp_kernel<<<div_up(na, 4), 128, 0, st>>>(p, seed, na, wf->pixel_id, wf->first_tick, wf->length,
+                                                              wf->offset, wf->samples, sim->disabled_mask, slot_scratch,
+                                                              out->hits_per_pixel, out->q_pixel);
     int rc = sim_ensure_scan_tmp(sim, na);
     if (rc) return rc;
     long long *batch_total = sim->d_counters + CNT_COUNT - 1;

@@ -364,3 +364,23 @@ def test_config3_full_spill(lartpc):
     print("config 3: %d segments, %d tiles, %d hits; TPCs %s alone: %d hits, identical inside the full spill"
           % (wl.n_segments, st.n_tiles, st.n_hits, busy, n_sub))
     sim.close()
+
+
+@pytest.mark.parametrize("variant", ["disc_noise", "periodic_reset", "low_threshold"])
+def test_electronics_variants(lartpc, variant):
+    """SURVEY 8(f) NEXT-4 options of S6: discriminator noise 650 e- (drawn every tick, so the
+    per-tick kernel runs instead of the warp-scan one), the periodic reset, and the low-threshold regime."""
+    over = dict(noise_reset_e=900.0, noise_uncorr_e=500.0)
+    if variant == "disc_noise":
+        over.update(noise_disc_e=650.0)
+    elif variant == "periodic_reset":
+        over.update(periodic_reset_ticks=97)
+    else:
+        over.update(threshold_e=3000.0, min_spacing_ticks=11)
+    wl = W.make_config(0, seed=11)
+    wl.params.update(over)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_hits(res, wl, dr, pm, wl.seed)
+    sim.close()
