@@ -206,7 +206,9 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
 
     std::vector<DevTpc> dt(n_tpcs);
     int64_t cp = 0, pix = 0;
+    s->cp_base_h.assign(n_tpcs + 1, 0);  s->pix_base_h.assign(n_tpcs + 1, 0);
     for (int k = 0; k < n_tpcs; ++k) {
+        s->cp_base_h[k] = cp;  s->pix_base_h[k] = pix;
         const lartpc_tpc_t &t = tpcs[k];
         if (t.nx < 1 || t.ny < 1 || (t.drift_sign != 1 && t.drift_sign != -1) || t.drift_len < 0 ||
             t.first_pixel_id != pix) {                                      // pixel ids must be dense, in table order
@@ -223,6 +225,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     }
     if (cp >= INT32_MAX || pix >= INT32_MAX) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
     s->n_cp = cp; s->n_pix = pix;
+    s->cp_base_h[n_tpcs] = cp;  s->pix_base_h[n_tpcs] = pix;
 
     // LUT re-laid out as [bin c = cb*nb+ca][pair q][RS][2]: pair q interleaves the rows of targets d = 2q and 2q+1
     // (d = dyi*W + dxi; row (c, d) is R[cy = nb*dyi + cb][cx = nb*dxi + ca][.]), LUT tick k at pair-word LUT_OFF + k

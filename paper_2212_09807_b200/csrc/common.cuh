@@ -90,6 +90,8 @@ struct lartpc_sim {
     // lists in slot order, per 128-slot block the OR of its tiles' block masks
     int32_t *tile_perm = nullptr;  TileDesc *tile_desc_p = nullptr;  int2 *tile_list_p = nullptr;
     int32_t *tb_mask = nullptr;  int32_t *cls_hist = nullptr;   // [tile_cap / 128 + 2], [32]: class counts then cursors
+    std::vector<int64_t> cp_base_h, pix_base_h;   // [n_tpcs + 1] first charged-pixel cell / first pixel of each TPC (host copy)
+    int64_t plan_pix_lo = 0, plan_pix_hi = 0;       // pixel range of the TPCs the current plan covers
     int batch_hint = 0;  size_t batch_hint_ws = 0;   // lartpc_run_spill: TPCs per batch that fitted the workspace last time
     bool tile_sort = true;               // env LARTPC_TILE_SORT=0: identity order, every block kept (measurement aid)
     void *seg_rec = nullptr;  int64_t seg_rec_cap = 0;   // per-segment records of the tensor-core splat (charge_tc.cuh)

@@ -8,11 +8,11 @@
 // order (target index ascending, chunk ascending), so the sum is reproducible bit for bit.
 // -------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-active_table_kernel(int64_t n_pix, const int32_t *__restrict__ act_first, const int32_t *__restrict__ act_last,
+active_table_kernel(int64_t pix0, int64_t n_pix, const int32_t *__restrict__ act_first, const int32_t *__restrict__ act_last,
                     const int32_t *__restrict__ act_slot, int32_t *pixel_id, int32_t *first_tick, int32_t *length)
 {
-    int64_t gp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gp >= n_pix) return;
+    int64_t gp = pix0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;    // pixels of the planned TPCs
+    if (gp >= pix0 + n_pix) return;
     int last = act_last[gp];
     if (last < 0) return;
     int slot = act_slot[gp];
@@ -132,7 +132,8 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
     }
     if (p.WW > 128) return LARTPC_ERR_UNSUPPORTED;
     ++g_lartpc_launches;
-    active_table_kernel<<<div_up(sim->n_pix, 256), 256, 0, st>>>(sim->n_pix, sim->act_first, sim->act_last,
+    active_table_kernel<<<div_up(sim->plan_pix_hi - sim->plan_pix_lo, 256), 256, 0, st>>>(
+        sim->plan_pix_lo, sim->plan_pix_hi - sim->plan_pix_lo, sim->act_first, sim->act_last,
                                                                 sim->act_slot, out->pixel_id, out->first_tick,
                                                                 out->length);
     int rc = sim_ensure_scan_tmp(sim, sim->n_active);

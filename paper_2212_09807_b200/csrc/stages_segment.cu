@@ -339,14 +339,14 @@ pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int3
 // one thread per charged-pixel grid cell: emit its tiles (one per window that holds charge) and mark the pixels
 // they can reach
 __global__ void __launch_bounds__(256)
-tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n_cp, const int32_t *__restrict__ pix_tile0,
+tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t cp0, int64_t n_cp, const int32_t *__restrict__ pix_tile0,
                  const unsigned long long *__restrict__ pix_mask, const int32_t *__restrict__ pix_jmin,
                  const int32_t *__restrict__ pix_start, const int32_t *__restrict__ pix_count,
                  int32_t *tile_cp, TileDesc *tile_desc, int2 *tile_list, int64_t tile_cap, int32_t *act_first, int32_t *act_last,
                  long long *counters)
 {
-    int64_t cp = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (cp >= n_cp) return;
+    int64_t cp = cp0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // cells [cp0, cp0 + n_cp) of the planned TPCs
+    if (cp >= cp0 + n_cp) return;
     unsigned long long mask[MASK_WORDS];
     bool any = false;
 #pragma unroll
@@ -515,17 +515,22 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
     if ((rc = sim_ensure_scan_tmp(sim, sim->n_cp > n ? sim->n_cp : (n > sim->n_pix ? n : sim->n_pix))) != 0) return rc;
     sim->have_plan = false;
     sim->have_signals = false;
+    if (tpc_lo < 0 || tpc_hi > p.n_tpcs || tpc_lo > tpc_hi) return LARTPC_ERR_BAD_ARGUMENT;
+    const int64_t cp_lo = sim->cp_base_h[tpc_lo], ncp = sim->cp_base_h[tpc_hi] - cp_lo;
+    const int64_t pix_lo = sim->pix_base_h[tpc_lo], npix = sim->pix_base_h[tpc_hi] - pix_lo;
+    sim->plan_pix_lo = pix_lo;  sim->plan_pix_hi = pix_lo + npix;
 
     for (int attempt = 0; attempt < 2; ++attempt) {
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_counters, 0, sizeof(long long) * CNT_COUNT, st));
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_count, 0, sizeof(int32_t) * sim->n_cp, st));
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_cursor, 0, sizeof(int32_t) * sim->n_cp, st));
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_mask, 0, sizeof(unsigned long long) * MASK_WORDS * sim->n_cp, st));
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->act_last, 0xff, sizeof(int32_t) * sim->n_pix, st));
+        // only the cells and pixels of the planned TPCs are touched (lartpc_run_spill plans a few TPCs at a time)
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_count + cp_lo, 0, sizeof(int32_t) * ncp, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_cursor + cp_lo, 0, sizeof(int32_t) * ncp, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_mask + cp_lo * MASK_WORDS, 0, sizeof(unsigned long long) * MASK_WORDS * ncp, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->act_last + pix_lo, 0xff, sizeof(int32_t) * npix, st));
         ++g_lartpc_launches;
-        fill_i32_kernel<<<div_up(sim->n_pix, 256), 256, 0, st>>>(sim->act_first, sim->n_pix, INT32_MAX);
+        fill_i32_kernel<<<div_up(npix, 256), 256, 0, st>>>(sim->act_first + pix_lo, npix, INT32_MAX);
         ++g_lartpc_launches;
-        fill_i32_kernel<<<div_up(sim->n_cp, 256), 256, 0, st>>>(sim->pix_jmin, sim->n_cp, INT32_MAX);
+        fill_i32_kernel<<<div_up(ncp, 256), 256, 0, st>>>(sim->pix_jmin + cp_lo, ncp, INT32_MAX);
         if (n > 0) {
             ++g_lartpc_launches;
             pixmap_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, s, n, dr->tpc, dr->q_anode, tpc_lo, tpc_hi,
@@ -536,7 +541,7 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         LARTPC_CUDA_TRY(lscan::exclusive_scan(n, NpixF{out->npix}, out->offsets, true,
                                               sim->d_counters + CNT_TOTAL_NPIX, sim->scan_tmp, st));
         // per charged pixel: start of its segment list
-        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_cp, NpixF{sim->pix_count}, sim->pix_start, false,
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(ncp, NpixF{sim->pix_count + cp_lo}, sim->pix_start + cp_lo, false,
                                               (long long *)nullptr, sim->scan_tmp, st));
         if (n > 0) {
             ++g_lartpc_launches;
@@ -545,23 +550,23 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
                                                             sim->pix_mask, sim->pair_seg, sim->pair_cap,
                                                             sim->d_counters);
             ++g_lartpc_launches;
-            pair_sort_kernel<<<div_up(sim->n_cp, 4), 128, 0, st>>>(sim->n_cp, sim->pix_start, sim->pix_count,
+            pair_sort_kernel<<<div_up(ncp, 4), 128, 0, st>>>(ncp, sim->pix_start + cp_lo, sim->pix_count + cp_lo,
                                                                   sim->pair_seg, sim->pair_cap);
         }
         // index of the first tile of every charged pixel (one tile per window that holds charge)
-        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_cp, PopcF{sim->pix_mask}, sim->pix_tile0, false,
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(ncp, PopcF{sim->pix_mask + cp_lo * MASK_WORDS}, sim->pix_tile0 + cp_lo, false,
                                               sim->d_counters + CNT_TILES, sim->scan_tmp, st));
         ++g_lartpc_launches;
-        tile_emit_kernel<<<div_up(sim->n_cp, 256), 256, 0, st>>>(p, sim->d_tpcs, sim->n_cp, sim->pix_tile0,
+        tile_emit_kernel<<<div_up(ncp, 256), 256, 0, st>>>(p, sim->d_tpcs, cp_lo, ncp, sim->pix_tile0,
                                                                 sim->pix_mask, sim->pix_jmin, sim->pix_start,
                                                                 sim->pix_count, sim->tile_cp, sim->tile_desc,
                                                                 sim->tile_list, sim->tile_cap, sim->act_first,
                                                                 sim->act_last, sim->d_counters);
         LARTPC_CUDA_TRY(cudaGetLastError());
         // active pixels: slot = rank among active pixels (sorted by id), total waveform samples
-        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_pix, ActiveF{sim->act_last}, sim->act_slot, false,
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(npix, ActiveF{sim->act_last + pix_lo}, sim->act_slot + pix_lo, false,
                                               sim->d_counters + CNT_ACTIVE_PIX, sim->scan_tmp, st));
-        LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_pix, ActiveLenF{sim->act_first, sim->act_last},
+        LARTPC_CUDA_TRY(lscan::exclusive_scan(npix, ActiveLenF{sim->act_first + pix_lo, sim->act_last + pix_lo},
                                               (long long *)nullptr, false, sim->d_counters + CNT_TOTAL_SAMPLES,
                                               sim->scan_tmp, st));
         LARTPC_CUDA_TRY(cudaMemcpyAsync(sim->h_counters, sim->d_counters, sizeof(long long) * CNT_COUNT,

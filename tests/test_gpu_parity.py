@@ -221,6 +221,9 @@ def test_short_drift_all_node_rules(lartpc):
         parts.append(W.line_segments([3.1 * pitch, y, z], [6.3 * pitch, y + 0.013, z], step, 0.0, W._mip(2.1)))        # along x
         parts.append(W.line_segments([9.4 * pitch, y, z], [9.4 * pitch + 0.01, y + 0.02, z + 0.6], step, 0.0, W._mip(2.1)))  # along the drift
         parts.append(W.line_segments([13.2 * pitch, y, z], [15.9 * pitch, y + 0.5 * pitch, z + 0.35], step, 0.0, W._mip(6.0)))  # oblique
+    # long segments (10 mm at 8 cm, 5 mm at 1 cm of drift): beyond the largest rule, they keep their own midpoints
+    parts.append(W.line_segments([2.2 * pitch, 21.3 * pitch, 8.0], [11.0 * pitch, 22.1 * pitch, 8.9], 1.0, 0.0, W._mip(2.1)))
+    parts.append(W.line_segments([14.2 * pitch, 21.6 * pitch, 1.0], [17.5 * pitch, 22.4 * pitch, 1.3], 0.5, 0.0, W._mip(2.1)))
     seg = W._concat(parts)
     wl = W.Workload("short-drift", 6, p, tpcs, seg, W.pad_response_lut(p))
     sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
