@@ -166,6 +166,19 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def reduce_over_ranks(ms: float, n_segments: int, world: int, device):
+    """Whole-job figures of a weak-scaling run (every rank simulates its own spill, no data-path collective): the time is
+    the MAX over ranks, the work the SUM of the ranks' segments."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    nseg = torch.tensor([float(n_segments)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(nseg, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(nseg.item())
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -229,12 +242,7 @@ def run_ours(args):
     launches = lartpc.kernel_launches() - launches0
     sim.set_profiling(False)
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    nseg = torch.tensor([float(n)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(nseg, op=dist.ReduceOp.SUM)
-    total_ms_max, n_all = float(t.item()), float(nseg.item())
+    total_ms_max, n_all = reduce_over_ranks(total_ms, n, world, dev)
 
     # ---- end to end through the C-ABI with host buffers ------------------------------------------
     e2e_ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
@@ -258,10 +266,7 @@ def run_ours(args):
     f1.record()
     torch.cuda.synchronize()
     flush_ms = f0.elapsed_time(f1)
-    te = torch.tensor([e2e_ev[0].elapsed_time(e2e_ev[1]) - flush_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_ms = float(te.item())
+    e2e_ms, _ = reduce_over_ranks(e2e_ev[0].elapsed_time(e2e_ev[1]) - flush_ms, n, world, dev)
 
     if rank == 0:
         n_resp = max(stage_n["induced_current_response"], 1)
