@@ -178,6 +178,35 @@ def pixel_currents(params, tpcs, lut, dr, pm, tpc_index: int, ixs, iys, threads:
     return waves, qp
 
 
+def pixel_currents_random(params, tpcs, lut, dr, pm, tpc_index: int, ixs, iys, m_perturb: int, seed: int,
+                          threads: Optional[int] = None):
+    """O4r, eq. (3.9) as printed: M = ``m_perturb`` random perturbations per sample point (Philox-keyed by
+    (seed; segment index, mu, nu)).  Returns waveforms [len(ixs)][n_readout_ticks] and Q_p."""
+    lib = _load()
+    if threads is not None:
+        os.environ["OMP_NUM_THREADS"] = str(int(threads))
+    ixs = np.ascontiguousarray(ixs, dtype=np.int32)
+    iys = np.ascontiguousarray(iys, dtype=np.int32)
+    npx, nt = ixs.shape[0], int(params["n_readout_ticks"])
+    waves, qp = np.zeros((npx, nt)), np.zeros(npx)
+    lutc = _f32(lut)
+    pp = _params(params)
+    n = dr["tpc"].shape[0]
+    lib.orc_plane_currents_random(C.byref(pp), C.c_int(tpc_index), _fp(lutc), C.c_int64(n), *_seg_args(dr, pm),
+                                  C.c_int(int(m_perturb)), C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF),
+                                  C.c_int64(npx), _ip(ixs), _ip(iys), _dp(waves), _dp(qp))
+    return waves, qp
+
+
+def perturbation_normals(seed: int, s: int, mu: int, nu: int, clamp: float):
+    """The three standard normals of perturbed point (segment s, mu, nu) (reading D25)."""
+    lib = _load()
+    z = (C.c_double * 3)()
+    lib.orc_perturbation_normals(C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF), C.c_uint32(s), C.c_uint32(mu), C.c_uint32(nu),
+                                 C.c_double(clamp), z)
+    return np.array(list(z))
+
+
 def direct_current(params, lut, dr, pm, tpc_index: int, ix: int, iy: int):
     """The literal nested sum of SURVEY.md 8(c.1) for one pixel (tiny inputs only)."""
     lib = _load()

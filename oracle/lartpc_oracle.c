@@ -17,6 +17,8 @@
  *   orc_pixmap      brute-force completeness / minimality, hand-worked rectangles
  *   orc_pixel_current  zero-diffusion point charge == LUT, charge conservation, long-track erf
  *                      closed form, per-electron Monte Carlo, direct 6-fold sum (orc_direct_current)
+ *   orc_pixel_current_random  (eq. 3.9 as printed) exact charge conservation, sigma = 0 identity with the
+ *                      expectation form, one perturbed point placed by hand, mean over seeds vs the expectation form
  *   orc_electronics hand cases, Philox4x32-10 known answer, normal moments
  */
 #include <math.h>
@@ -331,6 +333,106 @@ void orc_plane_currents(const orc_params *p, const orc_tpc *tpcs, int tpc_index,
         q_p[k] = orc_pixel_current(p, tpcs, tpc_index, lut, n, tpc, q_a, sigma_T, sigma_t,
                                    u_s, v_s, u_e, v_e, T_s, T_e, n_samples,
                                    ixs[k], iys[k], waves + (size_t)k * p->n_ticks);
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O4r  Eq. (3.9) as printed: every one of the N points of a segment is perturbed M times,
+ *   I(t) ~ Q_a/(N M) sum_mu sum_nu I_pixel(t - (z_mu + dz_mu_nu)/v_d, x_mu + dx_mu_nu, y_mu + dy_mu_nu),
+ * with (dx, dy) ~ N(0, sigma_T), dz/v_d ~ N(0, sigma_t).  Reading D25: the normals of point
+ * (segment s, mu, nu) are Box-Muller pairs of Philox4x32-10(counter = (s, mu, nu, 0x52414E44), key = seed):
+ * z1 = r01 cos, z2 = r01 sin, z3 = r23 cos, u_i = (x_i + 0.5) 2^-32, each clamped to +- n_sigma_map so that every
+ * perturbed point stays inside the rectangle and tick range O3 gives the segment.  The look-up is nearest-bin in
+ * x, y and t (D4), so a perturbed point adds Q_a/(N M) to exactly one LUT cell.  s is the index in the arrays
+ * passed in.  Same lattice-then-convolution order as orc_pixel_current.
+ * ------------------------------------------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+void orc_perturbation_normals(uint64_t seed, uint32_t s, uint32_t mu, uint32_t nu, double clamp, double z[3])
+{
+    uint32_t ctr[4] = { s, mu, nu, 0x52414E44u }, key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, x[4];
+    orc_philox4x32_10(ctr, key, x);
+    const double two_pi = 6.283185307179586476925286766559;
+    double u0 = ((double)x[0] + 0.5) * (1.0 / 4294967296.0), u1 = ((double)x[1] + 0.5) * (1.0 / 4294967296.0);
+    double u2 = ((double)x[2] + 0.5) * (1.0 / 4294967296.0), u3 = ((double)x[3] + 0.5) * (1.0 / 4294967296.0);
+    double r01 = sqrt(-2.0 * log(u0)), r23 = sqrt(-2.0 * log(u2));
+    z[0] = r01 * cos(two_pi * u1);
+    z[1] = r01 * sin(two_pi * u1);
+    z[2] = r23 * cos(two_pi * u3);
+    for (int k = 0; k < 3; ++k) { if (z[k] > clamp) z[k] = clamp; if (z[k] < -clamp) z[k] = -clamp; }
+}
+
+double orc_pixel_current_random(const orc_params *p, int tpc_index, const float *lut,
+                                int64_t n, const int32_t *tpc, const double *q_a,
+                                const double *sigma_T, const double *sigma_t,
+                                const double *u_s, const double *v_s, const double *u_e, const double *v_e,
+                                const double *T_s, const double *T_e, const int32_t *n_samples,
+                                int M, uint64_t seed, int ix, int iy, double *wave)
+{
+    const int nb = p->nb, W = p->wpix, K = p->klut, H = (W - 1) / 2, NB = W * nb;
+    const double bin = p->pitch / (double)nb;
+    const int64_t j_max = (int64_t)p->n_ticks - K;
+    const int64_t a_org = (int64_t)nb * (ix - H), b_org = (int64_t)nb * (iy - H);
+    memset(wave, 0, sizeof(double) * (size_t)p->n_ticks);
+    if (j_max < 0 || M < 1) return 0.0;
+    const size_t nj = (size_t)(j_max + 1);
+    double *G = (double *)calloc((size_t)NB * NB * nj, sizeof(double));
+    int64_t jlo_used = j_max + 1, jhi_used = -1;
+    for (int64_t s = 0; s < n; ++s) {
+        if (tpc[s] != tpc_index || !(q_a[s] > 0.0)) continue;
+        const double sT = sigma_T[s], st = sigma_t[s], reach = p->n_sigma_map * sT;
+        if (fmax(u_s[s], u_e[s]) + reach < (double)a_org * bin || fmin(u_s[s], u_e[s]) - reach > (double)(a_org + NB) * bin) continue;
+        if (fmax(v_s[s], v_e[s]) + reach < (double)b_org * bin || fmin(v_s[s], v_e[s]) - reach > (double)(b_org + NB) * bin) continue;
+        const int N = n_samples[s];
+        const double q = q_a[s] / (double)N / (double)M;          /* eq. (3.9): Q_a / (N M) per perturbed point */
+        for (int mu = 0; mu < N; ++mu) {
+            double f = ((double)mu + 0.5) / (double)N;
+            double u = u_s[s] + (u_e[s] - u_s[s]) * f;
+            double v = v_s[s] + (v_e[s] - v_s[s]) * f;
+            double T = T_s[s] + (T_e[s] - T_s[s]) * f;
+            for (int nu = 0; nu < M; ++nu) {
+                double z[3];
+                orc_perturbation_normals(seed, (uint32_t)s, (uint32_t)mu, (uint32_t)nu, p->n_sigma_map, z);
+                double uu = u + sT * z[0], vv = v + sT * z[1], TT = T + st * z[2];
+                int64_t a = (int64_t)floor(uu / bin) - a_org, b = (int64_t)floor(vv / bin) - b_org;
+                int64_t j = (int64_t)floor((TT - p->t_origin) / p->dt);
+                if (a < 0 || a >= NB || b < 0 || b >= NB || j < 0 || j > j_max) continue;
+                G[((size_t)b * NB + (size_t)a) * nj + (size_t)j] += q;
+                if (j < jlo_used) jlo_used = j;
+                if (j > jhi_used) jhi_used = j;
+            }
+        }
+    }
+    double total = 0.0;
+    if (jhi_used >= jlo_used) {
+        for (int cy = 0; cy < NB; ++cy)
+            for (int cx = 0; cx < NB; ++cx) {
+                const double *g = G + ((size_t)cy * NB + cx) * nj;
+                const float *r = lut + ((size_t)cy * NB + cx) * K;
+                for (int64_t j = jlo_used; j <= jhi_used; ++j) {
+                    double c = g[j];
+                    if (c == 0.0) continue;
+                    for (int k = 0; k < K; ++k) wave[j + k] += c * (double)r[k];
+                }
+            }
+        for (int nidx = 0; nidx < p->n_ticks; ++nidx) total += wave[nidx];
+    }
+    free(G);
+    return total;
+}
+
+void orc_plane_currents_random(const orc_params *p, int tpc_index, const float *lut,
+                               int64_t n, const int32_t *tpc, const double *q_a,
+                               const double *sigma_T, const double *sigma_t,
+                               const double *u_s, const double *v_s, const double *u_e, const double *v_e,
+                               const double *T_s, const double *T_e, const int32_t *n_samples,
+                               int M, uint64_t seed,
+                               int64_t npx, const int32_t *ixs, const int32_t *iys, double *waves, double *q_p)
+{
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < npx; ++k)
+        q_p[k] = orc_pixel_current_random(p, tpc_index, lut, n, tpc, q_a, sigma_T, sigma_t, u_s, v_s, u_e, v_e,
+                                          T_s, T_e, n_samples, M, seed, ixs[k], iys[k],
+                                          waves + (size_t)k * p->n_ticks);
 }
 
 /* The same quantity as the literal nested sum of SURVEY.md 8(c.1), one term at a time and without the

@@ -400,3 +400,83 @@ def test_electronics_noise_is_keyed_and_reproducible():
     z = oracle.noise_normals(42, 5, int(ht[0]))
     q = 400.0 * (ht[0] - 20 + 1)
     assert ha[0] == math.floor((580 + 4 * (q + 500.0 * z[1]) / 1000 - 288) / 3.953125)
+
+
+# ------------------------------------------------------------------ O4r eq. (3.9) as printed (random perturbations)
+def _random_case():
+    p, tpcs, lut = _small_setup(nx=14, ny=14, drift=12.0, n_ticks=1100)
+    pitch = p["pixel_pitch_cm"]
+    c = np.array([6.3 * pitch, 7.1 * pitch, 6.0])
+    d = np.array([0.6, 0.3, 0.74])
+    d /= np.linalg.norm(d)
+    seg = W.line_segments(c - 0.15 * d, c + 0.15 * d, 0.1, 2.0, lambda s, L, n: np.array([2.1, 6.0, 3.0]))
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    ix, iy = oracle.active_pixels(tpcs, pm, dr, 0)
+    return p, tpcs, lut, dr, pm, ix, iy
+
+
+def test_random_estimator_conserves_charge_exactly():
+    """Eq. (3.9): every perturbed point carries Q_a / (N M) into exactly one LUT cell, and every harness LUT
+    series over the centre pixel sums to one electron: the sum over pixels and ticks is sum Q_a whatever the
+    draws, for any M and seed."""
+    p, tpcs, lut, dr, pm, ix, iy = _random_case()
+    for m, seed in ((1, 3), (4, 99), (7, 2 ** 40 + 5)):
+        _, qp = oracle.pixel_currents_random(p, tpcs, lut, dr, pm, 0, ix, iy, m, seed)
+        assert qp.sum() == pytest.approx(dr["q_a"].sum(), rel=2e-6)
+
+
+def test_random_estimator_equals_expectation_without_diffusion():
+    """sigma = 0 (charge at the anode): the perturbations vanish and eq. (3.9) is the expectation form, term by term."""
+    p, tpcs, lut = _small_setup(nx=9, ny=9, drift=5.0, n_ticks=260)
+    pitch = p["pixel_pitch_cm"]
+    seg = W.line_segments([3.2 * pitch, 4.1 * pitch, 0.0], [4.9 * pitch, 4.6 * pitch, 0.0], 0.1, 0.7, W._mip(2.1))
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    assert np.all(dr["sigma_T"] == 0.0)
+    ix, iy = oracle.active_pixels(tpcs, pm, dr, 0)
+    w0, q0 = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, ix, iy)
+    w1, q1 = oracle.pixel_currents_random(p, tpcs, lut, dr, pm, 0, ix, iy, 3, 12345)
+    assert np.allclose(w1, w0, rtol=1e-12, atol=1e-9 * np.abs(w0).max())
+
+
+def test_random_estimator_one_point_by_hand():
+    """One segment with N = 1, M = 1: the single perturbed point, placed here with numpy from the Philox words
+    (counter (s, mu, nu, 'RAND'), key = seed; Box-Muller; reading D25), decides the one LUT cell that gets Q_a."""
+    p, tpcs, lut = _small_setup(nx=9, ny=9, drift=8.0, n_ticks=800)
+    pitch, nb, K = p["pixel_pitch_cm"], p["bins_per_pixel"], p["lut_ticks"]
+    x, y, z = 4.37 * pitch, 4.61 * pitch, 5.0
+    seg = _one_segment(x, y, z, x + 4e-4, y, z, 0.21, ts=0.4, te=0.4)
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    assert pm["n_samples"][0] == 1 and dr["sigma_T"][0] > 0
+    seed = 0x1234ABCD5678
+    xw = oracle.philox4x32_10((0, 0, 0, 0x52414E44), (seed & 0xFFFFFFFF, seed >> 32))
+    u = (np.array(xw, dtype=np.float64) + 0.5) / 4294967296.0
+    r01, r23 = math.sqrt(-2 * math.log(u[0])), math.sqrt(-2 * math.log(u[2]))
+    z1, z2, z3 = r01 * math.cos(2 * math.pi * u[1]), r01 * math.sin(2 * math.pi * u[1]), r23 * math.cos(2 * math.pi * u[3])
+    assert np.allclose(oracle.perturbation_normals(seed, 0, 0, 0, 5.0), [z1, z2, z3], rtol=1e-14)
+    um = 0.5 * (dr["u_s"][0] + dr["u_e"][0]) + dr["sigma_T"][0] * z1
+    vm = 0.5 * (dr["v_s"][0] + dr["v_e"][0]) + dr["sigma_T"][0] * z2
+    Tm = 0.5 * (dr["T_s"][0] + dr["T_e"][0]) + dr["sigma_t"][0] * z3
+    binw = pitch / nb
+    a, b, j = int(math.floor(um / binw)), int(math.floor(vm / binw)), int(math.floor(Tm / p["tick_us"]))
+    pix_x, pix_y = a // nb, b // nb
+    for (ix, iy) in [(pix_x, pix_y), (pix_x + 1, pix_y), (pix_x - 1, pix_y + 2)]:
+        waves, _ = oracle.pixel_currents_random(p, tpcs, lut, dr, pm, 0, [ix], [iy], 1, seed)
+        cx, cy = a - nb * (ix - 2), b - nb * (iy - 2)
+        want = np.zeros(p["n_readout_ticks"])
+        want[j:j + K] = dr["q_a"][0] * lut[cy, cx].astype(np.float64)
+        assert np.allclose(waves[0], want, rtol=1e-13, atol=1e-12)
+    # the clamp of reading D25
+    assert np.all(np.abs(oracle.perturbation_normals(seed, 0, 0, 0, 0.25)) <= 0.25)
+
+
+def test_random_estimator_is_unbiased():
+    """the M perturbations estimate the diffusion integral; their mean over independent seeds converges to
+    the expectation form (reading D1) within 5 standard errors on every pixel carrying charge."""
+    p, tpcs, lut, dr, pm, ix, iy = _random_case()
+    _, q_exp = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, ix, iy)
+    runs = np.array([oracle.pixel_currents_random(p, tpcs, lut, dr, pm, 0, ix, iy, 2, 1000 + k)[1] for k in range(24)])
+    mean, sem = runs.mean(axis=0), runs.std(axis=0, ddof=1) / math.sqrt(runs.shape[0])
+    big = np.abs(q_exp) > 1e-3 * np.abs(q_exp).max()
+    assert big.sum() >= 2
+    assert np.all(np.abs(mean - q_exp)[big] <= 5 * sem[big] + 1e-6 * np.abs(q_exp).max())
+    assert np.all(sem[big] > 0)                                   # the draws do differ from seed to seed
