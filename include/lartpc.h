@@ -213,6 +213,14 @@ int  lartpc_response_mode(const lartpc_sim_t *sim);
 /* Optional mask of disabled channels: HOST array of global pixel ids; S6 emits no hit for them. */
 int  lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *pixel_ids_host, int64_t n);
 
+/* Eq. (3.9) as printed: m > 0 makes S4 perturb each of the N sample points of a
+ * segment m times, (dx, dy) ~ N(0, sigma_T), dt ~ N(0, sigma_t), and look the LUT up at the nearest bin and tick of every
+ * perturbed point (charge Q_a / (N m) each), instead of taking the perturbation in expectation (m = 0, the default;
+ * DESIGN.md reading D1).  The normals of point (segment index s, mu, nu) are Box-Muller pairs of Philox4x32-10 with
+ * counter (s, mu, nu, 0x52414E44) and key (seed lo, seed hi), clamped to +- n_sigma_map (reading D25).  m <= 255.
+ * Tensor-core path with 5 or 10 bins per pixel only: LARTPC_ERR_UNSUPPORTED otherwise. */
+int  lartpc_set_random_perturbations(lartpc_sim_t *sim, int m, uint64_t seed);
+
 /* Arrival ticks per charge tile (window length) chosen for this LUT shape. */
 int  lartpc_chunk_ticks(const lartpc_sim_t *sim);
 

@@ -293,6 +293,17 @@ extern "C" int lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *ids,
     return LARTPC_OK;
 }
 
+extern "C" int lartpc_set_random_perturbations(lartpc_sim_t *sim, int m, uint64_t seed)
+{
+    if (!sim || m < 0 || m > 255) return LARTPC_ERR_BAD_ARGUMENT;
+    // the one-hot columns of the perturbed points exist in the tensor-core charge lattice only
+    if (m > 0 && !(sim->dp.tc_mode && sim->splat_tc && (sim->dp.nb == 10 || sim->dp.nb == 5))) return LARTPC_ERR_UNSUPPORTED;
+    sim->dp.rnd_m = m;
+    sim->dp.rnd_seed = seed;
+    sim->have_signals = false;
+    return LARTPC_OK;
+}
+
 extern "C" int lartpc_chunk_ticks(const lartpc_sim_t *sim) { return sim ? sim->dp.Jc : 0; }
 extern "C" int lartpc_response_mode(const lartpc_sim_t *sim)
 {

@@ -124,7 +124,8 @@ __device__ __forceinline__ int stage_segment(const DevParams &p, const SegRec &r
     L.inv_n4 = L.inv_n2 * L.inv_n2;
     L.rule = -1;
     int nq = r.N;
-    if (!L.zero_sigma && p.node_rules) {
+    if (p.rnd_m > 0) nq = r.N * p.rnd_m;                              // eq. (3.9) as printed: one column per perturbed point
+    else if (!L.zero_sigma && p.node_rules) {
         const float rho = r.rho;
         const int k = rho <= 3.5f ? 0 : rho <= 5.5f ? 1 : rho <= 8.f ? 2 : rho <= 12.f ? 3 : rho <= 16.f ? 4 : -1;
         if (k >= 0 && r.N >= 3 * c_quad_n[k]) { L.rule = c_quad_off[k]; nq = c_quad_n[k]; }
@@ -146,7 +147,7 @@ __device__ __forceinline__ void cp_async4(void *smem, const void *gmem)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-template <int NB>
+template <int NB, bool RND>       // RND: eq. (3.9) as printed, p.rnd_m random perturbations per sample point
 __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const SplatArgs a)
 {
     extern __shared__ unsigned char smem_dyn[];
@@ -273,26 +274,36 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                     for (int step = 16; step; step >>= 1)
                         if (li + step < nseg && pre[li + step] <= slot) li += step;
                     const SegLocal L = segs[li];
-                    const int mu = slot - pre[li];
+                    int mu = slot - pre[li], nu = 0;
+                    if (RND) { nu = mu % p.rnd_m;  mu /= p.rnd_m; }                 // column = perturbation nu of sample point mu
                     float f = ((float)mu + 0.5f) * (1.0f / (float)L.N), qw = L.q;   // position along the segment, charge
-                    if (L.rule >= 0) {
+                    if (RND) qw = L.q / (float)p.rnd_m;                            // Q_a / (N M)
+                    else if (L.rule >= 0) {
                         const float4 r = __ldg(&g_quad[L.rule + mu]);
                         f = r.x;
                         qw = L.qa * (r.y - r.z * L.inv_n2 + r.w * L.inv_n4);
                     }
                     // sigma = 0: the bin / tick is an integer decision taken in float64 in the oracle's order
                     int ia = -1, ib = -1, jj = -1;
-                    if (L.zero_sigma && real) {
+                    if ((RND || L.zero_sigma) && real) {
                         const int s = L.seg;
                         const double fd = xdiv(xadd((double)mu, 0.5), (double)L.N);
+                        double z[3] = {0.0, 0.0, 0.0}, sT = 0.0, st = 0.0;
+                        if (RND) {
+                            perturbation_normals(p.rnd_seed, (uint32_t)s, (uint32_t)mu, (uint32_t)nu, p.n_sigma_map, z);
+                            sT = (double)a.sigma_T[s];  st = (double)a.sigma_t[s];
+                        }
                         if (role_a) {
                             const double us = a.u_s[s], ue = a.u_e[s], vs = a.v_s[s], ve = a.v_e[s];
-                            const long long xa = (long long)floor(xdiv(xadd(us, xmul(xsub(ue, us), fd)), p.bin)) - A_t;
-                            const long long xb = (long long)floor(xdiv(xadd(vs, xmul(xsub(ve, vs), fd)), p.bin)) - B_t;
+                            const double uu = xadd(xadd(us, xmul(xsub(ue, us), fd)), xmul(sT, z[0]));
+                            const double vv = xadd(xadd(vs, xmul(xsub(ve, vs), fd)), xmul(sT, z[1]));
+                            const long long xa = (long long)floor(xdiv(uu, p.bin)) - A_t;
+                            const long long xb = (long long)floor(xdiv(vv, p.bin)) - B_t;
                             if (xa >= 0 && xa < NB && xb >= 0 && xb < NB) { ia = (int)xa; ib = (int)xb; }
                         } else {
                             const double Ts = a.T_s[s], Te = a.T_e[s];
-                            long long j = (long long)floor(xdiv(xsub(xadd(Ts, xmul(xsub(Te, Ts), fd)), p.t_origin), p.dt));
+                            const double TT = xadd(xadd(Ts, xmul(xsub(Te, Ts), fd)), xmul(st, z[2]));
+                            long long j = (long long)floor(xdiv(xsub(TT, p.t_origin), p.dt));
                             if (j >= 0 && j <= p.j_max && j - J_t >= 0 && j - J_t < p.Jc) jj = (int)(j - J_t);
                         }
                     }
@@ -301,7 +312,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                         if (!real) {
     #pragma unroll
                             for (int i = 0; i < NB; ++i) wx[i] = wy[i] = 0.f;
-                        } else if (L.zero_sigma) {
+                        } else if (RND || L.zero_sigma) {
     #pragma unroll
                             for (int i = 0; i < NB; ++i) { wx[i] = (i == ia) ? 1.f : 0.f; wy[i] = (i == ib) ? 1.f : 0.f; }
                         } else {
@@ -336,7 +347,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                             if (!real || j0 + 7 < L.jlo || j0 > L.jhi) {
     #pragma unroll
                                 for (int i = 0; i < 8; ++i) x[i] = 0.f;
-                            } else if (L.zero_sigma) {
+                            } else if (RND || L.zero_sigma) {
     #pragma unroll
                                 for (int i = 0; i < 8; ++i) x[i] = (j0 + i == jj) ? qw : 0.f;
                             } else {

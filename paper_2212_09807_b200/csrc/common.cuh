@@ -29,6 +29,8 @@ struct DevParams {
     int n_groups;                    // pair groups per tile = response passes over a tile (1 for W = 5, K = 200)
     int slab_floats;                 // packed charge lattice of one tile: header, bin items, charge rows
                                      // (tensor-core mode: NB2 * 64 = the tile's rows of the fp16 hi / lo operand image)
+    int rnd_m;                       // > 0: eq. (3.9) as printed, M random perturbations per sample point (lartpc_set_random_perturbations)
+    unsigned long long rnd_seed;
     int node_rules;                  // 1: the tensor-core splat may replace a segment's N midpoints by a node rule (charge_tc.cuh)
     int tc_mode;                     // 1: S4 response on the tensor cores (response_tc.cuh), 0: packed-FFMA2 response
     int NBW;                         // tensor-core mode: output columns per 16-tick arrival block, roundup16(K + 15)
@@ -141,6 +143,41 @@ __device__ __forceinline__ double drift_dist(const DevTpc &t, double z)
     if (d < 0.0) d = 0.0;
     if (d > t.drift_len) d = t.drift_len;
     return d;
+}
+
+
+// ---- Philox4x32-10 (Salmon et al., SC'11): counter (c0..c3), key (k0, k1) ----------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t lo0 = 0xD2511F53u * c0, hi0 = __umulhi(0xD2511F53u, c0);
+        const uint32_t lo1 = 0xCD9E8D57u * c2, hi1 = __umulhi(0xCD9E8D57u, c2);
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+
+// three standard normals of perturbed point (segment s, mu, nu) of eq. (3.9) as printed (reading D25): Box-Muller pairs
+// of Philox(counter (s, mu, nu, 'RAND'), key = seed), clamped to +- clamp
+__device__ __forceinline__ void perturbation_normals(unsigned long long seed, uint32_t s, uint32_t mu, uint32_t nu,
+                                                     double clamp, double (&z)[3])
+{
+    uint32_t x[4];
+    philox4x32_10(s, mu, nu, 0x52414E44u, (uint32_t)seed, (uint32_t)(seed >> 32), x);
+    const double sc = 1.0 / 4294967296.0, two_pi = 6.283185307179586476925286766559;
+    const double u0 = ((double)x[0] + 0.5) * sc, u1 = ((double)x[1] + 0.5) * sc;
+    const double u2 = ((double)x[2] + 0.5) * sc, u3 = ((double)x[3] + 0.5) * sc;
+    const double r01 = sqrt(-2.0 * log(u0)), r23 = sqrt(-2.0 * log(u2));
+    z[0] = r01 * cos(two_pi * u1);
+    z[1] = r01 * sin(two_pi * u1);
+    z[2] = r23 * cos(two_pi * u3);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) z[k] = fmin(fmax(z[k], -clamp), clamp);
 }
 
 // ---- launch helpers -----------------------------------------------------------------------------

@@ -663,12 +663,15 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     a.charge = out->charge;  a.tile_range = out->tile_range;
     a.fma_counter = sim->d_fma;
     a.rec = nullptr;  a.tile_list = nullptr;  a.work = nullptr;  a.n_tiles = 0;  a.tb_mask = sim->tb_mask;
+    if (p.rnd_m > 0 && !(p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5))) return LARTPC_ERR_UNSUPPORTED;
     if (p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5)) {
         // tensor-core splat (charge_tc.cuh); other bin counts use the FFMA2 splat below, which writes the same image
         static bool configured_tc = false;
         if (!configured_tc) {
-            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
-            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
+            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<10, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
+            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
+            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<10, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
+            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<5, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
             configured_tc = true;
         }
         if (n >= (1ll << 30) || sim->n_tiles >= INT32_MAX - 8 * (int64_t)sim->sm_count) return LARTPC_ERR_UNSUPPORTED;
@@ -689,8 +692,13 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
         const unsigned grid = (unsigned)std::min<int64_t>(sim->n_tiles, 4 * (int64_t)sim->sm_count);
         ++g_lartpc_launches;
-        if (p.nb == 10) charge_lattice_tc_kernel<10><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
-        else charge_lattice_tc_kernel<5><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+        if (p.rnd_m > 0) {
+            if (p.nb == 10) charge_lattice_tc_kernel<10, true><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+            else charge_lattice_tc_kernel<5, true><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+        } else {
+            if (p.nb == 10) charge_lattice_tc_kernel<10, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+            else charge_lattice_tc_kernel<5, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+        }
         LARTPC_CUDA_TRY(cudaGetLastError());
         return LARTPC_OK;
     }

@@ -160,20 +160,6 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
 // Noise: Philox4x32-10, counter (pixel id, tick, 0, 0), key (seed lo, seed hi); Box-Muller in float64 so
 // that the ADC decision is taken in the same precision as the oracle's.
 // -------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
-                                              uint32_t k1, uint32_t (&out)[4])
-{
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const uint32_t lo0 = 0xD2511F53u * c0, hi0 = __umulhi(0xD2511F53u, c0);
-        const uint32_t lo1 = 0xCD9E8D57u * c2, hi1 = __umulhi(0xCD9E8D57u, c2);
-        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
-        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-    }
-    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
-}
-
 __device__ __forceinline__ void noise_normals(unsigned long long seed, uint32_t pixel, uint32_t tick, double (&z)[3])
 {
     uint32_t x[4];

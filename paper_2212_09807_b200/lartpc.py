@@ -104,7 +104,8 @@ class Stats(C.Structure):
                [("n_batches", C.c_int32), ("reserved", C.c_int32), ("flops_current", C.c_double)]
 
 
-EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", "lartpc_sim_destroy", "lartpc_set_disabled_pixels", "lartpc_chunk_ticks",
+EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", "lartpc_sim_destroy", "lartpc_set_disabled_pixels",
+           "lartpc_set_random_perturbations", "lartpc_chunk_ticks",
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
            "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_run_spill",
            "lartpc_measure_fp32_peak", "lartpc_set_profiling", "lartpc_get_stage_ms", "lartpc_kernel_launches", "lartpc_strerror")
@@ -226,6 +227,12 @@ class Sim:
                 raise LartpcError("segment fields differ in length")
             setattr(s, k, v.data_ptr())
         return s, int(n)
+
+    def set_random_perturbations(self, m: int, seed: int = 0):
+        """S4 as eq. (3.9) prints it: m random perturbations per sample point (0 = expectation form, the default)."""
+        _check(self.lib.lartpc_set_random_perturbations(self.handle, C.c_int(int(m)),
+                                                        C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF)),
+               "lartpc_set_random_perturbations")
 
     def set_disabled_pixels(self, ids: np.ndarray):
         ids = np.ascontiguousarray(ids, dtype=np.int32)

@@ -387,3 +387,48 @@ def test_electronics_variants(lartpc, variant):
     dr, pm = _check_segment_stages(res, wl)
     _check_hits(res, wl, dr, pm, wl.seed)
     sim.close()
+
+
+@pytest.mark.parametrize("m,seed", [(1, 5), (3, 0xABCDEF0123)])
+def test_random_perturbations_same_draws(lartpc, m, seed):
+    """SURVEY 8(f) NEXT-1, eq. (3.9) as printed: M random perturbations per sample point, nearest-bin look-up.
+    Both sides key the normals by (seed; segment, mu, nu) (reading D25), so the comparison is draw for draw: the waveforms
+    and charges of every active pixel, and the hits, against the oracle's random estimator."""
+    wl = W.make_config(0, seed=21)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    sim.set_random_perturbations(m, seed)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    nt = wl.params["n_readout_ticks"]
+    dense = dense_waves(res, nt)
+    gpu_ids = res["waveforms"]["pixel_id"][:res["n_active"]]
+    t = wl.tpcs[0]
+    rel = gpu_ids - t["first_pixel_id"]
+    waves, qp = oracle.pixel_currents_random(wl.params, wl.tpcs, wl.lut, dr, pm, 0, rel % t["nx"], rel // t["nx"], m, seed)
+    assert qp.sum() > 0
+    gq = dense.sum(axis=1)
+    tol = np.maximum(1e-4 * np.abs(qp), 1.0)
+    assert np.all(np.abs(gq - qp) <= tol), (np.abs(gq - qp) / tol).max()
+    peak = np.abs(waves).max(axis=1, keepdims=True)
+    assert np.all(np.abs(dense - waves) <= 1e-4 * peak + 0.02)
+    # it is a different estimate from the expectation form, not the same numbers
+    _, q_exp = oracle.pixel_currents(wl.params, wl.tpcs, wl.lut, dr, pm, 0, rel % t["nx"], rel // t["nx"])
+    assert np.abs(qp - q_exp).max() > 10.0 and qp.sum() == pytest.approx(q_exp.sum(), rel=1e-5)
+    hp, ht, ha, _ = oracle.electronics(wl.params, wl.seed, gpu_ids.astype(np.int32), waves)
+    h = res["hits"]
+    n = int(h["counters"][0])
+    frac, near, ng, no = compare_hits((h["hit_pixel"][:n], h["hit_tick"][:n], h["hit_adc"][:n]), (hp, ht, ha))
+    assert no > 0 and frac >= 0.999 and near and ng == no
+    # back to the default
+    sim.set_random_perturbations(0)
+    res0 = run_staged(sim, wl)
+    assert np.allclose(dense_waves(res0, nt).sum(axis=1), q_exp, rtol=1e-4, atol=1.0)
+    sim.close()
+
+
+def test_random_perturbations_need_the_tensor_path(lartpc):
+    wl = W.make_config(0)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, response="ffma")
+    with pytest.raises(lartpc.LartpcError):
+        sim.set_random_perturbations(2, 1)
+    sim.close()
