@@ -264,6 +264,17 @@ int  lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n
                       lartpc_hits_t *out, lartpc_stats_t *stats, void *workspace, size_t ws_bytes,
                       void *stream);
 
+/* Packed hit output (BASELINE configs[3]: "16-bit packed hit output"; reading D18).  Regroups a hit list
+ * sorted by (pixel id, tick) -- what lartpc_electronics / lartpc_run_spill write -- by readout tile of tile_pixels x
+ * tile_pixels pixels (70 in the paper; <= 255), tiles numbered TPC by TPC in table order, row-major inside a TPC
+ * (planes whose size is not a multiple of tile_pixels end in partial tiles).  packed: device uint16[n_hits][3] =
+ * {pixel in tile = iy_in * tile_pixels + ix_in, tick, adc | flags << 12 (flags = 0)}, ordered by (tile, pixel in tile,
+ * tick); tile_offsets: device int64[lartpc_readout_tiles() + 1], hits of tile k are [tile_offsets[k], tile_offsets[k+1]).
+ * Bit-exact, order-defined.  n_readout_ticks <= 65536 and adc_bits <= 12, else LARTPC_ERR_UNSUPPORTED. */
+int64_t lartpc_readout_tiles(const lartpc_sim_t *sim, int tile_pixels);
+int  lartpc_pack_hits(lartpc_sim_t *sim, const lartpc_hits_t *hits, int64_t n_hits, int tile_pixels,
+                      uint16_t *packed, int64_t *tile_offsets, void *stream);
+
 /* ---- measurement aids ------------------------------------------------------------------------ */
 
 /* Runs an FFMA-chain microbenchmark on `stream` and returns the measured FP32 rate in TFLOP/s

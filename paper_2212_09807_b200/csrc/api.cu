@@ -43,6 +43,7 @@ static void sim_free(lartpc_sim *s)
     cudaFree(s->pix_count); cudaFree(s->pix_start); cudaFree(s->pix_tile0); cudaFree(s->pix_cursor);
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
     cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->tile_list); cudaFree(s->seg_rec);
+    cudaFree(s->pack_base); cudaFree(s->pack_count);
     cudaFree(s->tile_perm); cudaFree(s->tile_desc_p); cudaFree(s->tile_list_p); cudaFree(s->tb_mask); cudaFree(s->cls_hist); cudaFree(s->scan_tmp);
     cudaFree(s->d_counters); cudaFree(s->disabled_mask); cudaFree(s->elec_slots); cudaFree(s->elec_offs);
     cudaFree(s->d_fma); cudaFree(s->d_work); cudaFree(s->pix_jmin); cudaFree(s->d_end_row);
@@ -302,6 +303,25 @@ extern "C" int lartpc_set_random_perturbations(lartpc_sim_t *sim, int m, uint64_
     sim->dp.rnd_seed = seed;
     sim->have_signals = false;
     return LARTPC_OK;
+}
+
+extern "C" int64_t lartpc_readout_tiles(const lartpc_sim_t *sim, int tile_pixels)
+{
+    if (!sim || tile_pixels < 1 || tile_pixels > 255) return LARTPC_ERR_BAD_ARGUMENT;
+    int64_t n = 0;
+    for (const lartpc_tpc_t &t : sim->tpcs)
+        n += (int64_t)((t.nx + tile_pixels - 1) / tile_pixels) * ((t.ny + tile_pixels - 1) / tile_pixels);
+    return n;
+}
+
+extern "C" int lartpc_pack_hits(lartpc_sim_t *sim, const lartpc_hits_t *hits, int64_t n_hits, int tile_pixels,
+                                uint16_t *packed, int64_t *tile_offsets, void *stream)
+{
+    if (!sim || !hits || n_hits < 0 || tile_pixels < 1 || tile_pixels > 255 || !tile_offsets || (n_hits > 0 && !packed))
+        return LARTPC_ERR_BAD_ARGUMENT;
+    if (n_hits > 0 && (!hits->hit_pixel || !hits->hit_tick || !hits->hit_adc)) return LARTPC_ERR_BAD_ARGUMENT;
+    if (sim->dp.n_ticks > 65536 || sim->params.adc_bits > 12) return LARTPC_ERR_UNSUPPORTED;   // tick and adc must fit 16 / 12 bits
+    return launch_pack_hits(sim, hits, n_hits, tile_pixels, packed, tile_offsets, (cudaStream_t)stream);
 }
 
 extern "C" int lartpc_chunk_ticks(const lartpc_sim_t *sim) { return sim ? sim->dp.Jc : 0; }

@@ -94,6 +94,7 @@ struct lartpc_sim {
     int32_t *tb_mask = nullptr;  int32_t *cls_hist = nullptr;   // [tile_cap / 128 + 2], [32]: class counts then cursors
     std::vector<int64_t> cp_base_h, pix_base_h;   // [n_tpcs + 1] first charged-pixel cell / first pixel of each TPC (host copy)
     int64_t plan_pix_lo = 0, plan_pix_hi = 0;       // pixel range of the TPCs the current plan covers
+    int32_t *pack_base = nullptr, *pack_count = nullptr;  int pack_tile_pixels = 0;   // lartpc_pack_hits: readout-tile tables
     int batch_hint = 0;  size_t batch_hint_ws = 0;   // lartpc_run_spill: TPCs per batch that fitted the workspace last time
     bool tile_sort = true;               // env LARTPC_TILE_SORT=0: identity order, every block kept (measurement aid)
     void *seg_rec = nullptr;  int64_t seg_rec_cap = 0;   // per-segment records of the tensor-core splat (charge_tc.cuh)
@@ -199,6 +200,8 @@ static inline int64_t tiles_alloc(const DevParams &p, int64_t n_tiles)
 {
     return p.tc_mode ? (n_tiles + TC_TILE_BLOCK - 1) / TC_TILE_BLOCK * TC_TILE_BLOCK : n_tiles;
 }
+int launch_pack_hits(lartpc_sim *sim, const lartpc_hits_t *hits, int64_t n_hits, int tile_pixels, uint16_t *packed,
+                     int64_t *tile_offsets, cudaStream_t st);
 int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out, cudaStream_t st);
 int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
                        int32_t *slot_scratch, int32_t *scan_scratch, int64_t hit_base, cudaStream_t st);

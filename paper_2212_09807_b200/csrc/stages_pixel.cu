@@ -368,3 +368,102 @@ int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t s
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }
+
+
+// -------------------------------------------------------------------------------------------------
+// Packed hit output (BASELINE configs[3] "16-bit packed hit output", reading D18): the (pixel, tick)-sorted hit list
+// regrouped by readout tile (tile_pixels x tile_pixels pixels: 70 x 70) as three uint16 per hit
+// {pixel in tile = iy_in * tile_pixels + ix_in, tick, adc | flags << 12}, with an offset table per tile.
+// One CTA per readout tile; a pixel row of a tile is a contiguous run of the sorted list, found by binary search, so
+// the order inside a tile is (pixel in tile, tick) and nothing depends on atomics.
+// -------------------------------------------------------------------------------------------------
+struct PackGeom { const DevTpc *tpcs; const int32_t *tile_base; int n_tpcs, tile_pixels; };
+
+__device__ __forceinline__ int64_t lower_bound_i32(const int32_t *v, int64_t n, int32_t key)
+{
+    int64_t lo = 0, hi = n;
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (v[mid] < key) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+template <bool WRITE>
+__global__ void __launch_bounds__(128)
+pack_hits_kernel(PackGeom g, int64_t n_hits, const int32_t *__restrict__ hit_pixel, const int32_t *__restrict__ hit_tick,
+                 const int32_t *__restrict__ hit_adc, int32_t *tile_count, const int64_t *__restrict__ tile_off,
+                 uint16_t *packed)
+{
+    __shared__ long long s_start[256];
+    __shared__ int s_cnt[256], s_pre[257];
+    const int tile = blockIdx.x, tid = threadIdx.x;
+    int tpc = 0;
+    while (tpc + 1 < g.n_tpcs && g.tile_base[tpc + 1] <= tile) ++tpc;
+    const DevTpc &t = g.tpcs[tpc];
+    const int tp = g.tile_pixels, ntx = (t.nx + tp - 1) / tp;
+    const int rel = tile - g.tile_base[tpc], ty = rel / ntx, tx = rel - ty * ntx;
+    const int x0 = tx * tp, x1 = min(x0 + tp, t.nx), y0 = ty * tp, rows = min(y0 + tp, t.ny) - y0;
+    for (int r = tid; r < rows; r += blockDim.x) {
+        const int32_t id0 = t.first_pixel_id + (y0 + r) * t.nx + x0, id1 = id0 + (x1 - x0);
+        const int64_t a = lower_bound_i32(hit_pixel, n_hits, id0), b = lower_bound_i32(hit_pixel, n_hits, id1);
+        s_start[r] = a;  s_cnt[r] = (int)(b - a);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int run = 0;
+        for (int r = 0; r < rows; ++r) { s_pre[r] = run; run += s_cnt[r]; }
+        s_pre[rows] = run;
+        if (!WRITE) tile_count[tile] = run;
+    }
+    if (!WRITE) return;
+    __syncthreads();
+    const int64_t base = tile_off[tile];
+    for (int r = 0; r < rows; ++r) {
+        const int64_t src = s_start[r];
+        for (int k = tid; k < s_cnt[r]; k += blockDim.x) {
+            const int64_t h = src + k;
+            const int32_t id = hit_pixel[h] - t.first_pixel_id;
+            const int iy = id / t.nx, ix = id - iy * t.nx;
+            uint16_t *o = packed + 3 * (base + s_pre[r] + k);
+            o[0] = (uint16_t)((iy - y0) * tp + (ix - x0));
+            o[1] = (uint16_t)hit_tick[h];
+            o[2] = (uint16_t)(hit_adc[h] & 0x0fff);
+        }
+    }
+}
+
+struct TileCountF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
+
+int launch_pack_hits(lartpc_sim *sim, const lartpc_hits_t *hits, int64_t n_hits, int tile_pixels, uint16_t *packed,
+                     int64_t *tile_offsets, cudaStream_t st)
+{
+    const DevParams &p = sim->dp;
+    // readout tiles per TPC, in table order
+    std::vector<int32_t> base(p.n_tpcs + 1, 0);
+    for (int k = 0; k < p.n_tpcs; ++k) {
+        const lartpc_tpc_t &t = sim->tpcs[k];
+        base[k + 1] = base[k] + ((t.nx + tile_pixels - 1) / tile_pixels) * ((t.ny + tile_pixels - 1) / tile_pixels);
+    }
+    const int n_rt = base[p.n_tpcs];
+    if (sim->pack_tile_pixels != tile_pixels) {
+        cudaFree(sim->pack_base);  cudaFree(sim->pack_count);
+        sim->pack_base = nullptr;  sim->pack_count = nullptr;  sim->pack_tile_pixels = 0;
+        LARTPC_CUDA_TRY(cudaMalloc(&sim->pack_base, sizeof(int32_t) * (p.n_tpcs + 1)));
+        LARTPC_CUDA_TRY(cudaMalloc(&sim->pack_count, sizeof(int32_t) * (n_rt + 1)));
+        LARTPC_CUDA_TRY(cudaMemcpy(sim->pack_base, base.data(), sizeof(int32_t) * (p.n_tpcs + 1), cudaMemcpyHostToDevice));
+        sim->pack_tile_pixels = tile_pixels;
+    }
+    int rc = sim_ensure_scan_tmp(sim, n_rt);
+    if (rc) return rc;
+    PackGeom g{sim->d_tpcs, sim->pack_base, p.n_tpcs, tile_pixels};
+    g_lartpc_launches += 2;
+    pack_hits_kernel<false><<<n_rt, 128, 0, st>>>(g, n_hits, hits->hit_pixel, hits->hit_tick, hits->hit_adc,
+                                                  sim->pack_count, nullptr, nullptr);
+    LARTPC_CUDA_TRY(lscan::exclusive_scan((int64_t)n_rt, TileCountF{sim->pack_count}, tile_offsets, true,
+                                          (long long *)nullptr, sim->scan_tmp, st));
+    pack_hits_kernel<true><<<n_rt, 128, 0, st>>>(g, n_hits, hits->hit_pixel, hits->hit_tick, hits->hit_adc,
+                                                 sim->pack_count, tile_offsets, packed);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}

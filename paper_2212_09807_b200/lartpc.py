@@ -108,6 +108,7 @@ EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", 
            "lartpc_set_random_perturbations", "lartpc_chunk_ticks",
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
            "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_run_spill",
+           "lartpc_readout_tiles", "lartpc_pack_hits",
            "lartpc_measure_fp32_peak", "lartpc_set_profiling", "lartpc_get_stage_ms", "lartpc_kernel_launches", "lartpc_strerror")
 
 
@@ -367,6 +368,22 @@ class Sim:
                                          C.byref(st), C.c_void_p(workspace.data_ptr()),
                                          C.c_size_t(workspace.numel()), _stream_ptr(t)), "lartpc_run_spill")
         return out, st
+
+    def pack_hits(self, hits, n_hits: Optional[int] = None, tile_pixels: int = 70):
+        """16-bit packed hit output grouped by readout tile: returns (packed int16 tensor [n_hits, 3] holding the
+        uint16 words, tile_offsets int64 tensor [n_tiles + 1])."""
+        t = self.torch
+        n = int(hits["counters"][0].item()) if n_hits is None else int(n_hits)
+        self.lib.lartpc_readout_tiles.restype = C.c_int64
+        n_rt = int(self.lib.lartpc_readout_tiles(self.handle, C.c_int(int(tile_pixels))))
+        if n_rt < 0:
+            _check(n_rt, "lartpc_readout_tiles")
+        packed = self._empty(3 * max(n, 1), t.int16)
+        offs = self._empty(n_rt + 1, t.int64)
+        _check(self.lib.lartpc_pack_hits(self.handle, C.byref(hits["_struct"]), C.c_int64(n), C.c_int(int(tile_pixels)),
+                                         C.c_void_p(packed.data_ptr()), C.c_void_p(offs.data_ptr()), _stream_ptr(t)),
+               "lartpc_pack_hits")
+        return packed[:3 * n].view(n, 3), offs
 
 
 def hits_to_numpy(hits, n: Optional[int] = None):

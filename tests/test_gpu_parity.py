@@ -364,6 +364,10 @@ def test_config3_full_spill(lartpc):
         in_busy |= (hp >= t["first_pixel_id"]) & (hp < t["first_pixel_id"] + t["nx"] * t["ny"])
     assert in_busy.sum() == n_sub
     assert np.array_equal(hp[in_busy], sub_hits[0]) and np.array_equal(ht[in_busy], sub_hits[1]) and np.array_equal(ha[in_busy], sub_hits[2])
+    # (d) the 16-bit packed output of the whole spill (70 x 70 readout tiles, partial tiles at the plane edges)
+    packed, offs = sim.pack_hits(hits, st.n_hits, 70)
+    want_p, want_o = _pack_reference(wl, hp, ht, ha, 70)
+    assert np.array_equal(offs.cpu().numpy(), want_o) and np.array_equal(packed.cpu().numpy().view(np.uint16), want_p)
     print("config 3: %d segments, %d tiles, %d hits; TPCs %s alone: %d hits, identical inside the full spill"
           % (wl.n_segments, st.n_tiles, st.n_hits, busy, n_sub))
     sim.close()
@@ -431,4 +435,42 @@ def test_random_perturbations_need_the_tensor_path(lartpc):
     sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, response="ffma")
     with pytest.raises(lartpc.LartpcError):
         sim.set_random_perturbations(2, 1)
+    sim.close()
+
+
+def _pack_reference(wl, hp, ht, ha, tile_pixels):
+    """The packed layout written out with numpy from its definition (include/lartpc.h, lartpc_pack_hits)."""
+    tile_of, in_tile = np.zeros(len(hp), dtype=np.int64), np.zeros(len(hp), dtype=np.int64)
+    base = 0
+    for t in wl.tpcs:
+        ntx, nty = -(-t["nx"] // tile_pixels), -(-t["ny"] // tile_pixels)
+        m = (hp >= t["first_pixel_id"]) & (hp < t["first_pixel_id"] + t["nx"] * t["ny"])
+        rel = hp[m].astype(np.int64) - t["first_pixel_id"]
+        iy, ix = rel // t["nx"], rel % t["nx"]
+        tile_of[m] = base + (iy // tile_pixels) * ntx + ix // tile_pixels
+        in_tile[m] = (iy % tile_pixels) * tile_pixels + ix % tile_pixels
+        base += ntx * nty
+    order = np.lexsort((ht, in_tile, tile_of))
+    packed = np.stack([in_tile[order], ht[order], ha[order] & 0x0fff], axis=1).astype(np.uint16)
+    offs = np.concatenate([[0], np.cumsum(np.bincount(tile_of, minlength=base))]).astype(np.int64)
+    return packed, offs
+
+
+@pytest.mark.parametrize("tile_pixels", [70, 32])
+def test_packed_hit_output(lartpc, tile_pixels):
+    """BASELINE configs[3] "16-bit packed hit output" (D18) on the configs[2] spill: three uint16 per hit grouped by
+    readout tile with an offset table, bit-exact against the layout's definition; partial tiles at the plane edges."""
+    wl = W.make_config(2)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    seg = sim.upload_segments(wl.segments)
+    hits, st = sim.run_spill(seg, wl.seed, hit_capacity=1 << 20)
+    packed, offs = sim.pack_hits(hits, st.n_hits, tile_pixels)
+    hp, ht, ha = lartpc.hits_to_numpy(hits, st.n_hits)
+    want_p, want_o = _pack_reference(wl, hp, ht, ha, tile_pixels)
+    assert st.n_hits > 1000
+    assert np.array_equal(offs.cpu().numpy(), want_o)
+    assert np.array_equal(packed.cpu().numpy().view(np.uint16), want_p)
+    # empty list
+    packed0, offs0 = sim.pack_hits(hits, 0, tile_pixels)
+    assert packed0.shape[0] == 0 and np.all(offs0.cpu().numpy() == 0)
     sim.close()
