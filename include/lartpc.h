@@ -130,20 +130,22 @@ typedef struct {
 } lartpc_pixmap_info_t;
 
 /* S4 output.  A tile is (charged pixel P, window of lartpc_chunk_ticks() arrival ticks that starts at
- * j_start = first arrival tick on P, rounded down to even, + a multiple of the window length).
+ * j_start = first arrival tick on P, rounded down to a multiple of 4, + a multiple of the window length).
  *   charge      the charge lattice of eq. (3.8) in expectation, C[bin][j] electrons per (x, y) LUT bin of P and
  *               arrival tick, tile_charge_floats 32-bit words per tile.
- *               Tensor-core response (lartpc_response_mode() == LARTPC_RESPONSE_TENSOR): the fp16 operand image
- *               the MMA reads, [tile / 128][bin][hi | lo][tile % 128][64 ticks] with the 16-byte chunks of a row
- *               permuted by (tile % 8) (128-byte swizzle), C = (hi + lo) * 2^e with e in tile_range; the buffer
- *               must hold a whole number of 128-tile blocks: tile_capacity >= n_tiles rounded up to 128.
+ *               Tensor-core response (lartpc_response_mode() == LARTPC_RESPONSE_TENSOR): the operand image the MMAs
+ *               read, [slot / 128][bin][16-tick block][fp16 part | fp8 part][slot % 128][32 bytes], where a tile's
+ *               slot is given by the sim's plan (tiles that charge the same 16-tick blocks sit together); the fp16
+ *               part holds C 2^-e, the fp8 (e4m3) part {lo8 = (C 2^-e - fp16 part) 2^5, hi8 = C 2^-e 2^-7} per tick,
+ *               e in tile_range; blocks no tile of a 128-slot block charges are neither written nor read; the buffer
+ *               must hold a whole number of 128-slot blocks: tile_capacity >= n_tiles rounded up to 128.
  *               FFMA response: packed per tile as a header (bins, charge groups, first / last output block), one
  *               item per non-empty bin (bin, first tick, groups of 4 ticks, row offset) and the charge rows;
- *   partial     float32 [n_tiles][tile_targets][tile_ticks] (electrons per tick): the current that charge
- *               induces on the W x W pixels around P during readout ticks [j_start, j_start + tile_ticks);
- *   tile_range  int32 [n_tiles][4] = first / last 14-tick block of `partial` that can be non-zero (first > last:
- *               no charge), the scale exponent e, 0.
- * The tile -> pixel map is part of the sim's plan. */
+ *   partial     float32 [n_tiles][tile_targets][tile_ticks] (electrons per tick), indexed by slot: the current that
+ *               charge induces on the W x W pixels around P during readout ticks [j_start, j_start + tile_ticks);
+ *   tile_range  int32 [n_tiles][4], indexed by slot = first / last 14-tick block of `partial` that can be non-zero
+ *               (first > last: no charge), the scale exponent e, 0.
+ * The tile -> pixel and tile -> slot maps are part of the sim's plan (FFMA response: slot = tile). */
 typedef struct {
     int64_t  tile_capacity;             /* host value: tiles the charge buffer can hold (partial / tile_range: n_tiles) */
     float   *partial;

@@ -5,8 +5,16 @@
 //     C[b][a][j]  = sum_seg sum_mu (Q_a/N) wx[a] wy[b] wt[j]          (charge per LUT cell, eq. 3.8)
 //     I_p[n]      = sum_{a,b,j} C[b][a][j] * R[b - nb(iy-H)][a - nb(ix-H)][n - j]      (eq. 3.7)
 // which needs ~50x fewer operations and shares the charge lattice between neighbouring segments.
-// A tile is (charged pixel P, window of Jc arrival ticks).  Two kernels:
+// A tile is (charged pixel P, window of Jc arrival ticks).  Two kernels per path:
 //
+// Tensor-core path (default; charge_tc.cuh + response_tc.cuh): both factors are dense contractions on tcgen05.
+//   charge_lattice_tc_kernel  C = WXY WT^T over the operand columns (node-rule nodes or sample midpoints, or the perturbed
+//                             points of eq. (3.9) as printed) of a tile's segments; persistent CTAs, TMEM accumulator,
+//                             cp.async look-ahead for descriptors / ids / per-segment records.
+//   response_tc_kernel        I = C x Toeplitz(R): per (128-tile block, target, bin) the charged 16-tick blocks of the
+//                             operand image against one 16 x NBW LUT generator, fp16 main term + fp8 cross terms.
+//
+// FFMA2 path (this file; K > 241, bins per pixel other than 5 / 10, or on request):
 //   charge_lattice_kernel (one CTA per tile)
 //     splat the tile's segments into C[nb*nb][Jc] in shared memory (register-tiled outer products of
 //     per-sample erf-difference weights, no atomics, fixed order), then pack the non-empty bins: per bin the
