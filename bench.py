@@ -289,7 +289,8 @@ def run_ours(args):
             else:
                 peak, peak_src = 1590.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
             K, nb2, ww = int(wl.params["lut_ticks"]), int(wl.params["bins_per_pixel"]) ** 2, int(wl.params["window_pixels"]) ** 2
-            nbw = (K + 15 + 15) // 16 * 16
+            kq = K if (K + 15 + 15) // 16 * 16 <= 256 else 200               # LUT pieces of the tensor path
+            nbw, ww = (kq + 15 + 15) // 16 * 16, ww * ((K + kq - 1) // kq)
             tiles_per_launch = int(st.n_tiles) * args.steps / n_resp
             # 4 blocks x (one fp16 MMA of K = 16 + one fp8 MMA of K = 32, which occupies the pipe like an fp16 K = 16):
             # 8 fp16-equivalent MMA slots per (tile block, target, bin)

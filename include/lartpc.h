@@ -143,6 +143,8 @@ typedef struct {
  *               item per non-empty bin (bin, first tick, groups of 4 ticks, row offset) and the charge rows;
  *   partial     float32 [n_tiles][tile_targets][tile_ticks] (electrons per tick), indexed by slot: the current that
  *               charge induces on the W x W pixels around P during readout ticks [j_start, j_start + tile_ticks);
+ *               tile_targets = W*W, except on the tensor-core path with lut_ticks > 241, where the LUT is cut into
+ *               pieces of 200 ticks and row (target d, piece q) = d * pieces + q covers ticks from j_start + 200 q;
  *   tile_range  int32 [n_tiles][4], indexed by slot = first / last 14-tick block of `partial` that can be non-zero
  *               (first > last: no charge), the scale exponent e, 0.
  * The tile -> pixel and tile -> slot maps are part of the sim's plan (FFMA response: slot = tile). */
@@ -198,9 +200,10 @@ int  lartpc_sim_create(const lartpc_params_t *params, const lartpc_tpc_t *tpcs, 
 void lartpc_sim_destroy(lartpc_sim_t *sim);
 
 /* As lartpc_sim_create, choosing how S4 applies the response (eq. 3.7):
- *   LARTPC_RESPONSE_TENSOR  dense contraction of the charge lattice with the LUT on the tcgen05 tensor cores, fp16
- *                           operands split hi + lo (three products, fp32 accumulation); needs lut_ticks <= 241;
- *   LARTPC_RESPONSE_FFMA    sliding-window convolution on the FP32 pipe (packed FFMA2), any lut_ticks;
+ *   LARTPC_RESPONSE_TENSOR  dense contraction of the charge lattice with the LUT on the tcgen05 tensor cores, operands
+ *                           split hi + lo (fp16 main term, fp8 cross terms, fp32 accumulation); a LUT longer than
+ *                           241 ticks is applied in pieces of 200 ticks; window_pixels^2 <= 128;
+ *   LARTPC_RESPONSE_FFMA    sliding-window convolution on the FP32 pipe (packed FFMA2), any LUT shape;
  *   LARTPC_RESPONSE_AUTO    TENSOR where it applies, else FFMA (what lartpc_sim_create does).
  * Both give the same currents within the S4 tolerance; LARTPC_ERR_UNSUPPORTED when TENSOR
  * is asked for a LUT it cannot take. */

@@ -173,24 +173,27 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
         if (score > best) { best = score; best_groups = g; }
     }
     // Tensor-core response (response_tc.cuh): tiles of 64 arrival ticks, the accumulator of one target pixel
-    // (48 + NBW columns, NBW = roundup16(K + 15)) must fit the 512 TMEM columns with NBW <= 256 (one MMA's N).
-    const int nbw = (K + 15 + 15) & ~15;
-    const bool tc_ok = nbw <= 256 && p.WW <= 128;
+    // (48 + NBW columns, NBW = roundup16(KQ + 15)) must fit the 512 TMEM columns with NBW <= 256 (one MMA's N).  A LUT
+    // longer than 241 ticks is cut into pieces of KQ = 200 ticks: piece q is a LUT of its own whose response lands
+    // 200 q ticks later, one more row per (tile, target) in `partial`, which S5 adds like the rows of other tiles.
+    const int kq = ((K + 15 + 15) & ~15) <= 256 ? K : 200, nq = (K + kq - 1) / kq;
+    const int nbw = (kq + 15 + 15) & ~15;
+    const bool tc_ok = p.WW <= 128 && (long long)p.WW * nq <= 4096;
     if (response_mode == LARTPC_RESPONSE_TENSOR && !tc_ok) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
     p.tc_mode = (response_mode != LARTPC_RESPONSE_FFMA && tc_ok) ? 1 : 0;
     if (best_groups == 0 && !p.tc_mode) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
     if (p.tc_mode) {
-        p.NBW = nbw;
+        p.NBW = nbw;  p.KQ = kq;  p.nq = nq;
         p.n_groups = 1;  p.PG = n_pairs;  p.NP = n_pairs;                 // (unused by the tensor-core response)
         p.Jc = 64;  p.CJ = p.Jc + 4;
-        p.tile_ticks = (p.Jc + K - 1 + 7) & ~7;                           // 264 for K = 200
+        p.tile_ticks = (p.Jc + kq - 1 + 7) & ~7;                          // 264 for K = 200: ticks of one row of `partial`
         p.nblk_max = (p.tile_ticks + RESP_NO - 1) / RESP_NO;
         p.slab_floats = p.NB2 * p.Jc;                                     // NB2 rows of (64 hi + 64 lo) fp16
         if (lartpc_splat_smem(p) > smem_limit) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
     } else {
         p.n_groups = best_groups;  p.PG = (n_pairs + p.n_groups - 1) / p.n_groups;  p.NP = p.n_groups * p.PG;
         p.Jc = std::min(jc_cap, RESP_NO * (ncons / p.PG) - K + 1) & ~3;  p.CJ = p.Jc + 4;
-        p.nblk_max = (p.Jc + K - 2) / RESP_NO + 1;  p.tile_ticks = RESP_NO * p.nblk_max;
+        p.nblk_max = (p.Jc + K - 2) / RESP_NO + 1;  p.tile_ticks = RESP_NO * p.nblk_max;  p.KQ = K;  p.nq = 1;
         p.slab_floats = (SLAB_HDR + 2 * p.NB2 + p.NB2 * (4 + p.CJ) + 3) & ~3;
     }
     if (p.j_max / p.Jc + 2 > MAX_WINDOWS) {                                 // window masks are 128 bits
@@ -533,7 +536,7 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
         ar.used = mark;
         lartpc_signals_t sig;
         sig.tile_capacity = tiles_alloc(p, info.n_tiles);
-        sig.partial = ar.take<float>(info.n_tiles * p.WW * p.tile_ticks);
+        sig.partial = ar.take<float>(info.n_tiles * p.WW * p.nq * p.tile_ticks);
         sig.tile_range = ar.take<int32_t>(info.n_tiles * TILE_META);
         sig.charge = ar.take<float>(sig.tile_capacity * p.slab_floats);
         lartpc_waveforms_t wf;

@@ -33,7 +33,9 @@ struct DevParams {
     unsigned long long rnd_seed;
     int node_rules;                  // 1: the tensor-core splat may replace a segment's N midpoints by a node rule (charge_tc.cuh)
     int tc_mode;                     // 1: S4 response on the tensor cores (response_tc.cuh), 0: packed-FFMA2 response
-    int NBW;                         // tensor-core mode: output columns per 16-tick arrival block, roundup16(K + 15)
+    int NBW;                         // tensor-core mode: output columns per 16-tick arrival block, roundup16(KQ + 15)
+    int KQ, nq;                      // tensor-core mode: LUT ticks per piece and pieces (K <= 241: one piece of K ticks; longer
+                                     // LUTs are cut into pieces of 200 ticks, each a row of its own in `partial`, added by S5)
     int n_tpcs;
     // electronics
     double gain_mv_per_ke, v_cm, v_ref, v_ped, adc_full, threshold;

@@ -794,8 +794,8 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     if (sim->n_tiles >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.n_tiles = (int)sim->n_tiles;
     a.n_tb = (int)((sim->n_tiles + rtc::TB - 1) / rtc::TB);
-    a.NC = p.NB2;  a.WW = p.WW;  a.NBW = p.NBW;  a.tile_ticks = p.tile_ticks;
-    a.n_items = (long long)a.n_tb * p.WW;
+    a.NC = p.NB2;  a.WW = p.WW * p.nq;  a.NBW = p.NBW;  a.tile_ticks = p.tile_ticks;   // a row = (target, LUT piece)
+    a.n_items = (long long)a.n_tb * a.WW;
     if (a.n_items >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.work = sim->d_work;
     LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
@@ -812,20 +812,21 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     return LARTPC_OK;
 }
 
-// Bs[d][c][fp16 | fp8][NBW x 32 bytes] with Bs[n'][jj] = R[c][d][n' - jj] * 2^10 (0 outside the LUT): the fp16 image
+// Bs[d, q][c][fp16 | fp8][NBW x 32 bytes] with Bs[n'][jj] = R[c][d][KQ q + n' - jj] * 2^10 (0 outside piece q of the LUT): the fp16 image
 // (rtc::b_image_offset) and the fp8 image of the cross terms (rtc::b8_image_offset), both in the canonical un-swizzled
 // K-major layout.  Built once per sim on the host.
 size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_out)
 {
-    const int nb = p.nb, W = p.W, K = p.K, NBW = p.NBW, NB = W * nb;
-    const size_t half_elems = (size_t)NBW * 16, n = (size_t)p.WW * p.NB2 * 2 * half_elems;
+    const int nb = p.nb, W = p.W, NBW = p.NBW, NB = W * nb;
+    const size_t half_elems = (size_t)NBW * 16, n = (size_t)p.WW * p.nq * p.NB2 * 2 * half_elems;
     std::vector<__half> img(n);
-    for (int d = 0; d < p.WW; ++d) {
+    for (int dq = 0; dq < p.WW * p.nq; ++dq) {                         // row = (target d, LUT piece q): ticks [KQ q, KQ q + K)
+        const int d = dq / p.nq, q = dq - d * p.nq, K = std::min(p.KQ, p.K - p.KQ * q);
         const int dyi = d / W, dxi = d - dyi * W;
         for (int cb = 0; cb < nb; ++cb)
             for (int ca = 0; ca < nb; ++ca) {
-                const float *src = lut_host + ((size_t)(nb * dyi + cb) * NB + (nb * dxi + ca)) * K;
-                __half *hi = img.data() + ((size_t)d * p.NB2 + (cb * nb + ca)) * 2 * half_elems;
+                const float *src = lut_host + ((size_t)(nb * dyi + cb) * NB + (nb * dxi + ca)) * p.K + (size_t)p.KQ * q;
+                __half *hi = img.data() + ((size_t)dq * p.NB2 + (cb * nb + ca)) * 2 * half_elems;
                 unsigned char *f8 = (unsigned char *)(hi + half_elems);                  // NBW x 32 bytes
                 for (int nn = 0; nn < NBW; ++nn)
                     for (int jj = 0; jj < 16; ++jj) {

@@ -31,7 +31,8 @@ constexpr int SUM_LCAP = 192;      // partial rows listed per round (a pixel usu
 // ticks it can be non-zero on.  Then a thread owns the ticks i = tid mod 128 of the waveform and adds the listed rows in
 // list order (d ascending, window ascending): the loads of one tick are independent of each other, the row reads of a
 // warp are coalesced, and the order of the float32 additions -- hence every output bit -- is fixed.
-template <int VEC>                 // ticks per thread and load: 4 when tile_ticks is a multiple of 4 (rows 16-byte aligned), else 2
+template <int VEC, bool PIECES>    // VEC: ticks per thread and load, 4 when tile_ticks is a multiple of 4 (rows 16-byte aligned), else 2
+                                   // PIECES: a long LUT cut into pieces (tensor-core path, K > 241): nq rows per (tile, target)
 __global__ void __launch_bounds__(SUM_THREADS)
 sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__restrict__ pixel_id,
                  const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,
@@ -70,23 +71,31 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
         for (int d = 0; d < p.WW; ++d) s_base[d + 1] += s_base[d];
     }
     __syncthreads();
-    const int total = s_base[p.WW];
+    const int nq = PIECES ? p.nq : 1;                                 // rows per (tile, target): pieces of a long LUT
+    const int total = s_base[p.WW] * nq;
     const int64_t off = offset[slot];
     for (int r0 = 0; r0 < total; r0 += SUM_LCAP) {
         if (tid < p.WW) {
             const int d = tid, js = s_js[d];
-            int tix = s_tile0[d], gi = s_base[d] - r0;
+            int tix = s_tile0[d], gi = s_base[d] * nq - r0;
 #pragma unroll
             for (int wd = 0; wd < MASK_WORDS; ++wd)
-                for (unsigned long long m = s_mask[d][wd]; m; m &= m - 1, ++tix, ++gi) {
-                    if (gi < 0 || gi >= SUM_LCAP) continue;
+                for (unsigned long long m = s_mask[d][wd]; m; m &= m - 1, ++tix, gi += nq) {
+                    if (gi + nq <= 0 || gi >= SUM_LCAP) continue;
                     const int w = 64 * wd + __ffsll((long long)m) - 1;
                     const int ts = tile_perm ? tile_perm[tix] : tix;
                     const int2 rg = *(const int2 *)(tile_range + TILE_META * ts);       // first / last output block
                     const int j_start = js + w * p.Jc;
-                    e_row[gi] = partial + ((size_t)ts * p.WW + d) * p.tile_ticks - j_start;
-                    e_na[gi] = rg.x > rg.y ? INT_MAX : max(first, j_start + rg.x * RESP_NO);
-                    e_nb[gi] = rg.x > rg.y ? -1 : min(last, j_start + min(rg.y * RESP_NO + RESP_NO - 1, p.tile_ticks - 1));
+#pragma unroll 1
+                    for (int q = 0; q < nq; ++q) {                                      // piece q answers KQ q ticks later
+                        const int g = gi + q;
+                        if (g < 0 || g >= SUM_LCAP) continue;
+                        const int t0 = PIECES ? p.KQ * q : 0;
+                        const int lo = max(rg.x * RESP_NO, t0), hi = min(rg.y * RESP_NO + RESP_NO - 1, t0 + p.tile_ticks - 1);
+                        e_row[g] = partial + (((size_t)ts * p.WW + d) * nq + q) * p.tile_ticks - (j_start + t0);
+                        e_na[g] = (rg.x > rg.y || lo > hi) ? INT_MAX : max(first, j_start + lo);
+                        e_nb[g] = (rg.x > rg.y || lo > hi) ? -1 : min(last, j_start + hi);
+                    }
                 }
         }
         __syncthreads();
@@ -141,16 +150,13 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
     LARTPC_CUDA_TRY(lscan::exclusive_scan(sim->n_active, LenF{out->length}, out->offset, true, (long long *)nullptr,
                                           sim->scan_tmp, st));
     ++g_lartpc_launches;
-    if (p.tile_ticks % 4 == 0)
-        sum_pixel_kernel<4><<<(unsigned)sim->n_active, SUM_THREADS, 0, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
-                                                             out->length, out->offset, sim->pix_mask, sim->pix_tile0,
-                                                             sim->pix_jmin, sig->partial, sig->tile_range,
-                                                             p.tc_mode ? sim->tile_perm : nullptr, out->samples);
-    else
-        sum_pixel_kernel<2><<<(unsigned)sim->n_active, SUM_THREADS, 0, st>>>(p, sim->d_tpcs, out->pixel_id, out->first_tick,
-                                                             out->length, out->offset, sim->pix_mask, sim->pix_tile0,
-                                                             sim->pix_jmin, sig->partial, sig->tile_range,
-                                                             p.tc_mode ? sim->tile_perm : nullptr, out->samples);
+#define LARTPC_SUM_LAUNCH(V, P) sum_pixel_kernel<V, P><<<(unsigned)sim->n_active, SUM_THREADS, 0, st>>>( \
+        p, sim->d_tpcs, out->pixel_id, out->first_tick, out->length, out->offset, sim->pix_mask, sim->pix_tile0, \
+        sim->pix_jmin, sig->partial, sig->tile_range, p.tc_mode ? sim->tile_perm : nullptr, out->samples)
+    if (p.tc_mode && p.nq > 1) LARTPC_SUM_LAUNCH(4, true);             // (tile_ticks = 264 there)
+    else if (p.tile_ticks % 4 == 0) LARTPC_SUM_LAUNCH(4, false);
+    else LARTPC_SUM_LAUNCH(2, false);
+#undef LARTPC_SUM_LAUNCH
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }

@@ -611,7 +611,7 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         info->n_pairs = h[CNT_PAIRS];
         info->n_active_pixels = h[CNT_ACTIVE_PIX];
         info->total_samples = h[CNT_TOTAL_SAMPLES];
-        info->tile_targets = p.WW;
+        info->tile_targets = p.WW * p.nq;                               // rows of `partial` per tile
         info->tile_ticks = p.tile_ticks;
         info->tile_charge_floats = p.slab_floats;
         info->reserved = 0;

@@ -234,10 +234,12 @@ def test_short_drift_all_node_rules(lartpc):
     sim.close()
 
 
-@pytest.mark.parametrize("window,lut_ticks,mode", [(9, 200, "tensor"), (9, 200, "ffma"), (5, 500, "ffma"), (5, 120, "tensor")])
+@pytest.mark.parametrize("window,lut_ticks,mode", [(9, 200, "tensor"), (9, 200, "ffma"), (5, 500, "ffma"), (5, 120, "tensor"),
+                                                   (5, 500, "tensor"), (5, 1000, "tensor"), (9, 300, "tensor")])
 def test_config4_axes_small(lartpc, window, lut_ticks, mode):
     """BASELINE configs[4] sweep axes at a size the oracle finishes in seconds: 9x9 response window and LUT lengths
-    other than 200 ticks (K > 241 has no tensor-core path: NBW would exceed one MMA's N, the FFMA2 kernel takes it)."""
+    other than 200 ticks (K > 241: the tensor-core path cuts the LUT into pieces of 200 ticks, each a row of its own that S5
+    adds; the FFMA2 kernel takes any length as it is)."""
     p = W.default_params(window_pixels=window, lut_ticks=lut_ticks, n_readout_ticks=700 + lut_ticks)
     tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, 20.0, 20, 20, 0)]
     pitch = p["pixel_pitch_cm"]
