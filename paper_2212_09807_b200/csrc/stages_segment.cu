@@ -484,9 +484,20 @@ tile_scatter_kernel(int64_t n_tiles, int32_t *perm /* in: class, out: slot */, i
                     const int2 *__restrict__ tl, TileDesc *td_p, int2 *tl_p, int32_t *tb_mask, int sort)
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= n_tiles) return;
-    const int mask = perm[t];
-    const int slot = sort ? atomicAdd(&hist[16 + mask], 1) : (int)t;
+    const bool valid = t < n_tiles;
+    const int mask = valid ? perm[t] : 16;                            // 16: no tile (its own group below)
+    int slot = (int)t;
+    if (sort) {
+        // one atomic per (warp, class): the lanes of a class take consecutive slots
+        const int lane = threadIdx.x & 31;
+        const unsigned peers = __match_any_sync(0xffffffffu, mask);
+        const int leader = __ffs(peers) - 1;
+        int base = 0;
+        if (lane == leader && valid) base = atomicAdd(&hist[16 + mask], __popc(peers));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        slot = base + __popc(peers & ((1u << lane) - 1u));
+    }
+    if (!valid) return;
     perm[t] = slot;
     td_p[slot] = td[t];
     tl_p[slot] = tl[t];
