@@ -75,7 +75,8 @@ seg_record_kernel(DevParams p, int64_t n, const float *__restrict__ q_anode, con
                   const double *__restrict__ u_e, const double *__restrict__ v_e, const double *__restrict__ T_s,
                   const double *__restrict__ T_e, const int32_t *__restrict__ a_lo, const int32_t *__restrict__ a_hi,
                   const int32_t *__restrict__ b_lo, const int32_t *__restrict__ b_hi, const int32_t *__restrict__ jt0,
-                  const int32_t *__restrict__ jt1, const int32_t *__restrict__ n_samples, SegRec *__restrict__ rec)
+                  const int32_t *__restrict__ jt1, const int32_t *__restrict__ n_samples, SegRec *__restrict__ rec,
+                  long long *composite_flag)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -93,6 +94,14 @@ seg_record_kernel(DevParams p, int64_t n, const float *__restrict__ q_anode, con
                                 fabsf((float)(r.tk_e - r.tk_s)) * r.ist);
     r.N = n_samples[i];
     r.a_lo = a_lo[i]; r.a_hi = a_hi[i]; r.b_lo = b_lo[i]; r.b_hi = b_hi[i]; r.jt0 = jt0[i]; r.jt1 = jt1[i];
+    // a segment beyond the largest rule that is long enough to be cut into runs with a rule each: the splat then runs
+    // its composite instance (COMP below)
+    if (!zero_sigma && r.rho > 16.f && r.N < (1 << 24) && q_anode[i] > 0.f) {
+        const int pieces = min((int)ceilf(r.rho * (1.0f / 16.f)), 64);
+        const float rho = r.rho / (float)pieces;
+        const int k = rho <= 3.5f ? 0 : rho <= 5.5f ? 1 : rho <= 8.f ? 2 : rho <= 12.f ? 3 : rho <= 16.f ? 4 : -1;
+        if (k >= 0 && r.N / pieces >= 3 * c_quad_n[k]) *composite_flag = 1;          // (the choice stage_segment<true> makes)
+    }
     r.flags = (int)(i << 1) | (zero_sigma ? 1 : 0);                  // segment id (n < 2^30) and the sigma = 0 flag
     uint4 *dst = (uint4 *)(rec + i);
     const uint4 *src = (const uint4 *)&r;
@@ -101,6 +110,7 @@ seg_record_kernel(DevParams p, int64_t n, const float *__restrict__ q_anode, con
 }
 
 // record -> tile-relative staging entry; returns the number of operand columns the segment takes in this tile
+template <bool COMP>
 __device__ __forceinline__ int stage_segment(const DevParams &p, const SegRec &r, int s, int NB, int A_t, int B_t, int J_t,
                                              SegLocal &L)
 {
@@ -126,9 +136,17 @@ __device__ __forceinline__ int stage_segment(const DevParams &p, const SegRec &r
     int nq = r.N;
     if (p.rnd_m > 0) nq = r.N * p.rnd_m;                              // eq. (3.9) as printed: one column per perturbed point
     else if (!L.zero_sigma && p.node_rules) {
-        const float rho = r.rho;
+        // COMP: long or sharp segments are cut into `pieces` runs of consecutive midpoints (sizes differing by at most
+        // one), each run with its own rule -- the identity holds run by run; L.rule then also carries the nodes per
+        // piece (<< 8) and pieces - 1 (<< 16)
+        const int pieces = (!COMP || r.rho <= 16.f || r.N >= (1 << 24)) ? 1 : min((int)ceilf(r.rho * (1.0f / 16.f)), 64);
+        const float rho = r.rho / (float)pieces;
         const int k = rho <= 3.5f ? 0 : rho <= 5.5f ? 1 : rho <= 8.f ? 2 : rho <= 12.f ? 3 : rho <= 16.f ? 4 : -1;
-        if (k >= 0 && r.N >= 3 * c_quad_n[k]) { L.rule = c_quad_off[k]; nq = c_quad_n[k]; }
+        if (k >= 0 && r.N / pieces >= 3 * c_quad_n[k]) {
+            L.rule = c_quad_off[k];
+            nq = pieces * c_quad_n[k];
+            if (COMP) L.rule |= (c_quad_n[k] << 8) | ((pieces - 1) << 16);
+        }
     }
     return (L.jlo > L.jhi || L.alo > L.ahi || L.blo > L.bhi) ? 0 : nq;  // box misses this tile: no columns
 }
@@ -147,7 +165,8 @@ __device__ __forceinline__ void cp_async4(void *smem, const void *gmem)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-template <int NB, bool RND>       // RND: eq. (3.9) as printed, p.rnd_m random perturbations per sample point
+template <int NB, bool RND, bool COMP>   // RND: eq. (3.9) as printed, p.rnd_m random perturbations per sample point
+                                        // COMP: composite node rules for segments beyond the largest rule
 __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const SplatArgs a)
 {
     extern __shared__ unsigned char smem_dyn[];
@@ -240,7 +259,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                         for (int c = 0; c < 6; ++c) dst[c] = __ldg(src + c);
                     }
                     SegLocal L;
-                    n_eff = stage_segment(p, r, r.flags >> 1, NB, A_t, B_t, J_t, L);
+                    n_eff = stage_segment<COMP>(p, r, r.flags >> 1, NB, A_t, B_t, J_t, L);
                     segs[lane] = L;
                 }
                 int inc = n_eff;
@@ -279,9 +298,22 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                     float f = ((float)mu + 0.5f) * (1.0f / (float)L.N), qw = L.q;   // position along the segment, charge
                     if (RND) qw = L.q / (float)p.rnd_m;                            // Q_a / (N M)
                     else if (L.rule >= 0) {
-                        const float4 r = __ldg(&g_quad[L.rule + mu]);
-                        f = r.x;
-                        qw = L.qa * (r.y - r.z * L.inv_n2 + r.w * L.inv_n4);
+                        if (!COMP || (L.rule >> 16) == 0) {
+                            const float4 r = __ldg(&g_quad[(COMP ? (L.rule & 0xff) : L.rule) + mu]);
+                            f = r.x;
+                            qw = L.qa * (r.y - r.z * L.inv_n2 + r.w * L.inv_n4);
+                        } else {
+                            // column mu = node i of piece pc; the piece holds midpoints [s_p, e_p) of the segment's N
+                            // (N < 2^24 there: 32-bit products)
+                            const unsigned rule_n = (unsigned)(L.rule >> 8) & 0xffu, pieces = (unsigned)(L.rule >> 16) + 1u;
+                            const unsigned pc = (unsigned)mu / rule_n;
+                            const int i = mu - (int)(pc * rule_n);
+                            const int s_p = (int)(pc * (unsigned)L.N / pieces), e_p = (int)((pc + 1u) * (unsigned)L.N / pieces);
+                            const float n_p = (float)(e_p - s_p), inv_n = 1.0f / (float)L.N, i2 = 1.0f / (n_p * n_p);
+                            const float4 r = __ldg(&g_quad[(L.rule & 0xff) + i]);
+                            f = ((float)s_p + r.x * n_p) * inv_n;
+                            qw = L.qa * (n_p * inv_n) * (r.y - r.z * i2 + r.w * i2 * i2);
+                        }
                     }
                     // sigma = 0: the bin / tick is an integer decision taken in float64 in the oracle's order
                     int ia = -1, ib = -1, jj = -1;

@@ -68,7 +68,7 @@ constexpr int TC_TILE_BLOCK = 128;   // tiles per tensor-core tile block (MMA M)
 // device counters written by the planning kernels (mirrored to pinned host memory)
 enum {
     CNT_MAX_NPIX = 0, CNT_MAX_TICKS, CNT_ACTIVE_SEGS, CNT_PAIRS, CNT_TILES, CNT_ACTIVE_PIX,
-    CNT_TOTAL_SAMPLES, CNT_TOTAL_NPIX, CNT_OVERFLOW, CNT_COUNT = 16
+    CNT_TOTAL_SAMPLES, CNT_TOTAL_NPIX, CNT_OVERFLOW, CNT_COMPOSITE, CNT_COUNT = 16
 };
 
 struct lartpc_sim {
@@ -97,6 +97,7 @@ struct lartpc_sim {
     std::vector<int64_t> cp_base_h, pix_base_h;   // [n_tpcs + 1] first charged-pixel cell / first pixel of each TPC (host copy)
     int64_t plan_pix_lo = 0, plan_pix_hi = 0;       // pixel range of the TPCs the current plan covers
     int32_t *pack_base = nullptr, *pack_count = nullptr;  int pack_tile_pixels = 0;   // lartpc_pack_hits: readout-tile tables
+    bool need_composite = false;         // some segment of the planned input wants composite node rules (charge_tc.cuh COMP)
     int batch_hint = 0;  size_t batch_hint_ws = 0;   // lartpc_run_spill: TPCs per batch that fitted the workspace last time
     bool tile_sort = true;               // env LARTPC_TILE_SORT=0: identity order, every block kept (measurement aid)
     void *seg_rec = nullptr;  int64_t seg_rec_cap = 0;   // per-segment records of the tensor-core splat (charge_tc.cuh)
@@ -195,6 +196,7 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
                 int tpc_lo, int tpc_hi, lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, cudaStream_t st);
 int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
                          lartpc_signals_t *out, cudaStream_t st);
+int launch_seg_records(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n, cudaStream_t st);
 int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st);
 int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st);
 size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_out);   // returns bytes, 0 on failure

@@ -676,36 +676,30 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
         // tensor-core splat (charge_tc.cuh); other bin counts use the FFMA2 splat below, which writes the same image
         static bool configured_tc = false;
         if (!configured_tc) {
-            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<10, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
-            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<5, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
-            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<10, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
-            LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<5, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
+#define LARTPC_CT_ATTR(NBV, R, C) LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<NBV, R, C>, \
+                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM))
+            LARTPC_CT_ATTR(10, false, false);  LARTPC_CT_ATTR(5, false, false);
+            LARTPC_CT_ATTR(10, true, false);   LARTPC_CT_ATTR(5, true, false);
+            LARTPC_CT_ATTR(10, false, true);   LARTPC_CT_ATTR(5, false, true);
+#undef LARTPC_CT_ATTR
             configured_tc = true;
         }
         if (n >= (1ll << 30) || sim->n_tiles >= INT32_MAX - 8 * (int64_t)sim->sm_count) return LARTPC_ERR_UNSUPPORTED;
-        if (n > sim->seg_rec_cap) {
-            if (sim->seg_rec) cudaFree(sim->seg_rec);
-            sim->seg_rec = nullptr;  sim->seg_rec_cap = 0;
-            LARTPC_CUDA_TRY(cudaMalloc(&sim->seg_rec, sizeof(SegRec) * (size_t)(n + n / 8 + 1024)));
-            sim->seg_rec_cap = n + n / 8 + 1024;
-        }
-        if (n > 0) {
-            ++g_lartpc_launches;
-            seg_record_kernel<<<div_up(n, 256), 256, 0, st>>>(p, n, dr->q_anode, dr->sigma_T, dr->sigma_t, dr->u_s, dr->v_s,
-                                                             dr->u_e, dr->v_e, dr->T_s, dr->T_e, pm->a_lo, pm->a_hi, pm->b_lo,
-                                                             pm->b_hi, pm->jt0, pm->jt1, pm->n_samples, (SegRec *)sim->seg_rec);
-        }
+        if (n > sim->seg_rec_cap) return LARTPC_ERR_ORDER;                // records are written with the plan (launch_seg_records)
         a.rec = sim->seg_rec;  a.work = sim->d_work;  a.n_tiles = (int)sim->n_tiles;
         a.tile_desc = sim->tile_desc_p;  a.tile_list = sim->tile_list_p;        // physical (sorted) tile order
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
         const unsigned grid = (unsigned)std::min<int64_t>(sim->n_tiles, 4 * (int64_t)sim->sm_count);
         ++g_lartpc_launches;
         if (p.rnd_m > 0) {
-            if (p.nb == 10) charge_lattice_tc_kernel<10, true><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
-            else charge_lattice_tc_kernel<5, true><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+            if (p.nb == 10) charge_lattice_tc_kernel<10, true, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+            else charge_lattice_tc_kernel<5, true, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+        } else if (sim->need_composite) {                              // some segment is beyond the largest single rule
+            if (p.nb == 10) charge_lattice_tc_kernel<10, false, true><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+            else charge_lattice_tc_kernel<5, false, true><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
         } else {
-            if (p.nb == 10) charge_lattice_tc_kernel<10, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
-            else charge_lattice_tc_kernel<5, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+            if (p.nb == 10) charge_lattice_tc_kernel<10, false, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
+            else charge_lattice_tc_kernel<5, false, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
         }
         LARTPC_CUDA_TRY(cudaGetLastError());
         return LARTPC_OK;
@@ -719,6 +713,29 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     }
     ++g_lartpc_launches;
     charge_lattice_kernel<<<(unsigned)sim->n_tiles, NT1, smem, st>>>(a);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}
+
+
+// per-segment records of the tensor-core splat, written once per plan of the whole input (launch_plan with tpc_lo = 0);
+// sets d_counters[CNT_COMPOSITE] when some segment wants composite node rules
+int launch_seg_records(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n, cudaStream_t st)
+{
+    const DevParams &p = sim->dp;
+    if (!(p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5)) || n <= 0) return LARTPC_OK;
+    if (n >= (1ll << 30)) return LARTPC_ERR_UNSUPPORTED;
+    if (n > sim->seg_rec_cap) {
+        if (sim->seg_rec) cudaFree(sim->seg_rec);
+        sim->seg_rec = nullptr;  sim->seg_rec_cap = 0;
+        LARTPC_CUDA_TRY(cudaMalloc(&sim->seg_rec, sizeof(SegRec) * (size_t)(n + n / 8 + 1024)));
+        sim->seg_rec_cap = n + n / 8 + 1024;
+    }
+    ++g_lartpc_launches;
+    seg_record_kernel<<<div_up(n, 256), 256, 0, st>>>(p, n, dr->q_anode, dr->sigma_T, dr->sigma_t, dr->u_s, dr->v_s,
+                                                     dr->u_e, dr->v_e, dr->T_s, dr->T_e, pm->a_lo, pm->a_hi, pm->b_lo,
+                                                     pm->b_hi, pm->jt0, pm->jt1, pm->n_samples, (SegRec *)sim->seg_rec,
+                                                     sim->d_counters + CNT_COMPOSITE);
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }

@@ -548,6 +548,8 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
                                                          *out, sim->pix_count, sim->pix_jmin, sim->d_counters);
             LARTPC_CUDA_TRY(cudaGetLastError());
         }
+        // per-segment records of the tensor-core splat: once per plan of the whole input
+        if (tpc_lo == 0 && (rc = launch_seg_records(sim, dr, out, n, st)) != 0) return rc;
         // offsets[n+1] = exclusive scan of npix
         LARTPC_CUDA_TRY(lscan::exclusive_scan(n, NpixF{out->npix}, out->offsets, true,
                                               sim->d_counters + CNT_TOTAL_NPIX, sim->scan_tmp, st));
@@ -593,6 +595,7 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
     const long long *h = sim->h_counters;
     sim->plan_n = n;
     sim->n_tiles = h[CNT_TILES];
+    if (tpc_lo == 0) sim->need_composite = h[CNT_COMPOSITE] != 0;
     if (p.tc_mode && sim->n_tiles > 0) {
         const int sort = sim->tile_sort && sim->splat_tc ? 1 : 0;
         const int64_t nt = sim->n_tiles;
