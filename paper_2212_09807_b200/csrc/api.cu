@@ -480,7 +480,8 @@ extern "C" size_t lartpc_workspace_bytes(const lartpc_sim_t *sim, int64_t max_se
     // depend on the data; on the BASELINE configs there are up to ~1.5 tiles per segment of a batch, so 2 GiB +
     // 16 KiB per segment lets run_spill take several TPCs per batch; it halves its batches until they fit whatever
     // it is given (one TPC of configs[3] needs ~6 GiB).
-    return (size_t)max_segments * (160 + 16384) + ((size_t)2 << 30);
+    // (a LUT cut into pieces has one partial row per piece: 26.4 KB more per tile and piece)
+    return (size_t)max_segments * (160 + 16384 + (size_t)(sim->dp.tc_mode ? sim->dp.nq - 1 : 0) * 40000) + ((size_t)2 << 30);
 }
 
 extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg, int64_t n, uint64_t seed,

@@ -97,6 +97,7 @@ struct lartpc_sim {
     std::vector<int64_t> cp_base_h, pix_base_h;   // [n_tpcs + 1] first charged-pixel cell / first pixel of each TPC (host copy)
     int64_t plan_pix_lo = 0, plan_pix_hi = 0;       // pixel range of the TPCs the current plan covers
     int32_t *pack_base = nullptr, *pack_count = nullptr;  int pack_tile_pixels = 0;   // lartpc_pack_hits: readout-tile tables
+    int64_t boxes_n = -1;  const void *boxes_of = nullptr;   // input whose S3 boxes the last tpc_lo = 0 plan wrote (reused by later batches)
     bool need_composite = false;         // some segment of the planned input wants composite node rules (charge_tc.cuh COMP)
     int batch_hint = 0;  size_t batch_hint_ws = 0;   // lartpc_run_spill: TPCs per batch that fitted the workspace last time
     bool tile_sort = true;               // env LARTPC_TILE_SORT=0: identity order, every block kept (measurement aid)

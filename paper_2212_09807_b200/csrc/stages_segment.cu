@@ -211,17 +211,28 @@ __device__ __forceinline__ long long warp_sum_ll(long long v)
 __global__ void __launch_bounds__(256)
 pixmap_kernel(DevParams p, const DevTpc *__restrict__ tpcs, SegPtrs s, int64_t n, const int32_t *__restrict__ seg_tpc,
               const float *__restrict__ q_anode, int tpc_lo, int tpc_hi, lartpc_pixmap_t o,
-              int32_t *pix_count, int32_t *pix_jmin, long long *counters)
+              int32_t *pix_count, int32_t *pix_jmin, long long *counters, int reuse)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     long long m_npix = 0, m_ticks = 0, n_act = 0, n_pairs = 0;
     if (i < n) {
         int tpc = seg_tpc[i];
         SegBox b;
-        seg_box(p, tpcs, tpc, q_anode[i], s.xs[i], s.ys[i], s.zs[i], s.ts[i], s.xe[i], s.ye[i], s.ze[i], s.te[i], b);
-        o.a_lo[i] = b.a_lo; o.a_hi[i] = b.a_hi; o.b_lo[i] = b.b_lo; o.b_hi[i] = b.b_hi;
-        o.ix0[i] = b.ix0; o.ix1[i] = b.ix1; o.iy0[i] = b.iy0; o.iy1[i] = b.iy1;
-        o.jt0[i] = b.jt0; o.jt1[i] = b.jt1; o.npix[i] = b.npix; o.n_samples[i] = b.n_samples;
+        if (reuse) {
+            // a later TPC batch of the same input (lartpc_run_spill): the boxes are those the first batch wrote
+            b.deposits = false;
+            b.npix = 0;
+            if (tpc >= tpc_lo && tpc < tpc_hi) {
+                b.a_lo = o.a_lo[i]; b.a_hi = o.a_hi[i]; b.b_lo = o.b_lo[i]; b.b_hi = o.b_hi[i];
+                b.jt0 = o.jt0[i]; b.jt1 = o.jt1[i]; b.npix = o.npix[i];
+                if (b.npix > 0) chunk_and_cp_range(p, tpcs[tpc], b);
+            }
+        } else {
+            seg_box(p, tpcs, tpc, q_anode[i], s.xs[i], s.ys[i], s.zs[i], s.ts[i], s.xe[i], s.ye[i], s.ze[i], s.te[i], b);
+            o.a_lo[i] = b.a_lo; o.a_hi[i] = b.a_hi; o.b_lo[i] = b.b_lo; o.b_hi[i] = b.b_hi;
+            o.ix0[i] = b.ix0; o.ix1[i] = b.ix1; o.iy0[i] = b.iy0; o.iy1[i] = b.iy1;
+            o.jt0[i] = b.jt0; o.jt1[i] = b.jt1; o.npix[i] = b.npix; o.n_samples[i] = b.n_samples;
+        }
         if (b.npix > 0) {
             m_npix = b.npix;
             m_ticks = (long long)(b.jt1 - b.jt0 + 1) + p.K - 1;
@@ -530,6 +541,9 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
     const int64_t cp_lo = sim->cp_base_h[tpc_lo], ncp = sim->cp_base_h[tpc_hi] - cp_lo;
     const int64_t pix_lo = sim->pix_base_h[tpc_lo], npix = sim->pix_base_h[tpc_hi] - pix_lo;
     sim->plan_pix_lo = pix_lo;  sim->plan_pix_hi = pix_lo + npix;
+    // a later TPC batch of the input whose boxes the tpc_lo = 0 plan wrote into these very arrays (lartpc_run_spill)
+    const int reuse = (tpc_lo > 0 && sim->boxes_n == n && sim->boxes_of == (const void *)out->a_lo && n > 0) ? 1 : 0;
+    if (tpc_lo == 0) { sim->boxes_n = -1;  sim->boxes_of = nullptr; }
 
     for (int attempt = 0; attempt < 2; ++attempt) {
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_counters, 0, sizeof(long long) * CNT_COUNT, st));
@@ -545,14 +559,15 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         if (n > 0) {
             ++g_lartpc_launches;
             pixmap_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, s, n, dr->tpc, dr->q_anode, tpc_lo, tpc_hi,
-                                                         *out, sim->pix_count, sim->pix_jmin, sim->d_counters);
+                                                         *out, sim->pix_count, sim->pix_jmin, sim->d_counters, reuse);
             LARTPC_CUDA_TRY(cudaGetLastError());
         }
         // per-segment records of the tensor-core splat: once per plan of the whole input
         if (tpc_lo == 0 && (rc = launch_seg_records(sim, dr, out, n, st)) != 0) return rc;
         // offsets[n+1] = exclusive scan of npix
-        LARTPC_CUDA_TRY(lscan::exclusive_scan(n, NpixF{out->npix}, out->offsets, true,
-                                              sim->d_counters + CNT_TOTAL_NPIX, sim->scan_tmp, st));
+        if (!reuse)
+            LARTPC_CUDA_TRY(lscan::exclusive_scan(n, NpixF{out->npix}, out->offsets, true,
+                                                  sim->d_counters + CNT_TOTAL_NPIX, sim->scan_tmp, st));
         // per charged pixel: start of its segment list
         LARTPC_CUDA_TRY(lscan::exclusive_scan(ncp, NpixF{sim->pix_count + cp_lo}, sim->pix_start + cp_lo, false,
                                               (long long *)nullptr, sim->scan_tmp, st));
@@ -595,7 +610,7 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
     const long long *h = sim->h_counters;
     sim->plan_n = n;
     sim->n_tiles = h[CNT_TILES];
-    if (tpc_lo == 0) sim->need_composite = h[CNT_COMPOSITE] != 0;
+    if (tpc_lo == 0) { sim->need_composite = h[CNT_COMPOSITE] != 0;  sim->boxes_n = n;  sim->boxes_of = (const void *)out->a_lo; }
     if (p.tc_mode && sim->n_tiles > 0) {
         const int sort = sim->tile_sort && sim->splat_tc ? 1 : 0;
         const int64_t nt = sim->n_tiles;
