@@ -18,18 +18,20 @@
 // parts carry the extra powers of two below, which cancel in the product; the epilogue undoes the rest exactly.
 //
 // Kernel (persistent, one CTA per SM, 192 threads, whole TMEM):
-//   warp 0, one lane   producer: per (item = (tile block, d), bin c) one cp.async.bulk of the A image (hi + lo, 32 KB,
-//                      written by charge_lattice_kernel already in the 128-byte-swizzled K-major UMMA layout) and one of
-//                      the Bs image (hi + lo, 14 KB, canonical un-swizzled K-major layout built at create) into a ring
-//                      of 4 shared-memory stages, completion on an mbarrier per stage
-//   warp 1, one lane   MMA issuer: 8 tcgen05.mma (M = 128, N = NBW; 4 blocks b x (fp16 K = 16 + fp8 K = 32)) per
-//                      stage, tcgen05.commit frees the stage; after the last bin a commit signals the epilogue
-//   warps 2-5          epilogue: tcgen05.ld the 128 x 264 fp32 accumulator (thread = tile row), undo the scales, write
-//                      the partial waveform rows, re-zero the TMEM columns that only later blocks b touch
-// Items are taken from an atomic cursor by the producer (which hands the item to the MMA warp in a stage header and
-// from there to the epilogue), consecutive items share the tile block, so the 25 CTAs that stream one A block do it at
-// the same time and A is read from HBM once.  (A static round-robin deal lets the CTAs drift apart over a long
-// launch: measured, the L2 reuse of A is lost and the kernel becomes HBM-bound.)
+//   warp 0, one lane   producer: per (item, bin c) one cp.async.bulk per charged 16-tick block of the A image (8 KB each:
+//                      fp16 part + fp8 part, un-swizzled K-major, written by charge_lattice_tc_kernel) and one of the Bs
+//                      image (14 KB) into a ring of 3 shared-memory stages, completion on an mbarrier per stage
+//   warp 1, one lane   MMA issuer: per charged block one fp16 (K = 16) and one fp8 (K = 32) tcgen05.mma (M = 128, N = NBW),
+//                      tcgen05.commit frees the stage; after the last bin a commit signals the epilogue
+//   warps 2-5          epilogue: tcgen05.ld the fp32 accumulator(s) (thread = tile row), undo the scales, write the
+//                      partial waveform rows, zero the accumulator columns again (every MMA accumulates)
+// An item is (tile block, row d of the LUT image) -- or TWO neighbouring tile blocks with the same d when each charges at
+// most three consecutive 16-tick blocks (tiles are sorted by the blocks they charge, so most do): their accumulators,
+// 32 + NBW = 256 columns each counted from the first charged block, share the 512 TMEM columns and every Bs image is
+// fetched once for both.  Items are taken from an atomic cursor by the producer (which hands the item to the MMA warp in a
+// stage header and from there to the epilogue); consecutive items share their charge blocks, so the CTAs that stream one
+// tile block do it at the same time and A is read from HBM once.  (A static round-robin deal lets the CTAs drift apart
+// over a long launch: measured, the L2 reuse of A is lost and the kernel becomes HBM-bound.)
 #pragma once
 #include <cuda_fp16.h>
 #include <cuda_fp8.h>
@@ -40,7 +42,8 @@ namespace rtc {
 constexpr int TB = 128;            // tiles per tile block (MMA M)
 constexpr int JC = 64;             // arrival ticks per tile (K extent per bin): 4 blocks of 16
 constexpr int NBLK = JC / 16;
-constexpr int STAGES = 4;
+constexpr int STAGES = 3;
+constexpr int A_SLOTS = 6;          // charge blocks a stage can hold: 4 of one tile block, or 3 + 3 of a pair
 constexpr int THREADS = 192;
 constexpr int B_SCALE_LOG2 = 10;
 // fp8 parts: lo8(A) = e4m3(lo(A) 2^SA) meets hi8(B) = e4m3(B 2^-SA); hi8(A) = e4m3(A 2^-SB) meets lo8(B) = e4m3(lo(B) 2^SB)
@@ -55,7 +58,7 @@ struct Args {
     const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), 0
     const int32_t *tb_mask;        // [n_tb] 16-tick blocks that hold charge in any tile of the block (bit b)
     int n_tiles, n_tb, NC, WW, NBW, tile_ticks;
-    long long n_items;             // n_tb * WW
+    long long n_items;             // ceil(n_tb / 2) * WW * 2: (unit of two tile blocks, row, half)
     int *work;                     // item cursor, zero at launch: items are taken in order as CTAs become free, so the
                                    // CTAs that stream one tile block stay together however long the launch runs
 };
@@ -189,25 +192,34 @@ __device__ __forceinline__ void tmem_zero16(uint32_t taddr)
         "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};\n" ::"r"(taddr), "r"(z) : "memory");
 }
 
-constexpr int stage_bytes(int NBW) { return 2 * A_HALF_BYTES + 2 * NBW * 32; }
+constexpr int stage_bytes(int NBW) { return A_SLOTS * A_BLOCK_BYTES + 2 * NBW * 32; }
 constexpr int smem_bytes(int NBW) { return STAGES * stage_bytes(NBW) + 1024 /* alignment slack */ + 256 /* barriers, headers */; }
 constexpr int HDR_LAST = 1, HDR_END = 2;
+constexpr int PAIR_COL = 256;      // TMEM column of the second accumulator of a pair item
 
+// Two tile blocks share an item -- and with it every LUT generator the item streams -- when each charges at most three
+// consecutive 16-tick blocks: an accumulator then needs 32 + NBW <= 256 columns (counted from the block's first charged
+// block), and two fit the 512 TMEM columns.
+__device__ __forceinline__ bool pairable_mask(int m) { return m != 0 && (31 - __clz(m)) - (__ffs(m) - 1) <= 2; }
+
+// Work items.  Unit u = tile blocks 2u, 2u + 1; cursor value q = (u * rows + d) * 2 + h.  A pairable unit is one item per
+// row d (h = 0; h = 1 is skipped); otherwise h picks the tile block.  Consecutive q share their charge blocks.
 __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
 {
     extern __shared__ unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int NBW = a.NBW, NC = a.NC;
     const uint32_t b_half = (uint32_t)NBW * 32u;                       // bytes of one precision half of a Bs image
-    const uint32_t stage_sz = 2u * A_HALF_BYTES + 2u * b_half;         // multiple of 1024 (NBW multiple of 16)
-    // SWIZZLE_128B operands need 1024-byte aligned tiles
+    const uint32_t a_area = (uint32_t)A_SLOTS * A_BLOCK_BYTES;
+    const uint32_t stage_sz = a_area + 2u * b_half;                    // multiple of 1024 (NBW multiple of 16)
     const uint32_t base = (s32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bars = base + STAGES * stage_sz;                    // full[S], empty[S], tmem_full, tmem_empty, tmem ptr
     const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull = bars + 16 * STAGES, tempty = tfull + 8;
     const uint32_t titem = tempty + 8, tptr_addr = titem + 8;
     volatile uint32_t *tptr = (volatile uint32_t *)(smem_raw + (tptr_addr - s32(smem_raw)));
-    volatile int4 *hdr = (volatile int4 *)(smem_raw + (tptr_addr + 8 - s32(smem_raw)));   // [STAGES] {tb, d, c, flags}
-    volatile int4 *epi_item = hdr + STAGES;                                              // {tb, d, 0, flags}
+    volatile int4 *hdr = (volatile int4 *)(smem_raw + (tptr_addr + 8 - s32(smem_raw)));   // [STAGES] {tbA, d, c | masks, flags}
+    volatile int4 *epi_item = hdr + STAGES;                                              // {tbA, d, masks, flags}
+    const bool pairs_fit = 32 + NBW <= PAIR_COL;
 
     if (tid == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
@@ -224,7 +236,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tptr;
-    const int n_acc_cols = 16 * (NBLK - 1) + NBW;                      // accumulator columns in use (272)
+    const int n_acc_cols = 16 * (NBLK - 1) + NBW;                      // columns of a single item's accumulator (272)
 
     if (warp == 0) {
         // ------------------------------------------------------------------ producer
@@ -234,21 +246,34 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
             long long q = atomicAdd(a.work, 1);
             while (q < a.n_items) {
                 const long long q_next = atomicAdd(a.work, 1);         // in flight while this item streams
-                const int tb = (int)(q / a.WW), d = (int)(q - (long long)tb * a.WW);
-                const unsigned char *Ab = (const unsigned char *)a.A + (size_t)tb * NC * (2 * A_HALF_BYTES);
+                const int h = (int)(q & 1);
+                const long long ud = q >> 1;
+                const int u = (int)(ud / a.WW), d = (int)(ud - (long long)u * a.WW);
+                const int tb0 = 2 * u, tb1 = tb0 + 1;
+                const int m0 = a.tb_mask[tb0] & ((1 << NBLK) - 1), m1 = tb1 < a.n_tb ? a.tb_mask[tb1] & ((1 << NBLK) - 1) : 0;
+                const bool pair = pairs_fit && pairable_mask(m0) && pairable_mask(m1);
+                int tbA, bmA, bmB = 0;
+                if (pair) { tbA = tb0;  bmA = m0;  bmB = m1; }
+                else { tbA = h ? tb1 : tb0;  bmA = h ? m1 : m0; }
+                if ((pair && h) || bmA == 0) { q = q_next;  continue; }   // the pair went out with h = 0; nothing charged
+                const unsigned char *AbA = (const unsigned char *)a.A + (size_t)tbA * NC * (NBLK * A_BLOCK_BYTES);
+                const unsigned char *AbB = AbA + (size_t)NC * (NBLK * A_BLOCK_BYTES);   // tile block tbA + 1
                 const unsigned char *Bb = (const unsigned char *)a.B + (size_t)d * NC * (2 * b_half);
-                const int bm = a.tb_mask[tb] & ((1 << NBLK) - 1);
-                const uint32_t a_bytes = (uint32_t)__popc(bm) * A_BLOCK_BYTES;
-                for (int c = 0; c < NC && bm; ++c) {
+                const uint32_t a_bytes = (uint32_t)(__popc(bmA) + __popc(bmB)) * A_BLOCK_BYTES;
+                for (int c = 0; c < NC; ++c) {
                     mbar_wait(empty0 + 8 * s, ph ^ 1u);
                     const uint32_t st = base + s * stage_sz, fb = full0 + 8 * s;
-                    hdr[s].x = tb;  hdr[s].y = d;  hdr[s].z = c | (bm << 16);  hdr[s].w = (c == NC - 1) ? HDR_LAST : 0;
+                    hdr[s].x = tbA;  hdr[s].y = d;  hdr[s].z = c | (bmA << 16) | (bmB << 20);
+                    hdr[s].w = (c == NC - 1) ? HDR_LAST : 0;
                     mbar_expect_tx(fb, a_bytes + 2 * b_half);          // release: the header is visible to the waiter
-                    const unsigned char *Ac = Ab + (size_t)c * (NBLK * A_BLOCK_BYTES);
+                    uint32_t dst = st;
 #pragma unroll
                     for (int b = 0; b < NBLK; ++b)
-                        if (bm >> b & 1) bulk_g2s(st + b * A_BLOCK_BYTES, Ac + b * A_BLOCK_BYTES, A_BLOCK_BYTES, fb);
-                    bulk_g2s(st + 2 * A_HALF_BYTES, Bb + (size_t)c * (2 * b_half), 2 * b_half, fb);
+                        if (bmA >> b & 1) { bulk_g2s(dst, AbA + ((size_t)c * NBLK + b) * A_BLOCK_BYTES, A_BLOCK_BYTES, fb);  dst += A_BLOCK_BYTES; }
+#pragma unroll
+                    for (int b = 0; b < NBLK; ++b)
+                        if (bmB >> b & 1) { bulk_g2s(dst, AbB + ((size_t)c * NBLK + b) * A_BLOCK_BYTES, A_BLOCK_BYTES, fb);  dst += A_BLOCK_BYTES; }
+                    bulk_g2s(st + a_area, Bb + (size_t)c * (2 * b_half), 2 * b_half, fb);
                     if (++s == STAGES) { s = 0; ph ^= 1u; }
                 }
                 q = q_next;
@@ -267,8 +292,8 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
             uint32_t ph = 0, tph = 0;
             while (true) {
                 mbar_wait(full0 + 8 * s, ph);
-                const int tb = hdr[s].x, d = hdr[s].y, cz = hdr[s].z, flags = hdr[s].w;
-                const int c = cz & 0xffff, bm = cz >> 16;
+                const int tbA = hdr[s].x, d = hdr[s].y, cz = hdr[s].z, flags = hdr[s].w;
+                const int c = cz & 0xffff, bmA = (cz >> 16) & 15, bmB = (cz >> 20) & 15;
                 if (flags & HDR_END) {
                     mbar_wait(tempty, tph);                            // the epilogue has read the previous item slot
                     epi_item->w = HDR_END;
@@ -276,25 +301,35 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                     break;
                 }
                 if (c == 0) {
-                    mbar_wait(tempty, tph);                            // accumulator drained and zeroed
-                    epi_item->x = tb;  epi_item->y = d;  epi_item->w = 0;
+                    mbar_wait(tempty, tph);                            // accumulators drained and zeroed
+                    epi_item->x = tbA;  epi_item->y = d;  epi_item->z = bmA | (bmB << 4);  epi_item->w = 0;
                     mbar_arrive(titem);                                // release: hands the item to the epilogue
                 }
                 tc_fence_after();
                 const uint32_t st = base + s * stage_sz;
-                const uint64_t bd_hi = smem_desc(st + 2 * A_HALF_BYTES, 128, 256, 0);
-                const uint64_t bd_8 = smem_desc(st + 2 * A_HALF_BYTES + b_half, 128, 256, 0);
+                const uint64_t bd_hi = smem_desc(st + a_area, 128, 256, 0);
+                const uint64_t bd_8 = smem_desc(st + a_area + b_half, 128, 256, 0);
+                // single item: block b lands at column 16 b; pair: at 16 (b - first charged block) of its own accumulator
+                const int lbA = bmB ? __ffs(bmA) - 1 : 0, lbB = bmB ? __ffs(bmB) - 1 : 0;
+                uint32_t src = st;
 #pragma unroll
                 for (int b = 0; b < NBLK; ++b) {
-                    if (!(bm >> b & 1)) continue;                      // no tile of the block has charge in these 16 ticks
-                    const uint64_t ad_hi = smem_desc(st + b * A_BLOCK_BYTES, 128, 256, 0);
-                    const uint64_t ad_8 = smem_desc(st + b * A_BLOCK_BYTES + A_PART_BYTES, 128, 256, 0);
-                    const uint32_t dcol = tmem + 16 * b;
-                    tc_mma_f16(dcol, ad_hi, bd_hi, idesc, 1u);         // the epilogue leaves the whole accumulator zero
-                    tc_mma_f8(dcol, ad_8, bd_8, idesc, 1u);
+                    if (!(bmA >> b & 1)) continue;                     // no tile of the block has charge in these 16 ticks
+                    const uint32_t dcol = tmem + 16 * (b - lbA);
+                    tc_mma_f16(dcol, smem_desc(src, 128, 256, 0), bd_hi, idesc, 1u);   // the epilogue leaves the accumulators zero
+                    tc_mma_f8(dcol, smem_desc(src + A_PART_BYTES, 128, 256, 0), bd_8, idesc, 1u);
+                    src += A_BLOCK_BYTES;
+                }
+#pragma unroll
+                for (int b = 0; b < NBLK; ++b) {
+                    if (!(bmB >> b & 1)) continue;
+                    const uint32_t dcol = tmem + PAIR_COL + 16 * (b - lbB);
+                    tc_mma_f16(dcol, smem_desc(src, 128, 256, 0), bd_hi, idesc, 1u);
+                    tc_mma_f8(dcol, smem_desc(src + A_PART_BYTES, 128, 256, 0), bd_8, idesc, 1u);
+                    src += A_BLOCK_BYTES;
                 }
                 tc_commit(empty0 + 8 * s);                             // stage free once these MMAs have read it
-                if (flags & HDR_LAST) { tc_commit(tfull); tph ^= 1u; } // accumulator complete
+                if (flags & HDR_LAST) { tc_commit(tfull); tph ^= 1u; } // accumulators complete
                 if (++s == STAGES) { s = 0; ph ^= 1u; }
             }
         }
@@ -302,48 +337,64 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
         // ------------------------------------------------------------------ epilogue (warps 2-5)
         const int quad = warp & 3;                                     // TMEM lanes [32 quad, 32 quad + 32)
         const uint32_t tlane = tmem + ((uint32_t)(32 * quad) << 16);
-        // every MMA accumulates: the accumulator is zero before the first item and zeroed again after each read-out
-        for (int c0 = 0; c0 < n_acc_cols; c0 += 16) tmem_zero16(tlane + c0);
+        // every MMA accumulates: the accumulators are zero before the first item and zeroed again after each read-out
+        for (int c0 = 0; c0 < 512; c0 += 16) tmem_zero16(tlane + c0);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty);
         uint32_t tph = 0;
-        const int n_full = a.tile_ticks / 32, n_rem = a.tile_ticks - 32 * n_full;   // tile_ticks = 264: 8 x 32 + 8
         while (true) {
             mbar_wait(titem, tph);                                     // acquire: the MMA warp has published the item
             if (epi_item->w & HDR_END) break;
-            const int tb = epi_item->x, d = epi_item->y;
-            const int tile = tb * TB + 32 * quad + lane;
-            const bool live = tile < a.n_tiles;
-            float scale = 0.f;
-            if (live) scale = __int_as_float((127 + a.tile_meta[4 * tile + 2] - B_SCALE_LOG2) << 23);
-            float *dst = a.partial + ((size_t)(live ? tile : 0) * a.WW + d) * a.tile_ticks;
+            const int tbA = epi_item->x, d = epi_item->y, masks = epi_item->z;
+            const int bmA = masks & 15, bmB = (masks >> 4) & 15;
+            const int n_acc = bmB ? 2 : 1;
             mbar_wait(tfull, tph);
             tc_fence_after();
-            for (int ch = 0; ch < n_full; ++ch) {
-                uint32_t v[32];
-                tmem_ld32(tlane + 32 * ch, v);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (live) {
-#pragma unroll
-                    for (int i = 0; i < 8; ++i)
-                        __stcs((float4 *)(dst + 32 * ch) + i, make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
-                                                                     __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale));
+            for (int x = 0; x < n_acc; ++x) {
+                // accumulator x: tile block tbA + x; its column 0 is tick t0 of the tile's window
+                const int tile = (tbA + x) * TB + 32 * quad + lane;
+                const bool live = tile < a.n_tiles;
+                const int t0 = bmB ? 16 * (__ffs(x ? bmB : bmA) - 1) : 0;
+                const int n_cols = bmB ? min(PAIR_COL, a.tile_ticks - t0) : a.tile_ticks;     // multiples of 8
+                const uint32_t tcol = tlane + (x ? PAIR_COL : 0);
+                float scale = 0.f;
+                if (live) scale = __int_as_float((127 + a.tile_meta[4 * tile + 2] - B_SCALE_LOG2) << 23);
+                float *dst = a.partial + ((size_t)(live ? tile : 0) * a.WW + d) * a.tile_ticks + t0;
+                if (bmB && live) {
+                    // S5 reads whole 14-tick blocks around the charged range: the few ticks of the row the accumulator
+                    // does not cover (before the first charged block, after column 255) are zero
+                    float *row = dst - t0;
+                    for (int i = 0; i < t0; i += 4) __stcs((float4 *)(row + i), make_float4(0.f, 0.f, 0.f, 0.f));
+                    for (int i = t0 + n_cols; i < a.tile_ticks; i += 4) __stcs((float4 *)(row + i), make_float4(0.f, 0.f, 0.f, 0.f));
                 }
-            }
-            if (n_rem) {
-                uint32_t v[8];
-                tmem_ld8(tlane + 32 * n_full, v);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (live) {
+                const int n_full = n_cols / 32;
+                for (int ch = 0; ch < n_full; ++ch) {
+                    uint32_t v[32];
+                    tmem_ld32(tcol + 32 * ch, v);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    if (live) {
 #pragma unroll
-                    for (int i = 0; i < 2; ++i)
-                        __stcs((float4 *)(dst + 32 * n_full) + i, make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
+                        for (int i = 0; i < 8; ++i)
+                            __stcs((float4 *)(dst + 32 * ch) + i, make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
                                                                          __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale));
+                    }
+                }
+                for (int c0 = 32 * n_full; c0 < n_cols; c0 += 8) {
+                    uint32_t v[8];
+                    tmem_ld8(tcol + c0, v);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    if (live) {
+#pragma unroll
+                        for (int i = 0; i < 2; ++i)
+                            __stcs((float4 *)(dst + c0) + i, make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
+                                                                    __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale));
+                    }
                 }
             }
-            for (int c0 = 0; c0 < n_acc_cols; c0 += 16) tmem_zero16(tlane + c0);
+            const int n_zero = bmB ? 512 : n_acc_cols;
+            for (int c0 = 0; c0 < n_zero; c0 += 16) tmem_zero16(tlane + c0);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();

@@ -812,7 +812,7 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     a.n_tiles = (int)sim->n_tiles;
     a.n_tb = (int)((sim->n_tiles + rtc::TB - 1) / rtc::TB);
     a.NC = p.NB2;  a.WW = p.WW * p.nq;  a.NBW = p.NBW;  a.tile_ticks = p.tile_ticks;   // a row = (target, LUT piece)
-    a.n_items = (long long)a.n_tb * a.WW;
+    a.n_items = (long long)((a.n_tb + 1) / 2) * a.WW * 2;                 // (unit of two tile blocks, row, half): response_tc.cuh
     if (a.n_items >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.work = sim->d_work;
     LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
