@@ -323,7 +323,8 @@ def run_ours(args):
             "config": {"workload": WORKLOAD_NAMES[args.config], "n_segments": n, "n_pixels": wl.n_pixels,
                        "n_readout_ticks": int(wl.params["n_readout_ticks"]), "n_tpcs": len(wl.tpcs),
                        "seed": wl.seed, "l2": "256 MiB flush write between timed steps",
-                       "parallelism": "independent spill per GPU" if world > 1 else "single GPU"},
+                       "parallelism": "independent spill per GPU" if world > 1 else "single GPU",
+                       "input_sha256": {k: v[:16] for k, v in wl.sha256().items()}},
             "stats": {"n_tiles": int(st.n_tiles), "n_pairs": int(st.n_pairs), "n_active_pixels": int(st.n_active_pixels),
                       "total_samples": int(st.total_samples), "n_hits": int(st.n_hits),
                       "n_hits_dropped": int(st.n_hits_dropped), "n_batches": int(st.n_batches)},
