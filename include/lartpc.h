@@ -26,7 +26,8 @@
  *     max_hits_per_pixel hits on a pixel) are counted in the output bundle / stats and never write
  *     out of bounds.
  *   - There is no CPU fallback and no dispatch: lartpc_sim_create fails unless the current device
- *     has compute capability 10.x.
+ *     has compute capability 10.x.  The library reads no environment variable: which kernel runs is decided by
+ *     the parameters and the response mode alone.
  *   - A lartpc_sim_t holds the plan made by S3 for ONE batch of segments; S4/S5/S6 must follow on
  *     the same sim, in order, before the next S3.  A sim is not re-entrant across streams.
  */
@@ -194,7 +195,12 @@ typedef struct {
 /* Copies params, the TPC table and the response LUT (HOST pointer, float32 [W*nb][W*nb][K], tick
  * fastest, R[cy][cx][k] = electrons induced during LUT tick k on the centre pixel of the W x W window by
  * one electron above bin (cx, cy) that arrives during LUT tick K-1, D4, D5).  lut_elems must
- * equal (W*nb)^2 * K. */
+ * equal (W*nb)^2 * K (else LARTPC_ERR_LUT_SHAPE).  Values: any finite float32 in any units; the tensor-core response
+ * scales the table by a power of two chosen from max |R| (so a table in other units than the harness's "electrons per
+ * electron" keeps the same relative accuracy); a NaN or infinite entry is LARTPC_ERR_BAD_ARGUMENT.  Entries below
+ * 2^-21 max |R| keep their value to fp16-subnormal precision only (absolute error <= 2^-35 max |R|).
+ * The sim lives on the CUDA device that is current at creation; every later call runs there whatever the caller's
+ * current device is (several sims on several devices may coexist in one process). */
 int  lartpc_sim_create(const lartpc_params_t *params, const lartpc_tpc_t *tpcs, int n_tpcs,
                        const float *response_lut_host, size_t lut_elems, lartpc_sim_t **out);
 void lartpc_sim_destroy(lartpc_sim_t *sim);

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblartpc.so")
 SOURCES = ["api.cu", "stages_segment.cu", "stage_current.cu", "stages_pixel.cu"]
-HEADERS = ["common.cuh", "scan.cuh", os.path.join("..", "..", "include", "lartpc.h")]
+HEADER = os.path.join(HERE, "..", "include", "lartpc.h")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -18,15 +18,16 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh"))] + [HEADER]
+    return any(os.path.getmtime(f) > t for f in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile with nvcc for sm_100a (cross-compiles without a GPU)."""
+def build(force: bool = False, verbose: bool = False, extra=()) -> str:
+    """Compile with nvcc for sm_100a (cross-compiles without a GPU).  `extra`: more nvcc flags, e.g.
+    ("-DLARTPC_DEBUG_CLOCKS",) for a measurement build -- an explicit argument, never the environment."""
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        extra = os.environ.get("LARTPC_NVCC_EXTRA", "").split()       # e.g. -DLARTPC_DEBUG_CLOCKS (measurement builds)
-        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
+        cmd = [nvcc] + NVCC_FLAGS + list(extra) + (["-Xptxas", "-v"] if verbose else []) + \
               [os.path.join(CSRC, f) for f in SOURCES] + ["-o", LIB]
         subprocess.check_call(cmd)
     return LIB

@@ -3,7 +3,9 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <math.h>
 #include <algorithm>
+#include <cmath>
 #include <new>
 #include "common.cuh"
 
@@ -39,6 +41,7 @@ extern "C" const char *lartpc_strerror(int code)
 static void sim_free(lartpc_sim *s)
 {
     if (!s) return;
+    DeviceGuard dg(s->device);
     cudaFree(s->d_tpcs); cudaFree(s->d_lut); cudaFree(s->d_lut_tc);
     cudaFree(s->pix_count); cudaFree(s->pix_start); cudaFree(s->pix_tile0); cudaFree(s->pix_cursor);
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
@@ -136,8 +139,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     s->params = *prm;
     s->tpcs.assign(tpcs, tpcs + n_tpcs);
     s->sm_count = prop.multiProcessorCount;
-    { const char *e = getenv("LARTPC_SPLAT"); s->splat_tc = !(e && strcmp(e, "ffma") == 0); }   // measurement aid
-    { const char *e = getenv("LARTPC_TILE_SORT"); s->tile_sort = !(e && strcmp(e, "0") == 0); } // measurement aid
+    s->device = dev;
     DevParams &p = s->dp;
     memset(&p, 0, sizeof(p));
     p.eps = prm->e_field_kv_cm * prm->lar_density_g_cm3;  p.w_ion = prm->w_ion_mev;
@@ -146,7 +148,6 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     p.d_tran = prm->d_tran_cm2_us; p.dt = prm->tick_us; p.t_origin = prm->t_origin_us; p.pitch = prm->pixel_pitch_cm;
     p.bin = prm->pixel_pitch_cm / (double)nb;  p.sample_step = prm->sample_step_cm;  p.n_sigma_map = prm->n_sigma_map;
     p.recomb_model = prm->recomb_model;
-    { const char *e = getenv("LARTPC_NODE_RULES"); p.node_rules = !(e && strcmp(e, "0") == 0); }  // measurement aid
     p.nb = nb; p.W = W; p.H = (W - 1) / 2; p.K = K; p.WW = W * W; p.NB2 = nb * nb;
     p.n_ticks = prm->n_readout_ticks;  p.j_max = p.n_ticks - K;
     // S4 geometry.  A response task is (pair of target pixels, RESP_NO output ticks); the consumer threads of one CTA
@@ -156,8 +157,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     while ((p.RS & 1) != 0 || ((p.RS >> 1) & 1) == 0) ++p.RS;               // RS = 2 * odd: conflict-free LDS.128 rows
     const int n_pairs = (p.WW + 1) / 2, ncons = RESP_CONSUMERS;
     const size_t smem_limit = (size_t)prop.sharedMemPerBlockOptin;
-    int jc_cap = 120;
-    { const char *e = getenv("LARTPC_JC_CAP"); if (e && atoi(e) >= 8) jc_cap = std::min(120, atoi(e) & ~3); }   // debugging aid
+    const int jc_cap = 120;
     double best = 0.0;
     int best_groups = 0;
     for (int g = 1; g <= n_pairs; ++g) {
@@ -183,6 +183,16 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     p.tc_mode = (response_mode != LARTPC_RESPONSE_FFMA && tc_ok) ? 1 : 0;
     if (best_groups == 0 && !p.tc_mode) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
     if (p.tc_mode) {
+        // operand scale of the LUT: a power of two that puts max |R| into (2^9, 2^10], whatever units the table is in
+        // (fp16 operand, e4m3 cross-term parts: response_tc.cuh); a table with a non-finite entry is refused
+        float mx = 0.f;
+        for (size_t i = 0; i < lut_elems; ++i) {
+            if (!std::isfinite(lut_host[i])) { sim_free(s); return LARTPC_ERR_BAD_ARGUMENT; }
+            mx = std::max(mx, fabsf(lut_host[i]));
+        }
+        int e2 = 0;
+        if (mx > 0.f) { frexpf(mx, &e2); if (ldexpf(1.f, e2 - 1) == mx) --e2; }   // mx in (2^(e2-1), 2^e2]
+        p.b_scale_log2 = 10 - std::min(std::max(e2, -30), 30);
         p.NBW = nbw;  p.KQ = kq;  p.nq = nq;
         p.n_groups = 1;  p.PG = n_pairs;  p.NP = n_pairs;                 // (unused by the tensor-core response)
         p.Jc = 64;  p.CJ = p.Jc + 4;
@@ -286,6 +296,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
 extern "C" int lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *ids, int64_t n)
 {
     if (!sim || (n > 0 && !ids)) return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
     const size_t words = (size_t)(sim->n_pix + 31) / 32;
     std::vector<uint32_t> m(words, 0u);
     for (int64_t i = 0; i < n; ++i) {
@@ -301,7 +312,7 @@ extern "C" int lartpc_set_random_perturbations(lartpc_sim_t *sim, int m, uint64_
 {
     if (!sim || m < 0 || m > 255) return LARTPC_ERR_BAD_ARGUMENT;
     // the one-hot columns of the perturbed points exist in the tensor-core charge lattice only
-    if (m > 0 && !(sim->dp.tc_mode && sim->splat_tc && (sim->dp.nb == 10 || sim->dp.nb == 5))) return LARTPC_ERR_UNSUPPORTED;
+    if (m > 0 && !splat_on_tc(sim->dp)) return LARTPC_ERR_UNSUPPORTED;
     sim->dp.rnd_m = m;
     sim->dp.rnd_seed = seed;
     sim->have_signals = false;
@@ -324,6 +335,7 @@ extern "C" int lartpc_pack_hits(lartpc_sim_t *sim, const lartpc_hits_t *hits, in
         return LARTPC_ERR_BAD_ARGUMENT;
     if (n_hits > 0 && (!hits->hit_pixel || !hits->hit_tick || !hits->hit_adc)) return LARTPC_ERR_BAD_ARGUMENT;
     if (sim->dp.n_ticks > 65536 || sim->params.adc_bits > 12) return LARTPC_ERR_UNSUPPORTED;   // tick and adc must fit 16 / 12 bits
+    DeviceGuard dg(sim->device);
     return launch_pack_hits(sim, hits, n_hits, tile_pixels, packed, tile_offsets, (cudaStream_t)stream);
 }
 
@@ -338,6 +350,7 @@ extern "C" int lartpc_quench(lartpc_sim_t *sim, const lartpc_segments_t *seg, in
                              void *stream)
 {
     if (!sim || !seg || n < 0 || (n > 0 && (!dEdx || !n_e))) return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
     return launch_quench(sim, seg, n, dEdx, n_e, (cudaStream_t)stream);
 }
 
@@ -345,6 +358,7 @@ extern "C" int lartpc_drift(lartpc_sim_t *sim, const lartpc_segments_t *seg, int
                             lartpc_drifted_t *out, void *stream)
 {
     if (!sim || !seg || n < 0 || !out || (n > 0 && !n_e)) return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
     return launch_drift(sim, seg, n, n_e, out, (cudaStream_t)stream);
 }
 
@@ -353,6 +367,7 @@ extern "C" int lartpc_pixels_from_segments(lartpc_sim_t *sim, const lartpc_segme
                                            lartpc_pixmap_info_t *info, void *stream)
 {
     if (!sim || !seg || !dr || !out || n < 0) return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
     return launch_plan(sim, seg, dr, n, 0, sim->dp.n_tpcs, out, info, (cudaStream_t)stream);
 }
 
@@ -360,6 +375,7 @@ extern "C" int lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t 
                                       int64_t n, lartpc_signals_t *out, void *stream)
 {
     if (!sim || !dr || !pm || !out) return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
     if (!sim->have_plan || n != sim->plan_n) return LARTPC_ERR_ORDER;
     if (out->tile_capacity < tiles_alloc(sim->dp, sim->n_tiles)) return LARTPC_ERR_CAPACITY;
     if (sim->n_tiles > 0 && (!out->partial || !out->tile_range || !out->charge)) return LARTPC_ERR_BAD_ARGUMENT;
@@ -374,6 +390,7 @@ extern "C" int lartpc_sum_pixel_signals(lartpc_sim_t *sim, const lartpc_signals_
                                         void *stream)
 {
     if (!sim || !sig || !out) return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
     if (!sim->have_plan || !sim->have_signals) return LARTPC_ERR_ORDER;
     if (out->pixel_capacity < sim->n_active || out->sample_capacity < sim->total_samples) return LARTPC_ERR_CAPACITY;
     return launch_sum(sim, sig, out, (cudaStream_t)stream);
@@ -394,6 +411,7 @@ extern "C" int lartpc_electronics(lartpc_sim_t *sim, const lartpc_waveforms_t *w
 {
     if (!sim || !wf || !out || !out->counters) return LARTPC_ERR_BAD_ARGUMENT;
     if (wf->n_active > 0 && (!out->hits_per_pixel || !out->q_pixel)) return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
     cudaStream_t st = (cudaStream_t)stream;
     LARTPC_CUDA_TRY(cudaMemsetAsync(out->counters, 0, sizeof(int64_t) * 4, st));
     // the per-pixel hit slots live in sim-owned scratch, grown on demand (no allocation after warm-up)
@@ -489,6 +507,7 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
                                 void *stream)
 {
     if (!sim || !seg || !out || !out->counters || !workspace || n < 0) return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
     cudaStream_t st = (cudaStream_t)stream;
     const DevParams &p = sim->dp;
     Arena ar{(char *)workspace, ws_bytes, 0};

@@ -135,7 +135,7 @@ __device__ __forceinline__ int stage_segment(const DevParams &p, const SegRec &r
     L.rule = -1;
     int nq = r.N;
     if (p.rnd_m > 0) nq = r.N * p.rnd_m;                              // eq. (3.9) as printed: one column per perturbed point
-    else if (!L.zero_sigma && p.node_rules) {
+    else if (!L.zero_sigma) {
         // COMP: long or sharp segments are cut into `pieces` runs of consecutive midpoints (sizes differing by at most
         // one), each run with its own rule -- the identity holds run by run; L.rule then also carries the nodes per
         // piece (<< 8) and pieces - 1 (<< 16)

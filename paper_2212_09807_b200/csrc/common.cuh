@@ -31,9 +31,10 @@ struct DevParams {
                                      // (tensor-core mode: NB2 * 64 = the tile's rows of the fp16 hi / lo operand image)
     int rnd_m;                       // > 0: eq. (3.9) as printed, M random perturbations per sample point (lartpc_set_random_perturbations)
     unsigned long long rnd_seed;
-    int node_rules;                  // 1: the tensor-core splat may replace a segment's N midpoints by a node rule (charge_tc.cuh)
     int tc_mode;                     // 1: S4 response on the tensor cores (response_tc.cuh), 0: packed-FFMA2 response
     int NBW;                         // tensor-core mode: output columns per 16-tick arrival block, roundup16(KQ + 15)
+    int b_scale_log2;                // tensor-core mode: the LUT operand is R * 2^b_scale_log2, chosen per LUT so that max |R| lands
+                                     // in (2^9, 2^10] (fp16 / e4m3 range of the fixed part splits, response_tc.cuh)
     int KQ, nq;                      // tensor-core mode: LUT ticks per piece and pieces (K <= 241: one piece of K ticks; longer
                                      // LUTs are cut into pieces of 200 ticks, each a row of its own in `partial`, added by S5)
     int n_tpcs;
@@ -100,7 +101,6 @@ struct lartpc_sim {
     int64_t boxes_n = -1;  const void *boxes_of = nullptr;   // input whose S3 boxes the last tpc_lo = 0 plan wrote (reused by later batches)
     bool need_composite = false;         // some segment of the planned input wants composite node rules (charge_tc.cuh COMP)
     int batch_hint = 0;  size_t batch_hint_ws = 0;   // lartpc_run_spill: TPCs per batch that fitted the workspace last time
-    bool tile_sort = true;               // env LARTPC_TILE_SORT=0: identity order, every block kept (measurement aid)
     void *seg_rec = nullptr;  int64_t seg_rec_cap = 0;   // per-segment records of the tensor-core splat (charge_tc.cuh)
     // scan scratch + counters
     long long *scan_tmp = nullptr;  int64_t scan_tmp_elems = 0;
@@ -114,7 +114,7 @@ struct lartpc_sim {
     lartpc_drifted_t drifted_copy;
     lartpc_pixmap_t pixmap_copy;
     int sm_count = 148;
-    bool splat_tc = true;                // tensor-core mode: charge lattice on the tensor cores too (env LARTPC_SPLAT=ffma turns it off)
+    int device = 0;                      // CUDA device the sim was created on; every entry point runs there (DeviceGuard)
     // per-stage profiling of run_spill (lartpc_set_profiling)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;
@@ -187,6 +187,33 @@ __device__ __forceinline__ void perturbation_normals(unsigned long long seed, ui
 
 // ---- launch helpers -----------------------------------------------------------------------------
 static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// The charge lattice runs on the tensor cores (charge_tc.cuh) when the response does and the bins of a pixel fill one
+// 128-row operand the kernel is instantiated for; otherwise the FFMA2 splat writes the same operand image in the
+// tiles' original order.  ONE predicate for the plan (tile sort), the per-segment records and the splat dispatch.
+static inline bool splat_on_tc(const DevParams &p) { return p.tc_mode && (p.nb == 10 || p.nb == 5); }
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per device: remember, per kernel and device, what has been set
+constexpr int LARTPC_MAX_DEVICES = 64;
+struct SmemCfg { size_t bytes[LARTPC_MAX_DEVICES] = {}; };
+template <typename F> static inline cudaError_t ensure_dyn_smem(F func, SmemCfg &cfg, int device, size_t bytes)
+{
+    if (device < 0 || device >= LARTPC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    if (bytes <= cfg.bytes[device]) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) cfg.bytes[device] = bytes;
+    return e;
+}
+
+// entry points run on the sim's device whatever the caller's current device is, and restore it
+struct DeviceGuard {
+    int prev = -1;  bool switched = false;
+    explicit DeviceGuard(int device)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 // stage launchers (host, C++ linkage)
 int launch_quench(lartpc_sim *sim, const lartpc_segments_t *seg, int64_t n, float *dEdx, float *n_e, cudaStream_t st);

@@ -14,8 +14,9 @@
 //     [lo8(A) | hi8(A)] x [hi8(B) ; lo8(B)],
 // which costs the tensor pipe as much as one fp16 MMA of K = 16: two MMA slots per (bin, 16-tick block) instead of three
 // (error of the cross terms: 2^-4 x 2^-12 relative per product, random in sign; parity margins in the tests unchanged).
-// A carries a per-tile power-of-two scale (fp16 range), B a fixed 2^10 (keeps far-field LUT values normal); the fp8
-// parts carry the extra powers of two below, which cancel in the product; the epilogue undoes the rest exactly.
+// A carries a per-tile power-of-two scale (fp16 range), B a per-LUT one (lartpc_sim_create: max |R| 2^s in (2^9, 2^10], which
+// keeps far-field LUT values normal); the fp8 parts carry the extra powers of two below, which cancel in the product; the
+// epilogue undoes the rest exactly.
 //
 // Kernel (persistent, one CTA per SM, 192 threads, whole TMEM):
 //   warp 0, one lane   producer: per (item, bin c) one cp.async.bulk per charged 16-tick block of the A image (8 KB each:
@@ -45,7 +46,6 @@ constexpr int NBLK = JC / 16;
 constexpr int STAGES = 3;
 constexpr int A_SLOTS = 6;          // charge blocks a stage can hold: 4 of one tile block, or 3 + 3 of a pair
 constexpr int THREADS = 192;
-constexpr int B_SCALE_LOG2 = 10;
 // fp8 parts: lo8(A) = e4m3(lo(A) 2^SA) meets hi8(B) = e4m3(B 2^-SA); hi8(A) = e4m3(A 2^-SB) meets lo8(B) = e4m3(lo(B) 2^SB)
 // (|A| < 2^15, |lo(A)| <= 8, |B| <= 2^10, |lo(B)| <= 0.5: every part stays below e4m3's 448)
 constexpr int SA_LOG2 = 5, SB_LOG2 = 7;
@@ -58,6 +58,7 @@ struct Args {
     const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), 0
     const int32_t *tb_mask;        // [n_tb] 16-tick blocks that hold charge in any tile of the block (bit b)
     int n_tiles, n_tb, NC, WW, NBW, tile_ticks;
+    int b_scale_log2;              // B = R * 2^b_scale_log2 (DevParams)
     long long n_items;             // ceil(n_tb / 2) * WW * 2: (unit of two tile blocks, row, half)
     int *work;                     // item cursor, zero at launch: items are taken in order as CTAs become free, so the
                                    // CTAs that stream one tile block stay together however long the launch runs
@@ -360,7 +361,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 const int n_cols = bmB ? min(PAIR_COL, a.tile_ticks - t0) : a.tile_ticks;     // multiples of 8
                 const uint32_t tcol = tlane + (x ? PAIR_COL : 0);
                 float scale = 0.f;
-                if (live) scale = __int_as_float((127 + a.tile_meta[4 * tile + 2] - B_SCALE_LOG2) << 23);
+                if (live) scale = __int_as_float((127 + a.tile_meta[4 * tile + 2] - a.b_scale_log2) << 23);
                 float *dst = a.partial + ((size_t)(live ? tile : 0) * a.WW + d) * a.tile_ticks + t0;
                 if (bmB && live) {
                     // S5 reads whole 14-tick blocks around the charged range: the few ticks of the row the accumulator

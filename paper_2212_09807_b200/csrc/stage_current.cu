@@ -671,19 +671,15 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     a.charge = out->charge;  a.tile_range = out->tile_range;
     a.fma_counter = sim->d_fma;
     a.rec = nullptr;  a.tile_list = nullptr;  a.work = nullptr;  a.n_tiles = 0;  a.tb_mask = sim->tb_mask;
-    if (p.rnd_m > 0 && !(p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5))) return LARTPC_ERR_UNSUPPORTED;
-    if (p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5)) {
+    if (p.rnd_m > 0 && !splat_on_tc(p)) return LARTPC_ERR_UNSUPPORTED;
+    if (splat_on_tc(p)) {
         // tensor-core splat (charge_tc.cuh); other bin counts use the FFMA2 splat below, which writes the same image
-        static bool configured_tc = false;
-        if (!configured_tc) {
-#define LARTPC_CT_ATTR(NBV, R, C) LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_tc_kernel<NBV, R, C>, \
-                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM))
-            LARTPC_CT_ATTR(10, false, false);  LARTPC_CT_ATTR(5, false, false);
-            LARTPC_CT_ATTR(10, true, false);   LARTPC_CT_ATTR(5, true, false);
-            LARTPC_CT_ATTR(10, false, true);   LARTPC_CT_ATTR(5, false, true);
+        static SmemCfg cfg_tc[6];
+#define LARTPC_CT_ATTR(I, NBV, R, C) LARTPC_CUDA_TRY(ensure_dyn_smem(charge_lattice_tc_kernel<NBV, R, C>, cfg_tc[I], sim->device, CT_SMEM))
+        LARTPC_CT_ATTR(0, 10, false, false);  LARTPC_CT_ATTR(1, 5, false, false);
+        LARTPC_CT_ATTR(2, 10, true, false);   LARTPC_CT_ATTR(3, 5, true, false);
+        LARTPC_CT_ATTR(4, 10, false, true);   LARTPC_CT_ATTR(5, 5, false, true);
 #undef LARTPC_CT_ATTR
-            configured_tc = true;
-        }
         if (n >= (1ll << 30) || sim->n_tiles >= INT32_MAX - 8 * (int64_t)sim->sm_count) return LARTPC_ERR_UNSUPPORTED;
         if (n > sim->seg_rec_cap) return LARTPC_ERR_ORDER;                // records are written with the plan (launch_seg_records)
         a.rec = sim->seg_rec;  a.work = sim->d_work;  a.n_tiles = (int)sim->n_tiles;
@@ -705,12 +701,8 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
         return LARTPC_OK;
     }
     size_t smem = splat_smem_bytes(p);
-    static size_t configured = 0;
-    if (smem > configured) {
-        LARTPC_CUDA_TRY(cudaFuncSetAttribute(charge_lattice_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)smem));
-        configured = smem;
-    }
+    static SmemCfg cfg_splat;
+    LARTPC_CUDA_TRY(ensure_dyn_smem(charge_lattice_kernel, cfg_splat, sim->device, smem));
     ++g_lartpc_launches;
     charge_lattice_kernel<<<(unsigned)sim->n_tiles, NT1, smem, st>>>(a);
     LARTPC_CUDA_TRY(cudaGetLastError());
@@ -723,7 +715,7 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
 int launch_seg_records(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n, cudaStream_t st)
 {
     const DevParams &p = sim->dp;
-    if (!(p.tc_mode && sim->splat_tc && (p.nb == 10 || p.nb == 5)) || n <= 0) return LARTPC_OK;
+    if (!splat_on_tc(p) || n <= 0) return LARTPC_OK;
     if (n >= (1ll << 30)) return LARTPC_ERR_UNSUPPORTED;
     if (n > sim->seg_rec_cap) {
         if (sim->seg_rec) cudaFree(sim->seg_rec);
@@ -763,15 +755,10 @@ int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t
     a.end_row = sim->d_end_row;
     if (a.n_stages < 2) return LARTPC_ERR_UNSUPPORTED;
     size_t smem = (size_t)a.n_stages * a.stage_floats * 4 + 2 * (size_t)a.n_stages * sizeof(u64) + 64;   // + pair group per stage
-    static size_t configured = 0;
-    if (smem > configured) {
-        LARTPC_CUDA_TRY(cudaFuncSetAttribute(response_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = smem;
-    }
+    static SmemCfg cfg_resp;
+    LARTPC_CUDA_TRY(ensure_dyn_smem(response_kernel, cfg_resp, sim->device, smem));
     LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
-    int grid = (int)std::min<int64_t>(n_work, 2 * (int64_t)sim->sm_count);
-    { const char *e = getenv("LARTPC_RESP_GRID"); if (e && atoi(e) > 0) grid = std::min(grid, atoi(e)); }      // debugging aid
-    { const char *e = getenv("LARTPC_RESP_STAGES"); if (e && atoi(e) >= 2) a.n_stages = std::min(a.n_stages, atoi(e)); }
+    const int grid = (int)std::min<int64_t>(n_work, 2 * (int64_t)sim->sm_count);
     ++g_lartpc_launches;
     response_kernel<<<grid, NT2, smem, st>>>(a);
     LARTPC_CUDA_TRY(cudaGetLastError());
@@ -812,16 +799,14 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     a.n_tiles = (int)sim->n_tiles;
     a.n_tb = (int)((sim->n_tiles + rtc::TB - 1) / rtc::TB);
     a.NC = p.NB2;  a.WW = p.WW * p.nq;  a.NBW = p.NBW;  a.tile_ticks = p.tile_ticks;   // a row = (target, LUT piece)
+    a.b_scale_log2 = p.b_scale_log2;
     a.n_items = (long long)((a.n_tb + 1) / 2) * a.WW * 2;                 // (unit of two tile blocks, row, half): response_tc.cuh
     if (a.n_items >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.work = sim->d_work;
     LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
     const int smem = rtc::smem_bytes(p.NBW);
-    static int configured = 0;
-    if (smem > configured) {
-        LARTPC_CUDA_TRY(cudaFuncSetAttribute(rtc::response_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        configured = smem;
-    }
+    static SmemCfg cfg_rtc;
+    LARTPC_CUDA_TRY(ensure_dyn_smem(rtc::response_tc_kernel, cfg_rtc, sim->device, (size_t)smem));
     const int grid = (int)std::min<long long>(a.n_items, sim->sm_count);
     ++g_lartpc_launches;
     rtc::response_tc_kernel<<<grid, rtc::THREADS, smem, st>>>(a);
@@ -829,7 +814,7 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     return LARTPC_OK;
 }
 
-// Bs[d, q][c][fp16 | fp8][NBW x 32 bytes] with Bs[n'][jj] = R[c][d][KQ q + n' - jj] * 2^10 (0 outside piece q of the LUT): the fp16 image
+// Bs[d, q][c][fp16 | fp8][NBW x 32 bytes] with Bs[n'][jj] = R[c][d][KQ q + n' - jj] * 2^b_scale_log2 (0 outside piece q of the LUT): the fp16 image
 // (rtc::b_image_offset) and the fp8 image of the cross terms (rtc::b8_image_offset), both in the canonical un-swizzled
 // K-major layout.  Built once per sim on the host.
 size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_out)
@@ -848,7 +833,7 @@ size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_o
                 for (int nn = 0; nn < NBW; ++nn)
                     for (int jj = 0; jj < 16; ++jj) {
                         const int k = nn - jj;
-                        const float x = (k >= 0 && k < K) ? ldexpf(src[k], rtc::B_SCALE_LOG2) : 0.f;
+                        const float x = (k >= 0 && k < K) ? ldexpf(src[k], p.b_scale_log2) : 0.f;
                         const __half h = __float2half_rn(x);
                         hi[rtc::b_image_offset(nn, jj)] = h;
                         f8[rtc::b8_image_offset(nn, jj)] =

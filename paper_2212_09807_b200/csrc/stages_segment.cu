@@ -612,7 +612,8 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
     sim->n_tiles = h[CNT_TILES];
     if (tpc_lo == 0) { sim->need_composite = h[CNT_COMPOSITE] != 0;  sim->boxes_n = n;  sim->boxes_of = (const void *)out->a_lo; }
     if (p.tc_mode && sim->n_tiles > 0) {
-        const int sort = sim->tile_sort && sim->splat_tc ? 1 : 0;
+        // the FFMA2 splat (bins per pixel other than 5 / 10) writes the operand image in the tiles' original order
+        const int sort = splat_on_tc(p) ? 1 : 0;
         const int64_t nt = sim->n_tiles;
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->cls_hist, 0, sizeof(int32_t) * 32, st));
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->tb_mask, 0, sizeof(int32_t) * (nt / TC_TILE_BLOCK + 1), st));
