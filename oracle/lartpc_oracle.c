@@ -11,15 +11,29 @@
  *        (-ffp-contract=off: every integer decision below must come from individually rounded
  *         IEEE-754 double operations, in the order written.)
  *
- * Parity pins (tests/test_oracle_*.py, all "-m 'not gpu'"):
- *   orc_quench      closed forms eqs. (3.1)(3.2), printed "around 0.7" for a MIP
- *   orc_drift       exp(-t/tau), sigma = sqrt(2 D t) values; geometry P:L830-832
- *   orc_pixmap      brute-force completeness / minimality, hand-worked rectangles
- *   orc_pixel_current  zero-diffusion point charge == LUT, charge conservation, long-track erf
- *                      closed form, per-electron Monte Carlo, direct 6-fold sum (orc_direct_current)
+ * Parity pins (tests/test_oracle_pins.py, all "-m 'not gpu'"); every function AND branch below has one:
+ *   orc_quench      Birks / Box branches: closed forms eqs. (3.1)(3.2) (test_recombination_golden_values, printed "around
+ *                   0.7" for a MIP), invariants (1/R linear; exp(R xi) - xi = alpha); R < 0 clamp, L = 0, dE = 0
+ *                   (test_recombination_invariants)
+ *   orc_drift       exp(-t/tau), sigma = sqrt(2 D t) values (test_transport_golden_values); sign of eq. (3.3) for
+ *                   two-sided modules and the inactive branch (test_drift_two_sided_module_and_inactive)
+ *   orc_pixmap      hand-worked rectangles at sigma = 0 and at the plane edge (test_pixmap_hand_cases); charged-bin box
+ *                   and tick range jt0 / jt1 with sigma > 0 and t_origin != 0 (test_pixmap_tick_range_with_diffusion);
+ *                   brute-force completeness / minimality (test_pixmap_*_brute_force)
+ *   orc_pixel_current  zero-diffusion point charge == LUT (sigma = 0 indicator branch), charge conservation, long-track
+ *                   erf closed form, per-electron Monte Carlo, direct 6-fold sum (orc_direct_current)
  *   orc_pixel_current_random  (eq. 3.9 as printed) exact charge conservation, sigma = 0 identity with the
- *                      expectation form, one perturbed point placed by hand, mean over seeds vs the expectation form
- *   orc_electronics hand cases, Philox4x32-10 known answer, normal moments
+ *                   expectation form, one perturbed point placed by hand, mean over seeds vs the expectation form
+ *   orc_philox4x32_10 / orc_noise_normals   Random123 known answers; moments; the test's own pure-Python Philox +
+ *                   Box-Muller reproduces the three normals (test_python_philox_matches_the_published_vectors)
+ *   orc_electronics branch by branch, expected ticks / counts worked in the test from its own Philox normals:
+ *                   integrate / threshold (>=) / hold / ADC floor + clamp / window end   test_electronics_hand_cases
+ *                   reset noise q = noise_reset * z_r after the sample                    test_electronics_reset_noise_branch
+ *                   uncorrelated noise on the sampled value (z_u)                         test_electronics_uncorrelated_noise_branch
+ *                   discriminator noise on the threshold, fresh each tick (z_d)           test_electronics_discriminator_noise_branch
+ *                   periodic reset (armed only, before the tick's charge)                 test_electronics_periodic_reset_branch
+ *                   min-spacing re-arm (n >= sample + spacing - hold)                     test_electronics_min_spacing_branch
+ *   No function is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>

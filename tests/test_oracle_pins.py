@@ -402,6 +402,175 @@ def test_electronics_noise_is_keyed_and_reproducible():
     assert ha[0] == math.floor((580 + 4 * (q + 500.0 * z[1]) / 1000 - 288) / 3.953125)
 
 
+# ---- the four noise / timing branches of O6, each against values worked out HERE from the Philox words -----------------
+# (an independent pure-Python Philox4x32-10 + Box-Muller: nothing below calls the oracle's own normals)
+
+def _philox_py(ctr, key):
+    """Philox4x32-10 as published (Salmon et al., SC'11): 10 rounds of two 32x32 -> 64 multiplies, key bumped by the
+    Weyl constants each round."""
+    c0, c1, c2, c3 = ctr
+    k0, k1 = key
+    M = 0xFFFFFFFF
+    for _ in range(10):
+        p0, p1 = 0xD2511F53 * c0, 0xCD9E8D57 * c2
+        c0, c1, c2, c3 = ((p1 >> 32) ^ c1 ^ k0) & M, p1 & M, ((p0 >> 32) ^ c3 ^ k1) & M, p0 & M
+        k0, k1 = (k0 + 0x9E3779B9) & M, (k1 + 0xBB67AE85) & M
+    return [c0, c1, c2, c3]
+
+
+def _normals_py(seed, pixel, tick):
+    """(z_d, z_u, z_r) of SURVEY 8(c.1) O6 / reading D16: counter (pixel, tick, 0, 0), key (seed lo, seed hi),
+    u_i = (x_i + 0.5) 2^-32, z_d = r01 cos, z_u = r01 sin (pair u0, u1), z_r = r23 cos (pair u2, u3)."""
+    x = _philox_py((pixel, tick, 0, 0), (seed & 0xFFFFFFFF, seed >> 32))
+    u = [(xi + 0.5) / 4294967296.0 for xi in x]
+    r01, r23 = math.sqrt(-2 * math.log(u[0])), math.sqrt(-2 * math.log(u[2]))
+    return r01 * math.cos(2 * math.pi * u[1]), r01 * math.sin(2 * math.pi * u[1]), r23 * math.cos(2 * math.pi * u[3])
+
+
+def _adc(q_s):
+    return min(255, max(0, math.floor((580 + 4 * q_s / 1000 - 288) / 3.953125)))
+
+
+def test_python_philox_matches_the_published_vectors():
+    """The test's own generator against the Random123 known-answer vectors (tests/golden/philox4x32_10.txt), and the
+    oracle's normals against the test's for a spread of (seed, pixel, tick): both sides of every pin below are anchored."""
+    for row in _rows("philox4x32_10.txt"):
+        h = [int(x, 16) for x in row]
+        assert _philox_py(h[:4], h[4:6]) == h[6:]
+    for seed, pix, tick in ((0, 0, 0), (42, 5, 117), (2 ** 40 + 17, 10 ** 7, 3400), (0x22120983, 123456, 1)):
+        assert np.allclose(oracle.noise_normals(seed, pix, tick), _normals_py(seed, pix, tick), rtol=1e-13, atol=1e-15)
+
+
+def test_electronics_reset_noise_branch():
+    """P:L710 "random pedestal shift after every trigger reset" (reading D16: q = 900 z_r(pixel, sample tick) after the
+    reset, z_r from the SECOND Box-Muller pair).  Constant 1000 e-/tick: the first hit is noise-free (crossing at tick 6,
+    sample at 22, q_s = 23000); the second crossing is the first tick n > 22 with 900 z_r + 1000 (n - 22) >= 7000, its
+    sample 16 ticks later holds 900 z_r + 1000 (n_s - 22).  A reset that used z_d or z_u, or that was applied before the
+    sample was taken, or a q that kept the collected charge, gives other ticks / counts on these pixels."""
+    p = W.default_params(n_readout_ticks=120, noise_reset_e=900.0)
+    seed = 20221209
+    moved = other_z = 0
+    for pid in range(40, 64):
+        hp, ht, ha, cnt = oracle.electronics(p, seed, [pid], np.full((1, 120), 1000.0))
+        zd, zu, zr = _normals_py(seed, pid, 22)
+        q0 = 900.0 * zr
+        n_c2 = 22 + math.ceil((7000.0 - q0) / 1000.0)
+        assert ht[0] == 22 and ha[0] == _adc(23000.0)
+        assert ht[1] == n_c2 + 16 and ha[1] == _adc(q0 + 1000.0 * (n_c2 + 16 - 22))
+        zr2 = _normals_py(seed, pid, n_c2 + 16)[2]                 # and once more: third hit from the second reset
+        n_c3 = n_c2 + 16 + math.ceil((7000.0 - 900.0 * zr2) / 1000.0)
+        assert ht[2] == n_c3 + 16 and ha[2] == _adc(900.0 * zr2 + 1000.0 * (n_c3 - n_c2))
+        moved += (n_c2 != 29) or _adc(q0 + 1000.0 * (n_c2 - 6)) != _adc(23000.0)
+        for zalt in (zd, zu):
+            alt = 22 + math.ceil((7000.0 - 900.0 * zalt) / 1000.0)
+            other_z += (alt != n_c2) or _adc(900.0 * zalt + 1000.0 * (alt - 6)) != ha[1]
+    assert moved >= 12 and other_z >= 24          # the draws do move the result, and the wrong normal would not pass
+
+
+def test_electronics_uncorrelated_noise_branch():
+    """P:L710 uncorrelated noise 500 e- (reading D16: added to the SAMPLED value only, z_u = second normal of the first
+    Box-Muller pair of the (pixel, sample tick) draw; the integrated charge itself is untouched, so the timing is the
+    noise-free one).  400 e-/tick from tick 20: crossing at 37, sample at 53 with 13600 e- + 500 z_u."""
+    p = W.default_params(n_readout_ticks=120, noise_uncorr_e=500.0)
+    wave = np.zeros((1, 120))
+    wave[0, 20:80] = 400.0
+    seed, differs = 31337, 0
+    for pid in range(200, 240):
+        hp, ht, ha, cnt = oracle.electronics(p, seed, [pid], wave)
+        zd, zu, zr = _normals_py(seed, pid, 53)
+        assert ht[0] == 53 and ha[0] == _adc(13600.0 + 500.0 * zu)
+        differs += (_adc(13600.0 + 500.0 * zd) != ha[0]) + (_adc(13600.0 + 500.0 * zr) != ha[0]) + (_adc(13600.0) != ha[0])
+        # second hit: the reset left no charge (reset noise off), 26 more ticks of 400 e- remain: 10400 e- >= 7000 at tick 71
+        assert ht[1] == 71 + 16 and ha[1] == _adc(10400.0 + 500.0 * _normals_py(seed, pid, 87)[1])
+    assert differs >= 15          # (500 e- is half an ADC count: a wrong normal changes about one count in four)
+
+
+def test_electronics_discriminator_noise_branch():
+    """P:L710 discriminator noise 650 e- (reading D16: fresh every tick, on the threshold, z_d = FIRST normal of the
+    (pixel, tick) draw).  The charge ramps to 6800 e- in ten ticks and stays there, 200 e- = 0.31 sigma below the
+    threshold: the channel fires at the first tick n with q(n) >= 7000 + 650 z_d(pixel, n), taken from the per-tick
+    normals worked out here; the sample 16 ticks later reads 6800 e- (no other noise term is on)."""
+    p = W.default_params(n_readout_ticks=200, noise_disc_e=650.0)
+    wave = np.zeros((1, 200))
+    wave[0, :10] = 680.0
+    q = np.cumsum(wave[0])
+    seed = 777
+    late = not_first = 0
+    for pid in range(100, 130):
+        z = [_normals_py(seed, pid, n) for n in range(200)]
+        n_c = next(n for n in range(200) if q[n] >= 7000.0 + 650.0 * z[n][0])
+        hp, ht, ha, cnt = oracle.electronics(p, seed, [pid], wave)
+        assert ht[0] == n_c + 16 and ha[0] == _adc(q[n_c + 16])
+        late += n_c > 9
+        alt = [next(n for n in range(200) if q[n] >= 7000.0 + 650.0 * z[n][k]) for k in (1, 2)]
+        not_first += (alt[0] != n_c) + (alt[1] != n_c)
+        # after the sample the charge is gone (reset, no reset noise): nothing can fire again
+        assert cnt[0] == 1
+    assert late >= 10 and not_first >= 30          # several ticks "within +-650 z_d of 7000 e-", and z_u / z_r would differ
+
+
+def test_electronics_periodic_reset_branch():
+    """P:L708 "periodic reset" (reading D17: every periodic_reset_ticks an ARMED channel loses its charge, at the START
+    of the tick, before that tick's charge is integrated; a channel in its hold is not touched).
+    (i) 100 e-/tick crosses 7000 e- at tick 69 without the reset and never with a period of 50 ticks (at most 5000 e-).
+    (ii) 1000 e-/tick, period 7: crossing at 6 (7000 e- after ticks 0..6; a reset at tick 7 comes too late), sample 22;
+    ticks 23..27 collect 5000, tick 28 resets then adds 1000, ticks 29..34 reach 7000: crossing 34, sample 50; and so
+    on every 28 ticks, each sample holding 7000 + 16 x 1000 e-.  A reset applied AFTER the tick's charge would clear
+    the 6000 e- of tick 28 to zero and cross at 35."""
+    trickle = np.full((1, 400), 100.0)
+    assert oracle.electronics(W.default_params(n_readout_ticks=400), 0, [9], trickle)[1].tolist()[0] == 69 + 16
+    assert oracle.electronics(W.default_params(n_readout_ticks=400, periodic_reset_ticks=50), 0, [9], trickle)[3][0] == 0
+    p = W.default_params(n_readout_ticks=140, periodic_reset_ticks=7)
+    hp, ht, ha, cnt = oracle.electronics(p, 0, [9], np.full((1, 140), 1000.0))
+    assert ht.tolist() == [22, 50, 78, 106, 134]
+    assert ha.tolist() == [_adc(23000.0)] * 5
+    # during the hold (ticks 7, 14, 21 fall inside the first one) nothing is cleared: the sample holds all 23 ticks
+    assert _adc(23000.0) != _adc(23000.0 - 7000.0)
+
+
+def test_electronics_min_spacing_branch():
+    """consecutive samples are at least min_spacing_ticks apart (1.1 us = 11 ticks in the paper, where the 1.6 us
+    hold makes it moot; here 40 > hold + 1).  7000 e-/tick re-crosses at once after every reset, so the spacing is what
+    paces the hits: crossing at 0, sample 16; re-armed for a crossing at tick 16 + 40 - 16 = 40 (>=, not >), sample 56;
+    then 96, 136.  With the default spacing the same current gives a hit every 17 ticks."""
+    wave = np.full((1, 160), 7000.0)
+    p = W.default_params(n_readout_ticks=160, min_spacing_ticks=40)
+    hp, ht, ha, cnt = oracle.electronics(p, 0, [1], wave)
+    assert ht.tolist() == [16, 56, 96, 136]
+    # 17 x 7000 e- = 476 mV over the 580 mV pedestal -> count 194; 40 x 7000 e- saturates the 8-bit ADC
+    assert ha.tolist() == [194, 255, 255, 255] and _adc(17 * 7000.0) == 194
+    # charge keeps integrating while the channel waits to be re-armed: 40 ticks x 7000 e- at every later sample
+    p2 = W.default_params(n_readout_ticks=160, min_spacing_ticks=40, gain_mv_per_ke=0.01)
+    ha2 = oracle.electronics(p2, 0, [1], wave)[2]
+    lsb = (1300.0 - 288.0) / 256
+    assert ha2.tolist() == [math.floor((580 + 0.01 * 7 * 17 - 288) / lsb)] + [math.floor((580 + 0.01 * 7 * 40 - 288) / lsb)] * 3
+    ht0 = oracle.electronics(W.default_params(n_readout_ticks=160), 0, [1], wave)[1]
+    assert ht0.tolist() == list(range(16, 160, 17))
+
+
+def test_pixmap_tick_range_with_diffusion():
+    """O3 tick range and charged-bin box with sigma > 0 (reading D10), numbers worked by hand: one segment at 10 -> 10.05 cm
+    of drift, t_mid = 10.025 / 0.16 = 62.65625 us, sigma_L = sqrt(2 x 4e-6 x 62.65625) = 0.0223886 cm -> sigma_t =
+    0.1399288 us, 5 sigma_t = 0.699644 us; T_s = 62.5, T_e = 62.8125 us -> jt0 = floor(618.0036) = 618, jt1 =
+    floor(635.1214) = 635.  sigma_T = sqrt(2 x 8.8e-6 x 62.65625) = 0.0332077 cm, 5 sigma_T = 0.166038 cm; u from
+    2.3 pitch = 1.01982 to 1.04982 cm, bin 0.04434 cm -> a_lo = floor(19.2553) = 19, a_hi = floor(27.4213) = 27."""
+    p, tpcs, _ = _small_setup(nx=12, ny=12, drift=12.0)
+    pitch = p["pixel_pitch_cm"]
+    seg = _one_segment(2.3 * pitch, 5.5 * pitch, 10.0, 2.3 * pitch + 0.03, 5.5 * pitch, 10.05, 0.21)
+    _, _, dr, pm = _chain(p, tpcs, seg)
+    assert dr["sigma_t"][0] == pytest.approx(0.1399288, rel=1e-6) and dr["sigma_T"][0] == pytest.approx(0.0332077, rel=1e-6)
+    assert (pm["jt0"][0], pm["jt1"][0]) == (618, 635)
+    assert (pm["a_lo"][0], pm["a_hi"][0]) == (19, 27)
+    # v is constant at 5.5 pitch = bin 55.0: +- 0.166038 / 0.04434 = 3.7446 bins -> floor(51.255) .. floor(58.745)
+    assert (pm["b_lo"][0], pm["b_hi"][0]) == (51, 58)
+    # pixel rectangle: charged pixels 1..2 (x) and 5 (y), widened by H = 2
+    assert (pm["ix0"][0], pm["ix1"][0], pm["iy0"][0], pm["iy1"][0]) == (0, 4, 3, 7)
+    # t_origin shifts the ticks, not the box: 3.0 us later -> 30 ticks earlier
+    p2 = dict(p, t_origin_us=3.0)
+    pm2 = oracle.pixmap(p2, tpcs, seg, oracle.drift(p2, tpcs, seg, oracle.quench(p2, seg)[1]))
+    assert (pm2["jt0"][0], pm2["jt1"][0]) == (588, 605)
+
+
 # ------------------------------------------------------------------ O4r eq. (3.9) as printed (random perturbations)
 def _random_case():
     p, tpcs, lut = _small_setup(nx=14, ny=14, drift=12.0, n_ticks=1100)
