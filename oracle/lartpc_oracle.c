@@ -19,7 +19,7 @@
  *                   two-sided modules and the inactive branch (test_drift_two_sided_module_and_inactive)
  *   orc_pixmap      hand-worked rectangles at sigma = 0 and at the plane edge (test_pixmap_hand_cases); charged-bin box
  *                   and tick range jt0 / jt1 with sigma > 0 and t_origin != 0 (test_pixmap_tick_range_with_diffusion);
- *                   brute-force completeness / minimality (test_pixmap_*_brute_force)
+ *                   brute-force completeness / minimality (test_pixmap_complete_and_minimal)
  *   orc_pixel_current  zero-diffusion point charge == LUT (sigma = 0 indicator branch), charge conservation, long-track
  *                   erf closed form, per-electron Monte Carlo, direct 6-fold sum (orc_direct_current)
  *   orc_pixel_current_random  (eq. 3.9 as printed) exact charge conservation, sigma = 0 identity with the

@@ -204,7 +204,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
         p.n_groups = best_groups;  p.PG = (n_pairs + p.n_groups - 1) / p.n_groups;  p.NP = p.n_groups * p.PG;
         p.Jc = std::min(jc_cap, RESP_NO * (ncons / p.PG) - K + 1) & ~3;  p.CJ = p.Jc + 4;
         p.nblk_max = (p.Jc + K - 2) / RESP_NO + 1;  p.tile_ticks = RESP_NO * p.nblk_max;  p.KQ = K;  p.nq = 1;
-        p.slab_floats = (SLAB_HDR + 2 * p.NB2 + p.NB2 * (4 + p.CJ) + 3) & ~3;
+        p.slab_floats = (((SLAB_HDR + 2 * p.NB2 + 3) & ~3) + p.NB2 * (4 + p.CJ) + 3) & ~3;
     }
     if (p.j_max / p.Jc + 2 > MAX_WINDOWS) {                                 // window masks are 128 bits
         sim_free(s);

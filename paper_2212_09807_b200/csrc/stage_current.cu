@@ -304,7 +304,8 @@ __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs 
     __syncthreads();
     if (warp == 0) {
         // bin list in ascending bin order; row offsets = running sum of 4 * groups
-        int nbins = 0, tlo = INT_MAX, thi = -1, off = SLAB_HDR + 2 * NB2, groups = 0;
+        // (rows are copied by 16-byte bulk transfers: the first one starts on a multiple of four words)
+        int nbins = 0, tlo = INT_MAX, thi = -1, off = (SLAB_HDR + 2 * NB2 + 3) & ~3, groups = 0;
         for (int base = 0; base < NB2; base += 32) {
             const int c = base + lane;
             const bool f = c < NB2 && bin_jhi[c] >= 0;

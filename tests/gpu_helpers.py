@@ -36,15 +36,38 @@ def hit_table(pix, tick, adc):
 
 
 def compare_hits(gpu, orc):
-    """Fraction of oracle hits reproduced exactly, and whether every other hit is off by <= 1 tick or 1 count."""
-    g, o = hit_table(*gpu), hit_table(*orc)
-    exact = sum(1 for k, a in o.items() if g.get(k) == a)
-    near = True
-    for (p, t), a in o.items():
-        if g.get((p, t)) == a:
+    """Hit lists compared pixel by pixel, hit by hit, in tick order (BASELINE north_star: >= 99.9 % identical in pixel,
+    tick and ADC; the rest off by at most one tick or one count, at threshold crossings).
+
+    A pixel's hits are a chain: when the integrated charge sits within the rounding error of the threshold at a crossing,
+    the two sides may fire one tick apart, the reset then happens one tick apart, the reset noise is drawn for another
+    (pixel, tick) key and the charge of one tick moves between neighbouring samples -- every LATER hit of that pixel is a
+    consequence of that one near miss, not an independent disagreement.  So: the first differing hit of a pixel must be
+    within one tick and one count of its partner; the hits behind it count as not identical but are not held to the
+    nearness rule.  A pixel whose hit COUNT differs without such a near miss fails.
+    Returns (identical fraction of the oracle's hits, all differences explained, n_gpu, n_oracle, n_near_misses)."""
+    def by_pixel(pix, tick, adc):
+        d = {}
+        for p, t, a in zip(pix.tolist(), tick.tolist(), adc.tolist()):
+            d.setdefault(int(p), []).append((int(t), int(a)))
+        for v in d.values():
+            v.sort()
+        return d
+    g, o = by_pixel(*gpu), by_pixel(*orc)
+    exact = n_o = n_g = n_near = 0
+    ok = True
+    for p in set(g) | set(o):
+        gl, ol = g.get(p, []), o.get(p, [])
+        n_o += len(ol)
+        n_g += len(gl)
+        k = 0
+        while k < min(len(gl), len(ol)) and gl[k] == ol[k]:
+            k += 1
+        exact += k
+        if k == len(gl) == len(ol):
             continue
-        cands = [g.get((p, t + d)) for d in (-1, 0, 1)]
-        if not any(c is not None and abs(c - a) <= 1 for c in cands):
-            near = False
-    extra = [k for k in g if k not in o and (k[0], k[1] - 1) not in o and (k[0], k[1] + 1) not in o]
-    return exact / max(len(o), 1), near and not extra, len(g), len(o)
+        if k < min(len(gl), len(ol)) and abs(gl[k][0] - ol[k][0]) <= 1 and abs(gl[k][1] - ol[k][1]) <= 1:
+            n_near += 1                         # a near miss at a crossing; what follows on this pixel is its consequence
+        else:
+            ok = False                          # a missing / extra hit, or a first difference beyond one tick / one count
+    return exact / max(n_o, 1), ok, n_g, n_o, n_near

