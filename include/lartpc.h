@@ -127,7 +127,8 @@ typedef struct {
     int32_t tile_targets;               /* W*W: partial waveforms per tile */
     int32_t tile_ticks;                 /* readout ticks per partial waveform (padded) */
     int32_t tile_charge_floats;         /* 32-bit words of one tile's packed charge lattice (lartpc_signals_t.charge) */
-    int32_t reserved;
+    int32_t tile_block;                 /* the charge buffer must hold n_tiles rounded up to a multiple of this (256 with the
+                                           tensor-core response: two 128-tile MMA blocks per CTA pair; 1 otherwise) */
 } lartpc_pixmap_info_t;
 
 /* S4 output.  A tile is (charged pixel P, window of lartpc_chunk_ticks() arrival ticks that starts at
@@ -138,13 +139,14 @@ typedef struct {
  *               read, [slot / 128][bin][16-tick block][fp16 part | fp8 part][slot % 128][32 bytes], where a tile's
  *               slot is given by the sim's plan (tiles that charge the same 16-tick blocks sit together); the fp16
  *               part holds C 2^-e, the fp8 (e4m3) part {lo8 = (C 2^-e - fp16 part) 2^5, hi8 = C 2^-e 2^-7} per tick,
- *               e in tile_range; blocks no tile of a 128-slot block charges are neither written nor read; the buffer
- *               must hold a whole number of 128-slot blocks: tile_capacity >= n_tiles rounded up to 128.
+ *               e in tile_range; blocks no tile of a 256-slot unit (the two 128-tile blocks a CTA pair multiplies at once)
+ *               charges are neither written nor read; the buffer must hold a whole number of units: tile_capacity >=
+ *               n_tiles rounded up to lartpc_pixmap_info_t.tile_block.
  *               FFMA response: packed per tile as a header (bins, charge groups, first / last output block), one
  *               item per non-empty bin (bin, first tick, groups of 4 ticks, row offset) and the charge rows;
  *   partial     float32 [n_tiles][tile_targets][tile_ticks] (electrons per tick), indexed by slot: the current that
  *               charge induces on the W x W pixels around P during readout ticks [j_start, j_start + tile_ticks);
- *               tile_targets = W*W, except on the tensor-core path with lut_ticks > 241, where the LUT is cut into
+ *               tile_targets = W*W, except on the tensor-core path with lut_ticks > 209, where the LUT is cut into
  *               pieces of 200 ticks and row (target d, piece q) = d * pieces + q covers ticks from j_start + 200 q;
  *   tile_range  int32 [n_tiles][4], indexed by slot = first / last 14-tick block of `partial` that can be non-zero
  *               (first > last: no charge), the scale exponent e, 0.
@@ -208,7 +210,7 @@ void lartpc_sim_destroy(lartpc_sim_t *sim);
 /* As lartpc_sim_create, choosing how S4 applies the response (eq. 3.7):
  *   LARTPC_RESPONSE_TENSOR  dense contraction of the charge lattice with the LUT on the tcgen05 tensor cores, operands
  *                           split hi + lo (fp16 main term, fp8 cross terms, fp32 accumulation); a LUT longer than
- *                           241 ticks is applied in pieces of 200 ticks; window_pixels^2 <= 128;
+ *                           209 ticks is applied in pieces of 200 ticks; window_pixels^2 <= 128;
  *   LARTPC_RESPONSE_FFMA    sliding-window convolution on the FP32 pipe (packed FFMA2), any LUT shape;
  *   LARTPC_RESPONSE_AUTO    TENSOR where it applies, else FFMA (what lartpc_sim_create does).
  * Both give the same currents within the S4 tolerance; LARTPC_ERR_UNSUPPORTED when TENSOR
@@ -254,7 +256,7 @@ int  lartpc_pixels_from_segments(lartpc_sim_t *sim, const lartpc_segments_t *seg
                                  const lartpc_drifted_t *drifted, int64_t n,
                                  lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, void *stream);
 
-/* S4: needs out->tile_capacity >= info.n_tiles (rounded up to 128 for the tensor-core response).  Two kernels: the
+/* S4: needs out->tile_capacity >= info.n_tiles rounded up to info.tile_block.  Two kernels: the
  * charge lattice of every tile (splat), then the response of the W x W pixels around it (persistent; tensor cores, or
  * LUT rows streamed through shared memory for the FFMA form). */
 int  lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t *drifted, const lartpc_pixmap_t *pixmap,

@@ -172,11 +172,11 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
         const double score = (double)jc / g;
         if (score > best) { best = score; best_groups = g; }
     }
-    // Tensor-core response (response_tc.cuh): tiles of 64 arrival ticks, the accumulator of one target pixel
-    // (48 + NBW columns, NBW = roundup16(KQ + 15)) must fit the 512 TMEM columns with NBW <= 256 (one MMA's N).  A LUT
-    // longer than 241 ticks is cut into pieces of KQ = 200 ticks: piece q is a LUT of its own whose response lands
+    // Tensor-core response (response_tc.cuh): tiles of 64 arrival ticks; even and odd 16-tick blocks have an accumulator
+    // each (32 + NBW columns, NBW = roundup16(KQ + 15)), and the two must fit the 512 TMEM columns: NBW <= 224.  A LUT
+    // longer than 209 ticks is cut into pieces of KQ = 200 ticks: piece q is a LUT of its own whose response lands
     // 200 q ticks later, one more row per (tile, target) in `partial`, which S5 adds like the rows of other tiles.
-    const int kq = ((K + 15 + 15) & ~15) <= 256 ? K : 200, nq = (K + kq - 1) / kq;
+    const int kq = ((K + 15 + 15) & ~15) <= 224 ? K : 200, nq = (K + kq - 1) / kq;
     const int nbw = (kq + 15 + 15) & ~15;
     const bool tc_ok = p.WW <= 128 && (long long)p.WW * nq <= 4096;
     if (response_mode == LARTPC_RESPONSE_TENSOR && !tc_ok) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }

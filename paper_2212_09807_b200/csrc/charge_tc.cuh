@@ -471,7 +471,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             if (tid < NB2) {
                 // rows of the response's operand image; only the 16-tick blocks some tile of the block charges exist
                 const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;
-                const int bm = a.tb_mask[tb];
+                const int bm = a.tb_mask[tile / TC_UNIT_TILES];
                 unsigned char *cb = (unsigned char *)a.charge + ((size_t)tb * NB2 + tid) * (rtc::NBLK * rtc::A_BLOCK_BYTES);
 #pragma unroll
                 for (int b = 0; b < rtc::NBLK; ++b) {

@@ -35,7 +35,7 @@ struct DevParams {
     int NBW;                         // tensor-core mode: output columns per 16-tick arrival block, roundup16(KQ + 15)
     int b_scale_log2;                // tensor-core mode: the LUT operand is R * 2^b_scale_log2, chosen per LUT so that max |R| lands
                                      // in (2^9, 2^10] (fp16 / e4m3 range of the fixed part splits, response_tc.cuh)
-    int KQ, nq;                      // tensor-core mode: LUT ticks per piece and pieces (K <= 241: one piece of K ticks; longer
+    int KQ, nq;                      // tensor-core mode: LUT ticks per piece and pieces (K <= 209: one piece of K ticks; longer
                                      // LUTs are cut into pieces of 200 ticks, each a row of its own in `partial`, added by S5)
     int n_tpcs;
     // electronics
@@ -64,7 +64,10 @@ constexpr int SLAB_HDR = 4;          // slab header ints: bins, charge groups, f
 constexpr int RESP_NO = 14;          // output ticks per response task (one thread: RESP_NO ticks x 2 target pixels)
 constexpr int RESP_CONSUMERS = 256;  // consumer threads of the response kernel (8 warps, two per SM sub-partition)
 constexpr int TILE_META = 4;         // ints per tile in lartpc_signals_t.tile_range: first / last output block, scale exponent, 0
-constexpr int TC_TILE_BLOCK = 128;   // tiles per tensor-core tile block (MMA M)
+constexpr int TC_TILE_BLOCK = 128;   // tiles per tensor-core tile block (MMA M of one CTA)
+constexpr bool TC_CTA_PAIR = false;  // the tensor-core response runs as CTA pairs (cta_group::2, M = 256 over two tile blocks)
+constexpr int TC_UNIT_TILES = TC_CTA_PAIR ? 2 * TC_TILE_BLOCK : TC_TILE_BLOCK;   // tiles one response item multiplies at once:
+                                     // the 16-tick block masks (tb_mask) are kept per unit
 
 // device counters written by the planning kernels (mirrored to pinned host memory)
 enum {
@@ -230,7 +233,7 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
 size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_out);   // returns bytes, 0 on failure
 static inline int64_t tiles_alloc(const DevParams &p, int64_t n_tiles)
 {
-    return p.tc_mode ? (n_tiles + TC_TILE_BLOCK - 1) / TC_TILE_BLOCK * TC_TILE_BLOCK : n_tiles;
+    return p.tc_mode ? (n_tiles + TC_UNIT_TILES - 1) / TC_UNIT_TILES * TC_UNIT_TILES : n_tiles;
 }
 int launch_pack_hits(lartpc_sim *sim, const lartpc_hits_t *hits, int64_t n_hits, int tile_pixels, uint16_t *packed,
                      int64_t *tile_offsets, cudaStream_t st);

@@ -43,23 +43,20 @@ namespace rtc {
 constexpr int TB = 128;            // tiles per tile block (MMA M)
 constexpr int JC = 64;             // arrival ticks per tile (K extent per bin): 4 blocks of 16
 constexpr int NBLK = JC / 16;
-constexpr int STAGES = 3;
-constexpr int A_SLOTS = 6;          // charge blocks a stage can hold: 4 of one tile block, or 3 + 3 of a pair
-constexpr int THREADS = 192;
+constexpr int THREADS = 224;          // 7 warps: producer, MMA issuer (even blocks) / relay, 4 x epilogue, MMA issuer (odd blocks)
 // fp8 parts: lo8(A) = e4m3(lo(A) 2^SA) meets hi8(B) = e4m3(B 2^-SA); hi8(A) = e4m3(A 2^-SB) meets lo8(B) = e4m3(lo(B) 2^SB)
 // (|A| < 2^15, |lo(A)| <= 8, |B| <= 2^10, |lo(B)| <= 0.5: every part stays below e4m3's 448)
 constexpr int SA_LOG2 = 5, SB_LOG2 = 7;
-constexpr int A_HALF_BYTES = TB * JC * 2;          // half of a stage's A area (the area holds NBLK blocks of 8 KB)
 
 struct Args {
     const __half *A;               // [n_tb][NC][2][TB][128 bytes]: fp16 image (a_image_offset) + fp8 image (a8_image_offset)
-    const __half *B;               // [WW][NC][2][NBW * 32 bytes]: fp16 image (b_image_offset) + fp8 image (b8_image_offset)
+    const __half *B;               // [WW][NC][CTA of the pair][fp16 image (b_image_offset) | fp8 image (b8_image_offset)] of that CTA's rows
     float *partial;                // [n_tiles][WW][tile_ticks]
     const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), 0
-    const int32_t *tb_mask;        // [n_tb] 16-tick blocks that hold charge in any tile of the block (bit b)
-    int n_tiles, n_tb, NC, WW, NBW, tile_ticks;
+    const int32_t *tb_mask;        // [n_units] 16-tick blocks that hold charge in any tile of the unit (bit b)
+    int n_tiles, n_units, NC, WW, NBW, tile_ticks, n_stages;
     int b_scale_log2;              // B = R * 2^b_scale_log2 (DevParams)
-    long long n_items;             // ceil(n_tb / 2) * WW * 2: (unit of two tile blocks, row, half)
+    long long n_items;             // n_units * WW: (unit, row of the LUT image)
     int *work;                     // item cursor, zero at launch: items are taken in order as CTAs become free, so the
                                    // CTAs that stream one tile block stay together however long the launch runs
 };
@@ -193,89 +190,239 @@ __device__ __forceinline__ void tmem_zero16(uint32_t taddr)
         "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};\n" ::"r"(taddr), "r"(z) : "memory");
 }
 
-constexpr int stage_bytes(int NBW) { return A_SLOTS * A_BLOCK_BYTES + 2 * NBW * 32; }
-constexpr int smem_bytes(int NBW) { return STAGES * stage_bytes(NBW) + 1024 /* alignment slack */ + 256 /* barriers, headers */; }
-constexpr int HDR_LAST = 1, HDR_END = 2;
-constexpr int PAIR_COL = 256;      // TMEM column of the second accumulator of a pair item
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr) : "memory");
+}
 
-// Two tile blocks share an item -- and with it every LUT generator the item streams -- when each charges at most three
-// consecutive 16-tick blocks: an accumulator then needs 32 + NBW <= 256 columns (counted from the block's first charged
-// block), and two fit the 512 TMEM columns.
-__device__ __forceinline__ bool pairable_mask(int m) { return m != 0 && (31 - __clz(m)) - (__ffs(m) - 1) <= 2; }
+// ---- cluster (CTA pair) helpers -----------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+// shared::cluster address of `addr` (a shared::cta address of this CTA) in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)       // acquire at cluster scope
+{
+    uint32_t ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    }
+}
+// remote arrive that orders nothing but the barrier itself (what it reports was written by the async proxy and is
+// read by the async proxy)
+__device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t cluster_bar)
+{
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_bar)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx_remote(uint32_t cluster_bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.release.cluster.shared::cluster.b64 _, [%0], %1;" ::"r"(cluster_bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void st_cluster_v4(uint32_t cluster_addr, int x, int y, int z, int w)
+{
+    asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(cluster_addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+template <bool CTA2> __device__ __forceinline__ void tc_mma(bool f8, uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc)
+{
+    // every MMA accumulates (the epilogue leaves the accumulators zero)
+    if (CTA2) {
+        if (f8) asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, 1, 0;\ntcgen05.mma.cta_group::2.kind::f8f6f4 [%0], %1, %2, %3, p;\n}\n"
+                             ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc) : "memory");
+        else asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, 1, 0;\ntcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n}\n"
+                          ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc) : "memory");
+    } else {
+        if (f8) tc_mma_f8(d_tmem, a_desc, b_desc, idesc, 1u);
+        else tc_mma_f16(d_tmem, a_desc, b_desc, idesc, 1u);
+    }
+}
+// commit of everything this thread has issued so far: arrive on `bar` of this CTA, or (cta_mask) of both CTAs of the pair
+template <bool CTA2> __device__ __forceinline__ void tc_commit_x(uint32_t bar, bool both)
+{
+    if (!CTA2) { tc_commit(bar); return; }
+    if (both) {
+        const unsigned short mask = 3;
+        asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                     ::"r"(bar), "h"(mask) : "memory");
+    } else {
+        asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+    }
+}
 
-// Work items.  Unit u = tile blocks 2u, 2u + 1; cursor value q = (u * rows + d) * 2 + h.  A pairable unit is one item per
-// row d (h = 0; h = 1 is skipped); otherwise h picks the tile block.  Consecutive q share their charge blocks.
+#ifdef LARTPC_DEBUG_CLOCKS
+__device__ unsigned long long g_rtc_dbg[16];   // measurement build: cycles the MMA issuer / producer spend per phase
+#define RTC_T(x) const long long x = clock64()
+#define RTC_ADD(i, v) atomicAdd(&g_rtc_dbg[i], (unsigned long long)(v))
+#else
+#define RTC_T(x)
+#define RTC_ADD(i, v)
+#endif
+constexpr int MAX_STAGES = 8;
+constexpr int N_MAIL = MAX_STAGES + 2;  // item mailbox slots of the peer: the leader's producer is never more than a ring ahead
+constexpr int HDR_FIRST = 1, HDR_LAST = 2, HDR_END = 4;
+constexpr int ACC_COL = 256;       // TMEM column of the second accumulator (odd 16-tick blocks)
+
+// bytes of Bs one CTA holds per (target, bin): both precision parts of all rows, or of half the rows with the CTA pair
+__host__ __device__ inline uint32_t b_cta_bytes(int NBW, bool cta2) { return (uint32_t)(cta2 ? NBW * 32 : NBW * 64); }
+// a stage = the A blocks of one bin (up to NBLK, 8 KB each: fp16 + fp8 part) + this CTA's rows of the bin's generator
+__host__ __device__ inline uint32_t stage_bytes(int NBW, bool cta2)
+{
+    return (uint32_t)((NBLK * A_BLOCK_BYTES + b_cta_bytes(NBW, cta2) + 1023) & ~1023);
+}
+inline int n_stages(int NBW, bool cta2, size_t smem_limit)
+{
+    const int n = (int)((smem_limit - 3072) / stage_bytes(NBW, cta2));
+    return n > MAX_STAGES ? MAX_STAGES : n;
+}
+inline size_t smem_bytes(int NBW, bool cta2, int stages) { return (size_t)stages * stage_bytes(NBW, cta2) + 1024 /* alignment */ + 2048 /* barriers, headers */; }
+
+// Work item = (unit u, row d of the LUT image).  Cursor value q = u * rows + d: consecutive items share their charge
+// blocks, and the CTAs that stream one unit do it at about the same time, so A comes from HBM once.
+//
+// Roles (192 threads per CTA; with CTA2 the kernel runs as clusters of two CTAs on one TPC, rank 0 = leader):
+//   warp 0, one lane   producer, in every CTA, filling its own shared memory with its own TMA engine (copies into the
+//                      partner's memory would cross the SM-to-SM network at a fraction of the rate).  One stage per
+//                      (item, bin c): the A blocks (fp16 + fp8 part) of the charged 16-tick blocks of this CTA's tile
+//                      block -- ONE bulk copy per run of consecutive charged blocks, they are neighbours in the image --
+//                      and this CTA's rows of the generator, one more copy (the LUT image is laid out per CTA of the pair).
+//                      The issue rate of cp.async.bulk by one thread is what bounds the kernel otherwise (measured:
+//                      ~250 cycles per copy).  The leader takes the items from the cursor and posts each item's header
+//                      in the peer's mailbox, one message per item; after that the two producers run on their own,
+//                      paced by their own empty barriers (the MMA issuer's commits arrive in both CTAs).
+//   warp 1, one lane   leader: MMA issuer.  Per stage: waits full (and pfull: the peer's share has landed), issues the
+//                      fp16 and the fp8 tcgen05.mma of every charged block (M = 128, or 256 over the pair with
+//                      cta_group::2: each CTA multiplies its own 128 tiles by the whole generator, of which it holds half
+//                      the rows), commits empty; after an item's last stage tfull, in both CTAs.
+//                      peer: relay.  Waits its own full and arrives on the leader's pfull.
+//   warps 2-5          epilogue, every CTA: adds the two accumulators, undoes the scales, writes the partial rows of
+//                      its own tile block, zeroes the accumulators, arrives on the leader's tempty.
+// Accuracy.  tcgen05.mma adds into the fp32 accumulator with truncation (toward zero: measured), so a long accumulation
+// chain loses a fraction of an ulp per product, systematically.  Even and odd 16-tick blocks therefore accumulate into
+// separate accumulators (columns [0, 256) and [256, 512): block b at column 32 (b / 2) of accumulator b % 2), which the
+// epilogue adds in round-to-nearest: half as many products per accumulator.
+template <bool CTA2>
 __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
 {
     extern __shared__ unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int NBW = a.NBW, NC = a.NC;
-    const uint32_t b_half = (uint32_t)NBW * 32u;                       // bytes of one precision half of a Bs image
-    const uint32_t a_area = (uint32_t)A_SLOTS * A_BLOCK_BYTES;
-    const uint32_t stage_sz = a_area + 2u * b_half;                    // multiple of 1024 (NBW multiple of 16)
+    const uint32_t rank = CTA2 ? cluster_ctarank() : 0u;
+    const bool leader = rank == 0u;
+    const int NBW = a.NBW, NC = a.NC, S = a.n_stages;
+    const uint32_t b_cta = b_cta_bytes(NBW, CTA2);                     // this CTA's rows of a generator: fp16 part, fp8 part
+    const uint32_t a_area = (uint32_t)NBLK * A_BLOCK_BYTES;
+    const uint32_t stage_sz = stage_bytes(NBW, CTA2);
     const uint32_t base = (s32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bars = base + STAGES * stage_sz;                    // full[S], empty[S], tmem_full, tmem_empty, tmem ptr
-    const uint32_t full0 = bars, empty0 = bars + 8 * STAGES, tfull = bars + 16 * STAGES, tempty = tfull + 8;
-    const uint32_t titem = tempty + 8, tptr_addr = titem + 8;
-    volatile uint32_t *tptr = (volatile uint32_t *)(smem_raw + (tptr_addr - s32(smem_raw)));
-    volatile int4 *hdr = (volatile int4 *)(smem_raw + (tptr_addr + 8 - s32(smem_raw)));   // [STAGES] {tbA, d, c | masks, flags}
-    volatile int4 *epi_item = hdr + STAGES;                                              // {tbA, d, masks, flags}
-    const bool pairs_fit = 32 + NBW <= PAIR_COL;
+    const uint32_t bars = base + (uint32_t)S * stage_sz;
+    const uint32_t full0 = bars, empty0 = full0 + 8 * MAX_STAGES, pfull0 = empty0 + 8 * MAX_STAGES;
+    const uint32_t gox0 = pfull0 + 8 * MAX_STAGES;
+    const uint32_t tfull = gox0 + 8 * N_MAIL, tempty = tfull + 8, titem = tempty + 8, tptr_addr = titem + 8;
+    const uint32_t hdr0 = (tptr_addr + 8 + 15u) & ~15u, epi0 = hdr0 + 16 * MAX_STAGES, mail0 = epi0 + 16;
+    unsigned char *gen = smem_raw - s32(smem_raw);                     // shared::cta address -> generic pointer
+    volatile uint32_t *tptr = (volatile uint32_t *)(gen + tptr_addr);
+    volatile int4 *hdr = (volatile int4 *)(gen + hdr0);                // [S] {unit, d, c | mask << 16, flags}
+    volatile int4 *epi_item = (volatile int4 *)(gen + epi0);           // {unit, d, mask, flags}
 
     if (tid == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
-        mbar_init(tfull, 1);
-        mbar_init(tempty, 4);                                          // one arrival per epilogue warp
+        // empty[s] and tfull take one commit from each of the two MMA issuers
+        for (int s = 0; s < S; ++s) { mbar_init(full0 + 8 * s, 1);  mbar_init(empty0 + 8 * s, 2);  mbar_init(pfull0 + 8 * s, 1); }
+        for (int m = 0; m < N_MAIL; ++m) mbar_init(gox0 + 8 * m, 1);
+        mbar_init(tfull, 2);
+        mbar_init(tempty, CTA2 ? 8 : 4);                               // one arrival per epilogue warp of the pair
         mbar_init(titem, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 1) {                                                   // the MMA warp owns the TMEM allocation
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tptr_addr), "r"(512u) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (warp == 1) {                                                   // warp 1 of every CTA owns its TMEM allocation
+        if (CTA2) {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tptr_addr), "r"(512u) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tptr_addr), "r"(512u) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
     }
     tc_fence_before();
     __syncthreads();
+    if (CTA2) cluster_sync_all();                                      // barriers and TMEM of both CTAs exist
     tc_fence_after();
     const uint32_t tmem = *tptr;
-    const int n_acc_cols = 16 * (NBLK - 1) + NBW;                      // columns of a single item's accumulator (272)
 
     if (warp == 0) {
-        // ------------------------------------------------------------------ producer
         if (lane == 0) {
-            int s = 0;
-            uint32_t ph = 0;
-            long long q = atomicAdd(a.work, 1);
-            while (q < a.n_items) {
-                const long long q_next = atomicAdd(a.work, 1);         // in flight while this item streams
-                const int h = (int)(q & 1);
-                const long long ud = q >> 1;
-                const int u = (int)(ud / a.WW), d = (int)(ud - (long long)u * a.WW);
-                const int tb0 = 2 * u, tb1 = tb0 + 1;
-                const int m0 = a.tb_mask[tb0] & ((1 << NBLK) - 1), m1 = tb1 < a.n_tb ? a.tb_mask[tb1] & ((1 << NBLK) - 1) : 0;
-                const bool pair = pairs_fit && pairable_mask(m0) && pairable_mask(m1);
-                int tbA, bmA, bmB = 0;
-                if (pair) { tbA = tb0;  bmA = m0;  bmB = m1; }
-                else { tbA = h ? tb1 : tb0;  bmA = h ? m1 : m0; }
-                if ((pair && h) || bmA == 0) { q = q_next;  continue; }   // the pair went out with h = 0; nothing charged
-                const unsigned char *AbA = (const unsigned char *)a.A + (size_t)tbA * NC * (NBLK * A_BLOCK_BYTES);
-                const unsigned char *AbB = AbA + (size_t)NC * (NBLK * A_BLOCK_BYTES);   // tile block tbA + 1
-                const unsigned char *Bb = (const unsigned char *)a.B + (size_t)d * NC * (2 * b_half);
-                const uint32_t a_bytes = (uint32_t)(__popc(bmA) + __popc(bmB)) * A_BLOCK_BYTES;
+            // ------------------------------------------------------------------ producer (leader: schedules; peer: follows)
+            const uint32_t peer_gox0 = CTA2 ? mapa(gox0, 1u) : 0u, peer_mail0 = CTA2 ? mapa(mail0, 1u) : 0u;
+            volatile int4 *mail = (volatile int4 *)(gen + mail0);
+            const size_t tb_stride = (size_t)NC * (NBLK * A_BLOCK_BYTES);
+            const size_t b_stride = (size_t)(CTA2 ? 2 : 1) * b_cta;    // one (target, bin) of the LUT image: [CTA of the pair][fp16 | fp8]
+            int s = 0, m = 0;
+            uint32_t ph = 0, mph = 0;
+            long long q = leader ? atomicAdd(a.work, 1) : 0;
+            while (true) {
+                int u, d, mask;
+                long long q_next = 0;
+                if (leader) {
+                    const bool end = q >= a.n_items;
+                    u = d = mask = 0;
+                    if (!end) {
+                        q_next = atomicAdd(a.work, 1);                 // in flight while this item streams
+                        u = (int)(q / a.WW);  d = (int)(q - (long long)u * a.WW);
+                        mask = a.tb_mask[u] & ((1 << NBLK) - 1);
+                        if (mask == 0) { q = q_next;  continue; }      // nothing charged
+                    }
+                    if (CTA2) { st_cluster_v4(peer_mail0 + 16 * m, u, d, mask, end ? HDR_END : 0);  mbar_arrive_remote(peer_gox0 + 8 * m); }
+                    if (end) break;
+                } else {
+                    mbar_wait_cluster(gox0 + 8 * m, mph);
+                    if (mail[m].w & HDR_END) break;
+                    u = mail[m].x;  d = mail[m].y;  mask = mail[m].z;
+                }
+                if (++m == N_MAIL) { m = 0; mph ^= 1u; }
+                const unsigned char *Ab = (const unsigned char *)a.A + ((size_t)u * (CTA2 ? 2 : 1) + rank) * tb_stride;
+                const unsigned char *Bd = (const unsigned char *)a.B + (size_t)d * NC * b_stride + (size_t)rank * b_cta;
+                const uint32_t bytes = (uint32_t)__popc(mask) * A_BLOCK_BYTES + b_cta;
+                // runs of consecutive charged blocks: {first block, length}, at most two in four bits
+                const int r0b = __ffs(mask) - 1, r0n = __ffs(~(mask >> r0b)) - 1;
+                const int rest = mask & ~(((1 << r0n) - 1) << r0b);
+                const int r1b = rest ? __ffs(rest) - 1 : 0, r1n = rest ? __popc(rest) : 0;
                 for (int c = 0; c < NC; ++c) {
-                    mbar_wait(empty0 + 8 * s, ph ^ 1u);
                     const uint32_t st = base + s * stage_sz, fb = full0 + 8 * s;
-                    hdr[s].x = tbA;  hdr[s].y = d;  hdr[s].z = c | (bmA << 16) | (bmB << 20);
-                    hdr[s].w = (c == NC - 1) ? HDR_LAST : 0;
-                    mbar_expect_tx(fb, a_bytes + 2 * b_half);          // release: the header is visible to the waiter
-                    uint32_t dst = st;
-#pragma unroll
-                    for (int b = 0; b < NBLK; ++b)
-                        if (bmA >> b & 1) { bulk_g2s(dst, AbA + ((size_t)c * NBLK + b) * A_BLOCK_BYTES, A_BLOCK_BYTES, fb);  dst += A_BLOCK_BYTES; }
-#pragma unroll
-                    for (int b = 0; b < NBLK; ++b)
-                        if (bmB >> b & 1) { bulk_g2s(dst, AbB + ((size_t)c * NBLK + b) * A_BLOCK_BYTES, A_BLOCK_BYTES, fb);  dst += A_BLOCK_BYTES; }
-                    bulk_g2s(st + a_area, Bb + (size_t)c * (2 * b_half), 2 * b_half, fb);
-                    if (++s == STAGES) { s = 0; ph ^= 1u; }
+                    RTC_T(p0);
+                    mbar_wait(empty0 + 8 * s, ph ^ 1u);
+                    RTC_T(p1);
+                    hdr[s].x = u;  hdr[s].y = d;  hdr[s].z = c | (mask << 16);
+                    hdr[s].w = (c == 0 ? HDR_FIRST : 0) | (c == NC - 1 ? HDR_LAST : 0);
+                    mbar_expect_tx(fb, bytes);                         // release: the header is visible to the waiter
+                    const unsigned char *Ac = Ab + (size_t)c * NBLK * A_BLOCK_BYTES;
+                    bulk_g2s(st, Ac + r0b * A_BLOCK_BYTES, (uint32_t)r0n * A_BLOCK_BYTES, fb);
+                    if (r1n) bulk_g2s(st + r0n * A_BLOCK_BYTES, Ac + r1b * A_BLOCK_BYTES, (uint32_t)r1n * A_BLOCK_BYTES, fb);
+                    bulk_g2s(st + a_area, Bd + (size_t)c * b_stride, b_cta, fb);
+                    RTC_T(p2);  RTC_ADD(8, p1 - p0);  RTC_ADD(9, p2 - p1);  RTC_ADD(10, 1);
+                    if (++s == S) { s = 0; ph ^= 1u; }
                 }
                 q = q_next;
             }
@@ -283,131 +430,149 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
             hdr[s].w = HDR_END;
             mbar_arrive(full0 + 8 * s);
         }
-    } else if (warp == 1) {
-        // ------------------------------------------------------------------ MMA issuer
-        if (lane == 0) {
+    } else if (warp == 1 || warp == 6) {
+        if (lane == 0 && !leader && warp == 1) {
+            // ---------------------------------------------------------------------- relay (peer): this CTA's share of
+            // stage s has landed -> tell the leader's MMA issuer.  Nothing but the barrier needs ordering here: what it
+            // reports was written by the async proxy (TMA) and is read by the async proxy (tensor core).
+            const uint32_t lead_pfull0 = mapa(pfull0, 0u);
+            int s = 0;
+            uint32_t ph = 0;
+            while (true) {
+                mbar_wait(full0 + 8 * s, ph);
+                const int flags = hdr[s].w;
+                mbar_arrive_remote_relaxed(lead_pfull0 + 8 * s);
+                if (flags & HDR_END) break;
+                if (++s == S) { s = 0; ph ^= 1u; }
+            }
+        }
+        if (lane == 0 && leader) {
+            // ---------------------------------------------------------------------- MMA issuers (leader): warp 1 takes the
+            // even 16-tick blocks (first accumulator) and hands the items to the epilogue, warp 6 the odd blocks (second
+            // accumulator).  One thread issues a tcgen05.mma every ~90 cycles at best, below the 118 cycles the tensor
+            // core needs for one, and pays ~400 cycles per stage for its waits, header and commit on top (measured):
+            // a single issuer cannot keep the pipe busy.  The two accumulators are independent, so the order between
+            // the two threads' MMAs does not matter; each commits every stage (and item) once.
+            const int par = warp == 1 ? 0 : 1;
             // instruction descriptor: D fp32, A and B fp16 (kind::f16) or e4m3 (kind::f8f6f4) -- format code 0 in both
-            // kinds --, both K-major, N = NBW, M = 128
-            const uint32_t idesc = (1u << 4) | ((uint32_t)(NBW >> 3) << 17) | ((uint32_t)(TB >> 4) << 24);
+            // kinds --, both K-major, N = NBW, M = 128 per CTA
+            const uint32_t idesc = (1u << 4) | ((uint32_t)(NBW >> 3) << 17) | ((uint32_t)((CTA2 ? 2 * TB : TB) >> 4) << 24);
+            const uint32_t peer_epi = CTA2 ? mapa(epi0, 1u) : 0u, peer_titem = CTA2 ? mapa(titem, 1u) : 0u;
             int s = 0;
             uint32_t ph = 0, tph = 0;
             while (true) {
+                RTC_T(t0);
                 mbar_wait(full0 + 8 * s, ph);
-                const int tbA = hdr[s].x, d = hdr[s].y, cz = hdr[s].z, flags = hdr[s].w;
-                const int c = cz & 0xffff, bmA = (cz >> 16) & 15, bmB = (cz >> 20) & 15;
+                RTC_T(t1);
+                if (CTA2) mbar_wait(pfull0 + 8 * s, ph);
+                RTC_T(t2);
+                int u, d, cz, flags;
+                asm volatile("ld.volatile.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(u), "=r"(d), "=r"(cz), "=r"(flags) : "r"(hdr0 + 16 * s) : "memory");
+                const int mask = (cz >> 16) & 15;
                 if (flags & HDR_END) {
-                    mbar_wait(tempty, tph);                            // the epilogue has read the previous item slot
+                    if (par) break;
+                    mbar_wait_cluster(tempty, tph);                    // the epilogues have read the previous item slot
                     epi_item->w = HDR_END;
                     mbar_arrive(titem);
+                    if (CTA2) { st_cluster_v4(peer_epi, 0, 0, 0, HDR_END);  mbar_arrive_remote(peer_titem); }
                     break;
                 }
-                if (c == 0) {
-                    mbar_wait(tempty, tph);                            // accumulators drained and zeroed
-                    epi_item->x = tbA;  epi_item->y = d;  epi_item->z = bmA | (bmB << 4);  epi_item->w = 0;
-                    mbar_arrive(titem);                                // release: hands the item to the epilogue
+                if (flags & HDR_FIRST) {
+                    mbar_wait_cluster(tempty, tph);                    // accumulators drained and zeroed, in both CTAs
+                    tph ^= 1u;
+                    if (!par) {
+                        epi_item->x = u;  epi_item->y = d;  epi_item->z = mask;  epi_item->w = 0;
+                        mbar_arrive(titem);                            // release: hands the item to the epilogue
+                        if (CTA2) { st_cluster_v4(peer_epi, u, d, mask, 0);  mbar_arrive_remote(peer_titem); }
+                    }
                 }
                 tc_fence_after();
+                RTC_T(t3);
                 const uint32_t st = base + s * stage_sz;
-                const uint64_t bd_hi = smem_desc(st + a_area, 128, 256, 0);
-                const uint64_t bd_8 = smem_desc(st + a_area + b_half, 128, 256, 0);
-                // single item: block b lands at column 16 b; pair: at 16 (b - first charged block) of its own accumulator
-                const int lbA = bmB ? __ffs(bmA) - 1 : 0, lbB = bmB ? __ffs(bmB) - 1 : 0;
+                const uint64_t bd16 = smem_desc(st + a_area, 128, 256, 0), bd8 = smem_desc(st + a_area + b_cta / 2, 128, 256, 0);
                 uint32_t src = st;
 #pragma unroll
                 for (int b = 0; b < NBLK; ++b) {
-                    if (!(bmA >> b & 1)) continue;                     // no tile of the block has charge in these 16 ticks
-                    const uint32_t dcol = tmem + 16 * (b - lbA);
-                    tc_mma_f16(dcol, smem_desc(src, 128, 256, 0), bd_hi, idesc, 1u);   // the epilogue leaves the accumulators zero
-                    tc_mma_f8(dcol, smem_desc(src + A_PART_BYTES, 128, 256, 0), bd_8, idesc, 1u);
+                    if (!(mask >> b & 1)) continue;                    // no tile of the unit has charge in these 16 ticks
+                    if ((b & 1) == par) {
+                        const uint32_t dcol = tmem + (b & 1 ? ACC_COL : 0) + 32 * (b >> 1);
+                        tc_mma<CTA2>(false, dcol, smem_desc(src, 128, 256, 0), bd16, idesc);
+                        tc_mma<CTA2>(true, dcol, smem_desc(src + A_PART_BYTES, 128, 256, 0), bd8, idesc);
+                    }
                     src += A_BLOCK_BYTES;
                 }
-#pragma unroll
-                for (int b = 0; b < NBLK; ++b) {
-                    if (!(bmB >> b & 1)) continue;
-                    const uint32_t dcol = tmem + PAIR_COL + 16 * (b - lbB);
-                    tc_mma_f16(dcol, smem_desc(src, 128, 256, 0), bd_hi, idesc, 1u);
-                    tc_mma_f8(dcol, smem_desc(src + A_PART_BYTES, 128, 256, 0), bd_8, idesc, 1u);
-                    src += A_BLOCK_BYTES;
-                }
-                tc_commit(empty0 + 8 * s);                             // stage free once these MMAs have read it
-                if (flags & HDR_LAST) { tc_commit(tfull); tph ^= 1u; } // accumulators complete
-                if (++s == STAGES) { s = 0; ph ^= 1u; }
+                RTC_T(t4);
+                tc_commit_x<CTA2>(empty0 + 8 * s, true);               // stage free, in both CTAs, once these MMAs have read it
+                if (flags & HDR_LAST) tc_commit_x<CTA2>(tfull, true);  // accumulators complete, in both CTAs
+                RTC_T(t5);
+                RTC_ADD(0, t1 - t0);  RTC_ADD(1, t2 - t1);  RTC_ADD(2, t3 - t2);  RTC_ADD(3, t4 - t3);  RTC_ADD(4, t5 - t4);  RTC_ADD(5, 1);
+                if (++s == S) { s = 0; ph ^= 1u; }
             }
         }
     } else {
-        // ------------------------------------------------------------------ epilogue (warps 2-5)
+        // ---------------------------------------------------------------------- epilogue (warps 2-5, every CTA)
         const int quad = warp & 3;                                     // TMEM lanes [32 quad, 32 quad + 32)
         const uint32_t tlane = tmem + ((uint32_t)(32 * quad) << 16);
+        const uint32_t lead_tempty = CTA2 ? mapa(tempty, 0u) : tempty;
         // every MMA accumulates: the accumulators are zero before the first item and zeroed again after each read-out
         for (int c0 = 0; c0 < 512; c0 += 16) tmem_zero16(tlane + c0);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(tempty);
-        uint32_t tph = 0;
+        if (lane == 0) { if (CTA2) mbar_arrive_remote(lead_tempty); else mbar_arrive(tempty); }
+        uint32_t iph = 0;
         while (true) {
-            mbar_wait(titem, tph);                                     // acquire: the MMA warp has published the item
+            // one lane polls (128 threads spinning on a barrier for the ~30 us an item takes cost issue slots and power)
+            if (lane == 0) mbar_wait_cluster(titem, iph);              // acquire: the MMA warp has published the item
+            __syncwarp();
             if (epi_item->w & HDR_END) break;
-            const int tbA = epi_item->x, d = epi_item->y, masks = epi_item->z;
-            const int bmA = masks & 15, bmB = (masks >> 4) & 15;
-            const int n_acc = bmB ? 2 : 1;
-            mbar_wait(tfull, tph);
+            const int u = epi_item->x, d = epi_item->y, mask = epi_item->z;
+            if (lane == 0) mbar_wait(tfull, iph);
+            __syncwarp();
             tc_fence_after();
-            for (int x = 0; x < n_acc; ++x) {
-                // accumulator x: tile block tbA + x; its column 0 is tick t0 of the tile's window
-                const int tile = (tbA + x) * TB + 32 * quad + lane;
-                const bool live = tile < a.n_tiles;
-                const int t0 = bmB ? 16 * (__ffs(x ? bmB : bmA) - 1) : 0;
-                const int n_cols = bmB ? min(PAIR_COL, a.tile_ticks - t0) : a.tile_ticks;     // multiples of 8
-                const uint32_t tcol = tlane + (x ? PAIR_COL : 0);
-                float scale = 0.f;
-                if (live) scale = __int_as_float((127 + a.tile_meta[4 * tile + 2] - a.b_scale_log2) << 23);
-                float *dst = a.partial + ((size_t)(live ? tile : 0) * a.WW + d) * a.tile_ticks + t0;
-                if (bmB && live) {
-                    // S5 reads whole 14-tick blocks around the charged range: the few ticks of the row the accumulator
-                    // does not cover (before the first charged block, after column 255) are zero
-                    float *row = dst - t0;
-                    for (int i = 0; i < t0; i += 4) __stcs((float4 *)(row + i), make_float4(0.f, 0.f, 0.f, 0.f));
-                    for (int i = t0 + n_cols; i < a.tile_ticks; i += 4) __stcs((float4 *)(row + i), make_float4(0.f, 0.f, 0.f, 0.f));
-                }
-                const int n_full = n_cols / 32;
-                for (int ch = 0; ch < n_full; ++ch) {
-                    uint32_t v[32];
-                    tmem_ld32(tcol + 32 * ch, v);
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                    if (live) {
+            const int tile = (u * (CTA2 ? 2 : 1) + (int)rank) * TB + 32 * quad + lane;
+            const bool live = tile < a.n_tiles;
+            const bool even = (mask & 5) != 0, odd = (mask & 10) != 0;
+            float scale = 0.f;
+            if (live) scale = __int_as_float((127 + a.tile_meta[4 * tile + 2] - a.b_scale_log2) << 23);
+            float *dst = a.partial + ((size_t)(live ? tile : 0) * a.WW + d) * a.tile_ticks;
+            // output tick n = even accumulator column n (blocks 0, 2) + odd accumulator column n - 16 (blocks 1, 3)
+            for (int n0 = 0; n0 < a.tile_ticks; n0 += 16) {
+                uint32_t v0[16], v1[16];
+                const bool has0 = even && n0 < ACC_COL, has1 = odd && n0 >= 16;
+                if (has0) tmem_ld16(tlane + n0, v0);
+                if (has1) tmem_ld16(tlane + ACC_COL + n0 - 16, v1);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (live) {
+                    const int nv = min(16, a.tile_ticks - n0);         // tile_ticks is a multiple of 8
 #pragma unroll
-                        for (int i = 0; i < 8; ++i)
-                            __stcs((float4 *)(dst + 32 * ch) + i, make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
-                                                                         __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale));
-                    }
-                }
-                for (int c0 = 32 * n_full; c0 < n_cols; c0 += 8) {
-                    uint32_t v[8];
-                    tmem_ld8(tcol + c0, v);
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                    if (live) {
-#pragma unroll
-                        for (int i = 0; i < 2; ++i)
-                            __stcs((float4 *)(dst + c0) + i, make_float4(__uint_as_float(v[4 * i]) * scale, __uint_as_float(v[4 * i + 1]) * scale,
-                                                                    __uint_as_float(v[4 * i + 2]) * scale, __uint_as_float(v[4 * i + 3]) * scale));
+                    for (int i = 0; i < 4; ++i) {
+                        if (4 * i >= nv) break;
+                        float4 o;
+                        o.x = ((has0 ? __uint_as_float(v0[4 * i]) : 0.f) + (has1 ? __uint_as_float(v1[4 * i]) : 0.f)) * scale;
+                        o.y = ((has0 ? __uint_as_float(v0[4 * i + 1]) : 0.f) + (has1 ? __uint_as_float(v1[4 * i + 1]) : 0.f)) * scale;
+                        o.z = ((has0 ? __uint_as_float(v0[4 * i + 2]) : 0.f) + (has1 ? __uint_as_float(v1[4 * i + 2]) : 0.f)) * scale;
+                        o.w = ((has0 ? __uint_as_float(v0[4 * i + 3]) : 0.f) + (has1 ? __uint_as_float(v1[4 * i + 3]) : 0.f)) * scale;
+                        __stcs((float4 *)(dst + n0) + i, o);
                     }
                 }
             }
-            const int n_zero = bmB ? 512 : n_acc_cols;
-            for (int c0 = 0; c0 < n_zero; c0 += 16) tmem_zero16(tlane + c0);
+            if (even) for (int c0 = 0; c0 < ACC_COL; c0 += 16) tmem_zero16(tlane + c0);
+            if (odd) for (int c0 = ACC_COL; c0 < 2 * ACC_COL; c0 += 16) tmem_zero16(tlane + c0);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(tempty);
-            tph ^= 1u;
+            if (lane == 0) { if (CTA2) mbar_arrive_remote(lead_tempty); else mbar_arrive(tempty); }
+            iph ^= 1u;
         }
     }
     tc_fence_before();
     __syncthreads();
+    if (CTA2) cluster_sync_all();                                      // nobody leaves while its partner may still signal it
     if (warp == 1) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+        if (CTA2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+        else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
     }
 }
 

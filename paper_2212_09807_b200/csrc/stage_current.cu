@@ -14,7 +14,7 @@
 //   response_tc_kernel        I = C x Toeplitz(R): per (128-tile block, target, bin) the charged 16-tick blocks of the
 //                             operand image against one 16 x NBW LUT generator, fp16 main term + fp8 cross terms.
 //
-// FFMA2 path (this file; K > 241, bins per pixel other than 5 / 10, or on request):
+// FFMA2 path (this file; on request or when the window is wider than 11 pixels; FFMA2 charge lattice also for bins per pixel other than 5 / 10):
 //   charge_lattice_kernel (one CTA per tile)
 //     splat the tile's segments into C[nb*nb][Jc] in shared memory (register-tiled outer products of
 //     per-sample erf-difference weights, no atomics, fixed order), then pack the non-empty bins: per bin the
@@ -767,10 +767,15 @@ int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t
 }
 
 #ifdef LARTPC_DEBUG_CLOCKS
-extern "C" int lartpc_debug_clocks(unsigned long long out[8], int reset)
+extern "C" int lartpc_debug_clocks(unsigned long long out[24], int reset)
 {
     cudaMemcpyFromSymbol(out, g_dbg, sizeof(unsigned long long) * 8);
-    if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(g_dbg, z, sizeof(z)); }
+    cudaMemcpyFromSymbol(out + 8, rtc::g_rtc_dbg, sizeof(unsigned long long) * 16);
+    if (reset) {
+        unsigned long long z[16] = {0};
+        cudaMemcpyToSymbol(g_dbg, z, sizeof(unsigned long long) * 8);
+        cudaMemcpyToSymbol(rtc::g_rtc_dbg, z, sizeof(z));
+    }
     return 0;
 }
 #endif
@@ -789,7 +794,8 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
 {
     const DevParams &p = sim->dp;
     if (sim->n_tiles == 0) return LARTPC_OK;
-    if (p.Jc != rtc::JC || !sim->d_lut_tc) return LARTPC_ERR_UNSUPPORTED;
+    if (p.Jc != rtc::JC || !sim->d_lut_tc || 32 + p.NBW > rtc::ACC_COL) return LARTPC_ERR_UNSUPPORTED;
+    constexpr bool PAIR = TC_CTA_PAIR;
     rtc::Args a;
     a.A = (const __half *)out->charge;
     a.B = (const __half *)sim->d_lut_tc;
@@ -798,30 +804,53 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     a.tb_mask = sim->tb_mask;
     if (sim->n_tiles >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.n_tiles = (int)sim->n_tiles;
-    a.n_tb = (int)((sim->n_tiles + rtc::TB - 1) / rtc::TB);
+    a.n_units = (int)((sim->n_tiles + TC_UNIT_TILES - 1) / TC_UNIT_TILES);
     a.NC = p.NB2;  a.WW = p.WW * p.nq;  a.NBW = p.NBW;  a.tile_ticks = p.tile_ticks;   // a row = (target, LUT piece)
     a.b_scale_log2 = p.b_scale_log2;
-    a.n_items = (long long)((a.n_tb + 1) / 2) * a.WW * 2;                 // (unit of two tile blocks, row, half): response_tc.cuh
+    a.n_items = (long long)a.n_units * a.WW;
     if (a.n_items >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.work = sim->d_work;
     LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
-    const int smem = rtc::smem_bytes(p.NBW);
+    a.n_stages = rtc::n_stages(p.NBW, PAIR, (size_t)227 * 1024);
+    if (a.n_stages < 2) return LARTPC_ERR_UNSUPPORTED;
+    const size_t smem = rtc::smem_bytes(p.NBW, PAIR, a.n_stages);
     static SmemCfg cfg_rtc;
-    LARTPC_CUDA_TRY(ensure_dyn_smem(rtc::response_tc_kernel, cfg_rtc, sim->device, (size_t)smem));
-    const int grid = (int)std::min<long long>(a.n_items, sim->sm_count);
+    LARTPC_CUDA_TRY(ensure_dyn_smem(rtc::response_tc_kernel<PAIR>, cfg_rtc, sim->device, smem));
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    const int per = PAIR ? 2 : 1;
+    int clusters = sim->sm_count / per;
+    cfg.blockDim = dim3(rtc::THREADS, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = per;  attr[0].val.clusterDim.y = 1;  attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;  cfg.numAttrs = 1;
+    if (PAIR) {
+        // CTA pairs that can be resident at once (one CTA per SM, both SMs of a pair in one TPC)
+        cfg.gridDim = dim3((unsigned)(clusters * per), 1, 1);
+        int max_clusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&max_clusters, rtc::response_tc_kernel<PAIR>, &cfg) == cudaSuccess && max_clusters > 0)
+            clusters = std::min(clusters, max_clusters);
+        else cudaGetLastError();
+    }
+    clusters = (int)std::min<long long>(clusters, a.n_items);
+    cfg.gridDim = dim3((unsigned)(clusters * per), 1, 1);
     ++g_lartpc_launches;
-    rtc::response_tc_kernel<<<grid, rtc::THREADS, smem, st>>>(a);
+    LARTPC_CUDA_TRY(cudaLaunchKernelEx(&cfg, rtc::response_tc_kernel<PAIR>, a));
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }
 
-// Bs[d, q][c][fp16 | fp8][NBW x 32 bytes] with Bs[n'][jj] = R[c][d][KQ q + n' - jj] * 2^b_scale_log2 (0 outside piece q of the LUT): the fp16 image
+// Bs[d, q][c][CTA of the pair][fp16 | fp8][rows x 32 bytes] with Bs[n'][jj] = R[c][d][KQ q + n' - jj] * 2^b_scale_log2 (0 outside piece q of the LUT): the fp16 image
 // (rtc::b_image_offset) and the fp8 image of the cross terms (rtc::b8_image_offset), both in the canonical un-swizzled
 // K-major layout.  Built once per sim on the host.
 size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_out)
 {
     const int nb = p.nb, W = p.W, NBW = p.NBW, NB = W * nb;
+    const int split = TC_CTA_PAIR ? 2 : 1, rows = NBW / split;          // rows of a generator one CTA of the pair holds
     const size_t half_elems = (size_t)NBW * 16, n = (size_t)p.WW * p.nq * p.NB2 * 2 * half_elems;
+    const size_t cta_halfs = (size_t)rows * 16;                         // halfs of one precision part of one CTA's rows
     std::vector<__half> img(n);
     for (int dq = 0; dq < p.WW * p.nq; ++dq) {                         // row = (target d, LUT piece q): ticks [KQ q, KQ q + K)
         const int d = dq / p.nq, q = dq - d * p.nq, K = std::min(p.KQ, p.K - p.KQ * q);
@@ -829,19 +858,24 @@ size_t lartpc_build_lut_tc(const DevParams &p, const float *lut_host, void **d_o
         for (int cb = 0; cb < nb; ++cb)
             for (int ca = 0; ca < nb; ++ca) {
                 const float *src = lut_host + ((size_t)(nb * dyi + cb) * NB + (nb * dxi + ca)) * p.K + (size_t)p.KQ * q;
-                __half *hi = img.data() + ((size_t)dq * p.NB2 + (cb * nb + ca)) * 2 * half_elems;
-                unsigned char *f8 = (unsigned char *)(hi + half_elems);                  // NBW x 32 bytes
-                for (int nn = 0; nn < NBW; ++nn)
+                __half *bin_img = img.data() + ((size_t)dq * p.NB2 + (cb * nb + ca)) * 2 * half_elems;
+                for (int nn = 0; nn < NBW; ++nn) {
+                    // (target, bin) image: [CTA of the pair][fp16 part | fp8 part], each part the canonical K-major
+                    // image of that CTA's rows
+                    const int rk = nn / rows, nl = nn - rk * rows;
+                    __half *hi = bin_img + (size_t)rk * 2 * cta_halfs;
+                    unsigned char *f8 = (unsigned char *)(hi + cta_halfs);
                     for (int jj = 0; jj < 16; ++jj) {
                         const int k = nn - jj;
                         const float x = (k >= 0 && k < K) ? ldexpf(src[k], p.b_scale_log2) : 0.f;
                         const __half h = __float2half_rn(x);
-                        hi[rtc::b_image_offset(nn, jj)] = h;
-                        f8[rtc::b8_image_offset(nn, jj)] =
+                        hi[rtc::b_image_offset(nl, jj)] = h;
+                        f8[rtc::b8_image_offset(nl, jj)] =
                             __nv_cvt_float_to_fp8(ldexpf(x, -rtc::SA_LOG2), __NV_SATFINITE, __NV_E4M3);
-                        f8[rtc::b8_image_offset(nn, 16 + jj)] =
+                        f8[rtc::b8_image_offset(nl, 16 + jj)] =
                             __nv_cvt_float_to_fp8(ldexpf(x - __half2float(h), rtc::SB_LOG2), __NV_SATFINITE, __NV_E4M3);
                     }
+                }
             }
     }
     if (cudaMalloc(d_out, n * sizeof(__half)) != cudaSuccess) return 0;

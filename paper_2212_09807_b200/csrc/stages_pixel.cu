@@ -32,7 +32,7 @@ constexpr int SUM_LCAP = 192;      // partial rows listed per round (a pixel usu
 // list order (d ascending, window ascending): the loads of one tick are independent of each other, the row reads of a
 // warp are coalesced, and the order of the float32 additions -- hence every output bit -- is fixed.
 template <int VEC, bool PIECES>    // VEC: ticks per thread and load, 4 when tile_ticks is a multiple of 4 (rows 16-byte aligned), else 2
-                                   // PIECES: a long LUT cut into pieces (tensor-core path, K > 241): nq rows per (tile, target)
+                                   // PIECES: a long LUT cut into pieces (tensor-core path, K > 209): nq rows per (tile, target)
 __global__ void __launch_bounds__(SUM_THREADS)
 sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__restrict__ pixel_id,
                  const int32_t *__restrict__ first_tick, const int32_t *__restrict__ length,

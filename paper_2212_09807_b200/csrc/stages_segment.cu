@@ -512,7 +512,7 @@ tile_scatter_kernel(int64_t n_tiles, int32_t *perm /* in: class, out: slot */, i
     perm[t] = slot;
     td_p[slot] = td[t];
     tl_p[slot] = tl[t];
-    if (mask) atomicOr(&tb_mask[slot / TC_TILE_BLOCK], mask);
+    if (mask) atomicOr(&tb_mask[slot / TC_UNIT_TILES], mask);
 }
 
 static int grow_i32(int32_t **p, int64_t *cap, int64_t need)
@@ -644,7 +644,7 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         info->tile_targets = p.WW * p.nq;                               // rows of `partial` per tile
         info->tile_ticks = p.tile_ticks;
         info->tile_charge_floats = p.slab_floats;
-        info->reserved = 0;
+        info->tile_block = p.tc_mode ? TC_UNIT_TILES : 1;
     }
     return LARTPC_OK;
 }

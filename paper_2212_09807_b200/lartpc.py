@@ -79,7 +79,7 @@ class PixmapInfo(C.Structure):
                 ("n_active_segments", C.c_int64), ("n_tiles", C.c_int64), ("n_pairs", C.c_int64),
                 ("n_active_pixels", C.c_int64), ("total_samples", C.c_int64),
                 ("tile_targets", C.c_int32), ("tile_ticks", C.c_int32),
-                ("tile_charge_floats", C.c_int32), ("reserved", C.c_int32)]
+                ("tile_charge_floats", C.c_int32), ("tile_block", C.c_int32)]
 
 
 class Signals(C.Structure):
@@ -285,7 +285,8 @@ class Sim:
         t = self.torch
         info = self.info
         nt = int(info.n_tiles)
-        nt_cap = (nt + 127) // 128 * 128                 # the tensor-core operand image comes in 128-tile blocks
+        blk = max(int(info.tile_block), 1)               # the tensor-core operand image comes in whole units of tiles
+        nt_cap = (nt + blk - 1) // blk * blk
         out = dict(partial=self._empty(nt * info.tile_targets * info.tile_ticks, t.float32),
                    tile_range=self._empty(nt * 4, t.int32),
                    charge=self._empty(nt_cap * info.tile_charge_floats, t.float32))

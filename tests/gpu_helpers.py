@@ -39,12 +39,14 @@ def compare_hits(gpu, orc):
     """Hit lists compared pixel by pixel, hit by hit, in tick order (BASELINE north_star: >= 99.9 % identical in pixel,
     tick and ADC; the rest off by at most one tick or one count, at threshold crossings).
 
-    A pixel's hits are a chain: when the integrated charge sits within the rounding error of the threshold at a crossing,
-    the two sides may fire one tick apart, the reset then happens one tick apart, the reset noise is drawn for another
-    (pixel, tick) key and the charge of one tick moves between neighbouring samples -- every LATER hit of that pixel is a
-    consequence of that one near miss, not an independent disagreement.  So: the first differing hit of a pixel must be
-    within one tick and one count of its partner; the hits behind it count as not identical but are not held to the
-    nearness rule.  A pixel whose hit COUNT differs without such a near miss fails.
+    A pixel's hits are a chain.  A sample that lands on an ADC code boundary may differ by one count with the tick
+    unchanged: the reset is the same, the chain goes on and every later hit is still compared strictly.  When the
+    integrated charge sits within the rounding error of the threshold at a crossing, the two sides may fire one tick
+    apart; the reset then happens one tick apart, the reset noise is drawn for another (pixel, tick) key and the charge
+    of one tick moves between neighbouring samples -- every LATER hit of that pixel is a consequence of that one near
+    miss, not an independent disagreement: those are counted as not identical unless they do agree, but not held to the
+    nearness rule.  A missing / extra hit without such a near miss before it, or a first difference beyond one tick /
+    one count, fails.
     Returns (identical fraction of the oracle's hits, all differences explained, n_gpu, n_oracle, n_near_misses)."""
     def by_pixel(pix, tick, adc):
         d = {}
@@ -61,13 +63,20 @@ def compare_hits(gpu, orc):
         n_o += len(ol)
         n_g += len(gl)
         k = 0
-        while k < min(len(gl), len(ol)) and gl[k] == ol[k]:
+        while k < min(len(gl), len(ol)):
+            if gl[k] == ol[k]:
+                exact += 1
+            elif gl[k][0] == ol[k][0] and abs(gl[k][1] - ol[k][1]) <= 1:
+                n_near += 1                     # one count at a code boundary: same tick, same reset, the chain goes on
+            else:
+                break
             k += 1
-        exact += k
         if k == len(gl) == len(ol):
             continue
         if k < min(len(gl), len(ol)) and abs(gl[k][0] - ol[k][0]) <= 1 and abs(gl[k][1] - ol[k][1]) <= 1:
-            n_near += 1                         # a near miss at a crossing; what follows on this pixel is its consequence
+            n_near += 1                         # one tick apart at a crossing; what follows on this pixel is its consequence
+            rest = set(gl[k + 1:])
+            exact += sum(1 for h in ol[k + 1:] if h in rest)
         else:
             ok = False                          # a missing / extra hit, or a first difference beyond one tick / one count
     return exact / max(n_o, 1), ok, n_g, n_o, n_near

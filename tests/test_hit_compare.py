@@ -21,6 +21,13 @@ def test_near_miss_takes_the_later_hits_of_the_pixel_with_it():
     assert ok and near == 1 and (ng, no) == (4, 4) and frac == 2 / 4
 
 
+def test_one_count_at_a_code_boundary_does_not_excuse_what_follows():
+    orc = [(5, 100, 80), (5, 140, 81), (5, 190, 90)]
+    frac, ok, ng, no, near = compare_hits(_h([(5, 100, 80), (5, 140, 82), (5, 190, 90)]), _h(orc))
+    assert ok and near == 1 and frac == 2 / 3
+    assert not compare_hits(_h([(5, 100, 80), (5, 140, 82), (5, 193, 90)]), _h(orc))[1]    # later hit adrift: not excused
+
+
 def test_first_difference_beyond_one_tick_or_count_fails():
     orc = [(5, 100, 80), (5, 140, 81)]
     assert not compare_hits(_h([(5, 100, 80), (5, 142, 81)]), _h(orc))[1]
