@@ -10,10 +10,14 @@ synthetic spill.  Metric (BASELINE.json): segments/s (whole job) with ms/spill a
 * `value`     segments/s with the segment arrays already resident in HBM (device-timed, CUDA events).
 * `e2e`       same metric through the C-ABI with HOST (pinned) segment arrays: host->device copy of the nine
               float32 arrays and device->host read of the hit list inside the timed region.
-* `roofline`  the dominant kernel (S4 induced current): multiply-adds the method needs for the charge it found
-              (counted on the device) x 2 / its CUDA-event time, against the FP32 FMA peak measured on this GPU by the
-              library's FFMA-chain microbenchmark (MEASURED_PEAKS.json holds no FP32 figure).
-* `cpu_baseline`  the fp64 oracle (oracle/, as it stands) on this host's cores, on a bounded sample.
+* `roofline`  the dominant kernel (the S4 response on the tcgen05 tensor cores): multiply-adds the method needs for the
+              charge it found (counted on the device) x 2 / its CUDA-event time, against the measured bf16 / fp16 tensor
+              peak of MEASURED_PEAKS.json (sustained figure for launches longer than 50 ms); `executed_*` = the dense MMA
+              work actually issued (device-counted tcgen05.mma instructions); `traffic` = its DRAM bytes per launch.
+* `rooflines` one entry per kernel of the path: S1, S2, S3, S5, S6 against the measured HBM copy bandwidth (algorithmic bytes
+              of SURVEY.md 8(d) and the bytes the kernel moves), the charge lattice against the SM's thread-instruction
+              rate, the response against the tensor peak (DESIGN.md section 5 has every per-unit figure).
+* `cpu_baseline`  the fp64 oracle (oracle/, as it stands) on this host's cores, on a bounded sample: all cores, and one core.
 * `--impl reference`  times that oracle alone (there is no reference code for this paper).
 N > 1 (torchrun): every rank simulates its own independent spill (seed + rank), no data-path collective;
 `value` sums the ranks' segments over the max-over-ranks time ("scaling": "weak").
@@ -126,11 +130,11 @@ def oracle_sample(wl, n_sample: int):
         lo, lo + m, n)
 
 
-def time_oracle(wl, n_sample: int):
+def time_oracle(wl, n_sample: int, cores=None):
     import oracle
     oracle.build()
     sub, what = oracle_sample(wl, n_sample)
-    cores = os.cpu_count() or 1
+    cores = (os.cpu_count() or 1) if cores is None else cores
     t0 = time.perf_counter()
     res = oracle.run_chain(sub, threads=cores)
     dt = time.perf_counter() - t0
@@ -220,9 +224,9 @@ def run_ours(args):
     peak_scalar, peak_packed = lartpc.measure_fp32_peak(0), lartpc.measure_fp32_peak(1)
     sim.set_profiling(True)
     launches0 = lartpc.kernel_launches()
-    stage_ms = {k: 0.0 for k in sim.STAGES}
+    stage_ms = {k: [] for k in sim.STAGES}
     stage_n = {k: 0 for k in sim.STAGES}
-    fma = 0.0
+    cnt = {k: 0.0 for k in sim.COUNTERS}
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     clocks = ClockSampler(local)
     barrier()
@@ -232,17 +236,20 @@ def run_ours(args):
         ev[i][0].record()
         hits, st = sim.run_spill(seg, wl.seed, hit_cap, workspace=ws, hits=hits)
         ev[i][1].record()
-        ms, ln, f = sim.stage_ms()
+        ms, ln, _ = sim.stage_ms()
         for k in sim.STAGES:
-            stage_ms[k] += ms[k]
+            stage_ms[k].append(ms[k])
             stage_n[k] += ln[k]
-        fma += f
+        for k, v in sim.counters().items():
+            cnt[k] += v / args.steps
     barrier()
     clk = clocks.stop()
     launches = lartpc.kernel_launches() - launches0
     sim.set_profiling(False)
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
     total_ms_max, n_all = reduce_over_ranks(total_ms, n, world, dev)
+    median_ms, _ = reduce_over_ranks(float(np.median(step_ms)), n, world, dev)
 
     # ---- end to end through the C-ABI with host buffers ------------------------------------------
     e2e_ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
@@ -269,17 +276,63 @@ def run_ours(args):
     e2e_ms, _ = reduce_over_ranks(e2e_ev[0].elapsed_time(e2e_ev[1]) - flush_ms, n, world, dev)
 
     if rank == 0:
+        mp = {}
+        try:
+            mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        hbm_peak = float(mp.get("hbm_gbs", 6650.0))
+        hbm_src = "MEASURED_PEAKS.json hbm_gbs (measured copy)" if mp.get("hbm_gbs") else "fallback of B200_PROFILING.md"
+        per_step = {k: float(np.median(v)) for k, v in stage_ms.items()}          # ms per step, median over the steps
+        n_launch = {k: stage_n[k] / args.steps for k in sim.STAGES}
+        P = wl.params
+        K, nb2, ww = int(P["lut_ticks"]), int(P["bins_per_pixel"]) ** 2, int(P["window_pixels"]) ** 2
+        n_tiles, n_pairs, n_act, n_samp, n_hits = (int(st.n_tiles), int(st.n_pairs), int(st.n_active_pixels),
+                                                   int(st.total_samples), int(st.n_hits))
+        sm_hz = 1e6 * float(clk["sm_mhz"] or 1965.0)
+
+        def hbm_entry(stage, kernel, alg_bytes, moved_bytes, note):
+            t = per_step[stage] * 1e-3
+            return {"kernel": kernel, "stage": stage, "bound": "hbm", "unit": "GB/s", "peak": hbm_peak, "peak_source": hbm_src,
+                    "achieved": alg_bytes / t / 1e9 if t > 0 else None, "frac": alg_bytes / t / 1e9 / hbm_peak if t > 0 else None,
+                    "moved_gbs": moved_bytes / t / 1e9 if t > 0 else None,
+                    "moved_frac": moved_bytes / t / 1e9 / hbm_peak if t > 0 else None,
+                    "algorithmic_bytes_per_step": alg_bytes, "moved_bytes_per_step": moved_bytes,
+                    "ms_per_step": per_step[stage], "launches_per_step": n_launch[stage], "note": note}
+
+        rooflines = [
+            hbm_entry("quench", "quench_kernel (S1)", 44.0 * n, 36.0 * n,
+                      "algorithmic 36 B in + 8 B out per segment (SURVEY 8(d)); the kernel reads 7 of the 9 arrays"),
+            hbm_entry("drift", "drift_kernel (S2)", 80.0 * n, 100.0 * n,
+                      "algorithmic ~80 B per segment (SURVEY 8(d)); moved 32 B in + 4 B n_e + 64 B out (float64 end points)"),
+            hbm_entry("pixels_from_segments", "pixmap_kernel + tile plan (S3)", 64.0 * n,
+                      (44.0 + 56.0 + 96.0 + 40.0) * n + 16.0 * n_pairs + 120.0 * n_tiles,
+                      "algorithmic 64 B per segment (SURVEY 8(d)); moved (estimate from the kernels' accesses): boxes, 96 B record "
+                      "per segment, 4 B per (segment, charged pixel) pair written + sorted, tile descriptors / lists / slots"),
+        ]
+        # S4 charge lattice: thread-instruction rate of the SMs (the kernel is bound by issue slots: erf, products, splits)
+        t_ch = per_step["induced_current_charge"] * 1e-3
+        OPS_PER_COLUMN = 87 * 13 + 164 + 150      # 87 erf x 13 instructions, 164 products, 150 split / convert / store
+        alu_peak = sim_sm_count(torch, local) * 128 * sm_hz / 1e12                 # T thread-instructions / s (all four schedulers issuing)
+        ch_ops = cnt["charge_columns"] * OPS_PER_COLUMN
+        rooflines.append({"kernel": "charge_lattice_tc_kernel (S4a: charge per LUT cell, tcgen05 + erf weights)",
+                          "stage": "induced_current_charge", "bound": "alu", "unit": "T thread-instructions/s",
+                          "achieved": ch_ops / t_ch / 1e12 if t_ch > 0 else None, "peak": alu_peak,
+                          "frac": ch_ops / t_ch / 1e12 / alu_peak if t_ch > 0 else None,
+                          "peak_source": "SMs x 128 lanes x SM clock sampled during the run (one instruction per lane per cycle)",
+                          "operand_columns_per_step": cnt["charge_columns"], "instructions_per_column": OPS_PER_COLUMN,
+                          "tensor_tflops": cnt["charge_mma"] * 2.0 * 128 * 64 * 16 / t_ch / 1e12 if t_ch > 0 else None,
+                          "ms_per_step": per_step["induced_current_charge"],
+                          "launches_per_step": n_launch["induced_current_charge"],
+                          "note": "operand columns (rule nodes / sample points x tiles) counted on the device x instructions one "
+                                  "column costs (its weights: 87 erf, 164 products, fp16 splits and stores)"})
         n_resp = max(stage_n["induced_current_response"], 1)
-        s4_ms = stage_ms["induced_current_response"] / n_resp
-        fma_per_launch = fma / n_resp
+        s4_ms = sum(stage_ms["induced_current_response"]) / n_resp
+        t_rs = per_step["induced_current_response"] * 1e-3
+        fma_per_launch = cnt["fma_needed"] * args.steps / n_resp
         useful = 2.0 * fma_per_launch / (s4_ms * 1e-3) / 1e12 if s4_ms > 0 else 0.0
         if sim.response_mode == "tensor":
             # dense fp16 contraction on tcgen05: peak = measured bf16 GEMM peak (fp16 runs at the same rate)
-            mp = {}
-            try:
-                mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-            except Exception:
-                pass
             long_launch = s4_ms > 50.0
             if mp.get("bf16_tflops"):
                 peak = float(mp["bf16_tflops_sustained"] if long_launch and mp.get("bf16_tflops_sustained")
@@ -288,61 +341,88 @@ def run_ours(args):
                     "sustained" if long_launch else "burst")
             else:
                 peak, peak_src = 1590.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
-            K, nb2, ww = int(wl.params["lut_ticks"]), int(wl.params["bins_per_pixel"]) ** 2, int(wl.params["window_pixels"]) ** 2
-            kq = K if (K + 15 + 15) // 16 * 16 <= 256 else 200               # LUT pieces of the tensor path
-            nbw, ww = (kq + 15 + 15) // 16 * 16, ww * ((K + kq - 1) // kq)
-            tiles_per_launch = int(st.n_tiles) * args.steps / n_resp
-            # 4 blocks x (one fp16 MMA of K = 16 + one fp8 MMA of K = 32, which occupies the pipe like an fp16 K = 16):
-            # 8 fp16-equivalent MMA slots per (tile block, target, bin)
-            executed = 2.0 * (tiles_per_launch / 128.0) * ww * nb2 * 8 * 128.0 * nbw * 16
-            roof = {"kernel": "rtc::response_tc_kernel (S4 induced current, response on tcgen05)", "bound": "tensor",
+            kq = K if (K + 15 + 15) // 16 * 16 <= 224 else 200               # LUT pieces of the tensor path
+            nbw, rows = (kq + 15 + 15) // 16 * 16, ww * ((K + kq - 1) // kq)
+            # every tcgen05.mma of the response (fp16, K = 16, or fp8, K = 32) occupies the pipe like 128 x NBW x 16 fp16
+            # multiply-adds: fp16-equivalent flops of the instructions the kernel counted as it issued them
+            executed = cnt["response_mma"] * 2.0 * 128 * nbw * 16 * args.steps / n_resp
+            lut_bytes = rows * nb2 * nbw * 64.0
+            partial_bytes = 4.0 * n_tiles * rows * (((64 + kq - 1 + 7) // 8) * 8)
+            gen_bytes = cnt["response_items"] * nb2 * nbw * 64.0
+            a_once = max(cnt["response_bytes_to_smem"] - gen_bytes, 0.0) / rows      # every charge block is copied once per target row
+            dram = (a_once + partial_bytes + lut_bytes * n_launch["induced_current_response"]) / max(n_launch["induced_current_response"], 1)
+            roof = {"kernel": "rtc::response_tc_kernel (S4b: induced current, response on tcgen05)", "bound": "tensor",
                     "achieved": useful, "peak": peak, "unit": "TFLOP/s", "frac": useful / peak,
                     "achieved_note": "algorithmic: non-zero charge cells x in-plane targets x lut_ticks x 2 (counted on "
                                      "the device), what the method needs whatever the decomposition",
                     "executed_tflops": executed / (s4_ms * 1e-3) / 1e12 if s4_ms > 0 else 0.0,
                     "executed_frac": executed / (s4_ms * 1e-3) / 1e12 / peak if s4_ms > 0 else None,
-                    "executed_note": "dense MMA work issued in fp16-equivalent flops: tile blocks x targets x bins x 8 MMA slots (4 x (fp16 K=16 + fp8 K=32)) x 128 x NBW x 16 x 2",
-                    "fp32_alu_peak": max(peak_scalar, peak_packed), "peak_source": peak_src}
+                    "executed_note": "tcgen05.mma instructions counted by the kernel as it issues them x 128 x NBW x 16 x 2 "
+                                     "(an fp8 K = 32 instruction occupies the pipe like an fp16 K = 16 one)",
+                    "smem_fill_gbs": cnt["response_bytes_to_smem"] / t_rs / 1e9 if t_rs > 0 else None,
+                    "fp32_alu_peak": max(peak_scalar, peak_packed), "peak_source": peak_src,
+                    "traffic": dram,
+                    "traffic_note": "DRAM bytes per launch from the plan and the kernel's counters: charged A blocks read once "
+                                    "(the 25 target rows of a unit stream them at the same time through L2), partial rows "
+                                    "written, LUT image once; profiles/ holds the ncu dram__bytes capture it is checked against"}
         else:
             peak = max(peak_scalar, peak_packed)
             roof = {"kernel": "response_kernel (S4 induced current, response on the FP32 pipe)", "bound": "alu",
                     "achieved": useful, "peak": peak, "unit": "TFLOP/s", "frac": useful / peak if peak else None,
                     "peak_source": "lartpc_measure_fp32_peak on this GPU (scalar FFMA %.1f, packed FFMA2 %.1f)"
-                                   % (peak_scalar, peak_packed)}
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tpath):
-            try:
-                traffic = json.load(open(tpath)).get("induced_current_bytes_per_launch_" + sim.response_mode)
-            except Exception:
-                traffic = None
+                                   % (peak_scalar, peak_packed), "traffic": None}
+            partial_bytes = 4.0 * n_tiles * ww * 266
+        roof.update(launch_ms=s4_ms, flops_per_launch=2.0 * fma_per_launch, ms_per_step=per_step["induced_current_response"],
+                    launches_per_step=n_launch["induced_current_response"], stage="induced_current_response",
+                    share_of_step=per_step["induced_current_response"] / max(sum(per_step.values()), 1e-9))
+        rooflines.append(dict(roof))
+        rooflines.append(hbm_entry("sum_pixel_signals", "sum_pixel_kernel (S5)", 8.0 * n_samp, 0.87 * partial_bytes + 4.0 * n_samp,
+                                   "algorithmic 4 B in + 4 B out per stored waveform sample; moved (estimate): the charged part "
+                                   "(~87 %) of every tile's partial rows read once + the samples written"))
+        rooflines.append(hbm_entry("electronics", "electronics_warp_kernel + hit compaction (S6)", 4.0 * n_samp + 12.0 * n_hits,
+                                   4.0 * n_samp + 12.0 * n_hits + (4.0 * int(P["max_hits_per_pixel"]) + 24.0) * n_act,
+                                   "algorithmic 4 B in per sample + 12 B per hit (SURVEY 8(d)); moved adds the per-pixel hit slots"))
         line = {
-            "metric": METRIC, "value": n_all * args.steps / (total_ms_max * 1e-3), "unit": "segments/s",
-            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "metric": METRIC, "value": n_all / (median_ms * 1e-3), "unit": "segments/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": median_ms,
+            "ms_per_step_mean": total_ms_max / args.steps, "step_ms": step_ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": ("fp16 hi+lo operand splits with the cross terms in fp8 (e4m3), fp32 accumulate (S4 on tcgen05); fp32 "
+                      "elsewhere, fp64 where an integer is decided" if sim.response_mode == "tensor" else
+                      "f32 (S4 on the FP32 pipe), fp64 where an integer is decided"),
+            "data": "synthetic",
             "config": {"workload": WORKLOAD_NAMES[args.config], "n_segments": n, "n_pixels": wl.n_pixels,
                        "n_readout_ticks": int(wl.params["n_readout_ticks"]), "n_tpcs": len(wl.tpcs),
                        "seed": wl.seed, "l2": "256 MiB flush write between timed steps",
+                       "timing": "CUDA events per step on the launching stream; value from the median step",
                        "parallelism": "independent spill per GPU" if world > 1 else "single GPU",
                        "input_sha256": {k: v[:16] for k, v in wl.sha256().items()}},
-            "stats": {"n_tiles": int(st.n_tiles), "n_pairs": int(st.n_pairs), "n_active_pixels": int(st.n_active_pixels),
-                      "total_samples": int(st.total_samples), "n_hits": int(st.n_hits),
+            "stats": {"n_tiles": n_tiles, "n_pairs": n_pairs, "n_active_pixels": n_act,
+                      "total_samples": n_samp, "n_hits": n_hits,
                       "n_hits_dropped": int(st.n_hits_dropped), "n_batches": int(st.n_batches)},
-            "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
+            "counters_per_step": cnt,
+            "stage_ms_per_step": per_step,
             "e2e": {"value": n_all * args.steps / (e2e_ms * 1e-3), "unit": "segments/s",
                     "h2d_bytes_per_step": 9 * 4 * n, "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches),
             "clocks": clk,
-            "roofline": dict(roof, traffic=traffic, launch_ms=s4_ms, flops_per_launch=2.0 * fma_per_launch,
-                             share_of_step=stage_ms["induced_current_response"] / max(sum(stage_ms.values()), 1e-9)),
+            "roofline": roof,
+            "rooflines": rooflines,
             "response_mode": sim.response_mode,
         }
         if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"], _, _ = time_oracle(wl, args.cpu_sample)
+            base, _, _ = time_oracle(wl, args.cpu_sample)
+            one, _, _ = time_oracle(wl, max(40, args.cpu_sample // 10), cores=1)
+            base["one_core"] = one
+            line["cpu_baseline"] = base
         print(json.dumps(line))
     sim.close()
     if world > 1:
         dist.destroy_process_group()
+
+
+def sim_sm_count(torch, index):
+    return int(torch.cuda.get_device_properties(index).multi_processor_count)
 
 
 # --------------------------------------------------------------------------------------------------
@@ -433,7 +513,7 @@ def run_sweep(args):
     line = {"metric": "segments/s through S4 + S5 (induced current + per-pixel sum), configs[4] base point",
             "value": base["segments_per_s"], "unit": "segments/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": base["ms_s4_s5"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
+            "dtype": "fp16 hi+lo / fp8 (e4m3) cross terms, fp32 accumulate (S4 on tcgen05)", "data": "synthetic",
             "config": {"workload": "configs[4] induced-current sweep, one 226x677 plane, track-like placement",
                        "base": SWEEP_BASE, "l2": "256 MiB flush write between timed steps"},
             "fp32_alu_peak_tflops": fp32_peak, "hbm_peak_gbs": hbm_peak, "clocks": clk,

@@ -308,6 +308,18 @@ int  lartpc_set_profiling(lartpc_sim_t *sim, int on);
 int  lartpc_get_stage_ms(const lartpc_sim_t *sim, double ms[LARTPC_N_STAGES], int64_t launches[LARTPC_N_STAGES],
                          double *fma_current);
 
+/* Work counters of the last lartpc_run_spill, counted on the device by the S4 kernels (the numerators of bench.py's
+ * per-kernel roofline figures; tensor-core path):
+ *   [0] multiply-adds the method needs: non-zero charge cells x in-plane target pixels x lut_ticks (= fma_current above)
+ *   [1] tcgen05.mma instructions the response issued (each 128 tiles x NBW columns x 16 fp16 or 32 fp8 products deep)
+ *   [2] bytes the response copied from L2 / HBM into shared memory (charge blocks + LUT generators)
+ *   [3] operand columns (sample points / rule nodes x tiles) the charge lattice evaluated
+ *   [4] tcgen05.mma instructions the charge lattice issued (128 cells x 64 ticks x 16 columns deep)
+ *   [5] response work items (unit of tiles x target row) that held charge
+ *   [6], [7] reserved (0) */
+#define LARTPC_N_COUNTERS 8
+int  lartpc_get_counters(const lartpc_sim_t *sim, double out[LARTPC_N_COUNTERS]);
+
 /* Kernels the library has launched in this process so far (all sims; not thread-safe, a plain counter). */
 int64_t lartpc_kernel_launches(void);
 

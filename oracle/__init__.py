@@ -89,6 +89,11 @@ def _load():
     return _lib
 
 
+def set_threads(n: int) -> int:
+    """Threads the per-pixel loops use from now on (OpenMP); returns the count in effect."""
+    return int(_load().orc_set_threads(C.c_int(int(n))))
+
+
 def _f32(a):
     return np.ascontiguousarray(a, dtype=np.float32)
 
@@ -165,7 +170,7 @@ def pixel_currents(params, tpcs, lut, dr, pm, tpc_index: int, ixs, iys, threads:
     """O4+O5, eqs. (3.7)-(3.9): waveforms [len(ixs)][n_readout_ticks] (electrons per tick) and Q_p."""
     lib = _load()
     if threads is not None:
-        os.environ["OMP_NUM_THREADS"] = str(int(threads))
+        lib.orc_set_threads(C.c_int(int(threads)))
     ixs = np.ascontiguousarray(ixs, dtype=np.int32)
     iys = np.ascontiguousarray(iys, dtype=np.int32)
     npx, nt = ixs.shape[0], int(params["n_readout_ticks"])
@@ -184,7 +189,7 @@ def pixel_currents_random(params, tpcs, lut, dr, pm, tpc_index: int, ixs, iys, m
     (seed; segment index, mu, nu)).  Returns waveforms [len(ixs)][n_readout_ticks] and Q_p."""
     lib = _load()
     if threads is not None:
-        os.environ["OMP_NUM_THREADS"] = str(int(threads))
+        lib.orc_set_threads(C.c_int(int(threads)))
     ixs = np.ascontiguousarray(ixs, dtype=np.int32)
     iys = np.ascontiguousarray(iys, dtype=np.int32)
     npx, nt = ixs.shape[0], int(params["n_readout_ticks"])

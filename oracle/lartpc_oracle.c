@@ -40,6 +40,21 @@
 #include <stdlib.h>
 #include <string.h>
 
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+/* threads of the pixel loops (orc_plane_currents*); no arithmetic here.  Returns the count in effect. */
+int orc_set_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+    return omp_get_max_threads();
+#else
+    (void)n;
+    return 1;
+#endif
+}
+
 typedef struct {
     double e_field, rho, w_ion;              /* kV/cm, g/cm^3, MeV per electron */
     int    recomb_model;                     /* 0 Birks eq. (3.1), 1 modified Box eq. (3.2) */

@@ -283,8 +283,8 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     SIM_TRY(cudaMalloc(&s->act_slot, sizeof(int32_t) * pix));
     SIM_TRY(cudaMalloc(&s->d_counters, sizeof(long long) * CNT_COUNT));
     SIM_TRY(cudaMallocHost(&s->h_counters, sizeof(long long) * CNT_COUNT));
-    SIM_TRY(cudaMalloc(&s->d_fma, sizeof(unsigned long long)));
-    SIM_TRY(cudaMemset(s->d_fma, 0, sizeof(unsigned long long)));
+    SIM_TRY(cudaMalloc(&s->d_fma, sizeof(unsigned long long) * LARTPC_N_COUNTERS));
+    SIM_TRY(cudaMemset(s->d_fma, 0, sizeof(unsigned long long) * LARTPC_N_COUNTERS));
     s->pair_cap = 1 << 16;
     SIM_TRY(cudaMalloc(&s->pair_seg, sizeof(int32_t) * s->pair_cap));
     if (sim_grow_tiles(s, 1 << 14) != 0) { sim_free(s); return LARTPC_ERR_CUDA; }
@@ -490,6 +490,13 @@ extern "C" int lartpc_get_stage_ms(const lartpc_sim_t *sim, double ms[LARTPC_N_S
     return LARTPC_OK;
 }
 
+extern "C" int lartpc_get_counters(const lartpc_sim_t *sim, double out[LARTPC_N_COUNTERS])
+{
+    if (!sim || !out) return LARTPC_ERR_BAD_ARGUMENT;
+    for (int k = 0; k < LARTPC_N_COUNTERS; ++k) out[k] = sim->counters[k];
+    return LARTPC_OK;
+}
+
 extern "C" size_t lartpc_workspace_bytes(const lartpc_sim_t *sim, int64_t max_segments)
 {
     if (!sim) return 0;
@@ -515,7 +522,7 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
     memset(&stt, 0, sizeof(stt));
     stt.n_segments = n;
     LARTPC_CUDA_TRY(cudaMemsetAsync(out->counters, 0, sizeof(int64_t) * 4, st));
-    LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_fma, 0, sizeof(unsigned long long), st));
+    LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_fma, 0, sizeof(unsigned long long) * LARTPC_N_COUNTERS, st));
     StageTimer tm{sim, st};
     sim->ev_stage.clear();
 
@@ -597,13 +604,14 @@ extern "C" int lartpc_run_spill(lartpc_sim_t *sim, const lartpc_segments_t *seg,
         tpc_lo = tpc_hi;
     }
     long long hc[4];
-    unsigned long long fma = 0;
+    unsigned long long cnt[LARTPC_N_COUNTERS] = {};
     LARTPC_CUDA_TRY(cudaMemcpyAsync(hc, out->counters, sizeof(hc), cudaMemcpyDeviceToHost, st));
-    LARTPC_CUDA_TRY(cudaMemcpyAsync(&fma, sim->d_fma, sizeof(fma), cudaMemcpyDeviceToHost, st));
+    LARTPC_CUDA_TRY(cudaMemcpyAsync(cnt, sim->d_fma, sizeof(cnt), cudaMemcpyDeviceToHost, st));
     LARTPC_CUDA_TRY(cudaStreamSynchronize(st));
     tm.collect();
-    sim->fma_current = (double)fma;
-    stt.flops_current = 2.0 * (double)fma;
+    for (int k = 0; k < LARTPC_N_COUNTERS; ++k) sim->counters[k] = (double)cnt[k];
+    sim->fma_current = (double)cnt[0];
+    stt.flops_current = 2.0 * (double)cnt[0];
     stt.n_hits = hc[0]; stt.n_hits_total = hc[1]; stt.n_pixels_overflow = hc[2]; stt.n_hits_dropped = hc[3];
     if (stats) *stats = stt;
     return LARTPC_OK;

@@ -283,6 +283,10 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                 }
             }
             const int total = pre[nseg];
+            if (tid == 0 && total) {
+                atomicAdd(a.fma_counter + 3, (unsigned long long)total);
+                atomicAdd(a.fma_counter + 4, 3ull * (unsigned long long)((total + 15) / 16));   // hi hi + hi lo + lo hi per 16 columns
+            }
             for (int s0 = 0; s0 < total; s0 += CT_KB) {
                 const int nsb = min(CT_KB, total - s0), nk16 = (nsb + 15) >> 4;
                 if (s_in < 16 * nk16) {

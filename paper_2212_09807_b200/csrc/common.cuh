@@ -125,7 +125,8 @@ struct lartpc_sim {
     double stage_ms[LARTPC_N_STAGES] = {};
     int64_t stage_launches[LARTPC_N_STAGES] = {};
     double fma_current = 0.0;
-    unsigned long long *d_fma = nullptr; // device counter of S4 multiply-adds
+    unsigned long long *d_fma = nullptr; // device counters of S4, LARTPC_N_COUNTERS of them ([0]: multiply-adds the method needs)
+    double counters[8] = {};             // host copy after the last lartpc_run_spill (lartpc_get_counters)
     int *d_work = nullptr;               // work-queue cursor of the persistent response kernel
     int *d_end_row = nullptr;            // 16-byte row header with the END flag (terminates the consumers)
     unsigned char blk_of_slot[256];      // response kernel: output block of consumer-thread slot (balances the SM sub-partitions)

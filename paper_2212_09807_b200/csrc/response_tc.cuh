@@ -57,6 +57,7 @@ struct Args {
     int n_tiles, n_units, NC, WW, NBW, tile_ticks, n_stages;
     int b_scale_log2;              // B = R * 2^b_scale_log2 (DevParams)
     long long n_items;             // n_units * WW: (unit, row of the LUT image)
+    unsigned long long *stats;     // device counters (lartpc_get_counters): [1] MMAs issued, [2] bytes copied, [5] items
     int *work;                     // item cursor, zero at launch: items are taken in order as CTAs become free, so the
                                    // CTAs that stream one tile block stay together however long the launch runs
 };
@@ -423,6 +424,11 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                     bulk_g2s(st + a_area, Bd + (size_t)c * b_stride, b_cta, fb);
                     RTC_T(p2);  RTC_ADD(8, p1 - p0);  RTC_ADD(9, p2 - p1);  RTC_ADD(10, 1);
                     if (++s == S) { s = 0; ph ^= 1u; }
+                }
+                if (leader) {                                          // per item: stages x (2 MMAs per charged block), bytes of the unit
+                    atomicAdd(a.stats + 1, (unsigned long long)(2 * NC * __popc(mask)));
+                    atomicAdd(a.stats + 2, (unsigned long long)NC * bytes * (CTA2 ? 2ull : 1ull));
+                    atomicAdd(a.stats + 5, 1ull);
                 }
                 q = q_next;
             }

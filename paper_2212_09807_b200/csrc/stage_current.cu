@@ -810,6 +810,7 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     a.n_items = (long long)a.n_units * a.WW;
     if (a.n_items >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.work = sim->d_work;
+    a.stats = sim->d_fma;
     LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
     a.n_stages = rtc::n_stages(p.NBW, PAIR, (size_t)227 * 1024);
     if (a.n_stages < 2) return LARTPC_ERR_UNSUPPORTED;

@@ -109,7 +109,8 @@ EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", 
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
            "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_run_spill",
            "lartpc_readout_tiles", "lartpc_pack_hits",
-           "lartpc_measure_fp32_peak", "lartpc_set_profiling", "lartpc_get_stage_ms", "lartpc_kernel_launches", "lartpc_strerror")
+           "lartpc_measure_fp32_peak", "lartpc_set_profiling", "lartpc_get_stage_ms", "lartpc_get_counters", "lartpc_kernel_launches",
+           "lartpc_strerror")
 
 
 def load_library():
@@ -348,6 +349,14 @@ class Sim:
         fma = C.c_double(0.0)
         _check(self.lib.lartpc_get_stage_ms(self.handle, ms, ln, C.byref(fma)), "lartpc_get_stage_ms")
         return dict(zip(self.STAGES, ms)), dict(zip(self.STAGES, ln)), float(fma.value)
+
+    COUNTERS = ("fma_needed", "response_mma", "response_bytes_to_smem", "charge_columns", "charge_mma", "response_items")
+
+    def counters(self):
+        """Device-counted S4 work of the last run_spill (lartpc_get_counters)."""
+        out = (C.c_double * 8)()
+        _check(self.lib.lartpc_get_counters(self.handle, out), "lartpc_get_counters")
+        return dict(zip(self.COUNTERS, [float(x) for x in out]))
 
     def workspace_bytes(self, max_segments: int) -> int:
         return int(self.lib.lartpc_workspace_bytes(self.handle, C.c_int64(max_segments)))
