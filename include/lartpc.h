@@ -234,6 +234,16 @@ int  lartpc_set_disabled_pixels(lartpc_sim_t *sim, const int32_t *pixel_ids_host
  * Tensor-core path with 5 or 10 bins per pixel only: LARTPC_ERR_UNSUPPORTED otherwise. */
 int  lartpc_set_random_perturbations(lartpc_sim_t *sim, int m, uint64_t seed);
 
+/* Tensor-core response only.  tcgen05.mma adds every product into its fp32 accumulator with truncation toward zero
+ * (measured on B200: the integrated current of a pixel comes out low by 0.4 - 1.4e-5 of its gross value, growing with the
+ * number of charged LUT cells), a systematic loss that fp32 FMA accumulation (round to nearest) does not have and that
+ * moves hits across ADC code boundaries where a pixel's gross current is large.  The response's epilogue multiplies
+ * accumulator column n by 1 + kappa x (non-zero charge cells whose products that column summed), the expected loss;
+ * kappa = LARTPC_TRUNC_KAPPA_DEFAULT, measured against the fp64 oracle on configs[1..3] (residual bias <= 1.5e-6, rms
+ * <= 3.5e-6 of gross; reading D27), unless set here; 0 turns the compensation off.  0 <= kappa <= 1e-6. */
+#define LARTPC_TRUNC_KAPPA_DEFAULT 7.5e-9
+int  lartpc_set_truncation_compensation(lartpc_sim_t *sim, double kappa);
+
 /* Arrival ticks per charge tile (window length) chosen for this LUT shape. */
 int  lartpc_chunk_ticks(const lartpc_sim_t *sim);
 

@@ -262,6 +262,34 @@ def electronics(params, seed: int, pixel_ids, waves, max_hits: Optional[int] = N
             np.asarray(counts, dtype=np.int32))
 
 
+def segment_currents(params, tpcs, lut, dr, pm, tpc_index: int, ix: int, iy: int, sel, threads: Optional[int] = None):
+    """O7: I_{p,s}, eq. (3.9) for each listed segment alone, on pixel (ix, iy): [len(sel)][n_readout_ticks]."""
+    lib = _load()
+    if threads is not None:
+        lib.orc_set_threads(C.c_int(int(threads)))
+    sel = np.ascontiguousarray(sel, dtype=np.int64)
+    nt = int(params["n_readout_ticks"])
+    waves = np.zeros((len(sel), nt))
+    lutc = _f32(lut)
+    pp, tt = _params(params), _tpcs(tpcs)
+    lib.orc_segment_currents(C.byref(pp), tt, C.c_int(tpc_index), _fp(lutc), *_seg_args(dr, pm),
+                             C.c_int(int(ix)), C.c_int(int(iy)), C.c_int64(len(sel)), _p(sel, C.c_int64), _dp(waves))
+    return waves
+
+
+def hit_truth(params, hit_ticks, seg_waves):
+    """O7 (reading D26): for the hits of ONE pixel (sample ticks in increasing order) and the per-segment currents
+    ``seg_waves`` [n_sel][n_readout_ticks]: returns (n0 [n_hits] first integrated tick, share [n_hits][n_sel] electrons)."""
+    lib = _load()
+    pp = _params(params)
+    ticks = np.ascontiguousarray(hit_ticks, dtype=np.int32)
+    w = np.ascontiguousarray(seg_waves, dtype=np.float64)
+    n0 = np.zeros(len(ticks), dtype=np.int32)
+    share = np.zeros((len(ticks), w.shape[0]))
+    lib.orc_hit_truth(C.byref(pp), C.c_int(len(ticks)), _ip(ticks), C.c_int64(w.shape[0]), _dp(w), _ip(n0), _dp(share))
+    return n0, share
+
+
 def active_pixels(tpcs, pm, dr, tpc_index: int):
     """Union of the O3 rectangles of one TPC: sorted (iy, ix) pairs, row-major order."""
     t = tpcs[tpc_index]

@@ -33,6 +33,11 @@
  *                   discriminator noise on the threshold, fresh each tick (z_d)           test_electronics_discriminator_noise_branch
  *                   periodic reset (armed only, before the tick's charge)                 test_electronics_periodic_reset_branch
  *                   min-spacing re-arm (n >= sample + spacing - hold)                     test_electronics_min_spacing_branch
+ *   orc_segment_currents / orc_hit_truth  (O7, truth association)  three point charges placed by hand under a delta-like
+ *                   LUT: shares, fractions and window starts written out in the test (test_hit_truth_hand_case); the
+ *                   periodic-reset window start (test_hit_truth_periodic_reset_window); shares of all segments add up to the
+ *                   integral of orc_pixel_current's waveform over the window, and that integral reproduces the noise-free
+ *                   ADC code of orc_electronics (test_hit_truth_sums_to_the_sampled_charge)
  *   No function is "parity unpinned".
  */
 #include <math.h>
@@ -587,4 +592,56 @@ int orc_electronics(const orc_params *p, uint64_t seed, int32_t pixel_id, const 
         }
     }
     return nhits;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O7  Truth association: which segments fed a hit, and with what share of its charge.
+ *   The paper describes truth propagation for the light path only (section 4.4: "the true track segment
+ *   id ... contributing to each ADC sample"); this is the charge-side analogue, reading D26:
+ *   - By eqs. (3.7)-(3.9) the current on a pixel is a sum over segments, I_p[n] = sum_s I_{p,s}[n], where I_{p,s} is
+ *     eq. (3.9) evaluated for segment s alone (orc_pixel_current on a one-segment input).
+ *   - At the sample tick n_h of hit h the CSA of O6 holds q = (reset noise) + sum_{n = n0}^{n_h} I_p[n], n0 = the first
+ *     tick integrated since q was last set: the tick after the previous sample of that pixel (0 for its first hit),
+ *     or a later periodic-reset tick r = k * periodic_reset_ticks (k >= 1) with r <= n_h - hold_ticks, the crossing tick
+ *     (O6 clears q BEFORE it adds the charge of tick r, and only while armed, i.e. up to and including the crossing tick).
+ *   - Share of segment s in hit h:  q_{h,s} = sum_{n = n0}^{n_h} I_{p,s}[n]  (electrons; signed, a bipolar induced
+ *     current can make it negative); fraction f_{h,s} = q_{h,s} / sum_{s'} q_{h,s'}.  Noise belongs to no segment.
+ * ------------------------------------------------------------------------------------------- */
+
+/* I_{p,s} for the listed segments: waves[n_sel][n_ticks], one orc_pixel_current call per segment on that segment alone. */
+void orc_segment_currents(const orc_params *p, const orc_tpc *tpcs, int tpc_index, const float *lut,
+                          const int32_t *tpc, const double *q_a, const double *sigma_T, const double *sigma_t,
+                          const double *u_s, const double *v_s, const double *u_e, const double *v_e,
+                          const double *T_s, const double *T_e, const int32_t *n_samples,
+                          int ix, int iy, int64_t n_sel, const int64_t *sel, double *waves)
+{
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < n_sel; ++k) {
+        const int64_t s = sel[k];
+        orc_pixel_current(p, tpcs, tpc_index, lut, 1, tpc + s, q_a + s, sigma_T + s, sigma_t + s,
+                          u_s + s, v_s + s, u_e + s, v_e + s, T_s + s, T_e + s, n_samples + s,
+                          ix, iy, waves + (size_t)k * p->n_ticks);
+    }
+}
+
+/* hit_tick[n_hits]: the sample ticks of ONE pixel in increasing order (orc_electronics); seg_waves[n_sel][n_ticks].
+ * Out: n0[n_hits] first integrated tick of each hit, share[n_hits][n_sel] = q_{h,s}. */
+void orc_hit_truth(const orc_params *p, int n_hits, const int32_t *hit_tick,
+                   int64_t n_sel, const double *seg_waves, int32_t *n0, double *share)
+{
+    for (int h = 0; h < n_hits; ++h) {
+        int start = h > 0 ? hit_tick[h - 1] + 1 : 0;
+        if (p->periodic_reset_ticks > 0) {
+            int crossing = hit_tick[h] - p->hold_ticks;
+            int r = (crossing / p->periodic_reset_ticks) * p->periodic_reset_ticks;   /* last reset tick <= crossing */
+            if (r >= 1 && r > start) start = r;
+        }
+        n0[h] = start;
+        for (int64_t k = 0; k < n_sel; ++k) {
+            const double *w = seg_waves + (size_t)k * p->n_ticks;
+            double q = 0.0;
+            for (int n = start; n <= hit_tick[h]; ++n) q += w[n];
+            share[(size_t)h * n_sel + k] = q;
+        }
+    }
 }

@@ -194,6 +194,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
         if (mx > 0.f) { frexpf(mx, &e2); if (ldexpf(1.f, e2 - 1) == mx) --e2; }   // mx in (2^(e2-1), 2^e2]
         p.b_scale_log2 = 10 - std::min(std::max(e2, -30), 30);
         p.NBW = nbw;  p.KQ = kq;  p.nq = nq;
+        p.trunc_kappa = LARTPC_TRUNC_KAPPA_DEFAULT;
         p.n_groups = 1;  p.PG = n_pairs;  p.NP = n_pairs;                 // (unused by the tensor-core response)
         p.Jc = 64;  p.CJ = p.Jc + 4;
         p.tile_ticks = (p.Jc + kq - 1 + 7) & ~7;                          // 264 for K = 200: ticks of one row of `partial`
@@ -316,6 +317,13 @@ extern "C" int lartpc_set_random_perturbations(lartpc_sim_t *sim, int m, uint64_
     sim->dp.rnd_m = m;
     sim->dp.rnd_seed = seed;
     sim->have_signals = false;
+    return LARTPC_OK;
+}
+
+extern "C" int lartpc_set_truncation_compensation(lartpc_sim_t *sim, double kappa)
+{
+    if (!sim || !(kappa >= 0.0) || kappa > 1e-6) return LARTPC_ERR_BAD_ARGUMENT;
+    sim->dp.trunc_kappa = (float)kappa;
     return LARTPC_OK;
 }
 

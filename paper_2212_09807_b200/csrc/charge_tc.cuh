@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
     const uint32_t bar = sbase + 2 * CT_A_HALF + 2 * CT_B_HALF, tptr_addr = bar + 8;
     volatile uint32_t *tptr = (volatile uint32_t *)(ctl + 8);
     float *red = (float *)(ctl + 16);                                // [4] max, then ints
-    int *redi = (int *)(ctl + 32);                                   // [4][3] lo, hi, nz
+    int *redi = (int *)(ctl + 32);                                   // [4][4] lo, hi, non-zero cells of blocks 0 1 | 2 3
     int *pre = (int *)(ctl + 96);                                    // [SEGCAP + 1] running column counts
     volatile int *s_q = (volatile int *)(ctl + 240);                 // ring of 3: this tile, the next, the one after
     TileDesc *s_td = (TileDesc *)(ctl + 256);                        // [3] their descriptors
@@ -435,28 +435,40 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             rtc::tmem_ld32(tlane + 32, v[1]);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             float mx = 0.f;
-            int lo = INT_MAX, hi = -1, nz = 0;
+            int lo = INT_MAX, hi = -1;
+            int pk01 = 0, pk23 = 0;                                      // non-zero cells of this row per 16-tick block, 16 bits each
     #pragma unroll
             for (int j = 0; j < 64; ++j) {
                 const float x = __uint_as_float(v[j >> 5][j & 31]);
                 mx = fmaxf(mx, fabsf(x));
-                if (x != 0.f) { lo = min(lo, j); hi = j; ++nz; }
+                if (x != 0.f) {
+                    lo = min(lo, j); hi = j;
+                    if (j < 32) pk01 += 1 << (16 * (j >> 4)); else pk23 += 1 << (16 * ((j >> 4) - 2));
+                }
             }
             for (int d = 16; d; d >>= 1) {
                 mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, d));
                 lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, d));
                 hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, d));
-                nz += __shfl_xor_sync(0xffffffffu, nz, d);
+                pk01 += __shfl_xor_sync(0xffffffffu, pk01, d);           // <= 32 x 16 per field and warp, <= 1600 per tile
+                pk23 += __shfl_xor_sync(0xffffffffu, pk23, d);
             }
-            if (lane == 0) { red[warp] = mx; redi[3 * warp] = lo; redi[3 * warp + 1] = hi; redi[3 * warp + 2] = nz; }
+            if (lane == 0) { red[warp] = mx; redi[4 * warp] = lo; redi[4 * warp + 1] = hi; redi[4 * warp + 2] = pk01; redi[4 * warp + 3] = pk23; }
             __syncthreads();
     #pragma unroll
             for (int w = 0; w < CT_THREADS / 32; ++w) {
                 mx = w ? fmaxf(mx, red[w]) : red[0];
-                lo = w ? min(lo, redi[3 * w]) : redi[0];
-                hi = w ? max(hi, redi[3 * w + 1]) : redi[1];
-                nz = w ? nz + redi[3 * w + 2] : redi[2];
+                lo = w ? min(lo, redi[4 * w]) : redi[0];
+                hi = w ? max(hi, redi[4 * w + 1]) : redi[1];
+                pk01 = w ? pk01 + redi[4 * w + 2] : redi[2];
+                pk23 = w ? pk23 + redi[4 * w + 3] : redi[3];
             }
+            const int nzb0 = pk01 & 0xffff, nzb1 = pk01 >> 16, nzb2 = pk23 & 0xffff, nzb3 = pk23 >> 16;
+            const int nz = nzb0 + nzb1 + nzb2 + nzb3;
+            // what the response's epilogue needs to add back the expected truncation loss of the tensor-core accumulation
+            // (response_tc.cuh "Accuracy"): non-zero cells per 16-tick block, in units of 8 cells, one byte per block
+            const int nz_packed = min((nzb0 + 4) >> 3, 255) | min((nzb1 + 4) >> 3, 255) << 8 | min((nzb2 + 4) >> 3, 255) << 16 |
+                                  min((nzb3 + 4) >> 3, 255) << 24;
             int e = 0;
             if (mx >= 32768.f) e = min(((__float_as_int(mx) >> 23) & 0xff) - 127 - 14, 100);   // mx * 2^-e in [2^14, 2^15)
             if (!(mx < 3.0e38f)) e = 0;                                   // inf / nan charge: leave it visible
@@ -464,7 +476,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             if (tid == 0) {
                 if (nz == 0) *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(1, 0, 0, 0);
                 else {
-                    *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(lo / RESP_NO, (hi + p.K - 1) / RESP_NO, e, 0);
+                    *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(lo / RESP_NO, (hi + p.K - 1) / RESP_NO, e, nz_packed);
                     // multiply-adds the method needs here: non-zero cells x in-plane targets x K
                     const DevTpc &tp = a.tpcs[td.tpc];
                     const int vx = min(td.px + p.H, tp.nx - 1) - max(td.px - p.H, 0) + 1;

@@ -35,6 +35,8 @@ struct DevParams {
     int NBW;                         // tensor-core mode: output columns per 16-tick arrival block, roundup16(KQ + 15)
     int b_scale_log2;                // tensor-core mode: the LUT operand is R * 2^b_scale_log2, chosen per LUT so that max |R| lands
                                      // in (2^9, 2^10] (fp16 / e4m3 range of the fixed part splits, response_tc.cuh)
+    float trunc_kappa;               // tensor-core mode: expected relative loss per accumulated product to the truncating fp32
+                                     // accumulation of tcgen05.mma, added back by the response's epilogue (0 = off)
     int KQ, nq;                      // tensor-core mode: LUT ticks per piece and pieces (K <= 209: one piece of K ticks; longer
                                      // LUTs are cut into pieces of 200 ticks, each a row of its own in `partial`, added by S5)
     int n_tpcs;

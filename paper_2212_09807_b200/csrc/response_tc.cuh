@@ -52,10 +52,13 @@ struct Args {
     const __half *A;               // [n_tb][NC][2][TB][128 bytes]: fp16 image (a_image_offset) + fp8 image (a8_image_offset)
     const __half *B;               // [WW][NC][CTA of the pair][fp16 image (b_image_offset) | fp8 image (b8_image_offset)] of that CTA's rows
     float *partial;                // [n_tiles][WW][tile_ticks]
-    const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), 0
+    const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), non-zero cells
+                                   // per 16-tick block / 8 (one byte per block)
     const int32_t *tb_mask;        // [n_units] 16-tick blocks that hold charge in any tile of the unit (bit b)
     int n_tiles, n_units, NC, WW, NBW, tile_ticks, n_stages;
     int b_scale_log2;              // B = R * 2^b_scale_log2 (DevParams)
+    int K;                         // LUT ticks of a row (whole LUT, or one piece of it)
+    float kappa;                   // expected relative truncation loss per accumulated product (see "Accuracy"), 0 = off
     long long n_items;             // n_units * WW: (unit, row of the LUT image)
     unsigned long long *stats;     // device counters (lartpc_get_counters): [1] MMAs issued, [2] bytes copied, [5] items
     int *work;                     // item cursor, zero at launch: items are taken in order as CTAs become free, so the
@@ -540,28 +543,50 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
             const bool live = tile < a.n_tiles;
             const bool even = (mask & 5) != 0, odd = (mask & 10) != 0;
             float scale = 0.f;
-            if (live) scale = __int_as_float((127 + a.tile_meta[4 * tile + 2] - a.b_scale_log2) << 23);
+            float nzb[NBLK] = {0.f, 0.f, 0.f, 0.f};
+            if (live) {
+                const int4 tm = *(const int4 *)(a.tile_meta + 4 * tile);
+                scale = __int_as_float((127 + tm.z - a.b_scale_log2) << 23);
+#pragma unroll
+                for (int b = 0; b < NBLK; ++b) nzb[b] = (float)(((unsigned)tm.w >> (8 * b)) & 255u) * (8.f / 16.f) * a.kappa;
+            }
+            // 1 + kappa x (non-zero cells with arrival tick j in (n - K, n], of the blocks of one parity): what the
+            // accumulator column of output tick n lost to truncation, in expectation.  Cells are taken as spread evenly
+            // over the 16 ticks of their block; evaluated every 8 ticks, linear in between.
+            auto comp = [&](int n, int par) -> float {
+                const int m = n - a.K;
+                const int wa = min(max(n - 16 * par + 1, 0), 16) - min(max(m - 16 * par + 1, 0), 16);
+                const int wb = min(max(n - 16 * par - 31, 0), 16) - min(max(m - 16 * par - 31, 0), 16);
+                return fmaf(nzb[par], (float)wa, fmaf(nzb[par + 2], (float)wb, 1.f));
+            };
             float *dst = a.partial + ((size_t)(live ? tile : 0) * a.WW + d) * a.tile_ticks;
+            float g0e = comp(0, 0), g0o = comp(0, 1);
             // output tick n = even accumulator column n (blocks 0, 2) + odd accumulator column n - 16 (blocks 1, 3)
             for (int n0 = 0; n0 < a.tile_ticks; n0 += 16) {
                 uint32_t v0[16], v1[16];
                 const bool has0 = even && n0 < ACC_COL, has1 = odd && n0 >= 16;
                 if (has0) tmem_ld16(tlane + n0, v0);
                 if (has1) tmem_ld16(tlane + ACC_COL + n0 - 16, v1);
+                const float g1e = comp(n0 + 8, 0), g1o = comp(n0 + 8, 1), g2e = comp(n0 + 16, 0), g2o = comp(n0 + 16, 1);
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
                 if (live) {
                     const int nv = min(16, a.tile_ticks - n0);         // tile_ticks is a multiple of 8
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         if (4 * i >= nv) break;
-                        float4 o;
-                        o.x = ((has0 ? __uint_as_float(v0[4 * i]) : 0.f) + (has1 ? __uint_as_float(v1[4 * i]) : 0.f)) * scale;
-                        o.y = ((has0 ? __uint_as_float(v0[4 * i + 1]) : 0.f) + (has1 ? __uint_as_float(v1[4 * i + 1]) : 0.f)) * scale;
-                        o.z = ((has0 ? __uint_as_float(v0[4 * i + 2]) : 0.f) + (has1 ? __uint_as_float(v1[4 * i + 2]) : 0.f)) * scale;
-                        o.w = ((has0 ? __uint_as_float(v0[4 * i + 3]) : 0.f) + (has1 ? __uint_as_float(v1[4 * i + 3]) : 0.f)) * scale;
-                        __stcs((float4 *)(dst + n0) + i, o);
+                        const float be = (i < 2 ? g0e : g1e) * scale, bo = (i < 2 ? g0o : g1o) * scale;   // value at the 8-tick node
+                        const float se = (i < 2 ? g1e - g0e : g2e - g1e) * (0.125f * scale), so = (i < 2 ? g1o - g0o : g2o - g1o) * (0.125f * scale);
+                        float r[4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const float t = (float)((4 * i + k) & 7);
+                            const float x0 = has0 ? __uint_as_float(v0[4 * i + k]) : 0.f, x1 = has1 ? __uint_as_float(v1[4 * i + k]) : 0.f;
+                            r[k] = fmaf(x0, fmaf(se, t, be), x1 * fmaf(so, t, bo));
+                        }
+                        __stcs((float4 *)(dst + n0) + i, make_float4(r[0], r[1], r[2], r[3]));
                     }
                 }
+                g0e = g2e;  g0o = g2o;
             }
             if (even) for (int c0 = 0; c0 < ACC_COL; c0 += 16) tmem_zero16(tlane + c0);
             if (odd) for (int c0 = ACC_COL; c0 < 2 * ACC_COL; c0 += 16) tmem_zero16(tlane + c0);

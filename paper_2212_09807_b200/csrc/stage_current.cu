@@ -807,6 +807,7 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     a.n_units = (int)((sim->n_tiles + TC_UNIT_TILES - 1) / TC_UNIT_TILES);
     a.NC = p.NB2;  a.WW = p.WW * p.nq;  a.NBW = p.NBW;  a.tile_ticks = p.tile_ticks;   // a row = (target, LUT piece)
     a.b_scale_log2 = p.b_scale_log2;
+    a.K = p.KQ;  a.kappa = p.trunc_kappa;
     a.n_items = (long long)a.n_units * a.WW;
     if (a.n_items >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.work = sim->d_work;

@@ -105,7 +105,7 @@ class Stats(C.Structure):
 
 
 EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", "lartpc_sim_destroy", "lartpc_set_disabled_pixels",
-           "lartpc_set_random_perturbations", "lartpc_chunk_ticks",
+           "lartpc_set_random_perturbations", "lartpc_set_truncation_compensation", "lartpc_chunk_ticks",
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
            "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_run_spill",
            "lartpc_readout_tiles", "lartpc_pack_hits",
@@ -235,6 +235,12 @@ class Sim:
         _check(self.lib.lartpc_set_random_perturbations(self.handle, C.c_int(int(m)),
                                                         C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF)),
                "lartpc_set_random_perturbations")
+
+    def set_truncation_compensation(self, kappa: float):
+        """Tensor-core response: expected relative truncation loss per accumulated product that the epilogue adds back
+        (include/lartpc.h; 0 = off)."""
+        _check(self.lib.lartpc_set_truncation_compensation(self.handle, C.c_double(float(kappa))),
+               "lartpc_set_truncation_compensation")
 
     def set_disabled_pixels(self, ids: np.ndarray):
         ids = np.ascontiguousarray(ids, dtype=np.int32)

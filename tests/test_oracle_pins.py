@@ -649,3 +649,108 @@ def test_random_estimator_is_unbiased():
     assert big.sum() >= 2
     assert np.all(np.abs(mean - q_exp)[big] <= 5 * sem[big] + 1e-6 * np.abs(q_exp).max())
     assert np.all(sem[big] > 0)                                   # the draws do differ from seed to seed
+
+
+# ------------------------------------------------------------------ O7 truth association (reading D26)
+
+def _collect_lut(p):
+    """Hand-made LUT: an electron above the centre pixel of the window is collected whole during its arrival tick
+    (LUT tick K - 1), nothing is induced anywhere else."""
+    nb, Wp, K = p["bins_per_pixel"], p["window_pixels"], p["lut_ticks"]
+    lut = np.zeros((Wp * nb, Wp * nb, K), dtype=np.float32)
+    h = (Wp - 1) // 2
+    lut[h * nb:(h + 1) * nb, h * nb:(h + 1) * nb, K - 1] = 1.0
+    return lut
+
+
+def test_hit_truth_hand_case():
+    """Four short segments at the anode (sigma = 0) above pixel (4, 4) and one above its neighbour, under a LUT that
+    collects a charge whole at its arrival tick (readout tick j + K - 1, K = 8).  Arrival ticks 12, 20, 30, 60 ->
+    readout ticks 19, 27, 37, 67.  Charges: s0 alone stays below 7000 e-, s0 + s1 crosses at tick 27, the sample comes at
+    43 and holds s0 + s1 + s2 (s2 arrives during the hold, D15); s3 crosses alone at 67, sample 83, integrated from tick
+    44 on.  Shares are the charges themselves, fractions their ratios; the neighbour's segment s4 feeds nothing."""
+    p = W.default_params(lut_ticks=8, n_readout_ticks=120)
+    tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, 5.0, 9, 9, 0)]
+    lut = _collect_lut(p)
+    pitch = p["pixel_pitch_cm"]
+    x, y = 4.5 * pitch, 4.5 * pitch
+    f = lambda v: np.asarray(v, dtype=np.float32)
+    t = [1.23, 2.05, 3.04, 6.0, 2.05]
+    xs = [x, x + 0.01, x - 0.02, x, x - pitch]
+    dE = [0.15, 0.11, 0.05, 0.30, 0.4]
+    # 1 mm pieces along x (N = 100 sample points, all above the pixel and in one arrival tick)
+    seg = dict(xs=f([v - 0.05 for v in xs]), ys=f([y] * 5), zs=f([0.0] * 5), ts=f(t), xe=f([v + 0.05 for v in xs]), ye=f([y] * 5),
+               ze=f([0.0] * 5), te=f(t), dE=f(dE))
+    _, ne, dr, pm = _chain(p, tpcs, seg)
+    q = dr["q_a"]
+    assert np.all(dr["sigma_T"] == 0.0) and np.allclose(q, ne)
+    assert q[0] < 7000 <= q[0] + q[1] and q[3] >= 7000 and q[2] > 500
+    waves, _ = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, [4], [4])
+    hp, ht, ha, _ = oracle.electronics(p, 0, [40], waves)
+    assert ht.tolist() == [27 + 16, 67 + 16]
+    sw = oracle.segment_currents(p, tpcs, lut, dr, pm, 0, 4, 4, np.arange(5))
+    assert sw.shape == (5, 120)
+    for s, n in enumerate((19, 27, 37, 67)):                     # each segment alone: its charge at its readout tick
+        want = np.zeros(120)
+        want[n] = q[s]
+        assert np.allclose(sw[s], want, rtol=1e-12, atol=0)
+    assert not sw[4].any()
+    n0, share = oracle.hit_truth(p, ht, sw)
+    assert n0.tolist() == [0, 44]
+    assert np.allclose(share[0], [q[0], q[1], q[2], 0.0, 0.0], rtol=1e-12)
+    assert np.allclose(share[1], [0.0, 0.0, 0.0, q[3], 0.0], rtol=1e-12)
+    frac = share / share.sum(axis=1, keepdims=True)
+    assert frac[0, 0] == pytest.approx(q[0] / (q[0] + q[1] + q[2]), rel=1e-12) and frac[1, 3] == 1.0
+    # the sampled charge is what the ADC digitised (no noise): shares add up to it
+    assert ha.tolist() == [_adc(q[0] + q[1] + q[2]), _adc(q[3])]
+
+
+def test_hit_truth_periodic_reset_window():
+    """Window start with the periodic reset (D17 / D26): 1000 e-/tick from two segments (600 + 400), period 7.  The
+    electronics pin above gives samples at 22, 50, 78, each holding 23 ticks of charge: hit 0 integrates ticks 0..22 (no
+    reset at tick 0, the resets at 7, 14, 21 fall in its hold), hit 1 ticks 28..50 -- the reset at tick 28 clears what
+    ticks 23..27 brought, and tick 28 itself is integrated --, hit 2 ticks 56..78."""
+    p = W.default_params(n_readout_ticks=100, periodic_reset_ticks=7)
+    sw = np.stack([np.full(100, 600.0), np.full(100, 400.0)])
+    hp, ht, ha, _ = oracle.electronics(p, 0, [9], sw.sum(axis=0)[None, :])
+    assert ht.tolist() == [22, 50, 78]
+    n0, share = oracle.hit_truth(p, ht, sw)
+    assert n0.tolist() == [0, 28, 56]
+    assert np.array_equal(share, np.array([[13800.0, 9200.0]] * 3))
+    # without the reset the window of a later hit starts right after the previous sample
+    p2 = W.default_params(n_readout_ticks=100)
+    ht2 = oracle.electronics(p2, 0, [9], sw.sum(axis=0)[None, :])[1]
+    assert ht2.tolist() == [22, 45, 68, 91]
+    n0, share = oracle.hit_truth(p2, ht2, sw)
+    assert n0.tolist() == [0, 23, 46, 69] and np.array_equal(share[1], [600.0 * 23, 400.0 * 23])
+
+
+def test_hit_truth_sums_to_the_sampled_charge():
+    """A diffused track over several pixels, analytic pad LUT: for every hit the shares of all segments add up to the
+    integral of the pixel's total waveform (orc_pixel_current on all segments at once, a different summation order)
+    over the hit's window, that integral reproduces the noise-free ADC code, the fractions add up to one, and every
+    segment's shares over all hits of a pixel plus what was never sampled add up to its integrated current."""
+    p, tpcs, lut = _small_setup(nx=10, ny=10, drift=6.0)
+    pitch = p["pixel_pitch_cm"]
+    seg = W.line_segments([2.2 * pitch, 3.4 * pitch, 1.0], [7.6 * pitch, 5.1 * pitch, 3.0], 0.1, 0.0, W._mip(6.0))
+    _, ne, dr, pm = _chain(p, tpcs, seg)
+    n = len(dr["q_a"])
+    checked = 0
+    for ix, iy in [(3, 3), (4, 4), (5, 4), (6, 4), (7, 5)]:
+        waves, _ = oracle.pixel_currents(p, tpcs, lut, dr, pm, 0, [ix], [iy])
+        hp, ht, ha, _ = oracle.electronics(p, 0, [iy * 10 + ix], waves)
+        if len(ht) == 0:
+            continue
+        sw = oracle.segment_currents(p, tpcs, lut, dr, pm, 0, ix, iy, np.arange(n))
+        assert np.allclose(sw.sum(axis=0), waves[0], rtol=1e-9, atol=1e-9 * np.abs(waves[0]).max())
+        n0, share = oracle.hit_truth(p, ht, sw)
+        for h in range(len(ht)):
+            want = waves[0][n0[h]:ht[h] + 1].sum()
+            assert share[h].sum() == pytest.approx(want, rel=1e-9)
+            assert ha[h] == _adc(want)
+            assert (share[h] / share[h].sum()).sum() == pytest.approx(1.0, abs=1e-12)
+            assert n0[h] == (0 if h == 0 else ht[h - 1] + 1)
+        rest = sw[:, ht[-1] + 1:].sum(axis=1)
+        assert np.allclose(share.sum(axis=0) + rest, sw.sum(axis=1), rtol=1e-9, atol=1e-6)
+        checked += len(ht)
+    assert checked >= 4
