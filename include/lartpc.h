@@ -183,6 +183,16 @@ typedef struct {
                                            max_hits_per_pixel, hits dropped for hit_capacity */
 } lartpc_hits_t;
 
+/* Truth association (reading D26): per hit the k_max segments with the largest shares. */
+typedef struct {
+    int32_t  k_max;                     /* host value: entries per hit, 1 .. 64 */
+    int32_t  reserved;
+    int32_t *seg;                       /* [n_hits][k_max] segment index (into the arrays given to S2 / S3), -1 = unused entry */
+    float   *frac;                      /* [n_hits][k_max] q_{h,s} / q_signal[h]; entries by decreasing |q_{h,s}|, ties by index */
+    float   *q_signal;                  /* [n_hits] sum over ALL segments of q_{h,s}: the charge the sample holds, without noise */
+    int32_t *n_contrib;                 /* [n_hits] segments with a non-zero share */
+} lartpc_truth_t;
+
 typedef struct {
     int64_t n_segments, n_active_segments, n_tiles, n_pairs, n_active_pixels, total_samples;
     int64_t n_hits, n_hits_total, n_pixels_overflow, n_hits_dropped;
@@ -279,6 +289,19 @@ int  lartpc_sum_pixel_signals(lartpc_sim_t *sim, const lartpc_signals_t *signals
 /* S6: Philox4x32-10 noise keyed by (seed, pixel id, tick). */
 int  lartpc_electronics(lartpc_sim_t *sim, const lartpc_waveforms_t *waveforms, uint64_t seed,
                         lartpc_hits_t *out, void *stream);
+
+/* Truth association, an optional pass after S6 (the paper has it for the light path; reading D26).  By
+ * eqs. (3.7)-(3.9) the current on a pixel is a sum over segments; the share of segment s in hit h of pixel p is
+ *     q_{h,s} = sum_{n = n0}^{n_h} I_{p,s}[n],   I_{p,s} = eq. (3.9) for segment s alone,
+ * over the ticks the CSA integrated for that sample: n_h = hit_tick, n0 = hit_tick of the pixel's previous hit + 1 (0 for
+ * its first), or a later periodic-reset tick <= n_h - hold_ticks.  Shares are signed (bipolar induced currents); noise
+ * belongs to no segment.  `hits` must be sorted by (pixel, tick) as S6 / S7 write it, n_hits its length; drifted / pixmap /
+ * n are those the sim's current plan (S3) was made from (LARTPC_ERR_ORDER otherwise: after lartpc_run_spill the plan holds
+ * the last TPC batch only, so use the staged calls).  Not available with lartpc_set_random_perturbations (m > 0).
+ * Accuracy: a share is within max(1e-4 |q|, 1 e-) of the fp64 value (same weights as S4).  Cost: one pass over the charge
+ * cells of every (hit, segment, source pixel): seconds at configs[3] scale, it is not part of lartpc_run_spill. */
+int  lartpc_hit_truth(lartpc_sim_t *sim, const lartpc_drifted_t *drifted, const lartpc_pixmap_t *pixmap, int64_t n,
+                      const lartpc_hits_t *hits, int64_t n_hits, lartpc_truth_t *out, void *stream);
 
 /* S7: the whole path on device-resident segments; hits of all batches are appended to *out in
  * (pixel id, tick) order per batch (batches are TPC ranges, so the list is globally sorted).

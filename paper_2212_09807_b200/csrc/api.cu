@@ -42,7 +42,7 @@ static void sim_free(lartpc_sim *s)
 {
     if (!s) return;
     DeviceGuard dg(s->device);
-    cudaFree(s->d_tpcs); cudaFree(s->d_lut); cudaFree(s->d_lut_tc);
+    cudaFree(s->d_tpcs); cudaFree(s->d_lut); cudaFree(s->d_lut_tc); cudaFree(s->d_cum_lut);
     cudaFree(s->pix_count); cudaFree(s->pix_start); cudaFree(s->pix_tile0); cudaFree(s->pix_cursor);
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
     cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->tile_list); cudaFree(s->seg_rec);
@@ -182,6 +182,7 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     if (response_mode == LARTPC_RESPONSE_TENSOR && !tc_ok) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
     p.tc_mode = (response_mode != LARTPC_RESPONSE_FFMA && tc_ok) ? 1 : 0;
     if (best_groups == 0 && !p.tc_mode) { sim_free(s); return LARTPC_ERR_UNSUPPORTED; }
+    s->lut_copy.assign(lut_host, lut_host + lut_elems);
     if (p.tc_mode) {
         // operand scale of the LUT: a power of two that puts max |R| into (2^9, 2^10], whatever units the table is in
         // (fp16 operand, e4m3 cross-term parts: response_tc.cuh); a table with a non-finite entry is refused
@@ -392,6 +393,17 @@ extern "C" int lartpc_induced_current(lartpc_sim_t *sim, const lartpc_drifted_t 
                                        : launch_current_response(sim, out, (cudaStream_t)stream);
     if (rc == 0) sim->have_signals = true;
     return rc;
+}
+
+extern "C" int lartpc_hit_truth(lartpc_sim_t *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
+                                const lartpc_hits_t *hits, int64_t n_hits, lartpc_truth_t *out, void *stream)
+{
+    if (!sim || !dr || !pm || !hits || !out || n_hits < 0 || out->k_max < 1 || out->k_max > 64) return LARTPC_ERR_BAD_ARGUMENT;
+    if (n_hits > 0 && (!hits->hit_pixel || !hits->hit_tick || !out->seg || !out->frac || !out->q_signal || !out->n_contrib))
+        return LARTPC_ERR_BAD_ARGUMENT;
+    DeviceGuard dg(sim->device);
+    if (!sim->have_plan || n != sim->plan_n) return LARTPC_ERR_ORDER;
+    return launch_hit_truth(sim, dr, pm, hits, n_hits, out, (cudaStream_t)stream);
 }
 
 extern "C" int lartpc_sum_pixel_signals(lartpc_sim_t *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out,

@@ -83,6 +83,8 @@ struct lartpc_sim {
     DevParams dp;
     DevTpc *d_tpcs = nullptr;
     float *d_lut = nullptr;              // [NB2][WW][RS], zero padded rows
+    std::vector<float> lut_copy;         // the table as given (host): source of the running-sum table of lartpc_hit_truth
+    float *d_cum_lut = nullptr;          // [W nb][W nb][K] running sum over LUT ticks (built on the first lartpc_hit_truth)
     void *d_lut_tc = nullptr;            // tensor-core mode: fp16 hi / lo operand images of the LUT, [WW][NB2][2][NBW * 16]
     int64_t n_cp = 0;                    // charged-pixel grid cells over all TPCs
     int64_t n_pix = 0;                   // pixels over all TPCs (global pixel ids are 0 .. n_pix-1)
@@ -230,6 +232,8 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
                 int tpc_lo, int tpc_hi, lartpc_pixmap_t *out, lartpc_pixmap_info_t *info, cudaStream_t st);
 int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n,
                          lartpc_signals_t *out, cudaStream_t st);
+int launch_hit_truth(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, const lartpc_hits_t *hits,
+                     int64_t n_hits, lartpc_truth_t *out, cudaStream_t st);
 int launch_seg_records(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, int64_t n, cudaStream_t st);
 int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st);
 int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t st);

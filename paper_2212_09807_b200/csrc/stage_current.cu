@@ -410,6 +410,7 @@ __global__ void __launch_bounds__(NT1, 3) charge_lattice_kernel(const SplatArgs 
 
 #include "quadrature_tables.cuh"
 #include "charge_tc.cuh"
+#include "truth.cuh"
 
 size_t splat_smem_bytes(const DevParams &p)
 {
@@ -710,6 +711,53 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     return LARTPC_OK;
 }
 
+
+// Truth association (truth.cuh): shares of the segments in every hit of a list sorted by (pixel, tick)
+int launch_hit_truth(lartpc_sim *sim, const lartpc_drifted_t *dr, const lartpc_pixmap_t *pm, const lartpc_hits_t *hits,
+                     int64_t n_hits, lartpc_truth_t *out, cudaStream_t st)
+{
+    const DevParams &p = sim->dp;
+    if (n_hits == 0) return LARTPC_OK;
+    if (p.rnd_m > 0 || p.nb > 15 || n_hits >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
+    if (!sim->d_cum_lut) {
+        // running sum of the response over LUT ticks, built once per sim from the table lartpc_sim_create was given
+        const size_t elems = sim->lut_copy.size();
+        float *raw = nullptr;
+        LARTPC_CUDA_TRY(cudaMalloc(&raw, elems * sizeof(float)));
+        cudaError_t e = cudaMalloc(&sim->d_cum_lut, elems * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(raw, sim->lut_copy.data(), elems * sizeof(float), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) {
+            const long long n_series = (long long)(elems / (size_t)p.K);
+            ++g_lartpc_launches;
+            cum_lut_kernel<<<div_up(n_series, 128), 128, 0, st>>>(raw, sim->d_cum_lut, n_series, p.K);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cudaFree(raw);
+        if (e != cudaSuccess) {
+            if (sim->d_cum_lut) cudaFree(sim->d_cum_lut);
+            sim->d_cum_lut = nullptr;
+            lartpc_note_cuda_error(e, __FILE__, __LINE__);
+            return LARTPC_ERR_CUDA;
+        }
+    }
+    TruthArgs a;
+    a.p = p;
+    a.tpcs = sim->d_tpcs;
+    a.pix_start = sim->pix_start;  a.pix_count = sim->pix_count;  a.pair_seg = sim->pair_seg;
+    a.q_anode = dr->q_anode;  a.sigma_T = dr->sigma_T;  a.sigma_t = dr->sigma_t;
+    a.u_s = dr->u_s; a.v_s = dr->v_s; a.u_e = dr->u_e; a.v_e = dr->v_e; a.T_s = dr->T_s; a.T_e = dr->T_e;
+    a.a_lo = pm->a_lo; a.a_hi = pm->a_hi; a.b_lo = pm->b_lo; a.b_hi = pm->b_hi;
+    a.jt0 = pm->jt0; a.jt1 = pm->jt1; a.n_samples = pm->n_samples;
+    a.cum_lut = sim->d_cum_lut;
+    a.hit_pixel = hits->hit_pixel;  a.hit_tick = hits->hit_tick;
+    a.n_hits = n_hits;  a.k_max = out->k_max;
+    a.out_seg = out->seg;  a.out_frac = out->frac;  a.out_q = out->q_signal;  a.out_n = out->n_contrib;
+    ++g_lartpc_launches;
+    hit_truth_kernel<<<(unsigned)n_hits, TR_THREADS, 0, st>>>(a);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}
 
 // per-segment records of the tensor-core splat, written once per plan of the whole input (launch_plan with tpc_lo = 0);
 // sets d_counters[CNT_COMPOSITE] when some segment wants composite node rules

@@ -97,6 +97,10 @@ class Hits(C.Structure):
                 ("hits_per_pixel", _P), ("q_pixel", _P), ("counters", _P)]
 
 
+class Truth(C.Structure):
+    _fields_ = [("k_max", C.c_int32), ("reserved", C.c_int32), ("seg", _P), ("frac", _P), ("q_signal", _P), ("n_contrib", _P)]
+
+
 class Stats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n_segments", "n_active_segments", "n_tiles", "n_pairs", "n_active_pixels",
                                         "total_samples", "n_hits", "n_hits_total", "n_pixels_overflow",
@@ -107,7 +111,7 @@ class Stats(C.Structure):
 EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", "lartpc_sim_destroy", "lartpc_set_disabled_pixels",
            "lartpc_set_random_perturbations", "lartpc_set_truncation_compensation", "lartpc_chunk_ticks",
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
-           "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_run_spill",
+           "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_hit_truth", "lartpc_run_spill",
            "lartpc_readout_tiles", "lartpc_pack_hits",
            "lartpc_measure_fp32_peak", "lartpc_set_profiling", "lartpc_get_stage_ms", "lartpc_get_counters", "lartpc_kernel_launches",
            "lartpc_strerror")
@@ -341,6 +345,23 @@ class Sim:
                                            _stream_ptr(t)), "lartpc_electronics")
         out["_struct"] = h
         return out
+
+    def hit_truth(self, drifted, pixmap, hits, n_hits: Optional[int] = None, k_max: int = 4):
+        """Truth association after the staged S6 (reading D26): per hit the ``k_max`` segments with the largest shares.
+        Returns a dict: seg int32 [n_hits, k_max] (-1 = unused), frac float32 [n_hits, k_max], q_signal float32 [n_hits],
+        n_contrib int32 [n_hits]."""
+        t = self.torch
+        n = int(hits["counters"][0].item()) if n_hits is None else int(n_hits)
+        m = max(n, 1)
+        out = dict(seg=self._empty(m * k_max, t.int32), frac=self._empty(m * k_max, t.float32),
+                   q_signal=self._empty(m, t.float32), n_contrib=self._empty(m, t.int32))
+        tr = Truth(k_max=int(k_max), reserved=0, **{k: v.data_ptr() for k, v in out.items()})
+        n_seg = int(drifted["tpc"].numel())
+        _check(self.lib.lartpc_hit_truth(self.handle, C.byref(drifted["_struct"]), C.byref(pixmap["_struct"]), C.c_int64(n_seg),
+                                         C.byref(hits["_struct"]), C.c_int64(n), C.byref(tr), _stream_ptr(t)),
+               "lartpc_hit_truth")
+        return dict(seg=out["seg"][:n * k_max].view(n, k_max), frac=out["frac"][:n * k_max].view(n, k_max),
+                    q_signal=out["q_signal"][:n], n_contrib=out["n_contrib"][:n])
 
     STAGES = ("quench", "drift", "pixels_from_segments", "induced_current_charge", "induced_current_response",
               "sum_pixel_signals", "electronics")
