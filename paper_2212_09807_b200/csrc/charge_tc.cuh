@@ -68,6 +68,18 @@ __device__ __forceinline__ float erf_fast(float x)
 }
 
 
+// Node rule (quadrature_tables.cuh) for a segment, or a run of a segment's midpoints, whose extent over the diffusion
+// sigma is rho and that holds n_mid midpoints: index into c_quad_n / c_quad_off, -1 = keep the midpoints.  Thresholds:
+// the n-node rule reproduces the midpoint sum to a few 1e-6 of the largest cell for N = 100 and ~1e-5 for N = 50 (DESIGN.md
+// section 6 has the measured table); the rules below 8 nodes are used from 32 midpoints on.
+__device__ __forceinline__ int quad_rule_for(float rho, int n_mid)
+{
+    int k = rho <= 1.0f ? 0 : rho <= 1.75f ? 1 : rho <= 2.25f ? 2 : rho <= 3.5f ? 3 : rho <= 5.5f ? 4 : rho <= 8.f ? 5
+          : rho <= 12.f ? 6 : rho <= 16.f ? 7 : -1;
+    if (k >= 0 && k < 3 && n_mid < 32) k = 3;
+    return (k >= 0 && n_mid >= 3 * c_quad_n[k]) ? k : -1;
+}
+
 // one thread per segment: the record the tiles gather (every division of the old per-tile staging happens here, once)
 __global__ void __launch_bounds__(256)
 seg_record_kernel(DevParams p, int64_t n, const float *__restrict__ q_anode, const float *__restrict__ sigma_T,
@@ -99,8 +111,7 @@ seg_record_kernel(DevParams p, int64_t n, const float *__restrict__ q_anode, con
     if (!zero_sigma && r.rho > 16.f && r.N < (1 << 24) && q_anode[i] > 0.f) {
         const int pieces = min((int)ceilf(r.rho * (1.0f / 16.f)), 64);
         const float rho = r.rho / (float)pieces;
-        const int k = rho <= 3.5f ? 0 : rho <= 5.5f ? 1 : rho <= 8.f ? 2 : rho <= 12.f ? 3 : rho <= 16.f ? 4 : -1;
-        if (k >= 0 && r.N / pieces >= 3 * c_quad_n[k]) *composite_flag = 1;          // (the choice stage_segment<true> makes)
+        if (quad_rule_for(rho, r.N / pieces) >= 0) *composite_flag = 1;          // (the choice stage_segment<true> makes)
     }
     r.flags = (int)(i << 1) | (zero_sigma ? 1 : 0);                  // segment id (n < 2^30) and the sigma = 0 flag
     uint4 *dst = (uint4 *)(rec + i);
@@ -141,8 +152,8 @@ __device__ __forceinline__ int stage_segment(const DevParams &p, const SegRec &r
         // piece (<< 8) and pieces - 1 (<< 16)
         const int pieces = (!COMP || r.rho <= 16.f || r.N >= (1 << 24)) ? 1 : min((int)ceilf(r.rho * (1.0f / 16.f)), 64);
         const float rho = r.rho / (float)pieces;
-        const int k = rho <= 3.5f ? 0 : rho <= 5.5f ? 1 : rho <= 8.f ? 2 : rho <= 12.f ? 3 : rho <= 16.f ? 4 : -1;
-        if (k >= 0 && r.N / pieces >= 3 * c_quad_n[k]) {
+        const int k = quad_rule_for(rho, r.N / pieces);
+        if (k >= 0) {
             L.rule = c_quad_off[k];
             nq = pieces * c_quad_n[k];
             if (COMP) L.rule |= (c_quad_n[k] << 8) | ((pieces - 1) << 16);

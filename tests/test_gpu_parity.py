@@ -250,22 +250,22 @@ def test_empty_input(lartpc):
 
 def test_short_drift_all_node_rules(lartpc):
     """The tensor-core splat replaces a segment's N midpoints by an n-node rule chosen from its extent over the
-    diffusion sigma (n = 8 .. 32, or its own midpoints when the segment is sharp or short).  Tracks along x, along the
+    diffusion sigma (n = 4 .. 32, or its own midpoints when the segment is sharp or short).  Tracks along x, along the
     drift direction and oblique, at 0.2 .. 8 cm of drift, with 1 mm, 0.5 mm and 0.25 mm segments, walk through every
     rule and the fall-back; every pixel is compared with the oracle (which always sums the N midpoints)."""
     p = W.default_params(n_readout_ticks=1400)
-    tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, 12.0, 24, 24, 0)]
+    tpcs = [W.make_tpc(0.0, 0.0, 0.0, +1, 12.0, 24, 28, 0)]
     pitch = p["pixel_pitch_cm"]
     parts = []
     for k, (z, step) in enumerate([(0.2, 0.1), (0.5, 0.1), (1.0, 0.1), (2.0, 0.1), (4.0, 0.1), (8.0, 0.1),
-                                   (0.5, 0.05), (2.0, 0.05), (8.0, 0.025)]):
+                                   (0.5, 0.05), (2.0, 0.05), (8.0, 0.025), (5.5, 0.05), (8.0, 0.05)]):
         y = (2.2 + 2.1 * k) * pitch
         parts.append(W.line_segments([3.1 * pitch, y, z], [6.3 * pitch, y + 0.013, z], step, 0.0, W._mip(2.1)))        # along x
         parts.append(W.line_segments([9.4 * pitch, y, z], [9.4 * pitch + 0.01, y + 0.02, z + 0.6], step, 0.0, W._mip(2.1)))  # along the drift
         parts.append(W.line_segments([13.2 * pitch, y, z], [15.9 * pitch, y + 0.5 * pitch, z + 0.35], step, 0.0, W._mip(6.0)))  # oblique
     # long segments (10 mm at 8 cm, 5 mm at 1 cm of drift): beyond the largest rule, they keep their own midpoints
-    parts.append(W.line_segments([2.2 * pitch, 21.3 * pitch, 8.0], [11.0 * pitch, 22.1 * pitch, 8.9], 1.0, 0.0, W._mip(2.1)))
-    parts.append(W.line_segments([14.2 * pitch, 21.6 * pitch, 1.0], [17.5 * pitch, 22.4 * pitch, 1.3], 0.5, 0.0, W._mip(2.1)))
+    parts.append(W.line_segments([2.2 * pitch, 25.3 * pitch, 8.0], [11.0 * pitch, 26.1 * pitch, 8.9], 1.0, 0.0, W._mip(2.1)))
+    parts.append(W.line_segments([14.2 * pitch, 25.6 * pitch, 1.0], [17.5 * pitch, 26.4 * pitch, 1.3], 0.5, 0.0, W._mip(2.1)))
     seg = W._concat(parts)
     wl = W.Workload("short-drift", 6, p, tpcs, seg, W.pad_response_lut(p))
     sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
