@@ -238,6 +238,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
         const int tile1 = s_q[s1], tile2 = s_q[s2];
         const int A_t = td.px * NB, B_t = td.py * NB, J_t = td.j_start;
         const int lstart = tl.x, lcount = tl.y;
+        const int bm = __ldg(a.tb_mask + tile / TC_UNIT_TILES);          // for the read-out, in flight until then
         int q_new = 0;
         bool any_mma = false, fetched = false;
 
@@ -446,17 +447,17 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             rtc::tmem_ld32(tlane + 32, v[1]);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             float mx = 0.f;
-            int lo = INT_MAX, hi = -1;
-            int pk01 = 0, pk23 = 0;                                      // non-zero cells of this row per 16-tick block, 16 bits each
+            uint32_t nz_lo = 0u, nz_hi = 0u;                             // bit j: tick j of this row holds charge
     #pragma unroll
             for (int j = 0; j < 64; ++j) {
                 const float x = __uint_as_float(v[j >> 5][j & 31]);
                 mx = fmaxf(mx, fabsf(x));
-                if (x != 0.f) {
-                    lo = min(lo, j); hi = j;
-                    if (j < 32) pk01 += 1 << (16 * (j >> 4)); else pk23 += 1 << (16 * ((j >> 4) - 2));
-                }
+                if (x != 0.f) { if (j < 32) nz_lo |= 1u << j; else nz_hi |= 1u << (j - 32); }
             }
+            int lo = nz_lo ? __ffs(nz_lo) - 1 : nz_hi ? 31 + __ffs(nz_hi) : INT_MAX;
+            int hi = nz_hi ? 63 - __clz(nz_hi) : nz_lo ? 31 - __clz(nz_lo) : -1;
+            // non-zero cells of this row per 16-tick block, 16 bits each
+            int pk01 = __popc(nz_lo & 0xffffu) | __popc(nz_lo >> 16) << 16, pk23 = __popc(nz_hi & 0xffffu) | __popc(nz_hi >> 16) << 16;
             for (int d = 16; d; d >>= 1) {
                 mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, d));
                 lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, d));
@@ -484,7 +485,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             if (mx >= 32768.f) e = min(((__float_as_int(mx) >> 23) & 0xff) - 127 - 14, 100);   // mx * 2^-e in [2^14, 2^15)
             if (!(mx < 3.0e38f)) e = 0;                                   // inf / nan charge: leave it visible
             const float sc = __int_as_float((127 - e) << 23);
-            if (tid == 0) {
+            if (tid == CT_THREADS - 1) {                                  // a lane whose cell row does not exist: off the stores' path
                 if (nz == 0) *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(1, 0, 0, 0);
                 else {
                     *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(lo / RESP_NO, (hi + p.K - 1) / RESP_NO, e, nz_packed);
@@ -498,7 +499,6 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             if (tid < NB2) {
                 // rows of the response's operand image; only the 16-tick blocks some tile of the block charges exist
                 const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;
-                const int bm = a.tb_mask[tile / TC_UNIT_TILES];
                 unsigned char *cb = (unsigned char *)a.charge + ((size_t)tb * NB2 + tid) * (rtc::NBLK * rtc::A_BLOCK_BYTES);
 #pragma unroll
                 for (int b = 0; b < rtc::NBLK; ++b) {
