@@ -47,7 +47,7 @@ static void sim_free(lartpc_sim *s)
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
     cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->tile_list); cudaFree(s->seg_rec);
     cudaFree(s->pack_base); cudaFree(s->pack_count);
-    cudaFree(s->tile_perm); cudaFree(s->tile_desc_p); cudaFree(s->tile_list_p); cudaFree(s->tb_mask); cudaFree(s->cls_hist); cudaFree(s->scan_tmp);
+    cudaFree(s->tile_perm); cudaFree(s->tile_desc_p); cudaFree(s->tile_list_p); cudaFree(s->tb_mask); cudaFree(s->tc_cmask); cudaFree(s->cls_hist); cudaFree(s->scan_tmp);
     cudaFree(s->d_counters); cudaFree(s->disabled_mask); cudaFree(s->elec_slots); cudaFree(s->elec_offs);
     cudaFree(s->d_fma); cudaFree(s->d_work); cudaFree(s->pix_jmin); cudaFree(s->d_end_row);
     for (cudaEvent_t e : s->ev_pool) cudaEventDestroy(e);

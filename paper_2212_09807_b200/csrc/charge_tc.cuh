@@ -496,6 +496,16 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                     if (vx > 0 && vy > 0) atomicAdd(a.fma_counter, (unsigned long long)nz * (unsigned long long)(vx * vy * p.K));
                 }
             }
+            {
+                // blocks this cell row charges -> the unit's per-bin block mask the response skips by (4 bits per bin, 8 bins
+                // per word: the 8 lanes of a word combine first, one atomic per word and tile)
+                int bits = ((nz_lo & 0xffffu) ? 1 : 0) | ((nz_lo >> 16) ? 2 : 0) | ((nz_hi & 0xffffu) ? 4 : 0) | ((nz_hi >> 16) ? 8 : 0);
+                bits <<= 4 * (lane & 7);
+                bits |= __shfl_xor_sync(0xffffffffu, bits, 1);
+                bits |= __shfl_xor_sync(0xffffffffu, bits, 2);
+                bits |= __shfl_xor_sync(0xffffffffu, bits, 4);
+                if ((lane & 7) == 0 && bits) atomicOr(a.cmask + (size_t)(tile / TC_UNIT_TILES) * TC_CMASK_WORDS + (tid >> 3), bits);
+            }
             if (tid < NB2) {
                 // rows of the response's operand image; only the 16-tick blocks some tile of the block charges exist
                 const int tb = tile / rtc::TB, r = tile - tb * rtc::TB;

@@ -71,6 +71,12 @@ constexpr bool TC_CTA_PAIR = false;  // the tensor-core response runs as CTA pai
 constexpr int TC_UNIT_TILES = TC_CTA_PAIR ? 2 * TC_TILE_BLOCK : TC_TILE_BLOCK;   // tiles one response item multiplies at once:
                                      // the 16-tick block masks (tb_mask) are kept per unit
 
+constexpr int TC_BOXQ = 5;           // tile sort: classes per edge of the box of charged bins (bins 0-1, 2-3, .. 8-9 for 10 bins per pixel)
+constexpr int TC_BOX_CLASSES = TC_BOXQ * TC_BOXQ * TC_BOXQ * TC_BOXQ;
+constexpr int TC_CLASSES = 16 * TC_BOX_CLASSES;     // (16-tick block mask, box class)
+constexpr int TC_CMASK_WORDS = 16;   // tc_cmask: per unit, 4 bits per LUT bin (the 16-tick blocks of that bin some tile of the unit
+                                     // charges), 8 bins per 32-bit word, 128 operand rows
+
 // device counters written by the planning kernels (mirrored to pinned host memory)
 enum {
     CNT_MAX_NPIX = 0, CNT_MAX_TICKS, CNT_ACTIVE_SEGS, CNT_PAIRS, CNT_TILES, CNT_ACTIVE_PIX,
@@ -101,7 +107,8 @@ struct lartpc_sim {
     // tensor-core mode: tiles sorted by the 16-tick blocks they charge (launch_plan): slot of a tile, descriptors and
     // lists in slot order, per 128-slot block the OR of its tiles' block masks
     int32_t *tile_perm = nullptr;  TileDesc *tile_desc_p = nullptr;  int2 *tile_list_p = nullptr;
-    int32_t *tb_mask = nullptr;  int32_t *cls_hist = nullptr;   // [tile_cap / 128 + 2], [32]: class counts then cursors
+    int32_t *tb_mask = nullptr;  int32_t *cls_hist = nullptr;   // [tile_cap / 128 + 2], [2 TC_CLASSES]: class counts then cursors
+    int32_t *tc_cmask = nullptr;         // [tile_cap / 128 + 2][TC_CMASK_WORDS]: blocks charged per (unit, bin), written by the charge lattice
     std::vector<int64_t> cp_base_h, pix_base_h;   // [n_tpcs + 1] first charged-pixel cell / first pixel of each TPC (host copy)
     int64_t plan_pix_lo = 0, plan_pix_hi = 0;       // pixel range of the TPCs the current plan covers
     int32_t *pack_base = nullptr, *pack_count = nullptr;  int pack_tile_pixels = 0;   // lartpc_pack_hits: readout-tile tables

@@ -55,6 +55,7 @@ struct Args {
     const int32_t *tile_meta;      // [n_tiles][4]: first / last output block, scale exponent e (A = C * 2^-e), non-zero cells
                                    // per 16-tick block / 8 (one byte per block)
     const int32_t *tb_mask;        // [n_units] 16-tick blocks that hold charge in any tile of the unit (bit b)
+    const int32_t *cmask;          // [n_units][CMW] per bin (4 bits, 8 bins per word) the blocks some tile of the unit charges
     int n_tiles, n_units, NC, WW, NBW, tile_ticks, n_stages;
     int b_scale_log2;              // B = R * 2^b_scale_log2 (DevParams)
     int K;                         // LUT ticks of a row (whole LUT, or one piece of it)
@@ -291,6 +292,7 @@ constexpr int MAX_STAGES = 8;
 constexpr int N_MAIL = MAX_STAGES + 2;  // item mailbox slots of the peer: the leader's producer is never more than a ring ahead
 constexpr int HDR_FIRST = 1, HDR_LAST = 2, HDR_END = 4;
 constexpr int ACC_COL = 256;       // TMEM column of the second accumulator (odd 16-tick blocks)
+constexpr int CMW = 16;            // words of a unit's per-bin block mask (common.cuh TC_CMASK_WORDS)
 
 // bytes of Bs one CTA holds per (target, bin): both precision parts of all rows, or of half the rows with the CTA pair
 __host__ __device__ inline uint32_t b_cta_bytes(int NBW, bool cta2) { return (uint32_t)(cta2 ? NBW * 32 : NBW * 64); }
@@ -334,6 +336,7 @@ template <bool CTA2>
 __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
 {
     extern __shared__ unsigned char smem_raw[];
+    __shared__ uint32_t s_cm[CMW];                                     // producer: the current unit's per-bin block masks
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t rank = CTA2 ? cluster_ctarank() : 0u;
     const bool leader = rank == 0u;
@@ -408,29 +411,57 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 if (++m == N_MAIL) { m = 0; mph ^= 1u; }
                 const unsigned char *Ab = (const unsigned char *)a.A + ((size_t)u * (CTA2 ? 2 : 1) + rank) * tb_stride;
                 const unsigned char *Bd = (const unsigned char *)a.B + (size_t)d * NC * b_stride + (size_t)rank * b_cta;
-                const uint32_t bytes = (uint32_t)__popc(mask) * A_BLOCK_BYTES + b_cta;
-                // runs of consecutive charged blocks: {first block, length}, at most two in four bits
-                const int r0b = __ffs(mask) - 1, r0n = __ffs(~(mask >> r0b)) - 1;
-                const int rest = mask & ~(((1 << r0n) - 1) << r0b);
-                const int r1b = rest ? __ffs(rest) - 1 : 0, r1n = rest ? __popc(rest) : 0;
-                for (int c = 0; c < NC; ++c) {
+                // per bin the blocks some tile of the unit charges: a (bin, block) pair nobody charges is neither copied nor
+                // multiplied, a bin nobody charges takes no stage at all
+                int c_first = -1, c_last = -1;
+                {
+                    const uint4 *src = (const uint4 *)(a.cmask + (size_t)u * CMW);
+#pragma unroll
+                    for (int w4 = 0; w4 < CMW / 4; ++w4) {
+                        const uint4 x = __ldg(src + w4);
+                        const uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const int w = 4 * w4 + k;
+                            // keep only the blocks of the unit's mask, bin by bin (a nibble each), and the bins that exist
+                            uint32_t v = xs[k] & ((uint32_t)mask * 0x11111111u);
+                            if (8 * w >= NC) v = 0u;
+                            else if (8 * w + 8 > NC) v &= (1u << (4 * (NC - 8 * w))) - 1u;
+                            if (v) { if (c_first < 0) c_first = 8 * w + ((__ffs(v) - 1) >> 2);  c_last = 8 * w + ((31 - __clz(v)) >> 2); }
+                            s_cm[w] = v;                               // (this thread's own scratch)
+                        }
+                    }
+                }
+                if (c_first < 0) { q = q_next;  continue; }                // (CTA2: the peer computes the same and skips too)
+                unsigned long long n_mma = 0, n_bytes = 0;
+                for (int c = c_first; c <= c_last; ++c) {
+                    const uint32_t mc = (s_cm[c >> 3] >> (4 * (c & 7))) & 15u;
+                    if (mc == 0u) continue;                                // no tile of the unit charges this bin
+                    const uint32_t bytes = (uint32_t)__popc(mc) * A_BLOCK_BYTES + b_cta;
+                    // runs of consecutive charged blocks: {first block, length}, at most two in four bits
+                    const int r0b = __ffs(mc) - 1, r0n = __ffs(~(mc >> r0b)) - 1;
+                    const int rest = mc & ~(((1 << r0n) - 1) << r0b);
+                    const int r1b = rest ? __ffs(rest) - 1 : 0, r1n = rest ? __popc(rest) : 0;
                     const uint32_t st = base + s * stage_sz, fb = full0 + 8 * s;
                     RTC_T(p0);
                     mbar_wait(empty0 + 8 * s, ph ^ 1u);
                     RTC_T(p1);
-                    hdr[s].x = u;  hdr[s].y = d;  hdr[s].z = c | (mask << 16);
-                    hdr[s].w = (c == 0 ? HDR_FIRST : 0) | (c == NC - 1 ? HDR_LAST : 0);
+                    hdr[s].x = u;  hdr[s].y = d;  hdr[s].z = c | ((int)mc << 16) | (mask << 20);
+                    hdr[s].w = (c == c_first ? HDR_FIRST : 0) | (c == c_last ? HDR_LAST : 0);
                     mbar_expect_tx(fb, bytes);                         // release: the header is visible to the waiter
                     const unsigned char *Ac = Ab + (size_t)c * NBLK * A_BLOCK_BYTES;
+                    // the blocks of a stage sit back to back in charged-block order, whatever their number
                     bulk_g2s(st, Ac + r0b * A_BLOCK_BYTES, (uint32_t)r0n * A_BLOCK_BYTES, fb);
                     if (r1n) bulk_g2s(st + r0n * A_BLOCK_BYTES, Ac + r1b * A_BLOCK_BYTES, (uint32_t)r1n * A_BLOCK_BYTES, fb);
                     bulk_g2s(st + a_area, Bd + (size_t)c * b_stride, b_cta, fb);
                     RTC_T(p2);  RTC_ADD(8, p1 - p0);  RTC_ADD(9, p2 - p1);  RTC_ADD(10, 1);
+                    n_mma += 2ull * (unsigned long long)__popc(mc);
+                    n_bytes += bytes;
                     if (++s == S) { s = 0; ph ^= 1u; }
                 }
-                if (leader) {                                          // per item: stages x (2 MMAs per charged block), bytes of the unit
-                    atomicAdd(a.stats + 1, (unsigned long long)(2 * NC * __popc(mask)));
-                    atomicAdd(a.stats + 2, (unsigned long long)NC * bytes * (CTA2 ? 2ull : 1ull));
+                if (leader) {                                          // per item: 2 MMAs per charged (bin, block), bytes of the unit
+                    atomicAdd(a.stats + 1, n_mma);
+                    atomicAdd(a.stats + 2, n_bytes * (CTA2 ? 2ull : 1ull));
                     atomicAdd(a.stats + 5, 1ull);
                 }
                 q = q_next;
@@ -477,7 +508,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 RTC_T(t2);
                 int u, d, cz, flags;
                 asm volatile("ld.volatile.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(u), "=r"(d), "=r"(cz), "=r"(flags) : "r"(hdr0 + 16 * s) : "memory");
-                const int mask = (cz >> 16) & 15;
+                const int mask = (cz >> 16) & 15, umask = (cz >> 20) & 15;
                 if (flags & HDR_END) {
                     if (par) break;
                     mbar_wait_cluster(tempty, tph);                    // the epilogues have read the previous item slot
@@ -490,9 +521,9 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                     mbar_wait_cluster(tempty, tph);                    // accumulators drained and zeroed, in both CTAs
                     tph ^= 1u;
                     if (!par) {
-                        epi_item->x = u;  epi_item->y = d;  epi_item->z = mask;  epi_item->w = 0;
+                        epi_item->x = u;  epi_item->y = d;  epi_item->z = umask;  epi_item->w = 0;
                         mbar_arrive(titem);                            // release: hands the item to the epilogue
-                        if (CTA2) { st_cluster_v4(peer_epi, u, d, mask, 0);  mbar_arrive_remote(peer_titem); }
+                        if (CTA2) { st_cluster_v4(peer_epi, u, d, umask, 0);  mbar_arrive_remote(peer_titem); }
                     }
                 }
                 tc_fence_after();

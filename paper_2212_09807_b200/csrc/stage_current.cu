@@ -142,6 +142,7 @@ struct SplatArgs {
     int *work;                         // tile cursor, zero at launch
     int n_tiles;
     const int32_t *tb_mask;            // [tile blocks] 16-tick blocks that hold charge (bit b)
+    int32_t *cmask;                    // [units][TC_CMASK_WORDS] per LUT bin the blocks some tile of the unit charges (tensor-core splat)
 };
 
 struct SegLocal {               // one staged segment, tile-relative
@@ -672,7 +673,13 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
     a.jt0 = pm->jt0; a.jt1 = pm->jt1; a.n_samples = pm->n_samples;
     a.charge = out->charge;  a.tile_range = out->tile_range;
     a.fma_counter = sim->d_fma;
-    a.rec = nullptr;  a.tile_list = nullptr;  a.work = nullptr;  a.n_tiles = 0;  a.tb_mask = sim->tb_mask;
+    a.rec = nullptr;  a.tile_list = nullptr;  a.work = nullptr;  a.n_tiles = 0;  a.tb_mask = sim->tb_mask;  a.cmask = sim->tc_cmask;
+    if (p.tc_mode) {
+        // per-(unit, bin) block masks: the tensor-core splat ORs in what every tile charges; the FFMA2 splat does not
+        // keep them, every bin then counts as charged
+        const size_t words = (size_t)((sim->n_tiles + TC_UNIT_TILES - 1) / TC_UNIT_TILES) * TC_CMASK_WORDS;
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->tc_cmask, splat_on_tc(p) ? 0 : 0xff, sizeof(int32_t) * words, st));
+    }
     if (p.rnd_m > 0 && !splat_on_tc(p)) return LARTPC_ERR_UNSUPPORTED;
     if (splat_on_tc(p)) {
         // tensor-core splat (charge_tc.cuh); other bin counts use the FFMA2 splat below, which writes the same image
@@ -850,6 +857,8 @@ int launch_current_response_tc(lartpc_sim *sim, lartpc_signals_t *out, cudaStrea
     a.partial = out->partial;
     a.tile_meta = out->tile_range;
     a.tb_mask = sim->tb_mask;
+    a.cmask = sim->tc_cmask;
+    static_assert(rtc::CMW == TC_CMASK_WORDS, "one layout of the per-bin block masks");
     if (sim->n_tiles >= INT32_MAX) return LARTPC_ERR_UNSUPPORTED;
     a.n_tiles = (int)sim->n_tiles;
     a.n_units = (int)((sim->n_tiles + TC_UNIT_TILES - 1) / TC_UNIT_TILES);

@@ -435,9 +435,9 @@ int sim_ensure_scan_tmp(lartpc_sim *sim, int64_t elems)
 int sim_grow_tiles(lartpc_sim *sim, int64_t cap)
 {
     cudaFree(sim->tile_cp); cudaFree(sim->tile_desc); cudaFree(sim->tile_list); cudaFree(sim->tile_perm);
-    cudaFree(sim->tile_desc_p); cudaFree(sim->tile_list_p); cudaFree(sim->tb_mask);
+    cudaFree(sim->tile_desc_p); cudaFree(sim->tile_list_p); cudaFree(sim->tb_mask); cudaFree(sim->tc_cmask);
     sim->tile_cp = nullptr; sim->tile_desc = nullptr; sim->tile_list = nullptr; sim->tile_perm = nullptr;
-    sim->tile_desc_p = nullptr; sim->tile_list_p = nullptr; sim->tb_mask = nullptr; sim->tile_cap = 0;
+    sim->tile_desc_p = nullptr; sim->tile_list_p = nullptr; sim->tb_mask = nullptr; sim->tc_cmask = nullptr; sim->tile_cap = 0;
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_cp, sizeof(int32_t) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc, sizeof(TileDesc) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list, sizeof(int2) * cap));
@@ -445,49 +445,71 @@ int sim_grow_tiles(lartpc_sim *sim, int64_t cap)
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc_p, sizeof(TileDesc) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list_p, sizeof(int2) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tb_mask, sizeof(int32_t) * (cap / TC_TILE_BLOCK + 2)));
-    if (!sim->cls_hist) LARTPC_CUDA_TRY(cudaMalloc(&sim->cls_hist, sizeof(int32_t) * 32));
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->tc_cmask, sizeof(int32_t) * (cap / TC_TILE_BLOCK + 2) * TC_CMASK_WORDS));
+    if (!sim->cls_hist) LARTPC_CUDA_TRY(cudaMalloc(&sim->cls_hist, sizeof(int32_t) * 2 * TC_CLASSES));
     sim->tile_cap = cap;
     return LARTPC_OK;
 }
 
-// ---- tensor-core mode: tiles sorted by the 16-tick arrival blocks they charge ------------------------------------
-// The response multiplies 128 tiles at a time and can skip a 16-tick block only when none of the 128 charges it, so
-// tiles with the same block mask are given neighbouring slots (counting sort over the 16 masks; the order inside a class
-// is whatever the atomics give: a tile's slot only decides where its rows live, never a sum).
+// ---- tensor-core mode: tiles sorted by the 16-tick arrival blocks and the LUT bins they charge -----------------------
+// The response multiplies 128 tiles at a time and can skip a (bin, 16-tick block) pair only when none of the 128 charges
+// it (the charge lattice ORs what each tile really charges into a per-unit mask, tc_cmask).  So tiles that charge the
+// same blocks AND about the same bins are given neighbouring slots: class = (block mask, box of charged bins with its
+// four edges taken in steps of two bins), counting sort over the TC_CLASSES classes in that order; the order inside a
+// class is whatever the atomics give: a tile's slot only decides where its rows live, never a sum.  Measured on
+// configs[3] / configs[2]: 23 % / 33 % of the (unit, bin, block) pairs drop out (profiles/r2_response_bound.md).
+
 __global__ void __launch_bounds__(256)
 tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td, const int2 *__restrict__ tl,
-                  const int32_t *__restrict__ pair_seg, const int32_t *__restrict__ jt0, const int32_t *__restrict__ jt1,
-                  int32_t *cls, int32_t *hist, int sort)
+                  const int32_t *__restrict__ pair_seg, lartpc_pixmap_t pm, int32_t *cls, int32_t *hist, int sort)
 {
-    __shared__ int s_hist[16];
-    if (threadIdx.x < 16) s_hist[threadIdx.x] = 0;
-    __syncthreads();
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int c = TC_CLASSES;                                               // no tile (a group of its own below)
     if (t < n_tiles) {
-        int mask = 0;
+        int mask = 0, alo = p.nb, ahi = -1, blo = p.nb, bhi = -1;
         if (!sort) mask = 15;
         else {
             const TileDesc d = td[t];
             const int2 l = tl[t];
+            const int A_t = d.px * p.nb, B_t = d.py * p.nb;
             for (int k = 0; k < l.y; ++k) {
                 const int s = pair_seg[l.x + k];
-                const int jlo = max(max(jt0[s], 0) - d.j_start, 0), jhi = min(min(jt1[s], p.j_max) - d.j_start, p.Jc - 1);
-                if (jlo <= jhi) mask |= ((2 << (jhi >> 4)) - 1) & ~((1 << (jlo >> 4)) - 1);
+                const int jlo = max(max(pm.jt0[s], 0) - d.j_start, 0), jhi = min(min(pm.jt1[s], p.j_max) - d.j_start, p.Jc - 1);
+                if (jlo > jhi) continue;                              // the segment charges another window of this pixel
+                mask |= ((2 << (jhi >> 4)) - 1) & ~((1 << (jlo >> 4)) - 1);
+                alo = min(alo, max(pm.a_lo[s] - A_t, 0));  ahi = max(ahi, min(pm.a_hi[s] - A_t, p.nb - 1));
+                blo = min(blo, max(pm.b_lo[s] - B_t, 0));  bhi = max(bhi, min(pm.b_hi[s] - B_t, p.nb - 1));
             }
         }
-        cls[t] = mask;
-        atomicAdd(&s_hist[mask], 1);
+        // edges in TC_BOXQ steps over the pixel (any bins_per_pixel); an empty box sorts first
+        const int q = (p.nb + TC_BOXQ - 1) / TC_BOXQ;
+        const int e0 = ahi < alo ? 0 : alo / q, e1 = ahi < alo ? 0 : ahi / q, e2 = bhi < blo ? 0 : blo / q, e3 = bhi < blo ? 0 : bhi / q;
+        c = (((mask * TC_BOXQ + e0) * TC_BOXQ + e1) * TC_BOXQ + e2) * TC_BOXQ + e3;
+        cls[t] = c;
     }
-    __syncthreads();
-    if (threadIdx.x < 16 && s_hist[threadIdx.x]) atomicAdd(&hist[threadIdx.x], s_hist[threadIdx.x]);
+    // one atomic per (warp, class)
+    const int lane = threadIdx.x & 31;
+    const unsigned peers = __match_any_sync(0xffffffffu, c);
+    if (lane == __ffs(peers) - 1 && c < TC_CLASSES) atomicAdd(&hist[c], __popc(peers));
 }
 
-__global__ void class_offsets_kernel(int32_t *hist)                 // [0..15] counts -> [16..31] first slot of the class
+// hist[0 .. TC_CLASSES) counts -> hist[TC_CLASSES .. 2 TC_CLASSES) first slot of the class (one CTA of 1024 threads)
+__global__ void __launch_bounds__(1024) class_offsets_kernel(int32_t *hist)
 {
+    __shared__ int s_part[1024];
+    constexpr int PER = (TC_CLASSES + 1023) / 1024;
+    const int k0 = threadIdx.x * PER;
+    int sum = 0;
+    for (int k = k0; k < min(k0 + PER, TC_CLASSES); ++k) sum += hist[k];
+    s_part[threadIdx.x] = sum;
+    __syncthreads();
     if (threadIdx.x == 0) {
         int run = 0;
-        for (int k = 0; k < 16; ++k) { hist[16 + k] = run; run += hist[k]; }
+        for (int i = 0; i < 1024; ++i) { const int v = s_part[i];  s_part[i] = run;  run += v; }
     }
+    __syncthreads();
+    int run = s_part[threadIdx.x];
+    for (int k = k0; k < min(k0 + PER, TC_CLASSES); ++k) { hist[TC_CLASSES + k] = run;  run += hist[k]; }
 }
 
 __global__ void __launch_bounds__(256)
@@ -496,19 +518,20 @@ tile_scatter_kernel(int64_t n_tiles, int32_t *perm /* in: class, out: slot */, i
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = t < n_tiles;
-    const int mask = valid ? perm[t] : 16;                            // 16: no tile (its own group below)
+    const int c = valid ? perm[t] : TC_CLASSES;                       // TC_CLASSES: no tile (its own group below)
     int slot = (int)t;
     if (sort) {
         // one atomic per (warp, class): the lanes of a class take consecutive slots
         const int lane = threadIdx.x & 31;
-        const unsigned peers = __match_any_sync(0xffffffffu, mask);
+        const unsigned peers = __match_any_sync(0xffffffffu, c);
         const int leader = __ffs(peers) - 1;
         int base = 0;
-        if (lane == leader && valid) base = atomicAdd(&hist[16 + mask], __popc(peers));
+        if (lane == leader && valid) base = atomicAdd(&hist[TC_CLASSES + c], __popc(peers));
         base = __shfl_sync(0xffffffffu, base, leader);
         slot = base + __popc(peers & ((1u << lane) - 1u));
     }
     if (!valid) return;
+    const int mask = c / TC_BOX_CLASSES;
     perm[t] = slot;
     td_p[slot] = td[t];
     tl_p[slot] = tl[t];
@@ -615,12 +638,12 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         // the FFMA2 splat (bins per pixel other than 5 / 10) writes the operand image in the tiles' original order
         const int sort = splat_on_tc(p) ? 1 : 0;
         const int64_t nt = sim->n_tiles;
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->cls_hist, 0, sizeof(int32_t) * 32, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->cls_hist, 0, sizeof(int32_t) * 2 * TC_CLASSES, st));
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->tb_mask, 0, sizeof(int32_t) * (nt / TC_TILE_BLOCK + 1), st));
         g_lartpc_launches += 3;
-        tile_class_kernel<<<div_up(nt, 256), 256, 0, st>>>(p, nt, sim->tile_desc, sim->tile_list, sim->pair_seg, out->jt0,
-                                                          out->jt1, sim->tile_perm, sim->cls_hist, sort);
-        class_offsets_kernel<<<1, 32, 0, st>>>(sim->cls_hist);
+        tile_class_kernel<<<div_up(nt, 256), 256, 0, st>>>(p, nt, sim->tile_desc, sim->tile_list, sim->pair_seg, *out,
+                                                          sim->tile_perm, sim->cls_hist, sort);
+        class_offsets_kernel<<<1, 1024, 0, st>>>(sim->cls_hist);
         tile_scatter_kernel<<<div_up(nt, 256), 256, 0, st>>>(nt, sim->tile_perm, sim->cls_hist, sim->tile_desc,
                                                             sim->tile_list, sim->tile_desc_p, sim->tile_list_p,
                                                             sim->tb_mask, sort);
