@@ -12,7 +12,7 @@ synthetic spill.  Metric (BASELINE.json): segments/s (whole job) with ms/spill a
               float32 arrays and device->host read of the hit list inside the timed region.
 * `roofline`  the dominant kernel (the S4 response on the tcgen05 tensor cores): multiply-adds the method needs for the
               charge it found (counted on the device) x 2 / its CUDA-event time, against the measured bf16 / fp16 tensor
-              peak of MEASURED_PEAKS.json (sustained figure for launches longer than 50 ms); `executed_*` = the dense MMA
+              peak of MEASURED_PEAKS.json (sustained figure when the step is longer than 50 ms, else the burst figure); `executed_*` = the dense MMA
               work actually issued (device-counted tcgen05.mma instructions); `traffic` = its DRAM bytes per launch.
 * `rooflines` one entry per kernel of the path: S1, S2, S3, S5, S6 against the measured HBM copy bandwidth (algorithmic bytes
               of SURVEY.md 8(d) and the bytes the kernel moves), the charge lattice against the SM's thread-instruction
@@ -252,17 +252,30 @@ def run_ours(args):
     median_ms, _ = reduce_over_ranks(float(np.median(step_ms)), n, world, dev)
 
     # ---- end to end through the C-ABI with host buffers ------------------------------------------
+    # a user's loop: pinned host segment arrays in, pinned host hit arrays out, device buffers allocated once; one untimed
+    # pass first (pinned-buffer and allocator warm-up), then the timed passes with both copies inside
     e2e_ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    dseg = {k: torch.empty_like(v) for k, v in seg.items()}
+    n_out = int(st.n_hits * 1.25) + 4096
+    hout = {k: torch.empty(n_out, dtype=torch.int32).pin_memory() for k in ("hit_pixel", "hit_tick", "hit_adc")}
     d2h = 0
+
+    def e2e_step():
+        for k, v in host.items():
+            dseg[k].copy_(v, non_blocking=True)
+        h, st2 = sim.run_spill(dseg, wl.seed, hit_cap, workspace=ws, hits=hits)
+        nh = min(int(st2.n_hits), n_out)
+        for k in hout:
+            hout[k][:nh].copy_(h[k][:nh], non_blocking=True)
+        torch.cuda.synchronize()                                     # the hit list is in host memory
+        return 3 * 4 * nh + 32
+
+    e2e_step()
     barrier()
     e2e_ev[0].record()
     for i in range(args.steps):
         flush.zero_()
-        dseg = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
-        hits, st2 = sim.run_spill(dseg, wl.seed, hit_cap, workspace=ws, hits=hits)
-        nh = int(st2.n_hits)
-        out = [hits[k][:nh].cpu() for k in ("hit_pixel", "hit_tick", "hit_adc")]
-        d2h = sum(o.numel() * o.element_size() for o in out) + 32
+        d2h = e2e_step()
     e2e_ev[1].record()
     barrier()
     flush_ms = 0.0
@@ -333,7 +346,8 @@ def run_ours(args):
         useful = 2.0 * fma_per_launch / (s4_ms * 1e-3) / 1e12 if s4_ms > 0 else 0.0
         if sim.response_mode == "tensor":
             # dense fp16 contraction on tcgen05: peak = measured bf16 GEMM peak (fp16 runs at the same rate)
-            long_launch = s4_ms > 50.0
+            # timed inside a long step (> 50 ms of back-to-back kernels under the power cap): the sustained figure; else burst
+            long_launch = sum(per_step.values()) > 50.0
             if mp.get("bf16_tflops"):
                 peak = float(mp["bf16_tflops_sustained"] if long_launch and mp.get("bf16_tflops_sustained")
                              else mp["bf16_tflops"])
