@@ -329,3 +329,106 @@ def run_chain(wl, pixels: Optional[Dict[int, tuple]] = None, threads: Optional[i
     hp, ht, ha, cnt = electronics(wl.params, seed, res["pixel_id"], res["waves"])
     res.update(hit_pixel=hp, hit_tick=ht, hit_adc=ha, hits_per_pixel=cnt)
     return res
+
+
+# ---------------------------------------------------------------------------------------------------
+# Light simulation: O8-O12 of lartpc_oracle.c
+# ---------------------------------------------------------------------------------------------------
+class OrcLightParams(C.Structure):
+    _fields_ = [("w_ph", C.c_double), ("w_ion", C.c_double), ("dt", C.c_double), ("t_start", C.c_double),
+                ("n_ticks", C.c_int), ("lut_m", C.c_int), ("n_lut_t", C.c_int),
+                ("vx0", C.c_double), ("vy0", C.c_double), ("vz0", C.c_double), ("vsize", C.c_double),
+                ("nvx", C.c_int), ("nvy", C.c_int), ("nvz", C.c_int), ("n_det", C.c_int),
+                ("f_prompt", C.c_double), ("tau_p", C.c_double), ("tau_s", C.c_double), ("trunc_tau", C.c_double),
+                ("normal_above", C.c_double), ("n_resp", C.c_int), ("n_noise", C.c_int)]
+
+
+_LIGHT_MAP = dict(w_ph="w_ph_mev", w_ion="w_ion_mev", dt="tick_us", t_start="t_start_us", n_ticks="n_ticks", lut_m="lut_m",
+                  n_lut_t="n_lut_t", vx0="vox_x0", vy0="vox_y0", vz0="vox_z0", vsize="vox_size_cm", nvx="nvx", nvy="nvy",
+                  nvz="nvz", n_det="n_det", f_prompt="f_prompt", tau_p="tau_prompt_us", tau_s="tau_slow_us",
+                  trunc_tau="trunc_tau", normal_above="normal_above", n_resp="n_resp", n_noise="n_noise")
+
+
+def _light_params(d: Dict) -> OrcLightParams:
+    p = OrcLightParams()
+    for f, k in _LIGHT_MAP.items():
+        setattr(p, f, d[k])
+    return p
+
+
+def light_npe(lp, seg, n_e, eff, vis):
+    """O8, eqs. (4.1)(4.2): returns dict(vox int32[n], k0 int32[n], n_gamma[n], npe[n_det][n])."""
+    lib, n = _load(), seg["xs"].shape[0]
+    s = {k: _f32(v) for k, v in seg.items()}
+    pp = _light_params(lp)
+    nd = int(lp["n_det"])
+    out = dict(vox=np.zeros(n, np.int32), k0=np.zeros(n, np.int32), n_gamma=np.zeros(n), npe=np.zeros((nd, n)))
+    ne = np.ascontiguousarray(n_e, dtype=np.float64)
+    lib.orc_light_npe(C.byref(pp), C.c_int64(n), _fp(s["xs"]), _fp(s["ys"]), _fp(s["zs"]), _fp(s["ts"]),
+                      _fp(s["xe"]), _fp(s["ye"]), _fp(s["ze"]), _fp(s["te"]), _fp(s["dE"]), _dp(ne),
+                      _fp(_f32(eff)), _fp(_f32(vis)), _ip(out["vox"]), _ip(out["k0"]), _dp(out["n_gamma"]), _dp(out["npe"]))
+    return out
+
+
+def light_profile(lp, vox, k0, npe, tprof):
+    """O9, eq. (4.3): photoelectrons per tick [n_det][n_ticks]."""
+    lib = _load()
+    pp = _light_params(lp)
+    ipe = np.zeros((int(lp["n_det"]), int(lp["n_ticks"])))
+    lib.orc_light_profile(C.byref(pp), C.c_int64(len(vox)), _ip(np.ascontiguousarray(vox, np.int32)),
+                          _ip(np.ascontiguousarray(k0, np.int32)), _dp(np.ascontiguousarray(npe, np.float64)),
+                          _fp(_f32(tprof)), _dp(ipe))
+    return ipe
+
+
+def light_scint_weights(lp):
+    """O10: the weights f_scint(s dt) dt of eq. (4.5), s = 0 .. floor(trunc_tau tau_s / dt)."""
+    lib = _load()
+    pp = _light_params(lp)
+    cap = int(lp["trunc_tau"] * lp["tau_slow_us"] / lp["tick_us"]) + 8
+    w = np.zeros(cap)
+    s_max = lib.orc_light_scint_weights(C.byref(pp), _dp(w), C.c_int(cap))
+    return w[:s_max + 1].copy()
+
+
+def light_convolve(x, w, scale=None):
+    """Truncated causal convolution of eq. (4.5) / the sum of eq. (4.6): x [n_det][n_ticks], w [n_w], scale [n_det] or None."""
+    lib = _load()
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    out = np.zeros_like(x)
+    sc = _fp(_f32(scale)) if scale is not None else None
+    lib.orc_light_convolve(C.c_int(x.shape[0]), C.c_int(x.shape[1]), _dp(x), _dp(w), C.c_int(len(w)), sc, _dp(out))
+    return out
+
+
+def light_fluctuate(lp, seed: int, isc):
+    """O11: observed photoelectrons per (sensor, tick) (Poisson below normal_above, normal at or above)."""
+    lib = _load()
+    pp = _light_params(lp)
+    isc = np.ascontiguousarray(isc, dtype=np.float64)
+    out = np.zeros_like(isc)
+    lib.orc_light_fluctuate(C.byref(pp), C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF), _dp(isc), _dp(out))
+    return out
+
+
+def light_noise(lp, seed: int, amp, kf):
+    """O12 noise term of eq. (4.6) (reading D33): [n_det][n_ticks]."""
+    lib = _load()
+    pp = _light_params(lp)
+    out = np.zeros((int(lp["n_det"]), int(lp["n_ticks"])))
+    lib.orc_light_noise(C.byref(pp), C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF), _fp(_f32(amp)),
+                        _ip(np.ascontiguousarray(kf, np.int32)), _dp(out))
+    return out
+
+
+def light_chain(lp, ls, seg, n_e, seed: int):
+    """O8-O12 in sequence on a workload's segments; `ls` carries eff, gain, vis, tprof, resp, noise_amp, noise_k."""
+    a = light_npe(lp, seg, n_e, ls.eff, ls.vis)
+    ipe = light_profile(lp, a["vox"], a["k0"], a["npe"], ls.tprof)
+    isc = light_convolve(ipe, light_scint_weights(lp))
+    nobs = light_fluctuate(lp, seed, isc)
+    v = light_convolve(nobs, ls.resp.astype(np.float64), ls.gain)
+    if int(lp["n_noise"]) > 0:
+        v = v + light_noise(lp, seed, ls.noise_amp, ls.noise_k)
+    return dict(a, ipe=ipe, isc=isc, nobs=nobs, v=v)

@@ -38,6 +38,17 @@
  *                   periodic-reset window start (test_hit_truth_periodic_reset_window); shares of all segments add up to the
  *                   integral of orc_pixel_current's waveform over the window, and that integral reproduces the noise-free
  *                   ADC code of orc_electronics (test_hit_truth_sums_to_the_sampled_charge)
+ *   Light simulation (NEXT-3; tests/test_oracle_light_pins.py):
+ *   orc_light_npe             photon yield worked by hand from eqs. (3.2)(4.1), voxel / tick indices and the outside-the-grid
+ *                             branch by hand, N_gamma + n_e = dE / W_ph (test_light_photon_yield_and_voxels_by_hand)
+ *   orc_light_profile         hand-placed segments with lut_m = 2, light past the waveform dropped, conservation
+ *   orc_light_scint_weights   closed forms of the tick-integrated eq. (4.4), telescoping sum > 0.99, first-order
+ *                             agreement with f_scint(s dt) dt as eq. (4.5) prints it
+ *   orc_light_convolve        numpy.convolve, impulse, steady state
+ *   orc_light_fluctuate(_one) scipy.stats.poisson.ppf at the test's own Philox uniform (Poisson branch), Box-Muller by hand
+ *                             (normal branch), lambda <= 0, moments
+ *   orc_light_noise           one sensor's sinusoids by hand from the Philox phase, mean square
+ *   (whole chain: test_light_chain_conserves_light)
  *   No function is "parity unpinned".
  */
 #include <math.h>
@@ -642,6 +653,153 @@ void orc_hit_truth(const orc_params *p, int n_hits, const int32_t *hit_tick,
             double q = 0.0;
             for (int n = start; n <= hit_tick[h]; ++n) q += w[n];
             share[(size_t)h * n_sel + k] = q;
+        }
+    }
+}
+
+/* =============================================================================================
+ * Light simulation, eqs. (4.1)-(4.6); readings D28-D33 of DESIGN.md.
+ * Test infrastructure like the rest of this file; shares nothing with the CUDA path.
+ * ============================================================================================= */
+typedef struct {
+    double w_ph, w_ion;                 /* MeV per photon at zero field, MeV per electron */
+    double dt, t_start;                 /* simulation tick delta_t and the time of tick 0, us */
+    int    n_ticks;
+    int    lut_m, n_lut_t;              /* LUT time bin = lut_m ticks (D29), LUT time bins */
+    double vx0, vy0, vz0, vsize;        /* voxel grid origin and voxel edge, cm */
+    int    nvx, nvy, nvz, n_det;
+    double f_prompt, tau_p, tau_s;      /* eq. (4.4): ~0.3, ~0.007 us, ~1.6 us */
+    double trunc_tau;                   /* convolution truncated at trunc_tau * tau_s (5) */
+    double normal_above;                /* Poisson below, normal at or above this mean (30 p.e.) */
+    int    n_resp;                      /* taps of the impulse response, sampled at delta_t (D32) */
+    int    n_noise;                     /* sinusoids of the noise model (0 = no noise) */
+} orc_light_params;
+
+/* O8  Incident light, eqs. (4.1)(4.2).
+ *   N_gamma,j = (1/W_ph - R_j/W_ion) dE_j = dE_j / W_ph - n_e,j   (n_e,j = R_j dE_j / W_ion of O1; clamped at >= 0)
+ *   N_pe,ij   = eps_i V_i[voxel of segment j] N_gamma,j
+ * Reading D28: the voxel is the one holding the segment's midpoint; a midpoint outside the voxel grid sees no light
+ * (vox = -1); the deposition time t_0 of eq. (4.3) is the mean of the two end times, its tick k0 = floor((t_0 - t_start)/dt).
+ * npe is [n_det][n] (sensor-major). */
+void orc_light_npe(const orc_light_params *p, int64_t n,
+                   const float *xs, const float *ys, const float *zs, const float *ts,
+                   const float *xe, const float *ye, const float *ze, const float *te, const float *dE,
+                   const double *n_e, const float *eff, const float *vis,
+                   int32_t *vox, int32_t *k0, double *n_gamma, double *npe)
+{
+    const int64_t nvox = (int64_t)p->nvx * p->nvy * p->nvz;
+    for (int64_t j = 0; j < n; ++j) {
+        double xm = 0.5 * ((double)xs[j] + (double)xe[j]), ym = 0.5 * ((double)ys[j] + (double)ye[j]);
+        double zm = 0.5 * ((double)zs[j] + (double)ze[j]), t0 = 0.5 * ((double)ts[j] + (double)te[j]);
+        double ng = (double)dE[j] / p->w_ph - n_e[j];
+        if (!(ng > 0.0)) ng = 0.0;
+        n_gamma[j] = ng;
+        k0[j] = (int32_t)floor((t0 - p->t_start) / p->dt);
+        int64_t ix = (int64_t)floor((xm - p->vx0) / p->vsize), iy = (int64_t)floor((ym - p->vy0) / p->vsize);
+        int64_t iz = (int64_t)floor((zm - p->vz0) / p->vsize);
+        int inside = ix >= 0 && ix < p->nvx && iy >= 0 && iy < p->nvy && iz >= 0 && iz < p->nvz;
+        vox[j] = inside ? (int32_t)((iz * p->nvy + iy) * p->nvx + ix) : -1;
+        for (int i = 0; i < p->n_det; ++i)
+            npe[(size_t)i * n + j] = inside ? (double)eff[i] * (double)vis[(size_t)i * nvox + vox[j]] * ng : 0.0;
+    }
+}
+
+/* O9  Photocurrent time profile, eq. (4.3).  Reading D29: f_i[voxel][b] is the fraction of the sensor's light
+ * that arrives during LUT time bin b (it sums to 1 over b), a LUT bin spans lut_m simulation ticks, and I_pe is kept in
+ * photoelectrons PER TICK: segment j adds N_pe,ij f_i[vox_j][b] / lut_m to each of the ticks k0_j + b lut_m + r, r = 0 ..
+ * lut_m - 1, inside [0, n_ticks).  (The printed prefactor Delta_t_LUT / delta_t and the printed sum index are garbled,
+ * SURVEY D20; this is the reading that conserves photoelectrons.)  ipe is [n_det][n_ticks], overwritten. */
+void orc_light_profile(const orc_light_params *p, int64_t n, const int32_t *vox, const int32_t *k0,
+                       const double *npe, const float *tprof, double *ipe)
+{
+    const int64_t nvox = (int64_t)p->nvx * p->nvy * p->nvz;
+    memset(ipe, 0, sizeof(double) * (size_t)p->n_det * p->n_ticks);
+    for (int i = 0; i < p->n_det; ++i)
+        for (int64_t j = 0; j < n; ++j) {
+            if (vox[j] < 0) continue;
+            const float *f = tprof + ((size_t)i * nvox + vox[j]) * p->n_lut_t;
+            for (int b = 0; b < p->n_lut_t; ++b)
+                for (int r = 0; r < p->lut_m; ++r) {
+                    int64_t t = (int64_t)k0[j] + (int64_t)b * p->lut_m + r;
+                    if (t >= 0 && t < p->n_ticks) ipe[(size_t)i * p->n_ticks + t] += npe[(size_t)i * n + j] * (double)f[b] / (double)p->lut_m;
+                }
+        }
+}
+
+/* O10  Scintillation time structure, eqs. (4.4)(4.5).
+ *   f_scint(t) = f_p/tau_p exp(-t/tau_p) + (1 - f_p)/tau_s exp(-t/tau_s)
+ *   I_scint[t] = sum_{s = 0}^{s_max} I_pe[t - s] w[s],   s_max = floor(trunc_tau tau_s / dt)
+ * Reading D30: eq. (4.5) multiplies a per-tick quantity by the density f_scint((i_t - j_t) dt); the weight of lag s is taken
+ * as the integral of f_scint over that tick,
+ *   w[s] = f_p (e^{-s dt/tau_p} - e^{-(s+1) dt/tau_p}) + (1 - f_p) (e^{-s dt/tau_s} - e^{-(s+1) dt/tau_s}),
+ * which is f_scint(s dt) dt to first order in dt/tau and conserves the light for any tick (point samples of the 7 ns
+ * component at a 16 ns tick would add up to 1.46).  w[s_max + 1] receives the weights; isc is [n_det][n_ticks]. */
+int orc_light_scint_weights(const orc_light_params *p, double *w, int cap)
+{
+    const int s_max = (int)floor(p->trunc_tau * p->tau_s / p->dt);
+    for (int s = 0; s <= s_max && s < cap; ++s) {
+        double t = (double)s * p->dt;
+        w[s] = p->f_prompt * (exp(-t / p->tau_p) - exp(-(t + p->dt) / p->tau_p)) +
+               (1.0 - p->f_prompt) * (exp(-t / p->tau_s) - exp(-(t + p->dt) / p->tau_s));
+    }
+    return s_max;
+}
+
+/* truncated causal convolution out[i][t] = scale_i sum_{s=0}^{n_w-1} in[i][t-s] w[s]: eq. (4.5) with scale 1, and the sum
+ * of eq. (4.6) with scale G_i */
+void orc_light_convolve(int n_det, int n_ticks, const double *in, const double *w, int n_w, const float *scale, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < n_det; ++i)
+        for (int t = 0; t < n_ticks; ++t) {
+            double acc = 0.0;
+            for (int s = 0; s < n_w && s <= t; ++s) acc += in[(size_t)i * n_ticks + t - s] * w[s];
+            out[(size_t)i * n_ticks + t] = (scale ? (double)scale[i] : 1.0) * acc;
+        }
+}
+
+/* O11  Counting statistics per time profile bin: inverse-transform-sampling Poisson below `normal_above`
+ * expected photoelectrons (30), N(lambda, sqrt(lambda)) at or above.  Reading D31: the uniforms of (sensor i, tick t) are
+ * u_k = (x_k + 0.5) 2^-32 of Philox4x32-10(counter (i, t, 0, 0x4C474854 'LGHT'), key = seed); Poisson: the smallest k with
+ * CDF(k) >= u_0 (k = 0, p = exp(-lambda), c = p; while u_0 > c: k += 1, p *= lambda / k, c += p; at most 200 steps);
+ * normal: lambda + sqrt(lambda) sqrt(-2 ln u_0) cos(2 pi u_1), not rounded, not clamped.  lambda <= 0 gives 0. */
+double orc_light_fluctuate_one(const orc_light_params *p, uint64_t seed, uint32_t det, uint32_t tick, double lambda)
+{
+    if (!(lambda > 0.0)) return 0.0;
+    uint32_t ctr[4] = { det, tick, 0u, 0x4C474854u }, key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, x[4];
+    orc_philox4x32_10(ctr, key, x);
+    const double u0 = ((double)x[0] + 0.5) * (1.0 / 4294967296.0), u1 = ((double)x[1] + 0.5) * (1.0 / 4294967296.0);
+    if (lambda < p->normal_above) {
+        int k = 0;
+        double pk = exp(-lambda), c = pk;
+        while (u0 > c && k < 200) { ++k; pk *= lambda / (double)k; c += pk; }
+        return (double)k;
+    }
+    return lambda + sqrt(lambda) * (sqrt(-2.0 * log(u0)) * cos(6.283185307179586476925286766559 * u1));
+}
+
+void orc_light_fluctuate(const orc_light_params *p, uint64_t seed, const double *isc, double *nobs)
+{
+    for (int i = 0; i < p->n_det; ++i)
+        for (int t = 0; t < p->n_ticks; ++t)
+            nobs[(size_t)i * p->n_ticks + t] = orc_light_fluctuate_one(p, seed, (uint32_t)i, (uint32_t)t, isc[(size_t)i * p->n_ticks + t]);
+}
+
+/* O12  Light read-out electronics, eq. (4.6): V_i[t] = n_i[t] + G_i sum_s N_obs,i[t - s] i_resp[s]
+ * (reading D32: the response model is sampled at the simulation tick, Delta_t_resp / delta_t = 1; it is unit-normalised
+ * by its provider).  Noise (reading D33): "random phase sinusoids with appropriate amplitudes" from a user-given spectrum:
+ * n_i[t] = sum_f A_f cos(2 pi k_f t / n_ticks + phi_if), phi_if = 2 pi u_0 of Philox(counter (i, f, 1, 'LGHT'), key = seed). */
+void orc_light_noise(const orc_light_params *p, uint64_t seed, const float *amp, const int32_t *kf, double *noise)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int i = 0; i < p->n_det; ++i) {
+        for (int t = 0; t < p->n_ticks; ++t) noise[(size_t)i * p->n_ticks + t] = 0.0;
+        for (int f = 0; f < p->n_noise; ++f) {
+            uint32_t ctr[4] = { (uint32_t)i, (uint32_t)f, 1u, 0x4C474854u }, key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, x[4];
+            orc_philox4x32_10(ctr, key, x);
+            const double phi = two_pi * (((double)x[0] + 0.5) * (1.0 / 4294967296.0));
+            for (int t = 0; t < p->n_ticks; ++t)
+                noise[(size_t)i * p->n_ticks + t] += (double)amp[f] * cos(two_pi * (double)kf[f] * (double)t / (double)p->n_ticks + phi);
         }
     }
 }

@@ -455,3 +455,76 @@ def config4(seed=None, n_segments=100_000, seg_len_cm=0.1, drift_cm=30.0, window
 
 def make_config(k: int, **kw) -> Workload:
     return (config0, config1, config2, config3, config4)[k](**kw)
+
+
+# --------------------------------------------------------------------------------------
+# Light simulation inputs: a synthetic stand-in for the Geant4-made light LUT of P:L744
+# (visibility V_i[voxel] and relative arrival-time distribution f_i[voxel][time bin] per photosensor), sensor
+# efficiencies and gains, a unit-normalised impulse response and a noise spectrum.  Inputs only, no method arithmetic.
+# --------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class LightSetup:
+    params: Dict[str, float]
+    eff: np.ndarray            # float32 [n_det] detection efficiency eps_i (eq. 4.2)
+    gain: np.ndarray           # float32 [n_det] G_i of eq. (4.6), ADC per photoelectron
+    vis: np.ndarray            # float32 [n_det][nvz][nvy][nvx] visibility V_i
+    tprof: np.ndarray          # float32 [n_det][nvz][nvy][nvx][n_lut_t], sums to 1 over the last axis
+    resp: np.ndarray           # float32 [n_resp] impulse response sampled at the tick, sums to 1
+    noise_amp: np.ndarray      # float32 [n_noise] amplitudes of the noise sinusoids (ADC)
+    noise_k: np.ndarray        # int32 [n_noise] their frequencies in cycles per waveform
+
+
+def default_light_params(**over) -> Dict[str, float]:
+    p = dict(w_ph_mev=19.5e-6, w_ion_mev=23.6e-6, tick_us=0.016, t_start_us=-0.32, n_ticks=1024, lut_m=2, n_lut_t=16,
+             vox_x0=0.0, vox_y0=0.0, vox_z0=0.0, vox_size_cm=4.0, nvx=1, nvy=1, nvz=1, n_det=8,
+             f_prompt=0.3, tau_prompt_us=0.007, tau_slow_us=1.6, trunc_tau=5.0, normal_above=30.0, n_resp=32, n_noise=0)
+    p.update(over)
+    return p
+
+
+def light_setup(wl: "Workload", n_det: int = 16, vox_cm: float = 4.0, seed: Optional[int] = None, noise: bool = False,
+                **over) -> LightSetup:
+    """Voxel grid over the bounding box of the workload's TPCs, `n_det` sensors on the box's x faces, a solid-angle-like
+    visibility that is exactly 0 beyond 1.5 m, arrival-time profiles that widen with distance."""
+    rng = np.random.Generator(np.random.PCG64((wl.seed if seed is None else seed) + 77))
+    pitch = wl.params["pixel_pitch_cm"]
+    vb = _volume_bounds(wl.tpcs, pitch)
+    x0, x1, y0, y1, z0, z1 = (float(vb[:, 0].min()), float(vb[:, 1].max()), float(vb[:, 2].min()), float(vb[:, 3].max()),
+                              float(vb[:, 4].min()), float(vb[:, 5].max()))
+    nv = [max(1, int(math.ceil((b - a) / vox_cm))) for a, b in ((x0, x1), (y0, y1), (z0, z1))]
+    ts, te = wl.segments["ts"], wl.segments["te"]
+    span = float(max(te.max(initial=0.0), ts.max(initial=0.0))) if len(ts) else 0.0
+    p = default_light_params(vox_x0=x0, vox_y0=y0, vox_z0=z0, vox_size_cm=vox_cm, nvx=nv[0], nvy=nv[1], nvz=nv[2], n_det=n_det,
+                             w_ion_mev=wl.params["w_ion_mev"], n_noise=24 if noise else 0)
+    p.update(over)
+    tail = p["trunc_tau"] * p["tau_slow_us"] + (p["n_lut_t"] * p["lut_m"] + p["n_resp"]) * p["tick_us"]
+    if "n_ticks" not in over:
+        p["n_ticks"] = int(math.ceil((span - p["t_start_us"] + tail) / p["tick_us"] / 64.0)) * 64
+    # sensors on the two x faces of the box
+    sx = np.where(np.arange(n_det) % 2 == 0, x0 - 1.0, x1 + 1.0)
+    sy = rng.uniform(y0, y1, n_det)
+    sz = rng.uniform(z0, z1, n_det)
+    cx = x0 + (np.arange(nv[0]) + 0.5) * vox_cm
+    cy = y0 + (np.arange(nv[1]) + 0.5) * vox_cm
+    cz = z0 + (np.arange(nv[2]) + 0.5) * vox_cm
+    Z, Y, X = np.meshgrid(cz, cy, cx, indexing="ij")
+    vis = np.zeros((n_det,) + Z.shape, dtype=np.float32)
+    tprof = np.zeros((n_det,) + Z.shape + (p["n_lut_t"],), dtype=np.float32)
+    b = np.arange(p["n_lut_t"], dtype=np.float64)
+    for i in range(n_det):
+        r = np.sqrt((X - sx[i]) ** 2 + (Y - sy[i]) ** 2 + (Z - sz[i]) ** 2)
+        v = 0.04 * 25.0 / (r * r + 25.0)
+        v[r > 150.0] = 0.0
+        vis[i] = v.astype(np.float32)
+        mean = 0.5 + r / 40.0                                   # later and wider with distance (scattering)
+        width = 0.6 + r / 60.0
+        f = np.exp(-0.5 * ((b[None, None, None, :] - mean[..., None]) / width[..., None]) ** 2) + 1e-3
+        tprof[i] = (f / f.sum(axis=-1, keepdims=True)).astype(np.float32)
+    eff = rng.uniform(0.002, 0.006, n_det).astype(np.float32)
+    gain = rng.uniform(8.0, 12.0, n_det).astype(np.float32)
+    k = np.arange(p["n_resp"], dtype=np.float64)
+    resp = (k + 0.5) * np.exp(-(k + 0.5) / 4.0)
+    resp = (resp / resp.sum()).astype(np.float32)
+    namp = (2.0 / (1.0 + np.arange(p["n_noise"]))).astype(np.float32)
+    nk = (3 + 7 * np.arange(p["n_noise"])).astype(np.int32)
+    return LightSetup(p, eff, gain, vis, tprof, resp, namp, nk)
