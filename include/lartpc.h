@@ -321,6 +321,65 @@ int64_t lartpc_readout_tiles(const lartpc_sim_t *sim, int tile_pixels);
 int  lartpc_pack_hits(lartpc_sim_t *sim, const lartpc_hits_t *hits, int64_t n_hits, int tile_pixels,
                       uint16_t *packed, int64_t *tile_offsets, void *stream);
 
+/* ---- light simulation (eqs. 4.1-4.6; readings D28-D33) ------------------
+ * A second workload on the same segments: photons -> photoelectrons per photosensor -> time profile -> scintillation time
+ * structure -> counting statistics -> read-out waveform.  The light look-up table (made with Geant4 in the paper)
+ * is an input: visibility V_i[voxel] and relative arrival-time distribution f_i[voxel][time bin] per photosensor i over a
+ * regular voxel grid.  All waveforms are float32 [n_det][n_ticks], tick fastest; every array argument is a DEVICE pointer
+ * unless it says host.  The light trigger (serial by construction) and the final resampling are not part of it. */
+typedef struct lartpc_light lartpc_light_t;   /* opaque: device copies of the tables, sorting scratch */
+
+typedef struct {
+    double w_ph_mev, w_ion_mev;             /* energy per photon at zero field [19.5e-6], per electron [23.6e-6] */
+    double tick_us, t_start_us;             /* simulation tick delta_t [0.016] and the time of tick 0 */
+    int    n_ticks;                         /* ticks of every waveform */
+    int    lut_m, n_lut_t;                  /* a LUT time bin spans lut_m ticks (D29); LUT time bins */
+    double vox_x0, vox_y0, vox_z0, vox_size_cm;   /* voxel grid: origin (cm) and voxel edge */
+    int    nvx, nvy, nvz, n_det;            /* voxels per axis (x fastest), photosensors */
+    double f_prompt, tau_prompt_us, tau_slow_us;  /* eq. (4.4): [0.3, 0.007, 1.6] */
+    double trunc_tau;                       /* eq. (4.5) is truncated at trunc_tau * tau_slow [5] */
+    double normal_above;                    /* Poisson below, normal at or above this many expected p.e. [30] */
+    int    n_resp, n_noise;                 /* taps of the impulse response (sampled at the tick, D32); noise sinusoids (0: none) */
+} lartpc_light_params_t;
+
+/* Copies the tables (HOST pointers): eff[n_det] (eps_i of eq. 4.2), gain[n_det] (G_i of eq. 4.6), vis[n_det][nvz][nvy][nvx],
+ * tprof[n_det][nvz][nvy][nvx][n_lut_t] (each profile sums to 1), resp[n_resp] (unit-normalised), noise_amp[n_noise] and
+ * noise_k[n_noise] (amplitude and cycles per waveform of each noise sinusoid, D33; may be NULL when n_noise = 0).
+ * LARTPC_ERR_BAD_ARGUMENT for non-positive sizes or ticks, LARTPC_ERR_DEVICE off compute capability 10.x. */
+int  lartpc_light_create(const lartpc_light_params_t *params, const float *eff_host, const float *gain_host,
+                         const float *vis_host, const float *tprof_host, const float *resp_host,
+                         const float *noise_amp_host, const int32_t *noise_k_host, lartpc_light_t **out);
+void lartpc_light_destroy(lartpc_light_t *light);
+
+/* L1, eqs. (4.1)(4.2): N_gamma,j = dE_j / W_ph - n_e,j (n_e from lartpc_quench: the same recombination as the charge,
+ * P:L736; clamped at 0), N_pe,ij = eps_i V_i[voxel of the midpoint of segment j] N_gamma,j (D28).  Out: vox[n] (voxel index,
+ * -1 outside the grid: no light), k0[n] (tick of the deposition time (ts + te) / 2), n_gamma[n], npe[n_det][n]. */
+int  lartpc_light_npe(lartpc_light_t *light, const lartpc_segments_t *seg, int64_t n, const float *n_e,
+                      int32_t *vox, int32_t *k0, float *n_gamma, float *npe, void *stream);
+
+/* L2, eq. (4.3) as read in D29: ipe[i][t] = photoelectrons reaching sensor i during tick t = sum over segments of
+ * N_pe,ij f_i[vox_j][(t - k0_j) / lut_m] / lut_m.  Segments are sorted by deposition tick first (library scratch), every
+ * (sensor, tick) then adds its contributions in a fixed order: bit-reproducible. */
+int  lartpc_light_profile(lartpc_light_t *light, int64_t n, const int32_t *vox, const int32_t *k0, const float *npe,
+                          float *ipe, void *stream);
+
+/* L3, eqs. (4.4)(4.5): isc[i][t] = sum_{s=0}^{s_max} ipe[i][t-s] w[s], w[s] = integral of f_scint over tick s (D30),
+ * s_max = floor(trunc_tau tau_slow / tick). */
+int  lartpc_light_scintillation(lartpc_light_t *light, const float *ipe, float *isc, void *stream);
+
+/* L4: nobs[i][t] = inverse-transform Poisson sample of isc[i][t] below normal_above, isc + sqrt(isc) z at or above;
+ * uniforms from Philox4x32-10(counter (i, t, 0, 'LGHT'), key = seed) (D31); decisions in float64. */
+int  lartpc_light_fluctuate(lartpc_light_t *light, uint64_t seed, const float *isc, float *nobs, void *stream);
+
+/* L5, eq. (4.6): v[i][t] = n_i[t] + G_i sum_{s=0}^{n_resp-1} nobs[i][t-s] resp[s]; noise n_i as in D33 (keyed by seed). */
+int  lartpc_light_electronics(lartpc_light_t *light, uint64_t seed, const float *nobs, float *v, void *stream);
+
+/* L1..L5 on device-resident segments; intermediates live in `workspace` (lartpc_light_workspace_bytes(light, n) bytes,
+ * LARTPC_ERR_CAPACITY if smaller).  v: float32 [n_det][n_ticks]. */
+size_t lartpc_light_workspace_bytes(const lartpc_light_t *light, int64_t n);
+int  lartpc_light_run(lartpc_light_t *light, const lartpc_segments_t *seg, int64_t n, const float *n_e, uint64_t seed,
+                      float *v, void *workspace, size_t ws_bytes, void *stream);
+
 /* ---- measurement aids ------------------------------------------------------------------------ */
 
 /* Runs an FFMA-chain microbenchmark on `stream` and returns the measured FP32 rate in TFLOP/s

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblartpc.so")
-SOURCES = ["api.cu", "stages_segment.cu", "stage_current.cu", "stages_pixel.cu"]
+SOURCES = ["api.cu", "stages_segment.cu", "stage_current.cu", "stages_pixel.cu", "light.cu"]
 HEADER = os.path.join(HERE, "..", "include", "lartpc.h")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -101,6 +101,15 @@ class Truth(C.Structure):
     _fields_ = [("k_max", C.c_int32), ("reserved", C.c_int32), ("seg", _P), ("frac", _P), ("q_signal", _P), ("n_contrib", _P)]
 
 
+class LightParams(C.Structure):
+    _fields_ = [("w_ph_mev", C.c_double), ("w_ion_mev", C.c_double), ("tick_us", C.c_double), ("t_start_us", C.c_double),
+                ("n_ticks", C.c_int), ("lut_m", C.c_int), ("n_lut_t", C.c_int),
+                ("vox_x0", C.c_double), ("vox_y0", C.c_double), ("vox_z0", C.c_double), ("vox_size_cm", C.c_double),
+                ("nvx", C.c_int), ("nvy", C.c_int), ("nvz", C.c_int), ("n_det", C.c_int),
+                ("f_prompt", C.c_double), ("tau_prompt_us", C.c_double), ("tau_slow_us", C.c_double),
+                ("trunc_tau", C.c_double), ("normal_above", C.c_double), ("n_resp", C.c_int), ("n_noise", C.c_int)]
+
+
 class Stats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n_segments", "n_active_segments", "n_tiles", "n_pairs", "n_active_pixels",
                                         "total_samples", "n_hits", "n_hits_total", "n_pixels_overflow",
@@ -113,6 +122,9 @@ EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", 
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
            "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_hit_truth", "lartpc_run_spill",
            "lartpc_readout_tiles", "lartpc_pack_hits",
+           "lartpc_light_create", "lartpc_light_destroy", "lartpc_light_npe", "lartpc_light_profile",
+           "lartpc_light_scintillation", "lartpc_light_fluctuate", "lartpc_light_electronics", "lartpc_light_workspace_bytes",
+           "lartpc_light_run",
            "lartpc_measure_fp32_peak", "lartpc_set_profiling", "lartpc_get_stage_ms", "lartpc_get_counters", "lartpc_kernel_launches",
            "lartpc_strerror")
 
@@ -131,6 +143,10 @@ def load_library():
         lib.lartpc_kernel_launches.restype = C.c_int64
         lib.lartpc_sim_destroy.restype = None
         lib.lartpc_sim_destroy.argtypes = [C.c_void_p]
+        lib.lartpc_light_destroy.restype = None
+        lib.lartpc_light_destroy.argtypes = [C.c_void_p]
+        lib.lartpc_light_workspace_bytes.restype = C.c_size_t
+        lib.lartpc_light_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
         for name in EXPORTS:
             getattr(lib, name)
         _lib = lib
@@ -421,6 +437,122 @@ class Sim:
                                          C.c_void_p(packed.data_ptr()), C.c_void_p(offs.data_ptr()), _stream_ptr(t)),
                "lartpc_pack_hits")
         return packed[:3 * n].view(n, 3), offs
+
+
+class LightSim:
+    """Owns a ``lartpc_light_t``: the light look-up table, sensor efficiencies and gains, the impulse
+    response and the noise spectrum.  Argument marshalling only; every step runs in the library's kernels."""
+
+    def __init__(self, params: Dict, eff, gain, vis, tprof, resp, noise_amp=None, noise_k=None, device: str = "cuda:0"):
+        torch = _torch()
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.lib = load_library()
+        self.params = dict(params)
+        p = LightParams()
+        for name, _ in LightParams._fields_:
+            setattr(p, name, params[name])
+        f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+        eff, gain, vis, tprof, resp = f32(eff), f32(gain), f32(vis), f32(tprof), f32(resp)
+        nd, nvox = int(params["n_det"]), int(params["nvx"]) * int(params["nvy"]) * int(params["nvz"])
+        if eff.size != nd or gain.size != nd or vis.size != nd * nvox or tprof.size != nd * nvox * int(params["n_lut_t"]) \
+                or resp.size != int(params["n_resp"]):
+            raise LartpcError("light tables do not have the sizes the parameters give")
+        nn = int(params["n_noise"])
+        amp = f32(noise_amp if nn else np.zeros(1))
+        nk = np.ascontiguousarray(noise_k if nn else np.zeros(1), dtype=np.int32)
+        if nn and (amp.size != nn or nk.size != nn):
+            raise LartpcError("noise spectrum does not have n_noise entries")
+        ptr = lambda a: a.ctypes.data_as(C.c_void_p)
+        h = C.c_void_p()
+        _check(self.lib.lartpc_light_create(C.byref(p), ptr(eff), ptr(gain), ptr(vis), ptr(tprof), ptr(resp), ptr(amp), ptr(nk),
+                                            C.byref(h)), "lartpc_light_create")
+        self.handle = h
+        self.n_det, self.n_ticks = nd, int(params["n_ticks"])
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.lartpc_light_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _empty(self, n, dtype):
+        return self.torch.empty(int(max(n, 1)), dtype=dtype, device=self.device)
+
+    def _wave(self):
+        return self.torch.empty((self.n_det, self.n_ticks), dtype=self.torch.float32, device=self.device)
+
+    def _segs(self, seg):
+        s = Segments()
+        for k in SEG_FIELDS:
+            v = seg[k]
+            if v.dtype != self.torch.float32 or not v.is_cuda or not v.is_contiguous():
+                raise LartpcError("segment field %s must be a contiguous float32 CUDA tensor" % k)
+            setattr(s, k, v.data_ptr())
+        return s, int(seg["xs"].numel())
+
+    def npe(self, seg, n_e):
+        """L1, eqs. (4.1)(4.2): dict(vox, k0, n_gamma [n], npe [n_det, n])."""
+        t = self.torch
+        s, n = self._segs(seg)
+        out = dict(vox=self._empty(n, t.int32), k0=self._empty(n, t.int32), n_gamma=self._empty(n, t.float32),
+                   npe=self._empty(self.n_det * n, t.float32))
+        _check(self.lib.lartpc_light_npe(self.handle, C.byref(s), C.c_int64(n), C.c_void_p(n_e.data_ptr()),
+                                         C.c_void_p(out["vox"].data_ptr()), C.c_void_p(out["k0"].data_ptr()),
+                                         C.c_void_p(out["n_gamma"].data_ptr()), C.c_void_p(out["npe"].data_ptr()),
+                                         _stream_ptr(t)), "lartpc_light_npe")
+        out = {k: v[:n] if k != "npe" else v[:self.n_det * n].view(self.n_det, n) for k, v in out.items()}
+        out["_n"] = n
+        return out
+
+    def profile(self, a):
+        """L2, eq. (4.3): photoelectrons per tick [n_det, n_ticks]."""
+        out = self._wave()
+        _check(self.lib.lartpc_light_profile(self.handle, C.c_int64(a["_n"]), C.c_void_p(a["vox"].data_ptr()),
+                                             C.c_void_p(a["k0"].data_ptr()), C.c_void_p(a["npe"].data_ptr()),
+                                             C.c_void_p(out.data_ptr()), _stream_ptr(self.torch)), "lartpc_light_profile")
+        return out
+
+    def scintillation(self, ipe):
+        out = self._wave()
+        _check(self.lib.lartpc_light_scintillation(self.handle, C.c_void_p(ipe.data_ptr()), C.c_void_p(out.data_ptr()),
+                                                   _stream_ptr(self.torch)), "lartpc_light_scintillation")
+        return out
+
+    def fluctuate(self, isc, seed: int):
+        out = self._wave()
+        _check(self.lib.lartpc_light_fluctuate(self.handle, C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF), C.c_void_p(isc.data_ptr()),
+                                               C.c_void_p(out.data_ptr()), _stream_ptr(self.torch)), "lartpc_light_fluctuate")
+        return out
+
+    def electronics(self, nobs, seed: int):
+        out = self._wave()
+        _check(self.lib.lartpc_light_electronics(self.handle, C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF),
+                                                 C.c_void_p(nobs.data_ptr()), C.c_void_p(out.data_ptr()),
+                                                 _stream_ptr(self.torch)), "lartpc_light_electronics")
+        return out
+
+    def workspace_bytes(self, n: int) -> int:
+        return int(self.lib.lartpc_light_workspace_bytes(self.handle, C.c_int64(int(n))))
+
+    def run(self, seg, n_e, seed: int, workspace=None):
+        """L1..L5: the read-out waveforms [n_det, n_ticks]."""
+        t = self.torch
+        s, n = self._segs(seg)
+        if workspace is None:
+            workspace = t.empty(self.workspace_bytes(n), dtype=t.uint8, device=self.device)
+        out = self._wave()
+        _check(self.lib.lartpc_light_run(self.handle, C.byref(s), C.c_int64(n), C.c_void_p(n_e.data_ptr()),
+                                         C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF), C.c_void_p(out.data_ptr()),
+                                         C.c_void_p(workspace.data_ptr()), C.c_size_t(workspace.numel()), _stream_ptr(t)),
+               "lartpc_light_run")
+        return out
 
 
 def hits_to_numpy(hits, n: Optional[int] = None):

@@ -55,7 +55,7 @@ def _header_struct_fields(name):
     ("lartpc_params_t", "Params"), ("lartpc_tpc_t", "Tpc"), ("lartpc_segments_t", "Segments"),
     ("lartpc_drifted_t", "Drifted"), ("lartpc_pixmap_t", "Pixmap"), ("lartpc_pixmap_info_t", "PixmapInfo"),
     ("lartpc_signals_t", "Signals"), ("lartpc_waveforms_t", "Waveforms"), ("lartpc_hits_t", "Hits"),
-    ("lartpc_stats_t", "Stats"), ("lartpc_truth_t", "Truth")])
+    ("lartpc_stats_t", "Stats"), ("lartpc_truth_t", "Truth"), ("lartpc_light_params_t", "LightParams")])
 def test_binding_structs_follow_the_header(cname, pyname):
     from paper_2212_09807_b200 import lartpc
     want = _header_struct_fields(cname)
