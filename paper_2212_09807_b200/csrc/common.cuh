@@ -255,4 +255,3 @@ int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t 
 int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
                        int32_t *slot_scratch, int32_t *scan_scratch, int64_t hit_base, cudaStream_t st);
 int sim_ensure_scan_tmp(lartpc_sim *sim, int64_t elems);
-int launch_list_sort(int64_t n_lists, const int32_t *start, const int32_t *count, int32_t *items, int64_t cap, cudaStream_t st);

@@ -2,8 +2,9 @@
 //
 //   L1 light_npe_kernel       thread = segment: photon yield, voxel and deposition tick (float64 index path, as S2 / S3),
 //                             N_pe for every sensor (the visibility LUT is a gather), tick histogram for the sort
-//   L2 light_profile_kernel   segments counting-sorted by deposition tick (lists sorted by segment id, so every sum below has a
-//                             fixed order); thread = (sensor, tick): adds the segments whose light reaches that tick
+//   L2 light_tick_sum_kernel  segments counting-sorted by deposition tick (lists sorted by segment id, so every sum below has a
+//      light_profile_kernel   fixed order); CTA = (sensor, deposition tick): the light of that tick's segments per LUT time bin;
+//                             thread = (sensor, tick): adds the LUT bins of the deposition ticks that reach it
 //   L3 / L5 light_conv_kernel truncated causal convolution, CTA = (sensor, 256 ticks): input window and weights in shared
 //                             memory, ascending lag; L5 also scales by the gain and adds the noise sinusoids
 //   L4 light_fluct_kernel     thread = (sensor, tick): Philox4x32-10, inverse-transform Poisson / Box-Muller normal in float64
@@ -11,6 +12,7 @@
 // sort cuts that loop to the segments inside the LUT's time span.  None of it is a dense contraction worth a tensor core at
 // the sizes of P:L778 (a 501-tap convolution of n_det x n_ticks samples is ~1e9 multiply-adds): FP32 pipe, shared memory.
 #include <math.h>
+#include <algorithm>
 #include <vector>
 #include "common.cuh"
 #include "scan.cuh"
@@ -29,9 +31,10 @@ struct lartpc_light {
     float *noise_amp = nullptr, *phase = nullptr;   int32_t *noise_k = nullptr;
     // tick sort scratch: keys k0 + span - 1 in [0, n_keys)
     int n_keys = 0;
-    int32_t *key_count = nullptr, *key_start = nullptr, *key_cursor = nullptr;
+    int32_t *key_count = nullptr, *key_offs = nullptr, *key_start = nullptr;   int64_t table_cap = 0;   // [n_keys][blocks] (+1)
     int32_t *list = nullptr;  int64_t list_cap = 0;
-    long long *scan_tmp = nullptr;  int64_t scan_tmp_elems = 0;
+    float *tick_sums = nullptr;                    // A[n_det][n_keys][n_lut_t] of light_tick_sum_kernel
+    long long *scan_tmp = nullptr;
 };
 
 namespace {
@@ -63,46 +66,84 @@ light_npe_kernel(LightDev d, SegPtrs s, int64_t n, const float *__restrict__ n_e
     (void)key_count;
 }
 
-// keys of the tick sort: segment j can reach ticks k0 .. k0 + span - 1; key = k0 + span - 1 in [0, n_ticks + span - 1)
-__global__ void __launch_bounds__(256)
-light_key_count_kernel(LightDev d, int64_t n, const int32_t *__restrict__ vox, const int32_t *__restrict__ k0, int32_t *key_count)
+// Stable counting sort of the segments by deposition tick (key = k0 + span - 1 in [0, n_keys); a segment without light or
+// whose light misses the waveform has no key): count per (key, block of SORT_B segments), exclusive scan over the
+// [key][block] table, then every segment goes to offset[key][block] + its rank among the earlier segments of its block with
+// the same key.  No order-dependent atomics: the list of a tick is in segment order, run after run.
+constexpr int SORT_T = 256, SORT_B = 2048;
+__device__ __forceinline__ int light_key(const LightDev &d, int n_keys, int vox, int k0)
 {
-    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n || vox[j] < 0) return;
-    const long long key = (long long)k0[j] + d.span - 1;
-    if (key >= 0 && key < (long long)d.n_ticks + d.span - 1) atomicAdd(&key_count[key], 1);
+    const long long key = (long long)k0 + d.span - 1;
+    return (vox >= 0 && key >= 0 && key < n_keys) ? (int)key : -1;
 }
 
-__global__ void __launch_bounds__(256)
-light_key_fill_kernel(LightDev d, int64_t n, const int32_t *__restrict__ vox, const int32_t *__restrict__ k0,
-                      const int32_t *__restrict__ key_start, int32_t *key_cursor, int32_t *list)
+__global__ void __launch_bounds__(SORT_T)
+light_key_count_kernel(LightDev d, int n_keys, int64_t n, int n_blocks, const int32_t *__restrict__ vox,
+                       const int32_t *__restrict__ k0, int32_t *count)
 {
-    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n || vox[j] < 0) return;
-    const long long key = (long long)k0[j] + d.span - 1;
-    if (key >= 0 && key < (long long)d.n_ticks + d.span - 1) list[key_start[key] + atomicAdd(&key_cursor[key], 1)] = (int32_t)j;
+    for (int q = threadIdx.x; q < SORT_B; q += SORT_T) {
+        const int64_t j = (int64_t)blockIdx.x * SORT_B + q;
+        if (j >= n) break;
+        const int key = light_key(d, n_keys, vox[j], k0[j]);
+        if (key >= 0) atomicAdd(&count[(size_t)key * n_blocks + blockIdx.x], 1);   // a counter: the order of the adds is immaterial
+    }
+}
+
+__global__ void light_key_start_kernel(int n_keys, int n_blocks, const int32_t *__restrict__ offs, int32_t *key_start)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k <= n_keys) key_start[k] = offs[(size_t)k * n_blocks];                  // offs[n_keys * n_blocks] = total
+}
+
+__global__ void __launch_bounds__(SORT_T)
+light_key_scatter_kernel(LightDev d, int n_keys, int64_t n, int n_blocks, const int32_t *__restrict__ vox,
+                         const int32_t *__restrict__ k0, const int32_t *__restrict__ offs, int32_t *list)
+{
+    __shared__ int s_key[SORT_B];
+    const int64_t base = (int64_t)blockIdx.x * SORT_B;
+    for (int q = threadIdx.x; q < SORT_B; q += SORT_T)
+        s_key[q] = base + q < n ? light_key(d, n_keys, vox[base + q], k0[base + q]) : -1;
+    __syncthreads();
+    for (int q = threadIdx.x; q < SORT_B; q += SORT_T) {
+        const int key = s_key[q];
+        if (key < 0) continue;
+        int rank = 0;
+        for (int r = 0; r < q; ++r) rank += s_key[r] == key;
+        list[offs[(size_t)key * n_blocks + blockIdx.x] + rank] = (int32_t)(base + q);
+    }
 }
 
 struct CountF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
 
-// thread = (sensor i = blockIdx.y, tick t): the segments with k0 in [t - span + 1, t], i.e. keys t .. t + span - 1, in key
-// order and, inside a key, in segment order (the lists are sorted): a fixed order of float32 additions
-__global__ void __launch_bounds__(128)
-light_profile_kernel(LightDev d, int64_t n, const int32_t *__restrict__ vox, const float *__restrict__ npe,
-                     const float *__restrict__ tprof, const int32_t *__restrict__ key_start, const int32_t *__restrict__ list,
-                     float *ipe)
+// Eq. (4.3) in two steps.  (1) CTA = (deposition tick k, sensor i): A[i][k][b] = sum over the segments of that tick of
+// N_pe,ij f_i[vox_j][b], all LUT time bins b at once (the profile of a voxel is one contiguous read).  A spill puts the 1e4
+// segments of an interaction into ONE tick, so the list is cut into contiguous chunks, one per group of P lanes (P = LUT
+// bins rounded up to a power of two; 256 threads = 256 / P groups), each summed in list order with compensated (Kahan)
+// float32 additions, the chunks then added in chunk order: a fixed order whatever the launch.  (2) thread = (sensor, tick
+// t): ipe[i][t] = sum over k0 in [t - span + 1, t] of A[i][k0][(t - k0) / lut_m] / lut_m.
+constexpr int TS_THREADS = 256;
+__global__ void __launch_bounds__(TS_THREADS)
+light_tick_sum_kernel(LightDev d, int64_t n, int P, const int32_t *__restrict__ vox, const float *__restrict__ npe,
+                      const float *__restrict__ tprof, const int32_t *__restrict__ key_start, const int32_t *__restrict__ list,
+                      float *A)
 {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
-    if (t >= d.n_ticks) return;
+    __shared__ float s_part[TS_THREADS];
+    const int key = blockIdx.x, i = blockIdx.y, tid = threadIdx.x;
+    const int e0 = key_start[key], len = key_start[key + 1] - e0;
+    float *out = A + ((size_t)i * gridDim.x + key) * d.n_lut_t;
+    if (len == 0) {                                                             // CTA-uniform
+        if (tid < d.n_lut_t) out[tid] = 0.f;
+        return;
+    }
+    const int b = tid & (P - 1), g = tid / P, n_groups = TS_THREADS / P;
+    const int chunk = (len + n_groups - 1) / n_groups;
+    const int c0 = min(g * chunk, len), c1 = min(c0 + chunk, len);
     const float *np_i = npe + (size_t)i * n;
     const float *tp_i = tprof + (size_t)i * d.nvox * d.n_lut_t;
-    // a spill puts the 1e4 segments of an interaction into one tick: compensated (Kahan) summation keeps the float32 sum
-    // within a few ulp whatever the count
     float acc = 0.f, comp = 0.f;
-    for (int key = t; key < t + d.span; ++key) {
-        const int b = (t + d.span - 1 - key) / d.lut_m;                         // LUT time bin of lag t - k0
-        const int e0 = key_start[key], e1 = key_start[key + 1];
-        for (int e = e0; e < e1; ++e) {
+    if (b < d.n_lut_t) {
+#pragma unroll 4
+        for (int e = e0 + c0; e < e0 + c1; ++e) {
             const int j = __ldg(list + e);
             const float y = __fmul_rn(__ldg(np_i + j), __ldg(tp_i + (size_t)__ldg(vox + j) * d.n_lut_t + b)) - comp;
             const float sum = __fadd_rn(acc, y);
@@ -110,6 +151,24 @@ light_profile_kernel(LightDev d, int64_t n, const int32_t *__restrict__ vox, con
             acc = sum;
         }
     }
+    s_part[tid] = acc;
+    __syncthreads();
+    if (tid < d.n_lut_t) {
+        float tot = 0.f;
+        for (int q = 0; q < n_groups; ++q) tot += s_part[q * P + tid];
+        out[tid] = tot;
+    }
+}
+
+__global__ void __launch_bounds__(128)
+light_profile_kernel(LightDev d, int n_keys, const float *__restrict__ A, float *ipe)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+    if (t >= d.n_ticks) return;
+    const float *Ai = A + (size_t)i * n_keys * d.n_lut_t;
+    float acc = 0.f;
+    for (int key = t; key < t + d.span; ++key)                                  // key = k0 + span - 1
+        acc += Ai[(size_t)key * d.n_lut_t + (t + d.span - 1 - key) / d.lut_m];
     ipe[(size_t)i * d.n_ticks + t] = acc / (float)d.lut_m;                      // photoelectrons per tick (D29)
 }
 
@@ -190,7 +249,7 @@ static void light_free(lartpc_light *l)
     if (!l) return;
     cudaFree(l->eff); cudaFree(l->gain); cudaFree(l->vis); cudaFree(l->tprof); cudaFree(l->resp); cudaFree(l->w_scint);
     cudaFree(l->noise_amp); cudaFree(l->phase); cudaFree(l->noise_k);
-    cudaFree(l->key_count); cudaFree(l->key_start); cudaFree(l->key_cursor); cudaFree(l->list); cudaFree(l->scan_tmp);
+    cudaFree(l->key_count); cudaFree(l->key_start); cudaFree(l->key_offs); cudaFree(l->list); cudaFree(l->scan_tmp); cudaFree(l->tick_sums);
     delete l;
 }
 
@@ -244,13 +303,8 @@ extern "C" int lartpc_light_create(const lartpc_light_params_t *p, const float *
     if (e == cudaSuccess) e = upload(&l->noise_amp, noise_amp, (size_t)d.n_noise);
     if (e == cudaSuccess) e = upload(&l->noise_k, noise_k, (size_t)d.n_noise);
     if (e == cudaSuccess) e = cudaMalloc(&l->phase, sizeof(float) * (size_t)(d.n_det * d.n_noise + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&l->key_count, sizeof(int32_t) * (size_t)(l->n_keys + 1));
     if (e == cudaSuccess) e = cudaMalloc(&l->key_start, sizeof(int32_t) * (size_t)(l->n_keys + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&l->key_cursor, sizeof(int32_t) * (size_t)(l->n_keys + 1));
-    if (e == cudaSuccess) {
-        l->scan_tmp_elems = lscan::tmp_elems(l->n_keys + 1);
-        e = cudaMalloc(&l->scan_tmp, sizeof(long long) * (size_t)l->scan_tmp_elems);
-    }
+    if (e == cudaSuccess) e = cudaMalloc(&l->tick_sums, sizeof(float) * (size_t)d.n_det * (size_t)l->n_keys * (size_t)d.n_lut_t);
     if (e != cudaSuccess) { lartpc_note_cuda_error(e, __FILE__, __LINE__);  light_free(l);  return LARTPC_ERR_CUDA; }
     *out = l;
     return LARTPC_OK;
@@ -292,24 +346,37 @@ extern "C" int lartpc_light_profile(lartpc_light_t *l, int64_t n, const int32_t 
         LARTPC_CUDA_TRY(cudaMalloc(&l->list, sizeof(int32_t) * (size_t)(n + n / 8 + 1024)));
         l->list_cap = n + n / 8 + 1024;
     }
-    // counting sort of the segments by deposition tick, each tick's list then sorted by segment id
-    LARTPC_CUDA_TRY(cudaMemsetAsync(l->key_count, 0, sizeof(int32_t) * (size_t)(l->n_keys + 1), st));
-    LARTPC_CUDA_TRY(cudaMemsetAsync(l->key_cursor, 0, sizeof(int32_t) * (size_t)(l->n_keys + 1), st));
+    // stable counting sort of the segments by deposition tick
+    const int n_blocks = (int)std::max<int64_t>((n + SORT_B - 1) / SORT_B, 1);
+    const int64_t table = (int64_t)l->n_keys * n_blocks;
+    if (table + 1 >= (1ll << 31)) return LARTPC_ERR_UNSUPPORTED;
+    if (table + 1 > l->table_cap) {
+        cudaFree(l->key_count);  cudaFree(l->key_offs);  cudaFree(l->scan_tmp);
+        l->key_count = l->key_offs = nullptr;  l->scan_tmp = nullptr;  l->table_cap = 0;
+        LARTPC_CUDA_TRY(cudaMalloc(&l->key_count, sizeof(int32_t) * (size_t)(table + 1)));
+        LARTPC_CUDA_TRY(cudaMalloc(&l->key_offs, sizeof(int32_t) * (size_t)(table + 1)));
+        LARTPC_CUDA_TRY(cudaMalloc(&l->scan_tmp, sizeof(long long) * (size_t)lscan::tmp_elems(table + 1)));
+        l->table_cap = table + 1;
+    }
+    LARTPC_CUDA_TRY(cudaMemsetAsync(l->key_count, 0, sizeof(int32_t) * (size_t)(table + 1), st));
     if (n > 0) {
         ++g_lartpc_launches;
-        light_key_count_kernel<<<div_up(n, 256), 256, 0, st>>>(d, n, vox, k0, l->key_count);
+        light_key_count_kernel<<<n_blocks, SORT_T, 0, st>>>(d, l->n_keys, n, n_blocks, vox, k0, l->key_count);
     }
-    LARTPC_CUDA_TRY(lscan::exclusive_scan(l->n_keys, CountF{l->key_count}, l->key_start, true, (long long *)nullptr,
-                                          l->scan_tmp, st));
-    if (n > 0) {
-        ++g_lartpc_launches;
-        light_key_fill_kernel<<<div_up(n, 256), 256, 0, st>>>(d, n, vox, k0, l->key_start, l->key_cursor, l->list);
-        int rc = launch_list_sort(l->n_keys, l->key_start, l->key_count, l->list, l->list_cap, st);
-        if (rc) return rc;
-    }
+    LARTPC_CUDA_TRY(lscan::exclusive_scan(table, CountF{l->key_count}, l->key_offs, true, (long long *)nullptr, l->scan_tmp, st));
     ++g_lartpc_launches;
-    light_profile_kernel<<<dim3((unsigned)div_up(d.n_ticks, 128), (unsigned)d.n_det), 128, 0, st>>>(
-        d, n, vox, npe, l->tprof, l->key_start, l->list, ipe);
+    light_key_start_kernel<<<div_up(l->n_keys + 1, 256), 256, 0, st>>>(l->n_keys, n_blocks, l->key_offs, l->key_start);
+    if (n > 0) {
+        ++g_lartpc_launches;
+        light_key_scatter_kernel<<<n_blocks, SORT_T, 0, st>>>(d, l->n_keys, n, n_blocks, vox, k0, l->key_offs, l->list);
+    }
+    int P = 1;
+    while (P < d.n_lut_t) P <<= 1;
+    if (P > TS_THREADS) return LARTPC_ERR_UNSUPPORTED;
+    g_lartpc_launches += 2;
+    light_tick_sum_kernel<<<dim3((unsigned)l->n_keys, (unsigned)d.n_det), TS_THREADS, 0, st>>>(
+        d, n, P, vox, npe, l->tprof, l->key_start, l->list, l->tick_sums);
+    light_profile_kernel<<<dim3((unsigned)div_up(d.n_ticks, 128), (unsigned)d.n_det), 128, 0, st>>>(d, l->n_keys, l->tick_sums, ipe);
     LARTPC_CUDA_TRY(cudaGetLastError());
     return LARTPC_OK;
 }

@@ -347,17 +347,6 @@ pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int3
         }
 }
 
-// sorts each of n_lists lists of int32 items (list k = items[start[k] .. start[k] + count[k])) in place, one warp per list:
-// the plan's per-pixel segment lists, and the light simulation's per-tick lists (light.cu)
-int launch_list_sort(int64_t n_lists, const int32_t *start, const int32_t *count, int32_t *items, int64_t cap, cudaStream_t st)
-{
-    if (n_lists <= 0) return LARTPC_OK;
-    ++g_lartpc_launches;
-    pair_sort_kernel<<<div_up(n_lists, 4), 128, 0, st>>>(n_lists, start, count, items, cap);
-    LARTPC_CUDA_TRY(cudaGetLastError());
-    return LARTPC_OK;
-}
-
 // one thread per charged-pixel grid cell: emit its tiles (one per window that holds charge) and mark the pixels
 // they can reach
 __global__ void __launch_bounds__(256)

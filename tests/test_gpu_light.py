@@ -34,7 +34,9 @@ def _gpu_stages(lartpc, wl, ls, seed):
     nobs = light.fluctuate(isc, seed)
     v = light.electronics(nobs, seed)
     v_run = light.run(seg, ne, seed)
+    v_again = light.run(seg, ne, seed)
     torch.cuda.synchronize()
+    assert torch.equal(v_run, v_again)                              # fixed summation order: bit-identical from run to run
     out = dict(vox=a["vox"].cpu().numpy(), k0=a["k0"].cpu().numpy(), n_gamma=a["n_gamma"].cpu().numpy(),
                npe=a["npe"].cpu().numpy(), ipe=ipe.cpu().numpy(), isc=isc.cpu().numpy(), nobs=nobs.cpu().numpy(),
                v=v.cpu().numpy(), v_run=v_run.cpu().numpy(), n_e=ne.cpu().numpy())
