@@ -6,6 +6,7 @@ synthetic spill.  Metric (BASELINE.json): segments/s (whole job) with ms/spill a
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
   python bench.py --config 4            BASELINE configs[4]: the induced-current sweep (S4 + S5 only), one JSON line
+  python bench.py --light [--config k]  the light simulation on that config's segments, one JSON line
 
 * `value`     segments/s with the segment arrays already resident in HBM (device-timed, CUDA events).
 * `e2e`       same metric through the C-ABI with HOST (pinned) segment arrays: host->device copy of the nine
@@ -61,6 +62,9 @@ def parse_args():
     ap.add_argument("--segments", type=int, default=None, help="override the segment target of configs 2/3")
     ap.add_argument("--response", default="auto", choices=["auto", "tensor", "ffma"],
                     help="S4 response path: tcgen05 tensor cores or the FP32-pipe FFMA2 kernel")
+    ap.add_argument("--light", action="store_true",
+                    help="time the light simulation (SURVEY 8(f) NEXT-3, eqs. 4.1-4.6) on the chosen config's segments instead")
+    ap.add_argument("--light-sensors", type=int, default=None, help="photosensors of the --light run (default 64 at config 3, else 16)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=1000, help="segments in the oracle's bounded sample")
     return ap.parse_args()
@@ -535,10 +539,119 @@ def run_sweep(args):
     print(json.dumps(line))
 
 
+def run_light(args):
+    """Light simulation (NEXT-3) on the segments of configs[0..3]: S1 (recombination, shared with the charge path) and
+    L1-L5 per step; stage times from the staged calls, step time from lartpc_light_run; one JSON line."""
+    import torch
+    from paper_2212_09807_b200 import lartpc
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: the light path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    wl = make_workload(args.config, 0, args.segments)
+    n = wl.n_segments
+    n_det = args.light_sensors or (64 if args.config == 3 else 16)
+    ls = workloads.light_setup(wl, n_det=n_det, vox_cm=8.0 if args.config == 3 else 4.0, noise=True)
+    lp = ls.params
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    light = lartpc.LightSim(lp, ls.eff, ls.gain, ls.vis, ls.tprof, ls.resp, ls.noise_amp, ls.noise_k)
+    host = {k: torch.from_numpy(np.ascontiguousarray(wl.segments[k], dtype=np.float32)).pin_memory() for k in workloads.SEG_FIELDS}
+    seg = {k: v.to(dev) for k, v in host.items()}
+    ws = torch.empty(light.workspace_bytes(n), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    names = ("quench", "npe", "profile", "scintillation", "fluctuate", "electronics")
+    launches0 = lartpc.kernel_launches()
+
+    def staged():
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(7)]
+        e[0].record(); _, ne = sim.quench(seg)
+        e[1].record(); a = light.npe(seg, ne)
+        e[2].record(); ipe = light.profile(a)
+        e[3].record(); isc = light.scintillation(ipe)
+        e[4].record(); nobs = light.fluctuate(isc, wl.seed)
+        e[5].record(); v = light.electronics(nobs, wl.seed)
+        e[6].record()
+        torch.cuda.synchronize()
+        return [e[k].elapsed_time(e[k + 1]) for k in range(6)], ipe
+
+    for _ in range(args.warmup):
+        flush.zero_(); staged()
+    clocks = ClockSampler(0)
+    clocks.start()
+    per, steps = [], []
+    for _ in range(args.steps):
+        flush.zero_()
+        t, ipe = staged()
+        per.append(t)
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _, ne = sim.quench(seg)
+        v = light.run(seg, ne, wl.seed, workspace=ws)
+        e1.record()
+        torch.cuda.synchronize()
+        steps.append(e0.elapsed_time(e1))
+    clk = clocks.stop()
+    # end to end: pinned host segments in, pinned host waveforms out
+    dseg = {k: torch.empty_like(v_) for k, v_ in seg.items()}
+    hv = torch.empty((n_det, int(lp["n_ticks"])), dtype=torch.float32).pin_memory()
+
+    def e2e_step():
+        for k, v_ in host.items():
+            dseg[k].copy_(v_, non_blocking=True)
+        _, ne_ = sim.quench(dseg)
+        hv.copy_(light.run(dseg, ne_, wl.seed, workspace=ws), non_blocking=True)
+        torch.cuda.synchronize()
+
+    e2e_step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
+    mp = {}
+    try:
+        mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm = float(mp.get("hbm_gbs", 6650.0))
+    fp32 = lartpc.measure_fp32_peak(0)
+    med = {k: float(np.median([p_[i] for p_ in per])) for i, k in enumerate(names)}
+    ms = float(np.median(steps))
+    n_t, n_sc, n_rs, n_lt = int(lp["n_ticks"]), int(lp["trunc_tau"] * lp["tau_slow_us"] / lp["tick_us"]) + 1, int(lp["n_resp"]), int(lp["n_lut_t"])
+    npe_bytes = n * (36.0 + 4.0 + 12.0 + 4.0 * n_det)
+    prof_bytes = n * (8.0 + n_det * (4.0 + 4.0 * n_lt))                # ids / voxels once, per sensor N_pe and one LUT profile (L2 gathers)
+    rooflines = [
+        {"kernel": "light_npe_kernel (L1)", "bound": "hbm", "ms_per_step": med["npe"], "moved_bytes_per_step": npe_bytes,
+         "achieved": npe_bytes / (med["npe"] * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s", "frac": npe_bytes / (med["npe"] * 1e-3) / 1e9 / hbm},
+        {"kernel": "tick sort + light_tick_sum_kernel + light_profile_kernel (L2)", "bound": "hbm", "ms_per_step": med["profile"],
+         "moved_bytes_per_step": prof_bytes, "achieved": prof_bytes / (med["profile"] * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+         "frac": prof_bytes / (med["profile"] * 1e-3) / 1e9 / hbm,
+         "note": "bytes the sums read: N_pe once per sensor, one LUT time profile per (sensor, segment) through L2"},
+        {"kernel": "light_conv_kernel, scintillation (L3)", "bound": "alu", "ms_per_step": med["scintillation"],
+         "achieved": 2.0 * n_det * n_t * n_sc / (med["scintillation"] * 1e-3) / 1e12, "peak": fp32, "unit": "TFLOP/s",
+         "frac": 2.0 * n_det * n_t * n_sc / (med["scintillation"] * 1e-3) / 1e12 / fp32},
+        {"kernel": "light_conv_kernel, read-out (L5)", "bound": "alu", "ms_per_step": med["electronics"],
+         "achieved": 2.0 * n_det * n_t * n_rs / (med["electronics"] * 1e-3) / 1e12, "peak": fp32, "unit": "TFLOP/s",
+         "frac": 2.0 * n_det * n_t * n_rs / (med["electronics"] * 1e-3) / 1e12 / fp32},
+    ]
+    print(json.dumps({
+        "metric": "segments/s through the light simulation (S1 + eqs. 4.1-4.6; ms per spill in ms_per_step)", "value": n / (ms * 1e-3),
+        "unit": "segments/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 (float64 where an integer is decided)", "data": "synthetic",
+        "config": {"workload": WORKLOAD_NAMES[args.config] + "; light: %d photosensors, %d ticks of %g ns, synthetic light LUT of "
+                   "%d voxels x %d time bins" % (n_det, n_t, 1e3 * lp["tick_us"], ls.vis[0].size, n_lt),
+                   "n_segments": n, "l2": "256 MiB flush write between timed steps"},
+        "stage_ms_per_step": med, "rooflines": rooflines,
+        "e2e": {"value": n / (e2e_ms * 1e-3), "unit": "segments/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": 36 * n,
+                "d2h_bytes_per_step": 4 * n_det * n_t},
+        "photoelectrons": float(ipe.sum().item()), "clocks": clk, "gpu_launches": int(lartpc.kernel_launches() - launches0)}))
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.light:
+        run_light(args)
     elif args.config == 4:
         run_sweep(args)
     else:
