@@ -50,6 +50,12 @@ WORKLOAD_NAMES = {
 }
 
 
+# DRAM bytes per spill of the tensor-core response measured with ncu on the benched workload and launch configuration
+# (profiles/r2_traffic_c3.md: dram__bytes_read.sum + dram__bytes_write.sum over the 4 launches of one configs[3] spill),
+# keyed by (config, n_segments, n_tiles); any other workload reports the byte model of the plan instead and says so
+MEASURED_RESPONSE_TRAFFIC = {(3, 4805366, 3113102): 57788171776.0 + 82028080640.0}
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -379,10 +385,15 @@ def run_ours(args):
                                      "(an fp8 K = 32 instruction occupies the pipe like an fp16 K = 16 one)",
                     "smem_fill_gbs": cnt["response_bytes_to_smem"] / t_rs / 1e9 if t_rs > 0 else None,
                     "fp32_alu_peak": max(peak_scalar, peak_packed), "peak_source": peak_src,
-                    "traffic": dram,
-                    "traffic_note": "DRAM bytes per launch from the plan and the kernel's counters: charged A blocks read once "
-                                    "(the 25 target rows of a unit stream them at the same time through L2), partial rows "
-                                    "written, LUT image once; profiles/ holds the ncu dram__bytes capture it is checked against"}
+                    "traffic": None, "traffic_model": dram,
+                    "traffic_note": "traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu capture "
+                                    "of this workload (profiles/r2_traffic_c3.md), null for a workload without one; "
+                                    "traffic_model: bytes per launch from the plan and the kernel's counters (charged "
+                                    "operand blocks read once, partial rows written, LUT image once): 0.84 of the measured "
+                                    "figure at configs[3]"}
+            meas = MEASURED_RESPONSE_TRAFFIC.get((args.config, int(n), int(n_tiles)))
+            if meas is not None:
+                roof["traffic"] = meas / max(n_launch["induced_current_response"], 1)
         else:
             peak = max(peak_scalar, peak_packed)
             roof = {"kernel": "response_kernel (S4 induced current, response on the FP32 pipe)", "bound": "alu",
