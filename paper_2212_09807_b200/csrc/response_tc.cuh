@@ -66,10 +66,15 @@ struct Args {
                                    // CTAs that stream one tile block stay together however long the launch runs
 };
 
-// A image: [tile block][bin c][16-tick block b][fp16 part | fp8 part][128 rows x 32 bytes], each part a canonical
-// un-swizzled K-major operand of one MMA (row r = tile in block; 16-byte K chunks 128 B apart, 8-row groups 256 B apart),
-// so that a stage copies only the 16-tick blocks that hold charge.  Byte offset of K chunk kc (0 / 1) of row r in a part:
-__host__ __device__ __forceinline__ int a_part_offset(int r, int kc) { return (r >> 3) * 256 + kc * 128 + (r & 7) * 16; }
+// A image: [tile block][bin c][16-tick block b][fp16 part | fp8 part][128 rows x 32 bytes], each part a K-major operand of
+// one MMA in the 32-byte-swizzle canonical layout (row r = tile in block; a row's 32 bytes are contiguous, 8-row groups
+// 256 B apart), so that a stage copies only the 16-tick blocks that hold charge AND a tile's row is a whole 32-byte DRAM
+// sector: with the un-swizzled layout (16-byte pieces, two rows per sector, written by different CTAs at different times)
+// the charge lattice wrote every sector twice and read it back once in between (profiles/r2_traffic_c3.md).
+// Byte offset of K chunk kc (0 / 1) of row r in a part:
+// (32-byte swizzle atom: 8 rows x 32 bytes, the two 16-byte K chunks of rows 4-7 swapped -- address bit 7 XORed into bit 4)
+__host__ __device__ __forceinline__ int a_part_offset(int r, int kc) { return (r >> 3) * 256 + (r & 7) * 32 + ((kc ^ ((r >> 2) & 1)) * 16); }
+constexpr uint32_t A_LAYOUT = 6;                        // UMMA descriptor layout type SWIZZLE_32B
 constexpr int A_PART_BYTES = 128 * 32;                 // one part of one block: 4 KB
 constexpr int A_BLOCK_BYTES = 2 * A_PART_BYTES;        // fp16 part + fp8 part
 // canonical un-swizzled K-major image of Bs: row n' (output column), element jj: 8 x 16-byte core matrices,
@@ -536,8 +541,8 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                     if (!(mask >> b & 1)) continue;                    // no tile of the unit has charge in these 16 ticks
                     if ((b & 1) == par) {
                         const uint32_t dcol = tmem + (b & 1 ? ACC_COL : 0) + 32 * (b >> 1);
-                        tc_mma<CTA2>(false, dcol, smem_desc(src, 128, 256, 0), bd16, idesc);
-                        tc_mma<CTA2>(true, dcol, smem_desc(src + A_PART_BYTES, 128, 256, 0), bd8, idesc);
+                        tc_mma<CTA2>(false, dcol, smem_desc(src, 16, 256, A_LAYOUT), bd16, idesc);
+                        tc_mma<CTA2>(true, dcol, smem_desc(src + A_PART_BYTES, 16, 256, A_LAYOUT), bd8, idesc);
                     }
                     src += A_BLOCK_BYTES;
                 }

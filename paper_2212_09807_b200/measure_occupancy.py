@@ -39,9 +39,9 @@ def main(cfg: int) -> None:
     nt, nb2 = int(info.n_tiles), int(wl.params["bins_per_pixel"]) ** 2
     nu = (nt + 127) // 128
     ch = sig["charge"].view(torch.uint8)
-    # fp16 part of the image: [unit, bin, block, part 0, 8-row group, K chunk, row in group, 16 bytes]
-    img = ch[: nu * nb2 * 4 * 8192].view(nu, nb2, 4, 2, 16, 2, 8, 16)[:, :, :, 0]
-    nzr = (img != 0).any(dim=-1).any(dim=4).reshape(nu, nb2, 4, 128)          # [unit, bin, block, tile row]
+    # fp16 part of the image: [unit, bin, block, part 0, 8-row group, row in group, 32 bytes]
+    img = ch[: nu * nb2 * 4 * 8192].view(nu, nb2, 4, 2, 16, 8, 32)[:, :, :, 0]
+    nzr = (img != 0).any(dim=-1).reshape(nu, nb2, 4, 128)                     # [unit, bin, block, tile row]
     unit_blk = nzr.any(dim=3).any(dim=1)
     union = nzr.any(dim=3)
     tile_blk = nzr.any(dim=1)
