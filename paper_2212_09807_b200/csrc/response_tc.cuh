@@ -91,6 +91,12 @@ __host__ __device__ __forceinline__ int b8_image_offset(int n, int kb)
     return (n >> 3) * 256 + (kb >> 4) * 128 + (n & 7) * 16 + (kb & 15);
 }
 
+__device__ __forceinline__ void st_global_256(void *p, const uint4 &a, const uint4 &b)     // 32-byte aligned
+{
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w) : "memory");
+}
+
 // Writes 16 consecutive arrival ticks (one block b) of row r of one bin's A operand: x = C 2^-e, |x| < 2^15.
 // blk: start of that (bin, block) in the image (A_BLOCK_BYTES).  fp16 part: ticks 0-7 | 8-15; fp8 part: lo8 | hi8.
 __device__ __forceinline__ void store_a_block16(unsigned char *blk, int r, const float (&x)[16])
@@ -105,11 +111,11 @@ __device__ __forceinline__ void store_a_block16(unsigned char *blk, int r, const
         l8[i] = __nv_cvt_float2_to_fp8x2(make_float2((x[2 * i] - f.x) * sa, (x[2 * i + 1] - f.y) * sa), __NV_SATFINITE, __NV_E4M3);
         h8[i] = __nv_cvt_float2_to_fp8x2(make_float2(x[2 * i] * sb, x[2 * i + 1] * sb), __NV_SATFINITE, __NV_E4M3);
     }
-    const int o0 = a_part_offset(r, 0), o1 = a_part_offset(r, 1);
-    *(uint4 *)(blk + o0) = *(const uint4 *)&h[0];
-    *(uint4 *)(blk + o1) = *(const uint4 *)&h[4];
-    *(uint4 *)(blk + A_PART_BYTES + o0) = *(const uint4 *)l8;
-    *(uint4 *)(blk + A_PART_BYTES + o1) = *(const uint4 *)h8;
+    // a row of a part is one 32-byte sector: one 256-bit store each (the two K chunks swapped in rows 4-7 of an atom)
+    const bool sw = (r >> 2) & 1;
+    const uint4 c0 = *(const uint4 *)&h[0], c1 = *(const uint4 *)&h[4], d0 = *(const uint4 *)l8, d1 = *(const uint4 *)h8;
+    st_global_256(blk + a_part_offset(r, sw ? 1 : 0), sw ? c1 : c0, sw ? c0 : c1);
+    st_global_256(blk + A_PART_BYTES + a_part_offset(r, sw ? 1 : 0), sw ? d1 : d0, sw ? d0 : d1);
 }
 
 __device__ __forceinline__ uint32_t s32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
