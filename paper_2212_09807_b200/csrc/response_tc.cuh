@@ -198,12 +198,12 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8])
         : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
         : "r"(taddr) : "memory");
 }
-__device__ __forceinline__ void tmem_zero16(uint32_t taddr)
+__device__ __forceinline__ void tmem_zero64(uint32_t taddr)
 {
     const uint32_t z = 0u;
     asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
-        "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};\n" ::"r"(taddr), "r"(z) : "memory");
+        "tcgen05.st.sync.aligned.32x32b.x64.b32 [%0], "
+        "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};\n" ::"r"(taddr), "r"(z) : "memory");
 }
 
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
@@ -566,7 +566,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
         const uint32_t tlane = tmem + ((uint32_t)(32 * quad) << 16);
         const uint32_t lead_tempty = CTA2 ? mapa(tempty, 0u) : tempty;
         // every MMA accumulates: the accumulators are zero before the first item and zeroed again after each read-out
-        for (int c0 = 0; c0 < 512; c0 += 16) tmem_zero16(tlane + c0);
+        for (int c0 = 0; c0 < 512; c0 += 64) tmem_zero64(tlane + c0);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         tc_fence_before();
         __syncwarp();
@@ -614,24 +614,27 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 if (live) {
                     const int nv = min(16, a.tile_ticks - n0);         // tile_ticks is a multiple of 8
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        if (4 * i >= nv) break;
-                        const float be = (i < 2 ? g0e : g1e) * scale, bo = (i < 2 ? g0o : g1o) * scale;   // value at the 8-tick node
-                        const float se = (i < 2 ? g1e - g0e : g2e - g1e) * (0.125f * scale), so = (i < 2 ? g1o - g0o : g2o - g1o) * (0.125f * scale);
-                        float r[4];
+                    for (int i8 = 0; i8 < 2; ++i8) {                   // 8 ticks = one 32-byte sector of the row per store
+                        if (8 * i8 >= nv) break;
+                        const float be = (i8 == 0 ? g0e : g1e) * scale, bo = (i8 == 0 ? g0o : g1o) * scale;   // value at the 8-tick node
+                        const float se = (i8 == 0 ? g1e - g0e : g2e - g1e) * (0.125f * scale), so = (i8 == 0 ? g1o - g0o : g2o - g1o) * (0.125f * scale);
+                        float r[8];
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) {
-                            const float t = (float)((4 * i + k) & 7);
-                            const float x0 = has0 ? __uint_as_float(v0[4 * i + k]) : 0.f, x1 = has1 ? __uint_as_float(v1[4 * i + k]) : 0.f;
+                        for (int k = 0; k < 8; ++k) {
+                            const float t = (float)k;
+                            const float x0 = has0 ? __uint_as_float(v0[8 * i8 + k]) : 0.f, x1 = has1 ? __uint_as_float(v1[8 * i8 + k]) : 0.f;
                             r[k] = fmaf(x0, fmaf(se, t, be), x1 * fmaf(so, t, bo));
                         }
-                        __stcs((float4 *)(dst + n0) + i, make_float4(r[0], r[1], r[2], r[3]));
+                        // one 256-bit store per 8 ticks: each lane writes its own row, so the store path sees 32 sectors per
+                        // instruction either way, and half as many instructions (response 175 -> 167 ms at configs[3])
+                        st_global_256(dst + n0 + 8 * i8, make_uint4(__float_as_uint(r[0]), __float_as_uint(r[1]), __float_as_uint(r[2]), __float_as_uint(r[3])),
+                                      make_uint4(__float_as_uint(r[4]), __float_as_uint(r[5]), __float_as_uint(r[6]), __float_as_uint(r[7])));
                     }
                 }
                 g0e = g2e;  g0o = g2o;
             }
-            if (even) for (int c0 = 0; c0 < ACC_COL; c0 += 16) tmem_zero16(tlane + c0);
-            if (odd) for (int c0 = ACC_COL; c0 < 2 * ACC_COL; c0 += 16) tmem_zero16(tlane + c0);
+            if (even) for (int c0 = 0; c0 < ACC_COL; c0 += 64) tmem_zero64(tlane + c0);
+            if (odd) for (int c0 = ACC_COL; c0 < 2 * ACC_COL; c0 += 64) tmem_zero64(tlane + c0);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();
