@@ -26,7 +26,8 @@ struct __align__(16) SegRec {
     float isT, ist, qa, rho;            // 1 / (sqrt 2 sigma) in bins and ticks, Q_a, extent over sigma (node-rule choice)
     int N, a_lo, a_hi, b_lo, b_hi, jt0, jt1, flags;   // flags: segment id << 1 | (sigma = 0)
 };
-static_assert(sizeof(SegRec) == 96, "SegRec is six 16-byte chunks");
+static_assert(sizeof(SegRec) == SEG_REC_BYTES && offsetof(SegRec, N) == SEG_REC_BOX_OFFSET && offsetof(SegRec, jt1) == SEG_REC_BOX_OFFSET + 24,
+              "SegRec is six 16-byte chunks; the plan's tile classes read its last two (common.cuh)");
 constexpr int CT_CTL = 1024;                           // barriers, scratch, tile ring, prefetched ids
 constexpr int CT_SMEM = 2 * CT_A_HALF + 2 * CT_B_HALF + 128 + CT_CTL + sizeof(SegLocal) * SEGCAP + sizeof(SegRec) * SEGCAP;
 

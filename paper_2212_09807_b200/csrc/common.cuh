@@ -71,6 +71,8 @@ constexpr bool TC_CTA_PAIR = false;  // the tensor-core response runs as CTA pai
 constexpr int TC_UNIT_TILES = TC_CTA_PAIR ? 2 * TC_TILE_BLOCK : TC_TILE_BLOCK;   // tiles one response item multiplies at once:
                                      // the 16-tick block masks (tb_mask) are kept per unit
 
+constexpr int SEG_REC_BYTES = 96, SEG_REC_BOX_OFFSET = 64;   // per-segment record of the tensor-core splat (charge_tc.cuh SegRec):
+                                     // its last 32 bytes are the ints {N, a_lo, a_hi, b_lo, b_hi, jt0, jt1, flags}
 constexpr int TC_BOXQ = 5;           // tile sort: classes per edge of the box of charged bins (bins 0-1, 2-3, .. 8-9 for 10 bins per pixel)
 constexpr int TC_BOX_CLASSES = TC_BOXQ * TC_BOXQ * TC_BOXQ * TC_BOXQ;
 constexpr int TC_CLASSES = 16 * TC_BOX_CLASSES;     // (16-tick block mask, box class)

@@ -461,7 +461,8 @@ int sim_grow_tiles(lartpc_sim *sim, int64_t cap)
 
 __global__ void __launch_bounds__(256)
 tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td, const int2 *__restrict__ tl,
-                  const int32_t *__restrict__ pair_seg, lartpc_pixmap_t pm, int32_t *cls, int32_t *hist, int sort)
+                  const int32_t *__restrict__ pair_seg, lartpc_pixmap_t pm, const void *__restrict__ seg_rec, int32_t *cls,
+                  int32_t *hist, int sort)
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int c = TC_CLASSES;                                               // no tile (a group of its own below)
@@ -474,11 +475,21 @@ tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td,
             const int A_t = d.px * p.nb, B_t = d.py * p.nb;
             for (int k = 0; k < l.y; ++k) {
                 const int s = pair_seg[l.x + k];
-                const int jlo = max(max(pm.jt0[s], 0) - d.j_start, 0), jhi = min(min(pm.jt1[s], p.j_max) - d.j_start, p.Jc - 1);
+                // the segment's boxes: one 32-byte sector of its record (SEG_REC_BYTES / SEG_REC_BOX_OFFSET: the eight ints
+                // {N, a_lo, a_hi, b_lo | b_hi, jt0, jt1, flags} that end the record seg_record_kernel wrote), not six arrays
+                int s_alo, s_ahi, s_blo, s_bhi, s_jt0, s_jt1;
+                if (seg_rec) {
+                    const int4 *r = (const int4 *)((const char *)seg_rec + (size_t)SEG_REC_BYTES * s + SEG_REC_BOX_OFFSET);
+                    const int4 r0 = __ldg(r), r1 = __ldg(r + 1);
+                    s_alo = r0.y;  s_ahi = r0.z;  s_blo = r0.w;  s_bhi = r1.x;  s_jt0 = r1.y;  s_jt1 = r1.z;
+                } else {
+                    s_alo = pm.a_lo[s];  s_ahi = pm.a_hi[s];  s_blo = pm.b_lo[s];  s_bhi = pm.b_hi[s];  s_jt0 = pm.jt0[s];  s_jt1 = pm.jt1[s];
+                }
+                const int jlo = max(max(s_jt0, 0) - d.j_start, 0), jhi = min(min(s_jt1, p.j_max) - d.j_start, p.Jc - 1);
                 if (jlo > jhi) continue;                              // the segment charges another window of this pixel
                 mask |= ((2 << (jhi >> 4)) - 1) & ~((1 << (jlo >> 4)) - 1);
-                alo = min(alo, max(pm.a_lo[s] - A_t, 0));  ahi = max(ahi, min(pm.a_hi[s] - A_t, p.nb - 1));
-                blo = min(blo, max(pm.b_lo[s] - B_t, 0));  bhi = max(bhi, min(pm.b_hi[s] - B_t, p.nb - 1));
+                alo = min(alo, max(s_alo - A_t, 0));  ahi = max(ahi, min(s_ahi - A_t, p.nb - 1));
+                blo = min(blo, max(s_blo - B_t, 0));  bhi = max(bhi, min(s_bhi - B_t, p.nb - 1));
             }
         }
         // edges in TC_BOXQ steps over the pixel (any bins_per_pixel); an empty box sorts first
@@ -642,6 +653,7 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->tb_mask, 0, sizeof(int32_t) * (nt / TC_TILE_BLOCK + 1), st));
         g_lartpc_launches += 3;
         tile_class_kernel<<<div_up(nt, 256), 256, 0, st>>>(p, nt, sim->tile_desc, sim->tile_list, sim->pair_seg, *out,
+                                                          (sort && sim->seg_rec_cap >= n) ? sim->seg_rec : nullptr,
                                                           sim->tile_perm, sim->cls_hist, sort);
         class_offsets_kernel<<<1, 1024, 0, st>>>(sim->cls_hist);
         tile_scatter_kernel<<<div_up(nt, 256), 256, 0, st>>>(nt, sim->tile_perm, sim->cls_hist, sim->tile_desc,
