@@ -199,11 +199,13 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
     TileDesc *s_td = (TileDesc *)(ctl + 256);                        // [3] their descriptors
     int2 *s_tl = (int2 *)(ctl + 304);                                // [3] their segment lists {start, count}
     int *s_pid = (int *)(ctl + 336);                                 // [SEGCAP] segment ids of the next tile's first chunk
+    unsigned long long *s_cnt = (unsigned long long *)(ctl + 480);   // [3] this CTA's work counters, added to the global ones once
     SegLocal *segs = (SegLocal *)(ctl + CT_CTL);
     SegRec *s_rec = (SegRec *)(ctl + CT_CTL + sizeof(SegLocal) * SEGCAP);   // records of the next tile's first chunk
     const SegRec *rec = (const SegRec *)a.rec;
 
     if (tid == 0) {
+        s_cnt[0] = s_cnt[1] = s_cnt[2] = 0ull;
         rtc::mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         const int q0 = atomicAdd(a.work, 1), q1 = atomicAdd(a.work, 1), q2 = atomicAdd(a.work, 1);
@@ -297,8 +299,8 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             }
             const int total = pre[nseg];
             if (tid == 0 && total) {
-                atomicAdd(a.fma_counter + 3, (unsigned long long)total);
-                atomicAdd(a.fma_counter + 4, 3ull * (unsigned long long)((total + 15) / 16));   // hi hi + hi lo + lo hi per 16 columns
+                s_cnt[1] += (unsigned long long)total;                               // (thread 0 alone writes these two)
+                s_cnt[2] += 3ull * (unsigned long long)((total + 15) / 16);         // hi hi + hi lo + lo hi per 16 columns
             }
             for (int s0 = 0; s0 < total; s0 += CT_KB) {
                 const int nsb = min(CT_KB, total - s0), nk16 = (nsb + 15) >> 4;
@@ -494,7 +496,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                     const DevTpc &tp = a.tpcs[td.tpc];
                     const int vx = min(td.px + p.H, tp.nx - 1) - max(td.px - p.H, 0) + 1;
                     const int vy = min(td.py + p.H, tp.ny - 1) - max(td.py - p.H, 0) + 1;
-                    if (vx > 0 && vy > 0) atomicAdd(a.fma_counter, (unsigned long long)nz * (unsigned long long)(vx * vy * p.K));
+                    if (vx > 0 && vy > 0) s_cnt[0] += (unsigned long long)nz * (unsigned long long)(vx * vy * p.K);   // (this thread alone)
                 }
             }
             {
@@ -534,6 +536,11 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
     }
     rtc::tc_fence_before();
     __syncthreads();
+    if (tid == 0) {                                                  // one atomic per counter and CTA, not per tile
+        if (s_cnt[0]) atomicAdd(a.fma_counter, s_cnt[0]);
+        if (s_cnt[1]) atomicAdd(a.fma_counter + 3, s_cnt[1]);
+        if (s_cnt[2]) atomicAdd(a.fma_counter + 4, s_cnt[2]);
+    }
     if (warp == 0) {
         rtc::tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(64u) : "memory");
