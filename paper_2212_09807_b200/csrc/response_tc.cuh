@@ -294,10 +294,14 @@ template <bool CTA2> __device__ __forceinline__ void tc_commit_x(uint32_t bar, b
 #ifdef LARTPC_DEBUG_CLOCKS
 __device__ unsigned long long g_rtc_dbg[16];   // measurement build: cycles the MMA issuer / producer spend per phase
 #define RTC_T(x) const long long x = clock64()
-#define RTC_ADD(i, v) atomicAdd(&g_rtc_dbg[i], (unsigned long long)(v))
+#define RTC_DECL unsigned long long rtc_acc[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}
+#define RTC_ADD(i, v) rtc_acc[i] += (unsigned long long)(v)                 // per thread; one flush when the role ends
+#define RTC_FLUSH do { for (int i_ = 0; i_ < 16; ++i_) if (rtc_acc[i_]) atomicAdd(&g_rtc_dbg[i_], rtc_acc[i_]); } while (0)
 #else
 #define RTC_T(x)
+#define RTC_DECL
 #define RTC_ADD(i, v)
+#define RTC_FLUSH
 #endif
 constexpr int MAX_STAGES = 8;
 constexpr int N_MAIL = MAX_STAGES + 2;  // item mailbox slots of the peer: the leader's producer is never more than a ring ahead
@@ -393,6 +397,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
     if (warp == 0) {
         if (lane == 0) {
             // ------------------------------------------------------------------ producer (leader: schedules; peer: follows)
+            RTC_DECL;
             const uint32_t peer_gox0 = CTA2 ? mapa(gox0, 1u) : 0u, peer_mail0 = CTA2 ? mapa(mail0, 1u) : 0u;
             volatile int4 *mail = (volatile int4 *)(gen + mail0);
             const size_t tb_stride = (size_t)NC * (NBLK * A_BLOCK_BYTES);
@@ -480,6 +485,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
             mbar_wait(empty0 + 8 * s, ph ^ 1u);                        // terminator: a header-only stage
             hdr[s].w = HDR_END;
             mbar_arrive(full0 + 8 * s);
+            RTC_FLUSH;
         }
     } else if (warp == 1 || warp == 6) {
         if (lane == 0 && !leader && warp == 1) {
@@ -505,6 +511,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
             // a single issuer cannot keep the pipe busy.  The two accumulators are independent, so the order between
             // the two threads' MMAs does not matter; each commits every stage (and item) once.
             const int par = warp == 1 ? 0 : 1;
+            RTC_DECL;
             // instruction descriptor: D fp32, A and B fp16 (kind::f16) or e4m3 (kind::f8f6f4) -- format code 0 in both
             // kinds --, both K-major, N = NBW, M = 128 per CTA
             const uint32_t idesc = (1u << 4) | ((uint32_t)(NBW >> 3) << 17) | ((uint32_t)((CTA2 ? 2 * TB : TB) >> 4) << 24);
@@ -559,6 +566,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 RTC_ADD(0, t1 - t0);  RTC_ADD(1, t2 - t1);  RTC_ADD(2, t3 - t2);  RTC_ADD(3, t4 - t3);  RTC_ADD(4, t5 - t4);  RTC_ADD(5, 1);
                 if (++s == S) { s = 0; ph ^= 1u; }
             }
+            RTC_FLUSH;
         }
     } else {
         // ---------------------------------------------------------------------- epilogue (warps 2-5, every CTA)
