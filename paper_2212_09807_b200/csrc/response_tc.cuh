@@ -43,7 +43,16 @@ namespace rtc {
 constexpr int TB = 128;            // tiles per tile block (MMA M)
 constexpr int JC = 64;             // arrival ticks per tile (K extent per bin): 4 blocks of 16
 constexpr int NBLK = JC / 16;
-constexpr int THREADS = 224;          // 7 warps: producer, MMA issuer (even blocks) / relay, 4 x epilogue, MMA issuer (odd blocks)
+#ifndef LARTPC_EPI_GROUPS
+#define LARTPC_EPI_GROUPS 1
+#endif
+// An item's read-out (TMEM -> registers -> HBM) sits between two items' MMAs: the accumulators are single.  EPI_G warps per
+// TMEM lane quarter share its column chunks; measured at configs[3], 1 -> 2 -> 4 warps shorten it 7 700 -> 6 600 -> 6 500
+// cycles (TMEM reads at 64 B / cycle: 3 800 cycles for the two accumulators) and leave the kernel's time where it was
+// (profiles/r2_response_bound.md), so one warp per quarter it stays.
+constexpr int EPI_G = LARTPC_EPI_GROUPS;
+// warps: producer, MMA issuer (even blocks) / relay, 4 x epilogue, MMA issuer (odd blocks), 4 x epilogue per further group
+constexpr int THREADS = 224 + 128 * (EPI_G - 1);
 // fp8 parts: lo8(A) = e4m3(lo(A) 2^SA) meets hi8(B) = e4m3(B 2^-SA); hi8(A) = e4m3(A 2^-SB) meets lo8(B) = e4m3(lo(B) 2^SB)
 // (|A| < 2^15, |lo(A)| <= 8, |B| <= 2^10, |lo(B)| <= 0.5: every part stays below e4m3's 448)
 constexpr int SA_LOG2 = 5, SB_LOG2 = 7;
@@ -375,7 +384,7 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
         for (int s = 0; s < S; ++s) { mbar_init(full0 + 8 * s, 1);  mbar_init(empty0 + 8 * s, 2);  mbar_init(pfull0 + 8 * s, 1); }
         for (int m = 0; m < N_MAIL; ++m) mbar_init(gox0 + 8 * m, 1);
         mbar_init(tfull, 2);
-        mbar_init(tempty, CTA2 ? 8 : 4);                               // one arrival per epilogue warp of the pair
+        mbar_init(tempty, (CTA2 ? 8 : 4) * EPI_G);                     // one arrival per epilogue warp of the pair
         mbar_init(titem, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -536,7 +545,9 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                     break;
                 }
                 if (flags & HDR_FIRST) {
+                    RTC_T(w0);
                     mbar_wait_cluster(tempty, tph);                    // accumulators drained and zeroed, in both CTAs
+                    RTC_T(w1);  RTC_ADD(6, w1 - w0);  RTC_ADD(7, 1);
                     tph ^= 1u;
                     if (!par) {
                         epi_item->x = u;  epi_item->y = d;  epi_item->z = umask;  epi_item->w = 0;
@@ -571,24 +582,28 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
     } else {
         // ---------------------------------------------------------------------- epilogue (warps 2-5, every CTA)
         const int quad = warp & 3;                                     // TMEM lanes [32 quad, 32 quad + 32)
+        const int grp = warp < 6 ? 0 : 1 + (warp - 7) / 4;             // which of the quarter's EPI_G warps
         const uint32_t tlane = tmem + ((uint32_t)(32 * quad) << 16);
         const uint32_t lead_tempty = CTA2 ? mapa(tempty, 0u) : tempty;
+        // column chunks of 16 output ticks: group grp reads chunks [ch_lo, ch_hi)
+        const int n_ch = (a.tile_ticks + 15) / 16, ch_per = (n_ch + EPI_G - 1) / EPI_G;
+        const int ch_lo = min(grp * ch_per, n_ch), ch_hi = min(ch_lo + ch_per, n_ch);
         // every MMA accumulates: the accumulators are zero before the first item and zeroed again after each read-out
-        for (int c0 = 0; c0 < 512; c0 += 64) tmem_zero64(tlane + c0);
+        // (each group the 64-column blocks c0 / 64 = grp mod EPI_G, once all groups of the quarter have read)
+        for (int c0 = 64 * grp; c0 < 512; c0 += 64 * EPI_G) tmem_zero64(tlane + c0);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         tc_fence_before();
         __syncwarp();
         if (lane == 0) { if (CTA2) mbar_arrive_remote(lead_tempty); else mbar_arrive(tempty); }
         uint32_t iph = 0;
+        RTC_DECL;
         while (true) {
             // one lane polls (128 threads spinning on a barrier for the ~30 us an item takes cost issue slots and power)
             if (lane == 0) mbar_wait_cluster(titem, iph);              // acquire: the MMA warp has published the item
             __syncwarp();
             if (epi_item->w & HDR_END) break;
             const int u = epi_item->x, d = epi_item->y, mask = epi_item->z;
-            if (lane == 0) mbar_wait(tfull, iph);
-            __syncwarp();
-            tc_fence_after();
+            // (the tile's scale and block counts come from HBM / L2: fetched while the item's MMAs still run)
             const int tile = (u * (CTA2 ? 2 : 1) + (int)rank) * TB + 32 * quad + lane;
             const bool live = tile < a.n_tiles;
             const bool even = (mask & 5) != 0, odd = (mask & 10) != 0;
@@ -600,6 +615,10 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
 #pragma unroll
                 for (int b = 0; b < NBLK; ++b) nzb[b] = (float)(((unsigned)tm.w >> (8 * b)) & 255u) * (8.f / 16.f) * a.kappa;
             }
+            if (lane == 0) mbar_wait(tfull, iph);
+            __syncwarp();
+            tc_fence_after();
+            RTC_T(e0);
             // 1 + kappa x (non-zero cells with arrival tick j in (n - K, n], of the blocks of one parity): what the
             // accumulator column of output tick n lost to truncation, in expectation.  Cells are taken as spread evenly
             // over the 16 ticks of their block; evaluated every 8 ticks, linear in between.
@@ -610,9 +629,9 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                 return fmaf(nzb[par], (float)wa, fmaf(nzb[par + 2], (float)wb, 1.f));
             };
             float *dst = a.partial + ((size_t)(live ? tile : 0) * a.WW + d) * a.tile_ticks;
-            float g0e = comp(0, 0), g0o = comp(0, 1);
+            float g0e = comp(16 * ch_lo, 0), g0o = comp(16 * ch_lo, 1);
             // output tick n = even accumulator column n (blocks 0, 2) + odd accumulator column n - 16 (blocks 1, 3)
-            for (int n0 = 0; n0 < a.tile_ticks; n0 += 16) {
+            for (int n0 = 16 * ch_lo; n0 < 16 * ch_hi; n0 += 16) {
                 uint32_t v0[16], v1[16];
                 const bool has0 = even && n0 < ACC_COL, has1 = odd && n0 >= 16;
                 if (has0) tmem_ld16(tlane + n0, v0);
@@ -635,20 +654,33 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                         }
                         // one 256-bit store per 8 ticks: each lane writes its own row, so the store path sees 32 sectors per
                         // instruction either way, and half as many instructions (response 175 -> 167 ms at configs[3])
+#ifdef LARTPC_EXP_NOSTORE
+                        if (r[0] == 1.2345f)
+#endif
                         st_global_256(dst + n0 + 8 * i8, make_uint4(__float_as_uint(r[0]), __float_as_uint(r[1]), __float_as_uint(r[2]), __float_as_uint(r[3])),
                                       make_uint4(__float_as_uint(r[4]), __float_as_uint(r[5]), __float_as_uint(r[6]), __float_as_uint(r[7])));
                     }
                 }
                 g0e = g2e;  g0o = g2o;
             }
-            if (even) for (int c0 = 0; c0 < ACC_COL; c0 += 64) tmem_zero64(tlane + c0);
-            if (odd) for (int c0 = ACC_COL; c0 < 2 * ACC_COL; c0 += 64) tmem_zero64(tlane + c0);
+            RTC_T(eA);
+            if (EPI_G > 1) {                                           // the quarter's columns are read by all its groups
+                tc_fence_before();
+                asm volatile("bar.sync %0, %1;" ::"r"(1 + quad), "r"(32 * EPI_G) : "memory");
+                tc_fence_after();
+            }
+            for (int c0 = 64 * grp; c0 < 2 * ACC_COL; c0 += 64 * EPI_G)
+                if (c0 < ACC_COL ? even : odd) tmem_zero64(tlane + c0);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            RTC_T(eB);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) { if (CTA2) mbar_arrive_remote(lead_tempty); else mbar_arrive(tempty); }
             iph ^= 1u;
+            RTC_T(e1);
+            if (tid == 64) { RTC_ADD(11, e1 - e0);  RTC_ADD(12, 1);  RTC_ADD(13, eA - e0);  RTC_ADD(14, eB - eA); }
         }
+        if (tid == 64) RTC_FLUSH;
     }
     tc_fence_before();
     __syncthreads();
