@@ -16,6 +16,14 @@
 // sigma = 0 segments take the float64 indicator path of the oracle (one-hot weights), as in charge_lattice_kernel.
 
 constexpr int CT_THREADS = 128;
+#ifdef LARTPC_DEBUG_CLOCKS
+__device__ unsigned long long g_ct_dbg[16];   // measurement build: thread 0's cycles per phase of a tile
+#define CT_T(x) const long long x = clock64()
+#define CT_ADD(i, v) ct_acc[i] += (unsigned long long)(v)
+#else
+#define CT_T(x)
+#define CT_ADD(i, v)
+#endif
 constexpr int CT_KB = 64;                              // samples per batch
 constexpr int CT_A_HALF = 128 * CT_KB * 2;             // bytes of one precision half of the WXY operand (16 KB)
 constexpr int CT_B_HALF = 64 * CT_KB * 2;              // ... of the WT operand (8 KB)
@@ -232,7 +240,13 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
     int slot = 0;                                                    // ring position of the current tile
     bool have_rec = false;                                           // s_rec holds the first chunk of the current tile
 
+#ifdef LARTPC_DEBUG_CLOCKS
+    unsigned long long ct_acc[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+#endif
     while (true) {
+#ifdef LARTPC_DEBUG_CLOCKS
+        long long c_top = clock64();
+#endif
         const int tile = s_q[slot];
         if (tile >= a.n_tiles) break;                                // CTA-uniform: the ring is read after a barrier
         const TileDesc td = s_td[slot];
@@ -262,6 +276,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
             const int nseg = min(SEGCAP, lcount - l0);
             // The K dimension of the contraction is "sample", whichever segment it belongs to: the columns of the staged
             // segments are laid end to end (pre[] = running sum of their counts, in list order) and cut into batches of 64.
+            CT_T(c_s0);
             if (warp == 0) {
                 int n_eff = 0;
                 if (lane < nseg) {
@@ -285,7 +300,9 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                 pre[lane + 1] = inc;
                 if (lane == 0) pre[0] = 0;
             }
+            CT_T(c_s1);
             __syncthreads();
+            CT_T(c_staged);  CT_ADD(0, c_staged - c_top);  CT_ADD(8, c_s0 - c_top);  CT_ADD(9, c_s1 - c_s0);  CT_ADD(10, c_staged - c_s1);  CT_ADD(11, 1);
             if (l0 == 0 && warp == 0) {
                 // look-ahead: cursor for the tile three ahead, descriptor of the tile two ahead, ids of the next tile
                 if (lane == 0) {
@@ -303,6 +320,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                 s_cnt[2] += 3ull * (unsigned long long)((total + 15) / 16);         // hi hi + hi lo + lo hi per 16 columns
             }
             for (int s0 = 0; s0 < total; s0 += CT_KB) {
+                CT_T(c_b0);
                 const int nsb = min(CT_KB, total - s0), nk16 = (nsb + 15) >> 4;
                 if (s_in < 16 * nk16) {
                     const bool real = s_in < nsb;
@@ -416,7 +434,9 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                 }
                 // operands written by the generic proxy, read by the tensor core (async proxy)
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                CT_T(c_b1);
                 __syncthreads();
+                CT_T(c_b2);
                 if (tid == 0) {
                     rtc::tc_fence_after();
                     for (int k16 = 0; k16 < nk16; ++k16) {
@@ -436,9 +456,14 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                 any_mma = true;
                 rtc::mbar_wait(bar, mma_phase);                        // the MMAs have read the operands (and landed)
                 mma_phase ^= 1u;
+                CT_T(c_b3);  CT_ADD(1, c_b1 - c_b0);  CT_ADD(2, c_b2 - c_b1);  CT_ADD(3, c_b3 - c_b2);  CT_ADD(6, 1);
+#ifdef LARTPC_DEBUG_CLOCKS
+                c_top = c_b3;                                          // (a further chunk's staging counts from here)
+#endif
             }
         }
         if (!fetched && warp == 0) fetch_next_records();
+        CT_T(c_r0);
         // ------------------------------------------------------------------ accumulator -> operand image of the response
         if (!any_mma) {                                                   // CTA-uniform: no segment reaches this window
             if (tid == 0) *(int4 *)(a.tile_range + TILE_META * tile) = make_int4(1, 0, 0, 0);
@@ -523,6 +548,7 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
                 }
             }
         }
+        CT_T(c_r1);
         // the look-ahead of this tile has landed; hand the ring on
         if (warp == 0) {
             cp_async_wait_all();
@@ -533,7 +559,11 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
         rtc::tc_fence_before();
         __syncthreads();
         rtc::tc_fence_after();
+        CT_T(c_end);  CT_ADD(4, c_r1 - c_r0);  CT_ADD(5, c_end - c_r1);  CT_ADD(7, 1);
     }
+#ifdef LARTPC_DEBUG_CLOCKS
+    if (tid == 0) for (int i = 0; i < 16; ++i) atomicAdd(&g_ct_dbg[i], ct_acc[i]);
+#endif
     rtc::tc_fence_before();
     __syncthreads();
     if (tid == 0) {                                                  // one atomic per counter and CTA, not per tile

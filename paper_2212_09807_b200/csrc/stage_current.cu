@@ -822,13 +822,15 @@ int launch_current_response(lartpc_sim *sim, lartpc_signals_t *out, cudaStream_t
 }
 
 #ifdef LARTPC_DEBUG_CLOCKS
-extern "C" int lartpc_debug_clocks(unsigned long long out[24], int reset)
+extern "C" int lartpc_debug_clocks(unsigned long long out[32], int reset)
 {
-    cudaMemcpyFromSymbol(out, g_dbg, sizeof(unsigned long long) * 8);
+    cudaMemcpyFromSymbol(out, g_ct_dbg, sizeof(unsigned long long) * 8);   // charge lattice: thread 0's cycles per phase
+    cudaMemcpyFromSymbol(out + 24, g_ct_dbg, sizeof(unsigned long long) * 8, sizeof(unsigned long long) * 8);
     cudaMemcpyFromSymbol(out + 8, rtc::g_rtc_dbg, sizeof(unsigned long long) * 16);
     if (reset) {
         unsigned long long z[16] = {0};
-        cudaMemcpyToSymbol(g_dbg, z, sizeof(unsigned long long) * 8);
+        cudaMemcpyToSymbol(g_ct_dbg, z, sizeof(unsigned long long) * 8);
+        cudaMemcpyToSymbol(g_ct_dbg, z, sizeof(unsigned long long) * 8, sizeof(unsigned long long) * 8);
         cudaMemcpyToSymbol(rtc::g_rtc_dbg, z, sizeof(z));
     }
     return 0;

@@ -446,7 +446,7 @@ int sim_grow_tiles(lartpc_sim *sim, int64_t cap)
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list_p, sizeof(int2) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tb_mask, sizeof(int32_t) * (cap / TC_TILE_BLOCK + 2)));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tc_cmask, sizeof(int32_t) * (cap / TC_TILE_BLOCK + 2) * TC_CMASK_WORDS));
-    if (!sim->cls_hist) LARTPC_CUDA_TRY(cudaMalloc(&sim->cls_hist, sizeof(int32_t) * 2 * TC_CLASSES));
+    if (!sim->cls_hist) LARTPC_CUDA_TRY(cudaMalloc(&sim->cls_hist, sizeof(int32_t) * (2 * TC_CLASSES + 2)));   // + the own-list cursor
     sim->tile_cap = cap;
     return LARTPC_OK;
 }
@@ -460,9 +460,9 @@ int sim_grow_tiles(lartpc_sim *sim, int64_t cap)
 // configs[3] / configs[2]: 23 % / 33 % of the (unit, bin, block) pairs drop out (profiles/r2_response_bound.md).
 
 __global__ void __launch_bounds__(256)
-tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td, const int2 *__restrict__ tl,
-                  const int32_t *__restrict__ pair_seg, lartpc_pixmap_t pm, const void *__restrict__ seg_rec, int32_t *cls,
-                  int32_t *hist, int sort)
+tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td, int2 *tl, int32_t *pair_seg,
+                  lartpc_pixmap_t pm, const void *__restrict__ seg_rec, int32_t *cls, int32_t *hist, int sort,
+                  int64_t own_base, int64_t own_cap)
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int c = TC_CLASSES;                                               // no tile (a group of its own below)
@@ -473,6 +473,7 @@ tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td,
             const TileDesc d = td[t];
             const int2 l = tl[t];
             const int A_t = d.px * p.nb, B_t = d.py * p.nb;
+            int n_own = 0;
             for (int k = 0; k < l.y; ++k) {
                 const int s = pair_seg[l.x + k];
                 // the segment's boxes: one 32-byte sector of its record (SEG_REC_BYTES / SEG_REC_BOX_OFFSET: the eight ints
@@ -487,9 +488,32 @@ tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td,
                 }
                 const int jlo = max(max(s_jt0, 0) - d.j_start, 0), jhi = min(min(s_jt1, p.j_max) - d.j_start, p.Jc - 1);
                 if (jlo > jhi) continue;                              // the segment charges another window of this pixel
+                ++n_own;
                 mask |= ((2 << (jhi >> 4)) - 1) & ~((1 << (jlo >> 4)) - 1);
                 alo = min(alo, max(s_alo - A_t, 0));  ahi = max(ahi, min(s_ahi - A_t, p.nb - 1));
                 blo = min(blo, max(s_blo - B_t, 0));  bhi = max(bhi, min(s_bhi - B_t, p.nb - 1));
+            }
+            // The tile's own list: the charge lattice walks a tile's list segment by segment, and a pixel that is hit again
+            // and again over a spill (~120 segments at configs[3]) has ~7 in any one 64-tick window.  The segments found
+            // above are written out once more, in the same order, behind the pixels' lists (own_base); a tile that finds
+            // no room there keeps the list of its pixel.
+            if (n_own < l.y && own_cap > 0) {
+                const long long off = (long long)atomicAdd((unsigned long long *)(hist + 2 * TC_CLASSES), (unsigned long long)n_own);
+                if (off + n_own <= own_cap) {
+                    int32_t *dst = pair_seg + own_base + off;
+                    int w = 0;
+                    for (int k = 0; k < l.y && w < n_own; ++k) {
+                        const int s = pair_seg[l.x + k];
+                        int s_jt0, s_jt1;
+                        if (seg_rec) {
+                            const int4 r1 = __ldg((const int4 *)((const char *)seg_rec + (size_t)SEG_REC_BYTES * s + SEG_REC_BOX_OFFSET) + 1);
+                            s_jt0 = r1.y;  s_jt1 = r1.z;
+                        } else { s_jt0 = pm.jt0[s];  s_jt1 = pm.jt1[s]; }
+                        if (max(max(s_jt0, 0) - d.j_start, 0) > min(min(s_jt1, p.j_max) - d.j_start, p.Jc - 1)) continue;
+                        dst[w++] = s;
+                    }
+                    tl[t] = make_int2((int)(own_base + off), n_own);
+                }
             }
         }
         // edges in TC_BOXQ steps over the pixel (any bins_per_pixel); an empty box sorts first
@@ -556,6 +580,21 @@ static int grow_i32(int32_t **p, int64_t *cap, int64_t need)
     *p = nullptr;
     int64_t c = need + need / 4 + 1024;
     LARTPC_CUDA_TRY(cudaMalloc(p, sizeof(int32_t) * c));
+    *cap = c;
+    return LARTPC_OK;
+}
+
+// the same, keeping the first `keep` elements (the copy is ordered behind what wrote them on `st`)
+static int grow_i32_keep(int32_t **p, int64_t *cap, int64_t need, int64_t keep, cudaStream_t st)
+{
+    if (need <= *cap) return LARTPC_OK;
+    int32_t *q = nullptr;
+    const int64_t c = need + need / 8 + 1024;
+    LARTPC_CUDA_TRY(cudaMalloc(&q, sizeof(int32_t) * c));
+    if (*p && keep > 0) LARTPC_CUDA_TRY(cudaMemcpyAsync(q, *p, sizeof(int32_t) * keep, cudaMemcpyDeviceToDevice, st));
+    LARTPC_CUDA_TRY(cudaStreamSynchronize(st));
+    if (*p) cudaFree(*p);
+    *p = q;
     *cap = c;
     return LARTPC_OK;
 }
@@ -649,12 +688,18 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         // the FFMA2 splat (bins per pixel other than 5 / 10) writes the operand image in the tiles' original order
         const int sort = splat_on_tc(p) ? 1 : 0;
         const int64_t nt = sim->n_tiles;
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->cls_hist, 0, sizeof(int32_t) * 2 * TC_CLASSES, st));
+        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->cls_hist, 0, sizeof(int32_t) * (2 * TC_CLASSES + 2), st));
+        // room behind the pixels' lists for the tiles' own lists: a segment charges one or two windows of a pixel
+        int64_t own_cap = 0;
+        if (sort && h[CNT_PAIRS] > 0) {
+            own_cap = std::min<int64_t>(2 * h[CNT_PAIRS] + 4096, (int64_t)INT32_MAX - h[CNT_PAIRS] - 1);
+            if ((rc = grow_i32_keep(&sim->pair_seg, &sim->pair_cap, h[CNT_PAIRS] + own_cap, h[CNT_PAIRS], st)) != 0) return rc;
+        }
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->tb_mask, 0, sizeof(int32_t) * (nt / TC_TILE_BLOCK + 1), st));
         g_lartpc_launches += 3;
         tile_class_kernel<<<div_up(nt, 256), 256, 0, st>>>(p, nt, sim->tile_desc, sim->tile_list, sim->pair_seg, *out,
                                                           (sort && sim->seg_rec_cap >= n) ? sim->seg_rec : nullptr,
-                                                          sim->tile_perm, sim->cls_hist, sort);
+                                                          sim->tile_perm, sim->cls_hist, sort, h[CNT_PAIRS], own_cap);
         class_offsets_kernel<<<1, 1024, 0, st>>>(sim->cls_hist);
         tile_scatter_kernel<<<div_up(nt, 256), 256, 0, st>>>(nt, sim->tile_perm, sim->cls_hist, sim->tile_desc,
                                                             sim->tile_list, sim->tile_desc_p, sim->tile_list_p,
