@@ -45,7 +45,7 @@ static void sim_free(lartpc_sim *s)
     cudaFree(s->d_tpcs); cudaFree(s->d_lut); cudaFree(s->d_lut_tc); cudaFree(s->d_cum_lut);
     cudaFree(s->pix_count); cudaFree(s->pix_start); cudaFree(s->pix_tile0); cudaFree(s->pix_cursor);
     cudaFree(s->pix_mask); cudaFree(s->act_first); cudaFree(s->act_last); cudaFree(s->act_slot);
-    cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->tile_list); cudaFree(s->seg_rec);
+    cudaFree(s->pair_seg); cudaFree(s->tile_cp); cudaFree(s->tile_desc); cudaFree(s->tile_list); cudaFree(s->cell_list); cudaFree(s->seg_rec);
     cudaFree(s->pack_base); cudaFree(s->pack_count);
     cudaFree(s->tile_perm); cudaFree(s->tile_desc_p); cudaFree(s->tile_list_p); cudaFree(s->tb_mask); cudaFree(s->tc_cmask); cudaFree(s->cls_hist); cudaFree(s->scan_tmp);
     cudaFree(s->d_counters); cudaFree(s->disabled_mask); cudaFree(s->elec_slots); cudaFree(s->elec_offs);

@@ -82,7 +82,7 @@ constexpr int TC_CMASK_WORDS = 16;   // tc_cmask: per unit, 4 bits per LUT bin (
 // device counters written by the planning kernels (mirrored to pinned host memory)
 enum {
     CNT_MAX_NPIX = 0, CNT_MAX_TICKS, CNT_ACTIVE_SEGS, CNT_PAIRS, CNT_TILES, CNT_ACTIVE_PIX,
-    CNT_TOTAL_SAMPLES, CNT_TOTAL_NPIX, CNT_OVERFLOW, CNT_COMPOSITE, CNT_COUNT = 16
+    CNT_TOTAL_SAMPLES, CNT_TOTAL_NPIX, CNT_OVERFLOW, CNT_COMPOSITE, CNT_CELLS, CNT_COUNT = 16
 };
 
 struct lartpc_sim {
@@ -105,6 +105,7 @@ struct lartpc_sim {
     // growable planning arrays
     int32_t *pair_seg = nullptr;  int64_t pair_cap = 0;
     int32_t *tile_cp = nullptr;   TileDesc *tile_desc = nullptr;  int64_t tile_cap = 0;
+    int32_t *cell_list = nullptr;        // [tile_cap] the charged cells that hold tiles, in no particular order (tile_emit_kernel)
     int2 *tile_list = nullptr;           // [tile_cap] {start, count} of the tile's segment list in pair_seg
     // tensor-core mode: tiles sorted by the 16-tick blocks they charge (launch_plan): slot of a tile, descriptors and
     // lists in slot order, per 128-slot block the OR of its tiles' block masks

@@ -297,12 +297,14 @@ pair_fill_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t n, const 
 
 // the atomics above fill each list in arbitrary order; sort it by segment id so that the float32
 // accumulation order of S4 (and hence every output bit) is reproducible from run to run: one warp per list
+constexpr int PAIR_RANK_MAX = 512;
 __global__ void __launch_bounds__(128)
-pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int32_t *__restrict__ pix_count,
-                 int32_t *pair_seg, int64_t pair_cap)
+pair_sort_kernel(int64_t n_cells, const int32_t *__restrict__ cell_list, const int32_t *__restrict__ pix_start,
+                 const int32_t *__restrict__ pix_count, int32_t *pair_seg, int64_t pair_cap)
 {
-    int64_t cp = (int64_t)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5);
-    if (cp >= n_cp) return;
+    const int64_t ci = (int64_t)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5);
+    if (ci >= n_cells) return;
+    const int64_t cp = cell_list[ci];
     int cnt = pix_count[cp];
     if (cnt < 2) return;
     int lane = threadIdx.x & 31;
@@ -321,6 +323,22 @@ pair_sort_kernel(int64_t n_cp, const int32_t *__restrict__ pix_start, const int3
                 x = up ? min(x, y) : max(x, y);
             }
         if (lane < cnt) v[lane] = x;
+        return;
+    }
+    if (cnt <= PAIR_RANK_MAX) {
+        // up to 512: rank sort through shared memory (segment ids are distinct: the rank of an id is the number of smaller
+        // ones; n^2 / 32 comparisons per lane on broadcast reads beat a bitonic network that works in global memory --
+        // a pixel of a full spill holds ~120 segments)
+        __shared__ int32_t s_list[4][PAIR_RANK_MAX];
+        int32_t *sl = s_list[threadIdx.x >> 5];
+        for (int i = lane; i < cnt; i += 32) sl[i] = v[i];
+        __syncwarp();
+        for (int i = lane; i < cnt; i += 32) {
+            const int32_t x = sl[i];
+            int r = 0;
+            for (int j = 0; j < cnt; ++j) r += sl[j] < x ? 1 : 0;
+            v[r] = x;
+        }
         return;
     }
     // longer lists: the same-direction bitonic network on the list in place (first step of every merge pairs i with
@@ -353,8 +371,8 @@ __global__ void __launch_bounds__(256)
 tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t cp0, int64_t n_cp, const int32_t *__restrict__ pix_tile0,
                  const unsigned long long *__restrict__ pix_mask, const int32_t *__restrict__ pix_jmin,
                  const int32_t *__restrict__ pix_start, const int32_t *__restrict__ pix_count,
-                 int32_t *tile_cp, TileDesc *tile_desc, int2 *tile_list, int64_t tile_cap, int32_t *act_first, int32_t *act_last,
-                 long long *counters)
+                 int32_t *tile_cp, TileDesc *tile_desc, int2 *tile_list, int64_t tile_cap, int32_t *cell_list,
+                 int32_t *act_first, int32_t *act_last, long long *counters)
 {
     int64_t cp = cp0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // cells [cp0, cp0 + n_cp) of the planned TPCs
     if (cp >= cp0 + n_cp) return;
@@ -363,6 +381,15 @@ tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t cp0, int6
 #pragma unroll
     for (int wd = 0; wd < MASK_WORDS; ++wd) { mask[wd] = pix_mask[(size_t)cp * MASK_WORDS + wd]; any |= mask[wd] != 0; }
     if (!any) return;
+    {
+        // the cells that hold tiles, for the per-cell passes behind the plan's synchronisation (one atomic per warp)
+        const unsigned act = __activemask();
+        const int lane = threadIdx.x & 31, leader = __ffs(act) - 1;
+        long long base = 0;
+        if (lane == leader) base = (long long)atomicAdd((unsigned long long *)&counters[CNT_CELLS], (unsigned long long)__popc(act));
+        base = __shfl_sync(act, base, leader) + __popc(act & ((1u << lane) - 1u));
+        if (base < tile_cap) cell_list[base] = (int32_t)cp;
+    }
     int tpc = 0;
     while (tpc + 1 < p.n_tpcs && tpcs[tpc + 1].cp_base <= cp) ++tpc;
     const DevTpc &t = tpcs[tpc];
@@ -434,13 +461,14 @@ int sim_ensure_scan_tmp(lartpc_sim *sim, int64_t elems)
 // (re)allocates every per-tile planning array for `cap` tiles
 int sim_grow_tiles(lartpc_sim *sim, int64_t cap)
 {
-    cudaFree(sim->tile_cp); cudaFree(sim->tile_desc); cudaFree(sim->tile_list); cudaFree(sim->tile_perm);
+    cudaFree(sim->tile_cp); cudaFree(sim->tile_desc); cudaFree(sim->tile_list); cudaFree(sim->tile_perm); cudaFree(sim->cell_list);
     cudaFree(sim->tile_desc_p); cudaFree(sim->tile_list_p); cudaFree(sim->tb_mask); cudaFree(sim->tc_cmask);
-    sim->tile_cp = nullptr; sim->tile_desc = nullptr; sim->tile_list = nullptr; sim->tile_perm = nullptr;
+    sim->tile_cp = nullptr; sim->tile_desc = nullptr; sim->tile_list = nullptr; sim->tile_perm = nullptr; sim->cell_list = nullptr;
     sim->tile_desc_p = nullptr; sim->tile_list_p = nullptr; sim->tb_mask = nullptr; sim->tc_cmask = nullptr; sim->tile_cap = 0;
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_cp, sizeof(int32_t) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc, sizeof(TileDesc) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list, sizeof(int2) * cap));
+    LARTPC_CUDA_TRY(cudaMalloc(&sim->cell_list, sizeof(int32_t) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_perm, sizeof(int32_t) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_desc_p, sizeof(TileDesc) * cap));
     LARTPC_CUDA_TRY(cudaMalloc(&sim->tile_list_p, sizeof(int2) * cap));
@@ -459,70 +487,153 @@ int sim_grow_tiles(lartpc_sim *sim, int64_t cap)
 // class is whatever the atomics give: a tile's slot only decides where its rows live, never a sum.  Measured on
 // configs[3] / configs[2]: 23 % / 33 % of the (unit, bin, block) pairs drop out (profiles/r2_response_bound.md).
 
-__global__ void __launch_bounds__(256)
-tile_class_kernel(DevParams p, int64_t n_tiles, const TileDesc *__restrict__ td, int2 *tl, int32_t *pair_seg,
-                  lartpc_pixmap_t pm, const void *__restrict__ seg_rec, int32_t *cls, int32_t *hist, int sort,
-                  int64_t own_base, int64_t own_cap)
+// One warp per charged pixel.  Every tile of the pixel (one per 64-tick window that holds charge) needs the segments of the
+// pixel's list that reach its window: they give the tile's class (block mask, box of charged bins), and they are written
+// out once more, in the same order, behind the pixels' lists (own_base) as the tile's OWN list -- the charge lattice walks
+// a tile's list segment by segment, and a pixel that is hit again and again over a spill (~120 segments at configs[3])
+// has ~7 in any one window (charge lattice 100 -> 63 ms).  The lanes read the list 32 segments at a time, once to count
+// and classify, once to write; a segment names its windows itself, so the work is linear in the list, not list x tiles.
+// Tiles that find no room behind the lists keep the list of their pixel (tile_emit_kernel wrote it).
+constexpr int PC_WARPS = 8;
+__global__ void __launch_bounds__(32 * PC_WARPS)
+pixel_class_kernel(DevParams p, int64_t n_cells, const int32_t *__restrict__ cell_list, const int32_t *__restrict__ pix_start,
+                   const int32_t *__restrict__ pix_count, const int32_t *__restrict__ pix_tile0,
+                   const unsigned long long *__restrict__ pix_mask, const int32_t *__restrict__ pix_jmin,
+                   const TileDesc *__restrict__ td, int2 *tl, int32_t *pair_seg, lartpc_pixmap_t pm,
+                   const void *__restrict__ seg_rec, int32_t *cls, int32_t *hist, int64_t own_base, int64_t own_cap)
+{
+    __shared__ int s_w0[PC_WARPS][MAX_WINDOWS], s_w1[PC_WARPS][MAX_WINDOWS], s_n[PC_WARPS][MAX_WINDOWS];
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    const int64_t ci = (int64_t)blockIdx.x * PC_WARPS + wp;
+    if (ci >= n_cells) return;                                        // (warp-uniform, as everything below that returns)
+    const int64_t cp = cell_list[ci];
+    const unsigned long long m0 = pix_mask[(size_t)cp * MASK_WORDS], m1 = pix_mask[(size_t)cp * MASK_WORDS + 1];
+    static_assert(MASK_WORDS == 2, "two 64-bit window words per charged pixel");
+    const int cnt = pix_count[cp];
+    if ((m0 | m1) == 0ull) return;
+    const int nt = __popcll(m0) + __popcll(m1);
+    const int64_t tile0 = pix_tile0[cp];
+    if (cnt <= 0) {                                                   // (a window bit without a segment: not produced by the plan)
+        for (int r = lane; r < nt; r += 32) cls[tile0 + r] = 0;
+        return;
+    }
+    const int start = pix_start[cp];
+    const TileDesc d0 = td[tile0];
+    const int A_t = d0.px * p.nb, B_t = d0.py * p.nb, js = pix_jmin[cp] & ~3;   // window w starts at tick js + w Jc (tile_emit_kernel)
+    int *w0s = s_w0[wp], *w1s = s_w1[wp], *ns = s_n[wp];
+    for (int r = lane; r < nt; r += 32) { w0s[r] = 0;  w1s[r] = 0;  ns[r] = 0; }
+    __syncwarp();
+    auto has = [&](int w) { return w < 64 ? (m0 >> w & 1ull) != 0ull : (m1 >> (w - 64) & 1ull) != 0ull; };
+    auto rank = [&](int w) { return w < 64 ? __popcll(m0 & ((1ull << w) - 1ull)) : __popcll(m0) + __popcll(m1 & ((1ull << (w - 64)) - 1ull)); };
+    auto fdiv = [&](int x) { return x >= 0 ? x / p.Jc : -((-x + p.Jc - 1) / p.Jc); };
+    // segment k of the list: its id, the windows [wlo, whi] it reaches, its ticks clamped to the read-out, its bins on this pixel
+    auto load = [&](int k, int &sid, int &wlo, int &whi, int &t0, int &t1, int &abits, int &bbits) {
+        wlo = MAX_WINDOWS;  whi = -1;  abits = bbits = 0;  t0 = t1 = 0;  sid = 0;
+        if (k >= cnt) return;
+        const int s = pair_seg[start + k];
+        sid = s;
+        int s_alo, s_ahi, s_blo, s_bhi, s_jt0, s_jt1;
+        if (seg_rec) {
+            // one 32-byte sector of its record (SEG_REC_BYTES / SEG_REC_BOX_OFFSET: the eight ints {N, a_lo, a_hi, b_lo |
+            // b_hi, jt0, jt1, flags} that end the record seg_record_kernel wrote), not six arrays
+            const int4 *r = (const int4 *)((const char *)seg_rec + (size_t)SEG_REC_BYTES * s + SEG_REC_BOX_OFFSET);
+            const int4 r0 = __ldg(r), r1 = __ldg(r + 1);
+            s_alo = r0.y;  s_ahi = r0.z;  s_blo = r0.w;  s_bhi = r1.x;  s_jt0 = r1.y;  s_jt1 = r1.z;
+        } else {
+            s_alo = pm.a_lo[s];  s_ahi = pm.a_hi[s];  s_blo = pm.b_lo[s];  s_bhi = pm.b_hi[s];  s_jt0 = pm.jt0[s];  s_jt1 = pm.jt1[s];
+        }
+        t0 = max(s_jt0, 0);  t1 = min(s_jt1, p.j_max);
+        if (t0 > t1) return;                                          // never read out
+        wlo = max(fdiv(t0 - js), 0);  whi = min(fdiv(t1 - js), MAX_WINDOWS - 1);
+        const int al = max(s_alo - A_t, 0), ah = min(s_ahi - A_t, p.nb - 1), bl = max(s_blo - B_t, 0), bh = min(s_bhi - B_t, p.nb - 1);
+        if (al <= ah) abits = ((2 << ah) - 1) & ~((1 << al) - 1);
+        if (bl <= bh) bbits = ((2 << bh) - 1) & ~((1 << bl) - 1);
+    };
+    // pass 1: per tile the 16-tick blocks and bins its segments charge, and how many segments those are
+    for (int k0 = 0; k0 < cnt; k0 += 32) {
+        int sid, wlo, whi, t0, t1, abits, bbits;
+        load(k0 + lane, sid, wlo, whi, t0, t1, abits, bbits);
+        const int c_lo = __reduce_min_sync(0xffffffffu, wlo), c_hi = __reduce_max_sync(0xffffffffu, whi);
+        for (int w = c_lo; w <= c_hi; ++w) {
+            if (!has(w)) continue;
+            const bool m = wlo <= w && w <= whi;
+            const unsigned bal = __ballot_sync(0xffffffffu, m);
+            if (!bal) continue;
+            int v0 = 0;
+            if (m) {
+                const int jw = js + w * p.Jc, jlo = max(t0 - jw, 0), jhi = min(t1 - jw, p.Jc - 1);
+                v0 = (((2 << (jhi >> 4)) - 1) & ~((1 << (jlo >> 4)) - 1)) | (abits << 4);
+            }
+            const unsigned o0 = __reduce_or_sync(0xffffffffu, (unsigned)v0), o1 = __reduce_or_sync(0xffffffffu, (unsigned)(m ? bbits : 0));
+            if (lane == 0) { const int r = rank(w);  w0s[r] |= (int)o0;  w1s[r] |= (int)o1;  ns[r] += __popc(bal); }
+        }
+    }
+    __syncwarp();
+    // classes; where the tiles' own lists start (tiles that take the whole list keep it)
+    long long total = 0;
+    for (int r0 = 0; r0 < nt; r0 += 32) {
+        const int r = r0 + lane;
+        int own = 0;
+        if (r < nt) {
+            const int v0 = w0s[r], v1 = w1s[r], n = ns[r];
+            const int mask = v0 & 15, ab = v0 >> 4;
+            // edges in TC_BOXQ steps over the pixel (any bins_per_pixel); an empty box sorts first
+            const int q = (p.nb + TC_BOXQ - 1) / TC_BOXQ;
+            const int e0 = ab ? (__ffs(ab) - 1) / q : 0, e1 = ab ? (31 - __clz(ab)) / q : 0;
+            const int e2 = v1 ? (__ffs(v1) - 1) / q : 0, e3 = v1 ? (31 - __clz(v1)) / q : 0;
+            cls[tile0 + r] = (((mask * TC_BOXQ + e0) * TC_BOXQ + e1) * TC_BOXQ + e2) * TC_BOXQ + e3;
+            own = n < cnt ? n : 0;
+        }
+        int inc = own;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += y;
+        }
+        if (r < nt) w1s[r] = own ? (int)total + inc - own : -1;      // offset inside the pixel's block, -1: keeps the pixel's list
+        total += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (total == 0 || own_cap <= 0) return;
+    long long base = 0;
+    if (lane == 0) base = (long long)atomicAdd((unsigned long long *)(hist + 2 * TC_CLASSES), (unsigned long long)total);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (base + total > own_cap) return;
+    __syncwarp();
+    for (int r = lane; r < nt; r += 32)
+        if (w1s[r] >= 0) tl[tile0 + r] = make_int2((int)(own_base + base + w1s[r]), ns[r]);
+    int32_t *dst = pair_seg + own_base + base;
+    // pass 2: the same walk, writing (w1s[r]: next free place of tile r)
+    for (int k0 = 0; k0 < cnt; k0 += 32) {
+        int sid, wlo, whi, t0, t1, abits, bbits;
+        load(k0 + lane, sid, wlo, whi, t0, t1, abits, bbits);
+        const int c_lo = __reduce_min_sync(0xffffffffu, wlo), c_hi = __reduce_max_sync(0xffffffffu, whi);
+        for (int w = c_lo; w <= c_hi; ++w) {
+            if (!has(w)) continue;
+            const bool m = wlo <= w && w <= whi;
+            const unsigned bal = __ballot_sync(0xffffffffu, m);
+            if (!bal) continue;
+            const int r = rank(w), at = w1s[r];
+            __syncwarp();
+            if (at >= 0) {
+                if (m) dst[at + __popc(bal & ((1u << lane) - 1u))] = sid;
+                if (lane == 0) w1s[r] = at + __popc(bal);
+            }
+            __syncwarp();
+        }
+    }
+}
+
+// tiles in their original order (no sort): every block, no box
+__global__ void __launch_bounds__(256) tile_class_flat_kernel(int64_t n_tiles, int32_t *cls)
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    int c = TC_CLASSES;                                               // no tile (a group of its own below)
-    if (t < n_tiles) {
-        int mask = 0, alo = p.nb, ahi = -1, blo = p.nb, bhi = -1;
-        if (!sort) mask = 15;
-        else {
-            const TileDesc d = td[t];
-            const int2 l = tl[t];
-            const int A_t = d.px * p.nb, B_t = d.py * p.nb;
-            int n_own = 0;
-            for (int k = 0; k < l.y; ++k) {
-                const int s = pair_seg[l.x + k];
-                // the segment's boxes: one 32-byte sector of its record (SEG_REC_BYTES / SEG_REC_BOX_OFFSET: the eight ints
-                // {N, a_lo, a_hi, b_lo | b_hi, jt0, jt1, flags} that end the record seg_record_kernel wrote), not six arrays
-                int s_alo, s_ahi, s_blo, s_bhi, s_jt0, s_jt1;
-                if (seg_rec) {
-                    const int4 *r = (const int4 *)((const char *)seg_rec + (size_t)SEG_REC_BYTES * s + SEG_REC_BOX_OFFSET);
-                    const int4 r0 = __ldg(r), r1 = __ldg(r + 1);
-                    s_alo = r0.y;  s_ahi = r0.z;  s_blo = r0.w;  s_bhi = r1.x;  s_jt0 = r1.y;  s_jt1 = r1.z;
-                } else {
-                    s_alo = pm.a_lo[s];  s_ahi = pm.a_hi[s];  s_blo = pm.b_lo[s];  s_bhi = pm.b_hi[s];  s_jt0 = pm.jt0[s];  s_jt1 = pm.jt1[s];
-                }
-                const int jlo = max(max(s_jt0, 0) - d.j_start, 0), jhi = min(min(s_jt1, p.j_max) - d.j_start, p.Jc - 1);
-                if (jlo > jhi) continue;                              // the segment charges another window of this pixel
-                ++n_own;
-                mask |= ((2 << (jhi >> 4)) - 1) & ~((1 << (jlo >> 4)) - 1);
-                alo = min(alo, max(s_alo - A_t, 0));  ahi = max(ahi, min(s_ahi - A_t, p.nb - 1));
-                blo = min(blo, max(s_blo - B_t, 0));  bhi = max(bhi, min(s_bhi - B_t, p.nb - 1));
-            }
-            // The tile's own list: the charge lattice walks a tile's list segment by segment, and a pixel that is hit again
-            // and again over a spill (~120 segments at configs[3]) has ~7 in any one 64-tick window.  The segments found
-            // above are written out once more, in the same order, behind the pixels' lists (own_base); a tile that finds
-            // no room there keeps the list of its pixel.
-            if (n_own < l.y && own_cap > 0) {
-                const long long off = (long long)atomicAdd((unsigned long long *)(hist + 2 * TC_CLASSES), (unsigned long long)n_own);
-                if (off + n_own <= own_cap) {
-                    int32_t *dst = pair_seg + own_base + off;
-                    int w = 0;
-                    for (int k = 0; k < l.y && w < n_own; ++k) {
-                        const int s = pair_seg[l.x + k];
-                        int s_jt0, s_jt1;
-                        if (seg_rec) {
-                            const int4 r1 = __ldg((const int4 *)((const char *)seg_rec + (size_t)SEG_REC_BYTES * s + SEG_REC_BOX_OFFSET) + 1);
-                            s_jt0 = r1.y;  s_jt1 = r1.z;
-                        } else { s_jt0 = pm.jt0[s];  s_jt1 = pm.jt1[s]; }
-                        if (max(max(s_jt0, 0) - d.j_start, 0) > min(min(s_jt1, p.j_max) - d.j_start, p.Jc - 1)) continue;
-                        dst[w++] = s;
-                    }
-                    tl[t] = make_int2((int)(own_base + off), n_own);
-                }
-            }
-        }
-        // edges in TC_BOXQ steps over the pixel (any bins_per_pixel); an empty box sorts first
-        const int q = (p.nb + TC_BOXQ - 1) / TC_BOXQ;
-        const int e0 = ahi < alo ? 0 : alo / q, e1 = ahi < alo ? 0 : ahi / q, e2 = bhi < blo ? 0 : blo / q, e3 = bhi < blo ? 0 : bhi / q;
-        c = (((mask * TC_BOXQ + e0) * TC_BOXQ + e1) * TC_BOXQ + e2) * TC_BOXQ + e3;
-        cls[t] = c;
-    }
-    // one atomic per (warp, class)
+    if (t < n_tiles) cls[t] = 15 * TC_BOX_CLASSES;
+}
+
+// class counts: one atomic per (warp, class)
+__global__ void __launch_bounds__(256) class_hist_kernel(int64_t n_tiles, const int32_t *__restrict__ cls, int32_t *hist)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = t < n_tiles ? cls[t] : TC_CLASSES;                  // no tile: a group of its own
     const int lane = threadIdx.x & 31;
     const unsigned peers = __match_any_sync(0xffffffffu, c);
     if (lane == __ffs(peers) - 1 && c < TC_CLASSES) atomicAdd(&hist[c], __popc(peers));
@@ -650,9 +761,6 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
                                                             sim->pix_start, sim->pix_cursor, sim->pix_jmin,
                                                             sim->pix_mask, sim->pair_seg, sim->pair_cap,
                                                             sim->d_counters);
-            ++g_lartpc_launches;
-            pair_sort_kernel<<<div_up(ncp, 4), 128, 0, st>>>(ncp, sim->pix_start + cp_lo, sim->pix_count + cp_lo,
-                                                                  sim->pair_seg, sim->pair_cap);
         }
         // index of the first tile of every charged pixel (one tile per window that holds charge)
         LARTPC_CUDA_TRY(lscan::exclusive_scan(ncp, PopcF{sim->pix_mask + cp_lo * MASK_WORDS}, sim->pix_tile0 + cp_lo, false,
@@ -661,8 +769,8 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
         tile_emit_kernel<<<div_up(ncp, 256), 256, 0, st>>>(p, sim->d_tpcs, cp_lo, ncp, sim->pix_tile0,
                                                                 sim->pix_mask, sim->pix_jmin, sim->pix_start,
                                                                 sim->pix_count, sim->tile_cp, sim->tile_desc,
-                                                                sim->tile_list, sim->tile_cap, sim->act_first,
-                                                                sim->act_last, sim->d_counters);
+                                                                sim->tile_list, sim->tile_cap, sim->cell_list,
+                                                                sim->act_first, sim->act_last, sim->d_counters);
         LARTPC_CUDA_TRY(cudaGetLastError());
         // active pixels: slot = rank among active pixels (sorted by id), total waveform samples
         LARTPC_CUDA_TRY(lscan::exclusive_scan(npix, ActiveF{sim->act_last + pix_lo}, sim->act_slot + pix_lo, false,
@@ -683,6 +791,13 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
     const long long *h = sim->h_counters;
     sim->plan_n = n;
     sim->n_tiles = h[CNT_TILES];
+    const int64_t n_cells = h[CNT_CELLS];
+    if (n_cells > 0) {
+        // the atomics of pair_fill_kernel fill each list in arbitrary order: sort it by segment id (one warp per cell)
+        ++g_lartpc_launches;
+        pair_sort_kernel<<<div_up(n_cells, 4), 128, 0, st>>>(n_cells, sim->cell_list, sim->pix_start, sim->pix_count,
+                                                              sim->pair_seg, sim->pair_cap);
+    }
     if (tpc_lo == 0) { sim->need_composite = h[CNT_COMPOSITE] != 0;  sim->boxes_n = n;  sim->boxes_of = (const void *)out->a_lo; }
     if (p.tc_mode && sim->n_tiles > 0) {
         // the FFMA2 splat (bins per pixel other than 5 / 10) writes the operand image in the tiles' original order
@@ -696,10 +811,14 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
             if ((rc = grow_i32_keep(&sim->pair_seg, &sim->pair_cap, h[CNT_PAIRS] + own_cap, h[CNT_PAIRS], st)) != 0) return rc;
         }
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->tb_mask, 0, sizeof(int32_t) * (nt / TC_TILE_BLOCK + 1), st));
-        g_lartpc_launches += 3;
-        tile_class_kernel<<<div_up(nt, 256), 256, 0, st>>>(p, nt, sim->tile_desc, sim->tile_list, sim->pair_seg, *out,
-                                                          (sort && sim->seg_rec_cap >= n) ? sim->seg_rec : nullptr,
-                                                          sim->tile_perm, sim->cls_hist, sort, h[CNT_PAIRS], own_cap);
+        g_lartpc_launches += 4;
+        if (sort)
+            pixel_class_kernel<<<div_up(n_cells, PC_WARPS), 32 * PC_WARPS, 0, st>>>(
+                p, n_cells, sim->cell_list, sim->pix_start, sim->pix_count, sim->pix_tile0, sim->pix_mask, sim->pix_jmin, sim->tile_desc,
+                sim->tile_list, sim->pair_seg, *out, sim->seg_rec_cap >= n ? sim->seg_rec : nullptr, sim->tile_perm,
+                sim->cls_hist, h[CNT_PAIRS], own_cap);
+        else tile_class_flat_kernel<<<div_up(nt, 256), 256, 0, st>>>(nt, sim->tile_perm);
+        class_hist_kernel<<<div_up(nt, 256), 256, 0, st>>>(nt, sim->tile_perm, sim->cls_hist);
         class_offsets_kernel<<<1, 1024, 0, st>>>(sim->cls_hist);
         tile_scatter_kernel<<<div_up(nt, 256), 256, 0, st>>>(nt, sim->tile_perm, sim->cls_hist, sim->tile_desc,
                                                             sim->tile_list, sim->tile_desc_p, sim->tile_list_p,
