@@ -24,7 +24,7 @@ active_table_kernel(int64_t pix0, int64_t n_pix, const int32_t *__restrict__ act
 struct LenF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
 
 constexpr int SUM_THREADS = 128;
-constexpr int SUM_LCAP = 192;      // partial rows listed per round (a pixel usually has W*W x 1.3 of them)
+constexpr int SUM_LCAP = 448;      // partial rows listed per round (W*W x the charge windows of the pixels around: ~30 on a lone track, ~200 in a full spill)
 
 // CTA = active pixel.  Threads d < W*W first list, in parallel, the partial rows that reach the pixel: for target index d
 // of the W x W window and every charge window of that charged pixel, the row of the tile (through the slot map) and the
@@ -101,28 +101,51 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
         __syncthreads();
         const int ne = min(SUM_LCAP, total - r0);
         // a thread owns VEC consecutive ticks starting at a multiple of VEC: window origins are multiples of 4, so that is
-        // one aligned load of a row
-        const int n_al0 = first & ~(VEC - 1);
-        for (int iv = tid; VEC * iv < last - n_al0 + 1; iv += SUM_THREADS) {
-            const int n = n_al0 + VEC * iv;
+        // one aligned load of a row.  A warp owns 32 VEC consecutive ticks: its lanes first find, 32 listed rows at a time,
+        // the rows that reach that span at all (a pixel of a full spill lists ~200 rows, a span meets ~50 of them), then
+        // walk those four at a time -- four independent loads in flight per thread, added in list order.
+        const int n_al0 = first & ~(VEC - 1), lane = tid & 31;
+        for (int iv0 = tid & ~31; VEC * iv0 < last - n_al0 + 1; iv0 += SUM_THREADS) {   // (warp-uniform)
+            const int n = n_al0 + VEC * (iv0 + lane);
+            const int w_lo = n_al0 + VEC * iv0, w_hi = w_lo + 32 * VEC - 1;
+            const bool mine = n <= last;
             float a[VEC];
 #pragma unroll
             for (int k = 0; k < VEC; ++k) a[k] = (r0 && n + k >= first && n + k <= last) ? samples[off + (n + k - first)] : 0.f;
-#pragma unroll 8
-            for (int e = 0; e < ne; ++e) {
-                const int na = e_na[e], nb = e_nb[e];
-                if (n + VEC - 1 >= na && n <= nb) {
-                    float v[VEC];
-                    if (VEC == 4) { const float4 q = __ldcs((const float4 *)(e_row[e] + n)); v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; }
-                    else { const float2 q = __ldcs((const float2 *)(e_row[e] + n)); v[0] = q.x; v[1] = q.y; }
+            for (int e0 = 0; e0 < ne; e0 += 32) {
+                const int e = e0 + lane;
+                unsigned bal = __ballot_sync(0xffffffffu, e < ne && e_nb[e] >= w_lo && e_na[e] <= w_hi);
+                while (bal) {
+                    float v[4][VEC];
+                    int na[4], nb[4];
 #pragma unroll
-                    for (int k = 0; k < VEC; ++k)
-                        if (n + k >= na && n + k <= nb) a[k] += v[k];
+                    for (int i = 0; i < 4; ++i) {
+                        na[i] = INT_MAX;  nb[i] = -1;
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) v[i][k] = 0.f;
+                        if (bal) {
+                            const int x = e0 + __ffs(bal) - 1;
+                            bal &= bal - 1;
+                            const int xa = e_na[x], xb = e_nb[x];
+                            if (mine && n + VEC - 1 >= xa && n <= xb) {
+                                na[i] = xa;  nb[i] = xb;
+                                if (VEC == 4) { const float4 q = __ldcs((const float4 *)(e_row[x] + n)); v[i][0] = q.x; v[i][1] = q.y; v[i][2] = q.z; v[i][3] = q.w; }
+                                else { const float2 q = __ldcs((const float2 *)(e_row[x] + n)); v[i][0] = q.x; v[i][1] = q.y; }
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k)
+                            if (n + k >= na[i] && n + k <= nb[i]) a[k] += v[i][k];
                 }
             }
+            if (mine) {
 #pragma unroll
-            for (int k = 0; k < VEC; ++k)
-                if (n + k >= first && n + k <= last) samples[off + (n + k - first)] = a[k];
+                for (int k = 0; k < VEC; ++k)
+                    if (n + k >= first && n + k <= last) samples[off + (n + k - first)] = a[k];
+            }
         }
         __syncthreads();
     }

@@ -661,3 +661,31 @@ def test_packed_hit_output(lartpc, tile_pixels):
     packed0, offs0 = sim.pack_hits(hits, 0, tile_pixels)
     assert packed0.shape[0] == 0 and np.all(offs0.cpu().numpy() == 0)
     sim.close()
+
+
+def test_tiles_own_lists_run_out_of_room(lartpc):
+    """The plan gives every tile (pixel, 64-tick window) its own segment list behind the pixels' lists, in room for
+    2 n_pairs + 4 096 entries; a tile that finds none keeps the list of its pixel.  Tracks along the drift direction (4.5 cm:
+    ~270 ticks, 4 - 5 windows of every pixel they charge; 4 500 sample points, so the composite node rules run too) need
+    more than that: both kinds of tile are then in one launch and must give the oracle's currents."""
+    base = W.make_config(0)
+    rng = np.random.Generator(np.random.PCG64(4242))
+    side = base.tpcs[0]["nx"] * W.PITCH_CM
+    parts = []
+    for _ in range(1500):
+        x, y, z = rng.uniform(1.0, side - 1.0), rng.uniform(1.0, side - 1.0), rng.uniform(0.3, 4.5)
+        parts.append(W.line_segments([x, y, z], [x + 0.03, y - 0.02, z + 4.5], 10.0, 0.0, lambda s, L, n: np.full(n, 2.1)))
+    seg = {k: np.concatenate([p[k] for p in parts]).astype(np.float32) for k in parts[0]}
+    import dataclasses
+    wl = dataclasses.replace(base, segments=seg, name="drift_direction_tracks")
+    sim = lartpc.Sim(wl.params, wl.tpcs, wl.lut)
+    res = run_staged(sim, wl)
+    dr, pm = _check_segment_stages(res, wl)
+    # the premise, from the pixel mapping itself: own entries >= sum npix x (whole windows spanned) > the room there is
+    span = (pm["jt1"] - pm["jt0"]) // 64
+    nb = int(wl.params["bins_per_pixel"])
+    charged = (pm["a_hi"] // nb - pm["a_lo"] // nb + 1) * (pm["b_hi"] // nb - pm["b_lo"] // nb + 1)   # pixels under the box of bins
+    n_pairs = int(res["info"].n_pairs)
+    assert n_pairs <= int(charged.sum()) and int((charged * span).sum()) > 2 * int(charged.sum()) + 4096, (n_pairs, int(charged.sum()))
+    _check_currents(res, wl, dr, pm, max_pixels=24, seed=3)
+    sim.close()
