@@ -53,7 +53,7 @@ WORKLOAD_NAMES = {
 # DRAM bytes per spill of the tensor-core response measured with ncu on the benched workload and launch configuration
 # (profiles/r2_traffic_c3.md: dram__bytes_read.sum + dram__bytes_write.sum over the 4 launches of one configs[3] spill),
 # keyed by (config, n_segments, n_tiles); any other workload reports the byte model of the plan instead and says so
-MEASURED_RESPONSE_TRAFFIC = {(3, 4805366, 3113102): 57788171776.0 + 82028080640.0}
+MEASURED_RESPONSE_TRAFFIC = {(3, 4805366, 3113102): 62959459328.0 + 82048449024.0}
 
 
 def parse_args():
@@ -394,7 +394,7 @@ def run_ours(args):
                     "traffic_note": "traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu capture "
                                     "of this workload (profiles/r2_traffic_c3.md), null for a workload without one; "
                                     "traffic_model: bytes per launch from the plan and the kernel's counters (charged "
-                                    "operand blocks read once, partial rows written, LUT image once): 0.84 of the measured "
+                                    "operand blocks read once, partial rows written, LUT image once): 0.80 of the measured "
                                     "figure at configs[3]"}
             meas = MEASURED_RESPONSE_TRAFFIC.get((args.config, int(n), int(n_tiles)))
             if meas is not None:
