@@ -79,6 +79,34 @@ def main(cfg: int) -> None:
     for q in (2, 3):
         simulate(bm * 10000 + (alo // q) * 1000 + (ahi // q) * 100 + (blo // q) * 10 + bhi // q,
                  "by block mask and box edges in steps of %d bins" % q)
+    # more of the pattern in the key: which way the charged bins lean (a track's direction across the pixel), how full the box is
+    of = occ.float()
+    cnt = of.sum(dim=(1, 2)).clamp(min=1.0)
+    ia, ib = idx.float().view(1, 10, 1), idx.float().view(1, 1, 10)
+    # occ is [tile][b][a] or [tile][a][b]: the sign of the covariance is the same either way
+    ma, mb = (of * ia).sum(dim=(1, 2)) / cnt, (of * ib).sum(dim=(1, 2)) / cnt
+    cov = (of * ia * ib).sum(dim=(1, 2)) / cnt - ma * mb
+    lean = torch.where(cov > 0.5, 1, torch.where(cov < -0.5, 2, 0))
+    area = ((ahi - alo + 1) * (bhi - blo + 1)).float()
+    fill = (3.0 * (cnt / area).clamp(max=0.999)).long()
+    box2 = (alo // 2) * 1000 + (ahi // 2) * 100 + (blo // 2) * 10 + bhi // 2
+    simulate((bm * 10000 + box2) * 3 + lean, "by block mask, box in steps of 2 and lean of the pattern")
+    simulate(((bm * 10000 + box2) * 3 + lean) * 3 + fill, "... and how full the box is (3 levels)")
+    # the pattern itself as the key (columns of bins, most significant first): identical patterns meet, similar ones mostly do
+    colbits = (occ.long() * (1 << idx.long()).view(1, 1, 10)).sum(dim=2)                      # [tile][10] ten-bit words
+    key = bm.clone()
+    for c in range(10):
+        key = key * 1024 + colbits[:, c]
+        if c == 4:                                                    # (two 50-bit halves: sort by the second, then stably by the first)
+            key_hi, key = key, torch.zeros_like(bm)
+    order = torch.argsort(key, stable=True)
+    order = order[torch.argsort(key_hi[order], stable=True)]
+    ts = T[order]
+    pad = (-nt) % 128
+    if pad:
+        ts = torch.cat([ts, torch.zeros(pad, 100, 4, dtype=torch.bool, device=T.device)])
+    u = ts.reshape(-1, 128, 100, 4).any(dim=1)
+    print("%-52s %9d operands = %.3f of the plan's block masks" % ("by block mask and the pattern read as a number", int(u.sum()), int(u.sum()) / dense_now))
     sim.close()
 
 
