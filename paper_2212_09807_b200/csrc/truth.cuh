@@ -98,6 +98,7 @@ __global__ void __launch_bounds__(TR_THREADS) hit_truth_kernel(const TruthArgs a
     __shared__ float s_best[TR_THREADS / 32];
     __shared__ int s_besti[TR_THREADS / 32];
     __shared__ double s_other;
+    __shared__ int s_cand[TR_THREADS], s_wn[TR_THREADS / 32];       // segments of a list pass whose current can reach the hit
 
     const DevParams &p = a.p;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -135,8 +136,32 @@ __global__ void __launch_bounds__(TR_THREADS) hit_truth_kernel(const TruthArgs a
             const int lstart = a.pix_start[cp], lcount = a.pix_count[cp];
             // bin (al, bl) of the source pixel is seen by the hit's pixel through LUT column (al + nb (H - dx), ...): D5
             const int cx0 = nb * (p.H + dx), cy0 = nb * (p.H + dy);
-            for (int li = 0; li < lcount; ++li) {
-                const int s = a.pair_seg[lstart + li];
+            // the list holds every segment that ever charged the source pixel (~120 over a full spill); the threads first
+            // pick, 128 entries at a time and in list order, those whose current can reach [n0, n_h] at all (two loads each:
+            // a record costs nineteen), then the CTA takes the picked ones one by one
+            for (int base = 0; base < lcount; base += TR_THREADS) {
+            int n_cand;
+            {
+                const int li = base + tid;
+                bool keep = false;
+                int sc = -1;
+                if (li < lcount) {
+                    sc = a.pair_seg[lstart + li];
+                    const int lo = max(a.jt0[sc], 0), hi = min(a.jt1[sc], p.j_max);
+                    keep = lo <= hi && hi + K - 1 >= n0 && lo <= n_h;
+                }
+                const unsigned bal = __ballot_sync(0xffffffffu, keep);
+                __syncthreads();                                    // (the last pass is done with s_cand)
+                if (lane == 0) s_wn[warp] = __popc(bal);
+                __syncthreads();
+                int off = 0;
+                n_cand = 0;
+                for (int w = 0; w < TR_THREADS / 32; ++w) { if (w < warp) off += s_wn[w];  n_cand += s_wn[w]; }
+                if (keep) s_cand[off + __popc(bal & ((1u << lane) - 1u))] = sc;
+                __syncthreads();
+            }
+            for (int qi = 0; qi < n_cand; ++qi) {
+                const int s = s_cand[qi];
                 const SegRec rec = truth_record(a, s);
                 const int J_t = max(rec.jt0, 0) & ~3;
                 SegLocal L;
@@ -230,6 +255,7 @@ __global__ void __launch_bounds__(TR_THREADS) hit_truth_kernel(const TruthArgs a
                         else s_other += share;
                     }
                 }
+            }
             }
         }
     }
