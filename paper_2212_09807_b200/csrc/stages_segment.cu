@@ -329,14 +329,18 @@ pair_sort_kernel(int64_t n_cells, const int32_t *__restrict__ cell_list, const i
         // up to 512: rank sort through shared memory (segment ids are distinct: the rank of an id is the number of smaller
         // ones; n^2 / 32 comparisons per lane on broadcast reads beat a bitonic network that works in global memory --
         // a pixel of a full spill holds ~120 segments)
-        __shared__ int32_t s_list[4][PAIR_RANK_MAX];
+        __shared__ __align__(16) int32_t s_list[4][PAIR_RANK_MAX];
         int32_t *sl = s_list[threadIdx.x >> 5];
-        for (int i = lane; i < cnt; i += 32) sl[i] = v[i];
+        const int cnt4 = (cnt + 3) & ~3;                                // (padded with ids no segment has: never smaller)
+        for (int i = lane; i < cnt4; i += 32) sl[i] = i < cnt ? v[i] : INT32_MAX;
         __syncwarp();
         for (int i = lane; i < cnt; i += 32) {
             const int32_t x = sl[i];
             int r = 0;
-            for (int j = 0; j < cnt; ++j) r += sl[j] < x ? 1 : 0;
+            for (int j = 0; j < cnt4; j += 4) {                         // one broadcast 16-byte read per four comparisons
+                const int4 q = *(const int4 *)(sl + j);
+                r += (q.x < x ? 1 : 0) + (q.y < x ? 1 : 0) + (q.z < x ? 1 : 0) + (q.w < x ? 1 : 0);
+            }
             v[r] = x;
         }
         return;
