@@ -1,5 +1,5 @@
 // Device-wide exclusive prefix sum with an input transform (three launches: block sums, scan of the
-// sums in one block, final scan).  Used for the pre-sizing offsets of S3, the tile / pair /
+// sums in one block, final scan; one launch of one block up to 32 768 elements).  Used for the pre-sizing offsets of S3, the tile / pair /
 // active-pixel compaction and the hit compaction of S6.  Accumulates in 64-bit.
 #pragma once
 #include <cuda_runtime.h>
@@ -101,6 +101,39 @@ __global__ void final_scan_kernel(int64_t n, F f, const long long *sums, Out *ou
     }
 }
 
+// small inputs (the plans of configs[0] / [1], every scan of a small spill): the three steps in one block, one launch
+constexpr int64_t SMALL_N = 16 * TILE;
+template <typename F, typename Out>
+__global__ void small_scan_kernel(int64_t n, F f, Out *out, bool write_last, long long *total_dev)
+{
+    long long carry = 0;
+    for (int64_t base = 0; base < n; base += TILE) {
+        long long vals[ITEMS];
+        long long v = 0;
+#pragma unroll
+        for (int k = 0; k < ITEMS; ++k) {
+            const int64_t i = base + (int64_t)threadIdx.x * ITEMS + k;
+            vals[k] = i < n ? (long long)f(i) : 0;
+            v += vals[k];
+        }
+        long long total;
+        long long ex = block_excl_scan(v, &total) + carry;
+        if (out) {
+#pragma unroll
+            for (int k = 0; k < ITEMS; ++k) {
+                const int64_t i = base + (int64_t)threadIdx.x * ITEMS + k;
+                if (i < n) out[i] = (Out)ex;
+                ex += vals[k];
+            }
+        }
+        carry += total;
+    }
+    if (threadIdx.x == 0) {
+        if (total_dev) *total_dev = carry;
+        if (write_last && out) out[n] = (Out)carry;
+    }
+}
+
 // out[i] = sum_{k<i} f(k) for i in [0, n) (and out[n] = grand total when write_last);
 // *total_dev (optional) receives the grand total.  tmp must hold ceil(n / TILE) + 1 long longs.
 template <typename F, typename Out>
@@ -110,6 +143,11 @@ inline cudaError_t exclusive_scan(int64_t n, F f, Out *out, bool write_last, lon
     if (n <= 0) {
         if (total_dev) cudaMemsetAsync(total_dev, 0, sizeof(long long), st);
         if (write_last && out) cudaMemsetAsync(out, 0, sizeof(Out), st);
+        return cudaGetLastError();
+    }
+    if (n <= SMALL_N) {
+        ++g_lartpc_launches;
+        small_scan_kernel<<<1, THREADS, 0, st>>>(n, f, out, write_last, total_dev);
         return cudaGetLastError();
     }
     int64_t blocks = (n + TILE - 1) / TILE;

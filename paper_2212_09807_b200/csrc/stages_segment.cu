@@ -443,10 +443,19 @@ struct ActiveLenF {
     __device__ long long operator()(int64_t i) const { return last[i] >= 0 ? (long long)(last[i] - first[i] + 1) : 0; }
 };
 
-__global__ void fill_i32_kernel(int32_t *p, int64_t n, int32_t v)
+// the plan's tables of the cells / pixels of the planned TPCs and its counters, back to "nothing charged" (one launch)
+__global__ void __launch_bounds__(256)
+plan_reset_kernel(int64_t ncp, int64_t npix, int32_t *pix_count, int32_t *pix_cursor, unsigned long long *pix_mask, int32_t *pix_jmin,
+                  int32_t *act_first, int32_t *act_last, long long *counters)
 {
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) p[i] = v;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < ncp) {
+        pix_count[i] = 0;  pix_cursor[i] = 0;  pix_jmin[i] = INT32_MAX;
+#pragma unroll
+        for (int wd = 0; wd < MASK_WORDS; ++wd) pix_mask[i * MASK_WORDS + wd] = 0ull;
+    }
+    if (i < npix) { act_first[i] = INT32_MAX;  act_last[i] = -1; }
+    if (i < CNT_COUNT) counters[i] = 0;
 }
 
 int sim_ensure_scan_tmp(lartpc_sim *sim, int64_t elems)
@@ -734,16 +743,11 @@ int launch_plan(lartpc_sim *sim, const lartpc_segments_t *seg, const lartpc_drif
     if (tpc_lo == 0) { sim->boxes_n = -1;  sim->boxes_of = nullptr; }
 
     for (int attempt = 0; attempt < 2; ++attempt) {
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_counters, 0, sizeof(long long) * CNT_COUNT, st));
         // only the cells and pixels of the planned TPCs are touched (lartpc_run_spill plans a few TPCs at a time)
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_count + cp_lo, 0, sizeof(int32_t) * ncp, st));
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_cursor + cp_lo, 0, sizeof(int32_t) * ncp, st));
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->pix_mask + cp_lo * MASK_WORDS, 0, sizeof(unsigned long long) * MASK_WORDS * ncp, st));
-        LARTPC_CUDA_TRY(cudaMemsetAsync(sim->act_last + pix_lo, 0xff, sizeof(int32_t) * npix, st));
         ++g_lartpc_launches;
-        fill_i32_kernel<<<div_up(npix, 256), 256, 0, st>>>(sim->act_first + pix_lo, npix, INT32_MAX);
-        ++g_lartpc_launches;
-        fill_i32_kernel<<<div_up(ncp, 256), 256, 0, st>>>(sim->pix_jmin + cp_lo, ncp, INT32_MAX);
+        plan_reset_kernel<<<div_up(std::max<int64_t>(std::max(ncp, npix), CNT_COUNT), 256), 256, 0, st>>>(
+            ncp, npix, sim->pix_count + cp_lo, sim->pix_cursor + cp_lo, sim->pix_mask + cp_lo * MASK_WORDS, sim->pix_jmin + cp_lo,
+            sim->act_first + pix_lo, sim->act_last + pix_lo, sim->d_counters);
         if (n > 0) {
             ++g_lartpc_launches;
             pixmap_kernel<<<div_up(n, 256), 256, 0, st>>>(p, sim->d_tpcs, s, n, dr->tpc, dr->q_anode, tpc_lo, tpc_hi,
