@@ -655,19 +655,31 @@ __global__ void __launch_bounds__(256) class_hist_kernel(int64_t n_tiles, const 
 // hist[0 .. TC_CLASSES) counts -> hist[TC_CLASSES .. 2 TC_CLASSES) first slot of the class (one CTA of 1024 threads)
 __global__ void __launch_bounds__(1024) class_offsets_kernel(int32_t *hist)
 {
-    __shared__ int s_part[1024];
+    __shared__ int s_part[32];
     constexpr int PER = (TC_CLASSES + 1023) / 1024;
     const int k0 = threadIdx.x * PER;
     int sum = 0;
     for (int k = k0; k < min(k0 + PER, TC_CLASSES); ++k) sum += hist[k];
-    s_part[threadIdx.x] = sum;
+    // exclusive scan of the 1 024 partial sums: within warps by shuffles, then over the 32 warp totals
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    int inc = sum;
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += y;
+    }
+    if (lane == 31) s_part[wp] = inc;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        int run = 0;
-        for (int i = 0; i < 1024; ++i) { const int v = s_part[i];  s_part[i] = run;  run += v; }
+    if (wp == 0) {
+        const int t = s_part[lane];
+        int ti = t;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, ti, o);
+            if (lane >= o) ti += y;
+        }
+        s_part[lane] = ti - t;
     }
     __syncthreads();
-    int run = s_part[threadIdx.x];
+    int run = s_part[wp] + inc - sum;
     for (int k = k0; k < min(k0 + PER, TC_CLASSES); ++k) { hist[TC_CLASSES + k] = run;  run += hist[k]; }
 }
 
