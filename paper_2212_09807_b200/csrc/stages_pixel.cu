@@ -26,11 +26,10 @@ struct LenF { const int32_t *v; __device__ long long operator()(int64_t i) const
 constexpr int SUM_THREADS = 128;
 constexpr int SUM_LCAP = 448;      // partial rows listed per round (W*W x the charge windows of the pixels around: ~30 on a lone track, ~200 in a full spill)
 
-// CTA = active pixel.  Threads d < W*W first list, in parallel, the partial rows that reach the pixel: for target index d
-// of the W x W window and every charge window of that charged pixel, the row of the tile (through the slot map) and the
-// ticks it can be non-zero on.  Then a thread owns the ticks i = tid mod 128 of the waveform and adds the listed rows in
-// list order (d ascending, window ascending): the loads of one tick are independent of each other, the row reads of a
-// warp are coalesced, and the order of the float32 additions -- hence every output bit -- is fixed.
+// CTA = active pixel.  Its threads first list, one row each and all at once, the partial rows that reach the pixel: for target
+// index d of the W x W window and every charge window of that charged pixel (d ascending, window ascending), the row of the
+// tile (through the slot map) and the ticks it can be non-zero on.  Then a thread owns VEC consecutive ticks of the waveform
+// and adds the listed rows in list order: the order of the float32 additions -- hence every output bit -- is fixed.
 template <int VEC, bool PIECES>    // VEC: ticks per thread and load, 4 when tile_ticks is a multiple of 4 (rows 16-byte aligned), else 2
                                    // PIECES: a long LUT cut into pieces (tensor-core path, K > 209): nq rows per (tile, target)
 __global__ void __launch_bounds__(SUM_THREADS)
@@ -47,8 +46,7 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
     __shared__ int e_na[SUM_LCAP], e_nb[SUM_LCAP];
     const int slot = blockIdx.x, tid = threadIdx.x;
     const int gp = pixel_id[slot];
-    int tpc = 0;
-    while (tpc + 1 < p.n_tpcs && tpcs[tpc + 1].first_pixel_id <= gp) ++tpc;
+    const int tpc = tpc_of_pixel(tpcs, p.n_tpcs, gp);
     const DevTpc &t = tpcs[tpc];
     const int rel = gp - t.first_pixel_id, iy = rel / t.nx, ix = rel - iy * t.nx;
     const int first = first_tick[slot], len = length[slot], last = first + len - 1;
@@ -75,28 +73,28 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
     const int total = s_base[p.WW] * nq;
     const int64_t off = offset[slot];
     for (int r0 = 0; r0 < total; r0 += SUM_LCAP) {
-        if (tid < p.WW) {
-            const int d = tid, js = s_js[d];
-            int tix = s_tile0[d], gi = s_base[d] * nq - r0;
-#pragma unroll
-            for (int wd = 0; wd < MASK_WORDS; ++wd)
-                for (unsigned long long m = s_mask[d][wd]; m; m &= m - 1, ++tix, gi += nq) {
-                    if (gi + nq <= 0 || gi >= SUM_LCAP) continue;
-                    const int w = 64 * wd + __ffsll((long long)m) - 1;
-                    const int ts = tile_perm ? tile_perm[tix] : tix;
-                    const int2 rg = *(const int2 *)(tile_range + TILE_META * ts);       // first / last output block
-                    const int j_start = js + w * p.Jc;
-#pragma unroll 1
-                    for (int q = 0; q < nq; ++q) {                                      // piece q answers KQ q ticks later
-                        const int g = gi + q;
-                        if (g < 0 || g >= SUM_LCAP) continue;
-                        const int t0 = PIECES ? p.KQ * q : 0;
-                        const int lo = max(rg.x * RESP_NO, t0), hi = min(rg.y * RESP_NO + RESP_NO - 1, t0 + p.tile_ticks - 1);
-                        e_row[g] = partial + (((size_t)ts * p.WW + d) * nq + q) * p.tile_ticks - (j_start + t0);
-                        e_na[g] = (rg.x > rg.y || lo > hi) ? INT_MAX : max(first, j_start + lo);
-                        e_nb[g] = (rg.x > rg.y || lo > hi) ? -1 : min(last, j_start + hi);
-                    }
-                }
+        // one thread per listed row (all of them at once: the row's tile and tick range are two dependent gathers)
+        for (int g = tid; g < min(SUM_LCAP, total - r0); g += SUM_THREADS) {
+            const int pr = (g + r0) / nq, q = (g + r0) - pr * nq;     // (target, window) pair of the pixel; piece of a long LUT
+            int d = 0;                                                // its target: the last d with s_base[d] <= pr
+            for (int step = 64; step; step >>= 1)
+                if (d + step < p.WW && s_base[d + step] <= pr) d += step;
+            int r = pr - s_base[d];                                   // ... and window: the r-th set bit of that pixel's mask
+            const int tix = s_tile0[d] + r;
+            unsigned long long m = s_mask[d][0];
+            int wbase = 0;
+            static_assert(MASK_WORDS == 2, "two 64-bit window words per charged pixel");
+            if (r >= __popcll(m)) { r -= __popcll(m);  m = s_mask[d][1];  wbase = 64; }
+            for (int i = 0; i < r; ++i) m &= m - 1;
+            const int w = wbase + __ffsll((long long)m) - 1;
+            const int ts = tile_perm ? tile_perm[tix] : tix;
+            const int2 rg = *(const int2 *)(tile_range + TILE_META * ts);       // first / last output block
+            const int j_start = s_js[d] + w * p.Jc;
+            const int t0 = PIECES ? p.KQ * q : 0;                                // piece q answers KQ q ticks later
+            const int lo = max(rg.x * RESP_NO, t0), hi = min(rg.y * RESP_NO + RESP_NO - 1, t0 + p.tile_ticks - 1);
+            e_row[g] = partial + (((size_t)ts * p.WW + d) * nq + q) * p.tile_ticks - (j_start + t0);
+            e_na[g] = (rg.x > rg.y || lo > hi) ? INT_MAX : max(first, j_start + lo);
+            e_nb[g] = (rg.x > rg.y || lo > hi) ? -1 : min(last, j_start + hi);
         }
         __syncthreads();
         const int ne = min(SUM_LCAP, total - r0);

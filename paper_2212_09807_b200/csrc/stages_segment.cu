@@ -394,8 +394,7 @@ tile_emit_kernel(DevParams p, const DevTpc *__restrict__ tpcs, int64_t cp0, int6
         base = __shfl_sync(act, base, leader) + __popc(act & ((1u << lane) - 1u));
         if (base < tile_cap) cell_list[base] = (int32_t)cp;
     }
-    int tpc = 0;
-    while (tpc + 1 < p.n_tpcs && tpcs[tpc + 1].cp_base <= cp) ++tpc;
+    const int tpc = tpc_of_cell(tpcs, p.n_tpcs, cp);
     const DevTpc &t = tpcs[tpc];
     int rel = (int)(cp - t.cp_base);
     int px = rel % t.gw - p.H, py = rel / t.gw - p.H;
