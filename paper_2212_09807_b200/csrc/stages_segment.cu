@@ -535,7 +535,14 @@ pixel_class_kernel(DevParams p, int64_t n_cells, const int32_t *__restrict__ cel
     int *w0s = s_w0[wp], *w1s = s_w1[wp], *ns = s_n[wp];
     for (int r = lane; r < nt; r += 32) { w0s[r] = 0;  w1s[r] = 0;  ns[r] = 0; }
     __syncwarp();
-    auto has = [&](int w) { return w < 64 ? (m0 >> w & 1ull) != 0ull : (m1 >> (w - 64) & 1ull) != 0ull; };
+    // the bits of a mask word (windows base .. base + 63) that lie in windows [lo, hi]
+    auto clip = [](unsigned long long m, int base, int lo, int hi) {
+        lo -= base;  hi -= base;
+        if (hi < 0 || lo > 63) return 0ull;
+        if (lo > 0) m &= ~0ull << lo;
+        if (hi < 63) m &= (2ull << hi) - 1ull;
+        return m;
+    };
     auto rank = [&](int w) { return w < 64 ? __popcll(m0 & ((1ull << w) - 1ull)) : __popcll(m0) + __popcll(m1 & ((1ull << (w - 64)) - 1ull)); };
     auto fdiv = [&](int x) { return x >= 0 ? x / p.Jc : -((-x + p.Jc - 1) / p.Jc); };
     // segment k of the list: its id, the windows [wlo, whi] it reaches, its ticks clamped to the read-out, its bins on this pixel
@@ -566,8 +573,9 @@ pixel_class_kernel(DevParams p, int64_t n_cells, const int32_t *__restrict__ cel
         int sid, wlo, whi, t0, t1, abits, bbits;
         load(k0 + lane, sid, wlo, whi, t0, t1, abits, bbits);
         const int c_lo = __reduce_min_sync(0xffffffffu, wlo), c_hi = __reduce_max_sync(0xffffffffu, whi);
-        for (int w = c_lo; w <= c_hi; ++w) {
-            if (!has(w)) continue;
+        for (int wd = 0; wd < MASK_WORDS; ++wd)
+        for (unsigned long long mm = clip(wd ? m1 : m0, 64 * wd, c_lo, c_hi); mm; mm &= mm - 1) {   // the pixel's windows in [c_lo, c_hi]
+            const int w = 64 * wd + __ffsll((long long)mm) - 1;
             const bool m = wlo <= w && w <= whi;
             const unsigned bal = __ballot_sync(0xffffffffu, m);
             if (!bal) continue;
@@ -618,8 +626,9 @@ pixel_class_kernel(DevParams p, int64_t n_cells, const int32_t *__restrict__ cel
         int sid, wlo, whi, t0, t1, abits, bbits;
         load(k0 + lane, sid, wlo, whi, t0, t1, abits, bbits);
         const int c_lo = __reduce_min_sync(0xffffffffu, wlo), c_hi = __reduce_max_sync(0xffffffffu, whi);
-        for (int w = c_lo; w <= c_hi; ++w) {
-            if (!has(w)) continue;
+        for (int wd = 0; wd < MASK_WORDS; ++wd)
+        for (unsigned long long mm = clip(wd ? m1 : m0, 64 * wd, c_lo, c_hi); mm; mm &= mm - 1) {   // the pixel's windows in [c_lo, c_hi]
+            const int w = 64 * wd + __ffsll((long long)mm) - 1;
             const bool m = wlo <= w && w <= whi;
             const unsigned bal = __ballot_sync(0xffffffffu, m);
             if (!bal) continue;
