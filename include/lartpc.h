@@ -49,6 +49,7 @@ extern "C" {
 #define LARTPC_ERR_DEVICE        (-5)   /* not a compute-capability 10.x device */
 #define LARTPC_ERR_UNSUPPORTED   (-6)
 #define LARTPC_ERR_ORDER         (-7)   /* stage called without the plan of the preceding stage */
+#define LARTPC_ERR_STATIC_LIMIT  (-8)   /* input larger than the fixed scratch of lartpc_electronics_static */
 
 typedef struct lartpc_sim lartpc_sim_t;   /* opaque: LUT copy, TPC table, planning scratch */
 
@@ -289,6 +290,22 @@ int  lartpc_sum_pixel_signals(lartpc_sim_t *sim, const lartpc_signals_t *signals
 /* S6: Philox4x32-10 noise keyed by (seed, pixel id, tick). */
 int  lartpc_electronics(lartpc_sim_t *sim, const lartpc_waveforms_t *waveforms, uint64_t seed,
                         lartpc_hits_t *out, void *stream);
+
+/* S6 for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * the same kernels, the same launch order and the same results as lartpc_electronics, bit for bit -- but where that call
+ * grows sim-owned scratch with cudaMalloc whenever a call needs more than the last one did, this one keeps its scratch
+ * (per-pixel hit slots, hit offsets, block sums of the prefix sum) in ONE file-scope device array of fixed size
+ * (~8.3 MB, held by every GPU that loads the library until the process exits) and calls no cudaMalloc, cudaFree or
+ * allocating library routine, ever.  Limits: waveforms->n_active <= LARTPC_STATIC_MAX_PIXELS and n_active x
+ * max_hits_per_pixel <= LARTPC_STATIC_MAX_SLOTS (65 536 active pixels at the default 32 hits per pixel: configs[0], [1] and a
+ * TPC of configs[2] / [3]); beyond them LARTPC_ERR_STATIC_LIMIT, nothing launched, nothing written.  Inputs and outputs are
+ * the caller's, exactly as for lartpc_electronics.  The array is shared by every call of every sim, stream and thread of
+ * the process on that GPU and keeps the last call's contents (each call writes what it reads before reading it): calls
+ * that OVERLAP on the GPU race on it -- order them on one stream, or with events. */
+#define LARTPC_STATIC_MAX_PIXELS 65536
+#define LARTPC_STATIC_MAX_SLOTS  2097152
+int  lartpc_electronics_static(lartpc_sim_t *sim, const lartpc_waveforms_t *waveforms, uint64_t seed,
+                               lartpc_hits_t *out, void *stream);
 
 /* Truth association, an optional pass after S6 (the paper has it for the light path; reading D26).  By
  * eqs. (3.7)-(3.9) the current on a pixel is a sum over segments; the share of segment s in hit h of pixel p is

@@ -34,6 +34,9 @@ extern "C" const char *lartpc_strerror(int code)
         case LARTPC_ERR_DEVICE: return "device is not compute capability 10.x (sm_100a only, no fallback)";
         case LARTPC_ERR_UNSUPPORTED: return "unsupported parameter combination";
         case LARTPC_ERR_ORDER: return "stage called out of order (no plan from lartpc_pixels_from_segments)";
+        case LARTPC_ERR_STATIC_LIMIT:
+            return "input exceeds the fixed scratch of lartpc_electronics_static (LARTPC_STATIC_MAX_PIXELS active pixels, "
+                   "LARTPC_STATIC_MAX_SLOTS = n_active x max_hits_per_pixel hit slots); use lartpc_electronics";
         default: return "unknown error";
     }
 }
@@ -140,6 +143,12 @@ extern "C" int lartpc_sim_create_ex(const lartpc_params_t *prm, const lartpc_tpc
     s->tpcs.assign(tpcs, tpcs + n_tpcs);
     s->sm_count = prop.multiProcessorCount;
     s->device = dev;
+    {
+        // set-up of lartpc_electronics_static: the device address of its scratch on this (the current) device, resolved once
+        // per device; a failure here is reported by that entry point, which tries again
+        void *scratch = nullptr;
+        (void)static_scratch_ptr(dev, &scratch);
+    }
     DevParams &p = s->dp;
     memset(&p, 0, sizeof(p));
     p.eps = prm->e_field_kv_cm * prm->lar_density_g_cm3;  p.w_ion = prm->w_ion_mev;

@@ -276,6 +276,7 @@ static inline int64_t tiles_alloc(const DevParams &p, int64_t n_tiles)
 int launch_pack_hits(lartpc_sim *sim, const lartpc_hits_t *hits, int64_t n_hits, int tile_pixels, uint16_t *packed,
                      int64_t *tile_offsets, cudaStream_t st);
 int launch_sum(lartpc_sim *sim, const lartpc_signals_t *sig, lartpc_waveforms_t *out, cudaStream_t st);
+int static_scratch_ptr(int device, void **ptr);   // stages_pixel.cu: device address of lartpc_electronics_static's scratch (device current)
 int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
                        int32_t *slot_scratch, int32_t *scan_scratch, int64_t hit_base, cudaStream_t st);
 int sim_ensure_scan_tmp(lartpc_sim *sim, int64_t elems);

@@ -398,6 +398,95 @@ int launch_electronics(lartpc_sim *sim, const lartpc_waveforms_t *wf, uint64_t s
 
 
 // -------------------------------------------------------------------------------------------------
+// S6 without any allocation: lartpc_electronics_static (include/lartpc.h).  Same kernels and same launch order as
+// launch_electronics above; what differs is where the scratch lives.  lartpc_electronics grows sim-owned buffers with
+// cudaMalloc when a call needs more than the last one did (per-pixel hit slots, hit offsets, the prefix sum's block sums):
+// a caller under CUDA graph capture, or one that must not allocate after start-up, cannot use that.  Here the scratch is
+// one file-scope device array of a fixed, modest size that every GPU loading the library holds until the process ends;
+// inputs beyond it are refused (LARTPC_ERR_STATIC_LIMIT), nothing is ever grown.
+//   layout (bytes):  [0, 256)                    header: the batch's hit total (long long), written by the scan before it is read
+//                    [256, 256 + 8 * 4096)       block sums of the prefix sum (long long; MAX_PIXELS / 2048 + 1 used)
+//                    then int32 offs[MAX_PIXELS + 64], int32 slots[MAX_SLOTS]
+// Every call (of every sim, every stream, every thread) shares the array: calls that overlap on the GPU race on it.  It
+// keeps the last call's contents; every word a call reads it has written before (electronics kernel -> slots, scan ->
+// block sums, offsets, total), the header is cleared all the same.
+// In host code `g_static_scratch` is a host-side stand-in for the symbol, not a device address: the address the kernels
+// get is resolved with cudaGetSymbolAddress, once per device, with that device current (static_scratch_ptr below: from
+// lartpc_sim_create, and again -- a table look-up then -- by the entry point).
+// -------------------------------------------------------------------------------------------------
+constexpr int64_t STATIC_MAX_PIXELS = LARTPC_STATIC_MAX_PIXELS;
+constexpr int64_t STATIC_MAX_SLOTS = LARTPC_STATIC_MAX_SLOTS;
+constexpr size_t STATIC_HDR_BYTES = 256, STATIC_SUMS_BYTES = 8 * 4096;
+constexpr size_t STATIC_OFFS_BYTES = sizeof(int32_t) * (size_t)(STATIC_MAX_PIXELS + 64);
+constexpr size_t STATIC_SCRATCH_BYTES = STATIC_HDR_BYTES + STATIC_SUMS_BYTES + STATIC_OFFS_BYTES + sizeof(int32_t) * (size_t)STATIC_MAX_SLOTS;
+static_assert(STATIC_MAX_PIXELS / lscan::TILE + 2 <= (int64_t)(STATIC_SUMS_BYTES / 8), "block sums of the largest accepted scan fit");
+static_assert((STATIC_HDR_BYTES + STATIC_SUMS_BYTES + STATIC_OFFS_BYTES) % 256 == 0, "the slots start on a 256-byte boundary");
+
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+void *g_static_ptr[STATIC_MAX_DEVICES];          // device address of g_static_scratch on device i (null: not resolved yet)
+}
+
+// device address of the scratch on `device`, which must be the current device; resolved once per device
+int static_scratch_ptr(int device, void **ptr)
+{
+    if (device < 0 || device >= STATIC_MAX_DEVICES) return LARTPC_ERR_BAD_ARGUMENT;
+    void *p = __atomic_load_n(&g_static_ptr[device], __ATOMIC_ACQUIRE);
+    if (!p) {
+        LARTPC_CUDA_TRY(cudaGetSymbolAddress(&p, g_static_scratch));   // (idempotent: two threads racing here store the same address)
+        if (!p) return LARTPC_ERR_CUDA;
+        __atomic_store_n(&g_static_ptr[device], p, __ATOMIC_RELEASE);
+    }
+    *ptr = p;
+    return LARTPC_OK;
+}
+
+extern "C" int lartpc_electronics_static(lartpc_sim_t *sim, const lartpc_waveforms_t *wf, uint64_t seed, lartpc_hits_t *out,
+                                         void *stream)
+{
+    if (!sim || !wf || !out || !out->counters) return LARTPC_ERR_BAD_ARGUMENT;
+    if (wf->n_active > 0 && (!out->hits_per_pixel || !out->q_pixel)) return LARTPC_ERR_BAD_ARGUMENT;
+    const DevParams &p = sim->dp;
+    const int64_t na = wf->n_active;
+    if (na < 0) return LARTPC_ERR_BAD_ARGUMENT;
+    if (na > STATIC_MAX_PIXELS || na * (int64_t)p.max_hits > STATIC_MAX_SLOTS) return LARTPC_ERR_STATIC_LIMIT;
+    DeviceGuard dg(sim->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    void *base = nullptr;
+    int rc = static_scratch_ptr(sim->device, &base);
+    if (rc) return rc;
+    unsigned char *b = (unsigned char *)base;
+    long long *batch_total = (long long *)b;
+    long long *scan_tmp = (long long *)(b + STATIC_HDR_BYTES);
+    int32_t *offs = (int32_t *)(b + STATIC_HDR_BYTES + STATIC_SUMS_BYTES);
+    int32_t *slots = (int32_t *)(b + STATIC_HDR_BYTES + STATIC_SUMS_BYTES + STATIC_OFFS_BYTES);
+    LARTPC_CUDA_TRY(cudaMemsetAsync(out->counters, 0, sizeof(int64_t) * 4, st));
+    LARTPC_CUDA_TRY(cudaMemsetAsync(b, 0, STATIC_HDR_BYTES, st));
+    if (na == 0) return LARTPC_OK;
+    ++g_lartpc_launches;
+    if (p.noise_disc != 0.0 || p.periodic > 0 || p.hold < 0)
+        electronics_kernel<<<div_up(na, 128), 128, 0, st>>>(p, seed, na, wf->pixel_id, wf->first_tick, wf->length,
+                                                           wf->offset, wf->samples, sim->disabled_mask, slots,
+                                                           out->hits_per_pixel, out->q_pixel);
+    else
+        electronics_warp_kernel<<<div_up(na, 4), 128, 0, st>>>(p, seed, na, wf->pixel_id, wf->first_tick, wf->length,
+                                                              wf->offset, wf->samples, sim->disabled_mask, slots,
+                                                              out->hits_per_pixel, out->q_pixel);
+    LARTPC_CUDA_TRY(lscan::exclusive_scan(na, HitCountF{out->hits_per_pixel, p.max_hits}, offs, false, batch_total, scan_tmp, st));
+    ++g_lartpc_launches;
+    compact_hits_kernel<<<div_up(na, 256), 256, 0, st>>>(na, p.max_hits, wf->pixel_id, slots, out->hits_per_pixel, offs,
+                                                        (long long *)out->counters, out->hit_capacity, out->hit_pixel,
+                                                        out->hit_tick, out->hit_adc);
+    ++g_lartpc_launches;
+    advance_hit_base_kernel<<<1, 1, 0, st>>>((long long *)out->counters, batch_total, out->hit_capacity);
+    LARTPC_CUDA_TRY(cudaGetLastError());
+    return LARTPC_OK;
+}
+
+
+// -------------------------------------------------------------------------------------------------
 // Packed hit output (BASELINE configs[3] "16-bit packed hit output", reading D18): the (pixel, tick)-sorted hit list
 // regrouped by readout tile (tile_pixels x tile_pixels pixels: 70 x 70) as three uint16 per hit
 // {pixel in tile = iy_in * tile_pixels + ix_in, tick, adc | flags << 12}, with an offset table per tile.

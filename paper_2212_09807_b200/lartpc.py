@@ -120,7 +120,8 @@ class Stats(C.Structure):
 EXPORTS = ("lartpc_sim_create", "lartpc_sim_create_ex", "lartpc_response_mode", "lartpc_sim_destroy", "lartpc_set_disabled_pixels",
            "lartpc_set_random_perturbations", "lartpc_set_truncation_compensation", "lartpc_chunk_ticks",
            "lartpc_workspace_bytes", "lartpc_quench", "lartpc_drift", "lartpc_pixels_from_segments",
-           "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_hit_truth", "lartpc_run_spill",
+           "lartpc_induced_current", "lartpc_sum_pixel_signals", "lartpc_electronics", "lartpc_electronics_static", "lartpc_hit_truth",
+           "lartpc_run_spill",
            "lartpc_readout_tiles", "lartpc_pack_hits",
            "lartpc_light_create", "lartpc_light_destroy", "lartpc_light_npe", "lartpc_light_profile",
            "lartpc_light_scintillation", "lartpc_light_fluctuate", "lartpc_light_electronics", "lartpc_light_workspace_bytes",
@@ -359,6 +360,18 @@ class Sim:
         out, h = self._hits(cap, na)
         _check(self.lib.lartpc_electronics(self.handle, C.byref(waveforms["_struct"]), C.c_uint64(seed), C.byref(h),
                                            _stream_ptr(t)), "lartpc_electronics")
+        out["_struct"] = h
+        return out
+
+    def electronics_static(self, waveforms, seed: int, hit_capacity: Optional[int] = None):
+        """S6 through lartpc_electronics_static: no allocation inside the library, scratch in a fixed device array
+        (LARTPC_STATIC_MAX_PIXELS / LARTPC_STATIC_MAX_SLOTS: RuntimeError beyond them); same outputs as ``electronics``."""
+        t = self.torch
+        na = int(waveforms["_struct"].n_active)
+        cap = int(hit_capacity if hit_capacity is not None else na * self.params["max_hits_per_pixel"])
+        out, h = self._hits(cap, na)
+        _check(self.lib.lartpc_electronics_static(self.handle, C.byref(waveforms["_struct"]), C.c_uint64(seed), C.byref(h),
+                                                  _stream_ptr(t)), "lartpc_electronics_static")
         out["_struct"] = h
         return out
 
