@@ -88,7 +88,10 @@ constexpr int RESP_NO = 14;          // output ticks per response task (one thre
 constexpr int RESP_CONSUMERS = 256;  // consumer threads of the response kernel (8 warps, two per SM sub-partition)
 constexpr int TILE_META = 4;         // ints per tile in lartpc_signals_t.tile_range: first / last output block, scale exponent, 0
 constexpr int TC_TILE_BLOCK = 128;   // tiles per tensor-core tile block (MMA M of one CTA)
-constexpr bool TC_CTA_PAIR = false;  // the tensor-core response runs as CTA pairs (cta_group::2, M = 256 over two tile blocks)
+#ifndef LARTPC_CTA_PAIR
+#define LARTPC_CTA_PAIR 0
+#endif
+constexpr bool TC_CTA_PAIR = LARTPC_CTA_PAIR != 0;  // the tensor-core response runs as CTA pairs (cta_group::2, M = 256 over two tile blocks)
 constexpr int TC_UNIT_TILES = TC_CTA_PAIR ? 2 * TC_TILE_BLOCK : TC_TILE_BLOCK;   // tiles one response item multiplies at once:
                                      // the 16-tick block masks (tb_mask) are kept per unit
 
