@@ -3,7 +3,7 @@
 //     C[b][a][j] = sum_seg sum_mu (Q_a / N) wx_mu[a] wy_mu[b] wt_mu[j]
 // is, per tile, the matrix product  D[m = b nb + a][j] = sum_s WXY[m][s] WT[j][s]  over the samples s of every segment
 // that crosses the tile: M = 128 cell rows (nb^2 = 100 used), N = 64 arrival ticks, K = samples.  Persistent CTAs of
-// 128 threads (four per SM) take tiles from an atomic cursor; 64 samples per batch: warps 0-1 build the WXY operand of
+// 128 threads (five per SM) take tiles from an atomic cursor; 48 samples per batch: warps 0-1 build the WXY operand of
 // their sample (11 + 11 erf, 100 products), warps 2-3 the WT operand (up to 65 erf), both split hi + lo in fp16 and
 // stored MN-major (a thread writes 16-byte runs of cells / ticks of its own sample column: conflict-free STS.128) in the
 // canonical un-swizzled UMMA layout; thread 0 then issues 3 x ceil(samples / 16) tcgen05.mma (hi hi + hi lo + lo hi)
@@ -24,7 +24,16 @@ __device__ unsigned long long g_ct_dbg[16];   // measurement build: thread 0's c
 #define CT_T(x)
 #define CT_ADD(i, v)
 #endif
-constexpr int CT_KB = 64;                              // samples per batch
+#ifndef LARTPC_CT_KB
+#define LARTPC_CT_KB 48
+#endif
+#ifndef LARTPC_CT_CTAS
+#define LARTPC_CT_CTAS 5
+#endif
+// 48 columns per batch and five CTAs per SM (44 KB of shared memory and 96 registers each) against 64 and four: charge
+// lattice 62.2 -> 60.3 - 61.2 ms at configs[3], hit lists bit-identical (A/B on one box; 32 and six: 61.9 ms)
+constexpr int CT_KB = LARTPC_CT_KB;                      // samples per batch (a multiple of 16, at most 64: one thread of a role per column)
+static_assert(CT_KB % 16 == 0 && CT_KB >= 16 && CT_KB <= 64, "operand columns of a batch");
 constexpr int CT_A_HALF = 128 * CT_KB * 2;             // bytes of one precision half of the WXY operand (16 KB)
 constexpr int CT_B_HALF = 64 * CT_KB * 2;              // ... of the WT operand (8 KB)
 // per-segment record of the splat, written once per S4 call (coalesced) and gathered by the tiles
@@ -187,7 +196,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 template <int NB, bool RND, bool COMP>   // RND: eq. (3.9) as printed, p.rnd_m random perturbations per sample point
                                         // COMP: composite node rules for segments beyond the largest rule
-__global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const SplatArgs a)
+__global__ void __launch_bounds__(CT_THREADS, LARTPC_CT_CTAS) charge_lattice_tc_kernel(const SplatArgs a)
 {
     extern __shared__ unsigned char smem_dyn[];
     const DevParams &p = a.p;
@@ -234,8 +243,8 @@ __global__ void __launch_bounds__(CT_THREADS, 4) charge_lattice_tc_kernel(const 
     // instruction descriptor: D fp32, A / B fp16, both MN-major, N = 64, M = 128
     const uint32_t idesc = (1u << 4) | (1u << 15) | (1u << 16) | ((uint32_t)(64 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 
-    const int s_in = tid & (CT_KB - 1);                              // sample column of this thread
-    const bool role_a = tid < CT_KB;                                 // warps 0-1: WXY, warps 2-3: WT
+    const int s_in = tid & 63;                                       // sample column of this thread
+    const bool role_a = tid < 64;                                    // warps 0-1: WXY, warps 2-3: WT
     uint32_t mma_phase = 0;
     int slot = 0;                                                    // ring position of the current tile
     bool have_rec = false;                                           // s_rec holds the first chunk of the current tile

@@ -694,7 +694,7 @@ int launch_current_splat(lartpc_sim *sim, const lartpc_drifted_t *dr, const lart
         a.rec = sim->seg_rec;  a.work = sim->d_work;  a.n_tiles = (int)sim->n_tiles;
         a.tile_desc = sim->tile_desc_p;  a.tile_list = sim->tile_list_p;        // physical (sorted) tile order
         LARTPC_CUDA_TRY(cudaMemsetAsync(sim->d_work, 0, sizeof(int), st));
-        const unsigned grid = (unsigned)std::min<int64_t>(sim->n_tiles, 4 * (int64_t)sim->sm_count);
+        const unsigned grid = (unsigned)std::min<int64_t>(sim->n_tiles, LARTPC_CT_CTAS * (int64_t)sim->sm_count);
         ++g_lartpc_launches;
         if (p.rnd_m > 0) {
             if (p.nb == 10) charge_lattice_tc_kernel<10, true, false><<<grid, CT_THREADS, CT_SMEM, st>>>(a);
