@@ -23,6 +23,10 @@ active_table_kernel(int64_t pix0, int64_t n_pix, const int32_t *__restrict__ act
 
 struct LenF { const int32_t *v; __device__ long long operator()(int64_t i) const { return v[i]; } };
 
+#ifndef LARTPC_SUM_MLP
+#define LARTPC_SUM_MLP 4
+#endif
+constexpr int SUM_MLP = LARTPC_SUM_MLP;   // listed rows a thread loads before it adds them (in list order); measured at configs[3]: 4 -> 21.5 ms, 6 -> 22.0, 8 -> 24.4
 constexpr int SUM_THREADS = 128;
 constexpr int SUM_LCAP = 448;      // partial rows listed per round (W*W x the charge windows of the pixels around: ~30 on a lone track, ~200 in a full spill)
 
@@ -114,10 +118,10 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
                 const int e = e0 + lane;
                 unsigned bal = __ballot_sync(0xffffffffu, e < ne && e_nb[e] >= w_lo && e_na[e] <= w_hi);
                 while (bal) {
-                    float v[4][VEC];
-                    int na[4], nb[4];
+                    float v[SUM_MLP][VEC];
+                    int na[SUM_MLP], nb[SUM_MLP];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
+                    for (int i = 0; i < SUM_MLP; ++i) {
                         na[i] = INT_MAX;  nb[i] = -1;
 #pragma unroll
                         for (int k = 0; k < VEC; ++k) v[i][k] = 0.f;
@@ -133,7 +137,7 @@ sum_pixel_kernel(DevParams p, const DevTpc *__restrict__ tpcs, const int32_t *__
                         }
                     }
 #pragma unroll
-                    for (int i = 0; i < 4; ++i)
+                    for (int i = 0; i < SUM_MLP; ++i)
 #pragma unroll
                         for (int k = 0; k < VEC; ++k)
                             if (n + k >= na[i] && n + k <= nb[i]) a[k] += v[i][k];
