@@ -3,7 +3,7 @@
 //     C[b][a][j] = sum_seg sum_mu (Q_a / N) wx_mu[a] wy_mu[b] wt_mu[j]
 // is, per tile, the matrix product  D[m = b nb + a][j] = sum_s WXY[m][s] WT[j][s]  over the samples s of every segment
 // that crosses the tile: M = 128 cell rows (nb^2 = 100 used), N = 64 arrival ticks, K = samples.  Persistent CTAs of
-// 128 threads (five per SM) take tiles from an atomic cursor; 48 samples per batch: warps 0-1 build the WXY operand of
+// 128 threads (four per SM) take tiles from an atomic cursor; 64 samples per batch: warps 0-1 build the WXY operand of
 // their sample (11 + 11 erf, 100 products), warps 2-3 the WT operand (up to 65 erf), both split hi + lo in fp16 and
 // stored MN-major (a thread writes 16-byte runs of cells / ticks of its own sample column: conflict-free STS.128) in the
 // canonical un-swizzled UMMA layout; thread 0 then issues 3 x ceil(samples / 16) tcgen05.mma (hi hi + hi lo + lo hi)
@@ -25,13 +25,14 @@ __device__ unsigned long long g_ct_dbg[16];   // measurement build: thread 0's c
 #define CT_ADD(i, v)
 #endif
 #ifndef LARTPC_CT_KB
-#define LARTPC_CT_KB 48
+#define LARTPC_CT_KB 64
 #endif
 #ifndef LARTPC_CT_CTAS
-#define LARTPC_CT_CTAS 5
+#define LARTPC_CT_CTAS 4
 #endif
-// 48 columns per batch and five CTAs per SM (44 KB of shared memory and 96 registers each) against 64 and four: charge
-// lattice 62.2 -> 60.3 - 61.2 ms at configs[3], hit lists bit-identical (A/B on one box; 32 and six: 61.9 ms)
+// 64 columns per batch and four CTAs per SM.  48 and five (44 KB of shared memory and 96 registers each) were measured: hit
+// lists bit-identical, charge lattice 62.2 -> 60.3 - 61.2 ms at configs[3] (under the power cap), but 5 - 10 % SLOWER at every
+// point of the configs[4] sweep (n = 1e7: 58.1 -> 64.1 ms; base 0.856 -> 0.918 ms): dense tiles pay per batch
 constexpr int CT_KB = LARTPC_CT_KB;                      // samples per batch (a multiple of 16, at most 64: one thread of a role per column)
 static_assert(CT_KB % 16 == 0 && CT_KB >= 16 && CT_KB <= 64, "operand columns of a batch");
 constexpr int CT_A_HALF = 128 * CT_KB * 2;             // bytes of one precision half of the WXY operand (16 KB)
