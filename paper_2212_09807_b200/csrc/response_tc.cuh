@@ -102,7 +102,9 @@ __host__ __device__ __forceinline__ int b8_image_offset(int n, int kb)
 
 __device__ __forceinline__ void st_global_256(void *p, const uint4 &a, const uint4 &b)     // 32-byte aligned
 {
-    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+    // evict-first: the operand image (57 GB per configs[3] spill) and the partial rows (82 GB) are read back long after they
+    // have left the 126 MB L2; not letting them push the LUT images and the operand blocks in use out of it is worth 1 - 2 ms
+    asm volatile("st.global.cs.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
                  ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w) : "memory");
 }
 
