@@ -656,9 +656,6 @@ __global__ void __launch_bounds__(THREADS, 1) response_tc_kernel(const Args a)
                         }
                         // one 256-bit store per 8 ticks: each lane writes its own row, so the store path sees 32 sectors per
                         // instruction either way, and half as many instructions (response 175 -> 167 ms at configs[3])
-#ifdef LARTPC_EXP_NOSTORE
-                        if (r[0] == 1.2345f)
-#endif
                         st_global_256(dst + n0 + 8 * i8, make_uint4(__float_as_uint(r[0]), __float_as_uint(r[1]), __float_as_uint(r[2]), __float_as_uint(r[3])),
                                       make_uint4(__float_as_uint(r[4]), __float_as_uint(r[5]), __float_as_uint(r[6]), __float_as_uint(r[7])));
                     }
